@@ -1,0 +1,536 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix.
+
+None of these tests compares the oracle with itself or with the CUDA path: each expected value is a
+closed form, a library routine (numpy / scipy), a dense brute-force evaluation written independently
+here, or a value stored under tests/golden/ with its citation.
+"""
+import math
+import os
+from fractions import Fraction
+
+import numpy as np
+import pytest
+import scipy.fft
+import scipy.linalg
+import scipy.special
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+PI = math.pi
+
+
+def rel(a, b):
+    return float(np.max(np.abs(a - b)) / max(np.max(np.abs(b)), 1e-300))
+
+
+# --------------------------------------------------------------------------------------------- P1
+@pytest.mark.parametrize("n", [30, 32, 96, 192, 256, 1024, 1536])
+def test_fft_vs_definition_and_numpy(oracle, n):
+    rng = np.random.default_rng(n)
+    x = rng.standard_normal(n) + 1j * rng.standard_normal(n)
+    X = oracle.fft_c2c(x, -1)
+    j = np.arange(n)
+    W = np.exp(-2j * PI * np.outer(j, j) / n)       # the O(N^2) definition
+    assert rel(X, W @ x) < 1e-12
+    assert rel(X, np.fft.fft(x)) < 1e-13
+    assert rel(oracle.fft_c2c(X, +1) / n, x) < 1e-13  # inverse o forward
+    assert abs(np.sum(np.abs(X) ** 2) / n - np.sum(np.abs(x) ** 2)) < 1e-10 * n  # Parseval
+
+
+@pytest.mark.parametrize("n", [12, 96, 256])
+def test_dct_vs_definition_and_scipy(oracle, n):
+    rng = np.random.default_rng(n)
+    x = rng.standard_normal(n)
+    X = oracle.dct2(x)
+    k = np.arange(n)
+    C = np.cos(PI * np.outer(k, 2 * k + 1) / (2 * n))
+    assert rel(X, C @ x) < 1e-12
+    assert rel(X, 0.5 * scipy.fft.dct(x, type=2)) < 1e-13
+    assert rel(oracle.dct3(X), x) < 1e-13
+
+
+# --------------------------------------------------------------------------------------------- P2
+@pytest.mark.parametrize("n,cyclic", [(5, False), (64, False), (7, True), (64, True)])
+def test_thomas_vs_dense(oracle, n, cyclic):
+    rng = np.random.default_rng(7 * n + cyclic)
+    a, c = rng.standard_normal(n), rng.standard_normal(n)
+    b = 3.0 + np.abs(a) + np.abs(c)
+    d = rng.standard_normal(n)
+    A = np.diag(b) + np.diag(a[1:], -1) + np.diag(c[:-1], 1)
+    if cyclic:
+        A[0, n - 1] += a[0]; A[n - 1, 0] += c[n - 1]
+    assert rel(oracle.thomas(a, b, c, d, cyclic), np.linalg.solve(A, d)) < 1e-13
+
+
+# --------------------------------------------------------------------------------------------- P7
+def test_rk3_coefficients_and_third_order(oracle):
+    # PAPER.md:100
+    al = [Fraction(8, 15), Fraction(5, 12), Fraction(3, 4)]
+    be = [Fraction(0), Fraction(-17, 60), Fraction(-5, 12)]
+    for k in range(3):
+        a, b, g = oracle.rk3_coeffs(k)
+        assert a == float(al[k]) and b == float(be[k]) and abs(g - float(al[k] + be[k])) < 1e-16
+    assert sum(al) + sum(be) == 1
+    # amplification polynomial of u' = lam u under Eq. 11, in exact rationals (coefficients of z^0..z^3)
+    def mul_z(p):
+        return [Fraction(0)] + p
+    def add(p, q, s=1):
+        n = max(len(p), len(q)); p = p + [Fraction(0)] * (n - len(p)); q = q + [Fraction(0)] * (n - len(q))
+        return [x + s * y for x, y in zip(p, q)]
+    u0 = [Fraction(1)]
+    u1 = add(u0, [al[0] * c for c in mul_z(u0)])
+    u2 = add(add(u1, [al[1] * c for c in mul_z(u1)]), [be[1] * c for c in mul_z(u0)])
+    u3 = add(add(u2, [al[2] * c for c in mul_z(u2)]), [be[2] * c for c in mul_z(u1)])
+    assert u3 == [Fraction(1), Fraction(1), Fraction(1, 2), Fraction(1, 6)]
+
+
+# --------------------------------------------------------------------------------------------- grids
+def make(oracle, nx, ny, nz, bcs, stretch=False, lx=2 * PI, ly=PI, lz=2.0, **kw):
+    bc_y, bc_z = bcs
+    if stretch:
+        kw.update(zstretch=1, zstretch_factor=1.5)
+    return oracle.Oracle(nx, ny, nz, lx, ly, lz, bc_y=bc_y, bc_z=bc_z, **kw)
+
+
+def np_laplacian(S, phi):
+    """Independent numpy statement of the 7-point operator with periodic / Neumann closure."""
+    P = S.params
+    out = (np.roll(phi, -1, 2) - 2 * phi + np.roll(phi, 1, 2)) / S.dx ** 2
+    if P["bc_y"] == 0:
+        out += (np.roll(phi, -1, 1) - 2 * phi + np.roll(phi, 1, 1)) / S.dy ** 2
+    else:
+        e = np.concatenate([phi[:, :1], phi, phi[:, -1:]], axis=1)
+        out += (e[:, 2:] - 2 * phi + e[:, :-2]) / S.dy ** 2
+    nz = S.nz
+    if P["bc_z"] == 0:
+        dz = S.dzf[0]
+        out += (np.roll(phi, -1, 0) - 2 * phi + np.roll(phi, 1, 0)) / dz ** 2
+    else:
+        e = np.concatenate([phi[:1], phi, phi[-1:]], axis=0)
+        dzc = np.array([S.dzc(k) for k in range(-1, nz)])
+        up = (e[2:] - e[1:-1]) / dzc[1:, None, None]
+        dn = (e[1:-1] - e[:-2]) / dzc[:-1, None, None]
+        out += (up - dn) / S.dzf[:, None, None]
+    return out
+
+
+CASES = [((0, 0), False), ((0, 1), False), ((0, 1), True), ((1, 1), False), ((1, 1), True)]
+
+
+# --------------------------------------------------------------------------------------------- P3
+@pytest.mark.parametrize("bcs,stretch", CASES)
+def test_poisson_manufactured_discrete(oracle, bcs, stretch):
+    S = make(oracle, 24, 12, 16, bcs, stretch)
+    rng = np.random.default_rng(3)
+    phi = rng.standard_normal(S.shape)
+    phi -= np.sum(phi * S.dzf[:, None, None]) / (S.nx * S.ny * S.params["lz"])
+    f = np_laplacian(S, phi)
+    assert rel(S.laplacian(phi), f) < 1e-13          # the oracle's own plain stencil agrees with numpy's
+    got = S.poisson_solve(f)
+    assert rel(got, phi) < 1e-11
+    # gauge (reading S15): zero dzf-weighted mean, and an incompatible mean in f is discarded
+    got2 = S.poisson_solve(f + 3.0)
+    assert abs(np.sum(got2 * S.dzf[:, None, None])) < 1e-9
+    assert rel(got2, phi) < 1e-11
+
+
+def test_poisson_second_order_continuous(oracle):
+    errs = []
+    for n in (16, 32, 64):
+        S = oracle.Oracle(n, n, n, 2 * PI, 2.0, 1.0, bc_y=1, bc_z=1)
+        x = (np.arange(n) + 0.5) * S.dx; y = (np.arange(n) + 0.5) * S.dy; z = S.zc
+        ex = np.cos(x)[None, None, :] * np.cos(PI * y)[None, :, None] * np.cos(2 * PI * z)[:, None, None]
+        f = -(1.0 + PI ** 2 + 4 * PI ** 2) * ex
+        errs.append(np.max(np.abs(S.poisson_solve(f) - ex)))
+    assert 3.6 < errs[0] / errs[1] < 4.4 and 3.8 < errs[1] / errs[2] < 4.2
+
+
+# --------------------------------------------------------------------------------------------- P5
+def test_eigenvalues_are_those_of_the_stencil(oracle):
+    S = make(oracle, 24, 12, 16, (1, 1), False)
+    x = (np.arange(S.nx) + 0.5)
+    j = np.arange(S.ny)
+    for m, n in [(1, 0), (3, 5), (12, 11)]:
+        basis = np.cos(2 * PI * m * x / S.nx)[None, None, :] * np.cos(PI * n * (j + 0.5) / S.ny)[None, :, None] * np.ones((S.nz, 1, 1))
+        lam = -4 / S.dx ** 2 * math.sin(PI * m / S.nx) ** 2 - 4 / S.dy ** 2 * math.sin(PI * n / (2 * S.ny)) ** 2
+        assert np.max(np.abs(S.laplacian(basis) - lam * basis)) < 1e-11 * abs(lam)
+
+
+# --------------------------------------------------------------------------------------------- P4
+def random_solenoidal(S, seed=11, amp=1.0):
+    rng = np.random.default_rng(seed)
+    u, v, w = (amp * rng.standard_normal(S.shape) for _ in range(3))
+    if S.params["bc_z"] == 1:
+        w[-1] = 0.0
+    if S.params["bc_y"] == 1:
+        v[:, -1, :] = 0.0
+    S.set_velocity(u, v, w)
+    S.project()
+    return S.velocity()
+
+
+@pytest.mark.parametrize("bcs,stretch", CASES)
+def test_projection_removes_divergence(oracle, bcs, stretch):
+    S = make(oracle, 24, 12, 16, bcs, stretch)
+    random_solenoidal(S)
+    dmin = min(S.dx, S.dy, S.dzf.min())
+    assert np.max(np.abs(S.divergence())) * dmin < 1e-12
+
+
+# --------------------------------------------------------------------------------------------- P8
+@pytest.mark.parametrize("bcs,stretch", CASES)
+def test_advection_conserves_energy_and_momentum(oracle, bcs, stretch):
+    S = make(oracle, 24, 12, 16, bcs, stretch)
+    u, v, w = random_solenoidal(S)
+    au, av, aw = S.advection()
+    dzf = S.dzf[:, None, None]
+    dzc = np.array([S.dzc(k) for k in range(S.nz)])[:, None, None]
+    for q, a, vol in ((u, au, dzf), (v, av, dzf), (w, aw, dzc)):
+        assert abs(np.sum(q * a * vol)) < 1e-13 * np.sum(np.abs(q * a * vol))   # PAPER.md:38 energy-preserving
+    assert abs(np.sum(au * dzf)) < 1e-12 * np.sum(np.abs(au * dzf))              # momentum along periodic x
+    if bcs[0] == 0:
+        assert abs(np.sum(av * dzf)) < 1e-12 * np.sum(np.abs(av * dzf))
+
+
+def test_plain_mean_would_break_energy_on_stretched_grid(oracle):
+    """The dzf-weighted advecting velocity of reading S3 matters: the w-energy identity holds on tanh grids
+    (above) although the spacing ratio is far from 1 -- checked here to be a non-trivial statement."""
+    S = make(oracle, 24, 12, 16, (0, 1), True)
+    assert S.dzf.max() / S.dzf.min() > 3.0
+
+
+# --------------------------------------------------------------------------------------------- P9
+@pytest.mark.parametrize("bcs,stretch", CASES)
+def test_sgs_fluxes_telescope(oracle, bcs, stretch):
+    S = make(oracle, 24, 12, 16, bcs, stretch, sgs_model=1)
+    random_solenoidal(S)
+    rng = np.random.default_rng(5)
+    S.set(S.NUT, rng.random(S.shape))
+    su, sv, sw = S.sgs_term()
+    dzf = S.dzf[:, None, None]
+    assert abs(np.sum(su * dzf)) < 1e-12 * np.sum(np.abs(su * dzf))
+    if bcs[0] == 0:
+        assert abs(np.sum(sv * dzf)) < 1e-12 * np.sum(np.abs(sv * dzf))
+    if bcs[1] == 0:
+        assert abs(np.sum(sw)) < 1e-12 * np.sum(np.abs(sw))
+
+
+def test_sgs_with_constant_viscosity_is_the_laplacian(oracle):
+    S = make(oracle, 24, 12, 16, (0, 0), False, lz=3.0, nu=0.7, sgs_model=1)
+    random_solenoidal(S)
+    S.set(S.NUT, np.full(S.shape, 0.7))
+    for a, b in zip(S.sgs_term(), S.diffusion(0)):
+        assert rel(a, b) < 1e-11      # sign of reading S1: +nu_t L u_i, i.e. dissipative
+
+
+# --------------------------------------------------------------------------------------------- P10, P11
+@pytest.mark.parametrize("stretch", [False, True])
+@pytest.mark.parametrize("damp", [0, 1])
+def test_static_smagorinsky_linear_shear(oracle, stretch, damp):
+    G, cs, nu = 3.0, 0.1, 2e-3
+    S = make(oracle, 8, 6, 16, (0, 1), stretch, nu=nu, sgs_model=1, cs=cs, van_driest=damp, aplus=25.0)
+    u = G * S.zc[:, None, None] * np.ones(S.shape)
+    nut = S.eddy_viscosity(u, np.zeros(S.shape), np.zeros(S.shape))
+    delta = (S.dx * S.dy * S.dzf) ** (1.0 / 3.0)
+    D = 1.0 - np.exp(-(S.zc * math.sqrt(nu * G) / nu) / 25.0) if damp else 1.0
+    exp = ((cs * delta * D) ** 2 * G)[:, None, None] * np.ones(S.shape)
+    h = S.nz // 2
+    assert rel(nut[:h], exp[:h]) < 1e-13       # Eq. 4 exactly (the top wall is inconsistent with u = G z)
+
+
+def test_strain_of_linear_field(oracle):
+    A = np.array([[0.3, -1.1, 0.4], [0.7, 0.5, -0.2], [1.3, 0.9, -0.8]])   # trace 0
+    S = make(oracle, 12, 12, 14, (0, 1), True)
+    nx, ny, nz = S.nx, S.ny, S.nz
+    xc = (np.arange(nx) + 0.5) * S.dx; xf = (np.arange(nx) + 1.0) * S.dx
+    yc = (np.arange(ny) + 0.5) * S.dy; yf = (np.arange(ny) + 1.0) * S.dy
+    zc = S.zc; zf = S.zf[1:]
+    def lin(row, x, y, z):
+        return A[row, 0] * x[None, None, :] + A[row, 1] * y[None, :, None] + A[row, 2] * z[:, None, None]
+    S.set_velocity(lin(0, xf, yc, zc), lin(1, xc, yf, zc), lin(2, xc, yc, zf))
+    Sij, smag = S.strain()
+    sym = 0.5 * (A + A.T)
+    want = [sym[0, 0], sym[1, 1], sym[2, 2], sym[0, 1], sym[0, 2], sym[1, 2]]
+    inner = (slice(2, nz - 2), slice(2, ny - 2), slice(2, nx - 2))
+    for c in range(6):
+        assert np.max(np.abs(Sij[c][inner] - want[c])) < 1e-12
+    assert np.max(np.abs(smag[inner] - math.sqrt(2 * np.sum(sym * sym)))) < 1e-12
+
+
+# --------------------------------------------------------------------------------------------- P12
+def lambert_hplus(re, kappa=0.41, B=5.2):
+    y = scipy.special.lambertw(kappa * re * math.exp(kappa * B)).real
+    return kappa * re / y
+
+
+def test_loglaw_golden_values(oracle):
+    rows = [l.split() for l in open(os.path.join(GOLD, "loglaw_hplus.txt")) if l.strip() and not l.startswith("#")]
+    for re, hp in rows:
+        got, it = oracle.loglaw_hplus(float(re))
+        assert abs(got / float(hp) - 1.0) < 2e-6        # the stored values carry 6 significant digits
+        assert 1 <= it <= 9
+
+
+def test_loglaw_vs_lambert_w_and_iteration_count(oracle):
+    for re in np.logspace(-8, 7, 61):
+        got, it = oracle.loglaw_hplus(float(re))
+        assert abs(got / lambert_hplus(re) - 1.0) < 1e-13
+        # Eq. 10 residual
+        assert abs(re / got - (math.log(got) / 0.41 + 5.2)) < 1e-10 * max(1.0, re / got)
+        assert it <= 12
+    # PAPER.md:130 "3 to 7 iterations" to the 0.01 % tolerance; the count returned includes the one polish update (S9)
+    its = [oracle.loglaw_hplus(float(re))[1] - 1 for re in np.logspace(-8, 5, 53)]
+    assert 3 <= min(its) and max(its) <= 7
+
+
+def test_wall_stress_direction_interpolation_and_flux(oracle):
+    nu = 1e-3
+    S = make(oracle, 8, 6, 16, (0, 1), False, nu=nu, wall_model=1, h_wm=0.2, sgs_model=1)
+    a, b = 7.0, -3.0
+    # linear-in-z profiles: the interpolation to h_wm must be exact; distance measured from each wall
+    d = np.minimum(S.zc, 2.0 - S.zc)[:, None, None] * np.ones(S.shape)
+    S.set_velocity(a * d, b * d, np.zeros(S.shape))
+    tau = S.wall_stress()
+    U = math.hypot(a, b) * 0.2
+    ut = lambert_hplus(U * 0.2 / nu) * nu / 0.2
+    for wall in (0, 1):
+        assert rel(tau[wall, 0], np.full((S.ny, S.nx), ut ** 2 * a / math.hypot(a, b))) < 1e-12
+        assert rel(tau[wall, 1], np.full((S.ny, S.nx), ut ** 2 * b / math.hypot(a, b))) < 1e-12
+    # "the wall shear stress is directly provided by the wall model": the column integral of the
+    # z-diffusion term equals minus the two modelled stresses
+    du, dv, _ = S.diffusion(2)
+    col = np.sum(du * S.dzf[:, None, None], axis=0)
+    assert rel(col, -(tau[0, 0] + tau[1, 0])) < 1e-11
+    col = np.sum(dv * S.dzf[:, None, None], axis=0)
+    assert rel(col, -(tau[0, 1] + tau[1, 1])) < 1e-11
+
+
+# --------------------------------------------------------------------------------------------- P13
+def np_dsm_periodic(S, u, v, w, alpha2=4.0 ** (2.0 / 3.0)):
+    """Independent dense numpy evaluation of Eq. 5-9 in a triply periodic box (np.roll, 9-point filter)."""
+    dx, dy, dz = S.dx, S.dy, S.dzf[0]
+    r = np.roll
+    def filt(q):
+        out = np.zeros_like(q)
+        for dj, wj in ((-1, .25), (0, .5), (1, .25)):
+            for di, wi in ((-1, .25), (0, .5), (1, .25)):
+                out += wi * wj * r(r(q, -dj, 1), -di, 2)
+        return out
+    def strain(u, v, w):
+        s11 = (u - r(u, 1, 2)) / dx; s22 = (v - r(v, 1, 1)) / dy; s33 = (w - r(w, 1, 0)) / dz
+        e12 = 0.5 * ((r(u, -1, 1) - u) / dy + (r(v, -1, 2) - v) / dx)
+        e13 = 0.5 * ((r(u, -1, 0) - u) / dz + (r(w, -1, 2) - w) / dx)
+        e23 = 0.5 * ((r(v, -1, 0) - v) / dz + (r(w, -1, 1) - w) / dy)
+        s12 = 0.25 * (e12 + r(e12, 1, 2) + r(e12, 1, 1) + r(r(e12, 1, 1), 1, 2))
+        s13 = 0.25 * (e13 + r(e13, 1, 2) + r(e13, 1, 0) + r(r(e13, 1, 0), 1, 2))
+        s23 = 0.25 * (e23 + r(e23, 1, 1) + r(e23, 1, 0) + r(r(e23, 1, 0), 1, 1))
+        s = [s11, s22, s33, s12, s13, s23]
+        mag = np.sqrt(2 * (s11 ** 2 + s22 ** 2 + s33 ** 2) + 4 * (s12 ** 2 + s13 ** 2 + s23 ** 2))
+        return s, mag
+    s, mag = strain(u, v, w)
+    c = [0.5 * (u + r(u, 1, 2)), 0.5 * (v + r(v, 1, 1)), 0.5 * (w + r(w, 1, 0))]
+    pairs = [(0, 0), (1, 1), (2, 2), (0, 1), (0, 2), (1, 2)]
+    L = [filt(c[a] * c[b]) - filt(c[a]) * filt(c[b]) for a, b in pairs]
+    st, stmag = strain(filt(u), filt(v), filt(w))
+    d2 = (dx * dy * dz) ** (2.0 / 3.0)
+    M = [2 * d2 * (filt(mag * s[k]) - alpha2 * stmag * st[k]) for k in range(6)]
+    f = [1, 1, 1, 2, 2, 2]
+    lm = sum(f[k] * L[k] * M[k] for k in range(6)).sum(axis=(1, 2))
+    mm = sum(f[k] * M[k] * M[k] for k in range(6)).sum(axis=(1, 2))
+    cs = lm / mm
+    nut = np.maximum(cs, 0.0)[:, None, None] * d2 * mag
+    return np.array(L), np.array(M), cs, nut
+
+
+def test_dynamic_model_vs_dense_bruteforce(oracle):
+    S = oracle.Oracle(8, 8, 4, 2.0, 3.0, 1.0, bc_y=0, bc_z=0, sgs_model=2, dsm_avg_xy_plane=1)
+    u, v, w = random_solenoidal(S, seed=21)
+    nut = S.eddy_viscosity(u, v, w)
+    L, M, cs, nut_ref = np_dsm_periodic(S, u, v, w)
+    Lo, Mo = S.dsm_tensors()
+    assert rel(Lo, L) < 1e-12 and rel(Mo, M) < 1e-12
+    assert rel(S.get_cs(), cs) < 1e-11
+    assert rel(nut, nut_ref) < 1e-11
+    assert np.any(cs > 0) and np.any(nut > 0)
+
+
+def test_dynamic_model_laminar_scale_and_clip(oracle):
+    # (i) switches off in laminar shear
+    S = make(oracle, 8, 6, 16, (0, 1), False, sgs_model=2)
+    u = 3.0 * S.zc[:, None, None] * np.ones(S.shape)
+    nut = S.eddy_viscosity(u, np.zeros(S.shape), np.zeros(S.shape))
+    assert np.max(np.abs(nut)) < 1e-14 and np.max(np.abs(S.get_cs())) < 1e-12
+    # (ii) scale invariance
+    S = make(oracle, 12, 8, 10, (1, 1), False, sgs_model=2, dsm_avg_xy_plane=0, dsm_clip_total=1, nu=10.0)
+    u, v, w = random_solenoidal(S, seed=4)
+    n1 = S.eddy_viscosity(u, v, w); c1 = S.get_cs()
+    n2 = S.eddy_viscosity(2.5 * u, 2.5 * v, 2.5 * w); c2 = S.get_cs()
+    assert rel(c2, c1) < 1e-11 and rel(n2, 2.5 * n1) < 1e-11
+    assert np.any(c1 < 0) and np.any(n1 < 0)          # total-viscosity clip keeps negative values above -nu
+    # paper clip: c_s >= 0
+    S2 = make(oracle, 12, 8, 10, (1, 1), False, sgs_model=2, dsm_avg_xy_plane=0, dsm_clip_total=0)
+    n3 = S2.eddy_viscosity(u, v, w)
+    assert np.min(n3) >= 0.0 and rel(n3, np.maximum(n1, 0.0)) < 1e-11
+
+
+def test_dynamic_model_single_fourier_mode(oracle):
+    # (iii) v = A sin(m x): L_22 in closed form with the filter transfer function T(m) = cos^2(m dx/2)
+    nx, m, A = 16, 2, 1.3
+    S = oracle.Oracle(nx, 8, 6, 2 * PI, 2 * PI, 2 * PI, sgs_model=2)
+    x = (np.arange(nx) + 0.5) * S.dx
+    v = A * np.sin(m * x)[None, None, :] * np.ones(S.shape)
+    S.eddy_viscosity(np.zeros(S.shape), v, np.zeros(S.shape))
+    L, M = S.dsm_tensors()
+    T = lambda q: math.cos(q * S.dx / 2) ** 2
+    want = 0.5 * A * A * ((1 - T(m) ** 2) - (T(2 * m) - T(m) ** 2) * np.cos(2 * m * x))
+    assert np.max(np.abs(L[1] - want[None, None, :])) < 1e-13
+    for c in (0, 2, 3, 4, 5):
+        assert np.max(np.abs(L[c])) < 1e-14
+    for c in (0, 1, 2, 4, 5):
+        assert np.max(np.abs(M[c])) < 1e-13           # only M_12 survives
+    assert np.max(np.abs(M[3])) > 1e-3
+    assert np.max(np.abs(S.get_cs())) < 1e-12
+
+
+def test_filter_commutes_with_strain_and_extrapolation_identity(oracle):
+    S = oracle.Oracle(12, 8, 6, 2.0, 3.0, 1.0, sgs_model=2)
+    u, v, w = random_solenoidal(S, seed=8)
+    Sij, _ = S.strain()
+    fS = np.array([S.filter_xy(Sij[c]) for c in range(6)])
+    S.set_velocity(S.filter_xy(u), S.filter_xy(v), S.filter_xy(w))
+    Sf, _ = S.strain()
+    assert rel(Sf, fS) < 1e-12                         # (iv)
+    # filter weights: a constant is preserved, a 2-dx wave in x is annihilated
+    assert rel(S.filter_xy(np.ones(S.shape)), np.ones(S.shape)) < 1e-15
+    saw = ((-1.0) ** np.arange(12))[None, None, :] * np.ones(S.shape)
+    assert np.max(np.abs(S.filter_xy(saw))) < 1e-15
+    # (v) PAPER.md:128: symmetric 3-point filter after linear extrapolation to the ghost is the identity
+    #     -> in a wall-bounded y the first layers keep their value in y
+    W = oracle.Oracle(12, 8, 6, 2.0, 3.0, 1.0, bc_y=1, bc_z=1, sgs_model=2)
+    q = np.random.default_rng(0).standard_normal(W.shape)
+    fq = W.filter_xy(q)
+    xonly = 0.25 * np.roll(q, 1, 2) + 0.5 * q + 0.25 * np.roll(q, -1, 2)
+    assert rel(fq[:, 0], xonly[:, 0]) < 1e-14 and rel(fq[:, -1], xonly[:, -1]) < 1e-14
+    ghost = 2 * xonly[:, 0] - xonly[:, 1]
+    assert rel(0.25 * ghost + 0.5 * xonly[:, 0] + 0.25 * xonly[:, 1], fq[:, 0]) < 1e-13
+
+
+# --------------------------------------------------------------------------------------------- P6
+@pytest.mark.parametrize("plane", ["xy", "xz", "yz"])
+def test_taylor_green_decay(oracle, plane):
+    n, nu, dt, steps = 32, 1e-2, 5e-3, 20
+    S = oracle.Oracle(n, n, n, 2 * PI, 2 * PI, 2 * PI, nu=nu, sgs_model=0)
+    d = 2 * PI / n
+    c = (np.arange(n) + 0.5) * d
+    f = (np.arange(n) + 1.0) * d
+    one = np.ones((n, n, n))
+    ax = {"x": 2, "y": 1, "z": 0}
+    def along(a, vals):
+        sh = [1, 1, 1]; sh[ax[a]] = n
+        return vals.reshape(sh) * one
+    a, b = plane
+    ua = along(a, np.sin(f)) * along(b, np.cos(c))          # component a at its +a faces
+    ub = -along(a, np.cos(c)) * along(b, np.sin(f))
+    vel = {"x": np.zeros_like(one), "y": np.zeros_like(one), "z": np.zeros_like(one)}
+    vel[a], vel[b] = ua, ub
+    S.set_velocity(vel["x"], vel["y"], vel["z"])
+    for _ in range(steps):
+        S.step(dt)
+    keff2 = (math.sin(d / 2) / (d / 2)) ** 2
+    z = -2 * nu * keff2 * dt
+    G = 1 + z + z * z / 2 + z ** 3 / 6
+    got = dict(zip("xyz", S.velocity()))
+    assert rel(got[a], G ** steps * ua) < 1e-12
+    assert rel(got[b], G ** steps * ub) < 1e-12
+    third = [k for k in "xyz" if k not in plane][0]
+    assert np.max(np.abs(got[third])) < 1e-13
+    assert np.max(np.abs(S.divergence())) < 1e-12
+    # pressure: loose check of the closed form (F^2/4)(cos 2a + cos 2b) with the discrete factor cos^2(d/2)
+    p = S.get(S.P); p -= p.mean()
+    F2 = G ** (2 * steps)
+    pex = 0.25 * F2 * math.cos(d / 2) ** 2 * (along(a, np.cos(2 * c)) + along(b, np.cos(2 * c)))
+    assert rel(p, pex) < 2e-2
+    # continuous decay rate, second-order accurate
+    assert abs(G ** steps - math.exp(-2 * nu * dt * steps)) < 2 * nu * dt * steps * (1 - keff2) * 1.1 + 1e-9
+
+
+# --------------------------------------------------------------------------------------------- P14
+@pytest.mark.parametrize("comp", ["u", "w"])
+def test_crank_nicolson_z_eigenmode(oracle, comp):
+    nz, nmode, nu, dt = 16, 3, 0.05, 0.02
+    S = oracle.Oracle(8, 6, nz, 1.0, 1.0, 1.0, bc_z=1, nu=nu, implicit_z=1, sgs_model=0)
+    dz = 1.0 / nz
+    k = np.arange(nz)
+    lam = -4.0 / dz ** 2 * math.sin(PI * nmode / (2 * nz)) ** 2
+    zero = np.zeros(S.shape)
+    if comp == "u":
+        prof = np.sin(PI * nmode * (k + 0.5) / nz)
+        q0 = prof[:, None, None] * np.ones(S.shape)
+        S.set_velocity(q0, zero, zero)
+    else:
+        # w(z) alone is not solenoidal; use w = sin(pi n (k+1)/nz) * cos(2 pi x) pattern?  Instead keep the
+        # projection out of the way: a field w(x,y) independent of z is solenoidal but has no z-diffusion.
+        # So test v instead of w for the centred family and w through the Helmholtz residual below.
+        prof = np.sin(PI * nmode * (k + 0.5) / nz)
+        q0 = prof[:, None, None] * np.ones(S.shape)
+        S.set_velocity(zero, q0, zero)
+    S.step(dt)
+    fac = 1.0
+    for rk in range(3):
+        c = oracle.rk3_coeffs(rk)[2] * nu * dt / 2
+        fac *= (1 + c * lam) / (1 - c * lam)
+    got = S.velocity()[0 if comp == "u" else 1]
+    assert rel(got, fac * q0) < 1e-13
+
+
+def test_crank_nicolson_matches_explicit_to_second_order(oracle):
+    """Eq. 20-22 and Eq. 11-14 discretise the same equation: on a smooth solenoidal field their results differ
+    by O(dt^2) per step (the w family of the implicit solve is exercised here)."""
+    diffs = []
+    for dt in (2e-3, 1e-3):
+        res = []
+        for imp in (0, 1):
+            S = oracle.Oracle(16, 8, 16, 2 * PI, PI, 2.0, bc_z=1, nu=0.05, implicit_z=imp, sgs_model=0)
+            x = (np.arange(16) + 1.0) * S.dx; xc = x - 0.5 * S.dx
+            zc, zf = S.zc, S.zf[1:]
+            u = (np.sin(xc + 0.5 * S.dx)[None, None, :] * (PI / 2 * np.cos(PI * zc / 2) * np.sin(PI * zc / 2) * 2)[:, None, None]) * np.ones(S.shape)
+            w = (-np.cos(xc)[None, None, :] * (np.sin(PI * zf / 2) ** 2)[:, None, None]) * np.ones(S.shape)
+            S.set_velocity(u, np.zeros(S.shape), w); S.project()
+            for _ in range(4):
+                S.step(dt)
+            res.append(np.array(S.velocity()))
+        diffs.append(np.max(np.abs(res[0] - res[1])))
+    assert diffs[0] < 1e-4 and 2.5 < diffs[0] / diffs[1] < 6.0
+
+
+# --------------------------------------------------------------------------------------------- P15 + whole step
+def test_constant_flow_rate_and_projection_every_step(oracle):
+    S = make(oracle, 24, 12, 16, (0, 1), False, nu=1.0 / 2000, sgs_model=1, cs=0.1, wall_model=1, const_flow_rate=1, u_bulk=20.0)
+    rng = np.random.default_rng(2)
+    prof = np.log(np.minimum(S.zc, 2 - S.zc) * 2000) / 0.41 + 5.2
+    u = prof[:, None, None] + 2.0 * (2 * rng.random(S.shape) - 1)
+    v = 2.0 * (2 * rng.random(S.shape) - 1); w = 2.0 * (2 * rng.random(S.shape) - 1); w[-1] = 0
+    S.set_velocity(u, v, w)
+    for _ in range(3):
+        S.step(1e-3)
+        d = S.diagnostics()
+        assert abs(d["u_bulk"] - 20.0) < 1e-13 * 20
+        assert d["max_div"] * min(S.dx, S.dy, S.dzf.min()) / 20.0 < 1e-12
+        assert 3 <= d["wm_max_iters"] <= 9
+    assert np.all(S.get(S.NUT) >= 0) and np.max(S.get(S.NUT)) > 0
+    assert np.max(np.abs(S.get(S.W)[-1])) == 0.0
+
+
+def test_energy_decays_with_sgs_model(oracle):
+    """Sign of reading S1 once more, on the whole step: with nu = 0 the only energy sink is the SGS term."""
+    S = oracle.Oracle(16, 16, 16, 2 * PI, 2 * PI, 2 * PI, nu=0.0, sgs_model=1, cs=0.17)
+    random_solenoidal(S, seed=13)
+    S0 = oracle.Oracle(16, 16, 16, 2 * PI, 2 * PI, 2 * PI, nu=0.0, sgs_model=0)
+    S0.set_velocity(*S.velocity())
+    e0 = S.diagnostics()["kinetic_energy"]
+    for _ in range(5):
+        S.step(2e-3); S0.step(2e-3)
+    def energy(T):
+        u, v, w = T.velocity(); return 0.5 * float(np.mean(u * u + v * v + w * w))
+    eu0 = energy(S0); eu1 = energy(S)
+    assert eu1 < eu0                                   # the model dissipates
+    assert e0 > 0
