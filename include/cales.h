@@ -1,0 +1,160 @@
+/* cales.h -- C ABI of the B200-native (sm_100a, fp64 CUDA) hot path of CaLES (arXiv 2411.09364).
+ *
+ * One low-storage RK3 step of the incompressible staggered-grid finite-difference LES of the paper
+ * (Alg. 1; Alg. 2) on ONE GPU.  Every step of the
+ * path runs in hand-written CUDA kernels inside libcales.so; there is no CPU fallback and no cuFFT.
+ *
+ * Conventions:
+ *  - Axis convention of the solver: x streamwise (always periodic), y spanwise (periodic
+ *    or walls), z wall-normal (periodic or walls; the only direction that may be non-uniform; the
+ *    Thomas direction).  The paper's text calls this direction y: paper-y == our z, paper L_22 == L_zz.
+ *  - Arrays hold interior values only, fp64, C order [k][j][i], x fastest: idx = i + nx*(j + ny*k).
+ *    u sits on the +x face of cell (i,j,k), v on the +y face, w on the +z face; p, phi, nu_t at cell
+ *    centres.  In a wall-bounded direction the last face entry (w[nz-1], v[.][ny-1][.]) is the wall
+ *    itself and is kept at 0 by the library.
+ *  - Pointers marked DEVICE must be device pointers valid on `device`; HOST pointers are host memory.
+ *  - Ownership: the caller owns every buffer, including the workspace blob (size from
+ *    cales_workspace_bytes) that the library carves into its fields, work arrays and tables.  The
+ *    library never allocates device memory.  The workspace and the stream must outlive the solver.
+ *  - All work is enqueued on the caller's CUDA stream (`cuda_stream`, a cudaStream_t; NULL = the
+ *    legacy default stream).  cales_step / cales_poisson_solve / cales_eddy_viscosity / cales_wall_stress
+ *    are asynchronous; cales_create, cales_set_field / cales_get_field with host pointers and
+ *    cales_diagnostics synchronise the stream.
+ *  - Errors: every function returning int returns CALES_OK (0) or one of the codes below, never throws,
+ *    never aborts; cales_last_error() gives a thread-local message.  Argument errors are detected at
+ *    cales_create (nothing can fail for argument reasons at step time).
+ */
+#ifndef CALES_H
+#define CALES_H
+#include <stddef.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct cales_solver cales_solver; /* opaque */
+
+enum { CALES_OK = 0, CALES_EINVAL = 1, CALES_EUNSUPPORTED = 2, CALES_ENOMEM = 3, CALES_ECUDA = 4, CALES_ENUMERIC = 5 };
+enum { CALES_BC_PERIODIC = 0, CALES_BC_WALL = 1 };  /* per direction y, z (both sides share the type); a wall is
+                                                      no-slip unless wall_model=1, which turns the z-walls into
+                                                      modelled-stress walls */
+enum { CALES_SGS_NONE = 0, CALES_SGS_SMAG = 1, CALES_SGS_DSMAG = 2 };
+enum { CALES_Z_UNIFORM = 0, CALES_Z_TANH = 1, CALES_Z_USER = 2 };
+enum { CALES_U = 0, CALES_V = 1, CALES_W = 2, CALES_P = 3, CALES_NUT = 4 }; /* field ids */
+
+/* Everything the paper's statement of the problem needs. */
+typedef struct {
+  int nx, ny, nz;            /* cells; nx, ny even and of the form 2^a 3^b; nz >= 4 */
+  double lx, ly, lz;         /* box */
+  int zstretch;              /* CALES_Z_*; TANH: zf[k] = lz/2 (1 + tanh(a(2k/nz-1))/tanh a), a = zstretch_factor */
+  double zstretch_factor;
+  const double* zf_user;     /* HOST, nz+1 faces, read during cales_create only (CALES_Z_USER) */
+  int bc_y, bc_z;            /* CALES_BC_* */
+  double nu;                 /* molecular viscosity */
+  int sgs_model;             /* CALES_SGS_*: Eq. 4 / Eq. 5-9 */
+  double cs;                 /* Smagorinsky constant of Eq. 4 */
+  int van_driest;            /* D = 1 - exp(-z+/A+) */
+  double aplus;              /* <= 0 -> 25 */
+  int dsm_avg_xy_plane;      /* 1: <> over x-y planes, c_s(k); 0: over x lines, c_s(j,k) (Eq. 6) */
+  int dsm_clip_total;        /* 0: c_s = max(c_s, 0); 1: nu_t = max(nu_t, -nu) */
+  double dsm_alpha2d;        /* filter-width ratio of the x-y test filter; <= 0 -> 4^(1/3) */
+  int wall_model;            /* log-law wall model on the z walls (Eq. 10) */
+  double kappa, B;           /* <= 0 kappa -> 0.41; B as given (5.2 in the paper) */
+  double h_wm;               /* height of the wall-modelled layer; <= 0 -> first off-wall cell centre */
+  double wm_tol;             /* relative tolerance on tau_w; <= 0 -> 1e-4 */
+  int wm_maxit;              /* <= 0 -> 50 */
+  int implicit_z;            /* Crank-Nicolson in z, Eq. 20-22 */
+  int const_flow_rate;       /* uniform forcing that keeps the bulk velocity at u_bulk */
+  double u_bulk;
+  void* workspace;           /* DEVICE, 256-byte aligned, >= cales_workspace_bytes(params) */
+  size_t workspace_bytes;
+  void* cuda_stream;         /* cudaStream_t of the caller */
+  int device;                /* CUDA device ordinal the workspace lives on */
+} cales_params;
+
+typedef struct {
+  double max_div;            /* max |div u| over cells */
+  double u_bulk;             /* dzf-weighted volume mean of u */
+  double kinetic_energy;     /* volume mean of (uc^2+vc^2+wc^2)/2 at cell centres */
+  double forcing;            /* equivalent body force of the last substep's bulk correction */
+  int wm_max_iters;          /* max Newton iterations of the last wall-model evaluation */
+  int nan_count;             /* non-finite entries in u, v, w, p */
+  double ms_rhs, ms_implicit, ms_solver, ms_correction, ms_sgs, ms_wall; /* device ms of the last step, by
+                                phase, only when cales_set_timing(s, 1) was called before it; else 0 */
+} cales_diag;
+
+/* Fill *p with the defaults (everything off/zero, kappa 0.41, B 5.2, A+ 25, cs 0.17, averaging over planes). */
+void cales_default_params(cales_params* p);
+
+/* Bytes of workspace a solver with these parameters needs (0 on invalid parameters; see cales_last_error). */
+size_t cales_workspace_bytes(const cales_params* p);
+
+/* Create a solver.  Validates the parameters (CALES_EINVAL: bad sizes / null pointers / workspace too small;
+ * CALES_EUNSUPPORTED: sizes that do not factor into 2 and 3, odd nx or ny, periodic z with stretching, wall model
+ * without z walls or together with implicit_z, van Driest without z walls / with y walls / with the wall model),
+ * builds the grid and the transform tables on the host, uploads them into the workspace, zeroes all fields.
+ * Synchronises the stream. */
+int cales_create(const cales_params* p, cales_solver** out);
+
+/* The positional form named by the problem statement: grid, box, z-stretching, BCs, nu, sgs_model, wall_model,
+ * implicit_z; every other parameter takes its default.  The workspace is still the caller's. */
+int cales_create_basic(int nx, int ny, int nz, double lx, double ly, double lz, int zstretch, double zstretch_factor,
+                       int bc_y, int bc_z, double nu, int sgs_model, int wall_model, int implicit_z,
+                       void* workspace, size_t workspace_bytes, void* cuda_stream, int device, cales_solver** out);
+
+int cales_destroy(cales_solver* s);
+
+/* Copy a whole field (nz*ny*nx doubles) into / out of the solver state.  on_device != 0: DEVICE pointer,
+ * asynchronous on the stream; 0: HOST pointer, the call synchronises.  Setting a velocity component marks the
+ * closures (wall stress, nu_t) stale: they are recomputed at the start of the next cales_step (Alg. 1 l.1-2). */
+int cales_set_field(cales_solver* s, int field, const double* src, int src_on_device);
+int cales_get_field(cales_solver* s, int field, double* dst, int dst_on_device);
+
+/* One full RK3 step = 3 substeps of Alg. 1 with the coefficients of PAPER.md:100:
+ * u* from Eq. 11 (or Eq. 20-21), bulk forcing, Poisson Eq. 12, correction Eq. 13, pressure Eq. 14 / 22,
+ * wall stress Eq. 10, nu_t Eq. 4 / Eq. 5-9.  Asynchronous.  dt > 0. */
+int cales_step(cales_solver* s, double dt);
+
+/* Solve L_h phi = rhs with the solver's boundary conditions (Eq. 12; eigenfunction expansion,
+ * PAPER.md:126): real FFT along x, real FFT or DCT-II along y, (cyclic) Thomas along z.  The component of rhs
+ * incompatible with the singular operator is discarded; phi has zero dzf-weighted mean.  rhs_dev, phi_dev:
+ * DEVICE, nz*ny*nx, may alias.  Asynchronous. */
+int cales_poisson_solve(cales_solver* s, const double* rhs_dev, double* phi_dev);
+
+/* nu_t (Eq. 4 or Eq. 5-9) of a velocity field.  u, v, w: DEVICE fields, or all NULL = the solver's own velocity;
+ * nut: DEVICE output, nz*ny*nx (NULL = the solver's own nu_t).  Uses the stored wall stresses only through the
+ * velocity ghosts.  Asynchronous. */
+int cales_eddy_viscosity(cales_solver* s, const double* u, const double* v, const double* w, double* nut);
+
+/* Wall stresses of the log-law wall model from the solver's velocity (Eq. 10):
+ * tau_dev DEVICE [wall(0 bottom,1 top)][comp(0: tau_xz at u points, 1: tau_yz at v points)][ny][nx]
+ * (NULL = only refresh the internal planes).  Asynchronous. */
+int cales_wall_stress(cales_solver* s, double* tau_dev);
+
+/* Make the solver's velocity discretely solenoidal by one projection with gamma*dt = 1 (Eq. 12-13). */
+int cales_project(cales_solver* s);
+
+/* Dynamic coefficient of the last eddy-viscosity evaluation: cs_dev DEVICE, nz (plane averaging) or nz*ny. */
+int cales_get_cs(cales_solver* s, double* cs_dev);
+
+/* Batched 1-D transforms of the Poisson solver applied to a whole field, for tests (DEVICE, in place):
+ * dir 0: x, dir 1: y (FFT or DCT-II by bc_y); inverse != 0: the inverse transform (normalised). */
+int cales_transform(cales_solver* s, double* field_dev, int dir, int inverse);
+
+/* Tiled shared-memory transpose of every k-plane: dst[k][i][j] = src[k][j][i] (DEVICE, out of place). */
+int cales_transpose_xy(cales_solver* s, const double* src_dev, double* dst_dev);
+
+/* Per-phase device timing of cales_step (CUDA events; off by default). */
+int cales_set_timing(cales_solver* s, int on);
+
+/* Number of kernels cales_step launches per call with the current parameters (for bench.py's gpu_launches). */
+int cales_launches_per_step(cales_solver* s);
+
+/* max|div|, bulk velocity, kinetic energy, forcing, Newton iterations, NaN count, phase timings.  Synchronises. */
+int cales_diagnostics(cales_solver* s, cales_diag* out);
+
+const char* cales_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,448 @@
+// cales.cu -- C ABI (include/cales.h) and stream-ordered orchestration of one RK3 step of CaLES on one B200.
+//
+// Alg. 1 per substep:  K_rhs [-> K_cn_z x3] -> bulk sum -> K_fft_x_fwd(div fused) -> K_fft_y ->
+// K_poisson_z -> K_fft_y(inv) -> K_fft_x_inv -> K_correct -> K_wall_stress -> K_smag | K_dsm_*.
+// Everything is enqueued on the caller's stream; no host synchronisation inside a step; scalars (bulk shift,
+// dynamic coefficients, Newton iteration count) stay in device memory.
+#include "../../include/cales.h"
+#include "cales_common.cuh"
+#include "cales_fft.cuh"
+#include "cales_poisson.cuh"
+#include "cales_momentum.cuh"
+#include "cales_closures.cuh"
+#include "cales_host.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+using namespace cales;
+
+extern "C" const char* cales_last_error(void) { return g_err.c_str(); }
+
+#define CUDA_TRY(expr)                                                                                     \
+  do {                                                                                                     \
+    cudaError_t e_ = (expr);                                                                               \
+    if (e_ != cudaSuccess) return fail(CALES_ECUDA, std::string(#expr) + ": " + cudaGetErrorString(e_));   \
+  } while (0)
+
+struct cales_solver {
+  cales_params P;
+  Ctx c;
+  cudaStream_t st;
+  long long N, nxy;
+  // fields
+  double *u, *v, *w, *p, *nut, *us, *vs, *ws, *Ru, *Rv, *Rw, *W, *CP, *CQ, *smag;
+  double *tau;
+  // tables
+  double *dzf, *dzc, *zc, *ak, *ck, *lamx, *lamy, *cncoef, *partial, *stage1, *scal, *dsm_part, *dsm_cs;
+  double2 *twx, *twy, *dctw;
+  int* maxit;
+  FftPlan plx, ply;
+  PoissonTabs pt;
+  WallGeom wg;
+  int xB, yTI; size_t x_smem, y_smem; int x_threads, y_threads;
+  dim3 pgrid, pblock;   // point kernels
+  long long nblk;
+  bool fresh;
+  int timing; cudaEvent_t ev[3][7]; bool ev_valid;
+  int launches;
+};
+
+static size_t al32(size_t n) { return (n + 31) / 32 * 32; }
+
+// Carve the workspace.  With base == nullptr only the size is computed.
+static size_t carve(cales_solver* s, const cales_params* p, double* base) {
+  const size_t N = (size_t)p->nx * p->ny * p->nz, nxy = (size_t)p->nx * p->ny;
+  size_t off = 0;
+  auto take = [&](size_t n) { double* r = base ? base + off : nullptr; off += al32(n); return r; };
+  double* f[12];
+  for (int q = 0; q < 12; ++q) f[q] = take(N);
+  double* CP = take(N);
+  double* CQ = p->bc_z == CALES_BC_PERIODIC ? take(N) : nullptr;
+  double* smag = p->sgs_model == CALES_SGS_DSMAG ? take(N) : nullptr;
+  double* tau = take(4 * nxy);
+  double* dzf = take(p->nz + 2); double* dzc = take(p->nz + 2); double* zc = take(p->nz);
+  double* ak = take(p->nz); double* ck = take(p->nz);
+  double* lamx = take(p->nx); double* lamy = take(p->ny);
+  double* twx = take(2 * (size_t)p->nx); double* twy = take(2 * (size_t)p->ny); double* dctw = take(2 * ((size_t)p->ny / 2 + 1));
+  double* cncoef = take(6 * (size_t)p->nz);
+  const size_t nblk = (size_t)((p->nx + 31) / 32) * ((p->ny + 7) / 8) * p->nz;
+  double* partial = take(nblk > nxy ? nblk : nxy);
+  double* stage1 = take(4 * 1024);
+  double* scal = take(32);
+  const size_t ntx = (p->nx + DSM_TX - 1) / DSM_TX;
+  double* dsm_part = p->sgs_model == CALES_SGS_DSMAG ? take((size_t)p->nz * p->ny * ntx * 2) : nullptr;
+  double* dsm_cs = p->sgs_model == CALES_SGS_DSMAG ? take((size_t)p->nz * p->ny) : nullptr;
+  if (s && base) {
+    s->u = f[0]; s->v = f[1]; s->w = f[2]; s->p = f[3]; s->nut = f[4]; s->us = f[5]; s->vs = f[6]; s->ws = f[7];
+    s->Ru = f[8]; s->Rv = f[9]; s->Rw = f[10]; s->W = f[11]; s->CP = CP; s->CQ = CQ; s->smag = smag; s->tau = tau;
+    s->dzf = dzf; s->dzc = dzc; s->zc = zc; s->ak = ak; s->ck = ck; s->lamx = lamx; s->lamy = lamy;
+    s->twx = reinterpret_cast<double2*>(twx); s->twy = reinterpret_cast<double2*>(twy); s->dctw = reinterpret_cast<double2*>(dctw);
+    s->cncoef = cncoef; s->partial = partial; s->stage1 = stage1; s->scal = scal; s->maxit = reinterpret_cast<int*>(scal + 16);
+    s->dsm_part = dsm_part; s->dsm_cs = dsm_cs; s->nblk = (long long)nblk;
+  }
+  return off * sizeof(double);
+}
+
+extern "C" void cales_default_params(cales_params* p) {
+  if (!p) return;
+  std::memset(p, 0, sizeof(*p));
+  p->nu = 1e-3; p->cs = 0.17; p->aplus = 25.0; p->dsm_avg_xy_plane = 1; p->kappa = 0.41; p->B = 5.2; p->wm_tol = 1e-4; p->wm_maxit = 50;
+}
+
+extern "C" size_t cales_workspace_bytes(const cales_params* p) {
+  if (validate(p) != CALES_OK) return 0;
+  return carve(nullptr, p, nullptr);
+}
+
+static int check_launch(cales_solver* s, const char* what) {
+  ++s->launches;
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(CALES_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
+  return CALES_OK;
+}
+#define LAUNCH_TRY(what)                                  \
+  do { int rc_ = check_launch(s, what); if (rc_) return rc_; } while (0)
+
+extern "C" int cales_create(const cales_params* p, cales_solver** out) {
+  if (!out) return fail(CALES_EINVAL, "null output pointer");
+  *out = nullptr;
+  int rc = validate(p);
+  if (rc) return rc;
+  if (!p->workspace) return fail(CALES_EINVAL, "null workspace");
+  if (((size_t)p->workspace) % 256) return fail(CALES_EINVAL, "workspace must be 256-byte aligned");
+  const size_t need = carve(nullptr, p, nullptr);
+  if (p->workspace_bytes < need) return fail(CALES_EINVAL, "workspace too small");
+  CUDA_TRY(cudaSetDevice(p->device));
+  HostSetup H;
+  if ((rc = build_setup(p, H))) return rc;
+  cales_solver* s = new cales_solver();
+  s->P = H.P;
+  s->st = (cudaStream_t)p->cuda_stream;
+  const int nx = p->nx, ny = p->ny, nz = p->nz;
+  s->N = (long long)nx * ny * nz; s->nxy = (long long)nx * ny;
+  carve(s, p, (double*)p->workspace);
+  // ---- upload the tables
+  auto up = [&](double* dst, const std::vector<double>& src, size_t n) { return cudaMemcpyAsync(dst, src.data(), n * sizeof(double), cudaMemcpyHostToDevice, s->st); };
+  cudaError_t e = cudaSuccess;
+  if (e == cudaSuccess) e = cudaMemsetAsync(p->workspace, 0, need, s->st);
+  if (e == cudaSuccess) e = up(s->dzf, H.dzf, nz + 2);
+  if (e == cudaSuccess) e = up(s->dzc, H.dzc, nz + 1);
+  if (e == cudaSuccess) e = up(s->zc, H.zc, nz);
+  if (e == cudaSuccess) e = up(s->ak, H.ak, nz);
+  if (e == cudaSuccess) e = up(s->ck, H.ck, nz);
+  if (e == cudaSuccess) e = up(s->lamx, H.lamx, nx);
+  if (e == cudaSuccess) e = up(s->lamy, H.lamy, ny);
+  if (e == cudaSuccess) e = up(reinterpret_cast<double*>(s->twx), H.twx, H.twx.size());
+  if (e == cudaSuccess) e = up(reinterpret_cast<double*>(s->twy), H.twy, H.twy.size());
+  if (e == cudaSuccess) e = up(reinterpret_cast<double*>(s->dctw), H.dctw, H.dctw.size());
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s->st);
+  if (e != cudaSuccess) { delete s; return fail(CALES_ECUDA, std::string("table upload: ") + cudaGetErrorString(e)); }
+  s->c = H.c;
+  s->c.dzf = s->dzf + 1; s->c.dzc = s->dzc + 1; s->c.zc = s->zc; s->c.tau = s->tau;
+  s->pt.ak = s->ak; s->pt.ck = s->ck; s->pt.lamx = s->lamx; s->pt.lamy = s->lamy;
+  s->wg = H.wg;
+  s->plx = H.plx; s->plx.tw = s->twx;
+  s->ply = H.ply; s->ply.tw = s->twy; s->ply.dctw = s->dctw;
+  s->xB = H.xB; s->x_smem = H.x_smem; s->x_threads = H.x_threads;
+  s->yTI = H.yTI; s->y_smem = H.y_smem; s->y_threads = H.y_threads;
+  e = cudaFuncSetAttribute(k_fft_x_fwd<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fft_x_fwd<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fft_x_inv, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fft_y, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dsm_pass1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(DSM_SMEM_DOUBLES * sizeof(double)));
+  if (e != cudaSuccess) { delete s; return fail(CALES_ECUDA, std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e)); }
+  s->pblock = dim3(32, 8, 1);
+  s->pgrid = dim3((nx + 31) / 32, (ny + 7) / 8, nz);
+  s->fresh = false; s->timing = 0; s->ev_valid = false; s->launches = 0;
+  for (int a = 0; a < 3; ++a) for (int b = 0; b < 7; ++b) s->ev[a][b] = nullptr;
+  *out = s;
+  return CALES_OK;
+}
+
+extern "C" int cales_create_basic(int nx, int ny, int nz, double lx, double ly, double lz, int zstretch, double zstretch_factor,
+                                  int bc_y, int bc_z, double nu, int sgs_model, int wall_model, int implicit_z,
+                                  void* workspace, size_t workspace_bytes, void* cuda_stream, int device, cales_solver** out) {
+  cales_params p; cales_default_params(&p);
+  p.nx = nx; p.ny = ny; p.nz = nz; p.lx = lx; p.ly = ly; p.lz = lz; p.zstretch = zstretch; p.zstretch_factor = zstretch_factor;
+  p.bc_y = bc_y; p.bc_z = bc_z; p.nu = nu; p.sgs_model = sgs_model; p.wall_model = wall_model; p.implicit_z = implicit_z;
+  p.workspace = workspace; p.workspace_bytes = workspace_bytes; p.cuda_stream = cuda_stream; p.device = device;
+  return cales_create(&p, out);
+}
+
+extern "C" int cales_destroy(cales_solver* s) {
+  if (!s) return CALES_OK;
+  for (int a = 0; a < 3; ++a) for (int b = 0; b < 7; ++b) if (s->ev[a][b]) cudaEventDestroy(s->ev[a][b]);
+  delete s;
+  return CALES_OK;
+}
+
+static double* field_ptr(cales_solver* s, int f) {
+  switch (f) { case CALES_U: return s->u; case CALES_V: return s->v; case CALES_W: return s->w; case CALES_P: return s->p; case CALES_NUT: return s->nut; }
+  return nullptr;
+}
+
+extern "C" int cales_set_field(cales_solver* s, int field, const double* src, int on_device) {
+  if (!s || !src) return fail(CALES_EINVAL, "null argument");
+  double* d = field_ptr(s, field);
+  if (!d) return fail(CALES_EINVAL, "bad field id");
+  CUDA_TRY(cudaMemcpyAsync(d, src, s->N * sizeof(double), on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, s->st));
+  if (!on_device) CUDA_TRY(cudaStreamSynchronize(s->st));
+  if (field <= CALES_W) s->fresh = false;
+  return CALES_OK;
+}
+extern "C" int cales_get_field(cales_solver* s, int field, double* dst, int on_device) {
+  if (!s || !dst) return fail(CALES_EINVAL, "null argument");
+  double* d = field_ptr(s, field);
+  if (!d) return fail(CALES_EINVAL, "bad field id");
+  CUDA_TRY(cudaMemcpyAsync(dst, d, s->N * sizeof(double), on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, s->st));
+  if (!on_device) CUDA_TRY(cudaStreamSynchronize(s->st));
+  return CALES_OK;
+}
+
+// ---- building blocks ------------------------------------------------------------------------------------------
+static int run_transform_x_fwd(cales_solver* s, const double* src, const DivSrc* ds, double* dst) {
+  const long long nlines = (long long)s->c.ny * s->c.nz;
+  const unsigned grid = (unsigned)((nlines + s->xB - 1) / s->xB);
+  if (ds) k_fft_x_fwd<true><<<grid, s->x_threads, s->x_smem, s->st>>>(s->c, s->plx, s->xB, nullptr, *ds, dst);
+  else { DivSrc z{nullptr, nullptr, nullptr, 0.0}; k_fft_x_fwd<false><<<grid, s->x_threads, s->x_smem, s->st>>>(s->c, s->plx, s->xB, src, z, dst); }
+  LAUNCH_TRY("k_fft_x_fwd");
+  return CALES_OK;
+}
+static int run_transform_x_inv(cales_solver* s, const double* src, double* dst) {
+  const long long nlines = (long long)s->c.ny * s->c.nz;
+  const unsigned grid = (unsigned)((nlines + s->xB - 1) / s->xB);
+  k_fft_x_inv<<<grid, s->x_threads, s->x_smem, s->st>>>(s->c, s->plx, s->xB, src, dst);
+  LAUNCH_TRY("k_fft_x_inv");
+  return CALES_OK;
+}
+static int run_transform_y(cales_solver* s, double* A, int inverse) {
+  dim3 grid((s->c.nx + s->yTI - 1) / s->yTI, s->c.nz);
+  k_fft_y<<<grid, s->y_threads, s->y_smem, s->st>>>(s->c, s->ply, s->yTI, s->c.bc_y == BC_WALL ? 1 : 0, inverse, A);
+  LAUNCH_TRY("k_fft_y");
+  return CALES_OK;
+}
+static int run_poisson_z(cales_solver* s, double* A) {
+  const int th = 128;
+  k_poisson_z<<<(unsigned)((s->nxy + th - 1) / th), th, 0, s->st>>>(s->c, s->pt, A, s->CP, s->CQ);
+  LAUNCH_TRY("k_poisson_z");
+  return CALES_OK;
+}
+// spectral part of the Poisson solve, W already holds the x-transformed right-hand side
+static int run_poisson_core(cales_solver* s) {
+  int rc;
+  if ((rc = run_transform_y(s, s->W, 0))) return rc;
+  if ((rc = run_poisson_z(s, s->W))) return rc;
+  if ((rc = run_transform_y(s, s->W, 1))) return rc;
+  return CALES_OK;
+}
+static int run_wall_stress(cales_solver* s) {
+  if (!s->c.wall_model) return CALES_OK;
+  CUDA_TRY(cudaMemsetAsync(s->maxit, 0, sizeof(int), s->st));
+  dim3 grid(s->pgrid.x, s->pgrid.y, 4);
+  k_wall_stress<<<grid, s->pblock, 0, s->st>>>(s->c, s->wg, s->u, s->v, s->tau, s->maxit);
+  LAUNCH_TRY("k_wall_stress");
+  return CALES_OK;
+}
+static int run_eddy_viscosity(cales_solver* s, const double* u, const double* v, const double* w, double* nut) {
+  if (s->c.sgs == CALES_SGS_NONE) {
+    k_fill<<<1184, 256, 0, s->st>>>(nut, s->N, 0.0);
+    LAUNCH_TRY("k_fill");
+  } else if (s->c.sgs == CALES_SGS_SMAG) {
+    k_smag<<<s->pgrid, s->pblock, 0, s->st>>>(s->c, u, v, w, nut);
+    LAUNCH_TRY("k_smag");
+  } else {
+    dim3 grid((s->c.nx + DSM_TX - 1) / DSM_TX, (s->c.ny + DSM_TY - 1) / DSM_TY, s->c.nz);
+    k_dsm_pass1<<<grid, dim3(DSM_TX, DSM_TY), DSM_SMEM_DOUBLES * sizeof(double), s->st>>>(s->c, u, v, w, s->smag, s->dsm_part);
+    LAUNCH_TRY("k_dsm_pass1");
+    k_dsm_coef<<<s->c.nz, 128, 0, s->st>>>(s->c, s->dsm_part, (int)grid.x, s->dsm_cs);
+    LAUNCH_TRY("k_dsm_coef");
+    k_dsm_nut<<<s->pgrid, s->pblock, 0, s->st>>>(s->c, s->dsm_cs, s->smag, nut);
+    LAUNCH_TRY("k_dsm_nut");
+  }
+  return CALES_OK;
+}
+// Alg. 2 on the current velocity, then nu_t (Alg. 1 l.2 / l.12)
+static int refresh_closures(cales_solver* s) {
+  int rc;
+  if ((rc = run_wall_stress(s))) return rc;
+  if ((rc = run_eddy_viscosity(s, s->u, s->v, s->w, s->nut))) return rc;
+  s->fresh = true;
+  return CALES_OK;
+}
+
+static void mark(cales_solver* s, int rk, int b) {
+  if (!s->timing) return;
+  if (!s->ev[rk][b]) cudaEventCreate(&s->ev[rk][b]);
+  cudaEventRecord(s->ev[rk][b], s->st);
+}
+
+static int substep(cales_solver* s, int rk, double dt) {
+  int rc;
+  double al, be, ga; rk3_coeffs(rk, al, be, ga);
+  const Ctx& c = s->c;
+  const bool cfr = c.const_flow_rate != 0, imp = c.implicit_z != 0;
+  mark(s, rk, 0);
+  RhsArgs a;
+  a.u = s->u; a.v = s->v; a.w = s->w; a.p = s->p; a.nut = s->nut;
+  a.Ru0 = s->Ru; a.Rv0 = s->Rv; a.Rw0 = s->Rw; a.Ru1 = s->Ru; a.Rv1 = s->Rv; a.Rw1 = s->Rw;
+  a.us = s->us; a.vs = s->vs; a.ws = s->ws; a.dt = dt; a.al = al; a.be = be; a.ga = ga; a.store_R = rk < 2 ? 1 : 0;
+  k_rhs<<<s->pgrid, s->pblock, 0, s->st>>>(c, a, (cfr && !imp) ? s->partial : nullptr);
+  LAUNCH_TRY("k_rhs");
+  mark(s, rk, 1);
+  long long npart = s->nblk;
+  if (imp) {
+    const double cimp = 0.5 * ga * c.nu * dt;
+    k_cn_coef<<<1, 32, 0, s->st>>>(c, cimp, s->cncoef);
+    LAUNCH_TRY("k_cn_coef");
+    const int th = 128; const unsigned g = (unsigned)((s->nxy + th - 1) / th);
+    k_cn_z<<<g, th, 0, s->st>>>(c, s->cncoef, 0, s->us, cfr ? s->partial : nullptr); LAUNCH_TRY("k_cn_z(u)");
+    k_cn_z<<<g, th, 0, s->st>>>(c, s->cncoef, 1, s->vs, nullptr); LAUNCH_TRY("k_cn_z(v)");
+    k_cn_z<<<g, th, 0, s->st>>>(c, s->cncoef, 2, s->ws, nullptr); LAUNCH_TRY("k_cn_z(w)");
+    npart = g;
+  }
+  mark(s, rk, 2);
+  if (cfr) {
+    const int g1 = (int)(npart < 1024 ? npart : 1024);
+    k_sum_stage1<<<g1, 256, 0, s->st>>>(s->partial, npart, s->stage1); LAUNCH_TRY("k_sum_stage1");
+    k_bulk_finish<<<1, 256, 0, s->st>>>(c, s->stage1, g1, ga * dt, s->scal); LAUNCH_TRY("k_bulk_finish");
+  }
+  DivSrc ds{s->us, s->vs, s->ws, 1.0 / (ga * dt)};
+  if ((rc = run_transform_x_fwd(s, nullptr, &ds, s->W))) return rc;
+  if ((rc = run_poisson_core(s))) return rc;
+  if ((rc = run_transform_x_inv(s, s->W, s->W))) return rc;
+  mark(s, rk, 3);
+  CorrArgs ca;
+  ca.phi = s->W; ca.us = s->us; ca.vs = s->vs; ca.ws = s->ws; ca.u = s->u; ca.v = s->v; ca.w = s->w; ca.p = s->p;
+  ca.shift = cfr ? s->scal : nullptr; ca.gdt = ga * dt; ca.cimp = imp ? 0.5 * ga * c.nu * dt : 0.0; ca.update_p = 1;
+  k_correct<<<s->pgrid, s->pblock, 0, s->st>>>(c, ca);
+  LAUNCH_TRY("k_correct");
+  mark(s, rk, 4);
+  if ((rc = run_wall_stress(s))) return rc;
+  mark(s, rk, 5);
+  if ((rc = run_eddy_viscosity(s, s->u, s->v, s->w, s->nut))) return rc;
+  mark(s, rk, 6);
+  return CALES_OK;
+}
+
+extern "C" int cales_step(cales_solver* s, double dt) {
+  if (!s || !(dt > 0.0)) return fail(CALES_EINVAL, "bad step arguments");
+  int rc;
+  s->launches = 0;
+  if (!s->fresh && (rc = refresh_closures(s))) return rc;
+  for (int rk = 0; rk < 3; ++rk) if ((rc = substep(s, rk, dt))) return rc;
+  s->ev_valid = s->timing != 0;
+  return CALES_OK;
+}
+
+extern "C" int cales_launches_per_step(cales_solver* s) {
+  if (!s) return 0;
+  const Ctx& c = s->c;
+  int per = 1 /*rhs*/ + (c.implicit_z ? 4 : 0) + (c.const_flow_rate ? 2 : 0) + 5 /*solver*/ + 1 /*correct*/ + (c.wall_model ? 1 : 0) +
+            (c.sgs == CALES_SGS_DSMAG ? 3 : 1);
+  return 3 * per;
+}
+
+extern "C" int cales_poisson_solve(cales_solver* s, const double* rhs, double* phi) {
+  if (!s || !rhs || !phi) return fail(CALES_EINVAL, "null argument");
+  int rc;
+  if ((rc = run_transform_x_fwd(s, rhs, nullptr, s->W))) return rc;
+  if ((rc = run_poisson_core(s))) return rc;
+  if ((rc = run_transform_x_inv(s, s->W, phi))) return rc;
+  return CALES_OK;
+}
+
+extern "C" int cales_eddy_viscosity(cales_solver* s, const double* u, const double* v, const double* w, double* nut) {
+  if (!s) return fail(CALES_EINVAL, "null solver");
+  const bool own = !u && !v && !w;
+  if (!own && (!u || !v || !w)) return fail(CALES_EINVAL, "u, v, w must be all given or all NULL");
+  return run_eddy_viscosity(s, own ? s->u : u, own ? s->v : v, own ? s->w : w, nut ? nut : s->nut);
+}
+
+extern "C" int cales_wall_stress(cales_solver* s, double* tau_dev) {
+  if (!s) return fail(CALES_EINVAL, "null solver");
+  if (!s->c.wall_model) return fail(CALES_EINVAL, "solver has no wall model");
+  int rc = run_wall_stress(s);
+  if (rc) return rc;
+  if (tau_dev) CUDA_TRY(cudaMemcpyAsync(tau_dev, s->tau, 4 * s->nxy * sizeof(double), cudaMemcpyDeviceToDevice, s->st));
+  return CALES_OK;
+}
+
+extern "C" int cales_project(cales_solver* s) {
+  if (!s) return fail(CALES_EINVAL, "null solver");
+  int rc;
+  DivSrc ds{s->u, s->v, s->w, 1.0};
+  if ((rc = run_transform_x_fwd(s, nullptr, &ds, s->W))) return rc;
+  if ((rc = run_poisson_core(s))) return rc;
+  if ((rc = run_transform_x_inv(s, s->W, s->W))) return rc;
+  CorrArgs ca;
+  ca.phi = s->W; ca.us = s->u; ca.vs = s->v; ca.ws = s->w; ca.u = s->u; ca.v = s->v; ca.w = s->w; ca.p = s->p;
+  ca.shift = nullptr; ca.gdt = 1.0; ca.cimp = 0.0; ca.update_p = 0;
+  k_correct<<<s->pgrid, s->pblock, 0, s->st>>>(s->c, ca);
+  LAUNCH_TRY("k_correct");
+  s->fresh = false;
+  return CALES_OK;
+}
+
+extern "C" int cales_get_cs(cales_solver* s, double* cs_dev) {
+  if (!s || !cs_dev) return fail(CALES_EINVAL, "null argument");
+  if (s->c.sgs != CALES_SGS_DSMAG) return fail(CALES_EINVAL, "not a dynamic-model solver");
+  const size_t n = s->c.dsm_plane ? (size_t)s->c.nz : (size_t)s->c.nz * s->c.ny;
+  CUDA_TRY(cudaMemcpyAsync(cs_dev, s->dsm_cs, n * sizeof(double), cudaMemcpyDeviceToDevice, s->st));
+  return CALES_OK;
+}
+
+extern "C" int cales_transform(cales_solver* s, double* f, int dir, int inverse) {
+  if (!s || !f) return fail(CALES_EINVAL, "null argument");
+  if (dir == 0) return inverse ? run_transform_x_inv(s, f, f) : run_transform_x_fwd(s, f, nullptr, f);
+  if (dir == 1) return run_transform_y(s, f, inverse ? 1 : 0);
+  return fail(CALES_EINVAL, "dir must be 0 (x) or 1 (y)");
+}
+
+extern "C" int cales_transpose_xy(cales_solver* s, const double* src, double* dst) {
+  if (!s || !src || !dst || src == dst) return fail(CALES_EINVAL, "bad transpose arguments");
+  dim3 grid((s->c.nx + 31) / 32, (s->c.ny + 31) / 32, s->c.nz);
+  k_transpose_xy<<<grid, dim3(32, 8), 0, s->st>>>(s->c.nx, s->c.ny, src, dst);
+  LAUNCH_TRY("k_transpose_xy");
+  return CALES_OK;
+}
+
+extern "C" int cales_set_timing(cales_solver* s, int on) {
+  if (!s) return fail(CALES_EINVAL, "null solver");
+  s->timing = on ? 1 : 0; s->ev_valid = false;
+  return CALES_OK;
+}
+
+extern "C" int cales_diagnostics(cales_solver* s, cales_diag* out) {
+  if (!s || !out) return fail(CALES_EINVAL, "null argument");
+  std::memset(out, 0, sizeof(*out));
+  const long long nb = s->nblk;
+  double* part = s->CP;   // scratch (4*nblk <= N)
+  k_diag<<<s->pgrid, s->pblock, 0, s->st>>>(s->c, s->u, s->v, s->w, s->p, part);
+  LAUNCH_TRY("k_diag");
+  const int g1 = (int)(nb < 1024 ? nb : 1024);
+  k_max_stage<<<g1, 256, 0, s->st>>>(part, nb, s->stage1); LAUNCH_TRY("k_max_stage");
+  for (int q = 1; q < 4; ++q) { k_sum_stage1<<<g1, 256, 0, s->st>>>(part + q * nb, nb, s->stage1 + q * 1024); LAUNCH_TRY("k_sum_stage1"); }
+  std::vector<double> h(4 * 1024); double scal[4]; int mi = 0;
+  CUDA_TRY(cudaMemcpyAsync(h.data(), s->stage1, h.size() * sizeof(double), cudaMemcpyDeviceToHost, s->st));
+  CUDA_TRY(cudaMemcpyAsync(scal, s->scal, sizeof(scal), cudaMemcpyDeviceToHost, s->st));
+  CUDA_TRY(cudaMemcpyAsync(&mi, s->maxit, sizeof(int), cudaMemcpyDeviceToHost, s->st));
+  CUDA_TRY(cudaStreamSynchronize(s->st));
+  double md = 0, ub = 0, ke = 0, bad = 0;
+  for (int q = 0; q < g1; ++q) { md = std::fmax(md, h[q]); ub += h[1024 + q]; ke += h[2048 + q]; bad += h[3072 + q]; }
+  const double vol = (double)s->c.nx * s->c.ny * s->c.lz;
+  out->max_div = md; out->u_bulk = ub / vol; out->kinetic_energy = ke / vol; out->nan_count = (int)bad;
+  out->forcing = s->c.const_flow_rate ? scal[1] : 0.0; out->wm_max_iters = mi;
+  if (s->ev_valid) {
+    double acc[6] = {0, 0, 0, 0, 0, 0};
+    for (int rk = 0; rk < 3; ++rk) for (int b = 0; b < 6; ++b) {
+      float ms = 0.f;
+      if (s->ev[rk][b] && s->ev[rk][b + 1] && cudaEventElapsedTime(&ms, s->ev[rk][b], s->ev[rk][b + 1]) == cudaSuccess) acc[b] += ms;
+    }
+    out->ms_rhs = acc[0]; out->ms_implicit = acc[1]; out->ms_solver = acc[2]; out->ms_correction = acc[3]; out->ms_wall = acc[4]; out->ms_sgs = acc[5];
+  }
+  return CALES_OK;
+}

@@ -1,0 +1,124 @@
+// cales_common.cuh -- device-side context, boundary-condition accessors and small reductions.
+//
+// The GPU keeps NO ghost layers: every array holds interior values only,
+// [k][j][i] with x fastest, and the boundary conditions of PAPER.md:142 / Alg. 2 are
+// applied by index arithmetic when a neighbour is read.  The accessors below are the single place where
+// that happens.
+#pragma once
+#include <cuda_runtime.h>
+#include <math.h>
+
+#define CALES_HD __host__ __device__ __forceinline__
+
+namespace cales {
+
+enum { BC_PER = 0, BC_WALL = 1 };
+enum { GH_VISC = 0, GH_STRAIN = 1 };  // ghost of the wall-parallel velocity at a wall-model wall
+
+// Grid, options and table pointers, passed by value to every kernel.
+struct Ctx {
+  int nx, ny, nz;
+  int bc_y, bc_z, wall_model, sgs, van_driest, implicit_z, dsm_plane, dsm_clip_total, const_flow_rate;
+  int wm_maxit;
+  long long N;     // nx*ny*nz
+  long long nxy;   // nx*ny
+  double dx, dy, lz, nu, cs, aplus, alpha, kappa, Blog, h_wm, wm_tol, u_bulk;
+  // 1-D grid tables in device memory, offset so that the ghost entries are addressable:
+  const double* dzf;   // dzf[-1 .. nz]   cell heights (ghost = neighbour's / wrapped)
+  const double* dzc;   // dzc[-1 .. nz-1] centre spacings across face k+1 (mirrored ghost centre at walls)
+  const double* zc;    // zc[0 .. nz-1]
+  const double* tau;   // wall stress planes [wall][comp][ny][nx]
+};
+
+CALES_HD long long idx3(const Ctx& c, int i, int j, int k) { return (long long)i + (long long)c.nx * ((long long)j + (long long)c.ny * (long long)k); }
+CALES_HD int wrapi(int i, int n) { return i < 0 ? i + n : (i >= n ? i - n : i); }
+
+// Velocity component COMP (0 u, 1 v, 2 w) at (i,j,k) with -1 <= i <= nx, -1 <= j <= ny, -1 <= k <= nz.
+// Ghosts compose in the order z, then x, then y (as an explicit ghost fill would):
+//   x periodic;  y periodic, or walls: u, w mirrored (no slip), v = 0 on the wall faces and beyond;
+//   z periodic, or walls: w = 0 on the wall faces and beyond; u, v: no-slip mirror, or with the wall model
+//   GH_VISC   ghost = q0 - tau * dzc_wall / nu       (the modelled stress is the wall viscous flux)
+//   GH_STRAIN ghost = linear extrapolation of q0, q1 (one-sided derivative for the strain rate).
+template <int COMP>
+CALES_HD double velg(const Ctx& c, const double* __restrict__ q, int i, int j, int k, int mode) {
+  i = wrapi(i, c.nx);
+  double sy = 1.0;
+  if (c.bc_y == BC_PER) j = wrapi(j, c.ny);
+  else {
+    if (COMP == 1) { if (j < 0 || j >= c.ny - 1) return 0.0; }
+    else { if (j < 0) { j = 0; sy = -1.0; } else if (j >= c.ny) { j = c.ny - 1; sy = -1.0; } }
+  }
+  if (c.bc_z == BC_PER) return sy * q[idx3(c, i, j, wrapi(k, c.nz))];
+  if (COMP == 2) { if (k < 0 || k >= c.nz - 1) return 0.0; return sy * q[idx3(c, i, j, k)]; }
+  if (k >= 0 && k < c.nz) return sy * q[idx3(c, i, j, k)];
+  const bool bottom = k < 0;
+  const int k0 = bottom ? 0 : c.nz - 1;
+  const double q0 = q[idx3(c, i, j, k0)];
+  if (!c.wall_model) return -sy * q0;
+  if (mode == GH_VISC) {
+    const double t = c.tau[((long long)((bottom ? 0 : 2) + COMP) * c.ny + j) * c.nx + i];
+    const double dz = bottom ? c.dzc[-1] : c.dzc[c.nz - 1];
+    return sy * (q0 - t * dz / c.nu);
+  }
+  const int k1 = bottom ? 1 : c.nz - 2;
+  const double q1 = q[idx3(c, i, j, k1)];
+  const double r = bottom ? c.dzc[-1] / c.dzc[0] : c.dzc[c.nz - 1] / c.dzc[c.nz - 2];
+  return sy * (q0 + (q0 - q1) * r);
+}
+
+// Cell-centred scalar with ghost = sgn * interior at walls (sgn = +1: Neumann, p and phi; sgn = -1: nu_t,
+// which makes the edge viscosity and hence the SGS flux vanish on a wall) and periodic wrap otherwise.
+CALES_HD double scalg(const Ctx& c, const double* __restrict__ q, int i, int j, int k, double sgn) {
+  i = wrapi(i, c.nx);
+  double s = 1.0;
+  if (c.bc_y == BC_PER) j = wrapi(j, c.ny);
+  else { if (j < 0) { j = 0; s *= sgn; } else if (j >= c.ny) { j = c.ny - 1; s *= sgn; } }
+  if (c.bc_z == BC_PER) k = wrapi(k, c.nz);
+  else { if (k < 0) { k = 0; s *= sgn; } else if (k >= c.nz) { k = c.nz - 1; s *= sgn; } }
+  return s * q[idx3(c, i, j, k)];
+}
+
+// RK3 coefficients of PAPER.md:100.
+CALES_HD void rk3_coeffs(int rk, double& al, double& be, double& ga) {
+  al = rk == 0 ? 8.0 / 15.0 : (rk == 1 ? 5.0 / 12.0 : 3.0 / 4.0);
+  be = rk == 0 ? 0.0 : (rk == 1 ? -17.0 / 60.0 : -5.0 / 12.0);
+  ga = al + be;
+}
+
+#ifdef __CUDACC__
+// Sum over the thread block (result valid in thread 0).  blockDim.x*y*z <= 1024, multiple of 32.
+__device__ __forceinline__ double block_sum(double v, double* sh /* >= 32 doubles */) {
+  const int tid = threadIdx.x + blockDim.x * (threadIdx.y + blockDim.y * threadIdx.z);
+  const int nth = blockDim.x * blockDim.y * blockDim.z;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+  if ((tid & 31) == 0) sh[tid >> 5] = v;
+  __syncthreads();
+  double r = 0.0;
+  if (tid < 32) {
+    r = (tid < (nth + 31) / 32) ? sh[tid] : 0.0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) r += __shfl_down_sync(0xffffffffu, r, o);
+  }
+  __syncthreads();
+  return r;
+}
+__device__ __forceinline__ double block_max(double v, double* sh) {
+  const int tid = threadIdx.x + blockDim.x * (threadIdx.y + blockDim.y * threadIdx.z);
+  const int nth = blockDim.x * blockDim.y * blockDim.z;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_down_sync(0xffffffffu, v, o));
+  if ((tid & 31) == 0) sh[tid >> 5] = v;
+  __syncthreads();
+  double r = 0.0;
+  if (tid < 32) {
+    r = (tid < (nth + 31) / 32) ? sh[tid] : 0.0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) r = fmax(r, __shfl_down_sync(0xffffffffu, r, o));
+  }
+  __syncthreads();
+  return r;
+}
+#endif
+
+}  // namespace cales

@@ -1,0 +1,149 @@
+// cales_host.h -- host-side setup shared by the CUDA library and the host kernel emulator of tests/emu:
+// parameter validation, grid metrics, eigenvalues, twiddle tables, wall-model sampling geometry, transform plans
+// and launch shapes.  Plain C++ (no CUDA runtime calls); no arithmetic of the time step itself lives here.
+#pragma once
+#include "../../include/cales.h"
+#include "cales_common.cuh"
+#include "cales_fft.cuh"
+#include "cales_closures.cuh"
+
+#include <cmath>
+#include <string>
+#include <vector>
+
+namespace cales {
+
+static thread_local std::string g_err;
+static inline int fail(int code, const std::string& m) { g_err = m; return code; }
+
+static inline bool smooth23(int n) { if (n < 1) return false; while (n % 2 == 0) n /= 2; while (n % 3 == 0) n /= 3; return n == 1; }
+
+static inline int validate(const cales_params* p) {
+  if (!p) return fail(CALES_EINVAL, "null parameters");
+  if (p->nx < 2 || p->ny < 2 || p->nz < 4) return fail(CALES_EINVAL, "grid too small (nx, ny >= 2, nz >= 4)");
+  if (!(p->lx > 0.0) || !(p->ly > 0.0) || !(p->lz > 0.0)) return fail(CALES_EINVAL, "box lengths must be positive");
+  if (!(p->nu > 0.0)) return fail(CALES_EINVAL, "nu must be positive");
+  if (p->nx % 2 || p->ny % 2) return fail(CALES_EUNSUPPORTED, "nx and ny must be even");
+  if (!smooth23(p->nx) || !smooth23(p->ny)) return fail(CALES_EUNSUPPORTED, "nx, ny must factor into 2 and 3");
+  if (p->nx > 12288 || p->ny > 8192) return fail(CALES_EUNSUPPORTED, "nx <= 12288 and ny <= 8192 (line must fit shared memory)");
+  if (p->nz > 65535) return fail(CALES_EUNSUPPORTED, "nz <= 65535");
+  if (p->bc_y != CALES_BC_PERIODIC && p->bc_y != CALES_BC_WALL) return fail(CALES_EINVAL, "bad bc_y");
+  if (p->bc_z != CALES_BC_PERIODIC && p->bc_z != CALES_BC_WALL) return fail(CALES_EINVAL, "bad bc_z");
+  if (p->zstretch < 0 || p->zstretch > 2) return fail(CALES_EINVAL, "bad zstretch");
+  if (p->zstretch == CALES_Z_USER && !p->zf_user) return fail(CALES_EINVAL, "zf_user is null");
+  if (p->bc_z == CALES_BC_PERIODIC && p->zstretch != CALES_Z_UNIFORM) return fail(CALES_EUNSUPPORTED, "periodic z requires a uniform grid");
+  if (p->sgs_model < 0 || p->sgs_model > 2) return fail(CALES_EINVAL, "bad sgs_model");
+  if (p->wall_model && p->bc_z != CALES_BC_WALL) return fail(CALES_EUNSUPPORTED, "wall model needs z walls");
+  if (p->implicit_z && p->bc_z != CALES_BC_WALL) return fail(CALES_EUNSUPPORTED, "implicit z needs z walls");
+  if (p->implicit_z && p->wall_model) return fail(CALES_EUNSUPPORTED, "wall model with implicit z is not supported");
+  if (p->wall_model && p->h_wm > 0.0 && !(p->h_wm < 0.5 * p->lz)) return fail(CALES_EINVAL, "h_wm must lie below the half height");
+  if (p->van_driest && (p->bc_z != CALES_BC_WALL || p->bc_y == CALES_BC_WALL || p->wall_model))
+    return fail(CALES_EUNSUPPORTED, "van Driest damping: z walls only, no wall model");
+  return CALES_OK;
+}
+
+static inline void make_plan(FftPlan& pl, int n) {
+  pl.n = n; pl.n2 = n / 2; pl.npass = 0; pl.tw = nullptr; pl.dctw = nullptr;
+  int m = pl.n2;
+  while (m % 4 == 0) { pl.radix[pl.npass++] = 4; m /= 4; }
+  while (m % 2 == 0) { pl.radix[pl.npass++] = 2; m /= 2; }
+  while (m % 3 == 0) { pl.radix[pl.npass++] = 3; m /= 3; }
+}
+
+struct HostSetup {
+  cales_params P;                 // with the defaults filled in
+  std::vector<double> dzf, dzc, zc, ak, ck, lamx, lamy, twx, twy, dctw;   // dzf: index k+1 holds dzf[k], k=-1..nz; dzc: k+1 holds dzc[k], k=-1..nz-1
+  Ctx c;                          // table pointers NOT set
+  WallGeom wg;
+  FftPlan plx, ply;               // twiddle pointers NOT set
+  int xB, yTI, x_threads, y_threads; size_t x_smem, y_smem;
+};
+
+static inline int build_setup(const cales_params* p, HostSetup& H) {
+  const double PI_ = 3.14159265358979323846264338327950288;
+  int rc = validate(p);
+  if (rc) return rc;
+  H.P = *p; H.P.zf_user = nullptr;
+  if (H.P.wm_tol <= 0.0) H.P.wm_tol = 1e-4;
+  if (H.P.wm_maxit <= 0) H.P.wm_maxit = 50;
+  if (H.P.kappa <= 0.0) H.P.kappa = 0.41;
+  if (H.P.aplus <= 0.0) H.P.aplus = 25.0;
+  const int nx = p->nx, ny = p->ny, nz = p->nz;
+  // ---- grid (S16 for the tanh map)
+  std::vector<double> zf(nz + 1);
+  H.zc.assign(nz, 0.0); H.dzf.assign(nz + 2, 0.0); H.dzc.assign(nz + 2, 0.0);
+  for (int k = 0; k <= nz; ++k) {
+    if (p->zstretch == CALES_Z_UNIFORM) zf[k] = p->lz * (double)k / (double)nz;
+    else if (p->zstretch == CALES_Z_TANH) { const double a = p->zstretch_factor; zf[k] = 0.5 * p->lz * (1.0 + std::tanh(a * (2.0 * k / (double)nz - 1.0)) / std::tanh(a)); }
+    else zf[k] = p->zf_user[k];
+  }
+  zf[0] = 0.0; zf[nz] = p->lz;
+  for (int k = 0; k < nz; ++k) {
+    H.zc[k] = 0.5 * (zf[k] + zf[k + 1]); H.dzf[k + 1] = zf[k + 1] - zf[k];
+    if (!(H.dzf[k + 1] > 0.0)) return fail(CALES_EINVAL, "z faces must increase");
+  }
+  const bool zper = p->bc_z == CALES_BC_PERIODIC;
+  if (zper) { H.dzf[0] = H.dzf[nz]; H.dzf[nz + 1] = H.dzf[1]; } else { H.dzf[0] = H.dzf[1]; H.dzf[nz + 1] = H.dzf[nz]; }
+  for (int k = 0; k < nz - 1; ++k) H.dzc[k + 1] = H.zc[k + 1] - H.zc[k];
+  if (zper) { H.dzc[0] = H.dzf[1]; H.dzc[nz] = H.dzf[1]; } else { H.dzc[0] = 2.0 * H.zc[0]; H.dzc[nz] = 2.0 * (p->lz - H.zc[nz - 1]); }   // mirrored ghost centre
+  H.ak.resize(nz); H.ck.resize(nz);
+  for (int k = 0; k < nz; ++k) { H.ak[k] = 1.0 / (H.dzf[k + 1] * H.dzc[k]); H.ck[k] = 1.0 / (H.dzf[k + 1] * H.dzc[k + 1]); }
+  // ---- eigenvalues of the 3-point operators in the packed layouts (ref. [28])
+  const double dx = p->lx / nx, dy = p->ly / ny;
+  H.lamx.resize(nx); H.lamy.resize(ny);
+  for (int i = 0; i < nx; ++i) {
+    const int m = i == 0 ? 0 : (i == 1 ? nx / 2 : i / 2);
+    const double sn = std::sin(PI_ * m / (double)nx); H.lamx[i] = -4.0 / (dx * dx) * sn * sn;
+  }
+  for (int j = 0; j < ny; ++j) {
+    double sn;
+    if (p->bc_y == CALES_BC_PERIODIC) { const int m = j == 0 ? 0 : (j == 1 ? ny / 2 : j / 2); sn = std::sin(PI_ * m / (double)ny); }
+    else sn = std::sin(PI_ * j / (2.0 * ny));
+    H.lamy[j] = -4.0 / (dy * dy) * sn * sn;
+  }
+  // ---- twiddles in extended precision, rounded once to fp64
+  H.twx.resize(2 * (size_t)nx); H.twy.resize(2 * (size_t)ny); H.dctw.resize(2 * ((size_t)ny / 2 + 1));
+  const long double PIL = 3.14159265358979323846264338327950288L;
+  for (int q = 0; q < nx; ++q) { const long double a = 2.0L * PIL * q / nx; H.twx[2 * q] = (double)cosl(a); H.twx[2 * q + 1] = (double)(-sinl(a)); }
+  for (int q = 0; q < ny; ++q) { const long double a = 2.0L * PIL * q / ny; H.twy[2 * q] = (double)cosl(a); H.twy[2 * q + 1] = (double)(-sinl(a)); }
+  for (int m = 0; m <= ny / 2; ++m) { const long double a = PIL * m / (2.0L * ny); H.dctw[2 * m] = (double)cosl(a); H.dctw[2 * m + 1] = (double)(-sinl(a)); }
+  // ---- device context (pointers are set by the owner of the tables)
+  Ctx& c = H.c;
+  c.nx = nx; c.ny = ny; c.nz = nz; c.N = (long long)nx * ny * nz; c.nxy = (long long)nx * ny;
+  c.bc_y = p->bc_y; c.bc_z = p->bc_z; c.wall_model = p->wall_model; c.sgs = p->sgs_model; c.van_driest = p->van_driest;
+  c.implicit_z = p->implicit_z; c.dsm_plane = p->dsm_avg_xy_plane; c.dsm_clip_total = p->dsm_clip_total; c.const_flow_rate = p->const_flow_rate;
+  c.wm_maxit = H.P.wm_maxit; c.dx = dx; c.dy = dy; c.lz = p->lz; c.nu = p->nu; c.cs = p->cs; c.aplus = H.P.aplus;
+  c.alpha = p->dsm_alpha2d > 0.0 ? p->dsm_alpha2d : std::cbrt(4.0);
+  c.kappa = H.P.kappa; c.Blog = p->B; c.h_wm = p->h_wm; c.wm_tol = H.P.wm_tol; c.u_bulk = p->u_bulk;
+  c.dzf = nullptr; c.dzc = nullptr; c.zc = nullptr; c.tau = nullptr;
+  // ---- wall-model sampling geometry (linear interpolation between locations 1 and 2)
+  for (int wall = 0; wall < 2; ++wall) {
+    auto dist = [&](int q) { return wall == 0 ? H.zc[q] : p->lz - H.zc[nz - 1 - q]; };
+    const double h = p->h_wm > 0.0 ? p->h_wm : dist(0);
+    int q1 = 0; while (q1 + 2 < nz / 2 && dist(q1 + 1) <= h) ++q1;
+    H.wg.wgt[wall] = (h - dist(q1)) / (dist(q1 + 1) - dist(q1));
+    H.wg.ka[wall] = wall == 0 ? q1 : nz - 1 - q1; H.wg.kb[wall] = wall == 0 ? q1 + 1 : nz - 2 - q1; H.wg.h[wall] = h;
+  }
+  // ---- transform plans and launch shapes
+  make_plan(H.plx, nx);
+  make_plan(H.ply, ny);
+  {
+    const size_t per_line = 16 * (size_t)nx;             // two ping-pong buffers of nx/2 complex
+    int B = (int)(98304 / per_line); if (B < 1) B = 1; if (B > 16) B = 16;
+    const long long nlines = (long long)ny * nz; if (B > nlines) B = (int)nlines;
+    H.xB = B; H.x_smem = (size_t)B * per_line;
+    const long long work = (long long)B * (nx / 2) / 2;
+    H.x_threads = work >= 512 ? 512 : (work >= 256 ? 256 : (work >= 128 ? 128 : 64));
+  }
+  {
+    const size_t per_col = 16 * (size_t)ny;
+    int TI = (int)(131072 / per_col); if (TI < 1) TI = 1; if (TI > 32) TI = 32; if (TI > nx) TI = nx;
+    int t2 = 1; while (t2 * 2 <= TI) t2 *= 2; TI = t2;   // power of two keeps the row segments aligned
+    H.yTI = TI; H.y_smem = (size_t)TI * per_col;
+    const long long work = (long long)TI * (ny / 2) / 2;
+    H.y_threads = work >= 512 ? 512 : (work >= 256 ? 256 : (work >= 128 ? 128 : 64));
+  }
+  return CALES_OK;
+}
+
+}  // namespace cales

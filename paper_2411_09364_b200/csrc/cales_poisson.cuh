@@ -1,0 +1,163 @@
+// cales_poisson.cuh -- tridiagonal solves along z: the Thomas step of the eigenfunction-expansion Poisson
+// solver and the Crank-Nicolson z solve of Eq. 21.
+//
+// One thread per (i,j) column, consecutive threads on consecutive i, so every load and store of a k-level is
+// coalesced.  The forward sweep leaves d' in place and c' in a scratch field; the backward sweep overwrites d'
+// with the solution.
+#pragma once
+#include "cales_common.cuh"
+
+namespace cales {
+
+struct PoissonTabs {
+  const double* ak;    // a_k = 1/(dzf[k] dzc[k-1])
+  const double* ck;    // c_k = 1/(dzf[k] dzc[k])
+  const double* lamx;  // eigenvalue of slot i of the packed half-complex x spectrum
+  const double* lamy;  // eigenvalue of row j (packed half-complex, or DCT-II mode j)
+};
+
+// Poisson column (i,j): [a_k, b_k, c_k] phi = f with b_k = -(a_k + c_k) + lam_x + lam_y, a_0 and c_{nz-1} dropped from
+// b at walls (Neumann) or wrapped (periodic z: cyclic Thomas via Sherman-Morrison).  The singular (0,0) mode drops the
+// dzf-weighted mean of f, pins phi[0] = 0, and returns the solution with zero dzf-weighted mean (S15).
+CALES_HD void poisson_column(const Ctx& c, const PoissonTabs& T, int i, int j, double* __restrict__ A, double* __restrict__ CP, double* __restrict__ CQ) {
+  const int nz = c.nz;
+  const long long col = (long long)i + (long long)c.nx * j, st = c.nxy;
+  const double lam = T.lamx[i] + T.lamy[j];
+  const bool per = c.bc_z == BC_PER;
+  const bool zero = (i == 0 && j == 0);
+  if (zero || !per) {
+    double mean = 0.0;
+    if (zero) {
+      for (int k = 0; k < nz; ++k) mean += A[col + st * k] * c.dzf[k];
+      mean /= c.lz;
+    }
+    double cp = 0.0, dp = 0.0;
+    for (int k = 0; k < nz; ++k) {
+      const double a = T.ak[k], cc = T.ck[k];
+      double b = lam - ((k > 0 || per) ? a : 0.0) - ((k < nz - 1 || per) ? cc : 0.0);
+      double d = A[col + st * k] - mean;
+      if (zero && k == 0) { cp = 0.0; dp = 0.0; }   // row 0: phi[0] = 0
+      else {
+        const double r = 1.0 / (b - a * cp);
+        cp = cc * r; dp = (d - a * dp) * r;
+      }
+      CP[col + st * k] = cp; A[col + st * k] = dp;
+    }
+    double x = dp;
+    double s = x * c.dzf[nz - 1];
+    for (int k = nz - 2; k >= 0; --k) {
+      x = A[col + st * k] - CP[col + st * k] * x;
+      A[col + st * k] = x;
+      s += x * c.dzf[k];
+    }
+    if (zero) {
+      s /= c.lz;
+      for (int k = 0; k < nz; ++k) A[col + st * k] -= s;
+    }
+    return;
+  }
+  // cyclic: A = T + u v^T, u = (g,0,..,0,c[n-1])^T, v = (1,0,..,0,a[0]/g)^T, g = -b[0]
+  const double a0 = T.ak[0], cn = T.ck[nz - 1];
+  const double b0 = lam - T.ak[0] - T.ck[0];
+  const double g = -b0;
+  double cp = 0.0, dp = 0.0, qp = 0.0;
+  for (int k = 0; k < nz; ++k) {
+    const double a = T.ak[k], cc = T.ck[k];
+    double b = lam - a - cc;
+    if (k == 0) b -= g;
+    if (k == nz - 1) b -= a0 * cn / g;
+    const double uu = k == 0 ? g : (k == nz - 1 ? cn : 0.0);
+    const double d = A[col + st * k];
+    const double r = 1.0 / (k == 0 ? b : b - a * cp);
+    cp = cc * r;
+    dp = (k == 0 ? d : d - a * dp) * r;
+    qp = (k == 0 ? uu : uu - a * qp) * r;
+    CP[col + st * k] = cp; A[col + st * k] = dp; CQ[col + st * k] = qp;
+  }
+  double y = dp, q = qp;
+  const double yn = y, qn = q;
+  for (int k = nz - 2; k >= 0; --k) {
+    const double cpk = CP[col + st * k];
+    y = A[col + st * k] - cpk * y;
+    q = CQ[col + st * k] - cpk * q;
+    A[col + st * k] = y; CQ[col + st * k] = q;
+  }
+  const double vy = y + a0 * yn / g, vq = q + a0 * qn / g;
+  const double f = vy / (1.0 + vq);
+  for (int k = 0; k < nz; ++k) A[col + st * k] -= f * CQ[col + st * k];
+}
+
+// Crank-Nicolson coefficients of Eq. 21 for substep constant cimp = gamma nu dt / 2, computed once per substep by one
+// thread: for the centred components (u, v; no-slip ghost folded into the diagonal) and for w (faces 0..nz-2).
+// Layout of `coef`: [0] lower a, [1] c' (modified upper), [2] 1/den for u,v; [3],[4],[5] the same for w.
+CALES_HD void cn_coefficients(const Ctx& c, double cimp, double* coef) {
+  const int nz = c.nz;
+  double cp = 0.0;
+  for (int k = 0; k < nz; ++k) {
+    const double ak = 1.0 / (c.dzf[k] * c.dzc[k - 1]), ck = 1.0 / (c.dzf[k] * c.dzc[k]);
+    double b = 1.0 + cimp * (ak + ck);
+    if (k == 0) b += cimp * ak;
+    if (k == nz - 1) b += cimp * ck;
+    const double a = -cimp * ak, cc = -cimp * ck;
+    const double r = 1.0 / (k == 0 ? b : b - a * cp);
+    cp = cc * r;
+    coef[0 * nz + k] = a; coef[1 * nz + k] = cp; coef[2 * nz + k] = r;
+  }
+  cp = 0.0;
+  for (int k = 0; k < nz - 1; ++k) {
+    const double ak = 1.0 / (c.dzc[k] * c.dzf[k]), ck = 1.0 / (c.dzc[k] * c.dzf[k + 1]);
+    const double b = 1.0 + cimp * (ak + ck);
+    const double a = -cimp * ak, cc = -cimp * ck;
+    const double r = 1.0 / (k == 0 ? b : b - a * cp);
+    cp = cc * r;
+    coef[3 * nz + k] = a; coef[4 * nz + k] = cp; coef[5 * nz + k] = r;
+  }
+  coef[3 * nz + nz - 1] = 0.0; coef[4 * nz + nz - 1] = 0.0; coef[5 * nz + nz - 1] = 0.0;
+}
+
+// Solve (1 - c L_zz) q* = d in place for one column; m = number of unknowns (nz for u, v; nz-1 for w).
+// Returns sum_k q*[k] dzf[k] (used for the bulk velocity of u*).
+CALES_HD double cn_column(const Ctx& c, const double* coef, int m, long long col, double* __restrict__ Q) {
+  const int nz = c.nz; const long long st = c.nxy;
+  const double* a = coef; const double* cp = coef + nz; const double* r = coef + 2 * nz;
+  double dp = 0.0;
+  for (int k = 0; k < m; ++k) {
+    dp = (k == 0 ? Q[col] : Q[col + st * k] - a[k] * dp) * r[k];
+    Q[col + st * k] = dp;
+  }
+  double x = dp, s = x * c.dzf[m - 1];
+  for (int k = m - 2; k >= 0; --k) {
+    x = Q[col + st * k] - cp[k] * x;
+    Q[col + st * k] = x;
+    s += x * c.dzf[k];
+  }
+  return s;
+}
+
+#ifdef __CUDACC__
+__global__ void k_poisson_z(Ctx c, PoissonTabs T, double* __restrict__ A, double* __restrict__ CP, double* __restrict__ CQ) {
+  const long long col = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (col >= c.nxy) return;
+  poisson_column(c, T, (int)(col % c.nx), (int)(col / c.nx), A, CP, CQ);
+}
+__global__ void k_cn_coef(Ctx c, double cimp, double* coef) {
+  if (blockIdx.x == 0 && threadIdx.x == 0) cn_coefficients(c, cimp, coef);
+}
+// comp: 0 u, 1 v, 2 w.  For u the dzf-weighted column sums are reduced per block into partial[blockIdx.x].
+__global__ void k_cn_z(Ctx c, const double* __restrict__ coef, int comp, double* __restrict__ Q, double* __restrict__ partial) {
+  __shared__ double sh[32];
+  const long long col = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  double s = 0.0;
+  if (col < c.nxy) {
+    const int j = (int)(col / c.nx);
+    const bool skip = (comp == 1 && c.bc_y == BC_WALL && j == c.ny - 1);   // the +y wall face stays 0
+    if (!skip) s = cn_column(c, comp == 2 ? coef + 3 * c.nz : coef, comp == 2 ? c.nz - 1 : c.nz, col, Q);
+  }
+  if (partial) {
+    const double t = block_sum(s, sh);
+    if (threadIdx.x == 0) partial[blockIdx.x] = t;
+  }
+}
+#endif
+
+}  // namespace cales

@@ -1,0 +1,260 @@
+// cales_emu.cu -- HOST EMULATOR of the CUDA kernels of libcales.so.  TEST INFRASTRUCTURE ONLY.
+//
+// Purpose: the box that runs `pytest -m "not gpu"` has no GPU.  The kernels of paper_2411_09364_b200/csrc are
+// written as __host__ __device__ phase functions of (tid, nth) / per-point functions, with the block barriers in
+// the __global__ wrappers only.  This file steps those SAME functions on the host -- block by block, phase by
+// phase, thread by thread -- in the order cales.cu launches them, so that the device code's arithmetic and index
+// logic can be compared with the CPU oracle without a GPU.  It is NOT a fallback: nothing in the package loads
+// it, it is built only by tests/emu/build.py, and it is orders of magnitude slower than the oracle.
+// Not covered here (GPU tests only): launch shapes, shared-memory sizes, warp-shuffle reductions, stream order.
+#include "../../paper_2411_09364_b200/csrc/cales_host.h"
+#include "../../paper_2411_09364_b200/csrc/cales_poisson.cuh"
+#include "../../paper_2411_09364_b200/csrc/cales_momentum.cuh"
+
+#include <cstring>
+#include <vector>
+
+using namespace cales;
+
+struct emu_solver {
+  HostSetup H;
+  Ctx c;
+  FftPlan plx, ply;
+  PoissonTabs pt;
+  long long N, nxy;
+  std::vector<double> u, v, w, p, nut, us, vs, ws, Ru, Rv, Rw, W, CP, CQ, smag, tau, cncoef, dsm_part, dsm_cs;
+  double scal[4];
+  int maxit;
+  bool fresh;
+};
+
+extern "C" const char* emu_last_error(void) { return g_err.c_str(); }
+
+extern "C" int emu_create(const cales_params* p, emu_solver** out) {
+  emu_solver* s = new emu_solver();
+  int rc = build_setup(p, s->H);
+  if (rc) { delete s; return rc; }
+  HostSetup& H = s->H;
+  s->c = H.c; s->N = H.c.N; s->nxy = H.c.nxy;
+  const size_t N = (size_t)s->N;
+  for (auto* f : {&s->u, &s->v, &s->w, &s->p, &s->nut, &s->us, &s->vs, &s->ws, &s->Ru, &s->Rv, &s->Rw, &s->W, &s->CP, &s->CQ, &s->smag}) f->assign(N, 0.0);
+  s->tau.assign(4 * (size_t)s->nxy, 0.0);
+  s->cncoef.assign(6 * (size_t)p->nz, 0.0);
+  const size_t ntx = (p->nx + DSM_TX - 1) / DSM_TX;
+  s->dsm_part.assign((size_t)p->nz * p->ny * ntx * 2, 0.0);
+  s->dsm_cs.assign((size_t)p->nz * p->ny, 0.0);
+  s->c.dzf = H.dzf.data() + 1; s->c.dzc = H.dzc.data() + 1; s->c.zc = H.zc.data(); s->c.tau = s->tau.data();
+  s->plx = H.plx; s->plx.tw = reinterpret_cast<const double2*>(H.twx.data());
+  s->ply = H.ply; s->ply.tw = reinterpret_cast<const double2*>(H.twy.data()); s->ply.dctw = reinterpret_cast<const double2*>(H.dctw.data());
+  s->pt.ak = H.ak.data(); s->pt.ck = H.ck.data(); s->pt.lamx = H.lamx.data(); s->pt.lamy = H.lamy.data();
+  s->scal[0] = s->scal[1] = s->scal[2] = 0.0; s->maxit = 0; s->fresh = false;
+  *out = s;
+  return 0;
+}
+extern "C" void emu_destroy(emu_solver* s) { delete s; }
+
+static std::vector<double>* fld(emu_solver* s, int f) {
+  switch (f) { case 0: return &s->u; case 1: return &s->v; case 2: return &s->w; case 3: return &s->p; case 4: return &s->nut; }
+  return nullptr;
+}
+extern "C" int emu_set_field(emu_solver* s, int f, const double* src) { std::memcpy(fld(s, f)->data(), src, s->N * sizeof(double)); if (f <= 2) s->fresh = false; return 0; }
+extern "C" int emu_get_field(emu_solver* s, int f, double* dst) { std::memcpy(dst, fld(s, f)->data(), s->N * sizeof(double)); return 0; }
+
+// ---- kernel emulations: same block decomposition and phase order as the __global__ wrappers ----
+static int run_passes(int nth, double2* buf0, double2* buf1, const SmView& sv, const FftPlan& pl, int sign, int start) {
+  int cur = start, Ns = 1;
+  for (int p = 0; p < pl.npass; ++p) {
+    const int R = pl.radix[p];
+    for (int tid = 0; tid < nth; ++tid) fft_pass(tid, nth, cur ? buf1 : buf0, cur ? buf0 : buf1, sv, pl, Ns, R, sign);
+    Ns *= R; cur ^= 1;
+  }
+  return cur;
+}
+static void emu_fft_x_fwd(emu_solver* s, const double* src, const DivSrc* ds, double* dst) {
+  const Ctx& c = s->c; const FftPlan& pl = s->plx; const int B = s->H.xB, nth = s->H.x_threads;
+  std::vector<double2> sm(2 * (size_t)B * pl.n2);
+  double2* buf0 = sm.data(); double2* buf1 = buf0 + (size_t)B * pl.n2;
+  const long long nlines = (long long)c.ny * c.nz;
+  for (long long l0 = 0; l0 < nlines; l0 += B) {
+    const int nb = (int)std::min<long long>(B, nlines - l0);
+    SmView sv{1, pl.n2, B, false};
+    DivSrc none{nullptr, nullptr, nullptr, 0.0};
+    for (int tid = 0; tid < nth; ++tid) { if (ds) fx_load<true>(tid, nth, c, pl, B, l0, nb, nullptr, *ds, buf0); else fx_load<false>(tid, nth, c, pl, B, l0, nb, src, none, buf0); }
+    const int cur = run_passes(nth, buf0, buf1, sv, pl, -1, 0);
+    for (int tid = 0; tid < nth; ++tid) fx_store_fwd(tid, nth, pl, B, l0, nb, cur ? buf1 : buf0, dst);
+  }
+}
+static void emu_fft_x_inv(emu_solver* s, const double* src, double* dst) {
+  const Ctx& c = s->c; const FftPlan& pl = s->plx; const int B = s->H.xB, nth = s->H.x_threads;
+  std::vector<double2> sm(2 * (size_t)B * pl.n2);
+  double2* buf0 = sm.data(); double2* buf1 = buf0 + (size_t)B * pl.n2;
+  const long long nlines = (long long)c.ny * c.nz;
+  for (long long l0 = 0; l0 < nlines; l0 += B) {
+    const int nb = (int)std::min<long long>(B, nlines - l0);
+    SmView sv{1, pl.n2, B, false};
+    DivSrc none{nullptr, nullptr, nullptr, 0.0};
+    for (int tid = 0; tid < nth; ++tid) fx_load<false>(tid, nth, c, pl, B, l0, nb, src, none, buf0);
+    for (int tid = 0; tid < nth; ++tid) merge_inverse(tid, nth, buf0, buf1, sv, pl, false);
+    const int cur = run_passes(nth, buf0, buf1, sv, pl, +1, 1);
+    for (int tid = 0; tid < nth; ++tid) fx_store_inv(tid, nth, pl, B, l0, nb, cur ? buf1 : buf0, dst);
+  }
+}
+static void emu_fft_y(emu_solver* s, double* A, int inverse) {
+  const Ctx& c = s->c; const FftPlan& pl = s->ply; const int TI = s->H.yTI, nth = s->H.y_threads;
+  const bool dct = c.bc_y == BC_WALL;
+  std::vector<double2> sm(2 * (size_t)TI * pl.n2);
+  double2* buf0 = sm.data(); double2* buf1 = buf0 + (size_t)TI * pl.n2;
+  for (int k = 0; k < c.nz; ++k) for (int i0 = 0; i0 < c.nx; i0 += TI) {
+    const int nb = std::min(TI, c.nx - i0);
+    double* base = A + (long long)k * c.nxy + i0;
+    SmView sv{TI, 1, TI, true};
+    for (int tid = 0; tid < nth; ++tid) fy_load(tid, nth, c, pl, TI, dct, inverse != 0, base, nb, buf0);
+    if (!inverse) {
+      const int cur = run_passes(nth, buf0, buf1, sv, pl, -1, 0);
+      for (int tid = 0; tid < nth; ++tid) fy_store_fwd(tid, nth, c, pl, TI, dct, base, nb, cur ? buf1 : buf0);
+    } else {
+      for (int tid = 0; tid < nth; ++tid) merge_inverse(tid, nth, buf0, buf1, sv, pl, dct);
+      const int cur = run_passes(nth, buf0, buf1, sv, pl, +1, 1);
+      for (int tid = 0; tid < nth; ++tid) fy_store_inv(tid, nth, c, pl, TI, dct, base, nb, cur ? buf1 : buf0);
+    }
+  }
+}
+static void emu_poisson_core(emu_solver* s) {
+  emu_fft_y(s, s->W.data(), 0);
+  for (int j = 0; j < s->c.ny; ++j) for (int i = 0; i < s->c.nx; ++i) poisson_column(s->c, s->pt, i, j, s->W.data(), s->CP.data(), s->CQ.data());
+  emu_fft_y(s, s->W.data(), 1);
+}
+static void emu_tau(emu_solver* s) {
+  if (!s->c.wall_model) return;
+  s->maxit = 0;
+  for (int z = 0; z < 4; ++z) for (int j = 0; j < s->c.ny; ++j) for (int i = 0; i < s->c.nx; ++i) {
+    const int it = wall_stress_point(s->c, s->H.wg, s->u.data(), s->v.data(), z >> 1, z & 1, i, j, s->tau.data());
+    if (it > s->maxit) s->maxit = it;
+  }
+}
+static void emu_nut(emu_solver* s, const double* u, const double* v, const double* w, double* nut) {
+  const Ctx& c = s->c;
+  if (c.sgs == 0) { for (long long n = 0; n < s->N; ++n) nut[n] = 0.0; return; }
+  if (c.sgs == 1) {
+    for (int k = 0; k < c.nz; ++k) for (int j = 0; j < c.ny; ++j) for (int i = 0; i < c.nx; ++i) nut[idx3(c, i, j, k)] = smag_point(c, u, v, w, i, j, k);
+    return;
+  }
+  const int ntx = (c.nx + DSM_TX - 1) / DSM_TX, nty = (c.ny + DSM_TY - 1) / DSM_TY, nth = DSM_TX * DSM_TY;
+  std::vector<double> sm(DSM_SMEM_DOUBLES);
+  double* raw = sm.data(); double* flt = raw + DSM_RAW; double* mid = flt + DSM_FLT;
+  for (int k = 0; k < c.nz; ++k) for (int by = 0; by < nty; ++by) for (int bx = 0; bx < ntx; ++bx) {
+    const int i0 = bx * DSM_TX, j0 = by * DSM_TY;
+    for (int tid = 0; tid < nth; ++tid) dsm_load(tid, nth, c, u, v, w, i0, j0, k, raw);
+    for (int tid = 0; tid < nth; ++tid) dsm_mid(tid, nth, c, i0, j0, k, raw, flt, mid);
+    for (int ty = 0; ty < DSM_TY; ++ty) {
+      double lm = 0.0, mm = 0.0;
+      for (int tx = 0; tx < DSM_TX; ++tx) {
+        const int i = i0 + tx, j = j0 + ty;
+        if (i < c.nx && j < c.ny) {
+          double a, b, sg;
+          dsm_point(c, i0, j0, k, tx, ty, flt, mid, &a, &b, &sg);
+          s->smag[idx3(c, i, j, k)] = sg; lm += a; mm += b;
+        }
+      }
+      if (j0 + ty < c.ny) {
+        const long long row = (long long)k * c.ny + j0 + ty;
+        s->dsm_part[(row * ntx + bx) * 2] = lm; s->dsm_part[(row * ntx + bx) * 2 + 1] = mm;
+      }
+    }
+  }
+  for (int k = 0; k < c.nz; ++k) {
+    double pl = 0.0, pm = 0.0;
+    for (int j = 0; j < c.ny; ++j) {
+      double ll, mm;
+      dsm_row_sums(s->dsm_part.data(), ntx, (long long)k * c.ny + j, &ll, &mm);
+      if (!c.dsm_plane) s->dsm_cs[(long long)k * c.ny + j] = (mm > 0.0) ? ll / mm : 0.0;
+      pl += ll; pm += mm;
+    }
+    if (c.dsm_plane) s->dsm_cs[k] = (pm > 0.0) ? pl / pm : 0.0;
+  }
+  for (int k = 0; k < c.nz; ++k) for (int j = 0; j < c.ny; ++j) for (int i = 0; i < c.nx; ++i)
+    nut[idx3(c, i, j, k)] = dsm_nut_point(c, s->dsm_cs.data(), s->smag.data(), i, j, k);
+}
+static void emu_refresh(emu_solver* s) {
+  emu_tau(s);
+  emu_nut(s, s->u.data(), s->v.data(), s->w.data(), s->nut.data());
+  s->fresh = true;
+}
+static void emu_substep(emu_solver* s, int rk, double dt) {
+  const Ctx& c = s->c;
+  double al, be, ga; rk3_coeffs(rk, al, be, ga);
+  const bool cfr = c.const_flow_rate != 0, imp = c.implicit_z != 0;
+  RhsArgs a;
+  a.u = s->u.data(); a.v = s->v.data(); a.w = s->w.data(); a.p = s->p.data(); a.nut = s->nut.data();
+  a.Ru0 = s->Ru.data(); a.Rv0 = s->Rv.data(); a.Rw0 = s->Rw.data(); a.Ru1 = s->Ru.data(); a.Rv1 = s->Rv.data(); a.Rw1 = s->Rw.data();
+  a.us = s->us.data(); a.vs = s->vs.data(); a.ws = s->ws.data(); a.dt = dt; a.al = al; a.be = be; a.ga = ga; a.store_R = rk < 2 ? 1 : 0;
+  double sum = 0.0;
+  for (int k = 0; k < c.nz; ++k) for (int j = 0; j < c.ny; ++j) for (int i = 0; i < c.nx; ++i) sum += rhs_point(c, a, i, j, k) * c.dzf[k];
+  if (imp) {
+    const double cimp = 0.5 * ga * c.nu * dt;
+    cn_coefficients(c, cimp, s->cncoef.data());
+    sum = 0.0;
+    for (long long col = 0; col < s->nxy; ++col) {
+      const int j = (int)(col / c.nx);
+      sum += cn_column(c, s->cncoef.data(), c.nz, col, s->us.data());
+      if (!(c.bc_y == BC_WALL && j == c.ny - 1)) cn_column(c, s->cncoef.data(), c.nz, col, s->vs.data());
+      cn_column(c, s->cncoef.data() + 3 * c.nz, c.nz - 1, col, s->ws.data());
+    }
+  }
+  if (cfr) {
+    const double m = sum / ((double)c.nx * (double)c.ny * c.lz);
+    s->scal[0] = c.u_bulk - m; s->scal[1] = s->scal[0] / (ga * dt); s->scal[2] = m;
+  }
+  DivSrc ds{s->us.data(), s->vs.data(), s->ws.data(), 1.0 / (ga * dt)};
+  emu_fft_x_fwd(s, nullptr, &ds, s->W.data());
+  emu_poisson_core(s);
+  emu_fft_x_inv(s, s->W.data(), s->W.data());
+  CorrArgs ca;
+  ca.phi = s->W.data(); ca.us = s->us.data(); ca.vs = s->vs.data(); ca.ws = s->ws.data();
+  ca.u = s->u.data(); ca.v = s->v.data(); ca.w = s->w.data(); ca.p = s->p.data();
+  ca.shift = cfr ? s->scal : nullptr; ca.gdt = ga * dt; ca.cimp = imp ? 0.5 * ga * c.nu * dt : 0.0; ca.update_p = 1;
+  for (int k = 0; k < c.nz; ++k) for (int j = 0; j < c.ny; ++j) for (int i = 0; i < c.nx; ++i) correct_point(c, ca, i, j, k);
+  emu_refresh(s);
+}
+extern "C" int emu_step(emu_solver* s, double dt) {
+  if (!s->fresh) emu_refresh(s);
+  for (int rk = 0; rk < 3; ++rk) emu_substep(s, rk, dt);
+  return 0;
+}
+extern "C" int emu_poisson_solve(emu_solver* s, const double* rhs, double* phi) {
+  emu_fft_x_fwd(s, rhs, nullptr, s->W.data());
+  emu_poisson_core(s);
+  emu_fft_x_inv(s, s->W.data(), phi);
+  return 0;
+}
+extern "C" int emu_eddy_viscosity(emu_solver* s, const double* u, const double* v, const double* w, double* nut) {
+  if (u) emu_nut(s, u, v, w, nut); else emu_nut(s, s->u.data(), s->v.data(), s->w.data(), nut);
+  return 0;
+}
+extern "C" int emu_wall_stress(emu_solver* s, double* tau) { emu_tau(s); std::memcpy(tau, s->tau.data(), s->tau.size() * sizeof(double)); return 0; }
+extern "C" int emu_get_cs(emu_solver* s, double* cs) { const size_t n = s->c.dsm_plane ? s->c.nz : (size_t)s->c.nz * s->c.ny; std::memcpy(cs, s->dsm_cs.data(), n * sizeof(double)); return 0; }
+extern "C" int emu_transform(emu_solver* s, double* f, int dir, int inverse) {
+  if (dir == 0) { if (inverse) emu_fft_x_inv(s, f, f); else emu_fft_x_fwd(s, f, nullptr, f); }
+  else emu_fft_y(s, f, inverse);
+  return 0;
+}
+extern "C" int emu_project(emu_solver* s) {
+  const Ctx& c = s->c;
+  DivSrc ds{s->u.data(), s->v.data(), s->w.data(), 1.0};
+  emu_fft_x_fwd(s, nullptr, &ds, s->W.data());
+  emu_poisson_core(s);
+  emu_fft_x_inv(s, s->W.data(), s->W.data());
+  CorrArgs ca;
+  ca.phi = s->W.data(); ca.us = s->u.data(); ca.vs = s->v.data(); ca.ws = s->w.data();
+  ca.u = s->u.data(); ca.v = s->v.data(); ca.w = s->w.data(); ca.p = s->p.data();
+  ca.shift = nullptr; ca.gdt = 1.0; ca.cimp = 0.0; ca.update_p = 0;
+  for (int k = 0; k < c.nz; ++k) for (int j = 0; j < c.ny; ++j) for (int i = 0; i < c.nx; ++i) correct_point(c, ca, i, j, k);
+  s->fresh = false;
+  return 0;
+}
+extern "C" double emu_max_div(emu_solver* s) {
+  const Ctx& c = s->c; double md = 0.0;
+  for (int k = 0; k < c.nz; ++k) for (int j = 0; j < c.ny; ++j) for (int i = 0; i < c.nx; ++i)
+    md = std::fmax(md, std::fabs(divergence_point(c, s->u.data(), s->v.data(), s->w.data(), i, j, k)));
+  return md;
+}
