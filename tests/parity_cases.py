@@ -1,0 +1,67 @@
+"""Parity cases shared by the host-emulator tests (CPU) and the GPU tests: reduced replicas of the five
+BASELINE.json configurations with the same option sets, sized so that the oracle finishes in seconds while the
+grids still span several CUDA tiles and a ragged tail (nx not a multiple of 32, ny not a multiple of 8).
+
+Holds no arithmetic of the method: it only draws the seeded inputs (paper_2411_09364_b200.inputs), runs ONE side
+and compares arrays.  The initial field is made solenoidal by the oracle's own projection.
+"""
+import numpy as np
+
+from paper_2411_09364_b200 import inputs
+
+# name -> (config number, replica shape (nx, ny, nz), steps)
+SMALL = {
+    "cfg1_dit": (1, (24, 16, 12), 2),
+    "cfg2_wmles": (2, (48, 24, 16), 2),
+    "cfg3_wrles_cn": (3, (36, 24, 20), 2),
+    "cfg4_duct_dsm": (4, (48, 18, 16), 2),
+    "cfg5_wmles_dsm": (5, (36, 24, 16), 2),
+}
+# the sizes the GPU parity tests use: several tiles in every direction plus ragged tails
+GPU_CASES = {
+    "cfg1_dit32": (1, None, 10),                     # BASELINE config 1 at full size, 10 steps
+    "cfg2_wmles": (2, (96, 48, 32), 3),
+    "cfg3_wrles_cn": (3, (96, 72, 48), 3),
+    "cfg4_duct_dsm": (4, (192, 54, 48), 3),
+    "cfg5_wmles_dsm": (5, (192, 128, 64), 3),        # the replica SURVEY.md 8(d) names for config 5
+}
+
+
+def prepare(oracle, n, shape):
+    """(cfg, kwargs, (u, v, w), dt): seeded field, projected by the oracle, with its time step."""
+    cfg = inputs.config(n, shape)
+    u, v, w, ub = inputs.initial_fields(cfg)
+    kw = inputs.solver_kwargs(cfg, ub)
+    g = {k: kw[k] for k in ("nx", "ny", "nz", "lx", "ly", "lz")}
+    o = oracle.Oracle(g["nx"], g["ny"], g["nz"], g["lx"], g["ly"], g["lz"],
+                      **{k: v_ for k, v_ in kw.items() if k not in g})
+    o.set_velocity(u, v, w)
+    o.project()
+    u, v, w = o.velocity()
+    if kw["const_flow_rate"]:
+        # the projection leaves the bulk velocity unchanged in periodic x; keep the imposed value consistent
+        kw["u_bulk"] = float(np.sum(u * o.dzf[:, None, None]) / (g["nx"] * g["ny"] * g["lz"]))
+    dt = inputs.time_step(cfg, u, v, w)
+    return cfg, kw, (u, v, w), dt
+
+
+def make(cls, kw):
+    g = {k: kw[k] for k in ("nx", "ny", "nz", "lx", "ly", "lz")}
+    return cls(g["nx"], g["ny"], g["nz"], g["lx"], g["ly"], g["lz"], **{k: v for k, v in kw.items() if k not in g})
+
+
+def weighted_mean_removed(p, dzf):
+    m = np.sum(p * dzf[:, None, None]) / (np.sum(dzf) * p.shape[1] * p.shape[2])
+    return p - m
+
+
+def field_errors(got, ref, dzf, nu):
+    """max|delta| / max|field| for u, v, w, p (weighted mean removed), nu_t (scale max(nu_t) or nu)."""
+    out = {}
+    for name, a, b in zip("uvw", got[:3], ref[:3]):
+        out[name] = float(np.max(np.abs(a - b)) / max(np.max(np.abs(b)), 1e-300))
+    pa, pb = weighted_mean_removed(got[3], dzf), weighted_mean_removed(ref[3], dzf)
+    out["p"] = float(np.max(np.abs(pa - pb)) / max(np.max(np.abs(pb)), 1e-300))
+    sc = max(float(np.max(np.abs(ref[4]))), nu)
+    out["nut"] = float(np.max(np.abs(got[4] - ref[4])) / sc)
+    return out
