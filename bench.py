@@ -1,0 +1,335 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the CaLES hot path (one full RK3 step = all rows of SURVEY.md 8(a)) on B200.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl reference]
+
+Prints ONE JSON line (rank 0).  metric = fp64 grid-point RK3 steps per second (Gpts*step/s).
+  value     : N_points * K / t with the state resident in HBM (CUDA events on the launching stream, max over ranks)
+  e2e       : same metric through the C ABI with HOST buffers: every step copies u, v, w host->device
+              (cales_set_field), steps, and copies u, v, w, p device->host (cales_get_field)
+  roofline  : the dominant kernel of the step, algorithmic bytes / its mean launch duration (events recorded by the
+              library after every launch inside the timed region) against MEASURED_PEAKS.json's HBM copy rate
+  kernels   : the same figure for every kernel of the step
+  cpu_baseline : the CPU oracle as it stands on the host cores, on a bounded replica of the same option set
+Multi-GPU: replicas only: every rank steps its own simulation, no collective on the data path.
+`--impl reference` times the oracle (rank 0 only).
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "fp64 grid-point RK3 steps/sec (Gpts*step/s)"
+UNIT = "Gpts*step/s"
+L2_BYTES = 126 * 1024 * 1024
+
+# Algorithmic bytes per grid point per LAUNCH (fp64; every field a kernel needs read once, every result written once;
+# DESIGN.md "Kernels and their rooflines").  k_rhs: substeps read 5 (+3 R^{k-1}) fields and write
+# 3 (+3 R^k): 88 / 112 / 88 B/pt, mean 96.
+ALGO_BYTES = {
+    "k_rhs": 96.0, "k_cn_z": 16.0, "k_fft_x_fwd": 32.0, "k_fft_y_fwd": 16.0, "k_poisson_z": 16.0, "k_fft_y_inv": 16.0,
+    "k_fft_x_inv": 16.0, "k_correct": 72.0, "k_smag": 32.0, "k_dsm_pass1": 32.0, "k_dsm_nut": 16.0, "k_fill": 8.0,
+}
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits",
+                                          "-lms", "200"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True); self.th.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, reasons, pw = [], [], set(), []
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
+            except (ValueError, IndexError):
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+REPLICA = {1: None, 2: None, 3: (128, 128, 96), 4: (256, 64, 64), 5: (192, 128, 64)}   # bounded oracle samples
+
+
+def oracle_leg(cfg_no, steps, warmup):
+    """Time the CPU oracle as it stands (never tuned for this) on a bounded replica of config cfg_no's option set."""
+    import numpy as np
+    import oracle
+    from paper_2411_09364_b200 import inputs
+    shape = REPLICA[cfg_no]
+    cfg = inputs.config(cfg_no, shape)
+    u, v, w, ub = inputs.initial_fields(cfg)
+    kw = inputs.solver_kwargs(cfg, ub)
+    g = {k: kw.pop(k) for k in ("nx", "ny", "nz", "lx", "ly", "lz")}
+    o = oracle.Oracle(g["nx"], g["ny"], g["nz"], g["lx"], g["ly"], g["lz"], **kw)
+    o.set_velocity(u, v, w); o.project()
+    dt = inputs.time_step(cfg, *o.velocity())
+    for _ in range(warmup):
+        o.step(dt)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        o.step(dt)
+    t = time.perf_counter() - t0
+    npts = g["nx"] * g["ny"] * g["nz"]
+    assert np.isfinite(o.get(0)).all()
+    return {"value": npts * steps / t / 1e9, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": "config %d option set on a %dx%dx%d grid (%s), %d steps after %d warm-up" %
+                      (cfg_no, g["nx"], g["ny"], g["nz"], "full size" if shape is None else "reduced replica", steps, warmup),
+            "ms_per_step": 1e3 * t / steps, "workload": cfg["name"]}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cfg_no = args.config or 5
+    steps, warmup = args.steps, args.warmup
+    if REPLICA[cfg_no] is not None:            # keep the whole run within a few minutes on a small host
+        steps, warmup = min(steps, 5), min(warmup, 1)
+    r = oracle_leg(cfg_no, steps, warmup)
+    line = {"impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+            "warmup": warmup, "ms_per_step": r["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "config": {"workload": r["workload"], "sample": r["sample"]},
+            "cpu_baseline": {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")},
+            "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def pick_config(torch, requested):
+    if requested:
+        return requested
+    import psutil
+    free, _ = torch.cuda.mem_get_info()
+    host = psutil.virtual_memory().available
+    # config 5: 15 resident fields x 6.44 GB on the device; 4 pinned host fields + generation temporaries on the host
+    if free >= 110e9 and host >= 90e9:
+        return 5
+    return 4
+
+
+def host_register(torch, a):
+    """Pin an existing numpy array in place (no copy) so the e2e copies run from pinned host memory."""
+    rc = torch.cuda.cudart().cudaHostRegister(a.ctypes.data, a.nbytes, 0)
+    return int(rc) == 0
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_2411_09364_b200 import binding, inputs
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the CaLES hot path has no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    binding.lib()
+    cfg_no = pick_config(torch, args.config)
+    K, W = args.steps, max(args.warmup, 3)
+
+    # ---- seeded synthetic workload (inputs.py), every rank its own replica (seed + rank)
+    cfg = inputs.config(cfg_no)
+    cfg["seed"] += rank
+    t_gen = time.perf_counter()
+    u, v, w, ub = inputs.initial_fields(cfg)
+    dt = inputs.time_step(cfg, u, v, w)
+    kw = inputs.solver_kwargs(cfg, ub)
+    g = {k: kw.pop(k) for k in ("nx", "ny", "nz", "lx", "ly", "lz")}
+    npts = g["nx"] * g["ny"] * g["nz"]
+    p_host = np.zeros_like(u)
+    pinned = all(host_register(torch, a) for a in (u, v, w, p_host))
+    t_gen = time.perf_counter() - t_gen
+    s = binding.Solver(g["nx"], g["ny"], g["nz"], g["lx"], g["ly"], g["lz"], device=local, **kw)
+    s.set_velocity(u, v, w)
+    s.project()                      # discretely solenoidal start, by the GPU solver itself
+    for f, a in zip(range(3), (u, v, w)):
+        s.get_field(f, torch.from_numpy(a))       # the host copies now hold the projected field
+    flush = None
+    small = s.workspace_bytes < 2 * L2_BYTES
+    if small:
+        flush = torch.empty(2 * L2_BYTES // 8, dtype=torch.float64, device="cuda")
+    big = npts >= 4_000_000
+    for _ in range(W):
+        s.step(dt)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+
+    # ---- timed region: K steps, CUDA events on the launching stream (the solver runs on torch's current stream)
+    ktot = {}
+    def add_kernel_times():
+        for name, (ms, n) in s.kernel_times().items():
+            a = ktot.setdefault(name, [0.0, 0]); a[0] += ms; a[1] += n
+    sampler = ClockSampler(local); sampler.start()
+    s.set_timing(big)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+    for k in range(K):
+        if flush is not None:
+            flush.fill_(float(k))    # L2 flush between timed iterations (small configs only)
+        ev[k][0].record()
+        s.step(dt)
+        ev[k][1].record()
+        if big:
+            add_kernel_times()       # per-launch events of this step -> per-kernel totals (syncs, outside the event pair)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    ms = sum(a.elapsed_time(b) for a, b in ev)
+    if not big:                      # launch-bound sizes: per-launch events would perturb the timed region; second pass
+        s.set_timing(True)
+        for k in range(K):
+            if flush is not None:
+                flush.fill_(float(k))
+            s.step(dt); add_kernel_times()
+    s.set_timing(False)
+    diag = s.diagnostics()
+    launches = s.launches_per_step() * K
+    if world > 1:
+        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    value = world * npts * K / (ms * 1e-3) / 1e9
+
+    # ---- e2e: the same metric through the C ABI with HOST buffers, copies inside the timed region
+    Ke = max(1, min(K, 3))
+    hosts = [torch.from_numpy(a) for a in (u, v, w, p_host)]
+    def e2e_step():
+        for f in range(3):
+            s.set_field(f, hosts[f])            # H2D, synchronous (cales_set_field with a host pointer)
+        s.step(dt)
+        for f in range(4):
+            s.get_field(f, hosts[f])            # D2H of the step's result
+    e2e_step()                                  # warm-up
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    t0 = time.perf_counter()
+    for _ in range(Ke):
+        e2e_step()
+    torch.cuda.synchronize()
+    te = time.perf_counter() - t0
+    if world > 1:
+        t = torch.tensor([te], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        te = float(t.item())
+    e2e = {"value": world * npts * Ke / te / 1e9, "unit": UNIT, "h2d_bytes_per_step": 3 * npts * 8, "d2h_bytes_per_step": 4 * npts * 8,
+           "steps": Ke, "ms_per_step": 1e3 * te / Ke, "host_memory": "pinned (cudaHostRegister)" if pinned else "pageable",
+           "note": "each step: cales_set_field(u,v,w) from host, cales_step, cales_get_field(u,v,w,p) to host; a new velocity makes "
+                   "the library re-evaluate the wall stress and nu_t first"}
+
+    # ---- per-kernel roofline table (algorithmic bytes / mean launch duration) and the dominant kernel
+    peak, peak_src = measured_peaks()
+    kernels = {}
+    step_ms = sum(a[0] for a in ktot.values()) / K
+    for name, (tot, n) in sorted(ktot.items(), key=lambda kv: -kv[1][0]):
+        per = tot / n
+        row = {"ms_per_launch": per, "launches_per_step": n // K, "share_of_step": (tot / K) / step_ms if step_ms else None}
+        if name in ALGO_BYTES:
+            gbs = ALGO_BYTES[name] * npts / (per * 1e-3) / 1e9
+            row.update({"algo_bytes_per_pt": ALGO_BYTES[name], "achieved_gbs": gbs, "frac": gbs / peak})
+        kernels[name] = row
+    top = next((n for n in kernels if n in ALGO_BYTES), None)
+    roofline = None
+    if top:
+        r = kernels[top]
+        roofline = {"kernel": top, "bound": "hbm", "achieved": r["achieved_gbs"], "peak": peak, "unit": "GB/s", "frac": r["frac"],
+                    "traffic": None, "peak_source": peak_src, "algo_bytes_per_launch": ALGO_BYTES[top] * npts,
+                    "ms_per_launch": r["ms_per_launch"], "share_of_step": r["share_of_step"]}
+    # whole-step algorithmic traffic: the sum over the step's launches of the table above
+    step_bytes = sum(ALGO_BYTES.get(n, 0.0) * (a[1] // K) for n, a in ktot.items()) * npts
+    step_gbs = step_bytes / (ms / K * 1e-3) / 1e9
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms / K,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "config %d: %s %dx%dx%d" % (cfg_no, cfg["name"], g["nx"], g["ny"], g["nz"]), "points": npts,
+                       "dt": dt, "parallelism": "replicas x%d (no data-path collective)" % world,
+                       "l2": "L2 flushed between timed steps" if small else "state (%.1f GB) larger than L2" % (s.workspace_bytes / 1e9),
+                       "options": {k: kw[k] for k in ("bc_y", "bc_z", "zstretch", "sgs_model", "wall_model", "implicit_z", "const_flow_rate",
+                                                      "dsm_avg_xy_plane", "dsm_clip_total", "van_driest")}},
+            "step_hbm": {"algo_bytes_per_pt_step": step_bytes / npts, "achieved_gbs": step_gbs, "frac_of_measured_peak": step_gbs / peak,
+                         "frac_of_8TBs": step_gbs / 8000.0},
+            "e2e": e2e, "gpu_launches": launches, "clocks": clocks, "roofline": roofline, "kernels": kernels,
+            "diagnostics": {k: diag[k] for k in ("max_div", "u_bulk", "kinetic_energy", "wm_max_iters", "nan_count")},
+            "input_generation_s": t_gen}
+    if rank == 0:
+        if not args.no_cpu_baseline and world == 1:
+            r = oracle_leg(cfg_no, 2, 1)
+            line["cpu_baseline"] = {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")}
+        print(json.dumps(line), flush=True)
+    s.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=0, help="BASELINE.json config 1..5 (default: 5 if it fits, else 4)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        if not args.config:
+            try:
+                import torch
+                args.config = pick_config(torch, 0) if torch.cuda.is_available() else 5
+            except Exception:
+                args.config = 5
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

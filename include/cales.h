@@ -143,8 +143,17 @@ int cales_transform(cales_solver* s, double* field_dev, int dir, int inverse);
 /* Tiled shared-memory transpose of every k-plane: dst[k][i][j] = src[k][j][i] (DEVICE, out of place). */
 int cales_transpose_xy(cales_solver* s, const double* src_dev, double* dst_dev);
 
-/* Per-phase device timing of cales_step (CUDA events; off by default). */
+/* Per-kernel device timing of cales_step: when on, a CUDA event is recorded on the stream after every kernel
+ * launch of a step (off by default; costs one event record per launch). */
 int cales_set_timing(cales_solver* s, int on);
+
+/* Number of kernel ids known to cales_kernel_time. */
+int cales_kernel_count(void);
+
+/* Device time of kernel `kid` (0 <= kid < cales_kernel_count()) summed over its launches in the LAST cales_step
+ * that ran with timing on: *name = static string, *ms_total = milliseconds, *launches = launch count (any of
+ * the three may be NULL).  Synchronises the stream. */
+int cales_kernel_time(cales_solver* s, int kid, const char** name, double* ms_total, int* launches);
 
 /* Number of kernels cales_step launches per call with the current parameters (for bench.py's gpu_launches). */
 int cales_launches_per_step(cales_solver* s);

@@ -39,7 +39,7 @@ class CalesDiag(C.Structure):
 SYMBOLS = ["cales_default_params", "cales_workspace_bytes", "cales_create", "cales_create_basic", "cales_destroy",
            "cales_set_field", "cales_get_field", "cales_step", "cales_poisson_solve", "cales_eddy_viscosity",
            "cales_wall_stress", "cales_project", "cales_get_cs", "cales_transform", "cales_transpose_xy",
-           "cales_set_timing", "cales_launches_per_step", "cales_diagnostics", "cales_last_error"]
+           "cales_set_timing", "cales_kernel_count", "cales_kernel_time", "cales_launches_per_step", "cales_diagnostics", "cales_last_error"]
 
 _lib = None
 
@@ -70,6 +70,7 @@ def lib():
         L.cales_transpose_xy.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.cales_set_timing.argtypes = [C.c_void_p, C.c_int]
         L.cales_launches_per_step.argtypes = [C.c_void_p]
+        L.cales_kernel_time.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_char_p), C.POINTER(C.c_double), C.POINTER(C.c_int)]
         L.cales_diagnostics.argtypes = [C.c_void_p, C.POINTER(CalesDiag)]
         L.cales_create_basic.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, C.c_int, C.c_double,
                                          C.c_int, C.c_int, C.c_double, C.c_int, C.c_int, C.c_int,
@@ -231,6 +232,16 @@ class Solver:
 
     def set_timing(self, on=True):
         _chk(lib().cales_set_timing(self._h, 1 if on else 0))
+
+    def kernel_times(self):
+        """{kernel name: (total ms, launches)} of the last step that ran with timing on (synchronises)."""
+        out = {}
+        for kid in range(lib().cales_kernel_count()):
+            name, ms, n = C.c_char_p(), C.c_double(), C.c_int()
+            _chk(lib().cales_kernel_time(self._h, kid, C.byref(name), C.byref(ms), C.byref(n)))
+            if n.value:
+                out[name.value.decode()] = (ms.value, n.value)
+        return out
 
     def launches_per_step(self):
         return lib().cales_launches_per_step(self._h)

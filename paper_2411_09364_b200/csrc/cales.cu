@@ -47,7 +47,9 @@ struct cales_solver {
   dim3 pgrid, pblock;   // point kernels
   long long nblk;
   bool fresh;
-  int timing; cudaEvent_t ev[3][7]; bool ev_valid;
+  int timing; bool ev_valid;
+  std::vector<cudaEvent_t> evpool; std::vector<int> evkid; int evn;   // per-launch events of the last timed step
+  double kms[32]; int kcnt[32];                                       // per-kernel totals of the last timed step
   int launches;
 };
 
@@ -98,14 +100,30 @@ extern "C" size_t cales_workspace_bytes(const cales_params* p) {
   return carve(nullptr, p, nullptr);
 }
 
-static int check_launch(cales_solver* s, const char* what) {
+// Kernel ids for the per-kernel timing table (cales_kernel_time).
+enum { K_RHS = 0, K_CN_COEF, K_CN_Z, K_SUM, K_BULK, K_FFTX_FWD, K_FFTY_FWD, K_POISSON_Z, K_FFTY_INV, K_FFTX_INV, K_CORRECT,
+       K_WALL, K_SMAG, K_DSM_PASS1, K_DSM_COEF, K_DSM_NUT, K_FILL, K_TRANSPOSE, K_DIAG, K_COUNT };
+static const char* const k_names[K_COUNT] = {"k_rhs", "k_cn_coef", "k_cn_z", "k_sum_stage1", "k_bulk_finish", "k_fft_x_fwd", "k_fft_y_fwd",
+  "k_poisson_z", "k_fft_y_inv", "k_fft_x_inv", "k_correct", "k_wall_stress", "k_smag", "k_dsm_pass1", "k_dsm_coef", "k_dsm_nut", "k_fill",
+  "k_transpose_xy", "k_diag"};
+
+// record an event on the stream tagged with the kernel that just finished (kid < 0: a separator)
+static void tick(cales_solver* s, int kid) {
+  if (!s->timing) return;
+  if (s->evn == (int)s->evpool.size()) { cudaEvent_t e; cudaEventCreate(&e); s->evpool.push_back(e); s->evkid.push_back(-1); }
+  s->evkid[s->evn] = kid;
+  cudaEventRecord(s->evpool[s->evn], s->st);
+  ++s->evn;
+}
+static int check_launch(cales_solver* s, int kid) {
   ++s->launches;
   cudaError_t e = cudaGetLastError();
-  if (e != cudaSuccess) return fail(CALES_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
+  if (e != cudaSuccess) return fail(CALES_ECUDA, std::string(k_names[kid]) + ": " + cudaGetErrorString(e));
+  tick(s, kid);
   return CALES_OK;
 }
-#define LAUNCH_TRY(what)                                  \
-  do { int rc_ = check_launch(s, what); if (rc_) return rc_; } while (0)
+#define LAUNCH_TRY(kid)                                  \
+  do { int rc_ = check_launch(s, kid); if (rc_) return rc_; } while (0)
 
 extern "C" int cales_create(const cales_params* p, cales_solver** out) {
   if (!out) return fail(CALES_EINVAL, "null output pointer");
@@ -157,8 +175,8 @@ extern "C" int cales_create(const cales_params* p, cales_solver** out) {
   if (e != cudaSuccess) { delete s; return fail(CALES_ECUDA, std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e)); }
   s->pblock = dim3(32, 8, 1);
   s->pgrid = dim3((nx + 31) / 32, (ny + 7) / 8, nz);
-  s->fresh = false; s->timing = 0; s->ev_valid = false; s->launches = 0;
-  for (int a = 0; a < 3; ++a) for (int b = 0; b < 7; ++b) s->ev[a][b] = nullptr;
+  s->fresh = false; s->timing = 0; s->ev_valid = false; s->launches = 0; s->evn = 0;
+  for (int q = 0; q < 32; ++q) { s->kms[q] = 0.0; s->kcnt[q] = 0; }
   *out = s;
   return CALES_OK;
 }
@@ -175,7 +193,7 @@ extern "C" int cales_create_basic(int nx, int ny, int nz, double lx, double ly, 
 
 extern "C" int cales_destroy(cales_solver* s) {
   if (!s) return CALES_OK;
-  for (int a = 0; a < 3; ++a) for (int b = 0; b < 7; ++b) if (s->ev[a][b]) cudaEventDestroy(s->ev[a][b]);
+  for (cudaEvent_t e : s->evpool) cudaEventDestroy(e);
   delete s;
   return CALES_OK;
 }
@@ -209,26 +227,26 @@ static int run_transform_x_fwd(cales_solver* s, const double* src, const DivSrc*
   const unsigned grid = (unsigned)((nlines + s->xB - 1) / s->xB);
   if (ds) k_fft_x_fwd<true><<<grid, s->x_threads, s->x_smem, s->st>>>(s->c, s->plx, s->xB, nullptr, *ds, dst);
   else { DivSrc z{nullptr, nullptr, nullptr, 0.0}; k_fft_x_fwd<false><<<grid, s->x_threads, s->x_smem, s->st>>>(s->c, s->plx, s->xB, src, z, dst); }
-  LAUNCH_TRY("k_fft_x_fwd");
+  LAUNCH_TRY(K_FFTX_FWD);
   return CALES_OK;
 }
 static int run_transform_x_inv(cales_solver* s, const double* src, double* dst) {
   const long long nlines = (long long)s->c.ny * s->c.nz;
   const unsigned grid = (unsigned)((nlines + s->xB - 1) / s->xB);
   k_fft_x_inv<<<grid, s->x_threads, s->x_smem, s->st>>>(s->c, s->plx, s->xB, src, dst);
-  LAUNCH_TRY("k_fft_x_inv");
+  LAUNCH_TRY(K_FFTX_INV);
   return CALES_OK;
 }
 static int run_transform_y(cales_solver* s, double* A, int inverse) {
   dim3 grid((s->c.nx + s->yTI - 1) / s->yTI, s->c.nz);
   k_fft_y<<<grid, s->y_threads, s->y_smem, s->st>>>(s->c, s->ply, s->yTI, s->c.bc_y == BC_WALL ? 1 : 0, inverse, A);
-  LAUNCH_TRY("k_fft_y");
+  LAUNCH_TRY(inverse ? K_FFTY_INV : K_FFTY_FWD);
   return CALES_OK;
 }
 static int run_poisson_z(cales_solver* s, double* A) {
   const int th = 128;
   k_poisson_z<<<(unsigned)((s->nxy + th - 1) / th), th, 0, s->st>>>(s->c, s->pt, A, s->CP, s->CQ);
-  LAUNCH_TRY("k_poisson_z");
+  LAUNCH_TRY(K_POISSON_Z);
   return CALES_OK;
 }
 // spectral part of the Poisson solve, W already holds the x-transformed right-hand side
@@ -242,26 +260,27 @@ static int run_poisson_core(cales_solver* s) {
 static int run_wall_stress(cales_solver* s) {
   if (!s->c.wall_model) return CALES_OK;
   CUDA_TRY(cudaMemsetAsync(s->maxit, 0, sizeof(int), s->st));
+  tick(s, -1);
   dim3 grid(s->pgrid.x, s->pgrid.y, 4);
   k_wall_stress<<<grid, s->pblock, 0, s->st>>>(s->c, s->wg, s->u, s->v, s->tau, s->maxit);
-  LAUNCH_TRY("k_wall_stress");
+  LAUNCH_TRY(K_WALL);
   return CALES_OK;
 }
 static int run_eddy_viscosity(cales_solver* s, const double* u, const double* v, const double* w, double* nut) {
   if (s->c.sgs == CALES_SGS_NONE) {
     k_fill<<<1184, 256, 0, s->st>>>(nut, s->N, 0.0);
-    LAUNCH_TRY("k_fill");
+    LAUNCH_TRY(K_FILL);
   } else if (s->c.sgs == CALES_SGS_SMAG) {
     k_smag<<<s->pgrid, s->pblock, 0, s->st>>>(s->c, u, v, w, nut);
-    LAUNCH_TRY("k_smag");
+    LAUNCH_TRY(K_SMAG);
   } else {
     dim3 grid((s->c.nx + DSM_TX - 1) / DSM_TX, (s->c.ny + DSM_TY - 1) / DSM_TY, s->c.nz);
     k_dsm_pass1<<<grid, dim3(DSM_TX, DSM_TY), DSM_SMEM_DOUBLES * sizeof(double), s->st>>>(s->c, u, v, w, s->smag, s->dsm_part);
-    LAUNCH_TRY("k_dsm_pass1");
+    LAUNCH_TRY(K_DSM_PASS1);
     k_dsm_coef<<<s->c.nz, 128, 0, s->st>>>(s->c, s->dsm_part, (int)grid.x, s->dsm_cs);
-    LAUNCH_TRY("k_dsm_coef");
+    LAUNCH_TRY(K_DSM_COEF);
     k_dsm_nut<<<s->pgrid, s->pblock, 0, s->st>>>(s->c, s->dsm_cs, s->smag, nut);
-    LAUNCH_TRY("k_dsm_nut");
+    LAUNCH_TRY(K_DSM_NUT);
   }
   return CALES_OK;
 }
@@ -274,65 +293,53 @@ static int refresh_closures(cales_solver* s) {
   return CALES_OK;
 }
 
-static void mark(cales_solver* s, int rk, int b) {
-  if (!s->timing) return;
-  if (!s->ev[rk][b]) cudaEventCreate(&s->ev[rk][b]);
-  cudaEventRecord(s->ev[rk][b], s->st);
-}
-
 static int substep(cales_solver* s, int rk, double dt) {
   int rc;
   double al, be, ga; rk3_coeffs(rk, al, be, ga);
   const Ctx& c = s->c;
   const bool cfr = c.const_flow_rate != 0, imp = c.implicit_z != 0;
-  mark(s, rk, 0);
   RhsArgs a;
   a.u = s->u; a.v = s->v; a.w = s->w; a.p = s->p; a.nut = s->nut;
   a.Ru0 = s->Ru; a.Rv0 = s->Rv; a.Rw0 = s->Rw; a.Ru1 = s->Ru; a.Rv1 = s->Rv; a.Rw1 = s->Rw;
   a.us = s->us; a.vs = s->vs; a.ws = s->ws; a.dt = dt; a.al = al; a.be = be; a.ga = ga; a.store_R = rk < 2 ? 1 : 0;
   k_rhs<<<s->pgrid, s->pblock, 0, s->st>>>(c, a, (cfr && !imp) ? s->partial : nullptr);
-  LAUNCH_TRY("k_rhs");
-  mark(s, rk, 1);
+  LAUNCH_TRY(K_RHS);
   long long npart = s->nblk;
   if (imp) {
     const double cimp = 0.5 * ga * c.nu * dt;
     k_cn_coef<<<1, 32, 0, s->st>>>(c, cimp, s->cncoef);
-    LAUNCH_TRY("k_cn_coef");
+    LAUNCH_TRY(K_CN_COEF);
     const int th = 128; const unsigned g = (unsigned)((s->nxy + th - 1) / th);
-    k_cn_z<<<g, th, 0, s->st>>>(c, s->cncoef, 0, s->us, cfr ? s->partial : nullptr); LAUNCH_TRY("k_cn_z(u)");
-    k_cn_z<<<g, th, 0, s->st>>>(c, s->cncoef, 1, s->vs, nullptr); LAUNCH_TRY("k_cn_z(v)");
-    k_cn_z<<<g, th, 0, s->st>>>(c, s->cncoef, 2, s->ws, nullptr); LAUNCH_TRY("k_cn_z(w)");
+    k_cn_z<<<g, th, 0, s->st>>>(c, s->cncoef, 0, s->us, cfr ? s->partial : nullptr); LAUNCH_TRY(K_CN_Z);
+    k_cn_z<<<g, th, 0, s->st>>>(c, s->cncoef, 1, s->vs, nullptr); LAUNCH_TRY(K_CN_Z);
+    k_cn_z<<<g, th, 0, s->st>>>(c, s->cncoef, 2, s->ws, nullptr); LAUNCH_TRY(K_CN_Z);
     npart = g;
   }
-  mark(s, rk, 2);
   if (cfr) {
     const int g1 = (int)(npart < 1024 ? npart : 1024);
-    k_sum_stage1<<<g1, 256, 0, s->st>>>(s->partial, npart, s->stage1); LAUNCH_TRY("k_sum_stage1");
-    k_bulk_finish<<<1, 256, 0, s->st>>>(c, s->stage1, g1, ga * dt, s->scal); LAUNCH_TRY("k_bulk_finish");
+    k_sum_stage1<<<g1, 256, 0, s->st>>>(s->partial, npart, s->stage1); LAUNCH_TRY(K_SUM);
+    k_bulk_finish<<<1, 256, 0, s->st>>>(c, s->stage1, g1, ga * dt, s->scal); LAUNCH_TRY(K_BULK);
   }
   DivSrc ds{s->us, s->vs, s->ws, 1.0 / (ga * dt)};
   if ((rc = run_transform_x_fwd(s, nullptr, &ds, s->W))) return rc;
   if ((rc = run_poisson_core(s))) return rc;
   if ((rc = run_transform_x_inv(s, s->W, s->W))) return rc;
-  mark(s, rk, 3);
   CorrArgs ca;
   ca.phi = s->W; ca.us = s->us; ca.vs = s->vs; ca.ws = s->ws; ca.u = s->u; ca.v = s->v; ca.w = s->w; ca.p = s->p;
   ca.shift = cfr ? s->scal : nullptr; ca.gdt = ga * dt; ca.cimp = imp ? 0.5 * ga * c.nu * dt : 0.0; ca.update_p = 1;
   k_correct<<<s->pgrid, s->pblock, 0, s->st>>>(c, ca);
-  LAUNCH_TRY("k_correct");
-  mark(s, rk, 4);
+  LAUNCH_TRY(K_CORRECT);
   if ((rc = run_wall_stress(s))) return rc;
-  mark(s, rk, 5);
   if ((rc = run_eddy_viscosity(s, s->u, s->v, s->w, s->nut))) return rc;
-  mark(s, rk, 6);
   return CALES_OK;
 }
 
 extern "C" int cales_step(cales_solver* s, double dt) {
   if (!s || !(dt > 0.0)) return fail(CALES_EINVAL, "bad step arguments");
   int rc;
-  s->launches = 0;
+  s->launches = 0; s->evn = 0; s->ev_valid = false;
   if (!s->fresh && (rc = refresh_closures(s))) return rc;
+  tick(s, -1);
   for (int rk = 0; rk < 3; ++rk) if ((rc = substep(s, rk, dt))) return rc;
   s->ev_valid = s->timing != 0;
   return CALES_OK;
@@ -382,7 +389,7 @@ extern "C" int cales_project(cales_solver* s) {
   ca.phi = s->W; ca.us = s->u; ca.vs = s->v; ca.ws = s->w; ca.u = s->u; ca.v = s->v; ca.w = s->w; ca.p = s->p;
   ca.shift = nullptr; ca.gdt = 1.0; ca.cimp = 0.0; ca.update_p = 0;
   k_correct<<<s->pgrid, s->pblock, 0, s->st>>>(s->c, ca);
-  LAUNCH_TRY("k_correct");
+  LAUNCH_TRY(K_CORRECT);
   s->fresh = false;
   return CALES_OK;
 }
@@ -406,43 +413,70 @@ extern "C" int cales_transpose_xy(cales_solver* s, const double* src, double* ds
   if (!s || !src || !dst || src == dst) return fail(CALES_EINVAL, "bad transpose arguments");
   dim3 grid((s->c.nx + 31) / 32, (s->c.ny + 31) / 32, s->c.nz);
   k_transpose_xy<<<grid, dim3(32, 8), 0, s->st>>>(s->c.nx, s->c.ny, src, dst);
-  LAUNCH_TRY("k_transpose_xy");
+  LAUNCH_TRY(K_TRANSPOSE);
+  return CALES_OK;
+}
+
+// Turn the event list of the last timed step into per-kernel totals (synchronises the stream).
+static int collect_times(cales_solver* s) {
+  if (!s->ev_valid) return CALES_OK;
+  CUDA_TRY(cudaStreamSynchronize(s->st));
+  for (int q = 0; q < K_COUNT; ++q) { s->kms[q] = 0.0; s->kcnt[q] = 0; }
+  for (int e = 1; e < s->evn; ++e) {
+    const int kid = s->evkid[e];
+    if (kid < 0) continue;
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, s->evpool[e - 1], s->evpool[e]) == cudaSuccess) { s->kms[kid] += ms; ++s->kcnt[kid]; }
+  }
+  s->ev_valid = false; s->evn = 0;
+  return CALES_OK;
+}
+
+extern "C" int cales_kernel_count(void) { return K_COUNT; }
+
+extern "C" int cales_kernel_time(cales_solver* s, int kid, const char** name, double* ms_total, int* launches) {
+  if (!s || kid < 0 || kid >= K_COUNT) return fail(CALES_EINVAL, "bad kernel id");
+  int rc = collect_times(s);
+  if (rc) return rc;
+  if (name) *name = k_names[kid];
+  if (ms_total) *ms_total = s->kms[kid];
+  if (launches) *launches = s->kcnt[kid];
   return CALES_OK;
 }
 
 extern "C" int cales_set_timing(cales_solver* s, int on) {
   if (!s) return fail(CALES_EINVAL, "null solver");
-  s->timing = on ? 1 : 0; s->ev_valid = false;
+  s->timing = on ? 1 : 0; s->ev_valid = false; s->evn = 0;
   return CALES_OK;
 }
 
 extern "C" int cales_diagnostics(cales_solver* s, cales_diag* out) {
   if (!s || !out) return fail(CALES_EINVAL, "null argument");
   std::memset(out, 0, sizeof(*out));
+  int rc0 = collect_times(s);
+  if (rc0) return rc0;
+  const int timing_was = s->timing; s->timing = 0;   // the diagnostic kernels are not part of a step
   const long long nb = s->nblk;
   double* part = s->CP;   // scratch (4*nblk <= N)
   k_diag<<<s->pgrid, s->pblock, 0, s->st>>>(s->c, s->u, s->v, s->w, s->p, part);
-  LAUNCH_TRY("k_diag");
+  LAUNCH_TRY(K_DIAG);
   const int g1 = (int)(nb < 1024 ? nb : 1024);
-  k_max_stage<<<g1, 256, 0, s->st>>>(part, nb, s->stage1); LAUNCH_TRY("k_max_stage");
-  for (int q = 1; q < 4; ++q) { k_sum_stage1<<<g1, 256, 0, s->st>>>(part + q * nb, nb, s->stage1 + q * 1024); LAUNCH_TRY("k_sum_stage1"); }
+  k_max_stage<<<g1, 256, 0, s->st>>>(part, nb, s->stage1); LAUNCH_TRY(K_SUM);
+  for (int q = 1; q < 4; ++q) { k_sum_stage1<<<g1, 256, 0, s->st>>>(part + q * nb, nb, s->stage1 + q * 1024); LAUNCH_TRY(K_SUM); }
   std::vector<double> h(4 * 1024); double scal[4]; int mi = 0;
   CUDA_TRY(cudaMemcpyAsync(h.data(), s->stage1, h.size() * sizeof(double), cudaMemcpyDeviceToHost, s->st));
   CUDA_TRY(cudaMemcpyAsync(scal, s->scal, sizeof(scal), cudaMemcpyDeviceToHost, s->st));
   CUDA_TRY(cudaMemcpyAsync(&mi, s->maxit, sizeof(int), cudaMemcpyDeviceToHost, s->st));
   CUDA_TRY(cudaStreamSynchronize(s->st));
+  s->timing = timing_was;
   double md = 0, ub = 0, ke = 0, bad = 0;
   for (int q = 0; q < g1; ++q) { md = std::fmax(md, h[q]); ub += h[1024 + q]; ke += h[2048 + q]; bad += h[3072 + q]; }
   const double vol = (double)s->c.nx * s->c.ny * s->c.lz;
   out->max_div = md; out->u_bulk = ub / vol; out->kinetic_energy = ke / vol; out->nan_count = (int)bad;
   out->forcing = s->c.const_flow_rate ? scal[1] : 0.0; out->wm_max_iters = mi;
-  if (s->ev_valid) {
-    double acc[6] = {0, 0, 0, 0, 0, 0};
-    for (int rk = 0; rk < 3; ++rk) for (int b = 0; b < 6; ++b) {
-      float ms = 0.f;
-      if (s->ev[rk][b] && s->ev[rk][b + 1] && cudaEventElapsedTime(&ms, s->ev[rk][b], s->ev[rk][b + 1]) == cudaSuccess) acc[b] += ms;
-    }
-    out->ms_rhs = acc[0]; out->ms_implicit = acc[1]; out->ms_solver = acc[2]; out->ms_correction = acc[3]; out->ms_wall = acc[4]; out->ms_sgs = acc[5];
-  }
+  out->ms_rhs = s->kms[K_RHS]; out->ms_implicit = s->kms[K_CN_COEF] + s->kms[K_CN_Z];
+  out->ms_solver = s->kms[K_SUM] + s->kms[K_BULK] + s->kms[K_FFTX_FWD] + s->kms[K_FFTY_FWD] + s->kms[K_POISSON_Z] + s->kms[K_FFTY_INV] + s->kms[K_FFTX_INV];
+  out->ms_correction = s->kms[K_CORRECT]; out->ms_wall = s->kms[K_WALL];
+  out->ms_sgs = s->kms[K_SMAG] + s->kms[K_DSM_PASS1] + s->kms[K_DSM_COEF] + s->kms[K_DSM_NUT] + s->kms[K_FILL];
   return CALES_OK;
 }

@@ -102,7 +102,10 @@ def _dit(p, rng):
 
 
 def _noise(rng, shape, amp):
-    return amp * (2.0 * rng.random(shape) - 1.0)
+    r = rng.random(shape)          # uniform in [-amp, amp), built in place (config 5 is 6.4 GB per field)
+    r *= 2.0 * amp
+    r -= amp
+    return r
 
 
 def initial_fields(cfg):
@@ -135,7 +138,8 @@ def initial_fields(cfg):
         U = np.broadcast_to(U, shape)
     else:
         raise ValueError(cfg["init"])
-    u = U + _noise(rng, shape, 0.1 * ub)
+    u = _noise(rng, shape, 0.1 * ub)
+    u += U
     v = _noise(rng, shape, 0.1 * ub)
     w = _noise(rng, shape, 0.1 * ub)
     if p["bc_z"] == 1:
@@ -154,8 +158,12 @@ def time_step(cfg, u, v, w):
     zf = z_faces(p)
     dzf = (zf[1:] - zf[:-1])[:, None, None]
     dx, dy = p["lx"] / p["nx"], p["ly"] / p["ny"]
-    rate = np.abs(u) / dx + np.abs(v) / dy + np.abs(w) / dzf
-    return float(cfg["cfl"] / rate.max())
+    rmax = 0.0
+    step = max(1, (1 << 24) // (p["nx"] * p["ny"]))       # k-slabs of ~16 M points keep the temporaries small
+    for k0 in range(0, p["nz"], step):
+        sl = slice(k0, k0 + step)
+        rmax = max(rmax, float((np.abs(u[sl]) / dx + np.abs(v[sl]) / dy + np.abs(w[sl]) / dzf[sl]).max()))
+    return float(cfg["cfl"] / rmax)
 
 
 def solver_kwargs(cfg, u_bulk):

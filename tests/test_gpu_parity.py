@@ -1,0 +1,192 @@
+"""GPU parity tests proper: libcales.so (through the C ABI, via the ctypes binding) against the CPU oracle on the
+same seeded inputs, element by element.  Tolerances are north_star's: max|delta|/max|field| <= 1e-11 after one
+step and <= 1e-8 after 100 (we run fewer steps and still hold the 1-step bound scaled by the step count).
+"""
+import ctypes as C
+
+import numpy as np
+import pytest
+
+from tests import parity_cases as pc
+
+pytestmark = pytest.mark.gpu
+
+TOL_1STEP = 1e-11
+TOL_100 = 1e-8
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2411_09364_b200 import binding
+    binding.lib()
+    return binding
+
+
+def _gpu_fields(s):
+    return [s.get_numpy(f) for f in range(5)]
+
+
+@pytest.mark.parametrize("case", sorted(pc.GPU_CASES))
+def test_step_parity(oracle, gpu, case):
+    n, shape, steps = pc.GPU_CASES[case]
+    cfg, kw, (u, v, w), dt = pc.prepare(oracle, n, shape)
+    o = pc.make(oracle.Oracle, kw)
+    g = pc.make(gpu.Solver, kw)
+    o.set_velocity(u, v, w); g.set_velocity(u, v, w)
+    for s in range(steps):
+        o.step(dt); g.step(dt)
+        err = pc.field_errors(_gpu_fields(g), [o.get(f) for f in range(5)], o.dzf, kw["nu"])
+        tol = TOL_1STEP if s == 0 else min(TOL_100, TOL_1STEP * 10 * (s + 1))
+        assert max(err.values()) <= tol, (case, s, err)
+    d = g.diagnostics()
+    assert d["nan_count"] == 0
+    scale = np.max(np.abs(o.get(0))) / min(o.dx, o.dy, float(np.min(o.dzf)))
+    assert d["max_div"] <= 1e-12 * scale * 10, d           # P4 on the GPU state
+    if kw["const_flow_rate"]:
+        assert abs(d["u_bulk"] - kw["u_bulk"]) <= 1e-13 * abs(kw["u_bulk"])      # P15
+    if kw["wall_model"]:
+        assert 3 <= d["wm_max_iters"] <= 9                  # PAPER.md:130 "3 to 7" + the polish iteration
+    g.close()
+
+
+@pytest.mark.parametrize("bc_y,bc_z,stretch,shape", [
+    (0, 0, 0, (96, 48, 40)), (0, 1, 0, (192, 96, 33)), (0, 1, 1, (54, 36, 50)),
+    (1, 1, 0, (128, 54, 24)), (1, 1, 1, (72, 256, 20)), (0, 1, 0, (1536, 6, 8)), (1, 1, 0, (6, 1024, 8))])
+def test_poisson_parity_and_manufactured(oracle, gpu, bc_y, bc_z, stretch, shape):
+    import torch
+    nx, ny, nz = shape
+    kw = dict(bc_y=bc_y, bc_z=bc_z, zstretch=stretch, zstretch_factor=1.5 if stretch else 0.0)
+    o = oracle.Oracle(nx, ny, nz, 2.0, 1.5, 1.0, **kw)
+    g = gpu.Solver(nx, ny, nz, 2.0, 1.5, 1.0, **kw)
+    rng = np.random.default_rng(11)
+    # manufactured, discrete (P3): phi -> f = L_h phi by the oracle's plain stencil -> GPU solve -> phi back
+    phi = rng.standard_normal((nz, ny, nx))
+    phi = pc.weighted_mean_removed(phi, o.dzf)
+    f = o.laplacian(phi)
+    got = g.poisson_solve(torch.from_numpy(f).cuda()).cpu().numpy()
+    assert np.max(np.abs(got - phi)) <= 1e-10 * np.max(np.abs(phi))
+    # and against the oracle's own solve on a random right-hand side
+    rhs = rng.standard_normal((nz, ny, nx))
+    a = g.poisson_solve(torch.from_numpy(rhs).cuda()).cpu().numpy()
+    b = o.poisson_solve(rhs)
+    assert np.max(np.abs(a - b)) <= 1e-11 * np.max(np.abs(b))
+    # in place (rhs and phi alias)
+    t = torch.from_numpy(rhs).cuda()
+    g.poisson_solve(t, t)
+    assert np.array_equal(t.cpu().numpy(), a)
+    g.close()
+
+
+@pytest.mark.parametrize("n", [2, 6, 32, 96, 192, 256, 1024, 1536])
+def test_transforms_vs_numpy_scipy(gpu, n):
+    import scipy.fft
+    import torch
+    rng = np.random.default_rng(n)
+    g = gpu.Solver(n, 6, 5, 1.0, 1.0, 1.0, bc_z=1)
+    f = rng.standard_normal((5, 6, n))
+    F = g.transform(torch.from_numpy(f).cuda(), 0).cpu().numpy()
+    X = np.fft.rfft(f, axis=2)
+    sc = np.max(np.abs(X))
+    assert np.max(np.abs(F[..., 0] - X[..., 0].real)) <= 1e-13 * sc and np.max(np.abs(F[..., 1] - X[..., n // 2].real)) <= 1e-13 * sc
+    if n > 2:
+        assert np.max(np.abs(F[..., 2::2] - X[..., 1:n // 2].real)) <= 1e-13 * sc
+        assert np.max(np.abs(F[..., 3::2] - X[..., 1:n // 2].imag)) <= 1e-13 * sc
+    back = g.transform(torch.from_numpy(F).cuda(), 0, inverse=True).cpu().numpy()
+    assert np.max(np.abs(back - f)) <= 1e-13 * np.max(np.abs(f)) * 10
+    g.close()
+    for bc_y in (0, 1):
+        g = gpu.Solver(6, n, 5, 1.0, 1.0, 1.0, bc_y=bc_y, bc_z=1)
+        f = rng.standard_normal((5, n, 6))
+        F = g.transform(torch.from_numpy(f).cuda(), 1).cpu().numpy()
+        if bc_y == 0:
+            X = np.fft.rfft(f, axis=1); sc = np.max(np.abs(X))
+            assert np.max(np.abs(F[:, 0] - X[:, 0].real)) <= 1e-13 * sc and np.max(np.abs(F[:, 1] - X[:, n // 2].real)) <= 1e-13 * sc
+            if n > 2:
+                assert np.max(np.abs(F[:, 2::2] - X[:, 1:n // 2].real)) <= 1e-13 * sc
+                assert np.max(np.abs(F[:, 3::2] - X[:, 1:n // 2].imag)) <= 1e-13 * sc
+        else:
+            X = 0.5 * scipy.fft.dct(f, type=2, axis=1)
+            assert np.max(np.abs(F - X)) <= 1e-13 * np.max(np.abs(X)) * 10
+        back = g.transform(torch.from_numpy(F).cuda(), 1, inverse=True).cpu().numpy()
+        assert np.max(np.abs(back - f)) <= 1e-12 * np.max(np.abs(f))
+        g.close()
+
+
+def test_transpose_is_bit_exact(gpu):
+    import torch
+    g = gpu.Solver(70, 36, 5, 1.0, 1.0, 1.0)
+    a = torch.randn(5, 36, 70, dtype=torch.float64, device="cuda")
+    assert torch.equal(g.transpose_xy(a), a.transpose(1, 2).contiguous())
+    g.close()
+
+
+@pytest.mark.parametrize("n,shape", [(1, (40, 24, 20)), (3, (72, 36, 40)), (4, (96, 36, 24)), (5, (72, 48, 24)), (2, (72, 48, 24))])
+def test_eddy_viscosity_and_wall_stress_parity(oracle, gpu, n, shape):
+    import torch
+    cfg, kw, (u, v, w), dt = pc.prepare(oracle, n, shape)
+    o = pc.make(oracle.Oracle, kw)
+    g = pc.make(gpu.Solver, kw)
+    o.set_velocity(u, v, w); g.set_velocity(u, v, w)
+    if kw["wall_model"]:
+        a, b = g.wall_stress().cpu().numpy(), o.wall_stress()
+        assert np.max(np.abs(a - b)) <= 1e-12 * np.max(np.abs(b))
+    a = g.eddy_viscosity().cpu().numpy()
+    b = o.eddy_viscosity()
+    assert np.max(np.abs(a - b)) <= 1e-11 * max(np.max(np.abs(b)), kw["nu"])
+    if kw["sgs_model"] == 2:
+        ca = g.get_cs(per_plane=bool(kw["dsm_avg_xy_plane"])).cpu().numpy(); cb = o.get_cs()
+        assert np.max(np.abs(ca - cb)) <= 1e-9 * max(np.max(np.abs(cb)), 1e-300)
+    # external-field form of the call
+    a2 = g.eddy_viscosity(*(torch.from_numpy(q).cuda() for q in (u, v, w))).cpu().numpy()
+    assert np.array_equal(a, a2)
+    g.close()
+
+
+def test_closed_forms_on_gpu(gpu):
+    """Pins applied to the GPU path directly (not via the oracle): Taylor-Green amplitude G^n (P6) and
+    nu_t = (Cs Delta)^2 G on a linear shear (P10)."""
+    import math
+    n, nu, dt, steps = 32, 1e-2, 5e-3, 5
+    L = 2 * math.pi
+    g = gpu.Solver(n, n, 8, L, L, L / 4, nu=nu, sgs_model=0)
+    h = L / n
+    x = (np.arange(n) + 1) * h; xc = (np.arange(n) + 0.5) * h
+    u = np.broadcast_to(np.sin(x)[None, None, :] * np.cos(xc)[None, :, None], (8, n, n)).copy()
+    v = np.broadcast_to(-np.cos(xc)[None, None, :] * np.sin(x)[None, :, None], (8, n, n)).copy()
+    g.set_velocity(u, v, np.zeros_like(u))
+    for _ in range(steps):
+        g.step(dt)
+    keff2 = 2.0 * (math.sin(h / 2) / (h / 2)) ** 2
+    z = -nu * keff2 * dt
+    G = (1 + z + z * z / 2 + z ** 3 / 6) ** steps
+    assert np.max(np.abs(g.get_numpy(0) - G * u)) <= 1e-12
+    assert np.max(np.abs(g.get_numpy(1) - G * v)) <= 1e-12
+    g.close()
+    # linear shear between no-slip walls, static Smagorinsky without damping
+    nx, ny, nz, Gs, cs = 32, 16, 24, 3.0, 0.1
+    g = gpu.Solver(nx, ny, nz, 1.0, 1.0, 1.0, bc_z=1, sgs_model=1, cs=cs)
+    zc = (np.arange(nz) + 0.5) / nz
+    u = np.broadcast_to((Gs * zc)[:, None, None], (nz, ny, nx)).copy()
+    g.set_velocity(u, np.zeros_like(u), np.zeros_like(u))
+    nut = g.eddy_viscosity().cpu().numpy()
+    delta = (1.0 / nx * 1.0 / ny * 1.0 / nz) ** (1.0 / 3.0)
+    assert np.max(np.abs(nut[: nz // 2] - (cs * delta) ** 2 * Gs)) <= 1e-14 * (cs * delta) ** 2 * Gs * 10
+    g.close()
+
+
+def test_error_paths(gpu):
+    import torch
+    L = gpu.lib()
+    with pytest.raises(gpu.CalesError):
+        gpu.Solver(30, 14, 8, 1.0, 1.0, 1.0)                 # 14 = 2*7 does not factor into 2 and 3
+    with pytest.raises(gpu.CalesError):
+        gpu.Solver(32, 16, 8, 1.0, 1.0, 1.0, wall_model=1)   # wall model without z walls
+    P = gpu.make_params(32, 16, 8, 1.0, 1.0, 1.0)
+    need = L.cales_workspace_bytes(C.byref(P))
+    ws = torch.empty(need // 8 + 64, dtype=torch.float64, device="cuda")
+    P.workspace = ws.data_ptr() + ((-ws.data_ptr()) % 256); P.workspace_bytes = need - 8
+    h = C.c_void_p()
+    assert L.cales_create(C.byref(P), C.byref(h)) == 1 and b"small" in L.cales_last_error()
+    assert L.cales_step(None, 1.0) == 1
