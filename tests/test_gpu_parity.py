@@ -116,8 +116,8 @@ def test_transforms_vs_numpy_scipy(gpu, n):
 
 def test_transpose_is_bit_exact(gpu):
     import torch
-    g = gpu.Solver(70, 36, 5, 1.0, 1.0, 1.0)
-    a = torch.randn(5, 36, 70, dtype=torch.float64, device="cuda")
+    g = gpu.Solver(72, 36, 5, 1.0, 1.0, 1.0)
+    a = torch.randn(5, 36, 72, dtype=torch.float64, device="cuda")
     assert torch.equal(g.transpose_xy(a), a.transpose(1, 2).contiguous())
     g.close()
 
