@@ -37,7 +37,7 @@ struct cales_solver {
   double *u, *v, *w, *p, *nut, *us, *vs, *ws, *Ru, *Rv, *Rw, *W, *CP, *CQ, *smag;
   double *tau;
   // tables
-  double *dzf, *dzc, *zc, *ak, *ck, *lamx, *lamy, *cncoef, *partial, *stage1, *scal, *dsm_part, *dsm_cs;
+  double *dzf, *dzc, *rdzf, *rdzc, *delta, *zc, *ak, *ck, *lamx, *lamy, *cncoef, *partial, *stage1, *scal, *dsm_part, *dsm_cs;
   double2 *twx, *twy, *dctw;
   int* maxit;
   FftPlan plx, ply;
@@ -67,6 +67,7 @@ static size_t carve(cales_solver* s, const cales_params* p, double* base) {
   double* smag = p->sgs_model == CALES_SGS_DSMAG ? take(N) : nullptr;
   double* tau = take(4 * nxy);
   double* dzf = take(p->nz + 2); double* dzc = take(p->nz + 2); double* zc = take(p->nz);
+  double* rdzf = take(p->nz + 2); double* rdzc = take(p->nz + 2); double* delta = take(p->nz);
   double* ak = take(p->nz); double* ck = take(p->nz);
   double* lamx = take(p->nx); double* lamy = take(p->ny);
   double* twx = take(2 * (size_t)p->nx); double* twy = take(2 * (size_t)p->ny); double* dctw = take(2 * ((size_t)p->ny / 2 + 1));
@@ -81,7 +82,7 @@ static size_t carve(cales_solver* s, const cales_params* p, double* base) {
   if (s && base) {
     s->u = f[0]; s->v = f[1]; s->w = f[2]; s->p = f[3]; s->nut = f[4]; s->us = f[5]; s->vs = f[6]; s->ws = f[7];
     s->Ru = f[8]; s->Rv = f[9]; s->Rw = f[10]; s->W = f[11]; s->CP = CP; s->CQ = CQ; s->smag = smag; s->tau = tau;
-    s->dzf = dzf; s->dzc = dzc; s->zc = zc; s->ak = ak; s->ck = ck; s->lamx = lamx; s->lamy = lamy;
+    s->dzf = dzf; s->dzc = dzc; s->zc = zc; s->rdzf = rdzf; s->rdzc = rdzc; s->delta = delta; s->ak = ak; s->ck = ck; s->lamx = lamx; s->lamy = lamy;
     s->twx = reinterpret_cast<double2*>(twx); s->twy = reinterpret_cast<double2*>(twy); s->dctw = reinterpret_cast<double2*>(dctw);
     s->cncoef = cncoef; s->partial = partial; s->stage1 = stage1; s->scal = scal; s->maxit = reinterpret_cast<int*>(scal + 16);
     s->dsm_part = dsm_part; s->dsm_cs = dsm_cs; s->nblk = (long long)nblk;
@@ -150,6 +151,9 @@ extern "C" int cales_create(const cales_params* p, cales_solver** out) {
   if (e == cudaSuccess) e = up(s->dzf, H.dzf, nz + 2);
   if (e == cudaSuccess) e = up(s->dzc, H.dzc, nz + 1);
   if (e == cudaSuccess) e = up(s->zc, H.zc, nz);
+  if (e == cudaSuccess) e = up(s->rdzf, H.rdzf, nz + 2);
+  if (e == cudaSuccess) e = up(s->rdzc, H.rdzc, nz + 1);
+  if (e == cudaSuccess) e = up(s->delta, H.delta, nz);
   if (e == cudaSuccess) e = up(s->ak, H.ak, nz);
   if (e == cudaSuccess) e = up(s->ck, H.ck, nz);
   if (e == cudaSuccess) e = up(s->lamx, H.lamx, nx);
@@ -160,7 +164,7 @@ extern "C" int cales_create(const cales_params* p, cales_solver** out) {
   if (e == cudaSuccess) e = cudaStreamSynchronize(s->st);
   if (e != cudaSuccess) { delete s; return fail(CALES_ECUDA, std::string("table upload: ") + cudaGetErrorString(e)); }
   s->c = H.c;
-  s->c.dzf = s->dzf + 1; s->c.dzc = s->dzc + 1; s->c.zc = s->zc; s->c.tau = s->tau;
+  s->c.dzf = s->dzf + 1; s->c.dzc = s->dzc + 1; s->c.zc = s->zc; s->c.rdzf = s->rdzf + 1; s->c.rdzc = s->rdzc + 1; s->c.delta = s->delta; s->c.tau = s->tau;
   s->pt.ak = s->ak; s->pt.ck = s->ck; s->pt.lamx = s->lamx; s->pt.lamy = s->lamy;
   s->wg = H.wg;
   s->plx = H.plx; s->plx.tw = s->twx;
@@ -208,6 +212,11 @@ extern "C" int cales_set_field(cales_solver* s, int field, const double* src, in
   double* d = field_ptr(s, field);
   if (!d) return fail(CALES_EINVAL, "bad field id");
   CUDA_TRY(cudaMemcpyAsync(d, src, s->N * sizeof(double), on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, s->st));
+  // the wall faces are kept at exactly 0 (include/cales.h; the interior kernels rely on it)
+  if (field == CALES_V && s->c.bc_y == BC_WALL)
+    CUDA_TRY(cudaMemset2DAsync(d + (size_t)(s->c.ny - 1) * s->c.nx, (size_t)s->nxy * sizeof(double), 0, (size_t)s->c.nx * sizeof(double), (size_t)s->c.nz, s->st));
+  if (field == CALES_W && s->c.bc_z == BC_WALL)
+    CUDA_TRY(cudaMemsetAsync(d + (size_t)(s->c.nz - 1) * s->nxy, 0, (size_t)s->nxy * sizeof(double), s->st));
   if (!on_device) CUDA_TRY(cudaStreamSynchronize(s->st));
   if (field <= CALES_W) s->fresh = false;
   return CALES_OK;

@@ -95,11 +95,27 @@ CALES_HD double strain_at(GU U, GV V, GW W, double rdx, double rdy, double rdzf,
 // D = 1 - exp(-d+/A+) with the local u_tau of the nearest z wall (S5).
 CALES_HD double smag_point(const Ctx& c, const double* u, const double* v, const double* w, int i, int j, int k) {
   double S[6];
-  auto U = [&](int a, int b, int d) { return velg<0>(c, u, i + a, j + b, k + d, GH_STRAIN); };
-  auto V = [&](int a, int b, int d) { return velg<1>(c, v, i + a, j + b, k + d, GH_STRAIN); };
-  auto W = [&](int a, int b, int d) { return velg<2>(c, w, i + a, j + b, k + d, GH_STRAIN); };
-  const double smag = strain_at(U, V, W, 1.0 / c.dx, 1.0 / c.dy, 1.0 / c.dzf[k], 1.0 / c.dzc[k], 1.0 / c.dzc[k - 1], S);
-  const double delta = cbrt(c.dx * c.dy * c.dzf[k]);
+  double smag;
+  if (interior_row(c, j, k)) {
+    // no wall ghost in reach: direct loads at wrapped offsets
+    const long long n = idx3(c, i, j, k);
+    const Nbr o = neighbours(c, i, j, k);
+    const int im = o.im, ip = o.ip, jm = o.jm, jp = o.jp;
+    const long long km = o.km, kp = o.kp;
+    auto at = [&](const double* __restrict__ q, int a, int b, int d) {
+      return q[n + (d < 0 ? km : (d > 0 ? kp : 0)) + ((a < 0 ? im : (a > 0 ? ip : 0)) + (b < 0 ? jm : (b > 0 ? jp : 0)))];
+    };
+    auto U = [&](int a, int b, int d) { return at(u, a, b, d); };
+    auto V = [&](int a, int b, int d) { return at(v, a, b, d); };
+    auto W = [&](int a, int b, int d) { return at(w, a, b, d); };
+    smag = strain_at(U, V, W, c.rdx, c.rdy, c.rdzf[k], c.rdzc[k], c.rdzc[k - 1], S);
+  } else {
+    auto U = [&](int a, int b, int d) { return velg<0>(c, u, i + a, j + b, k + d, GH_STRAIN); };
+    auto V = [&](int a, int b, int d) { return velg<1>(c, v, i + a, j + b, k + d, GH_STRAIN); };
+    auto W = [&](int a, int b, int d) { return velg<2>(c, w, i + a, j + b, k + d, GH_STRAIN); };
+    smag = strain_at(U, V, W, c.rdx, c.rdy, c.rdzf[k], c.rdzc[k], c.rdzc[k - 1], S);
+  }
+  const double delta = c.delta[k];
   double D = 1.0;
   if (c.van_driest) {
     const double db = c.zc[k], dt = c.lz - c.zc[k];
@@ -175,7 +191,7 @@ CALES_HD void dsm_mid(int tid, int nth, const Ctx& c, int i0, int j0, int k, con
     }
     flt[idx] = s;
   }
-  const double rdx = 1.0 / c.dx, rdy = 1.0 / c.dy, rdzf = 1.0 / c.dzf[k], rdzc = 1.0 / c.dzc[k], rdzcm = 1.0 / c.dzc[k - 1];
+  const double rdx = c.rdx, rdy = c.rdy, rdzf = c.rdzf[k], rdzc = c.rdzc[k], rdzcm = c.rdzc[k - 1];
   for (int r = tid; r < per; r += nth) {
     const int my = r / DSM_MX, mx = r % DSM_MX;
     auto U = [&](int a, int b, int d) { return raw[dsm_raw_off(0, 1 + d, my + 1 + b, mx + 1 + a)]; };
@@ -224,8 +240,8 @@ CALES_HD void dsm_point(const Ctx& c, int i0, int j0, int k, int tx, int ty, con
   auto W = [&](int a, int b, int d) { return flt[((2 * 3 + 1 + d) * DSM_MY + my + b) * DSM_MX + mx + a]; };
   (void)fst;
   double St[6];
-  const double stmag = strain_at(U, V, W, 1.0 / c.dx, 1.0 / c.dy, 1.0 / c.dzf[k], 1.0 / c.dzc[k], 1.0 / c.dzc[k - 1], St);
-  const double d2 = pow(c.dx * c.dy * c.dzf[k], 2.0 / 3.0);
+  const double stmag = strain_at(U, V, W, c.rdx, c.rdy, c.rdzf[k], c.rdzc[k], c.rdzc[k - 1], St);
+  const double d2 = c.delta[k] * c.delta[k];
   double al = c.alpha;
   if (c.bc_y == BC_WALL && (gj == 0 || gj == c.ny - 1)) al = sqrt(c.alpha);
   double ll = 0.0, m2 = 0.0;
@@ -249,7 +265,7 @@ CALES_HD void dsm_row_sums(const double* part, int ntx, long long row, double* l
 // pass 2: nu_t = c_s Delta^2 |S| with the clip of PAPER.md:128 (c_s >= 0) or of the total viscosity (S14)
 CALES_HD double dsm_nut_point(const Ctx& c, const double* cs, const double* smag, int i, int j, int k) {
   const double cc = c.dsm_plane ? cs[k] : cs[(long long)k * c.ny + j];
-  const double d2 = pow(c.dx * c.dy * c.dzf[k], 2.0 / 3.0);
+  const double d2 = c.delta[k] * c.delta[k];
   const double sm = smag[idx3(c, i, j, k)];
   if (!c.dsm_clip_total) return (cc < 0.0 ? 0.0 : cc) * d2 * sm;
   const double t = cc * d2 * sm;

@@ -22,11 +22,14 @@ struct Ctx {
   int wm_maxit;
   long long N;     // nx*ny*nz
   long long nxy;   // nx*ny
-  double dx, dy, lz, nu, cs, aplus, alpha, kappa, Blog, h_wm, wm_tol, u_bulk;
+  double dx, dy, rdx, rdy, lz, nu, cs, aplus, alpha, kappa, Blog, h_wm, wm_tol, u_bulk;
   // 1-D grid tables in device memory, offset so that the ghost entries are addressable:
   const double* dzf;   // dzf[-1 .. nz]   cell heights (ghost = neighbour's / wrapped)
   const double* dzc;   // dzc[-1 .. nz-1] centre spacings across face k+1 (mirrored ghost centre at walls)
   const double* zc;    // zc[0 .. nz-1]
+  const double* rdzf;  // 1/dzf[-1 .. nz]
+  const double* rdzc;  // 1/dzc[-1 .. nz-1]
+  const double* delta; // filter width Delta_k = (dx dy dzf[k])^(1/3), k = 0..nz-1 (S4)
   const double* tau;   // wall stress planes [wall][comp][ny][nx]
 };
 
@@ -76,6 +79,28 @@ CALES_HD double scalg(const Ctx& c, const double* __restrict__ q, int i, int j, 
   if (c.bc_z == BC_PER) k = wrapi(k, c.nz);
   else { if (k < 0) { k = 0; s *= sgn; } else if (k >= c.nz) { k = c.nz - 1; s *= sgn; } }
   return s * q[idx3(c, i, j, k)];
+}
+
+// True when none of the neighbours of (.,j,k) read by rhs_point / the strain rate needs a wall ghost: periodic wrap is
+// plain index arithmetic, wall rows/planes go through the generic accessors.  Relies on the library keeping the wall
+// faces v[.][ny-1][.] and w[nz-1] at exactly 0 (cales_set_field zeroes them).
+CALES_HD bool interior_row(const Ctx& c, int j, int k) {
+  const bool yok = c.bc_y == BC_PER || (j >= 1 && j <= c.ny - 2);
+  const bool zok = c.bc_z == BC_PER || (k >= 1 && k <= c.nz - 2);
+  return yok && zok;
+}
+
+// Neighbour offsets of an interior point (periodic wrap only).
+struct Nbr { int im, ip, jm, jp; long long km, kp; };
+CALES_HD Nbr neighbours(const Ctx& c, int i, int j, int k) {
+  Nbr o;
+  o.im = (i == 0) ? c.nx - 1 : -1;
+  o.ip = (i == c.nx - 1) ? -(c.nx - 1) : 1;
+  o.jm = (j == 0) ? (c.ny - 1) * c.nx : -c.nx;
+  o.jp = (j == c.ny - 1) ? -(c.ny - 1) * c.nx : c.nx;
+  o.km = (k == 0) ? (long long)(c.nz - 1) * c.nxy : -c.nxy;
+  o.kp = (k == c.nz - 1) ? -(long long)(c.nz - 1) * c.nxy : c.nxy;
+  return o;
 }
 
 // RK3 coefficients of PAPER.md:100.

@@ -176,7 +176,7 @@ CALES_HD void fx_load(int tid, int nth, const Ctx& c, const FftPlan& pl, int B, 
         const double* vm = nullptr; const double* wm = nullptr;
         if (j > 0) vm = vl - n; else if (c.bc_y == BC_PER) vm = vl + (long long)(c.ny - 1) * n;
         if (k > 0) wm = wl - c.nxy; else if (c.bc_z == BC_PER) wm = wl + (long long)(c.nz - 1) * c.nxy;
-        const double rdx = 1.0 / c.dx, rdy = 1.0 / c.dy, rdz = 1.0 / c.dzf[k];
+        const double rdx = c.rdx, rdy = c.rdy, rdz = c.rdzf[k];
         const double2 uu = ld2(ul, t);
         const double um = ul[t == 0 ? n - 1 : 2 * t - 1];
         const double2 vv = ld2(vl, t);

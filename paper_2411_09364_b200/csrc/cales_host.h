@@ -52,7 +52,7 @@ static inline void make_plan(FftPlan& pl, int n) {
 
 struct HostSetup {
   cales_params P;                 // with the defaults filled in
-  std::vector<double> dzf, dzc, zc, ak, ck, lamx, lamy, twx, twy, dctw;   // dzf: index k+1 holds dzf[k], k=-1..nz; dzc: k+1 holds dzc[k], k=-1..nz-1
+  std::vector<double> dzf, dzc, rdzf, rdzc, delta, zc, ak, ck, lamx, lamy, twx, twy, dctw;   // dzf: index k+1 holds dzf[k], k=-1..nz; dzc: k+1 holds dzc[k], k=-1..nz-1
   Ctx c;                          // table pointers NOT set
   WallGeom wg;
   FftPlan plx, ply;               // twiddle pointers NOT set
@@ -86,6 +86,8 @@ static inline int build_setup(const cales_params* p, HostSetup& H) {
   if (zper) { H.dzf[0] = H.dzf[nz]; H.dzf[nz + 1] = H.dzf[1]; } else { H.dzf[0] = H.dzf[1]; H.dzf[nz + 1] = H.dzf[nz]; }
   for (int k = 0; k < nz - 1; ++k) H.dzc[k + 1] = H.zc[k + 1] - H.zc[k];
   if (zper) { H.dzc[0] = H.dzf[1]; H.dzc[nz] = H.dzf[1]; } else { H.dzc[0] = 2.0 * H.zc[0]; H.dzc[nz] = 2.0 * (p->lz - H.zc[nz - 1]); }   // mirrored ghost centre
+  H.rdzf.assign(nz + 2, 0.0); H.rdzc.assign(nz + 2, 0.0);
+  for (int k = 0; k < nz + 2; ++k) { H.rdzf[k] = 1.0 / H.dzf[k]; if (k <= nz) H.rdzc[k] = 1.0 / H.dzc[k]; }
   H.ak.resize(nz); H.ck.resize(nz);
   for (int k = 0; k < nz; ++k) { H.ak[k] = 1.0 / (H.dzf[k + 1] * H.dzc[k]); H.ck[k] = 1.0 / (H.dzf[k + 1] * H.dzc[k + 1]); }
   // ---- eigenvalues of the 3-point operators in the packed layouts (ref. [28])
@@ -101,6 +103,8 @@ static inline int build_setup(const cales_params* p, HostSetup& H) {
     else sn = std::sin(PI_ * j / (2.0 * ny));
     H.lamy[j] = -4.0 / (dy * dy) * sn * sn;
   }
+  H.delta.resize(nz);
+  for (int k = 0; k < nz; ++k) H.delta[k] = std::cbrt(dx * dy * H.dzf[k + 1]);
   // ---- twiddles in extended precision, rounded once to fp64
   H.twx.resize(2 * (size_t)nx); H.twy.resize(2 * (size_t)ny); H.dctw.resize(2 * ((size_t)ny / 2 + 1));
   const long double PIL = 3.14159265358979323846264338327950288L;
@@ -112,10 +116,10 @@ static inline int build_setup(const cales_params* p, HostSetup& H) {
   c.nx = nx; c.ny = ny; c.nz = nz; c.N = (long long)nx * ny * nz; c.nxy = (long long)nx * ny;
   c.bc_y = p->bc_y; c.bc_z = p->bc_z; c.wall_model = p->wall_model; c.sgs = p->sgs_model; c.van_driest = p->van_driest;
   c.implicit_z = p->implicit_z; c.dsm_plane = p->dsm_avg_xy_plane; c.dsm_clip_total = p->dsm_clip_total; c.const_flow_rate = p->const_flow_rate;
-  c.wm_maxit = H.P.wm_maxit; c.dx = dx; c.dy = dy; c.lz = p->lz; c.nu = p->nu; c.cs = p->cs; c.aplus = H.P.aplus;
+  c.wm_maxit = H.P.wm_maxit; c.dx = dx; c.dy = dy; c.rdx = 1.0 / dx; c.rdy = 1.0 / dy; c.lz = p->lz; c.nu = p->nu; c.cs = p->cs; c.aplus = H.P.aplus;
   c.alpha = p->dsm_alpha2d > 0.0 ? p->dsm_alpha2d : std::cbrt(4.0);
   c.kappa = H.P.kappa; c.Blog = p->B; c.h_wm = p->h_wm; c.wm_tol = H.P.wm_tol; c.u_bulk = p->u_bulk;
-  c.dzf = nullptr; c.dzc = nullptr; c.zc = nullptr; c.tau = nullptr;
+  c.dzf = nullptr; c.dzc = nullptr; c.zc = nullptr; c.rdzf = nullptr; c.rdzc = nullptr; c.delta = nullptr; c.tau = nullptr;
   // ---- wall-model sampling geometry (linear interpolation between locations 1 and 2)
   for (int wall = 0; wall < 2; ++wall) {
     auto dist = [&](int q) { return wall == 0 ? H.zc[q] : p->lz - H.zc[nz - 1 - q]; };

@@ -43,7 +43,7 @@ extern "C" int emu_create(const cales_params* p, emu_solver** out) {
   const size_t ntx = (p->nx + DSM_TX - 1) / DSM_TX;
   s->dsm_part.assign((size_t)p->nz * p->ny * ntx * 2, 0.0);
   s->dsm_cs.assign((size_t)p->nz * p->ny, 0.0);
-  s->c.dzf = H.dzf.data() + 1; s->c.dzc = H.dzc.data() + 1; s->c.zc = H.zc.data(); s->c.tau = s->tau.data();
+  s->c.dzf = H.dzf.data() + 1; s->c.dzc = H.dzc.data() + 1; s->c.zc = H.zc.data(); s->c.rdzf = H.rdzf.data() + 1; s->c.rdzc = H.rdzc.data() + 1; s->c.delta = H.delta.data(); s->c.tau = s->tau.data();
   s->plx = H.plx; s->plx.tw = reinterpret_cast<const double2*>(H.twx.data());
   s->ply = H.ply; s->ply.tw = reinterpret_cast<const double2*>(H.twy.data()); s->ply.dctw = reinterpret_cast<const double2*>(H.dctw.data());
   s->pt.ak = H.ak.data(); s->pt.ck = H.ck.data(); s->pt.lamx = H.lamx.data(); s->pt.lamy = H.lamy.data();
@@ -57,7 +57,14 @@ static std::vector<double>* fld(emu_solver* s, int f) {
   switch (f) { case 0: return &s->u; case 1: return &s->v; case 2: return &s->w; case 3: return &s->p; case 4: return &s->nut; }
   return nullptr;
 }
-extern "C" int emu_set_field(emu_solver* s, int f, const double* src) { std::memcpy(fld(s, f)->data(), src, s->N * sizeof(double)); if (f <= 2) s->fresh = false; return 0; }
+extern "C" int emu_set_field(emu_solver* s, int f, const double* src) {
+  std::memcpy(fld(s, f)->data(), src, s->N * sizeof(double));
+  const Ctx& c = s->c;
+  if (f == 1 && c.bc_y == BC_WALL) for (int k = 0; k < c.nz; ++k) for (int i = 0; i < c.nx; ++i) s->v[idx3(c, i, c.ny - 1, k)] = 0.0;
+  if (f == 2 && c.bc_z == BC_WALL) for (long long q = 0; q < s->nxy; ++q) s->w[(long long)(c.nz - 1) * s->nxy + q] = 0.0;
+  if (f <= 2) s->fresh = false;
+  return 0;
+}
 extern "C" int emu_get_field(emu_solver* s, int f, double* dst) { std::memcpy(dst, fld(s, f)->data(), s->N * sizeof(double)); return 0; }
 
 // ---- kernel emulations: same block decomposition and phase order as the __global__ wrappers ----
@@ -189,7 +196,7 @@ static void emu_substep(emu_solver* s, int rk, double dt) {
   a.Ru0 = s->Ru.data(); a.Rv0 = s->Rv.data(); a.Rw0 = s->Rw.data(); a.Ru1 = s->Ru.data(); a.Rv1 = s->Rv.data(); a.Rw1 = s->Rw.data();
   a.us = s->us.data(); a.vs = s->vs.data(); a.ws = s->ws.data(); a.dt = dt; a.al = al; a.be = be; a.ga = ga; a.store_R = rk < 2 ? 1 : 0;
   double sum = 0.0;
-  for (int k = 0; k < c.nz; ++k) for (int j = 0; j < c.ny; ++j) for (int i = 0; i < c.nx; ++i) sum += rhs_point(c, a, i, j, k) * c.dzf[k];
+  for (int k = 0; k < c.nz; ++k) for (int j = 0; j < c.ny; ++j) for (int i = 0; i < c.nx; ++i) sum += rhs_any(c, a, i, j, k) * c.dzf[k];
   if (imp) {
     const double cimp = 0.5 * ga * c.nu * dt;
     cn_coefficients(c, cimp, s->cncoef.data());

@@ -122,7 +122,7 @@ def test_transpose_is_bit_exact(gpu):
     g.close()
 
 
-@pytest.mark.parametrize("n,shape", [(1, (40, 24, 20)), (3, (72, 36, 40)), (4, (96, 36, 24)), (5, (72, 48, 24)), (2, (72, 48, 24))])
+@pytest.mark.parametrize("n,shape", [(1, (48, 24, 20)), (3, (72, 36, 40)), (4, (96, 36, 24)), (5, (72, 48, 24)), (2, (72, 48, 24))])
 def test_eddy_viscosity_and_wall_stress_parity(oracle, gpu, n, shape):
     import torch
     cfg, kw, (u, v, w), dt = pc.prepare(oracle, n, shape)
