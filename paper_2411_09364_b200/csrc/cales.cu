@@ -76,8 +76,8 @@ static size_t carve(cales_solver* s, const cales_params* p, double* base) {
   double* partial = take(nblk > nxy ? nblk : nxy);
   double* stage1 = take(4 * 1024);
   double* scal = take(32);
-  const size_t ntx = (p->nx + DSM_TX - 1) / DSM_TX;
-  double* dsm_part = p->sgs_model == CALES_SGS_DSMAG ? take((size_t)p->nz * p->ny * ntx * 2) : nullptr;
+  const size_t pslots = (size_t)dsm_shape(p->nx).pslots;
+  double* dsm_part = p->sgs_model == CALES_SGS_DSMAG ? take((size_t)p->nz * p->ny * pslots * 2) : nullptr;
   double* dsm_cs = p->sgs_model == CALES_SGS_DSMAG ? take((size_t)p->nz * p->ny) : nullptr;
   if (s && base) {
     s->u = f[0]; s->v = f[1]; s->w = f[2]; s->p = f[3]; s->nut = f[4]; s->us = f[5]; s->vs = f[6]; s->ws = f[7];
@@ -103,9 +103,9 @@ extern "C" size_t cales_workspace_bytes(const cales_params* p) {
 
 // Kernel ids for the per-kernel timing table (cales_kernel_time).
 enum { K_RHS = 0, K_CN_COEF, K_CN_Z, K_SUM, K_BULK, K_FFTX_FWD, K_FFTY_FWD, K_POISSON_Z, K_FFTY_INV, K_FFTX_INV, K_CORRECT,
-       K_WALL, K_SMAG, K_DSM_PASS1, K_DSM_COEF, K_DSM_NUT, K_FILL, K_TRANSPOSE, K_DIAG, K_COUNT };
+       K_WALL, K_SMAG, K_DSM_PASS1, K_DSM_COL, K_DSM_COEF, K_DSM_NUT, K_FILL, K_TRANSPOSE, K_DIAG, K_COUNT };
 static const char* const k_names[K_COUNT] = {"k_rhs", "k_cn_coef", "k_cn_z", "k_sum_stage1", "k_bulk_finish", "k_fft_x_fwd", "k_fft_y_fwd",
-  "k_poisson_z", "k_fft_y_inv", "k_fft_x_inv", "k_correct", "k_wall_stress", "k_smag", "k_dsm_pass1", "k_dsm_coef", "k_dsm_nut", "k_fill",
+  "k_poisson_z", "k_fft_y_inv", "k_fft_x_inv", "k_correct", "k_wall_stress", "k_smag", "k_dsm_pass1", "k_dsm_col", "k_dsm_coef", "k_dsm_nut", "k_fill",
   "k_transpose_xy", "k_diag"};
 
 // record an event on the stream tagged with the kernel that just finished (kid < 0: a separator)
@@ -283,10 +283,28 @@ static int run_eddy_viscosity(cales_solver* s, const double* u, const double* v,
     k_smag<<<s->pgrid, s->pblock, 0, s->st>>>(s->c, u, v, w, nut);
     LAUNCH_TRY(K_SMAG);
   } else {
-    dim3 grid((s->c.nx + DSM_TX - 1) / DSM_TX, (s->c.ny + DSM_TY - 1) / DSM_TY, s->c.nz);
-    k_dsm_pass1<<<grid, dim3(DSM_TX, DSM_TY), DSM_SMEM_DOUBLES * sizeof(double), s->st>>>(s->c, u, v, w, s->smag, s->dsm_part);
-    LAUNCH_TRY(K_DSM_PASS1);
-    k_dsm_coef<<<s->c.nz, 128, 0, s->st>>>(s->c, s->dsm_part, (int)grid.x, s->dsm_cs);
+    // pass 1: the column-marching kernel wherever the test filter is uniform in y; the tile kernel (Eq. 9 literally) on
+    // the DSM_TY rows next to each y wall, where filter and strain do not commute
+    const Ctx& c = s->c;
+    const DsmShape ds = dsm_shape(c.nx);
+    const bool ywall = c.bc_y == BC_WALL;
+    const bool split = ywall && c.ny >= 3 * DSM_TY;
+    const size_t tile_smem = DSM_SMEM_DOUBLES * sizeof(double);
+    const unsigned ntile = (unsigned)((c.nx + DSM_TX - 1) / DSM_TX);
+    if (ywall) {
+      if (split) k_dsm_pass1<<<dim3(ntile, 2, c.nz), dim3(DSM_TX, DSM_TY), tile_smem, s->st>>>(c, u, v, w, c.ny - DSM_TY, DSM_TY, c.ny - DSM_TY, ds.pslots, s->smag, s->dsm_part);
+      else k_dsm_pass1<<<dim3(ntile, (c.ny + DSM_TY - 1) / DSM_TY, c.nz), dim3(DSM_TX, DSM_TY), tile_smem, s->st>>>(c, u, v, w, DSM_TY, c.ny, c.ny, ds.pslots, s->smag, s->dsm_part);
+      LAUNCH_TRY(K_DSM_PASS1);
+    }
+    if (!ywall || split) {
+      const int jlo = ywall ? DSM_TY : 0, jhi = ywall ? c.ny - DSM_TY : c.ny;
+      dim3 grid(ds.nbx, (jhi - jlo + DSMC_LY - 1) / DSMC_LY, c.nz);
+      if (ds.txb == 64) k_dsm_col<64><<<grid, 64, 0, s->st>>>(c, u, v, w, jlo, jhi, ds.pslots, s->smag, s->dsm_part);
+      else if (ds.txb == 96) k_dsm_col<96><<<grid, 96, 0, s->st>>>(c, u, v, w, jlo, jhi, ds.pslots, s->smag, s->dsm_part);
+      else k_dsm_col<128><<<grid, 128, 0, s->st>>>(c, u, v, w, jlo, jhi, ds.pslots, s->smag, s->dsm_part);
+      LAUNCH_TRY(K_DSM_COL);
+    }
+    k_dsm_coef<<<s->c.nz, 128, 0, s->st>>>(s->c, s->dsm_part, ds.pslots, s->dsm_cs);
     LAUNCH_TRY(K_DSM_COEF);
     k_dsm_nut<<<s->pgrid, s->pblock, 0, s->st>>>(s->c, s->dsm_cs, s->smag, nut);
     LAUNCH_TRY(K_DSM_NUT);
@@ -358,7 +376,11 @@ extern "C" int cales_launches_per_step(cales_solver* s) {
   if (!s) return 0;
   const Ctx& c = s->c;
   int per = 1 /*rhs*/ + (c.implicit_z ? 4 : 0) + (c.const_flow_rate ? 2 : 0) + 5 /*solver*/ + 1 /*correct*/ + (c.wall_model ? 1 : 0) +
-            (c.sgs == CALES_SGS_DSMAG ? 3 : 1);
+            1 /*static nu_t or fill*/;
+  if (c.sgs == CALES_SGS_DSMAG) {
+    const bool ywall = c.bc_y == BC_WALL, split = ywall && c.ny >= 3 * DSM_TY;
+    per += -1 + (ywall ? 1 : 0) + ((!ywall || split) ? 1 : 0) + 2;   // pass 1 (tile and/or column kernel), coefficient, nu_t
+  }
   return 3 * per;
 }
 
@@ -486,6 +508,6 @@ extern "C" int cales_diagnostics(cales_solver* s, cales_diag* out) {
   out->ms_rhs = s->kms[K_RHS]; out->ms_implicit = s->kms[K_CN_COEF] + s->kms[K_CN_Z];
   out->ms_solver = s->kms[K_SUM] + s->kms[K_BULK] + s->kms[K_FFTX_FWD] + s->kms[K_FFTY_FWD] + s->kms[K_POISSON_Z] + s->kms[K_FFTY_INV] + s->kms[K_FFTX_INV];
   out->ms_correction = s->kms[K_CORRECT]; out->ms_wall = s->kms[K_WALL];
-  out->ms_sgs = s->kms[K_SMAG] + s->kms[K_DSM_PASS1] + s->kms[K_DSM_COEF] + s->kms[K_DSM_NUT] + s->kms[K_FILL];
+  out->ms_sgs = s->kms[K_SMAG] + s->kms[K_DSM_PASS1] + s->kms[K_DSM_COL] + s->kms[K_DSM_COEF] + s->kms[K_DSM_NUT] + s->kms[K_FILL];
   return CALES_OK;
 }

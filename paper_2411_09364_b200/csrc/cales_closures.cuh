@@ -254,6 +254,115 @@ CALES_HD void dsm_point(const Ctx& c, int i0, int j0, int k, int tx, int ty, con
   *lm = ll; *mm = m2; *smag_out = mid[dsm_mid_off(9, my, mx)];
 }
 
+// ------------------------------------------------------------------------------------------------------------
+// Dynamic Smagorinsky, pass 1, column-marching form (the production path; the tile kernel above serves the rows
+// next to y walls).  Where the test filter has uniform weights, F commutes with the (linear, x-y shift-invariant)
+// strain operator, so Eq. 9's strain of the filtered velocity equals the filtered strain, S~_ij = F(S_ij): the
+// kernel filters 21 centred quantities  q = (u_i^c [3], u_i^c u_j^c [6], |S| S_ij [6], S_ij [6])  and needs no
+// filtered face velocities.  A CTA is one row of TXB threads (TXB-2 output columns plus one halo column each side)
+// at a fixed k; it marches over LY+2 rows of y.  Per row: every thread evaluates the 10 base values
+// (u^c, v^c, w^c, S_ij, |S|) of its column, publishes them in shared memory, forms q and its x-filter from its two
+// neighbours' base values, and keeps the separable y-filter as a sliding window in registers:
+//   xq(r) = Fx q(r);   s(r) = xq(r-1) + xq(r);   F q(r-1) = (s(r-1) + s(r)) / 4.
+// ------------------------------------------------------------------------------------------------------------
+enum { DSMC_LY = 32, DSMC_NB = 10, DSMC_NQ = 21 };
+
+struct DsmColState {       // per-thread registers carried from row to row
+  double xq_prev[DSMC_NQ]; // Fx q of the previous row
+  double s_prev[DSMC_NQ];  // pair sum of the two rows before
+  double smag_prev;        // |S| of the previous row (this column)
+};
+
+// base values of column gi at row gj (both already wrapped / interior): b[0..2] = u^c, v^c, w^c; b[3..8] = S_ij; b[9] = |S|
+CALES_HD void dsmc_base(const Ctx& c, const double* __restrict__ u, const double* __restrict__ v, const double* __restrict__ w,
+                        int gi, int gj, int k, double* b) {
+  double S[6];
+  if (interior_row(c, gj, k)) {
+    const long long n = idx3(c, gi, gj, k);
+    const Nbr o = neighbours(c, gi, gj, k);
+    auto at = [&](const double* __restrict__ q, int a, int bb, int d) {
+      return q[n + (d < 0 ? o.km : (d > 0 ? o.kp : 0)) + ((a < 0 ? o.im : (a > 0 ? o.ip : 0)) + (bb < 0 ? o.jm : (bb > 0 ? o.jp : 0)))];
+    };
+    auto U = [&](int a, int bb, int d) { return at(u, a, bb, d); };
+    auto V = [&](int a, int bb, int d) { return at(v, a, bb, d); };
+    auto W = [&](int a, int bb, int d) { return at(w, a, bb, d); };
+    b[9] = strain_at(U, V, W, c.rdx, c.rdy, c.rdzf[k], c.rdzc[k], c.rdzc[k - 1], S);
+    b[0] = 0.5 * (U(-1, 0, 0) + U(0, 0, 0)); b[1] = 0.5 * (V(0, -1, 0) + V(0, 0, 0)); b[2] = 0.5 * (W(0, 0, -1) + W(0, 0, 0));
+  } else {
+    auto U = [&](int a, int bb, int d) { return velg<0>(c, u, gi + a, gj + bb, k + d, GH_STRAIN); };
+    auto V = [&](int a, int bb, int d) { return velg<1>(c, v, gi + a, gj + bb, k + d, GH_STRAIN); };
+    auto W = [&](int a, int bb, int d) { return velg<2>(c, w, gi + a, gj + bb, k + d, GH_STRAIN); };
+    b[9] = strain_at(U, V, W, c.rdx, c.rdy, c.rdzf[k], c.rdzc[k], c.rdzc[k - 1], S);
+    b[0] = 0.5 * (U(-1, 0, 0) + U(0, 0, 0)); b[1] = 0.5 * (V(0, -1, 0) + V(0, 0, 0)); b[2] = 0.5 * (W(0, 0, -1) + W(0, 0, 0));
+  }
+#pragma unroll
+  for (int q = 0; q < 6; ++q) b[3 + q] = S[q];
+}
+
+// q (21 values) from the base values
+CALES_HD void dsmc_q(const double* b, double* q) {
+  q[0] = b[0]; q[1] = b[1]; q[2] = b[2];
+  q[3] = b[0] * b[0]; q[4] = b[1] * b[1]; q[5] = b[2] * b[2]; q[6] = b[0] * b[1]; q[7] = b[0] * b[2]; q[8] = b[1] * b[2];
+#pragma unroll
+  for (int m = 0; m < 6; ++m) { q[9 + m] = b[9] * b[3 + m]; q[15 + m] = b[3 + m]; }
+}
+
+// Lilly contraction at one point from F q: returns L:M and M:M (Eq. 6-8, S2)
+CALES_HD void dsmc_contract(const double* Fq, double d2, double alpha, double* lm, double* mm) {
+  double L[6];
+  L[0] = Fq[3] - Fq[0] * Fq[0]; L[1] = Fq[4] - Fq[1] * Fq[1]; L[2] = Fq[5] - Fq[2] * Fq[2];
+  L[3] = Fq[6] - Fq[0] * Fq[1]; L[4] = Fq[7] - Fq[0] * Fq[2]; L[5] = Fq[8] - Fq[1] * Fq[2];
+  const double* St = Fq + 15;
+  const double stmag = sqrt(2.0 * (St[0] * St[0] + St[1] * St[1] + St[2] * St[2]) + 4.0 * (St[3] * St[3] + St[4] * St[4] + St[5] * St[5]));
+  const double a2s = alpha * alpha * stmag;
+  double ll = 0.0, m2 = 0.0;
+#pragma unroll
+  for (int m = 0; m < 6; ++m) {
+    const double M = 2.0 * d2 * (Fq[9 + m] - a2s * St[m]);
+    const double f = m < 3 ? 1.0 : 2.0;
+    ll += f * L[m] * M; m2 += f * M * M;
+  }
+  *lm = ll; *mm = m2;
+}
+
+// Row r of the march for thread t.  Phase A: base values of (column t, row r) into sh[buf][.][t] and regs `b`.
+// The global row is gj = wrap(j0 - 1 + r).
+CALES_HD void dsmc_phaseA(const Ctx& c, const double* u, const double* v, const double* w, int txb, int t, int i0, int gj, int k,
+                          double* shbuf /* [DSMC_NB][txb] */, double* b) {
+  const int gi = ((i0 - 1 + t) % c.nx + c.nx) % c.nx;
+  dsmc_base(c, u, v, w, gi, gj, k, b);
+#pragma unroll
+  for (int q = 0; q < DSMC_NB; ++q) shbuf[q * txb + t] = b[q];
+}
+
+// Phase B (threads 1..txb-2): x-filter of q, y-window update.  When r >= 2 the filtered row r-1 is complete:
+// returns true and sets *lm, *mm, *smag (of row r-1, this column).
+CALES_HD bool dsmc_phaseB(const Ctx& c, int txb, int t, int r, int k, const double* shbuf, const double* b, DsmColState& st,
+                          double* lm, double* mm, double* smag) {
+  double bl[DSMC_NB], br[DSMC_NB];
+#pragma unroll
+  for (int q = 0; q < DSMC_NB; ++q) { bl[q] = shbuf[q * txb + t - 1]; br[q] = shbuf[q * txb + t + 1]; }
+  double qc[DSMC_NQ], ql[DSMC_NQ], qr[DSMC_NQ];
+  dsmc_q(b, qc); dsmc_q(bl, ql); dsmc_q(br, qr);
+  bool done = false;
+  double Fq[DSMC_NQ];
+#pragma unroll
+  for (int m = 0; m < DSMC_NQ; ++m) {
+    const double xq = 0.25 * (ql[m] + qr[m]) + 0.5 * qc[m];
+    const double s = st.xq_prev[m] + xq;
+    Fq[m] = 0.25 * (st.s_prev[m] + s);
+    st.xq_prev[m] = xq; st.s_prev[m] = s;
+  }
+  if (r >= 2) {
+    const double d2 = c.delta[k] * c.delta[k];
+    dsmc_contract(Fq, d2, c.alpha, lm, mm);
+    *smag = st.smag_prev;
+    done = true;
+  }
+  st.smag_prev = b[9];
+  return done;
+}
+
 // Eq. 6 per row (j,k) from the x-tile partials, then per plane if requested; S13: <MM> = 0 -> c_s = 0.
 // part: [k][j][ntx][2].  cs: [k] or [k][j].
 CALES_HD void dsm_row_sums(const double* part, int ntx, long long row, double* ll, double* mm) {
@@ -289,31 +398,76 @@ __global__ void k_fill(double* __restrict__ q, long long n, double val) {
   for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (long long)gridDim.x * blockDim.x) q[t] = val;
 }
 // grid (ntx, nty, nz), block (32, 8)
+// rows: blockIdx.y -> j0 = jtile0 + blockIdx.y * jstride (wall-row tiles of the duct: jtile0 = 0, jstride = ny - DSM_TY);
+// only output rows with row_lo <= j < row_hi || j >= row_hi2 are written (the rest belongs to k_dsm_col).
 __global__ void __launch_bounds__(256) k_dsm_pass1(Ctx c, const double* __restrict__ u, const double* __restrict__ v, const double* __restrict__ w,
+                                                   int jstride, int row_hi, int row_lo2, int pslots,
                                                    double* __restrict__ smag, double* __restrict__ part) {
   extern __shared__ double dsm_sm[];
   double* raw = dsm_sm; double* flt = raw + DSM_RAW; double* mid = flt + DSM_FLT;
   const int tid = threadIdx.x + DSM_TX * threadIdx.y, nth = DSM_TX * DSM_TY;
-  const int i0 = blockIdx.x * DSM_TX, j0 = blockIdx.y * DSM_TY, k = blockIdx.z;
+  const int i0 = blockIdx.x * DSM_TX, j0 = blockIdx.y * jstride, k = blockIdx.z;
   dsm_load(tid, nth, c, u, v, w, i0, j0, k, raw);
   __syncthreads();
   dsm_mid(tid, nth, c, i0, j0, k, raw, flt, mid);
   __syncthreads();
   const int i = i0 + threadIdx.x, j = j0 + threadIdx.y;
   double lm = 0.0, mm = 0.0;
-  if (i < c.nx && j < c.ny) {
+  const bool mine = j < c.ny && (j < row_hi || j >= row_lo2);      // warp-uniform (one row per warp)
+  if (i < c.nx && mine) {
     double sm;
     dsm_point(c, i0, j0, k, threadIdx.x, threadIdx.y, flt, mid, &lm, &mm, &sm);
     smag[idx3(c, i, j, k)] = sm;
   }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) { lm += __shfl_down_sync(0xffffffffu, lm, o); mm += __shfl_down_sync(0xffffffffu, mm, o); }
-  if (threadIdx.x == 0 && j < c.ny) {
+  if (threadIdx.x == 0 && mine) {
     const long long row = (long long)k * c.ny + j;
-    part[(row * gridDim.x + blockIdx.x) * 2] = lm;
-    part[(row * gridDim.x + blockIdx.x) * 2 + 1] = mm;
+    part[(row * pslots + blockIdx.x) * 2] = lm;
+    part[(row * pslots + blockIdx.x) * 2 + 1] = mm;
   }
 }
+// Column-marching pass 1.  grid (ceil(nx/(TXB-2)), ceil((jhi-jlo)/DSMC_LY), nz), block TXB (multiple of 32).
+// Handles output rows [jlo, jhi); part: [k][j][pslots][2], this kernel fills slots blockIdx.x*nwarps + warp.
+template <int TXB>
+__global__ void __launch_bounds__(TXB) k_dsm_col(const __grid_constant__ Ctx c, const double* __restrict__ u, const double* __restrict__ v,
+                                                 const double* __restrict__ w, int jlo, int jhi, int pslots, double* __restrict__ smag,
+                                                 double* __restrict__ part) {
+  __shared__ double sh[2][DSMC_NB * TXB];
+  const int t = threadIdx.x, k = blockIdx.z;
+  const int i0 = blockIdx.x * (TXB - 2);
+  const int j0 = jlo + blockIdx.y * DSMC_LY;
+  const int jend = min(j0 + DSMC_LY, jhi);
+  const int nrows = jend - j0 + 2;
+  const int gi = i0 - 1 + t;                       // this thread's column (outputs: 1 <= t <= TXB-2, gi < nx)
+  const bool outcol = t >= 1 && t <= TXB - 2 && gi < c.nx;
+  DsmColState st;
+#pragma unroll
+  for (int m = 0; m < DSMC_NQ; ++m) { st.xq_prev[m] = 0.0; st.s_prev[m] = 0.0; }
+  st.smag_prev = 0.0;
+  for (int r = 0; r < nrows; ++r) {
+    int gj = j0 - 1 + r;
+    gj = gj < 0 ? gj + c.ny : (gj >= c.ny ? gj - c.ny : gj);
+    double b[DSMC_NB];
+    dsmc_phaseA(c, u, v, w, TXB, t, i0, gj, k, sh[r & 1], b);
+    __syncthreads();
+    double lm = 0.0, mm = 0.0, sm = 0.0;
+    bool done = false;
+    if (t >= 1 && t <= TXB - 2) done = dsmc_phaseB(c, TXB, t, r, k, sh[r & 1], b, st, &lm, &mm, &sm);
+    if (r >= 2) {      // block-uniform
+      const int jo = j0 + r - 2;
+      if (!(done && outcol)) { lm = 0.0; mm = 0.0; }
+      else smag[idx3(c, gi, jo, k)] = sm;
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) { lm += __shfl_down_sync(0xffffffffu, lm, o); mm += __shfl_down_sync(0xffffffffu, mm, o); }
+      if ((t & 31) == 0) {
+        const long long slot = ((long long)k * c.ny + jo) * pslots + blockIdx.x * (TXB / 32) + (t >> 5);
+        part[slot * 2] = lm; part[slot * 2 + 1] = mm;
+      }
+    }
+  }
+}
+
 // grid nz, block 128
 __global__ void k_dsm_coef(Ctx c, const double* __restrict__ part, int ntx, double* __restrict__ cs) {
   __shared__ double sh[32];

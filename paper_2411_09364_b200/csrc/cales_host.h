@@ -50,6 +50,22 @@ static inline void make_plan(FftPlan& pl, int n) {
   while (m % 3 == 0) { pl.radix[pl.npass++] = 3; m /= 3; }
 }
 
+// Launch shape of the dynamic-model pass 1: block width TXB of k_dsm_col (64, 96 or 128: least padded columns),
+// its number of x blocks, and the number of partial-sum slots per (k, j) row shared with the tile kernel.
+struct DsmShape { int txb, nbx, pslots; };
+static inline DsmShape dsm_shape(int nx) {
+  DsmShape d{64, 0, 0};
+  long long best = -1;
+  for (int t : {64, 96, 128}) {
+    const long long cost = (long long)((nx + t - 3) / (t - 2)) * t;
+    if (best < 0 || cost < best) { best = cost; d.txb = t; }
+  }
+  d.nbx = (nx + d.txb - 3) / (d.txb - 2);
+  const int tile_slots = (nx + DSM_TX - 1) / DSM_TX, col_slots = d.nbx * (d.txb / 32);
+  d.pslots = tile_slots > col_slots ? tile_slots : col_slots;
+  return d;
+}
+
 struct HostSetup {
   cales_params P;                 // with the defaults filled in
   std::vector<double> dzf, dzc, rdzf, rdzc, delta, zc, ak, ck, lamx, lamy, twx, twy, dctw;   // dzf: index k+1 holds dzf[k], k=-1..nz; dzc: k+1 holds dzc[k], k=-1..nz-1

@@ -40,8 +40,7 @@ extern "C" int emu_create(const cales_params* p, emu_solver** out) {
   for (auto* f : {&s->u, &s->v, &s->w, &s->p, &s->nut, &s->us, &s->vs, &s->ws, &s->Ru, &s->Rv, &s->Rw, &s->W, &s->CP, &s->CQ, &s->smag}) f->assign(N, 0.0);
   s->tau.assign(4 * (size_t)s->nxy, 0.0);
   s->cncoef.assign(6 * (size_t)p->nz, 0.0);
-  const size_t ntx = (p->nx + DSM_TX - 1) / DSM_TX;
-  s->dsm_part.assign((size_t)p->nz * p->ny * ntx * 2, 0.0);
+  s->dsm_part.assign((size_t)p->nz * p->ny * dsm_shape(p->nx).pslots * 2, 0.0);
   s->dsm_cs.assign((size_t)p->nz * p->ny, 0.0);
   s->c.dzf = H.dzf.data() + 1; s->c.dzc = H.dzc.data() + 1; s->c.zc = H.zc.data(); s->c.rdzf = H.rdzf.data() + 1; s->c.rdzc = H.rdzc.data() + 1; s->c.delta = H.delta.data(); s->c.tau = s->tau.data();
   s->plx = H.plx; s->plx.tw = reinterpret_cast<const double2*>(H.twx.data());
@@ -146,26 +145,60 @@ static void emu_nut(emu_solver* s, const double* u, const double* v, const doubl
     for (int k = 0; k < c.nz; ++k) for (int j = 0; j < c.ny; ++j) for (int i = 0; i < c.nx; ++i) nut[idx3(c, i, j, k)] = smag_point(c, u, v, w, i, j, k);
     return;
   }
-  const int ntx = (c.nx + DSM_TX - 1) / DSM_TX, nty = (c.ny + DSM_TY - 1) / DSM_TY, nth = DSM_TX * DSM_TY;
-  std::vector<double> sm(DSM_SMEM_DOUBLES);
-  double* raw = sm.data(); double* flt = raw + DSM_RAW; double* mid = flt + DSM_FLT;
-  for (int k = 0; k < c.nz; ++k) for (int by = 0; by < nty; ++by) for (int bx = 0; bx < ntx; ++bx) {
-    const int i0 = bx * DSM_TX, j0 = by * DSM_TY;
-    for (int tid = 0; tid < nth; ++tid) dsm_load(tid, nth, c, u, v, w, i0, j0, k, raw);
-    for (int tid = 0; tid < nth; ++tid) dsm_mid(tid, nth, c, i0, j0, k, raw, flt, mid);
-    for (int ty = 0; ty < DSM_TY; ++ty) {
-      double lm = 0.0, mm = 0.0;
-      for (int tx = 0; tx < DSM_TX; ++tx) {
-        const int i = i0 + tx, j = j0 + ty;
-        if (i < c.nx && j < c.ny) {
-          double a, b, sg;
-          dsm_point(c, i0, j0, k, tx, ty, flt, mid, &a, &b, &sg);
-          s->smag[idx3(c, i, j, k)] = sg; lm += a; mm += b;
+  const DsmShape dsh = dsm_shape(c.nx);
+  const int ntx = dsh.pslots;
+  const bool ywall = c.bc_y == BC_WALL, split = ywall && c.ny >= 3 * DSM_TY;
+  std::fill(s->dsm_part.begin(), s->dsm_part.end(), 0.0);
+  if (ywall) {   // tile kernel: all rows, or the DSM_TY rows next to each y wall
+    const int ntile = (c.nx + DSM_TX - 1) / DSM_TX, nth = DSM_TX * DSM_TY;
+    const int nby = split ? 2 : (c.ny + DSM_TY - 1) / DSM_TY, jstride = split ? c.ny - DSM_TY : DSM_TY;
+    const int row_hi = split ? DSM_TY : c.ny, row_lo2 = split ? c.ny - DSM_TY : c.ny;
+    std::vector<double> sm(DSM_SMEM_DOUBLES);
+    double* raw = sm.data(); double* flt = raw + DSM_RAW; double* mid = flt + DSM_FLT;
+    for (int k = 0; k < c.nz; ++k) for (int by = 0; by < nby; ++by) for (int bx = 0; bx < ntile; ++bx) {
+      const int i0 = bx * DSM_TX, j0 = by * jstride;
+      for (int tid = 0; tid < nth; ++tid) dsm_load(tid, nth, c, u, v, w, i0, j0, k, raw);
+      for (int tid = 0; tid < nth; ++tid) dsm_mid(tid, nth, c, i0, j0, k, raw, flt, mid);
+      for (int ty = 0; ty < DSM_TY; ++ty) {
+        const int j = j0 + ty;
+        const bool mine = j < c.ny && (j < row_hi || j >= row_lo2);
+        if (!mine) continue;
+        double lm = 0.0, mm = 0.0;
+        for (int tx = 0; tx < DSM_TX; ++tx) {
+          const int i = i0 + tx;
+          if (i < c.nx) {
+            double a, b, sg;
+            dsm_point(c, i0, j0, k, tx, ty, flt, mid, &a, &b, &sg);
+            s->smag[idx3(c, i, j, k)] = sg; lm += a; mm += b;
+          }
         }
-      }
-      if (j0 + ty < c.ny) {
-        const long long row = (long long)k * c.ny + j0 + ty;
+        const long long row = (long long)k * c.ny + j;
         s->dsm_part[(row * ntx + bx) * 2] = lm; s->dsm_part[(row * ntx + bx) * 2 + 1] = mm;
+      }
+    }
+  }
+  if (!ywall || split) {   // column-marching kernel, stepped row by row with the block barrier between the phases
+    const int T = dsh.txb, jlo = ywall ? DSM_TY : 0, jhi = ywall ? c.ny - DSM_TY : c.ny;
+    std::vector<double> sh(2 * DSMC_NB * T), breg((size_t)T * DSMC_NB);
+    std::vector<DsmColState> st(T);
+    for (int k = 0; k < c.nz; ++k) for (int by = 0; by * DSMC_LY < jhi - jlo; ++by) for (int bx = 0; bx < dsh.nbx; ++bx) {
+      const int i0 = bx * (T - 2), j0 = jlo + by * DSMC_LY, jend = std::min(j0 + DSMC_LY, jhi), nrows = jend - j0 + 2;
+      for (auto& q : st) { for (int m = 0; m < DSMC_NQ; ++m) { q.xq_prev[m] = 0.0; q.s_prev[m] = 0.0; } q.smag_prev = 0.0; }
+      for (int r = 0; r < nrows; ++r) {
+        int gj = j0 - 1 + r; gj = gj < 0 ? gj + c.ny : (gj >= c.ny ? gj - c.ny : gj);
+        double* buf = sh.data() + (r & 1) * DSMC_NB * T;
+        for (int t = 0; t < T; ++t) dsmc_phaseA(c, u, v, w, T, t, i0, gj, k, buf, &breg[(size_t)t * DSMC_NB]);
+        std::vector<double> wl(T / 32, 0.0), wm(T / 32, 0.0);
+        for (int t = 1; t <= T - 2; ++t) {
+          double lm = 0.0, mm = 0.0, sg = 0.0;
+          const bool done = dsmc_phaseB(c, T, t, r, k, buf, &breg[(size_t)t * DSMC_NB], st[t], &lm, &mm, &sg);
+          const int gi = i0 - 1 + t;
+          if (r >= 2 && done && gi < c.nx) { s->smag[idx3(c, gi, j0 + r - 2, k)] = sg; wl[t >> 5] += lm; wm[t >> 5] += mm; }
+        }
+        if (r >= 2) for (int wq = 0; wq < T / 32; ++wq) {
+          const long long slot = ((long long)k * c.ny + (j0 + r - 2)) * ntx + bx * (T / 32) + wq;
+          s->dsm_part[slot * 2] = wl[wq]; s->dsm_part[slot * 2 + 1] = wm[wq];
+        }
       }
     }
   }

@@ -14,8 +14,11 @@ SMALL = {
     "cfg1_dit": (1, (24, 16, 12), 2),
     "cfg2_wmles": (2, (48, 24, 16), 2),
     "cfg3_wrles_cn": (3, (36, 24, 20), 2),
-    "cfg4_duct_dsm": (4, (48, 18, 16), 2),
+    "cfg4_duct_dsm": (4, (48, 36, 16), 2),            # ny >= 24: wall-row tiles + column-marching kernel
+    "cfg4_duct_dsm_narrow": (4, (48, 18, 16), 1),     # ny < 24: tile kernel on every row
     "cfg5_wmles_dsm": (5, (36, 24, 16), 2),
+    "duct_static_smag": (4, (24, 12, 12), 2, dict(sgs_model=1, cs=0.1)),   # static model next to y walls
+    "cfg5_hwm_interp": (5, (24, 12, 16), 2, dict(h_wm=0.1)),               # wall model sampled between centres
 }
 # the sizes the GPU parity tests use: several tiles in every direction plus ragged tails
 GPU_CASES = {
@@ -24,14 +27,18 @@ GPU_CASES = {
     "cfg3_wrles_cn": (3, (96, 72, 48), 3),
     "cfg4_duct_dsm": (4, (192, 54, 48), 3),
     "cfg5_wmles_dsm": (5, (192, 128, 64), 3),        # the replica SURVEY.md 8(d) names for config 5
+    "duct_static_smag": (4, (96, 36, 24), 2, dict(sgs_model=1, cs=0.1)),
+    "cfg5_hwm_interp": (5, (96, 48, 32), 2, dict(h_wm=0.1)),
+    "cfg4_duct_dsm_narrow": (4, (72, 18, 16), 2),
 }
 
 
-def prepare(oracle, n, shape):
+def prepare(oracle, n, shape, overrides=None):
     """(cfg, kwargs, (u, v, w), dt): seeded field, projected by the oracle, with its time step."""
     cfg = inputs.config(n, shape)
     u, v, w, ub = inputs.initial_fields(cfg)
     kw = inputs.solver_kwargs(cfg, ub)
+    kw.update(overrides or {})
     g = {k: kw[k] for k in ("nx", "ny", "nz", "lx", "ly", "lz")}
     o = oracle.Oracle(g["nx"], g["ny"], g["nz"], g["lx"], g["ly"], g["lz"],
                       **{k: v_ for k, v_ in kw.items() if k not in g})

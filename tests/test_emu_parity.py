@@ -17,8 +17,8 @@ def emu():
 
 @pytest.mark.parametrize("case", sorted(pc.SMALL))
 def test_emulated_kernels_match_oracle(oracle, emu, case):
-    n, shape, steps = pc.SMALL[case]
-    cfg, kw, (u, v, w), dt = pc.prepare(oracle, n, shape)
+    n, shape, steps = pc.SMALL[case][:3]
+    cfg, kw, (u, v, w), dt = pc.prepare(oracle, n, shape, *pc.SMALL[case][3:])
     o = pc.make(oracle.Oracle, kw)
     e = pc.make(emu.Emu, kw)
     o.set_velocity(u, v, w); e.set_velocity(u, v, w)

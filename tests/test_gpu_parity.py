@@ -30,8 +30,8 @@ def _gpu_fields(s):
 
 @pytest.mark.parametrize("case", sorted(pc.GPU_CASES))
 def test_step_parity(oracle, gpu, case):
-    n, shape, steps = pc.GPU_CASES[case]
-    cfg, kw, (u, v, w), dt = pc.prepare(oracle, n, shape)
+    n, shape, steps = pc.GPU_CASES[case][:3]
+    cfg, kw, (u, v, w), dt = pc.prepare(oracle, n, shape, *pc.GPU_CASES[case][3:])
     o = pc.make(oracle.Oracle, kw)
     g = pc.make(gpu.Solver, kw)
     o.set_velocity(u, v, w); g.set_velocity(u, v, w)
