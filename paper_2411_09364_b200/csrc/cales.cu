@@ -9,6 +9,7 @@
 #include "cales_fft.cuh"
 #include "cales_poisson.cuh"
 #include "cales_momentum.cuh"
+#include "cales_rhs_tile.cuh"
 #include "cales_closures.cuh"
 #include "cales_host.h"
 
@@ -175,6 +176,7 @@ extern "C" int cales_create(const cales_params* p, cales_solver** out) {
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fft_x_fwd<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fft_x_inv, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fft_y, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rhs_tile, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(RT_SMEM_DOUBLES * sizeof(double)));
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dsm_pass1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(DSM_SMEM_DOUBLES * sizeof(double)));
   if (e != cudaSuccess) { delete s; return fail(CALES_ECUDA, std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e)); }
   s->pblock = dim3(32, 8, 1);
@@ -329,9 +331,11 @@ static int substep(cales_solver* s, int rk, double dt) {
   a.u = s->u; a.v = s->v; a.w = s->w; a.p = s->p; a.nut = s->nut;
   a.Ru0 = s->Ru; a.Rv0 = s->Rv; a.Rw0 = s->Rw; a.Ru1 = s->Ru; a.Rv1 = s->Rv; a.Rw1 = s->Rw;
   a.us = s->us; a.vs = s->vs; a.ws = s->ws; a.dt = dt; a.al = al; a.be = be; a.ga = ga; a.store_R = rk < 2 ? 1 : 0;
-  k_rhs<<<s->pgrid, s->pblock, 0, s->st>>>(c, a, (cfr && !imp) ? s->partial : nullptr);
+  const int kz = rt_chunk(c.nx, c.ny, c.nz);
+  const dim3 rgrid((c.nx + RT_TX - 1) / RT_TX, (c.ny + RT_TY - 1) / RT_TY, (c.nz + kz - 1) / kz);
+  k_rhs_tile<<<rgrid, RT_THREADS, RT_SMEM_DOUBLES * sizeof(double), s->st>>>(c, a, kz, (cfr && !imp) ? s->partial : nullptr);
   LAUNCH_TRY(K_RHS);
-  long long npart = s->nblk;
+  long long npart = (long long)rgrid.x * rgrid.y * rgrid.z;
   if (imp) {
     const double cimp = 0.5 * ga * c.nu * dt;
     k_cn_coef<<<1, 32, 0, s->st>>>(c, cimp, s->cncoef);

@@ -1,0 +1,224 @@
+// cales_rhs_tile.cuh -- the production momentum kernel: fused right-hand side + RK3 update of Eq. 11 / Eq. 20
+// as a z-marching, shared-memory staged stencil.
+//
+// A CTA owns an RT_TX x RT_TY tile of (i,j) columns and marches over a chunk of k-planes.  Each plane of
+// u, v, w, nu_t, p (tile + halo 1) is staged ONCE into a 4-slot shared-memory ring by asynchronous copies
+// (cp.async, LDGSTS) issued one plane ahead of the arithmetic, so every global value is fetched once per CTA, the
+// copy of plane k+2 overlaps the arithmetic of plane k, and all 50-odd stencil reads of a point are shared-memory
+// reads.  Boundary conditions (Alg. 2) are applied WHEN A HALO ELEMENT IS STAGED: periodic wrap
+// is address arithmetic of the async copy; wall ghosts (no-slip mirror, zero wall-normal face, Neumann p, nu_t = -
+// interior, wall-model stress ghost) are produced by the generic accessors velg / scalg and stored synchronously.
+// The arithmetic itself (rhs_core) is written once over an accessor and is shared with the host emulator.
+#pragma once
+#include "cales_common.cuh"
+#include "cales_momentum.cuh"
+
+namespace cales {
+
+enum { RT_TX = 32, RT_TY = 16, RT_RPT = 2, RT_TW = RT_TX + 2, RT_TH = RT_TY + 2, RT_PLANE = RT_TW * RT_TH, RT_NF = 5, RT_NSLOT = 4,
+       RT_THREADS = RT_TX * RT_TY / RT_RPT, RT_SMEM_DOUBLES = RT_NSLOT * RT_NF * RT_PLANE,
+       RT_EPT = (RT_PLANE + RT_THREADS - 1) / RT_THREADS };   // halo-tile positions per thread
+
+// Momentum right-hand side and RK update at one point over an accessor A with
+//   A.U(di,dj,dk), A.V, A.W : velocity components incl. ghosts (viscous-flux ghost at wall-model walls),
+//   A.NT(di,dj,dk)          : nu_t incl. ghosts,   A.P(di,dj,dk): pressure incl. ghosts.
+// Same discretisation as rhs_point (cales_momentum.cuh); the factors 1/2, 1/4 of the interpolations are folded into
+// the metric terms.  Returns u* at the point.
+template <class A>
+CALES_HD double rhs_core(const Ctx& c, const RhsArgs& a, const A& q, int i, int j, int k) {
+  const long long n = idx3(c, i, j, k);
+  const double rdx = c.rdx, rdy = c.rdy;
+  const double dzfk = c.dzf[k], dzfp = c.dzf[k + 1];
+  const double rdzf = c.rdzf[k], rdzfp = c.rdzf[k + 1], rdzc = c.rdzc[k], rdzcm = c.rdzc[k - 1];
+  const bool vact = !(c.bc_y == BC_WALL && j == c.ny - 1);
+  const bool wact = !(c.bc_z == BC_WALL && k == c.nz - 1);
+  const double u000 = q.U(0, 0, 0), up00 = q.U(1, 0, 0), um00 = q.U(-1, 0, 0), u0p0 = q.U(0, 1, 0), u0m0 = q.U(0, -1, 0),
+               ump0 = q.U(-1, 1, 0), u00p = q.U(0, 0, 1), u00m = q.U(0, 0, -1), um0p = q.U(-1, 0, 1);
+  const double v000 = q.V(0, 0, 0), vp00 = q.V(1, 0, 0), vm00 = q.V(-1, 0, 0), v0p0 = q.V(0, 1, 0), v0m0 = q.V(0, -1, 0),
+               vpm0 = q.V(1, -1, 0), v00p = q.V(0, 0, 1), v00m = q.V(0, 0, -1), v0mp = q.V(0, -1, 1);
+  const double w000 = q.W(0, 0, 0), wp00 = q.W(1, 0, 0), wm00 = q.W(-1, 0, 0), w0p0 = q.W(0, 1, 0), w0m0 = q.W(0, -1, 0),
+               w00p = q.W(0, 0, 1), w00m = q.W(0, 0, -1), wp0m = q.W(1, 0, -1), w0pm = q.W(0, 1, -1);
+  const double qx = 0.25 * rdx, qy = 0.25 * rdy, qzf = 0.25 * rdzf, qzc = 0.25 * rdzc;
+  double Ru, Rv, Rw;
+  {  // -d_j(u_i u_j), weights of DESIGN.md S3
+    const double uxp = u000 + up00, uxm = um00 + u000, uyp = u000 + u0p0, uym = u0m0 + u000;
+    const double vxp = v000 + vp00, vxm = v0m0 + vpm0, uzp = u000 + u00p, uzm = u00m + u000;
+    const double wxp = w000 + wp00, wxm = w00m + wp0m;
+    Ru = -((uxp * uxp - uxm * uxm) * qx + (uyp * vxp - uym * vxm) * qy + (uzp * wxp - uzm * wxm) * qzf);
+    const double vyp = v000 + v0p0, vym = v0m0 + v000, vxq = vm00 + v000, uym2 = um00 + ump0;
+    const double vzp = v000 + v00p, vzm = v00m + v000, wyp = w000 + w0p0, wym = w00m + w0pm;
+    Rv = -((vxp * uyp - vxq * uym2) * qx + (vyp * vyp - vym * vym) * qy + (vzp * wyp - vzm * wym) * qzf);
+    const double wzp = w000 + w00p, wzm = w00m + w000, wxq = wm00 + w000, wyq = w0m0 + w000;
+    const double uzP = u000 * dzfk + u00p * dzfp, uzM = um00 * dzfk + um0p * dzfp;
+    const double vzP = v000 * dzfk + v00p * dzfp, vzM = v0m0 * dzfk + v0mp * dzfp;
+    Rw = -(((wxp * uzP - wxq * uzM) * qx + (wyp * vzP - wyq * vzM) * qy) * rdzc + (wzp * wzp - wzm * wzm) * qzc);
+  }
+  const double rdx2 = rdx * rdx, rdy2 = rdy * rdy;
+  const double lzu = ((u00p - u000) * rdzc - (u000 - u00m) * rdzcm) * rdzf;
+  const double lzv = ((v00p - v000) * rdzc - (v000 - v00m) * rdzcm) * rdzf;
+  const double lzw = ((w00p - w000) * rdzfp - (w000 - w00m) * rdzf) * rdzc;
+  double du = (up00 - 2.0 * u000 + um00) * rdx2 + (u0p0 - 2.0 * u000 + u0m0) * rdy2;
+  double dv = (vp00 - 2.0 * v000 + vm00) * rdx2 + (v0p0 - 2.0 * v000 + v0m0) * rdy2;
+  double dw = (wp00 - 2.0 * w000 + wm00) * rdx2 + (w0p0 - 2.0 * w000 + w0m0) * rdy2;
+  if (!c.implicit_z) { du += lzu; dv += lzv; dw += lzw; }
+  Ru += c.nu * du; Rv += c.nu * dv; Rw += c.nu * dw;
+  if (c.sgs) {   // d_j(2 nu_t S_ij), edge viscosity = mean of the 4 surrounding centres (S6)
+    const double n000 = q.NT(0, 0, 0), np00 = q.NT(1, 0, 0), nm00 = q.NT(-1, 0, 0), n0p0 = q.NT(0, 1, 0), n0m0 = q.NT(0, -1, 0),
+                 n00p = q.NT(0, 0, 1), n00m = q.NT(0, 0, -1), npp0 = q.NT(1, 1, 0), npm0 = q.NT(1, -1, 0), nmp0 = q.NT(-1, 1, 0),
+                 np0p = q.NT(1, 0, 1), np0m = q.NT(1, 0, -1), nm0p = q.NT(-1, 0, 1), n0pp = q.NT(0, 1, 1), n0pm = q.NT(0, 1, -1),
+                 n0mp = q.NT(0, -1, 1);
+    const double nx0 = n000 + np00, ny0 = n000 + n0p0, nz0 = n000 + n00p;
+    const double exy_00 = (nx0 + n0p0 + npp0) * ((u0p0 - u000) * rdy + (vp00 - v000) * rdx);
+    const double exy_0m = (nx0 + n0m0 + npm0) * ((u000 - u0m0) * rdy + (vpm0 - v0m0) * rdx);
+    const double exy_m0 = (ny0 + nm00 + nmp0) * ((ump0 - um00) * rdy + (v000 - vm00) * rdx);
+    const double exz_00 = (nx0 + n00p + np0p) * ((u00p - u000) * rdzc + (wp00 - w000) * rdx);
+    const double exz_0m = (nx0 + n00m + np0m) * ((u000 - u00m) * rdzcm + (wp0m - w00m) * rdx);
+    const double exz_m0 = (nz0 + nm00 + nm0p) * ((um0p - um00) * rdzc + (w000 - wm00) * rdx);
+    const double eyz_00 = (ny0 + n00p + n0pp) * ((v00p - v000) * rdzc + (w0p0 - w000) * rdy);
+    const double eyz_0m = (ny0 + n00m + n0pm) * ((v000 - v00m) * rdzcm + (w0pm - w00m) * rdy);
+    const double eyz_m0 = (nz0 + n0m0 + n0mp) * ((v0mp - v0m0) * rdzc + (w000 - w0m0) * rdy);
+    Ru += (np00 * (up00 - u000) - n000 * (u000 - um00)) * (2.0 * rdx2) + (exy_00 - exy_0m) * qy + (exz_00 - exz_0m) * qzf;
+    Rv += (exy_00 - exy_m0) * qx + (n0p0 * (v0p0 - v000) - n000 * (v000 - v0m0)) * (2.0 * rdy2) + (eyz_00 - eyz_0m) * qzf;
+    Rw += (exz_00 - exz_m0) * qx + (eyz_00 - eyz_m0) * qy + (n00p * (w00p - w000) * rdzfp - n000 * (w000 - w00m) * rdzf) * (2.0 * rdzc);
+  }
+  const double p000 = q.P(0, 0, 0);
+  const double gpx = (q.P(1, 0, 0) - p000) * rdx, gpy = (q.P(0, 1, 0) - p000) * rdy, gpz = (q.P(0, 0, 1) - p000) * rdzc;
+  double ru0 = 0.0, rv0 = 0.0, rw0 = 0.0;
+  if (a.be != 0.0) { ru0 = a.Ru0[n]; rv0 = a.Rv0[n]; rw0 = a.Rw0[n]; }
+  if (!vact) Rv = 0.0;
+  if (!wact) Rw = 0.0;
+  double us = u000 + a.dt * (a.al * Ru + a.be * ru0 - a.ga * gpx);
+  double vs = v000 + a.dt * (a.al * Rv + a.be * rv0 - a.ga * gpy);
+  double ws = w000 + a.dt * (a.al * Rw + a.be * rw0 - a.ga * gpz);
+  if (c.implicit_z) {   // Eq. 20 explicit half + right-hand side of Eq. 21
+    const double f = a.dt * a.ga * c.nu - 0.5 * a.ga * c.nu * a.dt;
+    us += f * lzu; vs += f * lzv; ws += f * lzw;
+  }
+  if (!vact) vs = 0.0;
+  if (!wact) ws = 0.0;
+  a.us[n] = us; a.vs[n] = vs; a.ws[n] = ws;
+  if (a.store_R) { a.Ru1[n] = Ru; a.Rv1[n] = Rv; a.Rw1[n] = Rw; }
+  return us;
+}
+
+// Accessor over the generic boundary-condition accessors (any point, any boundary).
+struct GhostAcc {
+  const Ctx& c; const RhsArgs& a; int i, j, k;
+  CALES_HD double U(int di, int dj, int dk) const { return velg<0>(c, a.u, i + di, j + dj, k + dk, GH_VISC); }
+  CALES_HD double V(int di, int dj, int dk) const { return velg<1>(c, a.v, i + di, j + dj, k + dk, GH_VISC); }
+  CALES_HD double W(int di, int dj, int dk) const { return velg<2>(c, a.w, i + di, j + dj, k + dk, GH_VISC); }
+  CALES_HD double NT(int di, int dj, int dk) const { return scalg(c, a.nut, i + di, j + dj, k + dk, -1.0); }
+  CALES_HD double P(int di, int dj, int dk) const { return scalg(c, a.p, i + di, j + dj, k + dk, 1.0); }
+};
+
+// Value staged for field f (0 u, 1 v, 2 w, 3 nu_t, 4 p) at (gi,gj,gk), -1 <= gi <= nx, -1 <= gj <= ny, -1 <= gk <= nz.
+CALES_HD double rt_elem(const Ctx& c, const RhsArgs& a, int f, int gi, int gj, int gk) {
+  switch (f) {
+    case 0: return velg<0>(c, a.u, gi, gj, gk, GH_VISC);
+    case 1: return velg<1>(c, a.v, gi, gj, gk, GH_VISC);
+    case 2: return velg<2>(c, a.w, gi, gj, gk, GH_VISC);
+    case 3: return c.sgs ? scalg(c, a.nut, gi, gj, gk, -1.0) : 0.0;
+    default: return scalg(c, a.p, gi, gj, gk, 1.0);
+  }
+}
+
+// Accessor over three staged planes (k-1, k, k+1): sl[d] points at field 0 of the slot, ctr = (ly+1)*RT_TW + lx+1.
+struct TileAcc {
+  const double* sl[3]; int ctr;
+  CALES_HD double at(int f, int di, int dj, int dk) const { return sl[dk + 1][f * RT_PLANE + ctr + dj * RT_TW + di]; }
+  CALES_HD double U(int di, int dj, int dk) const { return at(0, di, dj, dk); }
+  CALES_HD double V(int di, int dj, int dk) const { return at(1, di, dj, dk); }
+  CALES_HD double W(int di, int dj, int dk) const { return at(2, di, dj, dk); }
+  CALES_HD double NT(int di, int dj, int dk) const { return at(3, di, dj, dk); }
+  CALES_HD double P(int di, int dj, int dk) const { return at(4, di, dj, dk); }
+};
+
+// k-planes per CTA: enough chunks for ~8 waves of 2 CTAs/SM on 148 SMs, at least 8 planes per chunk
+static inline int rt_chunk(int nx, int ny, int nz) {
+  const long long tiles = (long long)((nx + RT_TX - 1) / RT_TX) * ((ny + RT_TY - 1) / RT_TY);
+  long long want = (8 * 296 + tiles - 1) / tiles;
+  const long long maxc = nz / 8 > 0 ? nz / 8 : 1;
+  if (want > maxc) want = maxc;
+  if (want < 1) want = 1;
+  return (int)((nz + want - 1) / want);
+}
+
+#ifdef __CUDACC__
+__device__ __forceinline__ void cp_async8(double* smem_dst, const double* gsrc) {
+  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(d), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;\n" ::: "memory"); }
+
+// grid (ceil(nx/RT_TX), ceil(ny/RT_TY), ceil(nz/kz)), block RT_THREADS, dynamic smem RT_SMEM_DOUBLES*8.
+// partial[linear block id] = sum over the CTA's points of u* dzf[k] (or nullptr).
+__global__ void __launch_bounds__(RT_THREADS, 2) k_rhs_tile(const __grid_constant__ Ctx c, const __grid_constant__ RhsArgs a, int kz,
+                                                            double* __restrict__ partial) {
+  extern __shared__ double rt_sm[];
+  __shared__ double red[32];
+  const int tid = threadIdx.x, tx = tid & 31, ty = tid >> 5;
+  const int i0 = blockIdx.x * RT_TX, j0 = blockIdx.y * RT_TY, k0 = blockIdx.z * kz, k1 = min(k0 + kz, c.nz);
+  // ---- this thread's halo-tile positions (the same for every plane and field)
+  int goff[RT_EPT], soff[RT_EPT];      // in-plane global offset (>= 0: async copy; -1: unused; -2: y ghost, generic path)
+#pragma unroll
+  for (int e = 0; e < RT_EPT; ++e) {
+    const int pos = tid + e * RT_THREADS;
+    soff[e] = pos; goff[e] = -1;
+    if (pos < RT_PLANE) {
+      const int ry = pos / RT_TW, rx = pos - ry * RT_TW;
+      int gi = i0 - 1 + rx, gj = j0 - 1 + ry;
+      if (gi <= c.nx && gj <= c.ny) {
+        gi = gi < 0 ? c.nx - 1 : (gi == c.nx ? 0 : gi);
+        if (c.bc_y == BC_PER) { gj = gj < 0 ? c.ny - 1 : (gj == c.ny ? 0 : gj); goff[e] = gj * c.nx + gi; }
+        else goff[e] = (gj < 0 || gj >= c.ny) ? -2 : gj * c.nx + gi;
+      }
+    }
+  }
+  const double* fld[RT_NF] = {a.u, a.v, a.w, a.nut, a.p};
+  auto issue = [&](int kk) {
+    double* slot = rt_sm + ((kk + 4) & 3) * (RT_NF * RT_PLANE);
+    const bool zreg = c.bc_z == BC_PER || (kk >= 0 && kk < c.nz);
+    const long long kw = (long long)(kk < 0 ? kk + c.nz : (kk >= c.nz ? kk - c.nz : kk)) * c.nxy;
+#pragma unroll
+    for (int e = 0; e < RT_EPT; ++e) {
+      if (goff[e] == -1) continue;
+      if (zreg && goff[e] >= 0) {
+#pragma unroll
+        for (int f = 0; f < RT_NF; ++f) if (f != 3 || c.sgs) cp_async8(slot + f * RT_PLANE + soff[e], fld[f] + kw + goff[e]);
+      } else {
+        const int ry = soff[e] / RT_TW, rx = soff[e] - ry * RT_TW;
+#pragma unroll
+        for (int f = 0; f < RT_NF; ++f) slot[f * RT_PLANE + soff[e]] = rt_elem(c, a, f, i0 - 1 + rx, j0 - 1 + ry, kk);
+      }
+    }
+  };
+  issue(k0 - 1); issue(k0);
+  if (k0 + 1 <= k1) issue(k0 + 1);
+  cp_async_commit();
+  double acc = 0.0;
+  for (int k = k0; k < k1; ++k) {
+    cp_async_wait_all();
+    __syncthreads();
+    if (k + 2 <= k1) issue(k + 2);
+    cp_async_commit();
+    TileAcc q;
+    q.sl[0] = rt_sm + ((k + 3) & 3) * (RT_NF * RT_PLANE); q.sl[1] = rt_sm + (k & 3) * (RT_NF * RT_PLANE); q.sl[2] = rt_sm + ((k + 1) & 3) * (RT_NF * RT_PLANE);
+    const double dz = c.dzf[k];
+#pragma unroll
+    for (int r = 0; r < RT_RPT; ++r) {
+      const int ly = ty + r * (RT_TY / RT_RPT), i = i0 + tx, j = j0 + ly;
+      if (i < c.nx && j < c.ny) {
+        q.ctr = (ly + 1) * RT_TW + tx + 1;
+        acc += rhs_core(c, a, q, i, j, k) * dz;
+      }
+    }
+  }
+  if (partial) {
+    const double t = block_sum(acc, red);
+    if (tid == 0) partial[blockIdx.x + gridDim.x * (blockIdx.y + (long long)gridDim.y * blockIdx.z)] = t;
+  }
+}
+#endif
+
+}  // namespace cales

@@ -10,6 +10,7 @@
 #include "../../paper_2411_09364_b200/csrc/cales_host.h"
 #include "../../paper_2411_09364_b200/csrc/cales_poisson.cuh"
 #include "../../paper_2411_09364_b200/csrc/cales_momentum.cuh"
+#include "../../paper_2411_09364_b200/csrc/cales_rhs_tile.cuh"
 
 #include <cstring>
 #include <vector>
@@ -229,7 +230,21 @@ static void emu_substep(emu_solver* s, int rk, double dt) {
   a.Ru0 = s->Ru.data(); a.Rv0 = s->Rv.data(); a.Rw0 = s->Rw.data(); a.Ru1 = s->Ru.data(); a.Rv1 = s->Rv.data(); a.Rw1 = s->Rw.data();
   a.us = s->us.data(); a.vs = s->vs.data(); a.ws = s->ws.data(); a.dt = dt; a.al = al; a.be = be; a.ga = ga; a.store_R = rk < 2 ? 1 : 0;
   double sum = 0.0;
-  for (int k = 0; k < c.nz; ++k) for (int j = 0; j < c.ny; ++j) for (int i = 0; i < c.nx; ++i) sum += rhs_any(c, a, i, j, k) * c.dzf[k];
+  {  // k_rhs_tile: per CTA tile and plane, stage the three halo planes with the staging rule of the kernel (rt_elem), then
+     // evaluate rhs_core through the shared-memory accessor
+    std::vector<double> ring(3 * RT_NF * RT_PLANE);
+    for (int j0 = 0; j0 < c.ny; j0 += RT_TY) for (int i0 = 0; i0 < c.nx; i0 += RT_TX) for (int k = 0; k < c.nz; ++k) {
+      for (int d = 0; d < 3; ++d) for (int f = 0; f < RT_NF; ++f) for (int pos = 0; pos < RT_PLANE; ++pos) {
+        const int ry = pos / RT_TW, rx = pos % RT_TW, gi = i0 - 1 + rx, gj = j0 - 1 + ry;
+        ring[(d * RT_NF + f) * RT_PLANE + pos] = (gi <= c.nx && gj <= c.ny) ? rt_elem(c, a, f, gi, gj, k - 1 + d) : 0.0;
+      }
+      TileAcc q; for (int d = 0; d < 3; ++d) q.sl[d] = ring.data() + d * RT_NF * RT_PLANE;
+      for (int ly = 0; ly < RT_TY; ++ly) for (int tx = 0; tx < RT_TX; ++tx) {
+        const int i = i0 + tx, j = j0 + ly;
+        if (i < c.nx && j < c.ny) { q.ctr = (ly + 1) * RT_TW + tx + 1; sum += rhs_core(c, a, q, i, j, k) * c.dzf[k]; }
+      }
+    }
+  }
   if (imp) {
     const double cimp = 0.5 * ga * c.nu * dt;
     cn_coefficients(c, cimp, s->cncoef.data());
