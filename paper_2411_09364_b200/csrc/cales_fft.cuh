@@ -32,12 +32,81 @@ CALES_HD double2 cmulc(double2 a, double2 b) { return make_double2(a.x * b.x + a
 CALES_HD double2 cadd(double2 a, double2 b) { return make_double2(a.x + b.x, a.y + b.y); }
 CALES_HD double2 csub(double2 a, double2 b) { return make_double2(a.x - b.x, a.y - b.y); }
 
-// Shared-memory view of B lines of n2 complex numbers: element (b, t) at a[b*ls + t*es].
+// Shared-memory view of B lines of n2 complex numbers.  x layout (bfast = false): line b is contiguous with one padding
+// slot per 8 elements (element t at b*ls + t + t/8), which makes the stride-R writes of the first Stockham passes
+// bank-conflict free for R <= 8; y layout (bfast = true): element (b, t) at t*es + b, consecutive threads on consecutive b.
 struct SmView { int es, ls, B; bool bfast; };
-CALES_HD int sm_off(const SmView& v, int b, int t) { return b * v.ls + t * v.es; }
+CALES_HD int sm_pad(int t) { return t + (t >> 3); }
+CALES_HD int sm_off(const SmView& v, int b, int t) { return v.bfast ? b * v.ls + t * v.es : b * v.ls + sm_pad(t); }
+CALES_HD int sm_line(int n2) { return sm_pad(n2) + 1; }   // line stride of the x layout
 
-// One Stockham radix-R pass over all B lines: out <- pass(in).  sign = -1 forward, +1 inverse.
-CALES_HD void fft_pass(int tid, int nth, const double2* in, double2* out, const SmView& sv, const FftPlan& pl, int Ns, int R, int sign) {
+// ---- small in-register DFTs, natural order in and out, s = -1 forward / +1 inverse --------------------------------
+CALES_HD double2 cmul_i(double2 a, int s) { return s < 0 ? make_double2(a.y, -a.x) : make_double2(-a.y, a.x); }   // a * (s i)
+CALES_HD void dft2(double2& a, double2& b) { const double2 t = a; a = cadd(t, b); b = csub(t, b); }
+CALES_HD void dft3(double2& a, double2& b, double2& c, int s) {
+  const double s3 = 0.86602540378443864676372317075294;
+  const double2 t1 = cadd(b, c);
+  const double2 t2 = make_double2(a.x - 0.5 * t1.x, a.y - 0.5 * t1.y);
+  const double2 d = csub(b, c);
+  const double2 id = make_double2(-s3 * d.y, s3 * d.x);   // i * s3 * d
+  a = cadd(a, t1);
+  b = s < 0 ? csub(t2, id) : cadd(t2, id);
+  c = s < 0 ? cadd(t2, id) : csub(t2, id);
+}
+CALES_HD void dft4(double2& v0, double2& v1, double2& v2, double2& v3, int s) {
+  const double2 a0 = cadd(v0, v2), a1 = csub(v0, v2), a2 = cadd(v1, v3), a3 = cmul_i(csub(v1, v3), s);
+  v0 = cadd(a0, a2); v1 = cadd(a1, a3); v2 = csub(a0, a2); v3 = csub(a1, a3);
+}
+// a * exp(s i pi m / 8) for the constants the radix-8 / radix-16 butterflies need
+template <int M>
+CALES_HD double2 cmul_w16(double2 a, int s) {
+  const double c1 = 0.92387953251128675612818318939679, s1 = 0.38268343236508977172845998403040, r2 = 0.70710678118654752440084436210485;
+  const double sg = s < 0 ? -1.0 : 1.0;
+  if (M == 0) return a;
+  if (M == 4) return cmul_i(a, s);
+  double cr, ci;
+  if (M == 1) { cr = c1; ci = s1; } else if (M == 2) { cr = r2; ci = r2; } else if (M == 3) { cr = s1; ci = c1; }
+  else if (M == 6) { cr = -r2; ci = r2; } else /* M == 9 */ { cr = -c1; ci = -s1; }
+  ci *= sg;
+  return make_double2(a.x * cr - a.y * ci, a.x * ci + a.y * cr);
+}
+CALES_HD void dft8(double2* v, int s) {
+  dft4(v[0], v[2], v[4], v[6], s);
+  dft4(v[1], v[3], v[5], v[7], s);
+  const double2 o1 = cmul_w16<2>(v[3], s), o2 = cmul_i(v[5], s), o3 = cmul_w16<6>(v[7], s);
+  const double2 e0 = v[0], e1 = v[2], e2 = v[4], e3 = v[6], o0 = v[1];
+  v[0] = cadd(e0, o0); v[4] = csub(e0, o0);
+  v[1] = cadd(e1, o1); v[5] = csub(e1, o1);
+  v[2] = cadd(e2, o2); v[6] = csub(e2, o2);
+  v[3] = cadd(e3, o3); v[7] = csub(e3, o3);
+}
+CALES_HD void dft16(double2* v, int s) {
+  // n = 4a + b: step 1, DFT-4 over a for each b; step 2, twiddle W16^(b t1); step 3, DFT-4 over b for each t1
+#pragma unroll
+  for (int b = 0; b < 4; ++b) dft4(v[b], v[4 + b], v[8 + b], v[12 + b], s);      // v[4 t1 + b] = Y_b[t1]
+  v[5] = cmul_w16<1>(v[5], s); v[6] = cmul_w16<2>(v[6], s); v[7] = cmul_w16<3>(v[7], s);
+  v[9] = cmul_w16<2>(v[9], s); v[10] = cmul_w16<4>(v[10], s); v[11] = cmul_w16<6>(v[11], s);
+  v[13] = cmul_w16<3>(v[13], s); v[14] = cmul_w16<6>(v[14], s); v[15] = cmul_w16<9>(v[15], s);
+#pragma unroll
+  for (int t1 = 0; t1 < 4; ++t1) dft4(v[4 * t1], v[4 * t1 + 1], v[4 * t1 + 2], v[4 * t1 + 3], s);   // v[4 t1 + t2] = X[t1 + 4 t2]
+  // to natural order: X[m], m = t1 + 4 t2, sits at 4 t1 + t2 (a 4x4 transpose)
+#pragma unroll
+  for (int t1 = 0; t1 < 4; ++t1)
+#pragma unroll
+    for (int t2 = t1 + 1; t2 < 4; ++t2) { const double2 t = v[4 * t1 + t2]; v[4 * t1 + t2] = v[4 * t2 + t1]; v[4 * t2 + t1] = t; }
+}
+template <int R> CALES_HD void dft_small(double2* v, int s) {
+  if (R == 2) dft2(v[0], v[1]);
+  else if (R == 3) dft3(v[0], v[1], v[2], s);
+  else if (R == 4) dft4(v[0], v[1], v[2], v[3], s);
+  else if (R == 8) dft8(v, s);
+  else dft16(v, s);
+}
+
+// One Stockham radix-R pass over all B lines: out <- pass(in).  sign = -1 forward, +1 inverse.  Each butterfly lives in
+// registers; the inter-pass twiddles w^(t k) come from the table for t = 1, 2, 3 and by products above.
+template <int R>
+CALES_HD void fft_pass_r(int tid, int nth, const double2* in, double2* out, const SmView& sv, const FftPlan& pl, int Ns, int sign) {
   const int n2 = pl.n2, per = n2 / R, total = per * sv.B;
   const int tws = pl.n / (Ns * R);
   for (int idx = tid; idx < total; idx += nth) {
@@ -45,38 +114,34 @@ CALES_HD void fft_pass(int tid, int nth, const double2* in, double2* out, const 
     if (sv.bfast) { b = idx % sv.B; j = idx / sv.B; } else { j = idx % per; b = idx / per; }
     const int k = j % Ns;
     const int j0 = (j - k) * R + k;
-    double2 v[4];
+    double2 v[R];
 #pragma unroll
-    for (int t = 0; t < 4; ++t) if (t < R) v[t] = in[sm_off(sv, b, j + t * per)];
+    for (int t = 0; t < R; ++t) v[t] = in[sm_off(sv, b, j + t * per)];
     if (k != 0) {
-#pragma unroll
-      for (int t = 1; t < 4; ++t) if (t < R) {
-        const double2 w = pl.tw[t * k * tws];
-        v[t] = sign < 0 ? cmul(v[t], w) : cmulc(v[t], w);
+      double2 w[R];
+      w[1] = pl.tw[k * tws];
+      if (R > 2) w[2] = pl.tw[2 * k * tws];
+      if (R > 3) w[3] = pl.tw[3 * k * tws];
+      if (R > 4) { w[4] = cmul(w[2], w[2]); w[5] = cmul(w[4], w[1]); w[6] = cmul(w[4], w[2]); w[7] = cmul(w[4], w[3]); }
+      if (R > 8) {
+        w[8] = cmul(w[4], w[4]); w[9] = cmul(w[8], w[1]); w[10] = cmul(w[8], w[2]); w[11] = cmul(w[8], w[3]);
+        w[12] = cmul(w[8], w[4]); w[13] = cmul(w[12], w[1]); w[14] = cmul(w[12], w[2]); w[15] = cmul(w[12], w[3]);
       }
+#pragma unroll
+      for (int t = 1; t < R; ++t) v[t] = sign < 0 ? cmul(v[t], w[t]) : cmulc(v[t], w[t]);
     }
-    if (R == 4) {
-      const double2 a0 = cadd(v[0], v[2]), a1 = csub(v[0], v[2]), a2 = cadd(v[1], v[3]), d = csub(v[1], v[3]);
-      // forward: a3 = -i d = (d.y, -d.x); inverse: a3 = +i d = (-d.y, d.x)
-      const double2 a3 = sign < 0 ? make_double2(d.y, -d.x) : make_double2(-d.y, d.x);
-      out[sm_off(sv, b, j0)] = cadd(a0, a2);
-      out[sm_off(sv, b, j0 + Ns)] = cadd(a1, a3);
-      out[sm_off(sv, b, j0 + 2 * Ns)] = csub(a0, a2);
-      out[sm_off(sv, b, j0 + 3 * Ns)] = csub(a1, a3);
-    } else if (R == 2) {
-      out[sm_off(sv, b, j0)] = cadd(v[0], v[1]);
-      out[sm_off(sv, b, j0 + Ns)] = csub(v[0], v[1]);
-    } else {  // R == 3
-      const double s3 = 0.86602540378443864676372317075294;
-      const double2 t1 = cadd(v[1], v[2]);
-      const double2 t2 = make_double2(v[0].x - 0.5 * t1.x, v[0].y - 0.5 * t1.y);
-      const double2 d = csub(v[1], v[2]);
-      // forward: y1 = t2 - i s3 d, y2 = t2 + i s3 d;  i*d = (-d.y, d.x)
-      const double2 id = make_double2(-s3 * d.y, s3 * d.x);
-      out[sm_off(sv, b, j0)] = cadd(v[0], t1);
-      out[sm_off(sv, b, j0 + Ns)] = sign < 0 ? csub(t2, id) : cadd(t2, id);
-      out[sm_off(sv, b, j0 + 2 * Ns)] = sign < 0 ? cadd(t2, id) : csub(t2, id);
-    }
+    dft_small<R>(v, sign);
+#pragma unroll
+    for (int t = 0; t < R; ++t) out[sm_off(sv, b, j0 + t * Ns)] = v[t];
+  }
+}
+CALES_HD void fft_pass(int tid, int nth, const double2* in, double2* out, const SmView& sv, const FftPlan& pl, int Ns, int R, int sign) {
+  switch (R) {
+    case 2: fft_pass_r<2>(tid, nth, in, out, sv, pl, Ns, sign); break;
+    case 3: fft_pass_r<3>(tid, nth, in, out, sv, pl, Ns, sign); break;
+    case 4: fft_pass_r<4>(tid, nth, in, out, sv, pl, Ns, sign); break;
+    case 8: fft_pass_r<8>(tid, nth, in, out, sv, pl, Ns, sign); break;
+    default: fft_pass_r<16>(tid, nth, in, out, sv, pl, Ns, sign); break;
   }
 }
 
@@ -187,11 +252,11 @@ CALES_HD void fx_load(int tid, int nth, const Ctx& c, const FftPlan& pl, int B, 
         z.y = ((uu.y - uu.x) * rdx + (vv.y - vvm.y) * rdy + (ww.y - wwm.y) * rdz) * ds.inv_gdt;
       }
     }
-    buf[b * n2 + t] = z;
+    buf[b * sm_line(n2) + sm_pad(t)] = z;
   }
 }
 CALES_HD void fx_store_fwd(int tid, int nth, const FftPlan& pl, int B, long long l0, int nb, const double2* Z, double* dst) {
-  SmView sv{1, pl.n2, B, false};
+  SmView sv{1, sm_line(pl.n2), B, false};
   const int n = pl.n;
   split_forward(tid, nth, Z, sv, pl, false, nb, [&](int b, int sa, double va, int sb, double vb) {
     // FFT mode: slots (2m, 2m+1) are adjacent -> one 16-byte store
@@ -205,7 +270,7 @@ CALES_HD void fx_store_inv(int tid, int nth, const FftPlan& pl, int B, long long
   for (int idx = tid; idx < B * n2; idx += nth) {
     const int b = idx / n2, t = idx % n2;
     if (b >= nb) continue;
-    const double2 z = Z[b * n2 + t];
+    const double2 z = Z[b * sm_line(n2) + sm_pad(t)];
     reinterpret_cast<double2*>(dst + (l0 + b) * n)[t] = make_double2(z.x * sc, z.y * sc);
   }
 }
@@ -264,11 +329,11 @@ __device__ __forceinline__ int fft_run(int tid, int nth, double2* buf0, double2*
 template <bool DIV>
 __global__ void k_fft_x_fwd(const __grid_constant__ Ctx c, const __grid_constant__ FftPlan pl, int B, const double* __restrict__ src, DivSrc ds, double* __restrict__ dst) {
   extern __shared__ double2 smem[];
-  double2* buf0 = smem; double2* buf1 = smem + (size_t)B * pl.n2;
+  double2* buf0 = smem; double2* buf1 = smem + (size_t)B * sm_line(pl.n2);
   const long long nlines = (long long)c.ny * c.nz;
   const long long l0 = (long long)blockIdx.x * B;
   const int nb = (int)min((long long)B, nlines - l0);
-  SmView sv{1, pl.n2, B, false};
+  SmView sv{1, sm_line(pl.n2), B, false};
   const int tid = threadIdx.x, nth = blockDim.x;
   fx_load<DIV>(tid, nth, c, pl, B, l0, nb, src, ds, buf0);
   __syncthreads();
@@ -278,11 +343,11 @@ __global__ void k_fft_x_fwd(const __grid_constant__ Ctx c, const __grid_constant
 
 __global__ void k_fft_x_inv(const __grid_constant__ Ctx c, const __grid_constant__ FftPlan pl, int B, const double* __restrict__ src, double* __restrict__ dst) {
   extern __shared__ double2 smem[];
-  double2* buf0 = smem; double2* buf1 = smem + (size_t)B * pl.n2;
+  double2* buf0 = smem; double2* buf1 = smem + (size_t)B * sm_line(pl.n2);
   const long long nlines = (long long)c.ny * c.nz;
   const long long l0 = (long long)blockIdx.x * B;
   const int nb = (int)min((long long)B, nlines - l0);
-  SmView sv{1, pl.n2, B, false};
+  SmView sv{1, sm_line(pl.n2), B, false};
   const int tid = threadIdx.x, nth = blockDim.x;
   DivSrc none{nullptr, nullptr, nullptr, 0.0};
   fx_load<false>(tid, nth, c, pl, B, l0, nb, src, none, buf0);

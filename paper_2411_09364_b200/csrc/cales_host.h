@@ -8,6 +8,7 @@
 #include "cales_closures.cuh"
 
 #include <cmath>
+#include <cstdlib>
 #include <string>
 #include <vector>
 
@@ -42,12 +43,19 @@ static inline int validate(const cales_params* p) {
   return CALES_OK;
 }
 
+// Radix plan of the complex FFT of length n/2: factors of 3 first, then the power of two 2^a split into
+// ceil(a/4) passes of radix 2..16 of (nearly) equal size, smallest first (the first passes write with stride R).
 static inline void make_plan(FftPlan& pl, int n) {
   pl.n = n; pl.n2 = n / 2; pl.npass = 0; pl.tw = nullptr; pl.dctw = nullptr;
   int m = pl.n2;
-  while (m % 4 == 0) { pl.radix[pl.npass++] = 4; m /= 4; }
-  while (m % 2 == 0) { pl.radix[pl.npass++] = 2; m /= 2; }
   while (m % 3 == 0) { pl.radix[pl.npass++] = 3; m /= 3; }
+  int a = 0; while (m % 2 == 0) { ++a; m /= 2; }
+  if (a > 0) {
+    int maxbits = 4;
+    if (const char* e = std::getenv("CALES_FFT_MAXBITS")) { const int v = std::atoi(e); if (v >= 1 && v <= 4) maxbits = v; }
+    const int np = (a + maxbits - 1) / maxbits, base = a / np, extra = a % np;
+    for (int q = 0; q < np; ++q) pl.radix[pl.npass++] = 1 << (base + (q >= np - extra ? 1 : 0));
+  }
 }
 
 // Launch shape of the dynamic-model pass 1: block width TXB of k_dsm_col (64, 96 or 128: least padded columns),
@@ -148,20 +156,20 @@ static inline int build_setup(const cales_params* p, HostSetup& H) {
   make_plan(H.plx, nx);
   make_plan(H.ply, ny);
   {
-    const size_t per_line = 16 * (size_t)nx;             // two ping-pong buffers of nx/2 complex
+    const size_t per_line = 32 * (size_t)sm_line(nx / 2);  // two ping-pong buffers of nx/2 complex (padded)
     int B = (int)(98304 / per_line); if (B < 1) B = 1; if (B > 16) B = 16;
     const long long nlines = (long long)ny * nz; if (B > nlines) B = (int)nlines;
     H.xB = B; H.x_smem = (size_t)B * per_line;
-    const long long work = (long long)B * (nx / 2) / 2;
-    H.x_threads = work >= 512 ? 512 : (work >= 256 ? 256 : (work >= 128 ? 128 : 64));
+    long long th = ((long long)B * (nx / 2) / 8 + 31) / 32 * 32;      // ~8 complex elements per thread per pass
+    H.x_threads = (int)(th > 512 ? 512 : (th < 64 ? 64 : th));
   }
   {
     const size_t per_col = 16 * (size_t)ny;
     int TI = (int)(131072 / per_col); if (TI < 1) TI = 1; if (TI > 32) TI = 32; if (TI > nx) TI = nx;
     int t2 = 1; while (t2 * 2 <= TI) t2 *= 2; TI = t2;   // power of two keeps the row segments aligned
     H.yTI = TI; H.y_smem = (size_t)TI * per_col;
-    const long long work = (long long)TI * (ny / 2) / 2;
-    H.y_threads = work >= 512 ? 512 : (work >= 256 ? 256 : (work >= 128 ? 128 : 64));
+    long long th = ((long long)TI * (ny / 2) / 8 + 31) / 32 * 32;
+    H.y_threads = (int)(th > 512 ? 512 : (th < 64 ? 64 : th));
   }
   return CALES_OK;
 }

@@ -31,24 +31,48 @@ CALES_HD void poisson_column(const Ctx& c, const PoissonTabs& T, int i, int j, d
       for (int k = 0; k < nz; ++k) mean += A[col + st * k] * c.dzf[k];
       mean /= c.lz;
     }
+    // Both sweeps read their inputs TZ levels at a time into registers before the recurrence touches them, so that TZ
+    // independent loads per array are in flight per thread (the recurrence itself is a serial chain).
+    enum { TZ = 8 };
     double cp = 0.0, dp = 0.0;
-    for (int k = 0; k < nz; ++k) {
-      const double a = T.ak[k], cc = T.ck[k];
-      double b = lam - ((k > 0 || per) ? a : 0.0) - ((k < nz - 1 || per) ? cc : 0.0);
-      double d = A[col + st * k] - mean;
-      if (zero && k == 0) { cp = 0.0; dp = 0.0; }   // row 0: phi[0] = 0
-      else {
-        const double r = 1.0 / (b - a * cp);
-        cp = cc * r; dp = (d - a * dp) * r;
+    for (int k0 = 0; k0 < nz; k0 += TZ) {
+      double dd[TZ];
+#pragma unroll
+      for (int q = 0; q < TZ; ++q) dd[q] = (k0 + q < nz) ? A[col + st * (k0 + q)] : 0.0;
+#pragma unroll
+      for (int q = 0; q < TZ; ++q) {
+        const int k = k0 + q;
+        if (k < nz) {
+          const double a = T.ak[k], cc = T.ck[k];
+          const double b = lam - ((k > 0 || per) ? a : 0.0) - ((k < nz - 1 || per) ? cc : 0.0);
+          const double d = dd[q] - mean;
+          if (zero && k == 0) { cp = 0.0; dp = 0.0; }   // row 0: phi[0] = 0
+          else {
+            const double r = 1.0 / (b - a * cp);
+            cp = cc * r; dp = (d - a * dp) * r;
+          }
+          CP[col + st * k] = cp; A[col + st * k] = dp;
+        }
       }
-      CP[col + st * k] = cp; A[col + st * k] = dp;
     }
     double x = dp;
     double s = x * c.dzf[nz - 1];
-    for (int k = nz - 2; k >= 0; --k) {
-      x = A[col + st * k] - CP[col + st * k] * x;
-      A[col + st * k] = x;
-      s += x * c.dzf[k];
+    for (int k0 = nz - 2; k0 >= 0; k0 -= TZ) {
+      double dd[TZ], cc[TZ];
+#pragma unroll
+      for (int q = 0; q < TZ; ++q) {
+        const int k = k0 - q;
+        dd[q] = k >= 0 ? A[col + st * k] : 0.0; cc[q] = k >= 0 ? CP[col + st * k] : 0.0;
+      }
+#pragma unroll
+      for (int q = 0; q < TZ; ++q) {
+        const int k = k0 - q;
+        if (k >= 0) {
+          x = dd[q] - cc[q] * x;
+          A[col + st * k] = x;
+          s += x * c.dzf[k];
+        }
+      }
     }
     if (zero) {
       s /= c.lz;
@@ -120,16 +144,35 @@ CALES_HD void cn_coefficients(const Ctx& c, double cimp, double* coef) {
 CALES_HD double cn_column(const Ctx& c, const double* coef, int m, long long col, double* __restrict__ Q) {
   const int nz = c.nz; const long long st = c.nxy;
   const double* a = coef; const double* cp = coef + nz; const double* r = coef + 2 * nz;
+  enum { TZ = 8 };
   double dp = 0.0;
-  for (int k = 0; k < m; ++k) {
-    dp = (k == 0 ? Q[col] : Q[col + st * k] - a[k] * dp) * r[k];
-    Q[col + st * k] = dp;
+  for (int k0 = 0; k0 < m; k0 += TZ) {
+    double dd[TZ];
+#pragma unroll
+    for (int q = 0; q < TZ; ++q) dd[q] = (k0 + q < m) ? Q[col + st * (k0 + q)] : 0.0;
+#pragma unroll
+    for (int q = 0; q < TZ; ++q) {
+      const int k = k0 + q;
+      if (k < m) {
+        dp = (k == 0 ? dd[q] : dd[q] - a[k] * dp) * r[k];
+        Q[col + st * k] = dp;
+      }
+    }
   }
   double x = dp, s = x * c.dzf[m - 1];
-  for (int k = m - 2; k >= 0; --k) {
-    x = Q[col + st * k] - cp[k] * x;
-    Q[col + st * k] = x;
-    s += x * c.dzf[k];
+  for (int k0 = m - 2; k0 >= 0; k0 -= TZ) {
+    double dd[TZ];
+#pragma unroll
+    for (int q = 0; q < TZ; ++q) dd[q] = (k0 - q >= 0) ? Q[col + st * (k0 - q)] : 0.0;
+#pragma unroll
+    for (int q = 0; q < TZ; ++q) {
+      const int k = k0 - q;
+      if (k >= 0) {
+        x = dd[q] - cp[k] * x;
+        Q[col + st * k] = x;
+        s += x * c.dzf[k];
+      }
+    }
   }
   return s;
 }

@@ -79,12 +79,12 @@ static int run_passes(int nth, double2* buf0, double2* buf1, const SmView& sv, c
 }
 static void emu_fft_x_fwd(emu_solver* s, const double* src, const DivSrc* ds, double* dst) {
   const Ctx& c = s->c; const FftPlan& pl = s->plx; const int B = s->H.xB, nth = s->H.x_threads;
-  std::vector<double2> sm(2 * (size_t)B * pl.n2);
-  double2* buf0 = sm.data(); double2* buf1 = buf0 + (size_t)B * pl.n2;
+  std::vector<double2> sm(2 * (size_t)B * sm_line(pl.n2));
+  double2* buf0 = sm.data(); double2* buf1 = buf0 + (size_t)B * sm_line(pl.n2);
   const long long nlines = (long long)c.ny * c.nz;
   for (long long l0 = 0; l0 < nlines; l0 += B) {
     const int nb = (int)std::min<long long>(B, nlines - l0);
-    SmView sv{1, pl.n2, B, false};
+    SmView sv{1, sm_line(pl.n2), B, false};
     DivSrc none{nullptr, nullptr, nullptr, 0.0};
     for (int tid = 0; tid < nth; ++tid) { if (ds) fx_load<true>(tid, nth, c, pl, B, l0, nb, nullptr, *ds, buf0); else fx_load<false>(tid, nth, c, pl, B, l0, nb, src, none, buf0); }
     const int cur = run_passes(nth, buf0, buf1, sv, pl, -1, 0);
@@ -93,12 +93,12 @@ static void emu_fft_x_fwd(emu_solver* s, const double* src, const DivSrc* ds, do
 }
 static void emu_fft_x_inv(emu_solver* s, const double* src, double* dst) {
   const Ctx& c = s->c; const FftPlan& pl = s->plx; const int B = s->H.xB, nth = s->H.x_threads;
-  std::vector<double2> sm(2 * (size_t)B * pl.n2);
-  double2* buf0 = sm.data(); double2* buf1 = buf0 + (size_t)B * pl.n2;
+  std::vector<double2> sm(2 * (size_t)B * sm_line(pl.n2));
+  double2* buf0 = sm.data(); double2* buf1 = buf0 + (size_t)B * sm_line(pl.n2);
   const long long nlines = (long long)c.ny * c.nz;
   for (long long l0 = 0; l0 < nlines; l0 += B) {
     const int nb = (int)std::min<long long>(B, nlines - l0);
-    SmView sv{1, pl.n2, B, false};
+    SmView sv{1, sm_line(pl.n2), B, false};
     DivSrc none{nullptr, nullptr, nullptr, 0.0};
     for (int tid = 0; tid < nth; ++tid) fx_load<false>(tid, nth, c, pl, B, l0, nb, src, none, buf0);
     for (int tid = 0; tid < nth; ++tid) merge_inverse(tid, nth, buf0, buf1, sv, pl, false);
