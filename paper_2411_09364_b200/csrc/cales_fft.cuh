@@ -327,7 +327,7 @@ __device__ __forceinline__ int fft_run(int tid, int nth, double2* buf0, double2*
 }
 
 template <bool DIV>
-__global__ void k_fft_x_fwd(const __grid_constant__ Ctx c, const __grid_constant__ FftPlan pl, int B, const double* __restrict__ src, DivSrc ds, double* __restrict__ dst) {
+__global__ void __launch_bounds__(256, 2) k_fft_x_fwd(const __grid_constant__ Ctx c, const __grid_constant__ FftPlan pl, int B, const double* __restrict__ src, DivSrc ds, double* __restrict__ dst) {
   extern __shared__ double2 smem[];
   double2* buf0 = smem; double2* buf1 = smem + (size_t)B * sm_line(pl.n2);
   const long long nlines = (long long)c.ny * c.nz;
@@ -341,7 +341,7 @@ __global__ void k_fft_x_fwd(const __grid_constant__ Ctx c, const __grid_constant
   fx_store_fwd(tid, nth, pl, B, l0, nb, cur ? buf1 : buf0, dst);
 }
 
-__global__ void k_fft_x_inv(const __grid_constant__ Ctx c, const __grid_constant__ FftPlan pl, int B, const double* __restrict__ src, double* __restrict__ dst) {
+__global__ void __launch_bounds__(256, 2) k_fft_x_inv(const __grid_constant__ Ctx c, const __grid_constant__ FftPlan pl, int B, const double* __restrict__ src, double* __restrict__ dst) {
   extern __shared__ double2 smem[];
   double2* buf0 = smem; double2* buf1 = smem + (size_t)B * sm_line(pl.n2);
   const long long nlines = (long long)c.ny * c.nz;
@@ -358,7 +358,7 @@ __global__ void k_fft_x_inv(const __grid_constant__ Ctx c, const __grid_constant
   fx_store_inv(tid, nth, pl, B, l0, nb, cur ? buf1 : buf0, dst);
 }
 
-__global__ void k_fft_y(const __grid_constant__ Ctx c, const __grid_constant__ FftPlan pl, int TI, int dct, int inverse, double* __restrict__ A) {
+__global__ void __launch_bounds__(512, 1) k_fft_y(const __grid_constant__ Ctx c, const __grid_constant__ FftPlan pl, int TI, int dct, int inverse, double* __restrict__ A) {
   extern __shared__ double2 smem[];
   double2* buf0 = smem; double2* buf1 = smem + (size_t)TI * pl.n2;
   const int i0 = blockIdx.x * TI, k = blockIdx.y;

@@ -161,7 +161,7 @@ static inline int build_setup(const cales_params* p, HostSetup& H) {
     const long long nlines = (long long)ny * nz; if (B > nlines) B = (int)nlines;
     H.xB = B; H.x_smem = (size_t)B * per_line;
     long long th = ((long long)B * (nx / 2) / 8 + 31) / 32 * 32;      // ~8 complex elements per thread per pass
-    H.x_threads = (int)(th > 512 ? 512 : (th < 64 ? 64 : th));
+    H.x_threads = (int)(th > 256 ? 256 : (th < 64 ? 64 : th));   // k_fft_x_*: __launch_bounds__(256, 2)
   }
   {
     const size_t per_col = 16 * (size_t)ny;
