@@ -15,6 +15,7 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <vector>
@@ -301,9 +302,7 @@ static int run_eddy_viscosity(cales_solver* s, const double* u, const double* v,
     if (!ywall || split) {
       const int jlo = ywall ? DSM_TY : 0, jhi = ywall ? c.ny - DSM_TY : c.ny;
       dim3 grid(ds.nbx, (jhi - jlo + DSMC_LY - 1) / DSMC_LY, c.nz);
-      if (ds.txb == 64) k_dsm_col<64><<<grid, 64, 0, s->st>>>(c, u, v, w, jlo, jhi, ds.pslots, s->smag, s->dsm_part);
-      else if (ds.txb == 96) k_dsm_col<96><<<grid, 96, 0, s->st>>>(c, u, v, w, jlo, jhi, ds.pslots, s->smag, s->dsm_part);
-      else k_dsm_col<128><<<grid, 128, 0, s->st>>>(c, u, v, w, jlo, jhi, ds.pslots, s->smag, s->dsm_part);
+      k_dsm_col<64, 4><<<dim3(ds.nbx, grid.y, grid.z), 64, 0, s->st>>>(c, u, v, w, jlo, jhi, ds.pslots, s->smag, s->dsm_part);
       LAUNCH_TRY(K_DSM_COL);
     }
     k_dsm_coef<<<s->c.nz, 128, 0, s->st>>>(s->c, s->dsm_part, ds.pslots, s->dsm_cs);

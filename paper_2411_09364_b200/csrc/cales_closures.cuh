@@ -429,8 +429,8 @@ __global__ void __launch_bounds__(256) k_dsm_pass1(Ctx c, const double* __restri
 }
 // Column-marching pass 1.  grid (ceil(nx/(TXB-2)), ceil((jhi-jlo)/DSMC_LY), nz), block TXB (multiple of 32).
 // Handles output rows [jlo, jhi); part: [k][j][pslots][2], this kernel fills slots blockIdx.x*nwarps + warp.
-template <int TXB>
-__global__ void __launch_bounds__(TXB) k_dsm_col(const __grid_constant__ Ctx c, const double* __restrict__ u, const double* __restrict__ v,
+template <int TXB, int MINB>
+__global__ void __launch_bounds__(TXB, MINB) k_dsm_col(const __grid_constant__ Ctx c, const double* __restrict__ u, const double* __restrict__ v,
                                                  const double* __restrict__ w, int jlo, int jhi, int pslots, double* __restrict__ smag,
                                                  double* __restrict__ part) {
   __shared__ double sh[2][DSMC_NB * TXB];

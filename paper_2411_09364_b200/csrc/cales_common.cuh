@@ -111,6 +111,14 @@ CALES_HD void rk3_coeffs(int rk, double& al, double& be, double& ga) {
 }
 
 #ifdef __CUDACC__
+// 8-byte asynchronous global -> shared copies (LDGSTS)
+__device__ __forceinline__ void cp_async8(double* smem_dst, const double* gsrc) {
+  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(d), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;\n" ::: "memory"); }
+
 // Sum over the thread block (result valid in thread 0).  blockDim.x*y*z <= 1024, multiple of 32.
 __device__ __forceinline__ double block_sum(double v, double* sh /* >= 32 doubles */) {
   const int tid = threadIdx.x + blockDim.x * (threadIdx.y + blockDim.y * threadIdx.z);

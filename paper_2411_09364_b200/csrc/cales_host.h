@@ -64,13 +64,13 @@ struct DsmShape { int txb, nbx, pslots; };
 static inline DsmShape dsm_shape(int nx) {
   DsmShape d{64, 0, 0};
   long long best = -1;
-  for (int t : {64, 96, 128}) {
+  for (int t : {64}) {   // measured on B200: 64-thread CTAs (4 per SM at 224 registers) beat 32, 96 and 128
     const long long cost = (long long)((nx + t - 3) / (t - 2)) * t;
     if (best < 0 || cost < best) { best = cost; d.txb = t; }
   }
   d.nbx = (nx + d.txb - 3) / (d.txb - 2);
-  const int tile_slots = (nx + DSM_TX - 1) / DSM_TX, col_slots = d.nbx * (d.txb / 32);
-  d.pslots = tile_slots > col_slots ? tile_slots : col_slots;
+  d.pslots = (nx + DSM_TX - 1) / DSM_TX;
+  for (int t : {32, 64, 96, 128}) { const int cs = ((nx + t - 3) / (t - 2)) * (t / 32); if (cs > d.pslots) d.pslots = cs; }
   return d;
 }
 
@@ -165,7 +165,9 @@ static inline int build_setup(const cales_params* p, HostSetup& H) {
   }
   {
     const size_t per_col = 16 * (size_t)ny;
-    int TI = (int)(131072 / per_col); if (TI < 1) TI = 1; if (TI > 32) TI = 32; if (TI > nx) TI = nx;
+    size_t ybudget = 65536;     // measured: two or three smaller CTAs per SM overlap their load / transform / store phases
+    if (const char* e = std::getenv("CALES_FFT_YSMEM")) { const long v = std::atol(e); if (v >= 16384 && v <= 200 * 1024) ybudget = (size_t)v; }
+    int TI = (int)(ybudget / per_col); if (TI < 8) TI = (int)(131072 / per_col); if (TI < 1) TI = 1; if (TI > 32) TI = 32; if (TI > nx) TI = nx;
     int t2 = 1; while (t2 * 2 <= TI) t2 *= 2; TI = t2;   // power of two keeps the row segments aligned
     H.yTI = TI; H.y_smem = (size_t)TI * per_col;
     long long th = ((long long)TI * (ny / 2) / 8 + 31) / 32 * 32;

@@ -144,13 +144,6 @@ static inline int rt_chunk(int nx, int ny, int nz) {
 }
 
 #ifdef __CUDACC__
-__device__ __forceinline__ void cp_async8(double* smem_dst, const double* gsrc) {
-  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(d), "l"(gsrc) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;\n" ::: "memory"); }
-
 // grid (ceil(nx/RT_TX), ceil(ny/RT_TY), ceil(nz/kz)), block RT_THREADS, dynamic smem RT_SMEM_DOUBLES*8.
 // partial[linear block id] = sum over the CTA's points of u* dzf[k] (or nullptr).
 __global__ void __launch_bounds__(RT_THREADS, 2) k_rhs_tile(const __grid_constant__ Ctx c, const __grid_constant__ RhsArgs a, int kz,
