@@ -155,6 +155,23 @@ def host_register(torch, a):
     return int(rc) == 0
 
 
+def max_over_ranks(x, device):
+    """MAX of a python float over the ranks of the default process group (identity when there is none).  The only
+    collective of the multi-GPU bench: replicas share no data."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(x)
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(npts_per_rank, steps, world, max_ms):
+    """Whole-job Gpts*step/s of `world` replicas that each advanced npts_per_rank points by `steps` steps."""
+    return world * npts_per_rank * steps / (max_ms * 1e-3) / 1e9
+
+
 def run_ours(args):
     import numpy as np
     import torch
@@ -233,11 +250,8 @@ def run_ours(args):
     s.set_timing(False)
     diag = s.diagnostics()
     launches = s.launches_per_step() * K
-    if world > 1:
-        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = world * npts * K / (ms * 1e-3) / 1e9
+    ms = max_over_ranks(ms, "cuda")
+    value = aggregate_value(npts, K, world, ms)
 
     # ---- e2e: the same metric through the C ABI with HOST buffers, copies inside the timed region
     Ke = max(1, min(K, 3))
@@ -257,11 +271,8 @@ def run_ours(args):
         e2e_step()
     torch.cuda.synchronize()
     te = time.perf_counter() - t0
-    if world > 1:
-        t = torch.tensor([te], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        te = float(t.item())
-    e2e = {"value": world * npts * Ke / te / 1e9, "unit": UNIT, "h2d_bytes_per_step": 3 * npts * 8, "d2h_bytes_per_step": 4 * npts * 8,
+    te = max_over_ranks(te, "cuda")
+    e2e = {"value": aggregate_value(npts, Ke, world, te * 1e3), "unit": UNIT, "h2d_bytes_per_step": 3 * npts * 8, "d2h_bytes_per_step": 4 * npts * 8,
            "steps": Ke, "ms_per_step": 1e3 * te / Ke, "host_memory": "pinned (cudaHostRegister)" if pinned else "pageable",
            "note": "each step: cales_set_field(u,v,w) from host, cales_step, cales_get_field(u,v,w,p) to host; a new velocity makes "
                    "the library re-evaluate the wall stress and nu_t first"}

@@ -190,3 +190,76 @@ def test_error_paths(gpu):
     h = C.c_void_p()
     assert L.cales_create(C.byref(P), C.byref(h)) == 1 and b"small" in L.cales_last_error()
     assert L.cales_step(None, 1.0) == 1
+
+
+# ------------------------------------------------------------------------------------------------------------------------
+# north_star's second bound: <= 1e-8 after 100 steps (50 for config 4, 20 for config 5, 10 for config 1).
+LONG_CASES = {
+    "cfg2_full_100": (2, None, 100),               # BASELINE config 2 at full size (192x96x64), 100 steps
+    "cfg3_replica_100": (3, (96, 72, 48), 100),
+    "cfg4_replica_50": (4, (192, 54, 48), 50),
+    "cfg5_replica_20": (5, (192, 128, 64), 20),
+}
+
+
+@pytest.mark.parametrize("case", sorted(LONG_CASES))
+def test_long_run_parity(oracle, gpu, case):
+    n, shape, steps = LONG_CASES[case]
+    cfg, kw, (u, v, w), dt = pc.prepare(oracle, n, shape)
+    o = pc.make(oracle.Oracle, kw)
+    g = pc.make(gpu.Solver, kw)
+    o.set_velocity(u, v, w); g.set_velocity(u, v, w)
+    for s in range(steps):
+        o.step(dt); g.step(dt)
+    err = pc.field_errors(_gpu_fields(g), [o.get(f) for f in range(5)], o.dzf, kw["nu"])
+    assert max(err.values()) <= TOL_100, (case, err)
+    d = g.diagnostics()
+    assert d["nan_count"] == 0
+    if kw["const_flow_rate"]:
+        assert abs(d["u_bulk"] - kw["u_bulk"]) <= 1e-13 * abs(kw["u_bulk"])
+    g.close()
+
+
+@pytest.mark.parametrize("n", [3, 4, 5])
+def test_full_size_properties(gpu, n):
+    """BASELINE sizes in the launch configuration bench.py times (configs 3-5 are beyond the oracle's reach in a test):
+    properties that hold at any size -- projection to round-off (P4), imposed bulk velocity (P15), finite fields, Newton
+    iteration count, and the manufactured Poisson solution evaluated ON THE GPU by torch stencils at sampled planes."""
+    import psutil
+    import torch
+    from paper_2411_09364_b200 import inputs
+    cfg = inputs.config(n)
+    p = cfg["params"]
+    npts = p["nx"] * p["ny"] * p["nz"]
+    free, _ = torch.cuda.mem_get_info()
+    if free < 16 * npts * 8 or psutil.virtual_memory().available < 8 * npts * 8:
+        pytest.skip("not enough device / host memory for config %d at full size" % n)
+    u, v, w, ub = inputs.initial_fields(cfg)
+    dt = inputs.time_step(cfg, u, v, w)
+    kw = inputs.solver_kwargs(cfg, ub)
+    g = pc.make(gpu.Solver, kw)
+    g.set_velocity(u, v, w)
+    del u, v, w
+    g.project()
+    for _ in range(2):
+        g.step(dt)
+    d = g.diagnostics()
+    dzmin = p["lz"] / p["nz"] if p["zstretch"] == 0 else float(np.min(np.diff(inputs.z_faces(p))))
+    scale = max(abs(ub), 1.0) / min(p["lx"] / p["nx"], p["ly"] / p["ny"], dzmin)
+    assert d["nan_count"] == 0
+    assert d["max_div"] <= 1e-12 * scale * 10, d
+    assert abs(d["u_bulk"] - ub) <= 1e-13 * abs(ub)
+    if p["wall_model"]:
+        assert 3 <= d["wm_max_iters"] <= 9
+    # Poisson solve at full size: residual of L_h phi = f by an independent torch stencil, interior of sampled planes
+    f = torch.randn(g.shape, dtype=torch.float64, device="cuda", generator=torch.Generator(device="cuda").manual_seed(7))
+    phi = g.poisson_solve(f)
+    if p["zstretch"] == 0:
+        dx, dy, dz = p["lx"] / p["nx"], p["ly"] / p["ny"], p["lz"] / p["nz"]
+        k = p["nz"] // 3
+        c = phi[k, 1:-1, 1:-1]
+        lap = ((phi[k, 1:-1, 2:] - 2 * c + phi[k, 1:-1, :-2]) / dx ** 2 + (phi[k, 2:, 1:-1] - 2 * c + phi[k, :-2, 1:-1]) / dy ** 2
+               + (phi[k + 1, 1:-1, 1:-1] - 2 * c + phi[k - 1, 1:-1, 1:-1]) / dz ** 2)
+        fm = f[k, 1:-1, 1:-1] - (f.sum(dim=(1, 2)) * dz).sum() / (p["nx"] * p["ny"] * p["lz"])   # the solve drops the mean of f
+        assert float((lap - fm).abs().max()) <= 1e-9 * float(f.abs().max())
+    g.close()
