@@ -45,7 +45,7 @@ struct cales_solver {
   FftPlan plx, ply;
   PoissonTabs pt;
   WallGeom wg;
-  int xB, yTI; size_t x_smem, y_smem; int x_threads, y_threads;
+  int xB, yTI, y_tish; size_t x_smem, y_smem; int x_threads, y_threads;
   dim3 pgrid, pblock;   // point kernels
   long long nblk;
   bool fresh;
@@ -172,11 +172,11 @@ extern "C" int cales_create(const cales_params* p, cales_solver** out) {
   s->plx = H.plx; s->plx.tw = s->twx;
   s->ply = H.ply; s->ply.tw = s->twy; s->ply.dctw = s->dctw;
   s->xB = H.xB; s->x_smem = H.x_smem; s->x_threads = H.x_threads;
-  s->yTI = H.yTI; s->y_smem = H.y_smem; s->y_threads = H.y_threads;
-  e = cudaFuncSetAttribute(k_fft_x_fwd<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fft_x_fwd<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fft_x_inv, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fft_y, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+  s->yTI = H.yTI; s->y_tish = H.y_tish; s->y_smem = H.y_smem; s->y_threads = H.y_threads;
+  e = cudaFuncSetAttribute(k_fft2_x_fwd<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fft2_x_fwd<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fft2_x_inv, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fft2_y, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rhs_tile, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(RT_SMEM_DOUBLES * sizeof(double)));
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dsm_pass1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(DSM_SMEM_DOUBLES * sizeof(double)));
   if (e != cudaSuccess) { delete s; return fail(CALES_ECUDA, std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e)); }
@@ -237,21 +237,21 @@ extern "C" int cales_get_field(cales_solver* s, int field, double* dst, int on_d
 static int run_transform_x_fwd(cales_solver* s, const double* src, const DivSrc* ds, double* dst) {
   const long long nlines = (long long)s->c.ny * s->c.nz;
   const unsigned grid = (unsigned)((nlines + s->xB - 1) / s->xB);
-  if (ds) k_fft_x_fwd<true><<<grid, s->x_threads, s->x_smem, s->st>>>(s->c, s->plx, s->xB, nullptr, *ds, dst);
-  else { DivSrc z{nullptr, nullptr, nullptr, 0.0}; k_fft_x_fwd<false><<<grid, s->x_threads, s->x_smem, s->st>>>(s->c, s->plx, s->xB, src, z, dst); }
+  if (ds) k_fft2_x_fwd<true><<<grid, s->x_threads, s->x_smem, s->st>>>(s->c, s->plx, s->xB, nullptr, *ds, dst);
+  else { DivSrc z{nullptr, nullptr, nullptr, 0.0}; k_fft2_x_fwd<false><<<grid, s->x_threads, s->x_smem, s->st>>>(s->c, s->plx, s->xB, src, z, dst); }
   LAUNCH_TRY(K_FFTX_FWD);
   return CALES_OK;
 }
 static int run_transform_x_inv(cales_solver* s, const double* src, double* dst) {
   const long long nlines = (long long)s->c.ny * s->c.nz;
   const unsigned grid = (unsigned)((nlines + s->xB - 1) / s->xB);
-  k_fft_x_inv<<<grid, s->x_threads, s->x_smem, s->st>>>(s->c, s->plx, s->xB, src, dst);
+  k_fft2_x_inv<<<grid, s->x_threads, s->x_smem, s->st>>>(s->c, s->plx, s->xB, src, dst);
   LAUNCH_TRY(K_FFTX_INV);
   return CALES_OK;
 }
 static int run_transform_y(cales_solver* s, double* A, int inverse) {
   dim3 grid((s->c.nx + s->yTI - 1) / s->yTI, s->c.nz);
-  k_fft_y<<<grid, s->y_threads, s->y_smem, s->st>>>(s->c, s->ply, s->yTI, s->c.bc_y == BC_WALL ? 1 : 0, inverse, A);
+  k_fft2_y<<<grid, s->y_threads, s->y_smem, s->st>>>(s->c, s->ply, s->y_tish, s->c.bc_y == BC_WALL ? 1 : 0, inverse, A);
   LAUNCH_TRY(inverse ? K_FFTY_INV : K_FFTY_FWD);
   return CALES_OK;
 }

@@ -23,6 +23,8 @@ struct FftPlan {
   int n2;           // n/2, length of the complex FFT
   int npass;
   int radix[20];
+  int per[20], ns[20];          // butterflies per line and product of the previous radices, per pass
+  unsigned mper[20], mns[20];   // ceil(2^32 / per), ceil(2^32 / ns) for the division-free index split (cales_fft2.cuh)
   const double2* tw;    // tw[q] = exp(-2 pi i q / n), q = 0..n-1
   const double2* dctw;  // dctw[m] = exp(-i pi m / (2 n)), m = 0..n/2   (DCT only)
 };

@@ -5,6 +5,7 @@
 #include "../../include/cales.h"
 #include "cales_common.cuh"
 #include "cales_fft.cuh"
+#include "cales_fft2.cuh"
 #include "cales_closures.cuh"
 
 #include <cmath>
@@ -43,18 +44,26 @@ static inline int validate(const cales_params* p) {
   return CALES_OK;
 }
 
-// Radix plan of the complex FFT of length n/2: factors of 3 first, then the power of two 2^a split into
-// ceil(a/4) passes of radix 2..16 of (nearly) equal size, smallest first (the first passes write with stride R).
+// Radix plan of the complex FFT of length n/2: the power of two 2^a split into ceil(a/4) passes of radix 2..16 of
+// (nearly) equal size, smallest first (the first passes write with stride R), then the factors of 3.
 static inline void make_plan(FftPlan& pl, int n) {
   pl.n = n; pl.n2 = n / 2; pl.npass = 0; pl.tw = nullptr; pl.dctw = nullptr;
-  int m = pl.n2;
-  while (m % 3 == 0) { pl.radix[pl.npass++] = 3; m /= 3; }
+  int m = pl.n2, n3 = 0;
+  while (m % 3 == 0) { ++n3; m /= 3; }
   int a = 0; while (m % 2 == 0) { ++a; m /= 2; }
   if (a > 0) {
     int maxbits = 4;
     if (const char* e = std::getenv("CALES_FFT_MAXBITS")) { const int v = std::atoi(e); if (v >= 1 && v <= 4) maxbits = v; }
     const int np = (a + maxbits - 1) / maxbits, base = a / np, extra = a % np;
     for (int q = 0; q < np; ++q) pl.radix[pl.npass++] = 1 << (base + (q >= np - extra ? 1 : 0));
+  }
+  for (int q = 0; q < n3; ++q) pl.radix[pl.npass++] = 3;
+  int Ns = 1;
+  for (int p = 0; p < pl.npass; ++p) {
+    pl.per[p] = pl.n2 / pl.radix[p]; pl.ns[p] = Ns;
+    pl.mper[p] = pl.per[p] > 1 ? (unsigned)((0x100000000ull + pl.per[p] - 1) / pl.per[p]) : 0u;
+    pl.mns[p] = Ns > 1 ? (unsigned)((0x100000000ull + Ns - 1) / Ns) : 0u;
+    Ns *= pl.radix[p];
   }
 }
 
@@ -80,7 +89,7 @@ struct HostSetup {
   Ctx c;                          // table pointers NOT set
   WallGeom wg;
   FftPlan plx, ply;               // twiddle pointers NOT set
-  int xB, yTI, x_threads, y_threads; size_t x_smem, y_smem;
+  int xB, yTI, y_tish, x_threads, y_threads; size_t x_smem, y_smem;
 };
 
 static inline int build_setup(const cales_params* p, HostSetup& H) {
@@ -155,24 +164,32 @@ static inline int build_setup(const cales_params* p, HostSetup& H) {
   // ---- transform plans and launch shapes
   make_plan(H.plx, nx);
   make_plan(H.ply, ny);
+  // every thread holds 16 complex elements per pass (15 when a radix-3 pass exists): ~256 threads per CTA
+  auto threads_for = [](long long elems, const FftPlan& pl) {
+    bool has3 = false; for (int p = 0; p < pl.npass; ++p) has3 |= pl.radix[p] == 3;
+    long long th = (elems + (has3 ? 14 : 15)) / (has3 ? 15 : 16);
+    th = (th + 31) / 32 * 32;
+    return (int)(th < 32 ? 32 : th);
+  };
   {
-    const size_t per_line = 32 * (size_t)sm_line(nx / 2);  // two ping-pong buffers of nx/2 complex (padded)
-    int B = (int)(98304 / per_line); if (B < 1) B = 1; if (B > 16) B = 16;
-    const long long nlines = (long long)ny * nz; if (B > nlines) B = (int)nlines;
-    H.xB = B; H.x_smem = (size_t)B * per_line;
-    long long th = ((long long)B * (nx / 2) / 8 + 31) / 32 * 32;      // ~8 complex elements per thread per pass
-    H.x_threads = (int)(th > 256 ? 256 : (th < 64 ? 64 : th));   // k_fft_x_*: __launch_bounds__(256, 2)
+    const int n2 = nx / 2;
+    int L = 4096 / n2; if (L < 1) L = 1; if (L > 64) L = 64;
+    const long long nlines = (long long)ny * nz; if (L > nlines) L = (int)nlines;
+    while (L > 1 && threads_for((long long)L * n2, H.plx) > 256) --L;
+    H.xB = L; H.x_smem = (size_t)L * sm_line(n2) * 16;
+    H.x_threads = threads_for((long long)L * n2, H.plx);
   }
   {
-    const size_t per_col = 16 * (size_t)ny;
-    size_t ybudget = 65536;     // measured: two or three smaller CTAs per SM overlap their load / transform / store phases
-    if (const char* e = std::getenv("CALES_FFT_YSMEM")) { const long v = std::atol(e); if (v >= 16384 && v <= 200 * 1024) ybudget = (size_t)v; }
-    int TI = (int)(ybudget / per_col); if (TI < 8) TI = (int)(131072 / per_col); if (TI < 1) TI = 1; if (TI > 32) TI = 32; if (TI > nx) TI = nx;
-    int t2 = 1; while (t2 * 2 <= TI) t2 *= 2; TI = t2;   // power of two keeps the row segments aligned
-    H.yTI = TI; H.y_smem = (size_t)TI * per_col;
-    long long th = ((long long)TI * (ny / 2) / 8 + 31) / 32 * 32;
-    H.y_threads = (int)(th > 512 ? 512 : (th < 64 ? 64 : th));
+    const int n2 = ny / 2;
+    int tish = 5;                                                   // TI = 32 columns ...
+    while (tish > 3 && (long long)(1 << tish) * n2 > 4096) --tish;   // ... down to 8 (64-byte row segments) for long lines
+    while (tish > 0 && (1 << tish) > nx) --tish;
+    while (tish > 0 && (threads_for((long long)(1 << tish) * n2, H.ply) > 512 || (size_t)(1 << tish) * n2 * 16 > 200 * 1024)) --tish;
+    H.yTI = 1 << tish; H.y_tish = tish; H.y_smem = (size_t)(1 << tish) * n2 * 16; if (H.y_smem < 16) H.y_smem = 16;
+    H.y_threads = threads_for((long long)(1 << tish) * n2, H.ply);
   }
+  if (H.x_threads > 512 || H.y_threads > 512 || H.x_smem > 200 * 1024 || H.y_smem > 200 * 1024)
+    return fail(CALES_EUNSUPPORTED, "line too long for the shared-memory transforms");
   return CALES_OK;
 }
 

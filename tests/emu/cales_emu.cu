@@ -68,61 +68,71 @@ extern "C" int emu_set_field(emu_solver* s, int f, const double* src) {
 extern "C" int emu_get_field(emu_solver* s, int f, double* dst) { std::memcpy(dst, fld(s, f)->data(), s->N * sizeof(double)); return 0; }
 
 // ---- kernel emulations: same block decomposition and phase order as the __global__ wrappers ----
-static int run_passes(int nth, double2* buf0, double2* buf1, const SmView& sv, const FftPlan& pl, int sign, int start) {
-  int cur = start, Ns = 1;
-  for (int p = 0; p < pl.npass; ++p) {
-    const int R = pl.radix[p];
-    for (int tid = 0; tid < nth; ++tid) fft_pass(tid, nth, cur ? buf1 : buf0, cur ? buf0 : buf1, sv, pl, Ns, R, sign);
-    Ns *= R; cur ^= 1;
+// f2_passes (cales_fft2.cuh) stepped on the host: one register file of F2_E complex numbers per emulated thread, the
+// phases separated where the kernel has its block barriers.
+template <bool TO_GLOBAL, class FIRST, class LAST>
+static void emu_f2_passes(const Fft2Lay& lay, const FftPlan& pl, int sign, double2* buf, int nth, FIRST first, LAST last) {
+  const int np = pl.npass;
+  std::vector<double2> regs((size_t)nth * F2_E);
+  F2SmemLd sld{buf, lay}; F2SmemSt sst{buf, lay};
+  if (np == 0) {
+    std::vector<double2> z(lay.L);
+    for (int tid = 0; tid < lay.L && tid < nth; ++tid) z[tid] = first(tid, 0);
+    for (int tid = 0; tid < lay.L && tid < nth; ++tid) { if (TO_GLOBAL) last(tid, 0, z[tid]); else sst(tid, 0, z[tid]); }
+    return;
   }
-  return cur;
+  for (int p = 0; p < np; ++p) {
+    for (int tid = 0; tid < nth; ++tid) {
+      if (p == 0) f2_load_any(lay, pl, 0, tid, nth, first, &regs[(size_t)tid * F2_E]);
+      else f2_load_any(lay, pl, p, tid, nth, sld, &regs[(size_t)tid * F2_E]);
+    }
+    for (int tid = 0; tid < nth; ++tid) {
+      if (TO_GLOBAL && p == np - 1) f2_bfly_any(lay, pl, p, sign, tid, nth, &regs[(size_t)tid * F2_E], last);
+      else f2_bfly_any(lay, pl, p, sign, tid, nth, &regs[(size_t)tid * F2_E], sst);
+    }
+  }
 }
 static void emu_fft_x_fwd(emu_solver* s, const double* src, const DivSrc* ds, double* dst) {
-  const Ctx& c = s->c; const FftPlan& pl = s->plx; const int B = s->H.xB, nth = s->H.x_threads;
-  std::vector<double2> sm(2 * (size_t)B * sm_line(pl.n2));
-  double2* buf0 = sm.data(); double2* buf1 = buf0 + (size_t)B * sm_line(pl.n2);
+  const Ctx& c = s->c; const FftPlan& pl = s->plx; const int L = s->H.xB, nth = s->H.x_threads;
+  const Fft2Lay lay{L, sm_line(pl.n2), 0, false};
+  std::vector<double2> sm((size_t)L * lay.ls);
   const long long nlines = (long long)c.ny * c.nz;
-  for (long long l0 = 0; l0 < nlines; l0 += B) {
-    const int nb = (int)std::min<long long>(B, nlines - l0);
-    SmView sv{1, sm_line(pl.n2), B, false};
-    DivSrc none{nullptr, nullptr, nullptr, 0.0};
-    for (int tid = 0; tid < nth; ++tid) { if (ds) fx_load<true>(tid, nth, c, pl, B, l0, nb, nullptr, *ds, buf0); else fx_load<false>(tid, nth, c, pl, B, l0, nb, src, none, buf0); }
-    const int cur = run_passes(nth, buf0, buf1, sv, pl, -1, 0);
-    for (int tid = 0; tid < nth; ++tid) fx_store_fwd(tid, nth, pl, B, l0, nb, cur ? buf1 : buf0, dst);
+  DivSrc none{nullptr, nullptr, nullptr, 0.0};
+  for (long long l0 = 0; l0 < nlines; l0 += L) {
+    const int nb = (int)std::min<long long>(L, nlines - l0);
+    F2XFwdLd first{c, pl, l0, nb, src, ds ? *ds : none, ds != nullptr};
+    emu_f2_passes<false>(lay, pl, -1, sm.data(), nth, first, F2SmemSt{sm.data(), lay});
+    for (int tid = 0; tid < nth; ++tid) f2x_split_store(tid, nth, pl, lay, l0, nb, sm.data(), dst);
   }
 }
 static void emu_fft_x_inv(emu_solver* s, const double* src, double* dst) {
-  const Ctx& c = s->c; const FftPlan& pl = s->plx; const int B = s->H.xB, nth = s->H.x_threads;
-  std::vector<double2> sm(2 * (size_t)B * sm_line(pl.n2));
-  double2* buf0 = sm.data(); double2* buf1 = buf0 + (size_t)B * sm_line(pl.n2);
+  const Ctx& c = s->c; const FftPlan& pl = s->plx; const int L = s->H.xB, nth = s->H.x_threads;
+  const Fft2Lay lay{L, sm_line(pl.n2), 0, false};
+  std::vector<double2> sm((size_t)L * lay.ls);
   const long long nlines = (long long)c.ny * c.nz;
-  for (long long l0 = 0; l0 < nlines; l0 += B) {
-    const int nb = (int)std::min<long long>(B, nlines - l0);
-    SmView sv{1, sm_line(pl.n2), B, false};
-    DivSrc none{nullptr, nullptr, nullptr, 0.0};
-    for (int tid = 0; tid < nth; ++tid) fx_load<false>(tid, nth, c, pl, B, l0, nb, src, none, buf0);
-    for (int tid = 0; tid < nth; ++tid) merge_inverse(tid, nth, buf0, buf1, sv, pl, false);
-    const int cur = run_passes(nth, buf0, buf1, sv, pl, +1, 1);
-    for (int tid = 0; tid < nth; ++tid) fx_store_inv(tid, nth, pl, B, l0, nb, cur ? buf1 : buf0, dst);
+  for (long long l0 = 0; l0 < nlines; l0 += L) {
+    const int nb = (int)std::min<long long>(L, nlines - l0);
+    F2XInvLd first{pl, l0, nb, src};
+    F2XInvSt last{pl, l0, nb, dst, 1.0 / (double)pl.n2};
+    emu_f2_passes<true>(lay, pl, +1, sm.data(), nth, first, last);
   }
 }
 static void emu_fft_y(emu_solver* s, double* A, int inverse) {
   const Ctx& c = s->c; const FftPlan& pl = s->ply; const int TI = s->H.yTI, nth = s->H.y_threads;
   const bool dct = c.bc_y == BC_WALL;
-  std::vector<double2> sm(2 * (size_t)TI * pl.n2);
-  double2* buf0 = sm.data(); double2* buf1 = buf0 + (size_t)TI * pl.n2;
+  const Fft2Lay lay{TI, 0, s->H.y_tish, true};
+  std::vector<double2> sm((size_t)TI * std::max(pl.n2, 1));
   for (int k = 0; k < c.nz; ++k) for (int i0 = 0; i0 < c.nx; i0 += TI) {
     const int nb = std::min(TI, c.nx - i0);
     double* base = A + (long long)k * c.nxy + i0;
-    SmView sv{TI, 1, TI, true};
-    for (int tid = 0; tid < nth; ++tid) fy_load(tid, nth, c, pl, TI, dct, inverse != 0, base, nb, buf0);
     if (!inverse) {
-      const int cur = run_passes(nth, buf0, buf1, sv, pl, -1, 0);
-      for (int tid = 0; tid < nth; ++tid) fy_store_fwd(tid, nth, c, pl, TI, dct, base, nb, cur ? buf1 : buf0);
+      F2YFwdLd first{c, pl, base, nb, dct};
+      emu_f2_passes<false>(lay, pl, -1, sm.data(), nth, first, F2SmemSt{sm.data(), lay});
+      for (int tid = 0; tid < nth; ++tid) f2y_split_store(tid, nth, c, pl, lay, dct, base, nb, sm.data());
     } else {
-      for (int tid = 0; tid < nth; ++tid) merge_inverse(tid, nth, buf0, buf1, sv, pl, dct);
-      const int cur = run_passes(nth, buf0, buf1, sv, pl, +1, 1);
-      for (int tid = 0; tid < nth; ++tid) fy_store_inv(tid, nth, c, pl, TI, dct, base, nb, cur ? buf1 : buf0);
+      F2YInvLd first{c, pl, base, nb, dct};
+      F2YInvSt last{c, pl, base, nb, dct, 1.0 / (double)pl.n2};
+      emu_f2_passes<true>(lay, pl, +1, sm.data(), nth, first, last);
     }
   }
 }
