@@ -202,7 +202,11 @@ def run_ours(args):
     p_host = np.zeros_like(u)
     pinned = all(host_register(torch, a) for a in (u, v, w, p_host))
     t_gen = time.perf_counter() - t_gen
-    s = binding.Solver(g["nx"], g["ny"], g["nz"], g["lx"], g["ly"], g["lz"], device=local, **kw)
+    # a dedicated (non-default) stream: everything below -- the solver's kernels, torch's L2 flush, the CUDA events -- is
+    # issued on it, and cales_step can capture its substeps into a CUDA graph (the legacy default stream cannot be captured)
+    stream = torch.cuda.Stream(device=local)
+    torch.cuda.set_stream(stream)
+    s = binding.Solver(g["nx"], g["ny"], g["nz"], g["lx"], g["ly"], g["lz"], device=local, stream=stream, **kw)
     s.set_velocity(u, v, w)
     s.project()                      # discretely solenoidal start, by the GPU solver itself
     for f, a in zip(range(3), (u, v, w)):
@@ -303,6 +307,7 @@ def run_ours(args):
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": "config %d: %s %dx%dx%d" % (cfg_no, cfg["name"], g["nx"], g["ny"], g["nz"]), "points": npts,
                        "dt": dt, "parallelism": "replicas x%d (no data-path collective)" % world,
+                       "launch": "cales_step replays one CUDA graph per step" if not big else "plain stream launches (per-kernel events on)",
                        "l2": "L2 flushed between timed steps" if small else "state (%.1f GB) larger than L2" % (s.workspace_bytes / 1e9),
                        "options": {k: kw[k] for k in ("bc_y", "bc_z", "zstretch", "sgs_model", "wall_model", "implicit_z", "const_flow_rate",
                                                       "dsm_avg_xy_plane", "dsm_clip_total", "van_driest")}},

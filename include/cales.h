@@ -155,6 +155,10 @@ int cales_kernel_count(void);
  * the three may be NULL).  Synchronises the stream. */
 int cales_kernel_time(cales_solver* s, int kid, const char** name, double* ms_total, int* launches);
 
+/* cales_step replays its three substeps as one CUDA graph (captured per value of dt; on by default, bypassed while
+ * timing is on).  on = 0 returns to plain stream launches. */
+int cales_set_graph(cales_solver* s, int on);
+
 /* Number of kernels cales_step launches per call with the current parameters (for bench.py's gpu_launches). */
 int cales_launches_per_step(cales_solver* s);
 

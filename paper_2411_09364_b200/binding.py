@@ -39,7 +39,7 @@ class CalesDiag(C.Structure):
 SYMBOLS = ["cales_default_params", "cales_workspace_bytes", "cales_create", "cales_create_basic", "cales_destroy",
            "cales_set_field", "cales_get_field", "cales_step", "cales_poisson_solve", "cales_eddy_viscosity",
            "cales_wall_stress", "cales_project", "cales_get_cs", "cales_transform", "cales_transpose_xy",
-           "cales_set_timing", "cales_kernel_count", "cales_kernel_time", "cales_launches_per_step", "cales_diagnostics", "cales_last_error"]
+           "cales_set_timing", "cales_set_graph", "cales_kernel_count", "cales_kernel_time", "cales_launches_per_step", "cales_diagnostics", "cales_last_error"]
 
 _lib = None
 
@@ -69,6 +69,7 @@ def lib():
         L.cales_transform.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int]
         L.cales_transpose_xy.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.cales_set_timing.argtypes = [C.c_void_p, C.c_int]
+        L.cales_set_graph.argtypes = [C.c_void_p, C.c_int]
         L.cales_launches_per_step.argtypes = [C.c_void_p]
         L.cales_kernel_time.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_char_p), C.POINTER(C.c_double), C.POINTER(C.c_int)]
         L.cales_diagnostics.argtypes = [C.c_void_p, C.POINTER(CalesDiag)]
@@ -242,6 +243,9 @@ class Solver:
             if n.value:
                 out[name.value.decode()] = (ms.value, n.value)
         return out
+
+    def set_graph(self, on=True):
+        _chk(lib().cales_set_graph(self._h, 1 if on else 0))
 
     def launches_per_step(self):
         return lib().cales_launches_per_step(self._h)

@@ -49,6 +49,7 @@ struct cales_solver {
   dim3 pgrid, pblock;   // point kernels
   long long nblk;
   bool fresh;
+  int use_graph; cudaGraphExec_t gexec; double gdt;   // the three substeps captured as one CUDA graph, keyed by dt
   int timing; bool ev_valid;
   std::vector<cudaEvent_t> evpool; std::vector<int> evkid; int evn;   // per-launch events of the last timed step
   double kms[32]; int kcnt[32];                                       // per-kernel totals of the last timed step
@@ -183,6 +184,7 @@ extern "C" int cales_create(const cales_params* p, cales_solver** out) {
   s->pblock = dim3(32, 8, 1);
   s->pgrid = dim3((nx + 31) / 32, (ny + 7) / 8, nz);
   s->fresh = false; s->timing = 0; s->ev_valid = false; s->launches = 0; s->evn = 0;
+  s->use_graph = 1; s->gexec = nullptr; s->gdt = 0.0;
   for (int q = 0; q < 32; ++q) { s->kms[q] = 0.0; s->kcnt[q] = 0; }
   *out = s;
   return CALES_OK;
@@ -201,6 +203,7 @@ extern "C" int cales_create_basic(int nx, int ny, int nz, double lx, double ly, 
 extern "C" int cales_destroy(cales_solver* s) {
   if (!s) return CALES_OK;
   for (cudaEvent_t e : s->evpool) cudaEventDestroy(e);
+  if (s->gexec) cudaGraphExecDestroy(s->gexec);
   delete s;
   return CALES_OK;
 }
@@ -364,14 +367,50 @@ static int substep(cales_solver* s, int rk, double dt) {
   return CALES_OK;
 }
 
+extern "C" int cales_launches_per_step(cales_solver* s);
+
 extern "C" int cales_step(cales_solver* s, double dt) {
   if (!s || !(dt > 0.0)) return fail(CALES_EINVAL, "bad step arguments");
   int rc;
   s->launches = 0; s->evn = 0; s->ev_valid = false;
   if (!s->fresh && (rc = refresh_closures(s))) return rc;
+  // Launch-bound sizes (configs 1-2: ~25-40 launches of a few microseconds each): replay the three substeps as one CUDA
+  // graph.  The graph is captured on first use for a given dt (kernel arguments are baked in) and re-captured when dt
+  // changes; per-kernel timing needs the individual launches, so it bypasses the graph.
+  if (s->use_graph && !s->timing) {
+    if (s->gexec && s->gdt == dt) {
+      CUDA_TRY(cudaGraphLaunch(s->gexec, s->st));
+      s->launches = cales_launches_per_step(s);
+      return CALES_OK;
+    }
+    if (s->gexec) { cudaGraphExecDestroy(s->gexec); s->gexec = nullptr; }
+    cudaGraph_t g = nullptr;
+    if (cudaStreamBeginCapture(s->st, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+      rc = CALES_OK;
+      for (int rk = 0; rk < 3 && rc == CALES_OK; ++rk) rc = substep(s, rk, dt);
+      const cudaError_t ee = cudaStreamEndCapture(s->st, &g);
+      if (rc == CALES_OK && ee == cudaSuccess && g && cudaGraphInstantiate(&s->gexec, g, 0) == cudaSuccess) {
+        cudaGraphDestroy(g);
+        s->gdt = dt;
+        CUDA_TRY(cudaGraphLaunch(s->gexec, s->st));
+        return CALES_OK;
+      }
+      if (g) cudaGraphDestroy(g);
+      s->gexec = nullptr; s->use_graph = 0;      // capture unavailable: plain launches from now on
+      cudaGetLastError();
+      if (rc) return rc;
+    } else { s->use_graph = 0; cudaGetLastError(); }
+  }
   tick(s, -1);
   for (int rk = 0; rk < 3; ++rk) if ((rc = substep(s, rk, dt))) return rc;
   s->ev_valid = s->timing != 0;
+  return CALES_OK;
+}
+
+extern "C" int cales_set_graph(cales_solver* s, int on) {
+  if (!s) return fail(CALES_EINVAL, "null solver");
+  s->use_graph = on ? 1 : 0;
+  if (!on && s->gexec) { cudaGraphExecDestroy(s->gexec); s->gexec = nullptr; }
   return CALES_OK;
 }
 

@@ -176,6 +176,7 @@ static inline int build_setup(const cales_params* p, HostSetup& H) {
     int L = 4096 / n2; if (L < 1) L = 1; if (L > 64) L = 64;
     const long long nlines = (long long)ny * nz; if (L > nlines) L = (int)nlines;
     while (L > 1 && threads_for((long long)L * n2, H.plx) > 256) --L;
+    while (L > 1 && (nlines + L - 1) / L < 2 * 148) --L;            // small grids: at least two CTAs per SM if there is work for them
     H.xB = L; H.x_smem = (size_t)L * sm_line(n2) * 16;
     H.x_threads = threads_for((long long)L * n2, H.plx);
   }
@@ -184,6 +185,7 @@ static inline int build_setup(const cales_params* p, HostSetup& H) {
     int tish = 5;                                                   // TI = 32 columns ...
     while (tish > 3 && (long long)(1 << tish) * n2 > 4096) --tish;   // ... down to 8 (64-byte row segments) for long lines
     while (tish > 0 && (1 << tish) > nx) --tish;
+    while (tish > 3 && (long long)((nx + (1 << tish) - 1) >> tish) * nz < 2 * 148) --tish;
     while (tish > 0 && (threads_for((long long)(1 << tish) * n2, H.ply) > 512 || (size_t)(1 << tish) * n2 * 16 > 200 * 1024)) --tish;
     H.yTI = 1 << tish; H.y_tish = tish; H.y_smem = (size_t)(1 << tish) * n2 * 16; if (H.y_smem < 16) H.y_smem = 16;
     H.y_threads = threads_for((long long)(1 << tish) * n2, H.ply);

@@ -263,3 +263,24 @@ def test_full_size_properties(gpu, n):
         fm = f[k, 1:-1, 1:-1] - (f.sum(dim=(1, 2)) * dz).sum() / (p["nx"] * p["ny"] * p["lz"])   # the solve drops the mean of f
         assert float((lap - fm).abs().max()) <= 1e-9 * float(f.abs().max())
     g.close()
+
+
+def test_cuda_graph_replay_is_bit_identical(oracle, gpu):
+    """cales_step as one CUDA graph (non-default stream) against plain launches: same kernels, same order, same bits."""
+    import torch
+    cfg, kw, (u, v, w), dt = pc.prepare(oracle, 2, (48, 24, 16))
+    res = []
+    for graph in (False, True):
+        st = torch.cuda.Stream()
+        with torch.cuda.stream(st):
+            g = pc.make(lambda *a, **k: gpu.Solver(*a, stream=st, **k), kw)
+            g.set_graph(graph)
+            g.set_velocity(u, v, w)
+            for _ in range(4):
+                g.step(dt)
+            g.step(0.5 * dt)            # a new dt forces a re-capture
+            st.synchronize()
+            res.append(_gpu_fields(g))
+            g.close()
+    for a, b in zip(*res):
+        assert np.array_equal(a, b)
