@@ -11,6 +11,7 @@
 #include "cales_momentum.cuh"
 #include "cales_rhs_tile.cuh"
 #include "cales_closures.cuh"
+#include "cales_smag_tile.cuh"
 #include "cales_host.h"
 
 #include <cmath>
@@ -179,6 +180,7 @@ extern "C" int cales_create(const cales_params* p, cales_solver** out) {
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fft2_x_inv, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fft2_y, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rhs_tile, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(RT_SMEM_DOUBLES * sizeof(double)));
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_smag_tile, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(ST_SMEM_DOUBLES * sizeof(double)));
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dsm_pass1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(DSM_SMEM_DOUBLES * sizeof(double)));
   if (e != cudaSuccess) { delete s; return fail(CALES_ECUDA, std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e)); }
   s->pblock = dim3(32, 8, 1);
@@ -286,7 +288,9 @@ static int run_eddy_viscosity(cales_solver* s, const double* u, const double* v,
     k_fill<<<1184, 256, 0, s->st>>>(nut, s->N, 0.0);
     LAUNCH_TRY(K_FILL);
   } else if (s->c.sgs == CALES_SGS_SMAG) {
-    k_smag<<<s->pgrid, s->pblock, 0, s->st>>>(s->c, u, v, w, nut);
+    const int kz = rt_chunk(s->c.nx, s->c.ny, s->c.nz);
+    const dim3 g((s->c.nx + RT_TX - 1) / RT_TX, (s->c.ny + RT_TY - 1) / RT_TY, (s->c.nz + kz - 1) / kz);
+    k_smag_tile<<<g, RT_THREADS, ST_SMEM_DOUBLES * sizeof(double), s->st>>>(s->c, u, v, w, kz, nut);
     LAUNCH_TRY(K_SMAG);
   } else {
     // pass 1: the column-marching kernel wherever the test filter is uniform in y; the tile kernel (Eq. 9 literally) on

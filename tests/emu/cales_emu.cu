@@ -11,6 +11,7 @@
 #include "../../paper_2411_09364_b200/csrc/cales_poisson.cuh"
 #include "../../paper_2411_09364_b200/csrc/cales_momentum.cuh"
 #include "../../paper_2411_09364_b200/csrc/cales_rhs_tile.cuh"
+#include "../../paper_2411_09364_b200/csrc/cales_smag_tile.cuh"
 
 #include <cstring>
 #include <vector>
@@ -153,7 +154,22 @@ static void emu_nut(emu_solver* s, const double* u, const double* v, const doubl
   const Ctx& c = s->c;
   if (c.sgs == 0) { for (long long n = 0; n < s->N; ++n) nut[n] = 0.0; return; }
   if (c.sgs == 1) {
-    for (int k = 0; k < c.nz; ++k) for (int j = 0; j < c.ny; ++j) for (int i = 0; i < c.nx; ++i) nut[idx3(c, i, j, k)] = smag_point(c, u, v, w, i, j, k);
+    // k_smag_tile: stage the three halo planes with the kernel's staging rule (st_elem), evaluate through the tile accessor
+    std::vector<double> ring(3 * ST_NF * RT_PLANE);
+    for (int j0 = 0; j0 < c.ny; j0 += RT_TY) for (int i0 = 0; i0 < c.nx; i0 += RT_TX) for (int k = 0; k < c.nz; ++k) {
+      for (int d = 0; d < 3; ++d) for (int f = 0; f < ST_NF; ++f) for (int pos = 0; pos < RT_PLANE; ++pos) {
+        const int ry = pos / RT_TW, rx = pos % RT_TW, gi = i0 - 1 + rx, gj = j0 - 1 + ry;
+        ring[(d * ST_NF + f) * RT_PLANE + pos] = (gi <= c.nx && gj <= c.ny) ? st_elem(c, u, v, w, f, gi, gj, k - 1 + d) : 0.0;
+      }
+      const double* sl[3] = {ring.data(), ring.data() + ST_NF * RT_PLANE, ring.data() + 2 * ST_NF * RT_PLANE};
+      for (int ly = 0; ly < RT_TY; ++ly) for (int tx = 0; tx < RT_TX; ++tx) {
+        const int i = i0 + tx, j = j0 + ly;
+        if (i >= c.nx || j >= c.ny) continue;
+        double tauw[2] = {0.0, 0.0};
+        if (c.van_driest) smag_wall_shear(c, u, v, i, j, tauw);
+        nut[idx3(c, i, j, k)] = smag_tile_point(c, sl, (ly + 1) * RT_TW + tx + 1, k, tauw);
+      }
+    }
     return;
   }
   const DsmShape dsh = dsm_shape(c.nx);
