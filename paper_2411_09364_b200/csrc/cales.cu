@@ -50,6 +50,7 @@ struct cales_solver {
   dim3 pgrid, pblock;   // point kernels
   long long nblk;
   bool fresh;
+  long long tile_min;   // grids with at least this many points use the staged z-march for the static model
   int use_graph; cudaGraphExec_t gexec; double gdt;   // the three substeps captured as one CUDA graph, keyed by dt
   int timing; bool ev_valid;
   std::vector<cudaEvent_t> evpool; std::vector<int> evkid; int evn;   // per-launch events of the last timed step
@@ -187,6 +188,8 @@ extern "C" int cales_create(const cales_params* p, cales_solver** out) {
   s->pgrid = dim3((nx + 31) / 32, (ny + 7) / 8, nz);
   s->fresh = false; s->timing = 0; s->ev_valid = false; s->launches = 0; s->evn = 0;
   s->use_graph = 1; s->gexec = nullptr; s->gdt = 0.0;
+  s->tile_min = 4000000;
+  if (const char* e = std::getenv("CALES_TILE_MIN_POINTS")) s->tile_min = std::atoll(e);   // tests force either path
   for (int q = 0; q < 32; ++q) { s->kms[q] = 0.0; s->kcnt[q] = 0; }
   *out = s;
   return CALES_OK;
@@ -288,9 +291,11 @@ static int run_eddy_viscosity(cales_solver* s, const double* u, const double* v,
     k_fill<<<1184, 256, 0, s->st>>>(nut, s->N, 0.0);
     LAUNCH_TRY(K_FILL);
   } else if (s->c.sgs == CALES_SGS_SMAG) {
-    const int kz = rt_chunk(s->c.nx, s->c.ny, s->c.nz);
-    const dim3 g((s->c.nx + RT_TX - 1) / RT_TX, (s->c.ny + RT_TY - 1) / RT_TY, (s->c.nz + kz - 1) / kz);
-    k_smag_tile<<<g, RT_THREADS, ST_SMEM_DOUBLES * sizeof(double), s->st>>>(s->c, u, v, w, kz, nut);
+    if (s->N >= s->tile_min) {      // HBM-sized grids: staged z-march; launch-bound sizes: one thread per point
+      const int kz = rt_chunk(s->c.nx, s->c.ny, s->c.nz);
+      const dim3 g((s->c.nx + RT_TX - 1) / RT_TX, (s->c.ny + RT_TY - 1) / RT_TY, (s->c.nz + kz - 1) / kz);
+      k_smag_tile<<<g, RT_THREADS, ST_SMEM_DOUBLES * sizeof(double), s->st>>>(s->c, u, v, w, kz, nut);
+    } else k_smag<<<s->pgrid, s->pblock, 0, s->st>>>(s->c, u, v, w, nut);
     LAUNCH_TRY(K_SMAG);
   } else {
     // pass 1: the column-marching kernel wherever the test filter is uniform in y; the tile kernel (Eq. 9 literally) on

@@ -22,7 +22,7 @@ struct Ctx {
   int wm_maxit;
   long long N;     // nx*ny*nz
   long long nxy;   // nx*ny
-  double dx, dy, rdx, rdy, lz, nu, cs, aplus, alpha, kappa, Blog, h_wm, wm_tol, u_bulk;
+  double dx, dy, rdx, rdy, rnuap /* 1/(nu A+) */, lz, nu, cs, aplus, alpha, kappa, Blog, h_wm, wm_tol, u_bulk;
   // 1-D grid tables in device memory, offset so that the ghost entries are addressable:
   const double* dzf;   // dzf[-1 .. nz]   cell heights (ghost = neighbour's / wrapped)
   const double* dzc;   // dzc[-1 .. nz-1] centre spacings across face k+1 (mirrored ghost centre at walls)

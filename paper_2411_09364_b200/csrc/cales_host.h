@@ -149,7 +149,7 @@ static inline int build_setup(const cales_params* p, HostSetup& H) {
   c.nx = nx; c.ny = ny; c.nz = nz; c.N = (long long)nx * ny * nz; c.nxy = (long long)nx * ny;
   c.bc_y = p->bc_y; c.bc_z = p->bc_z; c.wall_model = p->wall_model; c.sgs = p->sgs_model; c.van_driest = p->van_driest;
   c.implicit_z = p->implicit_z; c.dsm_plane = p->dsm_avg_xy_plane; c.dsm_clip_total = p->dsm_clip_total; c.const_flow_rate = p->const_flow_rate;
-  c.wm_maxit = H.P.wm_maxit; c.dx = dx; c.dy = dy; c.rdx = 1.0 / dx; c.rdy = 1.0 / dy; c.lz = p->lz; c.nu = p->nu; c.cs = p->cs; c.aplus = H.P.aplus;
+  c.wm_maxit = H.P.wm_maxit; c.dx = dx; c.dy = dy; c.rdx = 1.0 / dx; c.rdy = 1.0 / dy; c.lz = p->lz; c.nu = p->nu; c.cs = p->cs; c.aplus = H.P.aplus; c.rnuap = 1.0 / (p->nu * H.P.aplus);
   c.alpha = p->dsm_alpha2d > 0.0 ? p->dsm_alpha2d : std::cbrt(4.0);
   c.kappa = H.P.kappa; c.Blog = p->B; c.h_wm = p->h_wm; c.wm_tol = H.P.wm_tol; c.u_bulk = p->u_bulk;
   c.dzf = nullptr; c.dzc = nullptr; c.zc = nullptr; c.rdzf = nullptr; c.rdzc = nullptr; c.delta = nullptr; c.tau = nullptr;

@@ -20,7 +20,7 @@ CALES_HD double st_elem(const Ctx& c, const double* u, const double* v, const do
 }
 
 // nu_t at one point from three staged planes (sl[d] -> field 0 of plane k-1+d; ctr as in TileAcc);
-// utau2[0], utau2[1]: nu * |u_c| / d1 at the bottom / top wall below / above this column (van Driest only, S5)
+// tauw[0], tauw[1]: u_tau = sqrt(nu |u_c| / d1) at the bottom / top wall of this column (van Driest only, S5)
 CALES_HD double smag_tile_point(const Ctx& c, const double* const* sl, int ctr, int k, const double* tauw) {
   auto at = [&](int f, int a, int b, int d) { return sl[d + 1][f * RT_PLANE + ctr + b * RT_TW + a]; };
   auto U = [&](int a, int b, int d) { return at(0, a, b, d); };
@@ -32,21 +32,21 @@ CALES_HD double smag_tile_point(const Ctx& c, const double* const* sl, int ctr, 
   if (c.van_driest) {
     const double db = c.zc[k], dt = c.lz - c.zc[k];
     const double d = (db <= dt) ? db : dt;
-    const double utau = sqrt((db <= dt) ? tauw[0] : tauw[1]);
-    D = 1.0 - exp(-(d * utau / c.nu) / c.aplus);
+    const double utau = (db <= dt) ? tauw[0] : tauw[1];          // u_tau of the nearer wall (precomputed per column)
+    D = 1.0 - exp(-(d * utau) * c.rnuap);
   }
   const double l = c.cs * c.delta[k] * D;
   return l * l * smag;
 }
 
-// local wall shear of the van Driest damping for column (i,j): tauw[0] bottom, tauw[1] top (same formula as smag_point)
+// local friction velocity of the van Driest damping for column (i,j): tauw[0] bottom, tauw[1] top (as in smag_point)
 CALES_HD void smag_wall_shear(const Ctx& c, const double* u, const double* v, int i, int j, double* tauw) {
   for (int wl = 0; wl < 2; ++wl) {
     const int kw = wl == 0 ? 0 : c.nz - 1;
     const double d1 = wl == 0 ? c.zc[0] : c.lz - c.zc[c.nz - 1];
     const double uc = 0.5 * (velg<0>(c, u, i - 1, j, kw, GH_STRAIN) + velg<0>(c, u, i, j, kw, GH_STRAIN));
     const double vc = 0.5 * (velg<1>(c, v, i, j - 1, kw, GH_STRAIN) + velg<1>(c, v, i, j, kw, GH_STRAIN));
-    tauw[wl] = c.nu * sqrt(uc * uc + vc * vc) / d1;
+    tauw[wl] = sqrt(c.nu * sqrt(uc * uc + vc * vc) / d1);        // u_tau = sqrt(tau_w)
   }
 }
 

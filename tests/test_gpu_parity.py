@@ -284,3 +284,19 @@ def test_cuda_graph_replay_is_bit_identical(oracle, gpu):
             g.close()
     for a, b in zip(*res):
         assert np.array_equal(a, b)
+
+
+@pytest.mark.parametrize("n,shape", [(1, (48, 24, 20)), (3, (72, 36, 40)), (2, (72, 48, 24))])
+def test_static_model_staged_kernel_parity(oracle, gpu, n, shape, monkeypatch):
+    """k_smag_tile (the staged z-march used on HBM-sized grids) forced on at test sizes."""
+    monkeypatch.setenv("CALES_TILE_MIN_POINTS", "0")
+    cfg, kw, (u, v, w), dt = pc.prepare(oracle, n, shape)
+    o = pc.make(oracle.Oracle, kw)
+    g = pc.make(gpu.Solver, kw)
+    o.set_velocity(u, v, w); g.set_velocity(u, v, w)
+    a, b = g.eddy_viscosity().cpu().numpy(), o.eddy_viscosity()
+    assert np.max(np.abs(a - b)) <= 1e-11 * max(np.max(np.abs(b)), kw["nu"])
+    o.step(dt); g.step(dt)
+    err = pc.field_errors(_gpu_fields(g), [o.get(f) for f in range(5)], o.dzf, kw["nu"])
+    assert max(err.values()) <= TOL_1STEP, err
+    g.close()
