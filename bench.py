@@ -39,6 +39,16 @@ ALGO_BYTES = {
 }
 
 
+# fp64 operations per grid point of the one kernel that is bound by the plain fp64 ALUs (ncu op counts of round 1,
+# profiles/r1_ncu_full.md: 0.30 DADD + 0.35 DMUL + 0.30 DFMA of 315 fp64 instructions per point; an FMA counts 2).
+ALGO_FLOPS = {"k_dsm_col": 415.0}
+# B200 plain fp64 peak derived in DESIGN.md section 4: 148 SMs x 64 FMA lanes x 2 flop x 1.965 GHz
+FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture (profiles/r1_ncu_full.md),
+# keyed by (config, kernel); None where no capture of that kernel at that size is committed.
+NCU_TRAFFIC = {(5, "k_dsm_col"): 56.2e9, (5, "k_rhs"): 98.8e9, (5, "k_correct"): 63.9e9, (5, "k_poisson_z"): 37.0e9}
+
+
 def measured_peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -258,7 +268,7 @@ def run_ours(args):
     value = aggregate_value(npts, K, world, ms)
 
     # ---- e2e: the same metric through the C ABI with HOST buffers, copies inside the timed region
-    Ke = max(1, min(K, 3))
+    Ke = max(1, min(K, 3)) if not args.no_e2e else 0
     hosts = [torch.from_numpy(a) for a in (u, v, w, p_host)]
     def e2e_step():
         for f in range(3):
@@ -266,7 +276,8 @@ def run_ours(args):
         s.step(dt)
         for f in range(4):
             s.get_field(f, hosts[f])            # D2H of the step's result
-    e2e_step()                                  # warm-up
+    if Ke:
+        e2e_step()                              # warm-up
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
@@ -276,7 +287,7 @@ def run_ours(args):
     torch.cuda.synchronize()
     te = time.perf_counter() - t0
     te = max_over_ranks(te, "cuda")
-    e2e = {"value": aggregate_value(npts, Ke, world, te * 1e3), "unit": UNIT, "h2d_bytes_per_step": 3 * npts * 8, "d2h_bytes_per_step": 4 * npts * 8,
+    e2e = None if not Ke else {"value": aggregate_value(npts, Ke, world, te * 1e3), "unit": UNIT, "h2d_bytes_per_step": 3 * npts * 8, "d2h_bytes_per_step": 4 * npts * 8,
            "steps": Ke, "ms_per_step": 1e3 * te / Ke, "host_memory": "pinned (cudaHostRegister)" if pinned else "pageable",
            "note": "each step: cales_set_field(u,v,w) from host, cales_step, cales_get_field(u,v,w,p) to host; a new velocity makes "
                    "the library re-evaluate the wall stress and nu_t first"}
@@ -297,8 +308,13 @@ def run_ours(args):
     if top:
         r = kernels[top]
         roofline = {"kernel": top, "bound": "hbm", "achieved": r["achieved_gbs"], "peak": peak, "unit": "GB/s", "frac": r["frac"],
-                    "traffic": None, "peak_source": peak_src, "algo_bytes_per_launch": ALGO_BYTES[top] * npts,
+                    "traffic": NCU_TRAFFIC.get((cfg_no, top)), "peak_source": peak_src, "algo_bytes_per_launch": ALGO_BYTES[top] * npts,
                     "ms_per_launch": r["ms_per_launch"], "share_of_step": r["share_of_step"]}
+        if top in ALGO_FLOPS:        # bound by the plain fp64 ALUs, not by HBM: report it against that peak
+            tf = ALGO_FLOPS[top] * npts / (r["ms_per_launch"] * 1e-3) / 1e12
+            roofline.update({"bound": "alu", "achieved": tf, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": tf / FP64_PEAK_TFLOPS,
+                             "peak_source": "derived: 148 SMs x 64 fp64 FMA lanes x 2 x 1.965 GHz (DESIGN.md section 4)",
+                             "algo_flops_per_launch": ALGO_FLOPS[top] * npts, "hbm_frac_of_measured_peak": r["frac"]})
     # whole-step algorithmic traffic: the sum over the step's launches of the table above
     step_bytes = sum(ALGO_BYTES.get(n, 0.0) * (a[1] // K) for n, a in ktot.items()) * npts
     step_gbs = step_bytes / (ms / K * 1e-3) / 1e9
@@ -316,14 +332,38 @@ def run_ours(args):
             "e2e": e2e, "gpu_launches": launches, "clocks": clocks, "roofline": roofline, "kernels": kernels,
             "diagnostics": {k: diag[k] for k in ("max_div", "u_bulk", "kinetic_energy", "wm_max_iters", "nan_count")},
             "input_generation_s": t_gen}
+    s.close()
+    del s
+    torch.cuda.empty_cache()
+    if world > 1:
+        dist.destroy_process_group()
     if rank == 0:
         if not args.no_cpu_baseline and world == 1:
             r = oracle_leg(cfg_no, 2, 1)
             line["cpu_baseline"] = {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")}
+        if not args.no_other_configs and world == 1:
+            # north_star: all five workloads at 1 GPU.  The other four run as short child processes of this same script
+            # (device-resident timing only) after this process has released its device memory.
+            for a in (u, v, w, p_host):
+                torch.cuda.cudart().cudaHostUnregister(a.ctypes.data)
+            del hosts, u, v, w, p_host
+            others = {}
+            for cno in (1, 2, 3, 4, 5):
+                if cno == cfg_no:
+                    continue
+                cmd = [sys.executable, os.path.abspath(__file__), "--config", str(cno), "--steps", "5", "--warmup", "3",
+                       "--no-cpu-baseline", "--no-other-configs", "--no-e2e"]
+                try:
+                    out = subprocess.run(cmd, capture_output=True, text=True, timeout=600)
+                    d = json.loads(out.stdout.strip().splitlines()[-1])
+                    others["config %d" % cno] = {"workload": d["config"]["workload"], "value": d["value"], "unit": UNIT,
+                                                 "ms_per_step": d["ms_per_step"], "launch": d["config"]["launch"], "l2": d["config"]["l2"],
+                                                 "step_hbm_frac_of_measured_peak": d["step_hbm"]["frac_of_measured_peak"],
+                                                 "top_kernels": {k: round(v["share_of_step"], 3) for k, v in list(d["kernels"].items())[:3]}}
+                except Exception as e:      # a failed side run must not lose the main line
+                    others["config %d" % cno] = {"error": repr(e)[:200]}
+            line["other_configs"] = others
         print(json.dumps(line), flush=True)
-    s.close()
-    if world > 1:
-        dist.destroy_process_group()
 
 
 def main():
@@ -334,6 +374,8 @@ def main():
     ap.add_argument("--config", type=int, default=0, help="BASELINE.json config 1..5 (default: 5 if it fits, else 4)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-other-configs", action="store_true", help="skip the short side runs of the other four workloads")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg")
     args = ap.parse_args()
     if args.impl == "reference":
         if not args.config:
