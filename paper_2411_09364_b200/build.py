@@ -27,7 +27,8 @@ def nvcc():
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in _deps()):
         return LIB
-    cmd = [nvcc()] + NVCC_FLAGS + ["-o", LIB] + SOURCES
+    extra = os.environ.get("CALES_NVCC_EXTRA", "").split()      # experiments only (e.g. -DCALES_F2_E=8)
+    cmd = [nvcc()] + NVCC_FLAGS + extra + ["-o", LIB] + SOURCES
     r = subprocess.run(cmd, capture_output=True, text=True)
     if verbose or r.returncode != 0:
         sys.stderr.write(r.stdout + r.stderr)

@@ -81,7 +81,7 @@ CALES_HD double scalg(const Ctx& c, const double* __restrict__ q, int i, int j, 
   return s * q[idx3(c, i, j, k)];
 }
 
-// True when none of the neighbours of (.,j,k) read by rhs_point / the strain rate needs a wall ghost: periodic wrap is
+// True when none of the neighbours of (.,j,k) read by the momentum / strain-rate stencils needs a wall ghost: periodic wrap is
 // plain index arithmetic, wall rows/planes go through the generic accessors.  Relies on the library keeping the wall
 // faces v[.][ny-1][.] and w[nz-1] at exactly 0 (cales_set_field zeroes them).
 CALES_HD bool interior_row(const Ctx& c, int j, int k) {

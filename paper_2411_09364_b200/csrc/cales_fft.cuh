@@ -6,13 +6,13 @@
 //   a real line x[0..n-1] (n even) -> h[0] = X[0], h[1] = X[n/2], h[2m] = Re X[m], h[2m+1] = Im X[m], 0<m<n/2,
 //   X[m] = sum_j x[j] exp(-2 pi i m j / n).  Re and Im of an x-mode transform independently along y.
 //   Neumann (wall) y: DCT-II  X[n] = sum_j x[j] cos(pi n (2j+1)/(2N)), row n holds mode n; inverse DCT-III.
-// A real transform of length n is one complex Stockham FFT of length n2 = n/2 (radix 4/2/3 passes, ping-pong
-// in shared memory) on z[t] = x[2t] + i x[2t+1] plus a split/merge pass; the DCT adds the even/odd
-// permutation and a quarter-wave twiddle.  All twiddles come from host-built fp64 tables.
+// A real transform of length n is one complex Stockham FFT of length n2 = n/2 on z[t] = x[2t] + i x[2t+1] plus a
+// split (forward) or merge (inverse) step; the DCT adds the even/odd permutation and a quarter-wave twiddle.  All
+// twiddles come from host-built tables (long double, rounded once).  This header holds the plan, the small in-register
+// DFTs (radix 2, 3, 4, 8, 16), the forward split and the standalone tiled transpose; the kernels are in cales_fft2.cuh.
 //
-// Every phase is a __host__ __device__ function of (tid, nth) so that the identical code can be stepped
-// phase by phase on the host by the test emulator (tests/emu); __syncthreads() sits between phases in the
-// __global__ wrappers only.
+// Every phase is a __host__ __device__ function of (tid, nth) so that the identical code can be stepped phase by
+// phase on the host by the test emulator (tests/emu); __syncthreads() sits between phases in the kernels only.
 #pragma once
 #include "cales_common.cuh"
 
@@ -105,48 +105,6 @@ template <int R> CALES_HD void dft_small(double2* v, int s) {
   else dft16(v, s);
 }
 
-// One Stockham radix-R pass over all B lines: out <- pass(in).  sign = -1 forward, +1 inverse.  Each butterfly lives in
-// registers; the inter-pass twiddles w^(t k) come from the table for t = 1, 2, 3 and by products above.
-template <int R>
-CALES_HD void fft_pass_r(int tid, int nth, const double2* in, double2* out, const SmView& sv, const FftPlan& pl, int Ns, int sign) {
-  const int n2 = pl.n2, per = n2 / R, total = per * sv.B;
-  const int tws = pl.n / (Ns * R);
-  for (int idx = tid; idx < total; idx += nth) {
-    int b, j;
-    if (sv.bfast) { b = idx % sv.B; j = idx / sv.B; } else { j = idx % per; b = idx / per; }
-    const int k = j % Ns;
-    const int j0 = (j - k) * R + k;
-    double2 v[R];
-#pragma unroll
-    for (int t = 0; t < R; ++t) v[t] = in[sm_off(sv, b, j + t * per)];
-    if (k != 0) {
-      double2 w[R];
-      w[1] = pl.tw[k * tws];
-      if (R > 2) w[2] = pl.tw[2 * k * tws];
-      if (R > 3) w[3] = pl.tw[3 * k * tws];
-      if (R > 4) { w[4] = cmul(w[2], w[2]); w[5] = cmul(w[4], w[1]); w[6] = cmul(w[4], w[2]); w[7] = cmul(w[4], w[3]); }
-      if (R > 8) {
-        w[8] = cmul(w[4], w[4]); w[9] = cmul(w[8], w[1]); w[10] = cmul(w[8], w[2]); w[11] = cmul(w[8], w[3]);
-        w[12] = cmul(w[8], w[4]); w[13] = cmul(w[12], w[1]); w[14] = cmul(w[12], w[2]); w[15] = cmul(w[12], w[3]);
-      }
-#pragma unroll
-      for (int t = 1; t < R; ++t) v[t] = sign < 0 ? cmul(v[t], w[t]) : cmulc(v[t], w[t]);
-    }
-    dft_small<R>(v, sign);
-#pragma unroll
-    for (int t = 0; t < R; ++t) out[sm_off(sv, b, j0 + t * Ns)] = v[t];
-  }
-}
-CALES_HD void fft_pass(int tid, int nth, const double2* in, double2* out, const SmView& sv, const FftPlan& pl, int Ns, int R, int sign) {
-  switch (R) {
-    case 2: fft_pass_r<2>(tid, nth, in, out, sv, pl, Ns, sign); break;
-    case 3: fft_pass_r<3>(tid, nth, in, out, sv, pl, Ns, sign); break;
-    case 4: fft_pass_r<4>(tid, nth, in, out, sv, pl, Ns, sign); break;
-    case 8: fft_pass_r<8>(tid, nth, in, out, sv, pl, Ns, sign); break;
-    default: fft_pass_r<16>(tid, nth, in, out, sv, pl, Ns, sign); break;
-  }
-}
-
 // ---- forward split: Z (complex FFT of the packed line) -> half-complex X[m]; thread handles (b, m), m = 0..n2-1.
 // Returns through `emit(b, slotA, valA, slotB, valB)`: two real outputs per (b, m).
 //   FFT mode: slots (2m, 2m+1) (m = 0: X[0], X[n2]).
@@ -177,37 +135,6 @@ CALES_HD void split_forward(int tid, int nth, const double2* Z, const SmView& sv
   }
 }
 
-// ---- inverse merge: raw staged reals (as double2 pairs: real index r lives in H(b, r/2).{x,y}) -> Z[m].
-CALES_HD double sm_real(const double2* H, const SmView& sv, int b, int r) {
-  const double2 v = H[sm_off(sv, b, r >> 1)];
-  return (r & 1) ? v.y : v.x;
-}
-CALES_HD double2 hc_mode(const double2* H, const SmView& sv, const FftPlan& pl, bool dct, int b, int m) {
-  // X[m] (FFT mode) or V[m] (DCT mode: V[m] = conj(w_m) (X[m] - i X[N-m]), X[N] = 0), 0 <= m <= n2
-  const int n2 = pl.n2;
-  if (!dct) {
-    if (m == 0) return make_double2(sm_real(H, sv, b, 0), 0.0);
-    if (m == n2) return make_double2(sm_real(H, sv, b, 1), 0.0);
-    return H[sm_off(sv, b, m)];
-  }
-  if (m == 0) return make_double2(sm_real(H, sv, b, 0), 0.0);
-  const double2 q = make_double2(sm_real(H, sv, b, m), -sm_real(H, sv, b, pl.n - m));
-  return cmulc(q, pl.dctw[m]);
-}
-CALES_HD void merge_inverse(int tid, int nth, const double2* H, double2* Z, const SmView& sv, const FftPlan& pl, bool dct) {
-  const int n2 = pl.n2, total = n2 * sv.B;
-  for (int idx = tid; idx < total; idx += nth) {
-    int b, m;
-    if (sv.bfast) { b = idx % sv.B; m = idx / sv.B; } else { m = idx % n2; b = idx / n2; }
-    const double2 xm = hc_mode(H, sv, pl, dct, b, m);
-    double2 xc = hc_mode(H, sv, pl, dct, b, n2 - m); xc.y = -xc.y;
-    const double2 e = make_double2(0.5 * (xm.x + xc.x), 0.5 * (xm.y + xc.y));
-    const double2 d = make_double2(0.5 * (xm.x - xc.x), 0.5 * (xm.y - xc.y));
-    const double2 o = cmulc(d, pl.tw[m]);   // conj(W^m) * d
-    Z[sm_off(sv, b, m)] = make_double2(e.x - o.y, e.y + o.x);   // e + i o
-  }
-}
-
 // position in the packed complex line of real sample r of the (possibly DCT-permuted) input:
 //   FFT: v = x.   DCT-II: v[q] = x[2q] (q < N/2), v[N-1-q'] = x[2q'+1].
 CALES_HD int perm_fwd(int r, int n, bool dct) {
@@ -224,163 +151,7 @@ struct DivSrc { const double* us; const double* vs; const double* ws; double inv
 
 CALES_HD double2 ld2(const double* p, int t) { return reinterpret_cast<const double2*>(p)[t]; }
 
-// load B lines starting at line l0 into buf (as packed complex); DIV: build f = div(u*)/(gamma dt) on the fly
-template <bool DIV>
-CALES_HD void fx_load(int tid, int nth, const Ctx& c, const FftPlan& pl, int B, long long l0, int nb, const double* src, const DivSrc& ds, double2* buf) {
-  const int n = pl.n, n2 = pl.n2;
-  for (int idx = tid; idx < B * n2; idx += nth) {
-    const int b = idx / n2, t = idx % n2;
-    double2 z = make_double2(0.0, 0.0);
-    if (b < nb) {
-      const long long l = l0 + b;
-      if (!DIV) z = ld2(src + l * n, t);
-      else {
-        const int j = (int)(l % c.ny), k = (int)(l / c.ny);
-        const double* ul = ds.us + l * n;
-        const double* vl = ds.vs + l * n;
-        const double* wl = ds.ws + l * n;
-        // neighbours of the line: v(j-1), w(k-1); ghosts by the boundary conditions of u*
-        const double* vm = nullptr; const double* wm = nullptr;
-        if (j > 0) vm = vl - n; else if (c.bc_y == BC_PER) vm = vl + (long long)(c.ny - 1) * n;
-        if (k > 0) wm = wl - c.nxy; else if (c.bc_z == BC_PER) wm = wl + (long long)(c.nz - 1) * c.nxy;
-        const double rdx = c.rdx, rdy = c.rdy, rdz = c.rdzf[k];
-        const double2 uu = ld2(ul, t);
-        const double um = ul[t == 0 ? n - 1 : 2 * t - 1];
-        const double2 vv = ld2(vl, t);
-        const double2 vvm = vm ? ld2(vm, t) : make_double2(0.0, 0.0);
-        const double2 ww = ld2(wl, t);
-        const double2 wwm = wm ? ld2(wm, t) : make_double2(0.0, 0.0);
-        z.x = ((uu.x - um) * rdx + (vv.x - vvm.x) * rdy + (ww.x - wwm.x) * rdz) * ds.inv_gdt;
-        z.y = ((uu.y - uu.x) * rdx + (vv.y - vvm.y) * rdy + (ww.y - wwm.y) * rdz) * ds.inv_gdt;
-      }
-    }
-    buf[b * sm_line(n2) + sm_pad(t)] = z;
-  }
-}
-CALES_HD void fx_store_fwd(int tid, int nth, const FftPlan& pl, int B, long long l0, int nb, const double2* Z, double* dst) {
-  SmView sv{1, sm_line(pl.n2), B, false};
-  const int n = pl.n;
-  split_forward(tid, nth, Z, sv, pl, false, nb, [&](int b, int sa, double va, int sb, double vb) {
-    // FFT mode: slots (2m, 2m+1) are adjacent -> one 16-byte store
-    reinterpret_cast<double2*>(dst + (l0 + b) * n)[sa >> 1] = make_double2(va, vb);
-    (void)sb;
-  });
-}
-CALES_HD void fx_store_inv(int tid, int nth, const FftPlan& pl, int B, long long l0, int nb, const double2* Z, double* dst) {
-  const int n = pl.n, n2 = pl.n2;
-  const double sc = 1.0 / (double)n2;
-  for (int idx = tid; idx < B * n2; idx += nth) {
-    const int b = idx / n2, t = idx % n2;
-    if (b >= nb) continue;
-    const double2 z = Z[b * sm_line(n2) + sm_pad(t)];
-    reinterpret_cast<double2*>(dst + (l0 + b) * n)[t] = make_double2(z.x * sc, z.y * sc);
-  }
-}
-
-// ------------------------------------------------------------------------------------------------------------
-// y transforms: a CTA owns TI adjacent x-columns of one k-plane, stages the [ny][TI] tile in shared memory
-// (the x<->y transpose of the pencil solver, fused into the load and the store), transforms the
-// TI lines of length ny, and writes the tile back in place.  Shared-memory element (b, t) at t*TI + b, so
-// consecutive threads touch consecutive banks in every pass.
-// ------------------------------------------------------------------------------------------------------------
-// load rows (coalesced over b); forward: scatter real sample r to its place in the packed (DCT-permuted) line
-CALES_HD void fy_load(int tid, int nth, const Ctx& c, const FftPlan& pl, int TI, bool dct, bool inverse, const double* base, int nb, double2* buf) {
-  const int n = pl.n;
-  SmView sv{TI, 1, TI, true};
-  double* rb = reinterpret_cast<double*>(buf);
-  for (int idx = tid; idx < TI * n; idx += nth) {
-    const int b = idx % TI, r = idx / TI;
-    const double x = b < nb ? base[(long long)r * c.nx + b] : 0.0;
-    const int q = inverse ? r : perm_fwd(r, n, dct);
-    rb[2 * sm_off(sv, b, q >> 1) + (q & 1)] = x;
-  }
-}
-CALES_HD void fy_store_fwd(int tid, int nth, const Ctx& c, const FftPlan& pl, int TI, bool dct, double* base, int nb, const double2* Z) {
-  SmView sv{TI, 1, TI, true};
-  split_forward(tid, nth, Z, sv, pl, dct, nb, [&](int b, int sa, double va, int sb, double vb) {
-    base[(long long)sa * c.nx + b] = va;
-    base[(long long)sb * c.nx + b] = vb;
-  });
-}
-CALES_HD void fy_store_inv(int tid, int nth, const Ctx& c, const FftPlan& pl, int TI, bool dct, double* base, int nb, const double2* Z) {
-  const int n = pl.n;
-  SmView sv{TI, 1, TI, true};
-  const double* Zr = reinterpret_cast<const double*>(Z);
-  const double sc = 1.0 / (double)pl.n2;
-  for (int idx = tid; idx < TI * n; idx += nth) {
-    const int b = idx % TI, r = idx / TI;
-    if (b >= nb) continue;
-    const int q = perm_fwd(r, n, dct);
-    base[(long long)r * c.nx + b] = Zr[2 * sm_off(sv, b, q >> 1) + (q & 1)] * sc;
-  }
-}
-
 #ifdef __CUDACC__
-// all Stockham passes with a block barrier after each; returns the index (0/1) of the buffer holding the result
-__device__ __forceinline__ int fft_run(int tid, int nth, double2* buf0, double2* buf1, const SmView& sv, const FftPlan& pl, int sign, int start) {
-  int cur = start, Ns = 1;
-  for (int p = 0; p < pl.npass; ++p) {
-    const int R = pl.radix[p];
-    fft_pass(tid, nth, cur ? buf1 : buf0, cur ? buf0 : buf1, sv, pl, Ns, R, sign);
-    __syncthreads();
-    Ns *= R; cur ^= 1;
-  }
-  return cur;
-}
-
-template <bool DIV>
-__global__ void __launch_bounds__(256, 2) k_fft_x_fwd(const __grid_constant__ Ctx c, const __grid_constant__ FftPlan pl, int B, const double* __restrict__ src, DivSrc ds, double* __restrict__ dst) {
-  extern __shared__ double2 smem[];
-  double2* buf0 = smem; double2* buf1 = smem + (size_t)B * sm_line(pl.n2);
-  const long long nlines = (long long)c.ny * c.nz;
-  const long long l0 = (long long)blockIdx.x * B;
-  const int nb = (int)min((long long)B, nlines - l0);
-  SmView sv{1, sm_line(pl.n2), B, false};
-  const int tid = threadIdx.x, nth = blockDim.x;
-  fx_load<DIV>(tid, nth, c, pl, B, l0, nb, src, ds, buf0);
-  __syncthreads();
-  const int cur = fft_run(tid, nth, buf0, buf1, sv, pl, -1, 0);
-  fx_store_fwd(tid, nth, pl, B, l0, nb, cur ? buf1 : buf0, dst);
-}
-
-__global__ void __launch_bounds__(256, 2) k_fft_x_inv(const __grid_constant__ Ctx c, const __grid_constant__ FftPlan pl, int B, const double* __restrict__ src, double* __restrict__ dst) {
-  extern __shared__ double2 smem[];
-  double2* buf0 = smem; double2* buf1 = smem + (size_t)B * sm_line(pl.n2);
-  const long long nlines = (long long)c.ny * c.nz;
-  const long long l0 = (long long)blockIdx.x * B;
-  const int nb = (int)min((long long)B, nlines - l0);
-  SmView sv{1, sm_line(pl.n2), B, false};
-  const int tid = threadIdx.x, nth = blockDim.x;
-  DivSrc none{nullptr, nullptr, nullptr, 0.0};
-  fx_load<false>(tid, nth, c, pl, B, l0, nb, src, none, buf0);
-  __syncthreads();
-  merge_inverse(tid, nth, buf0, buf1, sv, pl, false);
-  __syncthreads();
-  const int cur = fft_run(tid, nth, buf0, buf1, sv, pl, +1, 1);
-  fx_store_inv(tid, nth, pl, B, l0, nb, cur ? buf1 : buf0, dst);
-}
-
-__global__ void __launch_bounds__(512, 1) k_fft_y(const __grid_constant__ Ctx c, const __grid_constant__ FftPlan pl, int TI, int dct, int inverse, double* __restrict__ A) {
-  extern __shared__ double2 smem[];
-  double2* buf0 = smem; double2* buf1 = smem + (size_t)TI * pl.n2;
-  const int i0 = blockIdx.x * TI, k = blockIdx.y;
-  const int nb = min(TI, c.nx - i0);
-  double* base = A + (long long)k * c.nxy + i0;
-  SmView sv{TI, 1, TI, true};
-  const int tid = threadIdx.x, nth = blockDim.x;
-  fy_load(tid, nth, c, pl, TI, dct != 0, inverse != 0, base, nb, buf0);
-  __syncthreads();
-  if (!inverse) {
-    const int cur = fft_run(tid, nth, buf0, buf1, sv, pl, -1, 0);
-    fy_store_fwd(tid, nth, c, pl, TI, dct != 0, base, nb, cur ? buf1 : buf0);
-  } else {
-    merge_inverse(tid, nth, buf0, buf1, sv, pl, dct != 0);
-    __syncthreads();
-    const int cur = fft_run(tid, nth, buf0, buf1, sv, pl, +1, 1);
-    fy_store_inv(tid, nth, c, pl, TI, dct != 0, base, nb, cur ? buf1 : buf0);
-  }
-}
-
 // Tiled shared-memory transpose of every k-plane: dst[k][i][j] = src[k][j][i]  (32x32 tiles, padded).
 __global__ void k_transpose_xy(int nx, int ny, const double* __restrict__ src, double* __restrict__ dst) {
   __shared__ double tile[32][33];

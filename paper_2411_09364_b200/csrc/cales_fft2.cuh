@@ -15,7 +15,10 @@
 
 namespace cales {
 
-enum { F2_E = 16 };
+#ifndef CALES_F2_E
+#define CALES_F2_E 16
+#endif
+enum { F2_E = CALES_F2_E };     // complex elements per thread per pass (16: radix <= 16; 8: radix <= 8, half the registers)
 
 struct Fft2Lay { int L, ls, tish; bool ylay; };     // x: line stride ls (padded); y: TI = 1 << tish columns
 CALES_HD int f2_off(const Fft2Lay& g, int b, int t) { return g.ylay ? (t << g.tish) + b : b * g.ls + sm_pad(t); }
@@ -30,7 +33,7 @@ CALES_HD unsigned f2_div(unsigned n, unsigned d, unsigned magic) {
 #endif
 }
 
-template <int R> struct F2G { enum { G = (R == 3) ? 5 : F2_E / R }; };
+template <int R> struct F2G { enum { G = (R == 3) ? F2_E / 3 : (F2_E / R > 0 ? F2_E / R : 1) }; };
 
 // butterfly g of this thread in pass p -> (line b, butterfly index j); false if beyond the work of the pass
 CALES_HD bool f2_item(const Fft2Lay& lay, const FftPlan& pl, int p, int tid, int nth, int g, int& b, int& j) {
@@ -114,7 +117,7 @@ CALES_HD int perm_inv(int q, int n, bool dct) {
   return q < n / 2 ? 2 * q : 2 * (n - 1 - q) + 1;
 }
 
-// Z[m] of the inverse transforms from the half-complex (or DCT) modes: Z = e + i conj(W^m) d (see merge_inverse)
+// Z[m] of the inverse transforms from the half-complex (or DCT) modes: Z = e + i conj(W^m) d (X_m = E_m + W^m O_m inverted for the packed line z = even + i odd)
 CALES_HD double2 f2_merge(const FftPlan& pl, int m, double2 xm, double2 xc /* mode n2 - m, NOT yet conjugated */) {
   xc.y = -xc.y;
   const double2 e = make_double2(0.5 * (xm.x + xc.x), 0.5 * (xm.y + xc.y));

@@ -52,7 +52,7 @@ static inline void make_plan(FftPlan& pl, int n) {
   while (m % 3 == 0) { ++n3; m /= 3; }
   int a = 0; while (m % 2 == 0) { ++a; m /= 2; }
   if (a > 0) {
-    int maxbits = 4;
+    int maxbits = F2_E >= 16 ? 4 : 3;
     if (const char* e = std::getenv("CALES_FFT_MAXBITS")) { const int v = std::atoi(e); if (v >= 1 && v <= 4) maxbits = v; }
     const int np = (a + maxbits - 1) / maxbits, base = a / np, extra = a % np;
     for (int q = 0; q < np; ++q) pl.radix[pl.npass++] = 1 << (base + (q >= np - extra ? 1 : 0));
@@ -167,13 +167,14 @@ static inline int build_setup(const cales_params* p, HostSetup& H) {
   // every thread holds 16 complex elements per pass (15 when a radix-3 pass exists): ~256 threads per CTA
   auto threads_for = [](long long elems, const FftPlan& pl) {
     bool has3 = false; for (int p = 0; p < pl.npass; ++p) has3 |= pl.radix[p] == 3;
-    long long th = (elems + (has3 ? 14 : 15)) / (has3 ? 15 : 16);
+    const int per_thread = has3 ? 3 * (F2_E / 3) : F2_E;
+    long long th = (elems + per_thread - 1) / per_thread;
     th = (th + 31) / 32 * 32;
     return (int)(th < 32 ? 32 : th);
   };
   {
     const int n2 = nx / 2;
-    int L = 4096 / n2; if (L < 1) L = 1; if (L > 64) L = 64;
+    int L = 256 * F2_E / n2; if (L < 1) L = 1; if (L > 64) L = 64;
     const long long nlines = (long long)ny * nz; if (L > nlines) L = (int)nlines;
     while (L > 1 && threads_for((long long)L * n2, H.plx) > 256) --L;
     while (L > 1 && (nlines + L - 1) / L < 2 * 148) --L;            // small grids: at least two CTAs per SM if there is work for them
@@ -183,7 +184,7 @@ static inline int build_setup(const cales_params* p, HostSetup& H) {
   {
     const int n2 = ny / 2;
     int tish = 5;                                                   // TI = 32 columns ...
-    while (tish > 3 && (long long)(1 << tish) * n2 > 4096) --tish;   // ... down to 8 (64-byte row segments) for long lines
+    while (tish > 3 && (long long)(1 << tish) * n2 > 256 * F2_E) --tish;   // ... down to 8 (64-byte row segments) for long lines
     while (tish > 0 && (1 << tish) > nx) --tish;
     while (tish > 3 && (long long)((nx + (1 << tish) - 1) >> tish) * nz < 2 * 148) --tish;
     while (tish > 0 && (threads_for((long long)(1 << tish) * n2, H.ply) > 512 || (size_t)(1 << tish) * n2 * 16 > 200 * 1024)) --tish;

@@ -22,7 +22,7 @@ enum { RT_TX = 32, RT_TY = 16, RT_RPT = 2, RT_TW = RT_TX + 2, RT_TH = RT_TY + 2,
 // Momentum right-hand side and RK update at one point over an accessor A with
 //   A.U(di,dj,dk), A.V, A.W : velocity components incl. ghosts (viscous-flux ghost at wall-model walls),
 //   A.NT(di,dj,dk)          : nu_t incl. ghosts,   A.P(di,dj,dk): pressure incl. ghosts.
-// Same discretisation as rhs_point (cales_momentum.cuh); the factors 1/2, 1/4 of the interpolations are folded into
+// Second-order central, divergence-form advection (S1, S3); the factors 1/2, 1/4 of the interpolations are folded into
 // the metric terms.  Returns u* at the point.
 template <class A>
 CALES_HD double rhs_core(const Ctx& c, const RhsArgs& a, const A& q, int i, int j, int k) {

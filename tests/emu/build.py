@@ -15,7 +15,7 @@ def build(force=False):
         return LIB
     nvcc = "/usr/local/cuda/bin/nvcc" if os.path.exists("/usr/local/cuda/bin/nvcc") else "nvcc"
     cmd = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O2", "-std=c++17", "--extended-lambda", "-Xcompiler", "-fPIC",
-           "-shared", "-o", LIB, SRC]
+           "-shared", "-o", LIB, SRC] + os.environ.get("CALES_NVCC_EXTRA", "").split()
     subprocess.run(cmd, check=True)
     return LIB
 
