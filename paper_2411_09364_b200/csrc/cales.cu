@@ -314,7 +314,7 @@ static int run_eddy_viscosity(cales_solver* s, const double* u, const double* v,
     if (!ywall || split) {
       const int jlo = ywall ? DSM_TY : 0, jhi = ywall ? c.ny - DSM_TY : c.ny;
       dim3 grid(ds.nbx, (jhi - jlo + DSMC_LY - 1) / DSMC_LY, c.nz);
-      k_dsm_col<64, 4><<<dim3(ds.nbx, grid.y, grid.z), 64, 0, s->st>>>(c, u, v, w, jlo, jhi, ds.pslots, s->smag, s->dsm_part);
+      k_dsm_col_sm<64, 6><<<dim3(ds.nbx, grid.y, grid.z), 64, 0, s->st>>>(c, u, v, w, jlo, jhi, ds.pslots, s->smag, s->dsm_part);
       LAUNCH_TRY(K_DSM_COL);
     }
     k_dsm_coef<<<s->c.nz, 128, 0, s->st>>>(s->c, s->dsm_part, ds.pslots, s->dsm_cs);

@@ -262,16 +262,10 @@ CALES_HD void dsm_point(const Ctx& c, int i0, int j0, int k, int tx, int ty, con
 // filtered face velocities.  A CTA is one row of TXB threads (TXB-2 output columns plus one halo column each side)
 // at a fixed k; it marches over LY+2 rows of y.  Per row: every thread evaluates the 10 base values
 // (u^c, v^c, w^c, S_ij, |S|) of its column, publishes them in shared memory, forms q and its x-filter from its two
-// neighbours' base values, and keeps the separable y-filter as a sliding window in registers:
-//   xq(r) = Fx q(r);   s(r) = xq(r-1) + xq(r);   F q(r-1) = (s(r-1) + s(r)) / 4.
+// neighbours' base values, and keeps the separable y-filter as a two-row sliding window of Fx q in shared memory:
+//   xq(r) = Fx q(r);   F q(r-1) = (xq(r-2) + 2 xq(r-1) + xq(r)) / 4.
 // ------------------------------------------------------------------------------------------------------------
 enum { DSMC_LY = 32, DSMC_NB = 10, DSMC_NQ = 21 };
-
-struct DsmColState {       // per-thread registers carried from row to row
-  double xq_prev[DSMC_NQ]; // Fx q of the previous row
-  double s_prev[DSMC_NQ];  // pair sum of the two rows before
-  double smag_prev;        // |S| of the previous row (this column)
-};
 
 // base values of column gi at row gj (both already wrapped / interior): b[0..2] = u^c, v^c, w^c; b[3..8] = S_ij; b[9] = |S|
 CALES_HD void dsmc_base(const Ctx& c, const double* __restrict__ u, const double* __restrict__ v, const double* __restrict__ w,
@@ -335,31 +329,35 @@ CALES_HD void dsmc_phaseA(const Ctx& c, const double* u, const double* v, const 
   for (int q = 0; q < DSMC_NB; ++q) shbuf[q * txb + t] = b[q];
 }
 
-// Phase B (threads 1..txb-2): x-filter of q, y-window update.  When r >= 2 the filtered row r-1 is complete:
-// returns true and sets *lm, *mm, *smag (of row r-1, this column).
-CALES_HD bool dsmc_phaseB(const Ctx& c, int txb, int t, int r, int k, const double* shbuf, const double* b, DsmColState& st,
-                          double* lm, double* mm, double* smag) {
+// Phase B (threads 1..txb-2): x-filter of q from the neighbours' base values, then the y-filter over a window kept in
+// SHARED memory: ring[slot][m][txb] holds Fx q of the two previous rows of every column (thread-private slots, so no
+// barrier protects them); F q(r-1) = (xq(r-2) + 2 xq(r-1) + xq(r)) / 4.  When r >= 2 the filtered row r-1 is complete:
+// returns true and sets *lm, *mm, *smag (of row r-1, this column).  (A register-resident window was measured slower:
+// 224 registers per thread, and 19 % of all instructions were register moves of the sliding window.)
+CALES_HD bool dsmc_phaseB_sm(const Ctx& c, int txb, int t, int r, int k, const double* shbuf, const double* b, double* ring,
+                             double* smag_prev, double* lm, double* mm, double* smag) {
   double bl[DSMC_NB], br[DSMC_NB];
 #pragma unroll
   for (int q = 0; q < DSMC_NB; ++q) { bl[q] = shbuf[q * txb + t - 1]; br[q] = shbuf[q * txb + t + 1]; }
   double qc[DSMC_NQ], ql[DSMC_NQ], qr[DSMC_NQ];
   dsmc_q(b, qc); dsmc_q(bl, ql); dsmc_q(br, qr);
-  bool done = false;
+  double* r1 = ring + ((r + 1) & 1) * (DSMC_NQ * txb) + t;     // xq(r-1)
+  double* r2 = ring + (r & 1) * (DSMC_NQ * txb) + t;           // xq(r-2); overwritten with xq(r)
   double Fq[DSMC_NQ];
 #pragma unroll
   for (int m = 0; m < DSMC_NQ; ++m) {
     const double xq = 0.25 * (ql[m] + qr[m]) + 0.5 * qc[m];
-    const double s = st.xq_prev[m] + xq;
-    Fq[m] = 0.25 * (st.s_prev[m] + s);
-    st.xq_prev[m] = xq; st.s_prev[m] = s;
+    Fq[m] = 0.25 * (r2[m * txb] + xq) + 0.5 * r1[m * txb];
+    r2[m * txb] = xq;
   }
+  bool done = false;
   if (r >= 2) {
     const double d2 = c.delta[k] * c.delta[k];
     dsmc_contract(Fq, d2, c.alpha, lm, mm);
-    *smag = st.smag_prev;
+    *smag = *smag_prev;
     done = true;
   }
-  st.smag_prev = b[9];
+  *smag_prev = b[9];
   return done;
 }
 
@@ -430,21 +428,21 @@ __global__ void __launch_bounds__(256) k_dsm_pass1(Ctx c, const double* __restri
 // Column-marching pass 1.  grid (ceil(nx/(TXB-2)), ceil((jhi-jlo)/DSMC_LY), nz), block TXB (multiple of 32).
 // Handles output rows [jlo, jhi); part: [k][j][pslots][2], this kernel fills slots blockIdx.x*nwarps + warp.
 template <int TXB, int MINB>
-__global__ void __launch_bounds__(TXB, MINB) k_dsm_col(const __grid_constant__ Ctx c, const double* __restrict__ u, const double* __restrict__ v,
-                                                 const double* __restrict__ w, int jlo, int jhi, int pslots, double* __restrict__ smag,
-                                                 double* __restrict__ part) {
+__global__ void __launch_bounds__(TXB, MINB) k_dsm_col_sm(const __grid_constant__ Ctx c, const double* __restrict__ u, const double* __restrict__ v,
+                                                          const double* __restrict__ w, int jlo, int jhi, int pslots, double* __restrict__ smag,
+                                                          double* __restrict__ part) {
   __shared__ double sh[2][DSMC_NB * TXB];
+  __shared__ double ring[2 * DSMC_NQ * TXB];
   const int t = threadIdx.x, k = blockIdx.z;
   const int i0 = blockIdx.x * (TXB - 2);
   const int j0 = jlo + blockIdx.y * DSMC_LY;
   const int jend = min(j0 + DSMC_LY, jhi);
   const int nrows = jend - j0 + 2;
-  const int gi = i0 - 1 + t;                       // this thread's column (outputs: 1 <= t <= TXB-2, gi < nx)
+  const int gi = i0 - 1 + t;
   const bool outcol = t >= 1 && t <= TXB - 2 && gi < c.nx;
-  DsmColState st;
 #pragma unroll
-  for (int m = 0; m < DSMC_NQ; ++m) { st.xq_prev[m] = 0.0; st.s_prev[m] = 0.0; }
-  st.smag_prev = 0.0;
+  for (int m = 0; m < 2 * DSMC_NQ; ++m) ring[m * TXB + t] = 0.0;
+  double smag_prev = 0.0;
   for (int r = 0; r < nrows; ++r) {
     int gj = j0 - 1 + r;
     gj = gj < 0 ? gj + c.ny : (gj >= c.ny ? gj - c.ny : gj);
@@ -453,8 +451,8 @@ __global__ void __launch_bounds__(TXB, MINB) k_dsm_col(const __grid_constant__ C
     __syncthreads();
     double lm = 0.0, mm = 0.0, sm = 0.0;
     bool done = false;
-    if (t >= 1 && t <= TXB - 2) done = dsmc_phaseB(c, TXB, t, r, k, sh[r & 1], b, st, &lm, &mm, &sm);
-    if (r >= 2) {      // block-uniform
+    if (t >= 1 && t <= TXB - 2) done = dsmc_phaseB_sm(c, TXB, t, r, k, sh[r & 1], b, ring, &smag_prev, &lm, &mm, &sm);
+    if (r >= 2) {
       const int jo = j0 + r - 2;
       if (!(done && outcol)) { lm = 0.0; mm = 0.0; }
       else smag[idx3(c, gi, jo, k)] = sm;

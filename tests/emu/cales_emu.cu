@@ -207,10 +207,10 @@ static void emu_nut(emu_solver* s, const double* u, const double* v, const doubl
   if (!ywall || split) {   // column-marching kernel, stepped row by row with the block barrier between the phases
     const int T = dsh.txb, jlo = ywall ? DSM_TY : 0, jhi = ywall ? c.ny - DSM_TY : c.ny;
     std::vector<double> sh(2 * DSMC_NB * T), breg((size_t)T * DSMC_NB);
-    std::vector<DsmColState> st(T);
+    std::vector<double> ring(2 * DSMC_NQ * T), smprev(T);
     for (int k = 0; k < c.nz; ++k) for (int by = 0; by * DSMC_LY < jhi - jlo; ++by) for (int bx = 0; bx < dsh.nbx; ++bx) {
       const int i0 = bx * (T - 2), j0 = jlo + by * DSMC_LY, jend = std::min(j0 + DSMC_LY, jhi), nrows = jend - j0 + 2;
-      for (auto& q : st) { for (int m = 0; m < DSMC_NQ; ++m) { q.xq_prev[m] = 0.0; q.s_prev[m] = 0.0; } q.smag_prev = 0.0; }
+      std::fill(ring.begin(), ring.end(), 0.0); std::fill(smprev.begin(), smprev.end(), 0.0);
       for (int r = 0; r < nrows; ++r) {
         int gj = j0 - 1 + r; gj = gj < 0 ? gj + c.ny : (gj >= c.ny ? gj - c.ny : gj);
         double* buf = sh.data() + (r & 1) * DSMC_NB * T;
@@ -218,7 +218,7 @@ static void emu_nut(emu_solver* s, const double* u, const double* v, const doubl
         std::vector<double> wl(T / 32, 0.0), wm(T / 32, 0.0);
         for (int t = 1; t <= T - 2; ++t) {
           double lm = 0.0, mm = 0.0, sg = 0.0;
-          const bool done = dsmc_phaseB(c, T, t, r, k, buf, &breg[(size_t)t * DSMC_NB], st[t], &lm, &mm, &sg);
+          const bool done = dsmc_phaseB_sm(c, T, t, r, k, buf, &breg[(size_t)t * DSMC_NB], ring.data(), &smprev[t], &lm, &mm, &sg);
           const int gi = i0 - 1 + t;
           if (r >= 2 && done && gi < c.nx) { s->smag[idx3(c, gi, j0 + r - 2, k)] = sg; wl[t >> 5] += lm; wm[t >> 5] += mm; }
         }
