@@ -334,7 +334,9 @@ CALES_HD void dsmc_phaseA(const Ctx& c, const double* u, const double* v, const 
 // barrier protects them); F q(r-1) = (xq(r-2) + 2 xq(r-1) + xq(r)) / 4.  When r >= 2 the filtered row r-1 is complete:
 // returns true and sets *lm, *mm, *smag (of row r-1, this column).  (A register-resident window was measured slower:
 // 224 registers per thread, and 19 % of all instructions were register moves of the sliding window.)
-CALES_HD bool dsmc_phaseB_sm(const Ctx& c, int txb, int t, int r, int k, const double* shbuf, const double* b, double* ring,
+// The first NREG quantities keep their window in registers (wreg[2 * NREG]: xq(r-1), xq(r-2)), the rest in the ring.
+template <int NREG>
+CALES_HD bool dsmc_phaseB_sm(const Ctx& c, int txb, int t, int r, int k, const double* shbuf, const double* b, double* ring, double* wreg,
                              double* smag_prev, double* lm, double* mm, double* smag) {
   double bl[DSMC_NB], br[DSMC_NB];
 #pragma unroll
@@ -347,8 +349,13 @@ CALES_HD bool dsmc_phaseB_sm(const Ctx& c, int txb, int t, int r, int k, const d
 #pragma unroll
   for (int m = 0; m < DSMC_NQ; ++m) {
     const double xq = 0.25 * (ql[m] + qr[m]) + 0.5 * qc[m];
-    Fq[m] = 0.25 * (r2[m * txb] + xq) + 0.5 * r1[m * txb];
-    r2[m * txb] = xq;
+    if (m < NREG) {
+      Fq[m] = 0.25 * (wreg[NREG + m] + xq) + 0.5 * wreg[m];
+      wreg[NREG + m] = wreg[m]; wreg[m] = xq;
+    } else {
+      Fq[m] = 0.25 * (r2[m * txb] + xq) + 0.5 * r1[m * txb];
+      r2[m * txb] = xq;
+    }
   }
   bool done = false;
   if (r >= 2) {
@@ -427,7 +434,7 @@ __global__ void __launch_bounds__(256) k_dsm_pass1(Ctx c, const double* __restri
 }
 // Column-marching pass 1.  grid (ceil(nx/(TXB-2)), ceil((jhi-jlo)/DSMC_LY), nz), block TXB (multiple of 32).
 // Handles output rows [jlo, jhi); part: [k][j][pslots][2], this kernel fills slots blockIdx.x*nwarps + warp.
-template <int TXB, int MINB>
+template <int TXB, int MINB, int NREG>
 __global__ void __launch_bounds__(TXB, MINB) k_dsm_col_sm(const __grid_constant__ Ctx c, const double* __restrict__ u, const double* __restrict__ v,
                                                           const double* __restrict__ w, int jlo, int jhi, int pslots, double* __restrict__ smag,
                                                           double* __restrict__ part) {
@@ -443,6 +450,9 @@ __global__ void __launch_bounds__(TXB, MINB) k_dsm_col_sm(const __grid_constant_
 #pragma unroll
   for (int m = 0; m < 2 * DSMC_NQ; ++m) ring[m * TXB + t] = 0.0;
   double smag_prev = 0.0;
+  double wreg[2 * NREG + 1];
+#pragma unroll
+  for (int m = 0; m < 2 * NREG + 1; ++m) wreg[m] = 0.0;
   for (int r = 0; r < nrows; ++r) {
     int gj = j0 - 1 + r;
     gj = gj < 0 ? gj + c.ny : (gj >= c.ny ? gj - c.ny : gj);
@@ -451,7 +461,7 @@ __global__ void __launch_bounds__(TXB, MINB) k_dsm_col_sm(const __grid_constant_
     __syncthreads();
     double lm = 0.0, mm = 0.0, sm = 0.0;
     bool done = false;
-    if (t >= 1 && t <= TXB - 2) done = dsmc_phaseB_sm(c, TXB, t, r, k, sh[r & 1], b, ring, &smag_prev, &lm, &mm, &sm);
+    if (t >= 1 && t <= TXB - 2) done = dsmc_phaseB_sm<NREG>(c, TXB, t, r, k, sh[r & 1], b, ring, wreg, &smag_prev, &lm, &mm, &sm);
     if (r >= 2) {
       const int jo = j0 + r - 2;
       if (!(done && outcol)) { lm = 0.0; mm = 0.0; }

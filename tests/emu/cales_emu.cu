@@ -218,7 +218,7 @@ static void emu_nut(emu_solver* s, const double* u, const double* v, const doubl
         std::vector<double> wl(T / 32, 0.0), wm(T / 32, 0.0);
         for (int t = 1; t <= T - 2; ++t) {
           double lm = 0.0, mm = 0.0, sg = 0.0;
-          const bool done = dsmc_phaseB_sm(c, T, t, r, k, buf, &breg[(size_t)t * DSMC_NB], ring.data(), &smprev[t], &lm, &mm, &sg);
+          double wnone[1]; const bool done = dsmc_phaseB_sm<0>(c, T, t, r, k, buf, &breg[(size_t)t * DSMC_NB], ring.data(), wnone, &smprev[t], &lm, &mm, &sg);
           const int gi = i0 - 1 + t;
           if (r >= 2 && done && gi < c.nx) { s->smag[idx3(c, gi, j0 + r - 2, k)] = sg; wl[t >> 5] += lm; wm[t >> 5] += mm; }
         }
