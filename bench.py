@@ -147,14 +147,15 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
-def pick_config(torch, requested):
+def pick_config(torch, requested, ranks_on_node=1):
+    """Config 5 (the largest single-GPU workload) when the device and the host have room for it, else config 4."""
     if requested:
         return requested
     import psutil
     free, _ = torch.cuda.mem_get_info()
     host = psutil.virtual_memory().available
-    # config 5: 15 resident fields x 6.44 GB on the device; 4 pinned host fields + generation temporaries on the host
-    if free >= 110e9 and host >= 90e9:
+    # config 5: 15 resident fields x 6.44 GB on the device; per rank 4 pinned host fields + generation temporaries (~50 GB)
+    if free >= 110e9 and host >= 60e9 * ranks_on_node + 30e9:
         return 5
     return 4
 
@@ -197,7 +198,11 @@ def run_ours(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     binding.lib()
-    cfg_no = pick_config(torch, args.config)
+    cfg_no = pick_config(torch, args.config, int(os.environ.get("LOCAL_WORLD_SIZE", str(world))))
+    if world > 1:                    # every replica runs the same workload: rank 0 decides
+        box = [cfg_no]
+        dist.broadcast_object_list(box, src=0)
+        cfg_no = int(box[0])
     K, W = args.steps, max(args.warmup, 3)
 
     # ---- seeded synthetic workload (inputs.py), every rank its own replica (seed + rank)

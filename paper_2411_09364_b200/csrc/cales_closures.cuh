@@ -458,6 +458,16 @@ __global__ void __launch_bounds__(TXB, MINB) k_dsm_col_sm(const __grid_constant_
     gj = gj < 0 ? gj + c.ny : (gj >= c.ny ? gj - c.ny : gj);
     double b[DSMC_NB];
     dsmc_phaseA(c, u, v, w, TXB, t, i0, gj, k, sh[r & 1], b);
+    if (r + 2 < nrows && (t & 3) == 0 && k >= 1 && k <= c.nz - 2) {     // the row after next: pull its lines towards L1
+      int gp = j0 + 1 + r + 1; gp = gp >= c.ny ? gp - c.ny : gp;
+      const long long nn = idx3(c, ((i0 - 1 + t) % c.nx + c.nx) % c.nx, gp, k);
+#pragma unroll
+      for (int d = -1; d <= 1; ++d) {
+        asm volatile("prefetch.global.L1 [%0];" ::"l"(u + nn + d * c.nxy));
+        asm volatile("prefetch.global.L1 [%0];" ::"l"(v + nn + d * c.nxy));
+        asm volatile("prefetch.global.L1 [%0];" ::"l"(w + nn + d * c.nxy));
+      }
+    }
     __syncthreads();
     double lm = 0.0, mm = 0.0, sm = 0.0;
     bool done = false;

@@ -24,12 +24,15 @@ enum { RT_TX = 32, RT_TY = 16, RT_RPT = 2, RT_TW = RT_TX + 2, RT_TH = RT_TY + 2,
 //   A.NT(di,dj,dk)          : nu_t incl. ghosts,   A.P(di,dj,dk): pressure incl. ghosts.
 // Second-order central, divergence-form advection (S1, S3); the factors 1/2, 1/4 of the interpolations are folded into
 // the metric terms.  Returns u* at the point.
+// z metrics of one plane, loaded once per plane by the marching kernel
+struct ZMet { double dzfk, dzfp, rdzf, rdzfp, rdzc, rdzcm; };
+CALES_HD ZMet zmet_at(const Ctx& c, int k) { return ZMet{c.dzf[k], c.dzf[k + 1], c.rdzf[k], c.rdzf[k + 1], c.rdzc[k], c.rdzc[k - 1]}; }
+
 template <class A>
-CALES_HD double rhs_core(const Ctx& c, const RhsArgs& a, const A& q, int i, int j, int k) {
+CALES_HD double rhs_core(const Ctx& c, const RhsArgs& a, const A& q, int i, int j, int k, const ZMet& zm) {
   const long long n = idx3(c, i, j, k);
   const double rdx = c.rdx, rdy = c.rdy;
-  const double dzfk = c.dzf[k], dzfp = c.dzf[k + 1];
-  const double rdzf = c.rdzf[k], rdzfp = c.rdzf[k + 1], rdzc = c.rdzc[k], rdzcm = c.rdzc[k - 1];
+  const double dzfk = zm.dzfk, dzfp = zm.dzfp, rdzf = zm.rdzf, rdzfp = zm.rdzfp, rdzc = zm.rdzc, rdzcm = zm.rdzcm;
   const bool vact = !(c.bc_y == BC_WALL && j == c.ny - 1);
   const bool wact = !(c.bc_z == BC_WALL && k == c.nz - 1);
   const double u000 = q.U(0, 0, 0), up00 = q.U(1, 0, 0), um00 = q.U(-1, 0, 0), u0p0 = q.U(0, 1, 0), u0m0 = q.U(0, -1, 0),
@@ -195,15 +198,28 @@ __global__ void __launch_bounds__(RT_THREADS, 2) k_rhs_tile(const __grid_constan
     __syncthreads();
     if (k + 2 <= k1) issue(k + 2);
     cp_async_commit();
+    if (a.be != 0.0 && k + 1 < k1) {     // R^{k-1} of the next plane: pull the lines towards L1 while this plane is computed
+#pragma unroll
+      for (int r = 0; r < RT_RPT; ++r) {
+        const int i = i0 + tx, j = j0 + ty + r * (RT_TY / RT_RPT);
+        if (i < c.nx && j < c.ny && (tx & 3) == 0) {       // one prefetch per 32-byte sector
+          const long long nn = idx3(c, i, j, k + 1);
+          asm volatile("prefetch.global.L1 [%0];" ::"l"(a.Ru0 + nn));
+          asm volatile("prefetch.global.L1 [%0];" ::"l"(a.Rv0 + nn));
+          asm volatile("prefetch.global.L1 [%0];" ::"l"(a.Rw0 + nn));
+        }
+      }
+    }
     TileAcc q;
     q.sl[0] = rt_sm + ((k + 3) & 3) * (RT_NF * RT_PLANE); q.sl[1] = rt_sm + (k & 3) * (RT_NF * RT_PLANE); q.sl[2] = rt_sm + ((k + 1) & 3) * (RT_NF * RT_PLANE);
-    const double dz = c.dzf[k];
+    const ZMet zm = zmet_at(c, k);
+    const double dz = zm.dzfk;
 #pragma unroll
     for (int r = 0; r < RT_RPT; ++r) {
       const int ly = ty + r * (RT_TY / RT_RPT), i = i0 + tx, j = j0 + ly;
       if (i < c.nx && j < c.ny) {
         q.ctr = (ly + 1) * RT_TW + tx + 1;
-        acc += rhs_core(c, a, q, i, j, k) * dz;
+        acc += rhs_core(c, a, q, i, j, k, zm) * dz;
       }
     }
   }

@@ -267,7 +267,7 @@ static void emu_substep(emu_solver* s, int rk, double dt) {
       TileAcc q; for (int d = 0; d < 3; ++d) q.sl[d] = ring.data() + d * RT_NF * RT_PLANE;
       for (int ly = 0; ly < RT_TY; ++ly) for (int tx = 0; tx < RT_TX; ++tx) {
         const int i = i0 + tx, j = j0 + ly;
-        if (i < c.nx && j < c.ny) { q.ctr = (ly + 1) * RT_TW + tx + 1; sum += rhs_core(c, a, q, i, j, k) * c.dzf[k]; }
+        if (i < c.nx && j < c.ny) { q.ctr = (ly + 1) * RT_TW + tx + 1; sum += rhs_core(c, a, q, i, j, k, zmet_at(c, k)) * c.dzf[k]; }
       }
     }
   }
