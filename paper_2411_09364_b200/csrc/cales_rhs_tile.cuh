@@ -201,7 +201,7 @@ __global__ void __launch_bounds__(RT_THREADS, 2) k_rhs_tile(const __grid_constan
     if (a.be != 0.0 && k + 1 < k1) {     // R^{k-1} of the next plane: pull the lines towards L1 while this plane is computed
 #pragma unroll
       for (int r = 0; r < RT_RPT; ++r) {
-        const int i = i0 + tx, j = j0 + ty + r * (RT_TY / RT_RPT);
+        const int i = i0 + tx, j = j0 + ty * RT_RPT + r;
         if (i < c.nx && j < c.ny && (tx & 3) == 0) {       // one prefetch per 32-byte sector
           const long long nn = idx3(c, i, j, k + 1);
           asm volatile("prefetch.global.L1 [%0];" ::"l"(a.Ru0 + nn));
@@ -216,7 +216,7 @@ __global__ void __launch_bounds__(RT_THREADS, 2) k_rhs_tile(const __grid_constan
     const double dz = zm.dzfk;
 #pragma unroll
     for (int r = 0; r < RT_RPT; ++r) {
-      const int ly = ty + r * (RT_TY / RT_RPT), i = i0 + tx, j = j0 + ly;
+      const int ly = ty * RT_RPT + r, i = i0 + tx, j = j0 + ly;   // adjacent rows: their stencils share shared-memory loads
       if (i < c.nx && j < c.ny) {
         q.ctr = (ly + 1) * RT_TW + tx + 1;
         acc += rhs_core(c, a, q, i, j, k, zm) * dz;

@@ -98,7 +98,7 @@ __global__ void __launch_bounds__(RT_THREADS, 3) k_smag_tile(const __grid_consta
 #pragma unroll
   for (int r = 0; r < RT_RPT; ++r) {
     tauw[r][0] = tauw[r][1] = 0.0;
-    const int i = i0 + tx, j = j0 + ty + r * (RT_TY / RT_RPT);
+    const int i = i0 + tx, j = j0 + ty * RT_RPT + r;
     if (c.van_driest && i < c.nx && j < c.ny) smag_wall_shear(c, u, v, i, j, tauw[r]);
   }
   for (int k = k0; k < k1; ++k) {
@@ -109,7 +109,7 @@ __global__ void __launch_bounds__(RT_THREADS, 3) k_smag_tile(const __grid_consta
     const double* sl[3] = {st_sm + ((k + 3) & 3) * (ST_NF * RT_PLANE), st_sm + (k & 3) * (ST_NF * RT_PLANE), st_sm + ((k + 1) & 3) * (ST_NF * RT_PLANE)};
 #pragma unroll
     for (int r = 0; r < RT_RPT; ++r) {
-      const int ly = ty + r * (RT_TY / RT_RPT), i = i0 + tx, j = j0 + ly;
+      const int ly = ty * RT_RPT + r, i = i0 + tx, j = j0 + ly;   // adjacent rows: their stencils share shared-memory loads
       if (i < c.nx && j < c.ny) nut[idx3(c, i, j, k)] = smag_tile_point(c, sl, (ly + 1) * RT_TW + tx + 1, k, tauw[r]);
     }
   }
