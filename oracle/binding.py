@@ -197,6 +197,12 @@ class Oracle:
         L = np.empty((6,) + self.shape); M = np.empty((6,) + self.shape)
         _chk(lib().oracle_get_dsm_tensors(self._h, _p(L), _p(M))); return L, M
 
+    def cfl_dt(self, cfl):
+        dt = C.c_double(); _chk(lib().oracle_cfl_dt(self._h, C.c_double(cfl), C.byref(dt))); return dt.value
+
+    def plane_stats(self):
+        out = np.empty((8, self.nz)); _chk(lib().oracle_plane_stats(self._h, _p(out))); return out
+
     def project(self):
         _chk(lib().oracle_project(self._h))
 

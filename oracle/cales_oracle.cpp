@@ -972,3 +972,36 @@ extern "C" int oracle_diagnostics(oracle_solver* S, double* max_div, double* u_b
   if (forcing) *forcing = S->forcing; if (wm_max_iters) *wm_max_iters = S->wm_max_iters;
   return 0;
 }
+
+// ---- adaptive time step and on-line plane statistics -----------------------------------------
+// dt = cfl / max over cells of (|u_c|/dx + |v_c|/dy + |w_c|/dzf) with the velocities averaged to the cell centre
+// (reading S18; "0.95 x the stability limit", formula silent).
+extern "C" int oracle_cfl_dt(oracle_solver* S, double cfl, double* dt) {
+  if (!S || !dt) return fail("null");
+  int nx = S->nx, ny = S->ny, nz = S->nz;
+  bc_velocity(*S, S->u, S->v, S->w, GH_STRAIN);
+  double rmax = 0.0;
+  for (int k = 0; k < nz; ++k) for (int j = 0; j < ny; ++j) for (int i = 0; i < nx; ++i) {
+    double uc = 0.5 * (S->u(i - 1, j, k) + S->u(i, j, k)), vc = 0.5 * (S->v(i, j - 1, k) + S->v(i, j, k)), wc = 0.5 * (S->w(i, j, k - 1) + S->w(i, j, k));
+    double r = std::fabs(uc) / S->dx + std::fabs(vc) / S->dy + std::fabs(wc) / S->dzf(k);
+    if (r > rmax) rmax = r;
+  }
+  *dt = rmax > 0.0 ? cfl / rmax : 0.0;
+  return 0;
+}
+// Plane (x-y) means per k of the centre-averaged velocity, its products and nu_t (the profiles of PAPER.md:237):
+// out[q][k], q = 0 <u>, 1 <v>, 2 <w>, 3 <uu>, 4 <vv>, 5 <ww>, 6 <uw>, 7 <nu_t>.
+extern "C" int oracle_plane_stats(oracle_solver* S, double* out) {
+  if (!S || !out) return fail("null");
+  int nx = S->nx, ny = S->ny, nz = S->nz;
+  bc_velocity(*S, S->u, S->v, S->w, GH_STRAIN);
+  for (int k = 0; k < nz; ++k) {
+    double a[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    for (int j = 0; j < ny; ++j) for (int i = 0; i < nx; ++i) {
+      double uc = 0.5 * (S->u(i - 1, j, k) + S->u(i, j, k)), vc = 0.5 * (S->v(i, j - 1, k) + S->v(i, j, k)), wc = 0.5 * (S->w(i, j, k - 1) + S->w(i, j, k));
+      a[0] += uc; a[1] += vc; a[2] += wc; a[3] += uc * uc; a[4] += vc * vc; a[5] += wc * wc; a[6] += uc * wc; a[7] += S->nut(i, j, k);
+    }
+    for (int q = 0; q < 8; ++q) out[(size_t)q * nz + k] = a[q] / ((double)nx * ny);
+  }
+  return 0;
+}

@@ -90,6 +90,10 @@ int oracle_get_dsm_tensors(oracle_solver* s, double* L, double* M);
 int oracle_project(oracle_solver* s);
 /* diagnostics of the internal state */
 int oracle_diagnostics(oracle_solver* s, double* max_div, double* u_bulk, double* kinetic_energy, double* forcing, int* wm_max_iters);
+/* SURVEY.md 8(f) item 4.  dt = cfl / max(|u_c|/dx + |v_c|/dy + |w_c|/dzf), velocities averaged to cell centres (reading S18) */
+int oracle_cfl_dt(oracle_solver* s, double cfl, double* dt);
+/* x-y plane means per k: out[q][k], q = <u>,<v>,<w>,<uu>,<vv>,<ww>,<uw>,<nu_t> of the centre-averaged velocity */
+int oracle_plane_stats(oracle_solver* s, double* out);
 /* threads used by the OpenMP loops */
 int oracle_num_threads(void);
 

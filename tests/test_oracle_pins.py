@@ -534,3 +534,35 @@ def test_energy_decays_with_sgs_model(oracle):
     eu0 = energy(S0); eu1 = energy(S)
     assert eu1 < eu0                                   # the model dissipates
     assert e0 > 0
+
+
+# ----------------------------------------------------------------------------- SURVEY.md 8(f) item 4
+@pytest.mark.parametrize("bc_y,bc_z,stretch", [(0, 0, 0), (0, 1, 1), (1, 1, 0)])
+def test_cfl_time_step_and_plane_statistics_vs_numpy(oracle, bc_y, bc_z, stretch):
+    """dt = cfl / max(|u_c|/dx + |v_c|/dy + |w_c|/dzf) (reading S18) and the x-y plane means of the centre-averaged
+    velocity, its products and nu_t, re-evaluated here with numpy shifts (wall faces and the faces beyond them are 0)."""
+    nx, ny, nz = 12, 8, 10
+    o = oracle.Oracle(nx, ny, nz, 2.0, 1.5, 1.0, bc_y=bc_y, bc_z=bc_z, zstretch=stretch, zstretch_factor=1.5 if stretch else 0.0,
+                      sgs_model=1, cs=0.1)
+    rng = np.random.default_rng(3)
+    u, v, w = (rng.standard_normal((nz, ny, nx)) for _ in range(3))
+    if bc_y:
+        v[:, -1, :] = 0.0
+    if bc_z:
+        w[-1] = 0.0
+    o.set_velocity(u, v, w)
+    nut = o.eddy_viscosity(); o.set(4, nut)
+    um = np.roll(u, 1, axis=2)
+    vm = np.roll(v, 1, axis=1)
+    wm = np.roll(w, 1, axis=0)
+    if bc_y:
+        vm[:, 0, :] = 0.0
+    if bc_z:
+        wm[0] = 0.0
+    uc, vc, wc = 0.5 * (u + um), 0.5 * (v + vm), 0.5 * (w + wm)
+    rate = np.abs(uc) / o.dx + np.abs(vc) / o.dy + np.abs(wc) / o.dzf[:, None, None]
+    assert abs(o.cfl_dt(0.5) - 0.5 / rate.max()) <= 1e-15 * 0.5 / rate.max() * 10
+    st = o.plane_stats()
+    ref = [uc, vc, wc, uc * uc, vc * vc, wc * wc, uc * wc, nut]
+    for q in range(8):
+        assert np.max(np.abs(st[q] - ref[q].mean(axis=(1, 2)))) <= 1e-13 * max(1.0, np.max(np.abs(ref[q])))
