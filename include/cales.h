@@ -133,6 +133,15 @@ int cales_wall_stress(cales_solver* s, double* tau_dev);
 /* Make the solver's velocity discretely solenoidal by one projection with gamma*dt = 1 (Eq. 12-13). */
 int cales_project(cales_solver* s);
 
+/* Adaptive time step (a fixed fraction of the stability limit; reading S18):
+ * *dt_host = cfl / max over cells of (|u_c|/dx + |v_c|/dy + |w_c|/dzf), velocities averaged to the cell centres.
+ * HOST output; synchronises the stream. */
+int cales_cfl_dt(cales_solver* s, double cfl, double* dt_host);
+
+/* On-line statistics: x-y plane means per k of the centre-averaged u, v, w, uu, vv, ww, uw and of nu_t.
+ * out_dev: DEVICE, [8][nz].  Asynchronous. */
+int cales_plane_stats(cales_solver* s, double* out_dev);
+
 /* Dynamic coefficient of the last eddy-viscosity evaluation: cs_dev DEVICE, nz (plane averaging) or nz*ny. */
 int cales_get_cs(cales_solver* s, double* cs_dev);
 

@@ -38,7 +38,7 @@ class CalesDiag(C.Structure):
 # every symbol include/cales.h declares
 SYMBOLS = ["cales_default_params", "cales_workspace_bytes", "cales_create", "cales_create_basic", "cales_destroy",
            "cales_set_field", "cales_get_field", "cales_step", "cales_poisson_solve", "cales_eddy_viscosity",
-           "cales_wall_stress", "cales_project", "cales_get_cs", "cales_transform", "cales_transpose_xy",
+           "cales_wall_stress", "cales_project", "cales_cfl_dt", "cales_plane_stats", "cales_get_cs", "cales_transform", "cales_transpose_xy",
            "cales_set_timing", "cales_set_graph", "cales_kernel_count", "cales_kernel_time", "cales_launches_per_step", "cales_diagnostics", "cales_last_error"]
 
 _lib = None
@@ -66,6 +66,8 @@ def lib():
         L.cales_wall_stress.argtypes = [C.c_void_p, C.c_void_p]
         L.cales_project.argtypes = [C.c_void_p]
         L.cales_get_cs.argtypes = [C.c_void_p, C.c_void_p]
+        L.cales_cfl_dt.argtypes = [C.c_void_p, C.c_double, C.POINTER(C.c_double)]
+        L.cales_plane_stats.argtypes = [C.c_void_p, C.c_void_p]
         L.cales_transform.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int]
         L.cales_transpose_xy.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.cales_set_timing.argtypes = [C.c_void_p, C.c_int]
@@ -215,6 +217,16 @@ class Solver:
 
     def project(self):
         _chk(lib().cales_project(self._h))
+
+    def cfl_dt(self, cfl):
+        dt = C.c_double()
+        _chk(lib().cales_cfl_dt(self._h, float(cfl), C.byref(dt)))
+        return dt.value
+
+    def plane_stats(self):
+        out = self._torch.empty((8, self.nz), dtype=self._torch.float64, device=self.device)
+        _chk(lib().cales_plane_stats(self._h, C.c_void_p(out.data_ptr())))
+        return out
 
     def get_cs(self, per_plane=True):
         n = self.nz if per_plane else self.nz * self.ny

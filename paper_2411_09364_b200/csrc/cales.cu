@@ -477,6 +477,34 @@ extern "C" int cales_project(cales_solver* s) {
   return CALES_OK;
 }
 
+// adaptive time step (0.95 x the stability limit in the paper; reading S18)
+extern "C" int cales_cfl_dt(cales_solver* s, double cfl, double* dt_host) {
+  if (!s || !dt_host || !(cfl > 0.0)) return fail(CALES_EINVAL, "bad cfl_dt arguments");
+  const int timing_was = s->timing; s->timing = 0;
+  double* part = s->CP;   // scratch, nblk <= N
+  k_cfl_rate<<<s->pgrid, s->pblock, 0, s->st>>>(s->c, s->u, s->v, s->w, part);
+  LAUNCH_TRY(K_DIAG);
+  const long long nb = s->nblk; const int g1 = (int)(nb < 1024 ? nb : 1024);
+  k_max_stage<<<g1, 256, 0, s->st>>>(part, nb, s->stage1); LAUNCH_TRY(K_SUM);
+  std::vector<double> h(g1);
+  CUDA_TRY(cudaMemcpyAsync(h.data(), s->stage1, g1 * sizeof(double), cudaMemcpyDeviceToHost, s->st));
+  CUDA_TRY(cudaStreamSynchronize(s->st));
+  s->timing = timing_was;
+  double r = 0.0; for (int q = 0; q < g1; ++q) r = std::fmax(r, h[q]);
+  *dt_host = r > 0.0 ? cfl / r : 0.0;
+  return CALES_OK;
+}
+
+// x-y plane means of u, v, w, uu, vv, ww, uw (centre-averaged) and nu_t: out_dev DEVICE [8][nz] (PAPER.md:237 profiles)
+extern "C" int cales_plane_stats(cales_solver* s, double* out_dev) {
+  if (!s || !out_dev) return fail(CALES_EINVAL, "null argument");
+  const int timing_was = s->timing; s->timing = 0;
+  k_plane_stats<<<s->c.nz, 1024, 0, s->st>>>(s->c, s->u, s->v, s->w, s->nut, out_dev);
+  const int rc = check_launch(s, K_DIAG);
+  s->timing = timing_was;
+  return rc;
+}
+
 extern "C" int cales_get_cs(cales_solver* s, double* cs_dev) {
   if (!s || !cs_dev) return fail(CALES_EINVAL, "null argument");
   if (s->c.sgs != CALES_SGS_DSMAG) return fail(CALES_EINVAL, "not a dynamic-model solver");

@@ -111,6 +111,45 @@ __global__ void __launch_bounds__(256) k_diag(Ctx c, const double* u, const doub
   const double s1 = block_sum(ub, sh), s2 = block_sum(ke, sh), s3 = block_sum(bad, sh);
   if (threadIdx.x == 0 && threadIdx.y == 0) { part[b] = md; part[nb + b] = s1; part[2 * nb + b] = s2; part[3 * nb + b] = s3; }
 }
+// SURVEY.md 8(f) item 4.  CFL rate |u_c|/dx + |v_c|/dy + |w_c|/dzf at a cell centre (S18)
+CALES_HD double cfl_rate_point(const Ctx& c, const double* u, const double* v, const double* w, int i, int j, int k) {
+  const double uc = 0.5 * (velg<0>(c, u, i - 1, j, k, GH_STRAIN) + velg<0>(c, u, i, j, k, GH_STRAIN));
+  const double vc = 0.5 * (velg<1>(c, v, i, j - 1, k, GH_STRAIN) + velg<1>(c, v, i, j, k, GH_STRAIN));
+  const double wc = 0.5 * (velg<2>(c, w, i, j, k - 1, GH_STRAIN) + velg<2>(c, w, i, j, k, GH_STRAIN));
+  return fabs(uc) * c.rdx + fabs(vc) * c.rdy + fabs(wc) * c.rdzf[k];
+}
+// the 8 plane-statistics quantities at a cell centre: u, v, w, uu, vv, ww, uw (centre-averaged velocity), nu_t
+CALES_HD void stats_point(const Ctx& c, const double* u, const double* v, const double* w, const double* nut, int i, int j, int k, double* q) {
+  const double uc = 0.5 * (velg<0>(c, u, i - 1, j, k, GH_STRAIN) + velg<0>(c, u, i, j, k, GH_STRAIN));
+  const double vc = 0.5 * (velg<1>(c, v, i, j - 1, k, GH_STRAIN) + velg<1>(c, v, i, j, k, GH_STRAIN));
+  const double wc = 0.5 * (velg<2>(c, w, i, j, k - 1, GH_STRAIN) + velg<2>(c, w, i, j, k, GH_STRAIN));
+  q[0] = uc; q[1] = vc; q[2] = wc; q[3] = uc * uc; q[4] = vc * vc; q[5] = wc * wc; q[6] = uc * wc; q[7] = nut[idx3(c, i, j, k)];
+}
+// per-block max of the CFL rate -> part[block] (grid as the point kernels)
+__global__ void __launch_bounds__(256) k_cfl_rate(Ctx c, const double* u, const double* v, const double* w, double* __restrict__ part) {
+  __shared__ double sh[32];
+  const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y * blockDim.y + threadIdx.y, k = blockIdx.z;
+  double r = 0.0;
+  if (i < c.nx && j < c.ny) r = cfl_rate_point(c, u, v, w, i, j, k);
+  const double m = block_max(r, sh);
+  if (threadIdx.x == 0 && threadIdx.y == 0) part[blockIdx.x + gridDim.x * (blockIdx.y + (long long)gridDim.y * blockIdx.z)] = m;
+}
+// x-y plane means: grid (nz), block 1024; out[q * nz + k] (deterministic: fixed thread -> point assignment and tree order)
+__global__ void __launch_bounds__(1024) k_plane_stats(Ctx c, const double* u, const double* v, const double* w, const double* nut, double* __restrict__ out) {
+  __shared__ double sh[32];
+  const int k = blockIdx.x;
+  double a[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+  for (long long n = threadIdx.x; n < c.nxy; n += blockDim.x) {
+    double q[8];
+    stats_point(c, u, v, w, nut, (int)(n % c.nx), (int)(n / c.nx), k, q);
+#pragma unroll
+    for (int m = 0; m < 8; ++m) a[m] += q[m];
+  }
+  for (int m = 0; m < 8; ++m) {
+    const double t = block_sum(a[m], sh);
+    if (threadIdx.x == 0) out[(long long)m * c.nz + k] = t / (double)c.nxy;
+  }
+}
 __global__ void k_max_stage(const double* __restrict__ in, long long n, double* __restrict__ out) {
   __shared__ double sh[32];
   const long long per = (n + gridDim.x - 1) / gridDim.x;

@@ -14,6 +14,7 @@ def lib():
         L = C.CDLL(_build.build())
         L.emu_last_error.restype = C.c_char_p
         L.emu_max_div.restype = C.c_double
+        L.emu_cfl_dt.restype = C.c_double
         L.emu_destroy.restype = None
         _lib = L
     return _lib
@@ -87,3 +88,9 @@ class Emu:
 
     def max_div(self):
         return lib().emu_max_div(self._h)
+
+    def cfl_dt(self, cfl):
+        return lib().emu_cfl_dt(self._h, C.c_double(cfl))
+
+    def plane_stats(self):
+        out = np.empty((8, self.nz)); lib().emu_plane_stats(self._h, _p(out)); return out

@@ -339,3 +339,21 @@ extern "C" double emu_max_div(emu_solver* s) {
     md = std::fmax(md, std::fabs(divergence_point(c, s->u.data(), s->v.data(), s->w.data(), i, j, k)));
   return md;
 }
+extern "C" double emu_cfl_dt(emu_solver* s, double cfl) {
+  const Ctx& c = s->c; double r = 0.0;
+  for (int k = 0; k < c.nz; ++k) for (int j = 0; j < c.ny; ++j) for (int i = 0; i < c.nx; ++i)
+    r = std::fmax(r, cfl_rate_point(c, s->u.data(), s->v.data(), s->w.data(), i, j, k));
+  return r > 0.0 ? cfl / r : 0.0;
+}
+extern "C" int emu_plane_stats(emu_solver* s, double* out) {
+  const Ctx& c = s->c;
+  for (int k = 0; k < c.nz; ++k) {
+    double a[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    for (long long n = 0; n < c.nxy; ++n) {
+      double q[8]; stats_point(c, s->u.data(), s->v.data(), s->w.data(), s->nut.data(), (int)(n % c.nx), (int)(n / c.nx), k, q);
+      for (int m = 0; m < 8; ++m) a[m] += q[m];
+    }
+    for (int m = 0; m < 8; ++m) out[(long long)m * c.nz + k] = a[m] / (double)c.nxy;
+  }
+  return 0;
+}

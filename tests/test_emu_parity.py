@@ -26,6 +26,9 @@ def test_emulated_kernels_match_oracle(oracle, emu, case):
         o.step(dt); e.step(dt)
         err = pc.field_errors([e.get(f) for f in range(5)], [o.get(f) for f in range(5)], o.dzf, kw["nu"])
         assert max(err.values()) <= 1e-11, (case, s, err)
+    assert abs(e.cfl_dt(0.95) - o.cfl_dt(0.95)) <= 1e-12 * o.cfl_dt(0.95)
+    sa, sb = e.plane_stats(), o.plane_stats()
+    assert np.max(np.abs(sa - sb)) <= 1e-11 * np.max(np.abs(sb))
     # projection quality of the emulated device path (north_star: <= 1e-12 x velocity scale)
     scale = max(np.max(np.abs(o.get(0))), 1e-300) / min(o.dx, o.dy, float(np.min(o.dzf)))
     assert e.max_div() <= 1e-12 * scale * 10

@@ -300,3 +300,19 @@ def test_static_model_staged_kernel_parity(oracle, gpu, n, shape, monkeypatch):
     err = pc.field_errors(_gpu_fields(g), [o.get(f) for f in range(5)], o.dzf, kw["nu"])
     assert max(err.values()) <= TOL_1STEP, err
     g.close()
+
+
+@pytest.mark.parametrize("n,shape", [(1, (48, 24, 20)), (3, (72, 36, 40)), (4, (96, 36, 24)), (5, (72, 48, 24))])
+def test_cfl_dt_and_plane_stats_parity(oracle, gpu, n, shape):
+    """adaptive time step and on-line plane statistics against the oracle."""
+    cfg, kw, (u, v, w), dt = pc.prepare(oracle, n, shape)
+    o = pc.make(oracle.Oracle, kw)
+    g = pc.make(gpu.Solver, kw)
+    o.set_velocity(u, v, w); g.set_velocity(u, v, w)
+    o.step(dt); g.step(dt)
+    a, b = g.cfl_dt(0.95), o.cfl_dt(0.95)
+    assert abs(a - b) <= 1e-12 * b
+    sa, sb = g.plane_stats().cpu().numpy(), o.plane_stats()
+    for q in range(8):
+        assert np.max(np.abs(sa[q] - sb[q])) <= 1e-11 * max(np.max(np.abs(sb[q])), 1e-300 if q < 7 else kw["nu"]), q
+    g.close()
