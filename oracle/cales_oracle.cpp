@@ -714,7 +714,6 @@ extern "C" int oracle_create(const oracle_params* p, oracle_solver** out) {
   if (p->bc_z == BC_PER && p->zstretch != 0) return fail("periodic z requires a uniform grid");
   if (p->wall_model && p->bc_z != BC_WALL) return fail("wall model needs z walls");
   if (p->implicit_z && p->bc_z != BC_WALL) return fail("implicit z needs z walls");
-  if (p->implicit_z && p->wall_model) return fail("wall model with implicit z: not supported (next)");
   if (p->wall_model && p->h_wm > 0.0 && !(p->h_wm < 0.5 * p->lz)) return fail("h_wm must lie below the half height");
   if (p->van_driest && (p->bc_z != BC_WALL || p->bc_y == BC_WALL || p->wall_model)) return fail("van Driest: z walls only, no wall model");
   oracle_solver* S = new oracle_solver();
@@ -817,12 +816,23 @@ static void substep(oracle_solver& S, int rk, double dt) {
         for (int comp = 0; comp < 2; ++comp) {     // u, v: centred in z, no-slip ghost folded into the diagonal
           F3& q = comp == 0 ? us : vs; const double* lz = comp == 0 ? dzu.data() : dzv.data();
           if (comp == 1 && j >= jvmax) continue;
+          const F3& q0 = comp == 0 ? S.u : S.v;
           for (int k = 0; k < nz; ++k) {
             double ak = 1.0 / (S.dzf(k) * S.dzc(k - 1)), ck = 1.0 / (S.dzf(k) * S.dzc(k));
             a[k] = -cimp * ak; c[k] = -cimp * ck; b[k] = 1.0 + cimp * (ak + ck);
-            if (k == 0) b[k] += cimp * ak;           // u[-1] = -u[0]
-            if (k == nz - 1) b[k] += cimp * ck;      // u[nz] = -u[nz-1]
-            d[k] = q(i, j, k) - cimp * (lz[S.id(i, j, k)] / nu);
+            if (!S.P.wall_model) {
+              if (k == 0) b[k] += cimp * ak;           // u[-1] = -u[0]
+              if (k == nz - 1) b[k] += cimp * ck;      // u[nz] = -u[nz-1]
+              d[k] = q(i, j, k) - cimp * (lz[S.id(i, j, k)] / nu);
+            } else {
+              // with the wall model the wall flux is the prescribed, lagged stress: it
+              // is a source s in L_zz u = Lt u + s that appears on both sides of Eq. 21 and cancels; the implicit operator
+              // Lt has the zero-flux (Neumann) closure at the walls, and the right-hand side uses Lt u^k.
+              if (k == 0) b[k] -= cimp * ak;
+              if (k == nz - 1) b[k] -= cimp * ck;
+              double lt = ((k < nz - 1 ? (q0(i, j, k + 1) - q0(i, j, k)) / S.dzc(k) : 0.0) - (k > 0 ? (q0(i, j, k) - q0(i, j, k - 1)) / S.dzc(k - 1) : 0.0)) / S.dzf(k);
+              d[k] = q(i, j, k) - cimp * lt;
+            }
           }
           oracle_thomas(nz, a.data(), b.data(), c.data(), d.data(), x.data());
           for (int k = 0; k < nz; ++k) q(i, j, k) = x[k];

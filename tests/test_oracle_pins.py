@@ -566,3 +566,48 @@ def test_cfl_time_step_and_plane_statistics_vs_numpy(oracle, bc_y, bc_z, stretch
     ref = [uc, vc, wc, uc * uc, vc * vc, wc * wc, uc * wc, nut]
     for q in range(8):
         assert np.max(np.abs(st[q] - ref[q].mean(axis=(1, 2)))) <= 1e-13 * max(1.0, np.max(np.abs(ref[q])))
+
+
+# ----------------------------------------------------------------------------- SURVEY.md 8(f) item 1
+def test_wall_model_with_implicit_z_matches_explicit_to_second_order(oracle):
+    """Crank-Nicolson in z together with the wall model: the modelled stress is a lagged source, the implicit
+    operator has the zero-flux closure.  Against the explicit scheme the difference after a fixed NUMBER of steps must
+    shrink ~4x per halving of dt (a wrong closure or a dropped source leaves an O(dt) difference per step: ratio 2)."""
+    nx, ny, nz = 8, 6, 16
+    kw = dict(bc_z=1, nu=2e-3, sgs_model=1, cs=0.1, wall_model=1, const_flow_rate=0)
+    rng = np.random.default_rng(9)
+    zc = (np.arange(nz) + 0.5) * 2.0 / nz
+    u0 = np.broadcast_to((np.log(np.minimum(zc, 2 - zc) * 500) / 0.41 + 5.2)[:, None, None], (nz, ny, nx)) + 0.3 * rng.standard_normal((nz, ny, nx))
+    v0 = 0.3 * rng.standard_normal((nz, ny, nx)); w0 = 0.3 * rng.standard_normal((nz, ny, nx)); w0[-1] = 0.0
+    o = oracle.Oracle(nx, ny, nz, 3.0, 2.0, 2.0, **kw); o.set_velocity(u0, v0, w0); o.project(); u0, v0, w0 = o.velocity()
+    errs = []
+    for dt in (2e-3, 1e-3, 5e-4):              # 4 steps each: the per-step (local) difference is O(dt^2), as in P14's pin
+        res = []
+        for imp in (0, 1):
+            s = oracle.Oracle(nx, ny, nz, 3.0, 2.0, 2.0, implicit_z=imp, **kw)
+            s.set_velocity(u0, v0, w0)
+            for _ in range(4):
+                s.step(dt)
+            res.append(s.get(0))
+        errs.append(np.max(np.abs(res[0] - res[1])))
+    assert errs[0] < 1e-3 * np.max(np.abs(u0))
+    assert 3.0 < errs[0] / errs[1] < 5.5 and 3.0 < errs[1] / errs[2] < 5.5, errs
+
+
+def test_wall_model_with_implicit_z_momentum_balance(oracle):
+    """Uniform-in-x,y field, no advection, no SGS: over one step the dzf-weighted column sum of u changes by
+    -sum_substeps gamma dt (tau_bottom + tau_top) exactly; with nu so small that tau barely moves over the step the three
+    lagged stresses equal the initial one to O(dt), which bounds the check."""
+    nx, ny, nz = 4, 4, 12
+    o = oracle.Oracle(nx, ny, nz, 1.0, 1.0, 2.0, bc_z=1, nu=1e-3, sgs_model=0, wall_model=1, implicit_z=1)
+    zc = o.zc
+    prof = np.log(np.minimum(zc, 2 - zc) * 1000) / 0.41 + 5.2
+    u = np.broadcast_to(prof[:, None, None], (nz, ny, nx)).copy()
+    o.set_velocity(u, np.zeros_like(u), np.zeros_like(u))
+    tau = o.wall_stress()                      # [wall][comp][ny][nx]
+    dt = 1e-4
+    m0 = np.sum(o.get(0)[:, 0, 0] * o.dzf)
+    o.step(dt)
+    m1 = np.sum(o.get(0)[:, 0, 0] * o.dzf)
+    expect = -dt * (tau[0, 0, 0, 0] + tau[1, 0, 0, 0])
+    assert abs((m1 - m0) - expect) <= 2e-3 * abs(expect)
