@@ -90,7 +90,7 @@ size_t cales_workspace_bytes(const cales_params* p);
 
 /* Create a solver.  Validates the parameters (CALES_EINVAL: bad sizes / null pointers / workspace too small;
  * CALES_EUNSUPPORTED: sizes that do not factor into 2 and 3, odd nx or ny, periodic z with stretching, wall model
- * without z walls or together with implicit_z, van Driest without z walls / with y walls / with the wall model),
+ * without z walls, van Driest without z walls / with y walls / with the wall model),
  * builds the grid and the transform tables on the host, uploads them into the workspace, zeroes all fields.
  * Synchronises the stream. */
 int cales_create(const cales_params* p, cales_solver** out);

@@ -37,7 +37,6 @@ static inline int validate(const cales_params* p) {
   if (p->sgs_model < 0 || p->sgs_model > 2) return fail(CALES_EINVAL, "bad sgs_model");
   if (p->wall_model && p->bc_z != CALES_BC_WALL) return fail(CALES_EUNSUPPORTED, "wall model needs z walls");
   if (p->implicit_z && p->bc_z != CALES_BC_WALL) return fail(CALES_EUNSUPPORTED, "implicit z needs z walls");
-  if (p->implicit_z && p->wall_model) return fail(CALES_EUNSUPPORTED, "wall model with implicit z is not supported");
   if (p->wall_model && p->h_wm > 0.0 && !(p->h_wm < 0.5 * p->lz)) return fail(CALES_EINVAL, "h_wm must lie below the half height");
   if (p->van_driest && (p->bc_z != CALES_BC_WALL || p->bc_y == CALES_BC_WALL || p->wall_model))
     return fail(CALES_EUNSUPPORTED, "van Driest damping: z walls only, no wall model");

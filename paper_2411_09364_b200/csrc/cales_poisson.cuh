@@ -120,8 +120,10 @@ CALES_HD void cn_coefficients(const Ctx& c, double cimp, double* coef) {
   for (int k = 0; k < nz; ++k) {
     const double ak = 1.0 / (c.dzf[k] * c.dzc[k - 1]), ck = 1.0 / (c.dzf[k] * c.dzc[k]);
     double b = 1.0 + cimp * (ak + ck);
-    if (k == 0) b += cimp * ak;
-    if (k == nz - 1) b += cimp * ck;
+    // walls: no-slip ghost folded into the diagonal, or -- with the wall model, whose lagged stress is a source that cancels in
+    // Eq. 21 -- the zero-flux closure
+    if (k == 0) b += c.wall_model ? -cimp * ak : cimp * ak;
+    if (k == nz - 1) b += c.wall_model ? -cimp * ck : cimp * ck;
     const double a = -cimp * ak, cc = -cimp * ck;
     const double r = 1.0 / (k == 0 ? b : b - a * cp);
     cp = cc * r;

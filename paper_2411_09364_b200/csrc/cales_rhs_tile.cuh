@@ -94,8 +94,14 @@ CALES_HD double rhs_core(const Ctx& c, const RhsArgs& a, const A& q, int i, int 
   double vs = v000 + a.dt * (a.al * Rv + a.be * rv0 - a.ga * gpy);
   double ws = w000 + a.dt * (a.al * Rw + a.be * rw0 - a.ga * gpz);
   if (c.implicit_z) {   // Eq. 20 explicit half + right-hand side of Eq. 21
-    const double f = a.dt * a.ga * c.nu - 0.5 * a.ga * c.nu * a.dt;
-    us += f * lzu; vs += f * lzv; ws += f * lzw;
+    const double fe = a.dt * a.ga * c.nu, fi = 0.5 * a.ga * c.nu * a.dt;
+    double ltu = lzu, ltv = lzv;        // L_zz of the implicit operator applied to u^k
+    if (c.wall_model) {                 // zero-flux closure: the modelled wall stress is a source outside the implicit operator
+      const double up = (k < c.nz - 1) ? 1.0 : 0.0, lo = (k > 0) ? 1.0 : 0.0;
+      ltu = (up * (u00p - u000) * rdzc - lo * (u000 - u00m) * rdzcm) * rdzf;
+      ltv = (up * (v00p - v000) * rdzc - lo * (v000 - v00m) * rdzcm) * rdzf;
+    }
+    us += fe * lzu - fi * ltu; vs += fe * lzv - fi * ltv; ws += (fe - fi) * lzw;
   }
   if (!vact) vs = 0.0;
   if (!wact) ws = 0.0;

@@ -19,6 +19,7 @@ SMALL = {
     "cfg5_wmles_dsm": (5, (36, 24, 16), 2),
     "duct_static_smag": (4, (24, 12, 12), 2, dict(sgs_model=1, cs=0.1)),   # static model next to y walls
     "cfg5_hwm_interp": (5, (24, 12, 16), 2, dict(h_wm=0.1)),               # wall model sampled between centres
+    "cfg2_wm_implicit": (2, (24, 12, 16), 2, dict(implicit_z=1)),          # wall model + Crank-Nicolson in z (8(f) item 1)
 }
 # the sizes the GPU parity tests use: several tiles in every direction plus ragged tails
 GPU_CASES = {
@@ -30,6 +31,8 @@ GPU_CASES = {
     "duct_static_smag": (4, (96, 36, 24), 2, dict(sgs_model=1, cs=0.1)),
     "cfg5_hwm_interp": (5, (96, 48, 32), 2, dict(h_wm=0.1)),
     "cfg4_duct_dsm_narrow": (4, (72, 18, 16), 2),
+    "cfg2_wm_implicit": (2, (96, 48, 32), 3, dict(implicit_z=1)),
+    "cfg5_wm_implicit_dsm": (5, (96, 48, 32), 2, dict(implicit_z=1, h_wm=0.1)),
 }
 
 

@@ -54,7 +54,6 @@ def test_defaults_and_workspace_size(binding):
     (dict(bc_z=0, zstretch=1), "uniform"),
     (dict(wall_model=1, bc_z=0), "wall model needs z walls"),
     (dict(implicit_z=1, bc_z=0), "implicit z needs z walls"),
-    (dict(implicit_z=1, wall_model=1, bc_z=1), "not supported"),
     (dict(van_driest=1, bc_z=0), "van Driest"),
     (dict(nu=0.0), "nu must be positive"),
     (dict(lx=-1.0), "positive"),
