@@ -50,7 +50,6 @@ struct cales_solver {
   dim3 pgrid, pblock;   // point kernels
   long long nblk;
   bool fresh;
-  int zs_tile;          // shared-memory tile form of the z solves (0: thread-per-column kernels only; tests)
   long long tile_min;   // grids with at least this many points use the staged z-march for the static model
   int use_graph; cudaGraphExec_t gexec; double gdt;   // the three substeps captured as one CUDA graph, keyed by dt
   int timing; bool ev_valid;
@@ -60,12 +59,6 @@ struct cales_solver {
 };
 
 static size_t al32(size_t n) { return (n + 31) / 32 * 32; }
-
-// columns per CTA of the shared-memory z solves (narr staged arrays of nz doubles per column): 32 or 16, 0 = does not fit
-static int zs_tc(int nz, int narr) {
-  for (int tc : {32, 16}) if ((size_t)narr * nz * tc * sizeof(double) <= 72 * 1024) return tc;
-  return 0;
-}
 
 // Carve the workspace.  With base == nullptr only the size is computed.
 static size_t carve(cales_solver* s, const cales_params* p, double* base) {
@@ -188,8 +181,6 @@ extern "C" int cales_create(const cales_params* p, cales_solver** out) {
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fft2_x_inv, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fft2_y, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rhs_tile, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(RT_SMEM_DOUBLES * sizeof(double)));
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_poisson_z_tile, cudaFuncAttributeMaxDynamicSharedMemorySize, 80 * 1024);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_cn_z_tile, cudaFuncAttributeMaxDynamicSharedMemorySize, 80 * 1024);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_smag_tile, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(ST_SMEM_DOUBLES * sizeof(double)));
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dsm_pass1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(DSM_SMEM_DOUBLES * sizeof(double)));
   if (e != cudaSuccess) { delete s; return fail(CALES_ECUDA, std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e)); }
@@ -198,8 +189,6 @@ extern "C" int cales_create(const cales_params* p, cales_solver** out) {
   s->fresh = false; s->timing = 0; s->ev_valid = false; s->launches = 0; s->evn = 0;
   s->use_graph = 1; s->gexec = nullptr; s->gdt = 0.0;
   s->tile_min = 4000000;
-  s->zs_tile = 1;
-  if (const char* e = std::getenv("CALES_ZS_TILE")) s->zs_tile = std::atoi(e);
   if (const char* e = std::getenv("CALES_TILE_MIN_POINTS")) s->tile_min = std::atoll(e);   // tests force either path
   for (int q = 0; q < 32; ++q) { s->kms[q] = 0.0; s->kcnt[q] = 0; }
   *out = s;
@@ -275,9 +264,8 @@ static int run_transform_y(cales_solver* s, double* A, int inverse) {
   return CALES_OK;
 }
 static int run_poisson_z(cales_solver* s, double* A) {
-  const int TC = s->c.bc_z == BC_WALL ? zs_tc(s->c.nz, 2) : 0;
-  if (TC && s->zs_tile) k_poisson_z_tile<<<(unsigned)((s->nxy + TC - 1) / TC), 256, (size_t)2 * s->c.nz * TC * sizeof(double), s->st>>>(s->c, s->pt, TC, A);
-  else { const int th = 128; k_poisson_z<<<(unsigned)((s->nxy + th - 1) / th), th, 0, s->st>>>(s->c, s->pt, A, s->CP, s->CQ); }
+  const int th = 128;
+  k_poisson_z<<<(unsigned)((s->nxy + th - 1) / th), th, 0, s->st>>>(s->c, s->pt, A, s->CP, s->CQ);
   LAUNCH_TRY(K_POISSON_Z);
   return CALES_OK;
 }
@@ -364,18 +352,10 @@ static int substep(cales_solver* s, int rk, double dt) {
     const double cimp = 0.5 * ga * c.nu * dt;
     k_cn_coef<<<1, 32, 0, s->st>>>(c, cimp, s->cncoef);
     LAUNCH_TRY(K_CN_COEF);
-    const int TC = zs_tc(c.nz, 1);
-    unsigned g;
-    if (TC && s->zs_tile) {
-      g = (unsigned)((s->nxy + TC - 1) / TC);
-      k_cn_z_tile<<<dim3(g, 3), 256, (size_t)c.nz * TC * sizeof(double), s->st>>>(c, s->cncoef, TC, s->us, s->vs, s->ws, cfr ? s->partial : nullptr);
-      LAUNCH_TRY(K_CN_Z);
-    } else {
-      const int th = 128; g = (unsigned)((s->nxy + th - 1) / th);
-      k_cn_z<<<g, th, 0, s->st>>>(c, s->cncoef, 0, s->us, cfr ? s->partial : nullptr); LAUNCH_TRY(K_CN_Z);
-      k_cn_z<<<g, th, 0, s->st>>>(c, s->cncoef, 1, s->vs, nullptr); LAUNCH_TRY(K_CN_Z);
-      k_cn_z<<<g, th, 0, s->st>>>(c, s->cncoef, 2, s->ws, nullptr); LAUNCH_TRY(K_CN_Z);
-    }
+    const int th = 128; const unsigned g = (unsigned)((s->nxy + th - 1) / th);
+    k_cn_z<<<g, th, 0, s->st>>>(c, s->cncoef, 0, s->us, cfr ? s->partial : nullptr); LAUNCH_TRY(K_CN_Z);
+    k_cn_z<<<g, th, 0, s->st>>>(c, s->cncoef, 1, s->vs, nullptr); LAUNCH_TRY(K_CN_Z);
+    k_cn_z<<<g, th, 0, s->st>>>(c, s->cncoef, 2, s->ws, nullptr); LAUNCH_TRY(K_CN_Z);
     npart = g;
   }
   if (cfr) {
@@ -447,7 +427,7 @@ extern "C" int cales_set_graph(cales_solver* s, int on) {
 extern "C" int cales_launches_per_step(cales_solver* s) {
   if (!s) return 0;
   const Ctx& c = s->c;
-  int per = 1 /*rhs*/ + (c.implicit_z ? ((zs_tc(c.nz, 1) && s->zs_tile) ? 2 : 4) : 0) + (c.const_flow_rate ? 2 : 0) + 5 /*solver*/ + 1 /*correct*/ + (c.wall_model ? 1 : 0) +
+  int per = 1 /*rhs*/ + (c.implicit_z ? 4 : 0) + (c.const_flow_rate ? 2 : 0) + 5 /*solver*/ + 1 /*correct*/ + (c.wall_model ? 1 : 0) +
             1 /*static nu_t or fill*/;
   if (c.sgs == CALES_SGS_DSMAG) {
     const bool ywall = c.bc_y == BC_WALL, split = ywall && c.ny >= 3 * DSM_TY;

@@ -19,11 +19,9 @@ struct PoissonTabs {
 // Poisson column (i,j): [a_k, b_k, c_k] phi = f with b_k = -(a_k + c_k) + lam_x + lam_y, a_0 and c_{nz-1} dropped from
 // b at walls (Neumann) or wrapped (periodic z: cyclic Thomas via Sherman-Morrison).  The singular (0,0) mode drops the
 // dzf-weighted mean of f, pins phi[0] = 0, and returns the solution with zero dzf-weighted mean (S15).
-// `_at`: A, CP, CQ already point at level 0 of the column and consecutive levels are `st` elements apart (global field:
-// st = nx*ny; shared-memory tile: st = columns per tile).
-CALES_HD void poisson_column_at(const Ctx& c, const PoissonTabs& T, int i, int j, double* __restrict__ A, double* __restrict__ CP, double* __restrict__ CQ, long long st) {
+CALES_HD void poisson_column(const Ctx& c, const PoissonTabs& T, int i, int j, double* __restrict__ A, double* __restrict__ CP, double* __restrict__ CQ) {
   const int nz = c.nz;
-  const long long col = 0;
+  const long long col = (long long)i + (long long)c.nx * j, st = c.nxy;
   const double lam = T.lamx[i] + T.lamy[j];
   const bool per = c.bc_z == BC_PER;
   const bool zero = (i == 0 && j == 0);
@@ -145,8 +143,8 @@ CALES_HD void cn_coefficients(const Ctx& c, double cimp, double* coef) {
 
 // Solve (1 - c L_zz) q* = d in place for one column; m = number of unknowns (nz for u, v; nz-1 for w).
 // Returns sum_k q*[k] dzf[k] (used for the bulk velocity of u*).
-CALES_HD double cn_column_at(const Ctx& c, const double* coef, int m, double* __restrict__ Q, long long st) {
-  const int nz = c.nz; const long long col = 0;
+CALES_HD double cn_column(const Ctx& c, const double* coef, int m, long long col, double* __restrict__ Q) {
+  const int nz = c.nz; const long long st = c.nxy;
   const double* a = coef; const double* cp = coef + nz; const double* r = coef + 2 * nz;
   enum { TZ = 8 };
   double dp = 0.0;
@@ -181,12 +179,6 @@ CALES_HD double cn_column_at(const Ctx& c, const double* coef, int m, double* __
   return s;
 }
 
-CALES_HD void poisson_column(const Ctx& c, const PoissonTabs& T, int i, int j, double* __restrict__ A, double* __restrict__ CP, double* __restrict__ CQ) {
-  const long long col = (long long)i + (long long)c.nx * j;
-  poisson_column_at(c, T, i, j, A + col, CP + col, CQ ? CQ + col : nullptr, c.nxy);
-}
-CALES_HD double cn_column(const Ctx& c, const double* coef, int m, long long col, double* __restrict__ Q) { return cn_column_at(c, coef, m, Q + col, c.nxy); }
-
 #ifdef __CUDACC__
 __global__ void k_poisson_z(Ctx c, PoissonTabs T, double* __restrict__ A, double* __restrict__ CP, double* __restrict__ CQ) {
   const long long col = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -208,68 +200,6 @@ __global__ void k_cn_z(Ctx c, const double* __restrict__ coef, int comp, double*
   }
   if (partial) {
     const double t = block_sum(s, sh);
-    if (threadIdx.x == 0) partial[blockIdx.x] = t;
-  }
-}
-// ------------------------------------------------------------------------------------------------------------
-// Shared-memory tile form of the z solves (wall-bounded z, nz small enough for the tile): a CTA stages TC adjacent
-// columns x all nz levels by cp.async, TC threads run the serial sweeps on the staged tile (the forward-sweep
-// intermediates d', c' never leave shared memory), then all threads write the solution back: 16 B per point of HBM
-// traffic instead of 32 (Crank-Nicolson) / 46 (Poisson), with 3-4 CTAs per SM overlapping their load / solve / store phases.
-// Columns are the flattened (i + nx j) index, so a tile is contiguous in memory at every level.
-// ------------------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void zs_load_tile(const Ctx& c, const double* __restrict__ src, long long col0, int ncols, int TC, double* tile) {
-  for (int e = threadIdx.x; e < c.nz * TC; e += blockDim.x) {
-    const int k = e / TC, cc = e - k * TC;
-    if (cc < ncols) cp_async8(tile + e, src + col0 + cc + c.nxy * (long long)k);
-  }
-  cp_async_commit();
-}
-__device__ __forceinline__ void zs_store_tile(const Ctx& c, double* __restrict__ dst, long long col0, int ncols, int TC, const double* tile) {
-  for (int e = threadIdx.x; e < c.nz * TC; e += blockDim.x) {
-    const int k = e / TC, cc = e - k * TC;
-    if (cc < ncols) dst[col0 + cc + c.nxy * (long long)k] = tile[e];
-  }
-}
-// grid ceil(nxy / TC), dynamic smem 2 * nz * TC doubles
-__global__ void __launch_bounds__(256) k_poisson_z_tile(const __grid_constant__ Ctx c, PoissonTabs T, int TC, double* __restrict__ A) {
-  extern __shared__ double zs_sm[];
-  double* D = zs_sm; double* CPs = zs_sm + (size_t)c.nz * TC;
-  const long long col0 = (long long)blockIdx.x * TC;
-  const int ncols = (int)min((long long)TC, c.nxy - col0);
-  zs_load_tile(c, A, col0, ncols, TC, D);
-  cp_async_wait_all();
-  __syncthreads();
-  if ((int)threadIdx.x < ncols) {
-    const long long col = col0 + threadIdx.x;
-    poisson_column_at(c, T, (int)(col % c.nx), (int)(col / c.nx), D + threadIdx.x, CPs + threadIdx.x, nullptr, TC);
-  }
-  __syncthreads();
-  zs_store_tile(c, A, col0, ncols, TC, D);
-}
-// grid (ceil(nxy / TC), 3 components), dynamic smem nz * TC doubles; partial[blockIdx.x] = sum of u* dzf over the tile (comp 0)
-__global__ void __launch_bounds__(256) k_cn_z_tile(const __grid_constant__ Ctx c, const double* __restrict__ coef, int TC, double* __restrict__ us,
-                                                   double* __restrict__ vs, double* __restrict__ ws, double* __restrict__ partial) {
-  extern __shared__ double zs_sm[];
-  __shared__ double red[32];
-  const int comp = blockIdx.y;
-  double* Q = comp == 0 ? us : (comp == 1 ? vs : ws);
-  const long long col0 = (long long)blockIdx.x * TC;
-  const int ncols = (int)min((long long)TC, c.nxy - col0);
-  zs_load_tile(c, Q, col0, ncols, TC, zs_sm);
-  cp_async_wait_all();
-  __syncthreads();
-  double s = 0.0;
-  if ((int)threadIdx.x < ncols) {
-    const long long col = col0 + threadIdx.x;
-    const int j = (int)(col / c.nx);
-    const bool skip = (comp == 1 && c.bc_y == BC_WALL && j == c.ny - 1);   // the +y wall face stays 0
-    if (!skip) s = cn_column_at(c, comp == 2 ? coef + 3 * c.nz : coef, comp == 2 ? c.nz - 1 : c.nz, zs_sm + threadIdx.x, TC);
-  }
-  __syncthreads();
-  zs_store_tile(c, Q, col0, ncols, TC, zs_sm);
-  if (comp == 0 && partial) {
-    const double t = block_sum(s, red);
     if (threadIdx.x == 0) partial[blockIdx.x] = t;
   }
 }

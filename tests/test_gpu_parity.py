@@ -318,19 +318,3 @@ def test_cfl_dt_and_plane_stats_parity(oracle, gpu, n, shape):
     for q in range(8):
         assert np.max(np.abs(sa[q] - sb[q])) <= 1e-11 * scale[q], q
     g.close()
-
-
-@pytest.mark.parametrize("n,shape", [(3, (96, 72, 48)), (4, (96, 36, 24)), (2, (72, 48, 24))])
-def test_thread_per_column_z_solves_parity(oracle, gpu, n, shape, monkeypatch):
-    """The thread-per-column Thomas kernels (used when the column tile does not fit shared memory, e.g. nz = 512) forced on
-    at test sizes; the default at these sizes is the shared-memory tile form."""
-    monkeypatch.setenv("CALES_ZS_TILE", "0")
-    cfg, kw, (u, v, w), dt = pc.prepare(oracle, n, shape)
-    o = pc.make(oracle.Oracle, kw)
-    g = pc.make(gpu.Solver, kw)
-    o.set_velocity(u, v, w); g.set_velocity(u, v, w)
-    for _ in range(2):
-        o.step(dt); g.step(dt)
-    err = pc.field_errors(_gpu_fields(g), [o.get(f) for f in range(5)], o.dzf, kw["nu"])
-    assert max(err.values()) <= 1e-10, err
-    g.close()
