@@ -50,7 +50,6 @@ struct cales_solver {
   dim3 pgrid, pblock;   // point kernels
   long long nblk;
   bool fresh;
-  int pz_ck;            // checkpointed Thomas sweeps for wall-bounded z (0: store c', d' of every level; tests)
   long long tile_min;   // grids with at least this many points use the staged z-march for the static model
   int use_graph; cudaGraphExec_t gexec; double gdt;   // the three substeps captured as one CUDA graph, keyed by dt
   int timing; bool ev_valid;
@@ -190,8 +189,6 @@ extern "C" int cales_create(const cales_params* p, cales_solver** out) {
   s->fresh = false; s->timing = 0; s->ev_valid = false; s->launches = 0; s->evn = 0;
   s->use_graph = 1; s->gexec = nullptr; s->gdt = 0.0;
   s->tile_min = 4000000;
-  s->pz_ck = 1;
-  if (const char* e = std::getenv("CALES_PZ_CK")) s->pz_ck = std::atoi(e);
   if (const char* e = std::getenv("CALES_TILE_MIN_POINTS")) s->tile_min = std::atoll(e);   // tests force either path
   for (int q = 0; q < 32; ++q) { s->kms[q] = 0.0; s->kcnt[q] = 0; }
   *out = s;
@@ -268,8 +265,7 @@ static int run_transform_y(cales_solver* s, double* A, int inverse) {
 }
 static int run_poisson_z(cales_solver* s, double* A) {
   const int th = 128;
-  if (s->c.bc_z == BC_WALL && s->pz_ck) k_poisson_z_ck<<<(unsigned)((s->nxy + th - 1) / th), th, 0, s->st>>>(s->c, s->pt, A, s->CP);
-  else k_poisson_z<<<(unsigned)((s->nxy + th - 1) / th), th, 0, s->st>>>(s->c, s->pt, A, s->CP, s->CQ);
+  k_poisson_z<<<(unsigned)((s->nxy + th - 1) / th), th, 0, s->st>>>(s->c, s->pt, A, s->CP, s->CQ);
   LAUNCH_TRY(K_POISSON_Z);
   return CALES_OK;
 }

@@ -111,69 +111,6 @@ CALES_HD void poisson_column(const Ctx& c, const PoissonTabs& T, int i, int j, d
   for (int k = 0; k < nz; ++k) A[col + st * k] -= f * CQ[col + st * k];
 }
 
-// Wall-bounded z, checkpointed form: the forward sweep keeps only (c', d') at the start of every PZ_SEG-level segment
-// (in the column's slot of the scratch field CP: 2 values per segment); the backward pass walks the segments from the
-// top, re-runs the forward recurrence of one segment from its checkpoint into a small per-thread scratch (shared memory
-// on the GPU) and back-substitutes it.  The right-hand side is read twice and the solution written once: 24 B per point
-// of HBM traffic instead of 46 for storing and re-reading c' and d' of every level.  In place: a segment's right-hand
-// side is re-read before the solution overwrites it, and lower segments are still untouched at that time.
-// scratch: 2*PZ_SEG doubles of this thread, level l at scratch[(2l) * sst] (c') and scratch[(2l+1) * sst] (d').
-enum { PZ_SEG = 16 };
-CALES_HD void poisson_column_ck(const Ctx& c, const PoissonTabs& T, int i, int j, double* __restrict__ A, double* __restrict__ CP,
-                                double* __restrict__ scratch, int sst) {
-  const int nz = c.nz;
-  const long long col = (long long)i + (long long)c.nx * j, st = c.nxy;
-  const double lam = T.lamx[i] + T.lamy[j];
-  const bool zero = (i == 0 && j == 0);
-  const int nseg = (nz + PZ_SEG - 1) / PZ_SEG;
-  double mean = 0.0;
-  if (zero) {
-    for (int k = 0; k < nz; ++k) mean += A[col + st * k] * c.dzf[k];
-    mean /= c.lz;
-  }
-  // one level of the forward recurrence (row 0 of the singular mode pins phi[0] = 0)
-  auto fwd = [&](int k, double d, double& cp, double& dp) {
-    const double a = T.ak[k], cc = T.ck[k];
-    const double b = lam - (k > 0 ? a : 0.0) - (k < nz - 1 ? cc : 0.0);
-    if (zero && k == 0) { cp = 0.0; dp = 0.0; }
-    else { const double r = 1.0 / (b - a * cp); cp = cc * r; dp = (d - mean - a * dp) * r; }
-  };
-  double cp = 0.0, dp = 0.0;
-  for (int sg = 0; sg < nseg; ++sg) {
-    const int k0 = sg * PZ_SEG;
-    CP[col + st * (2 * sg)] = cp; CP[col + st * (2 * sg + 1)] = dp;       // state entering the segment (2*nseg <= nz slots)
-    double dd[PZ_SEG];
-#pragma unroll
-    for (int q = 0; q < PZ_SEG; ++q) dd[q] = (k0 + q < nz) ? A[col + st * (k0 + q)] : 0.0;
-#pragma unroll
-    for (int q = 0; q < PZ_SEG; ++q) if (k0 + q < nz) fwd(k0 + q, dd[q], cp, dp);
-  }
-  double x = 0.0, s = 0.0;
-  for (int sg = nseg - 1; sg >= 0; --sg) {
-    const int k0 = sg * PZ_SEG, k1 = (k0 + PZ_SEG < nz) ? k0 + PZ_SEG : nz;
-    double dd[PZ_SEG];
-#pragma unroll
-    for (int q = 0; q < PZ_SEG; ++q) dd[q] = (k0 + q < nz) ? A[col + st * (k0 + q)] : 0.0;
-    double cq = CP[col + st * (2 * sg)], dq = CP[col + st * (2 * sg + 1)];
-#pragma unroll
-    for (int q = 0; q < PZ_SEG; ++q) if (k0 + q < nz) {
-      fwd(k0 + q, dd[q], cq, dq);
-      scratch[(2 * q) * sst] = cq; scratch[(2 * q + 1) * sst] = dq;
-    }
-#pragma unroll
-    for (int q = PZ_SEG - 1; q >= 0; --q) if (k0 + q < k1) {
-      const int k = k0 + q;
-      x = (k == nz - 1) ? scratch[(2 * q + 1) * sst] : scratch[(2 * q + 1) * sst] - scratch[(2 * q) * sst] * x;
-      A[col + st * k] = x;
-      s += x * c.dzf[k];
-    }
-  }
-  if (zero) {
-    s /= c.lz;
-    for (int k = 0; k < nz; ++k) A[col + st * k] -= s;
-  }
-}
-
 // Crank-Nicolson coefficients of Eq. 21 for substep constant cimp = gamma nu dt / 2, computed once per substep by one
 // thread: for the centred components (u, v; no-slip ghost folded into the diagonal) and for w (faces 0..nz-2).
 // Layout of `coef`: [0] lower a, [1] c' (modified upper), [2] 1/den for u,v; [3],[4],[5] the same for w.
@@ -247,13 +184,6 @@ __global__ void k_poisson_z(Ctx c, PoissonTabs T, double* __restrict__ A, double
   const long long col = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (col >= c.nxy) return;
   poisson_column(c, T, (int)(col % c.nx), (int)(col / c.nx), A, CP, CQ);
-}
-// wall-bounded z: checkpointed sweeps, 2*PZ_SEG doubles of shared-memory scratch per thread (level stride = blockDim.x)
-__global__ void __launch_bounds__(128) k_poisson_z_ck(Ctx c, PoissonTabs T, double* __restrict__ A, double* __restrict__ CP) {
-  __shared__ double pz_scr[2 * PZ_SEG * 128];
-  const long long col = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (col >= c.nxy) return;
-  poisson_column_ck(c, T, (int)(col % c.nx), (int)(col / c.nx), A, CP, pz_scr + threadIdx.x, 128);
 }
 __global__ void k_cn_coef(Ctx c, double cimp, double* coef) {
   if (blockIdx.x == 0 && threadIdx.x == 0) cn_coefficients(c, cimp, coef);

@@ -139,11 +139,7 @@ static void emu_fft_y(emu_solver* s, double* A, int inverse) {
 }
 static void emu_poisson_core(emu_solver* s) {
   emu_fft_y(s, s->W.data(), 0);
-  double scr[2 * PZ_SEG];
-  for (int j = 0; j < s->c.ny; ++j) for (int i = 0; i < s->c.nx; ++i) {
-    if (s->c.bc_z == BC_WALL) poisson_column_ck(s->c, s->pt, i, j, s->W.data(), s->CP.data(), scr, 1);
-    else poisson_column(s->c, s->pt, i, j, s->W.data(), s->CP.data(), s->CQ.data());
-  }
+  for (int j = 0; j < s->c.ny; ++j) for (int i = 0; i < s->c.nx; ++i) poisson_column(s->c, s->pt, i, j, s->W.data(), s->CP.data(), s->CQ.data());
   emu_fft_y(s, s->W.data(), 1);
 }
 static void emu_tau(emu_solver* s) {
