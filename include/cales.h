@@ -121,8 +121,8 @@ int cales_step(cales_solver* s, double dt);
 int cales_poisson_solve(cales_solver* s, const double* rhs_dev, double* phi_dev);
 
 /* nu_t (Eq. 4 or Eq. 5-9) of a velocity field.  u, v, w: DEVICE fields, or all NULL = the solver's own velocity;
- * nut: DEVICE output, nz*ny*nx (NULL = the solver's own nu_t).  Uses the stored wall stresses only through the
- * velocity ghosts.  Asynchronous. */
+ * nut: DEVICE output, nz*ny*nx (NULL = the solver's own nu_t).  External fields must hold 0 on the wall faces
+ * (v[.][ny-1][.] with y walls, w[nz-1] with z walls), as the solver's own fields always do.  Asynchronous. */
 int cales_eddy_viscosity(cales_solver* s, const double* u, const double* v, const double* w, double* nut);
 
 /* Wall stresses of the log-law wall model from the solver's velocity (Eq. 10):
