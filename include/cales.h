@@ -111,7 +111,8 @@ int cales_get_field(cales_solver* s, int field, double* dst, int dst_on_device);
 
 /* One full RK3 step = 3 substeps of Alg. 1 with the coefficients of PAPER.md:100:
  * u* from Eq. 11 (or Eq. 20-21), bulk forcing, Poisson Eq. 12, correction Eq. 13, pressure Eq. 14 / 22,
- * wall stress Eq. 10, nu_t Eq. 4 / Eq. 5-9.  Asynchronous.  dt > 0. */
+ * wall stress Eq. 10, nu_t Eq. 4 / Eq. 5-9.  Asynchronous, except that the first call with a new dt in implicit-z mode
+ * uploads the Crank-Nicolson coefficient tables of that dt and synchronises the stream once.  dt > 0. */
 int cales_step(cales_solver* s, double dt);
 
 /* Solve L_h phi = rhs with the solver's boundary conditions (Eq. 12; eigenfunction expansion,

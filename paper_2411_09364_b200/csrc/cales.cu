@@ -51,6 +51,7 @@ struct cales_solver {
   long long nblk;
   bool fresh;
   long long tile_min;   // grids with at least this many points use the staged z-march for the static model
+  std::vector<double> h_dzf, h_dzc, h_cn; Ctx hc; double cn_dt;   // host copies for the per-dt CN coefficient tables
   int use_graph; cudaGraphExec_t gexec; double gdt;   // the three substeps captured as one CUDA graph, keyed by dt
   int timing; bool ev_valid;
   std::vector<cudaEvent_t> evpool; std::vector<int> evkid; int evn;   // per-launch events of the last timed step
@@ -76,7 +77,7 @@ static size_t carve(cales_solver* s, const cales_params* p, double* base) {
   double* ak = take(p->nz); double* ck = take(p->nz);
   double* lamx = take(p->nx); double* lamy = take(p->ny);
   double* twx = take(2 * (size_t)p->nx); double* twy = take(2 * (size_t)p->ny); double* dctw = take(2 * ((size_t)p->ny / 2 + 1));
-  double* cncoef = take(6 * (size_t)p->nz);
+  double* cncoef = take(18 * (size_t)p->nz);      // Crank-Nicolson coefficient tables of the three substeps
   const size_t nblk = (size_t)((p->nx + 31) / 32) * ((p->ny + 7) / 8) * p->nz;
   double* partial = take(nblk > nxy ? nblk : nxy);
   double* stage1 = take(4 * 1024);
@@ -188,6 +189,7 @@ extern "C" int cales_create(const cales_params* p, cales_solver** out) {
   s->pgrid = dim3((nx + 31) / 32, (ny + 7) / 8, nz);
   s->fresh = false; s->timing = 0; s->ev_valid = false; s->launches = 0; s->evn = 0;
   s->use_graph = 1; s->gexec = nullptr; s->gdt = 0.0;
+  s->h_dzf = H.dzf; s->h_dzc = H.dzc; s->hc = s->c; s->hc.dzf = s->h_dzf.data() + 1; s->hc.dzc = s->h_dzc.data() + 1; s->cn_dt = 0.0;
   s->tile_min = 4000000;
   if (const char* e = std::getenv("CALES_TILE_MIN_POINTS")) s->tile_min = std::atoll(e);   // tests force either path
   for (int q = 0; q < 32; ++q) { s->kms[q] = 0.0; s->kcnt[q] = 0; }
@@ -349,13 +351,10 @@ static int substep(cales_solver* s, int rk, double dt) {
   LAUNCH_TRY(K_RHS);
   long long npart = (long long)rgrid.x * rgrid.y * rgrid.z;
   if (imp) {
-    const double cimp = 0.5 * ga * c.nu * dt;
-    k_cn_coef<<<1, 32, 0, s->st>>>(c, cimp, s->cncoef);
-    LAUNCH_TRY(K_CN_COEF);
     const int th = 128; const unsigned g = (unsigned)((s->nxy + th - 1) / th);
-    k_cn_z<<<g, th, 0, s->st>>>(c, s->cncoef, 0, s->us, cfr ? s->partial : nullptr); LAUNCH_TRY(K_CN_Z);
-    k_cn_z<<<g, th, 0, s->st>>>(c, s->cncoef, 1, s->vs, nullptr); LAUNCH_TRY(K_CN_Z);
-    k_cn_z<<<g, th, 0, s->st>>>(c, s->cncoef, 2, s->ws, nullptr); LAUNCH_TRY(K_CN_Z);
+    k_cn_z<<<g, th, 0, s->st>>>(c, s->cncoef + (size_t)rk * 6 * c.nz, 0, s->us, cfr ? s->partial : nullptr); LAUNCH_TRY(K_CN_Z);
+    k_cn_z<<<g, th, 0, s->st>>>(c, s->cncoef + (size_t)rk * 6 * c.nz, 1, s->vs, nullptr); LAUNCH_TRY(K_CN_Z);
+    k_cn_z<<<g, th, 0, s->st>>>(c, s->cncoef + (size_t)rk * 6 * c.nz, 2, s->ws, nullptr); LAUNCH_TRY(K_CN_Z);
     npart = g;
   }
   if (cfr) {
@@ -384,6 +383,18 @@ extern "C" int cales_step(cales_solver* s, double dt) {
   int rc;
   s->launches = 0; s->evn = 0; s->ev_valid = false;
   if (!s->fresh && (rc = refresh_closures(s))) return rc;
+  if (s->c.implicit_z && dt != s->cn_dt) {
+    // Eq. 21's tridiagonal coefficients depend on k and on gamma*nu*dt only: like the grid metrics they are a host-built table,
+    // rebuilt when dt changes (the forward elimination of the constant matrix is a serial recurrence over nz levels)
+    s->h_cn.resize(18 * (size_t)s->c.nz);
+    for (int rk = 0; rk < 3; ++rk) {
+      double al, be, ga; rk3_coeffs(rk, al, be, ga);
+      cn_coefficients(s->hc, 0.5 * ga * s->c.nu * dt, s->h_cn.data() + (size_t)rk * 6 * s->c.nz);
+    }
+    CUDA_TRY(cudaMemcpyAsync(s->cncoef, s->h_cn.data(), s->h_cn.size() * sizeof(double), cudaMemcpyHostToDevice, s->st));
+    CUDA_TRY(cudaStreamSynchronize(s->st));     // h_cn may be rewritten by the next call
+    s->cn_dt = dt;
+  }
   // Launch-bound sizes (configs 1-2: ~25-40 launches of a few microseconds each): replay the three substeps as one CUDA
   // graph.  The graph is captured on first use for a given dt (kernel arguments are baked in) and re-captured when dt
   // changes; per-kernel timing needs the individual launches, so it bypasses the graph.
@@ -427,7 +438,7 @@ extern "C" int cales_set_graph(cales_solver* s, int on) {
 extern "C" int cales_launches_per_step(cales_solver* s) {
   if (!s) return 0;
   const Ctx& c = s->c;
-  int per = 1 /*rhs*/ + (c.implicit_z ? 4 : 0) + (c.const_flow_rate ? 2 : 0) + 5 /*solver*/ + 1 /*correct*/ + (c.wall_model ? 1 : 0) +
+  int per = 1 /*rhs*/ + (c.implicit_z ? 3 : 0) + (c.const_flow_rate ? 2 : 0) + 5 /*solver*/ + 1 /*correct*/ + (c.wall_model ? 1 : 0) +
             1 /*static nu_t or fill*/;
   if (c.sgs == CALES_SGS_DSMAG) {
     const bool ywall = c.bc_y == BC_WALL, split = ywall && c.ny >= 3 * DSM_TY;
