@@ -266,7 +266,7 @@ static int run_transform_y(cales_solver* s, double* A, int inverse) {
   return CALES_OK;
 }
 static int run_poisson_z(cales_solver* s, double* A) {
-  const int th = 128;
+  const int th = (s->nxy / 128 < 4 * 148) ? 64 : 128;      // small planes: smaller CTAs spread over more SMs
   k_poisson_z<<<(unsigned)((s->nxy + th - 1) / th), th, 0, s->st>>>(s->c, s->pt, A, s->CP, s->CQ);
   LAUNCH_TRY(K_POISSON_Z);
   return CALES_OK;
@@ -351,10 +351,8 @@ static int substep(cales_solver* s, int rk, double dt) {
   LAUNCH_TRY(K_RHS);
   long long npart = (long long)rgrid.x * rgrid.y * rgrid.z;
   if (imp) {
-    const int th = 128; const unsigned g = (unsigned)((s->nxy + th - 1) / th);
-    k_cn_z<<<g, th, 0, s->st>>>(c, s->cncoef + (size_t)rk * 6 * c.nz, 0, s->us, cfr ? s->partial : nullptr); LAUNCH_TRY(K_CN_Z);
-    k_cn_z<<<g, th, 0, s->st>>>(c, s->cncoef + (size_t)rk * 6 * c.nz, 1, s->vs, nullptr); LAUNCH_TRY(K_CN_Z);
-    k_cn_z<<<g, th, 0, s->st>>>(c, s->cncoef + (size_t)rk * 6 * c.nz, 2, s->ws, nullptr); LAUNCH_TRY(K_CN_Z);
+    const int th = (s->nxy / 128 < 4 * 148) ? 64 : 128; const unsigned g = (unsigned)((s->nxy + th - 1) / th);
+    k_cn_z<<<dim3(g, 3), th, 0, s->st>>>(c, s->cncoef + (size_t)rk * 6 * c.nz, s->us, s->vs, s->ws, cfr ? s->partial : nullptr); LAUNCH_TRY(K_CN_Z);
     npart = g;
   }
   if (cfr) {
@@ -438,7 +436,7 @@ extern "C" int cales_set_graph(cales_solver* s, int on) {
 extern "C" int cales_launches_per_step(cales_solver* s) {
   if (!s) return 0;
   const Ctx& c = s->c;
-  int per = 1 /*rhs*/ + (c.implicit_z ? 3 : 0) + (c.const_flow_rate ? 2 : 0) + 5 /*solver*/ + 1 /*correct*/ + (c.wall_model ? 1 : 0) +
+  int per = 1 /*rhs*/ + (c.implicit_z ? 1 : 0) + (c.const_flow_rate ? 2 : 0) + 5 /*solver*/ + 1 /*correct*/ + (c.wall_model ? 1 : 0) +
             1 /*static nu_t or fill*/;
   if (c.sgs == CALES_SGS_DSMAG) {
     const bool ywall = c.bc_y == BC_WALL, split = ywall && c.ny >= 3 * DSM_TY;

@@ -188,9 +188,13 @@ __global__ void k_poisson_z(Ctx c, PoissonTabs T, double* __restrict__ A, double
 __global__ void k_cn_coef(Ctx c, double cimp, double* coef) {
   if (blockIdx.x == 0 && threadIdx.x == 0) cn_coefficients(c, cimp, coef);
 }
-// comp: 0 u, 1 v, 2 w.  For u the dzf-weighted column sums are reduced per block into partial[blockIdx.x].
-__global__ void k_cn_z(Ctx c, const double* __restrict__ coef, int comp, double* __restrict__ Q, double* __restrict__ partial) {
+// grid (ceil(nxy / blockDim), 3): blockIdx.y = component (0 u, 1 v, 2 w), one launch for the three independent solves so that
+// small planes still fill the machine.  For u the dzf-weighted column sums are reduced per block into partial[blockIdx.x].
+__global__ void k_cn_z(Ctx c, const double* __restrict__ coef, double* __restrict__ us, double* __restrict__ vs, double* __restrict__ ws,
+                       double* __restrict__ partial) {
   __shared__ double sh[32];
+  const int comp = blockIdx.y;
+  double* Q = comp == 0 ? us : (comp == 1 ? vs : ws);
   const long long col = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   double s = 0.0;
   if (col < c.nxy) {
@@ -198,7 +202,7 @@ __global__ void k_cn_z(Ctx c, const double* __restrict__ coef, int comp, double*
     const bool skip = (comp == 1 && c.bc_y == BC_WALL && j == c.ny - 1);   // the +y wall face stays 0
     if (!skip) s = cn_column(c, comp == 2 ? coef + 3 * c.nz : coef, comp == 2 ? c.nz - 1 : c.nz, col, Q);
   }
-  if (partial) {
+  if (comp == 0 && partial) {
     const double t = block_sum(s, sh);
     if (threadIdx.x == 0) partial[blockIdx.x] = t;
   }
