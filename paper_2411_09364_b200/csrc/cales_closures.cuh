@@ -142,7 +142,7 @@ CALES_HD double smag_point(const Ctx& c, const double* u, const double* v, const
 // Each output point forms L_ij (Eq. 7), M_ij (Eq. 8, S2), stores |S| and contributes L:M and M:M to the
 // per-(k, j, x-tile) partial sums of Eq. 6.
 // ------------------------------------------------------------------------------------------------------------
-enum { DSM_TX = 32, DSM_TY = 8, DSM_RX = DSM_TX + 4, DSM_RY = DSM_TY + 4, DSM_MX = DSM_TX + 2, DSM_MY = DSM_TY + 2 };
+enum { DSM_TX = 32, DSM_TY = 2 /* exactly the two rows next to a y wall where F and the strain do not commute */, DSM_RX = DSM_TX + 4, DSM_RY = DSM_TY + 4, DSM_MX = DSM_TX + 2, DSM_MY = DSM_TY + 2 };
 enum { DSM_RAW = 9 * DSM_RX * DSM_RY, DSM_FLT = 9 * DSM_MX * DSM_MY, DSM_MID = 10 * DSM_MX * DSM_MY,
        DSM_SMEM_DOUBLES = DSM_RAW + DSM_FLT + DSM_MID };
 

@@ -14,8 +14,8 @@ SMALL = {
     "cfg1_dit": (1, (24, 16, 12), 2),
     "cfg2_wmles": (2, (48, 24, 16), 2),
     "cfg3_wrles_cn": (3, (36, 24, 20), 2),
-    "cfg4_duct_dsm": (4, (48, 36, 16), 2),            # ny >= 24: wall-row tiles + column-marching kernel
-    "cfg4_duct_dsm_narrow": (4, (48, 18, 16), 1),     # ny < 24: tile kernel on every row
+    "cfg4_duct_dsm": (4, (48, 36, 16), 2),            # wall-row tiles + column-marching kernel
+    "cfg4_duct_dsm_narrow": (4, (48, 4, 16), 1),      # ny < 6: tile kernel on every row
     "cfg5_wmles_dsm": (5, (36, 24, 16), 2),
     "duct_static_smag": (4, (24, 12, 12), 2, dict(sgs_model=1, cs=0.1)),   # static model next to y walls
     "cfg5_hwm_interp": (5, (24, 12, 16), 2, dict(h_wm=0.1)),               # wall model sampled between centres
@@ -30,7 +30,7 @@ GPU_CASES = {
     "cfg5_wmles_dsm": (5, (192, 128, 64), 3),        # the replica SURVEY.md 8(d) names for config 5
     "duct_static_smag": (4, (96, 36, 24), 2, dict(sgs_model=1, cs=0.1)),
     "cfg5_hwm_interp": (5, (96, 48, 32), 2, dict(h_wm=0.1)),
-    "cfg4_duct_dsm_narrow": (4, (72, 18, 16), 2),
+    "cfg4_duct_dsm_narrow": (4, (72, 4, 16), 2),
     "cfg2_wm_implicit": (2, (96, 48, 32), 3, dict(implicit_z=1)),
     "cfg5_wm_implicit_dsm": (5, (96, 48, 32), 2, dict(implicit_z=1, h_wm=0.1)),
 }
