@@ -35,7 +35,7 @@ L2_BYTES = 126 * 1024 * 1024
 # 3 (+3 R^k): 88 / 112 / 88 B/pt, mean 96.
 ALGO_BYTES = {
     "k_rhs": 96.0, "k_cn_z": 48.0, "k_fft_x_fwd": 32.0, "k_fft_y_fwd": 16.0, "k_poisson_z": 16.0, "k_fft_y_inv": 16.0,
-    "k_fft_x_inv": 16.0, "k_correct": 72.0, "k_smag": 32.0, "k_dsm_pass1": 32.0, "k_dsm_col": 32.0, "k_dsm_nut": 16.0, "k_fill": 8.0,
+    "k_fft_x_inv": 16.0, "k_correct": 72.0, "k_smag": 32.0, "k_dsm_col": 32.0, "k_dsm_nut": 16.0, "k_fill": 8.0,
 }
 
 
