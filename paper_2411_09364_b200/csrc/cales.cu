@@ -50,6 +50,7 @@ struct cales_solver {
   dim3 pgrid, pblock;   // point kernels
   long long nblk;
   bool fresh;
+  long long rhs_tile_min;   // below this many points the momentum kernel runs one thread per point
   long long tile_min;   // grids with at least this many points use the staged z-march for the static model
   std::vector<double> h_dzf, h_dzc, h_cn; Ctx hc; double cn_dt;   // host copies for the per-dt CN coefficient tables
   int use_graph; cudaGraphExec_t gexec; double gdt;   // the three substeps captured as one CUDA graph, keyed by dt
@@ -191,6 +192,8 @@ extern "C" int cales_create(const cales_params* p, cales_solver** out) {
   s->use_graph = 1; s->gexec = nullptr; s->gdt = 0.0;
   s->h_dzf = H.dzf; s->h_dzc = H.dzc; s->hc = s->c; s->hc.dzf = s->h_dzf.data() + 1; s->hc.dzc = s->h_dzc.data() + 1; s->cn_dt = 0.0;
   s->tile_min = 4000000;
+  s->rhs_tile_min = 200000;
+  if (const char* e = std::getenv("CALES_RHS_TILE_MIN_POINTS")) s->rhs_tile_min = std::atoll(e);   // tests force either path
   if (const char* e = std::getenv("CALES_TILE_MIN_POINTS")) s->tile_min = std::atoll(e);   // tests force either path
   for (int q = 0; q < 32; ++q) { s->kms[q] = 0.0; s->kcnt[q] = 0; }
   *out = s;
@@ -346,8 +349,9 @@ static int substep(cales_solver* s, int rk, double dt) {
   a.Ru0 = s->Ru; a.Rv0 = s->Rv; a.Rw0 = s->Rw; a.Ru1 = s->Ru; a.Rv1 = s->Rv; a.Rw1 = s->Rw;
   a.us = s->us; a.vs = s->vs; a.ws = s->ws; a.dt = dt; a.al = al; a.be = be; a.ga = ga; a.store_R = rk < 2 ? 1 : 0;
   const int kz = rt_chunk(c.nx, c.ny, c.nz);
-  const dim3 rgrid((c.nx + RT_TX - 1) / RT_TX, (c.ny + RT_TY - 1) / RT_TY, (c.nz + kz - 1) / kz);
-  k_rhs_tile<<<rgrid, RT_THREADS, RT_SMEM_DOUBLES * sizeof(double), s->st>>>(c, a, kz, (cfr && !imp) ? s->partial : nullptr);
+  dim3 rgrid((c.nx + RT_TX - 1) / RT_TX, (c.ny + RT_TY - 1) / RT_TY, (c.nz + kz - 1) / kz);
+  if (s->N >= s->rhs_tile_min) k_rhs_tile<<<rgrid, RT_THREADS, RT_SMEM_DOUBLES * sizeof(double), s->st>>>(c, a, kz, (cfr && !imp) ? s->partial : nullptr);
+  else { rgrid = s->pgrid; k_rhs_point<<<s->pgrid, s->pblock, 0, s->st>>>(c, a, (cfr && !imp) ? s->partial : nullptr); }
   LAUNCH_TRY(K_RHS);
   long long npart = (long long)rgrid.x * rgrid.y * rgrid.z;
   if (imp) {

@@ -153,6 +153,19 @@ static inline int rt_chunk(int nx, int ny, int nz) {
 }
 
 #ifdef __CUDACC__
+// Launch-bound grids (config 1: 32^3): one thread per point through the generic boundary accessors; a z-marching CTA has
+// too few planes to amortise its pipeline fill there.  grid (ceil(nx/32), ceil(ny/8), nz), block (32, 8).
+__global__ void __launch_bounds__(256) k_rhs_point(const __grid_constant__ Ctx c, const __grid_constant__ RhsArgs a, double* __restrict__ partial) {
+  __shared__ double red[32];
+  const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y * blockDim.y + threadIdx.y, k = blockIdx.z;
+  double s = 0.0;
+  if (i < c.nx && j < c.ny) { const GhostAcc q{c, a, i, j, k}; s = rhs_core(c, a, q, i, j, k, zmet_at(c, k)) * c.dzf[k]; }
+  if (partial) {
+    const double t = block_sum(s, red);
+    if (threadIdx.x == 0 && threadIdx.y == 0) partial[blockIdx.x + gridDim.x * (blockIdx.y + (long long)gridDim.y * blockIdx.z)] = t;
+  }
+}
+
 // grid (ceil(nx/RT_TX), ceil(ny/RT_TY), ceil(nz/kz)), block RT_THREADS, dynamic smem RT_SMEM_DOUBLES*8.
 // partial[linear block id] = sum over the CTA's points of u* dzf[k] (or nullptr).
 __global__ void __launch_bounds__(RT_THREADS, 2) k_rhs_tile(const __grid_constant__ Ctx c, const __grid_constant__ RhsArgs a, int kz,

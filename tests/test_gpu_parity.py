@@ -318,3 +318,20 @@ def test_cfl_dt_and_plane_stats_parity(oracle, gpu, n, shape):
     for q in range(8):
         assert np.max(np.abs(sa[q] - sb[q])) <= 1e-11 * scale[q], q
     g.close()
+
+
+@pytest.mark.parametrize("min_points", ["0", "1000000000"])
+@pytest.mark.parametrize("n,shape", [(1, (48, 24, 20)), (2, (72, 48, 24)), (4, (96, 36, 24))])
+def test_momentum_kernel_both_forms_parity(oracle, gpu, n, shape, min_points, monkeypatch):
+    """The staged z-marching momentum kernel (min_points = 0) and the one-thread-per-point form used on launch-bound
+    grids (min_points huge), each forced on at test sizes."""
+    monkeypatch.setenv("CALES_RHS_TILE_MIN_POINTS", min_points)
+    cfg, kw, (u, v, w), dt = pc.prepare(oracle, n, shape)
+    o = pc.make(oracle.Oracle, kw)
+    g = pc.make(gpu.Solver, kw)
+    o.set_velocity(u, v, w); g.set_velocity(u, v, w)
+    for _ in range(2):
+        o.step(dt); g.step(dt)
+    err = pc.field_errors(_gpu_fields(g), [o.get(f) for f in range(5)], o.dzf, kw["nu"])
+    assert max(err.values()) <= 1e-10, err
+    g.close()
