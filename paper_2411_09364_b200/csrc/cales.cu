@@ -350,13 +350,19 @@ static int substep(cales_solver* s, int rk, double dt) {
   a.us = s->us; a.vs = s->vs; a.ws = s->ws; a.dt = dt; a.al = al; a.be = be; a.ga = ga; a.store_R = rk < 2 ? 1 : 0;
   const int kz = rt_chunk(c.nx, c.ny, c.nz);
   dim3 rgrid((c.nx + RT_TX - 1) / RT_TX, (c.ny + RT_TY - 1) / RT_TY, (c.nz + kz - 1) / kz);
-  const BulkFin bf_on{s->partial, reinterpret_cast<unsigned*>(s->maxit + 1), s->scal, ga * dt}, bf_off{nullptr, nullptr, nullptr, 1.0};
-  if (s->N >= s->rhs_tile_min) k_rhs_tile<<<rgrid, RT_THREADS, RT_SMEM_DOUBLES * sizeof(double), s->st>>>(c, a, kz, (cfr && !imp) ? bf_on : bf_off);
-  else k_rhs_point<<<s->pgrid, s->pblock, 0, s->st>>>(c, a, (cfr && !imp) ? bf_on : bf_off);
+  if (s->N >= s->rhs_tile_min) k_rhs_tile<<<rgrid, RT_THREADS, RT_SMEM_DOUBLES * sizeof(double), s->st>>>(c, a, kz, (cfr && !imp) ? s->partial : nullptr);
+  else { rgrid = s->pgrid; k_rhs_point<<<s->pgrid, s->pblock, 0, s->st>>>(c, a, (cfr && !imp) ? s->partial : nullptr); }
   LAUNCH_TRY(K_RHS);
+  long long npart = (long long)rgrid.x * rgrid.y * rgrid.z;
   if (imp) {
     const int th = (s->nxy / 128 < 4 * 148) ? 64 : 128; const unsigned g = (unsigned)((s->nxy + th - 1) / th);
-    k_cn_z<<<dim3(g, 3), th, 0, s->st>>>(c, s->cncoef + (size_t)rk * 6 * c.nz, s->us, s->vs, s->ws, cfr ? bf_on : bf_off); LAUNCH_TRY(K_CN_Z);
+    k_cn_z<<<dim3(g, 3), th, 0, s->st>>>(c, s->cncoef + (size_t)rk * 6 * c.nz, s->us, s->vs, s->ws, cfr ? s->partial : nullptr); LAUNCH_TRY(K_CN_Z);
+    npart = g;
+  }
+  if (cfr) {
+    const int g1 = (int)(npart < 1024 ? npart : 1024);
+    k_sum_stage1<<<g1, 256, 0, s->st>>>(s->partial, npart, s->stage1); LAUNCH_TRY(K_SUM);
+    k_bulk_finish<<<1, 256, 0, s->st>>>(c, s->stage1, g1, ga * dt, s->scal); LAUNCH_TRY(K_BULK);
   }
   DivSrc ds{s->us, s->vs, s->ws, 1.0 / (ga * dt)};
   if ((rc = run_transform_x_fwd(s, nullptr, &ds, s->W))) return rc;
@@ -434,7 +440,7 @@ extern "C" int cales_set_graph(cales_solver* s, int on) {
 extern "C" int cales_launches_per_step(cales_solver* s) {
   if (!s) return 0;
   const Ctx& c = s->c;
-  int per = 1 /*rhs*/ + (c.implicit_z ? 1 : 0) + 5 /*solver*/ + 1 /*correct*/ + (c.wall_model ? 1 : 0) +
+  int per = 1 /*rhs*/ + (c.implicit_z ? 1 : 0) + (c.const_flow_rate ? 2 : 0) + 5 /*solver*/ + 1 /*correct*/ + (c.wall_model ? 1 : 0) +
             1 /*static nu_t or fill*/;
   if (c.sgs == CALES_SGS_DSMAG) {
     const bool ywall = c.bc_y == BC_WALL, split = ywall && c.ny >= 3 * DSM_TY;

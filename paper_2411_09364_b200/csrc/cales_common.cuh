@@ -152,34 +152,6 @@ __device__ __forceinline__ double block_max(double v, double* sh) {
   __syncthreads();
   return r;
 }
-// Grid-wide dzf-weighted sum of u* finished by the LAST CTA to arrive (ticket counter), which then sets the uniform shift
-// that restores the bulk velocity (S12): scal[0] = shift, scal[1] = shift / (gamma dt) (the
-// equivalent body force), scal[2] = mean.  Deterministic: the partials are summed in a fixed order whichever CTA is last.
-// t: this CTA's total (valid in thread 0); all threads of the CTA must call; sh: >= 33 doubles of shared memory.
-struct BulkFin { double* partial; unsigned* counter; double* scal; double gdt; };
-__device__ __forceinline__ void bulk_finish_last_block(const Ctx& c, const BulkFin& f, double t, double* sh) {
-  const int tid = threadIdx.x + blockDim.x * (threadIdx.y + blockDim.y * threadIdx.z);
-  const int nth = blockDim.x * blockDim.y * blockDim.z;
-  const long long nb = (long long)gridDim.x * gridDim.y * gridDim.z;
-  const long long bid = blockIdx.x + gridDim.x * (blockIdx.y + (long long)gridDim.y * blockIdx.z);
-  if (tid == 0) {
-    f.partial[bid] = t;
-    __threadfence();
-    sh[32] = (atomicAdd(f.counter, 1u) == (unsigned)(nb - 1)) ? 1.0 : 0.0;
-  }
-  __syncthreads();
-  if (sh[32] == 0.0) return;
-  __threadfence();
-  double s = 0.0;
-  for (long long q = tid; q < nb; q += nth) s += __ldcg(f.partial + q);
-  const double tot = block_sum(s, sh);
-  if (tid == 0) {
-    const double m = tot / ((double)c.nx * (double)c.ny * c.lz);
-    const double shf = c.u_bulk - m;
-    f.scal[0] = shf; f.scal[1] = shf / f.gdt; f.scal[2] = m;
-    *f.counter = 0u;
-  }
-}
 #endif
 
 }  // namespace cales

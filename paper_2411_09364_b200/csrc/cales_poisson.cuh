@@ -189,10 +189,10 @@ __global__ void k_cn_coef(Ctx c, double cimp, double* coef) {
   if (blockIdx.x == 0 && threadIdx.x == 0) cn_coefficients(c, cimp, coef);
 }
 // grid (ceil(nxy / blockDim), 3): blockIdx.y = component (0 u, 1 v, 2 w), one launch for the three independent solves so that
-// small planes still fill the machine.  With bf.partial set, the dzf-weighted sum of u* is reduced over the grid (last CTA).
+// small planes still fill the machine.  For u the dzf-weighted column sums are reduced per block into partial[blockIdx.x].
 __global__ void k_cn_z(Ctx c, const double* __restrict__ coef, double* __restrict__ us, double* __restrict__ vs, double* __restrict__ ws,
-                       BulkFin bf) {
-  __shared__ double sh[33];
+                       double* __restrict__ partial) {
+  __shared__ double sh[32];
   const int comp = blockIdx.y;
   double* Q = comp == 0 ? us : (comp == 1 ? vs : ws);
   const long long col = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -202,9 +202,9 @@ __global__ void k_cn_z(Ctx c, const double* __restrict__ coef, double* __restric
     const bool skip = (comp == 1 && c.bc_y == BC_WALL && j == c.ny - 1);   // the +y wall face stays 0
     if (!skip) s = cn_column(c, comp == 2 ? coef + 3 * c.nz : coef, comp == 2 ? c.nz - 1 : c.nz, col, Q);
   }
-  if (bf.partial) {      // every CTA takes a ticket (components 1, 2 contribute 0) so that the last one sees all partials
-    const double t = block_sum(comp == 0 ? s : 0.0, sh);
-    bulk_finish_last_block(c, bf, t, sh);
+  if (comp == 0 && partial) {
+    const double t = block_sum(s, sh);
+    if (threadIdx.x == 0) partial[blockIdx.x] = t;
   }
 }
 #endif

@@ -155,20 +155,23 @@ static inline int rt_chunk(int nx, int ny, int nz) {
 #ifdef __CUDACC__
 // Launch-bound grids (config 1: 32^3): one thread per point through the generic boundary accessors; a z-marching CTA has
 // too few planes to amortise its pipeline fill there.  grid (ceil(nx/32), ceil(ny/8), nz), block (32, 8).
-__global__ void __launch_bounds__(256) k_rhs_point(const __grid_constant__ Ctx c, const __grid_constant__ RhsArgs a, BulkFin bf) {
-  __shared__ double red[33];
+__global__ void __launch_bounds__(256) k_rhs_point(const __grid_constant__ Ctx c, const __grid_constant__ RhsArgs a, double* __restrict__ partial) {
+  __shared__ double red[32];
   const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y * blockDim.y + threadIdx.y, k = blockIdx.z;
   double s = 0.0;
   if (i < c.nx && j < c.ny) { const GhostAcc q{c, a, i, j, k}; s = rhs_core(c, a, q, i, j, k, zmet_at(c, k)) * c.dzf[k]; }
-  if (bf.partial) bulk_finish_last_block(c, bf, block_sum(s, red), red);
+  if (partial) {
+    const double t = block_sum(s, red);
+    if (threadIdx.x == 0 && threadIdx.y == 0) partial[blockIdx.x + gridDim.x * (blockIdx.y + (long long)gridDim.y * blockIdx.z)] = t;
+  }
 }
 
 // grid (ceil(nx/RT_TX), ceil(ny/RT_TY), ceil(nz/kz)), block RT_THREADS, dynamic smem RT_SMEM_DOUBLES*8.
-// bf.partial != nullptr: the dzf-weighted sum of u* is reduced over the grid and the bulk shift set by the last CTA.
+// partial[linear block id] = sum over the CTA's points of u* dzf[k] (or nullptr).
 __global__ void __launch_bounds__(RT_THREADS, 2) k_rhs_tile(const __grid_constant__ Ctx c, const __grid_constant__ RhsArgs a, int kz,
-                                                            BulkFin bf) {
+                                                            double* __restrict__ partial) {
   extern __shared__ double rt_sm[];
-  __shared__ double red[33];
+  __shared__ double red[32];
   const int tid = threadIdx.x, tx = tid & 31, ty = tid >> 5;
   const int i0 = blockIdx.x * RT_TX, j0 = blockIdx.y * RT_TY, k0 = blockIdx.z * kz, k1 = min(k0 + kz, c.nz);
   // ---- this thread's halo-tile positions (the same for every plane and field)
@@ -239,7 +242,10 @@ __global__ void __launch_bounds__(RT_THREADS, 2) k_rhs_tile(const __grid_constan
       }
     }
   }
-  if (bf.partial) bulk_finish_last_block(c, bf, block_sum(acc, red), red);
+  if (partial) {
+    const double t = block_sum(acc, red);
+    if (tid == 0) partial[blockIdx.x + gridDim.x * (blockIdx.y + (long long)gridDim.y * blockIdx.z)] = t;
+  }
 }
 #endif
 
