@@ -185,9 +185,6 @@ __global__ void k_poisson_z(Ctx c, PoissonTabs T, double* __restrict__ A, double
   if (col >= c.nxy) return;
   poisson_column(c, T, (int)(col % c.nx), (int)(col / c.nx), A, CP, CQ);
 }
-__global__ void k_cn_coef(Ctx c, double cimp, double* coef) {
-  if (blockIdx.x == 0 && threadIdx.x == 0) cn_coefficients(c, cimp, coef);
-}
 // grid (ceil(nxy / blockDim), 3): blockIdx.y = component (0 u, 1 v, 2 w), one launch for the three independent solves so that
 // small planes still fill the machine.  For u the dzf-weighted column sums are reduced per block into partial[blockIdx.x].
 __global__ void k_cn_z(Ctx c, const double* __restrict__ coef, double* __restrict__ us, double* __restrict__ vs, double* __restrict__ ws,

@@ -73,3 +73,47 @@ def test_emulated_transforms_match_numpy_scipy(emu, n):
         else:
             assert np.allclose(F, 0.5 * scipy.fft.dct(f, type=2, axis=1), atol=1e-12)
         assert np.allclose(e.transform(F, 1, inverse=True), f, atol=1e-12)
+
+
+def _fuzz_cases():
+    """Seeded random option sets on small, awkward grids (sizes of the form 2^a 3^b down to 2, all boundary combinations)."""
+    rng = np.random.default_rng(20241109)
+    sizes_xy = [2, 4, 6, 8, 12, 16, 18, 24, 32, 36, 48]
+    out = []
+    for t in range(14):
+        bc_z = int(rng.integers(0, 2)); bc_y = int(rng.integers(0, 2)) if bc_z else 0
+        nx, ny = int(rng.choice(sizes_xy)), int(rng.choice(sizes_xy)); nz = int(rng.integers(4, 14))
+        stretch = int(bc_z and rng.integers(0, 2))
+        sgs = int(rng.integers(0, 3))
+        wm = int(bc_z and rng.integers(0, 2))
+        imp = int(bc_z and rng.integers(0, 2))
+        vd = int(sgs == 1 and bc_z and not bc_y and not wm and rng.integers(0, 2))
+        kw = dict(bc_y=bc_y, bc_z=bc_z, zstretch=stretch, zstretch_factor=1.3 if stretch else 0.0, nu=float(rng.uniform(1e-3, 2e-2)),
+                  sgs_model=sgs, cs=0.12, van_driest=vd, dsm_avg_xy_plane=int(rng.integers(0, 2)), dsm_clip_total=int(rng.integers(0, 2)),
+                  wall_model=wm, h_wm=float(rng.choice([0.0, 0.12])) if wm else 0.0, implicit_z=imp,
+                  const_flow_rate=int(rng.integers(0, 2)), u_bulk=1.0)
+        out.append((t, nx, ny, nz, kw))
+    return out
+
+
+@pytest.mark.parametrize("t,nx,ny,nz,kw", _fuzz_cases())
+def test_fuzzed_option_sets_match_oracle(oracle, emu, t, nx, ny, nz, kw):
+    rng = np.random.default_rng(100 + t)
+    lz = 2.0
+    u = 1.0 + 0.3 * rng.standard_normal((nz, ny, nx)); v = 0.3 * rng.standard_normal((nz, ny, nx)); w = 0.3 * rng.standard_normal((nz, ny, nx))
+    if kw["bc_z"]:
+        w[-1] = 0.0
+    if kw["bc_y"]:
+        v[:, -1, :] = 0.0
+    o = oracle.Oracle(nx, ny, nz, 3.0, 2.0, lz, **kw)
+    o.set_velocity(u, v, w); o.project(); u, v, w = o.velocity()
+    if kw["const_flow_rate"]:
+        kw = dict(kw, u_bulk=float(np.sum(u * o.dzf[:, None, None]) / (nx * ny * lz)))
+        o = oracle.Oracle(nx, ny, nz, 3.0, 2.0, lz, **kw)
+    e = emu.Emu(nx, ny, nz, 3.0, 2.0, lz, **kw)
+    o.set_velocity(u, v, w); e.set_velocity(u, v, w)
+    dt = 0.2 * min(3.0 / nx, 2.0 / ny, float(np.min(o.dzf))) / 2.0
+    for s in range(2):
+        o.step(dt); e.step(dt)
+    err = pc.field_errors([e.get(f) for f in range(5)], [o.get(f) for f in range(5)], o.dzf, kw["nu"])
+    assert max(err.values()) <= 1e-10, (t, nx, ny, nz, kw, err)

@@ -335,3 +335,62 @@ def test_momentum_kernel_both_forms_parity(oracle, gpu, n, shape, min_points, mo
     err = pc.field_errors(_gpu_fields(g), [o.get(f) for f in range(5)], o.dzf, kw["nu"])
     assert max(err.values()) <= 1e-10, err
     g.close()
+
+
+def _fuzz():
+    from tests.test_emu_parity import _fuzz_cases
+    return _fuzz_cases()
+
+
+@pytest.mark.parametrize("t,nx,ny,nz,kw", _fuzz())
+def test_fuzzed_option_sets_match_oracle_on_gpu(oracle, gpu, t, nx, ny, nz, kw):
+    """Seeded random option sets on small, awkward grids (down to 2 x 2 x 4): every boundary / model combination the
+    library accepts, against the oracle."""
+    rng = np.random.default_rng(100 + t)
+    lz = 2.0
+    u = 1.0 + 0.3 * rng.standard_normal((nz, ny, nx)); v = 0.3 * rng.standard_normal((nz, ny, nx)); w = 0.3 * rng.standard_normal((nz, ny, nx))
+    if kw["bc_z"]:
+        w[-1] = 0.0
+    if kw["bc_y"]:
+        v[:, -1, :] = 0.0
+    o = oracle.Oracle(nx, ny, nz, 3.0, 2.0, lz, **kw)
+    o.set_velocity(u, v, w); o.project(); u, v, w = o.velocity()
+    if kw["const_flow_rate"]:
+        kw = dict(kw, u_bulk=float(np.sum(u * o.dzf[:, None, None]) / (nx * ny * lz)))
+        o = oracle.Oracle(nx, ny, nz, 3.0, 2.0, lz, **kw)
+    g = gpu.Solver(nx, ny, nz, 3.0, 2.0, lz, **kw)
+    o.set_velocity(u, v, w); g.set_velocity(u, v, w)
+    dt = 0.2 * min(3.0 / nx, 2.0 / ny, float(np.min(o.dzf))) / 2.0
+    for s in range(2):
+        o.step(dt); g.step(dt)
+    err = pc.field_errors(_gpu_fields(g), [o.get(f) for f in range(5)], o.dzf, kw["nu"])
+    assert max(err.values()) <= 1e-10, (t, nx, ny, nz, kw, err)
+    g.close()
+
+
+@pytest.mark.parametrize("shape,bc_y", [((2, 2, 4), 0), ((12288, 2, 4), 0), ((2, 8192, 4), 0), ((2, 8192, 4), 1), ((4096, 6, 4), 0),
+                                         ((6, 4096, 4), 1), ((6144, 4, 4), 0)])
+def test_extreme_line_lengths(oracle, gpu, shape, bc_y):
+    """Smallest and largest supported transform lengths (nx <= 12288, ny <= 8192): round trip, numpy/scipy, Poisson vs oracle."""
+    import scipy.fft
+    import torch
+    nx, ny, nz = shape
+    g = gpu.Solver(nx, ny, nz, 2.0, 1.5, 1.0, bc_y=bc_y, bc_z=1)
+    rng = np.random.default_rng(5)
+    f = rng.standard_normal((nz, ny, nx))
+    F = g.transform(torch.from_numpy(f).cuda(), 0).cpu().numpy()
+    X = np.fft.rfft(f, axis=2)
+    assert np.max(np.abs(F[..., 0] - X[..., 0].real)) <= 1e-12 * np.max(np.abs(X))
+    if nx > 2:
+        assert np.max(np.abs(F[..., 2::2] - X[..., 1:nx // 2].real)) <= 1e-12 * np.max(np.abs(X))
+    back = g.transform(torch.from_numpy(F).cuda(), 0, inverse=True).cpu().numpy()
+    assert np.max(np.abs(back - f)) <= 1e-12 * np.max(np.abs(f))
+    Fy = g.transform(torch.from_numpy(f).cuda(), 1).cpu().numpy()
+    if bc_y:
+        assert np.max(np.abs(Fy - 0.5 * scipy.fft.dct(f, type=2, axis=1))) <= 1e-12 * np.max(np.abs(Fy))
+    backy = g.transform(torch.from_numpy(Fy).cuda(), 1, inverse=True).cpu().numpy()
+    assert np.max(np.abs(backy - f)) <= 1e-12 * np.max(np.abs(f))
+    o = oracle.Oracle(nx, ny, nz, 2.0, 1.5, 1.0, bc_y=bc_y, bc_z=1)
+    a, b = g.poisson_solve(torch.from_numpy(f).cuda()).cpu().numpy(), o.poisson_solve(f)
+    assert np.max(np.abs(a - b)) <= 1e-10 * np.max(np.abs(b))
+    g.close()
