@@ -227,11 +227,13 @@ __device__ __forceinline__ void f2_passes(const Fft2Lay& lay, const FftPlan& pl,
   const int tid = threadIdx.x, nth = blockDim.x, np = pl.npass;
   double2 v[F2_E];
   F2SmemLd sld{buf, lay}; F2SmemSt sst{buf, lay};
-  if (np == 0) {                 // n = 2: a single complex element per line
-    double2 z = make_double2(0.0, 0.0);
-    if (tid < lay.L) z = first(tid, 0);
+  if (np == 0) {                 // n = 2: a single complex element per line (lines b = tid, tid + nth, ...; L <= 64 <= 2 * nth)
+    double2 z0 = make_double2(0.0, 0.0), z1 = z0;
+    if (tid < lay.L) z0 = first(tid, 0);
+    if (tid + nth < lay.L) z1 = first(tid + nth, 0);
     __syncthreads();
-    if (tid < lay.L) { if (TO_GLOBAL) last(tid, 0, z); else sst(tid, 0, z); }
+    if (tid < lay.L) { if (TO_GLOBAL) last(tid, 0, z0); else sst(tid, 0, z0); }
+    if (tid + nth < lay.L) { if (TO_GLOBAL) last(tid + nth, 0, z1); else sst(tid + nth, 0, z1); }
     __syncthreads();
     return;
   }

@@ -78,8 +78,8 @@ static void emu_f2_passes(const Fft2Lay& lay, const FftPlan& pl, int sign, doubl
   F2SmemLd sld{buf, lay}; F2SmemSt sst{buf, lay};
   if (np == 0) {
     std::vector<double2> z(lay.L);
-    for (int tid = 0; tid < lay.L && tid < nth; ++tid) z[tid] = first(tid, 0);
-    for (int tid = 0; tid < lay.L && tid < nth; ++tid) { if (TO_GLOBAL) last(tid, 0, z[tid]); else sst(tid, 0, z[tid]); }
+    for (int b = 0; b < lay.L && b < 2 * nth; ++b) z[b] = first(b, 0);       // thread tid owns lines tid and tid + nth
+    for (int b = 0; b < lay.L && b < 2 * nth; ++b) { if (TO_GLOBAL) last(b, 0, z[b]); else sst(b, 0, z[b]); }
     return;
   }
   for (int p = 0; p < np; ++p) {
