@@ -52,7 +52,6 @@ static inline void make_plan(FftPlan& pl, int n) {
   int a = 0; while (m % 2 == 0) { ++a; m /= 2; }
   if (a > 0) {
     int maxbits = F2_E >= 16 ? 4 : 3;
-    if (const char* e = std::getenv("CALES_FFT_MAXBITS")) { const int v = std::atoi(e); if (v >= 1 && v <= 4) maxbits = v; }
     const int np = (a + maxbits - 1) / maxbits, base = a / np, extra = a % np;
     for (int q = 0; q < np; ++q) pl.radix[pl.npass++] = 1 << (base + (q >= np - extra ? 1 : 0));
   }
