@@ -20,6 +20,7 @@ class OracleParams(C.Structure):
         ("wm_tol", C.c_double), ("wm_maxit", C.c_int),
         ("implicit_z", C.c_int),
         ("const_flow_rate", C.c_int), ("u_bulk", C.c_double),
+        ("wall_model_y", C.c_int),
     ]
 
 
@@ -96,7 +97,7 @@ def rk3_coeffs(k):
 PARAM_DEFAULTS = dict(
     zstretch=0, zstretch_factor=0.0, bc_y=0, bc_z=0, nu=1e-3, sgs_model=0, cs=0.17, van_driest=0, aplus=25.0,
     dsm_avg_xy_plane=1, dsm_clip_total=0, dsm_alpha2d=0.0, wall_model=0, kappa=0.41, B=5.2, h_wm=0.0,
-    wm_tol=1e-4, wm_maxit=50, implicit_z=0, const_flow_rate=0, u_bulk=0.0)
+    wm_tol=1e-4, wm_maxit=50, implicit_z=0, const_flow_rate=0, u_bulk=0.0, wall_model_y=0)
 
 
 class Oracle:
@@ -164,6 +165,9 @@ class Oracle:
 
     def wall_stress(self):
         tau = np.empty((2, 2, self.ny, self.nx)); _chk(lib().oracle_wall_stress(self._h, _p(tau))); return tau
+
+    def wall_stress_y(self):
+        tau = np.empty((2, 2, self.nz, self.nx)); _chk(lib().oracle_wall_stress_y(self._h, _p(tau))); return tau
 
     def _three(self, fn, *extra):
         a, b, c = (np.empty(self.shape) for _ in range(3))

@@ -213,6 +213,7 @@ struct oracle_solver {
   F3 u, v, w, p, nut;
   std::vector<double> Ru, Rv, Rw;             // R^{k-1}
   std::vector<double> tau;                    // [wall][comp][ny][nx]
+  std::vector<double> tauy;                   // y walls: [wall][comp (0 tau_xy at u points, 1 tau_zy at w points)][nz][nx]
   std::vector<double> cs;                     // dynamic coefficient per k or per (k,j)
   std::vector<double> Lij, Mij;               // tensors of the last dynamic evaluation (for the pins)
   bool fresh = false;                         // wall stress + nu_t consistent with the velocity
@@ -222,6 +223,11 @@ struct oracle_solver {
   ~oracle_solver() { delete plx; delete ply; delete pdy; }
   inline size_t id(int i, int j, int k) const { return (size_t)i + (size_t)nx * ((size_t)j + (size_t)ny * (size_t)k); }
   inline double& tw(int wall, int comp, int i, int j) { return tau[((size_t)(wall * 2 + comp) * ny + j) * nx + i]; }
+  // y-wall stress seen from any (i,k) incl. ghosts: i periodic, k clamped to the interior
+  inline double& twy(int wall, int comp, int i, int k) {
+    int ii = i < 0 ? i + nx : (i >= nx ? i - nx : i), kk = k < 0 ? 0 : (k >= nz ? nz - 1 : k);
+    return tauy[((size_t)(wall * 2 + comp) * nz + kk) * nx + ii];
+  }
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -284,7 +290,21 @@ static void bc_velocity(oracle_solver& S, F3& u, F3& v, F3& w, int mode) {
   // --- y
   if (S.P.bc_y == BC_PER) { wrap_y(u); wrap_y(v); wrap_y(w); }
   else {
-    mirror_y(u, -1.0); mirror_y(w, -1.0);
+    if (!S.P.wall_model_y) { mirror_y(u, -1.0); mirror_y(w, -1.0); }
+    else {
+      // SURVEY.md 8(f) item 1 (duct WMLES): the y walls carry the wall model too; same two ghost kinds as in z,
+      // with the uniform spacing dy (ghost centre mirrored at distance dy from the first centre)
+      const double dy = S.dy, nu = S.P.nu;
+      for (int k = -1; k <= nz; ++k) for (int i = -1; i <= nx; ++i) {
+        if (mode == GH_VISC) {
+          u(i, -1, k) = u(i, 0, k) - S.twy(0, 0, i, k) * dy / nu; u(i, ny, k) = u(i, ny - 1, k) - S.twy(1, 0, i, k) * dy / nu;
+          w(i, -1, k) = w(i, 0, k) - S.twy(0, 1, i, k) * dy / nu; w(i, ny, k) = w(i, ny - 1, k) - S.twy(1, 1, i, k) * dy / nu;
+        } else {
+          u(i, -1, k) = 2.0 * u(i, 0, k) - u(i, 1, k); u(i, ny, k) = 2.0 * u(i, ny - 1, k) - u(i, ny - 2, k);
+          w(i, -1, k) = 2.0 * w(i, 0, k) - w(i, 1, k); w(i, ny, k) = 2.0 * w(i, ny - 1, k) - w(i, ny - 2, k);
+        }
+      }
+    }
     for (int k = -1; k <= nz; ++k) for (int i = -1; i <= nx; ++i) { v(i, ny - 1, k) = 0.0; v(i, -1, k) = 0.0; v(i, ny, k) = 0.0; }
   }
 }
@@ -295,10 +315,34 @@ static void bc_velocity(oracle_solver& S, F3& u, F3& v, F3& w, int mode) {
 // (each interpolated to h_wm), U = sqrt(u_wm^2+v_wm^2), Newton for u_tau, tau_xz = u_tau^2 u_wm / U.
 // Same at v-points with u interpolated -> tau_yz.  Needs x/y ghosts of u, v (call after bc_velocity).
 // ------------------------------------------------------------------------------------------------
-static void wall_stress(oracle_solver& S) {
-  if (!S.P.wall_model) return;
+// y walls (duct WMLES): sampled at the first off-wall centre, h = dy/2.  tau_xy at the u points (i+1/2, k) from u and the
+// 4 surrounding w points; tau_zy at the w points (i, k+1/2) from w and the 4 surrounding u points.
+static void wall_stress_y(oracle_solver& S, int& maxit) {
   int nx = S.nx, ny = S.ny, nz = S.nz;
+  const double h = 0.5 * S.dy;
+  for (int wall = 0; wall < 2; ++wall) {
+    const int j0 = wall == 0 ? 0 : ny - 1;
+    for (int k = 0; k < nz; ++k) for (int i = 0; i < nx; ++i) for (int comp = 0; comp < 2; ++comp) {
+      double a, b;
+      if (comp == 0) { a = S.u(i, j0, k); b = 0.25 * (S.w(i, j0, k) + S.w(i + 1, j0, k) + S.w(i, j0, k - 1) + S.w(i + 1, j0, k - 1)); }
+      else { a = S.w(i, j0, k); b = 0.25 * (S.u(i, j0, k) + S.u(i - 1, j0, k) + S.u(i, j0, k + 1) + S.u(i - 1, j0, k + 1)); }
+      double U = std::sqrt(a * a + b * b), t = 0.0;
+      if (U > 0.0) {
+        int it = 0;
+        double hp = oracle_loglaw_hplus(U * h / S.P.nu, S.P.kappa, S.P.B, S.P.wm_tol, S.P.wm_maxit, &it);
+        double utau = hp * S.P.nu / h;
+        t = utau * utau * a / U;
+        if (it > maxit) maxit = it;
+      }
+      S.tauy[((size_t)(wall * 2 + comp) * nz + k) * nx + i] = t;
+    }
+  }
+}
+static void wall_stress(oracle_solver& S) {
   int maxit = 0;
+  if (S.P.wall_model_y) wall_stress_y(S, maxit);
+  if (!S.P.wall_model) { if (S.P.wall_model_y) S.wm_max_iters = maxit; return; }
+  int nx = S.nx, ny = S.ny, nz = S.nz;
   for (int wall = 0; wall < 2; ++wall) {
     // distance of centre number q (counted from this wall) to the wall
     auto dist = [&](int q) { return wall == 0 ? S.zc[q] : S.P.lz - S.zc[nz - 1 - q]; };
@@ -713,6 +757,7 @@ extern "C" int oracle_create(const oracle_params* p, oracle_solver** out) {
   if (!smooth23(p->nx) || !smooth23(p->ny)) return fail("nx, ny must factor into 2 and 3");
   if (p->bc_z == BC_PER && p->zstretch != 0) return fail("periodic z requires a uniform grid");
   if (p->wall_model && p->bc_z != BC_WALL) return fail("wall model needs z walls");
+  if (p->wall_model_y && p->bc_y != BC_WALL) return fail("wall model on y walls needs y walls");
   if (p->implicit_z && p->bc_z != BC_WALL) return fail("implicit z needs z walls");
   if (p->wall_model && p->h_wm > 0.0 && !(p->h_wm < 0.5 * p->lz)) return fail("h_wm must lie below the half height");
   if (p->van_driest && (p->bc_z != BC_WALL || p->bc_y == BC_WALL || p->wall_model)) return fail("van Driest: z walls only, no wall model");
@@ -736,6 +781,7 @@ extern "C" int oracle_create(const oracle_params* p, oracle_solver** out) {
   S->u = F3(p->nx, p->ny, nz); S->v = S->u; S->w = S->u; S->p = S->u; S->nut = S->u;
   S->Ru.assign(S->N, 0.0); S->Rv.assign(S->N, 0.0); S->Rw.assign(S->N, 0.0);
   S->tau.assign((size_t)4 * p->nx * p->ny, 0.0);
+  S->tauy.assign((size_t)4 * p->nx * p->nz, 0.0);
   S->alpha2d = p->dsm_alpha2d > 0.0 ? p->dsm_alpha2d : std::cbrt(4.0);
   if (S->P.wm_tol <= 0.0) S->P.wm_tol = 1e-4;
   if (S->P.wm_maxit <= 0) S->P.wm_maxit = 50;
@@ -919,6 +965,13 @@ extern "C" int oracle_wall_stress(oracle_solver* S, double* tau) {
   bc_velocity(*S, S->u, S->v, S->w, GH_STRAIN);
   wall_stress(*S);
   std::memcpy(tau, S->tau.data(), S->tau.size() * sizeof(double));
+  return 0;
+}
+extern "C" int oracle_wall_stress_y(oracle_solver* S, double* tauy) {
+  if (!S || !tauy) return fail("null");
+  bc_velocity(*S, S->u, S->v, S->w, GH_STRAIN);
+  wall_stress(*S);
+  std::memcpy(tauy, S->tauy.data(), S->tauy.size() * sizeof(double));
   return 0;
 }
 extern "C" int oracle_advection(oracle_solver* S, double* au, double* av, double* aw) {

@@ -38,6 +38,7 @@ typedef struct {
   int wall_model; double kappa, B, h_wm, wm_tol; int wm_maxit;
   int implicit_z;
   int const_flow_rate; double u_bulk;
+  int wall_model_y;        /* log-law wall model on the y walls too (duct WMLES); needs bc_y = wall */
 } oracle_params;
 
 /* ---- 1-D primitives (pinned against numpy/scipy and O(N^2) definitions in tests) ---- */
@@ -73,6 +74,8 @@ int oracle_laplacian(oracle_solver* s, const double* phi, double* out);
 int oracle_eddy_viscosity(oracle_solver* s, const double* u, const double* v, const double* w, double* nut);
 /* wall stress planes from the internal velocity: tau[wall(0 bottom,1 top)][comp(0 xz at u-points,1 yz at v-points)][ny][nx] */
 int oracle_wall_stress(oracle_solver* s, double* tau);
+/* y-wall stress planes: tau[wall(0: j=0 side, 1: j=ny-1 side)][comp(0 xy at u-points, 1 zy at w-points)][nz][nx] */
+int oracle_wall_stress_y(oracle_solver* s, double* tau);
 /* individual explicit terms on the internal velocity / nu_t (each output nz*ny*nx): */
 int oracle_advection(oracle_solver* s, double* au, double* av, double* aw);    /* -d_j(u_i u_j) */
 int oracle_diffusion(oracle_solver* s, double* du, double* dv, double* dw, int which); /* which: 0 all, 1 x+y only, 2 z only; nu*L u_i */

@@ -611,3 +611,35 @@ def test_wall_model_with_implicit_z_momentum_balance(oracle):
     m1 = np.sum(o.get(0)[:, 0, 0] * o.dzf)
     expect = -dt * (tau[0, 0, 0, 0] + tau[1, 0, 0, 0])
     assert abs((m1 - m0) - expect) <= 2e-3 * abs(expect)
+
+
+# ----------------------------------------------------------------------------- SURVEY.md 8(f) item 1, y walls
+def test_wall_model_on_y_walls_is_the_z_wall_model_rotated(oracle):
+    """Duct WMLES: the wall model on the y walls must be the (already pinned) z-wall model with the roles of
+    y and z exchanged.  Case A: z walls with the wall model, periodic y.  Case B: the same field with y and z swapped
+    (v <-> w), y walls with the wall model, periodic z.  Stresses and one full step must agree under the swap."""
+    nx, n1, n2 = 12, 8, 6             # n1 points across the walls, n2 along the periodic direction
+    L1, L2 = 2.0, 1.5
+    rng = np.random.default_rng(21)
+    prof = np.log(np.minimum((np.arange(n1) + 0.5) * L1 / n1, L1 - (np.arange(n1) + 0.5) * L1 / n1) * 800) / 0.41 + 5.2
+    # case A arrays [z = wall dir (n1)][y = periodic (n2)][x]
+    uA = prof[:, None, None] + 0.4 * rng.standard_normal((n1, n2, nx))
+    pA = 0.4 * rng.standard_normal((n1, n2, nx))          # periodic-direction component
+    qA = 0.4 * rng.standard_normal((n1, n2, nx)); qA[-1] = 0.0   # wall-normal component (faces; last = wall)
+    kw = dict(nu=1.0 / 800, sgs_model=1, cs=0.1)
+    A = oracle.Oracle(nx, n2, n1, 3.0, L2, L1, bc_z=1, wall_model=1, **kw)
+    A.set_velocity(uA, pA, qA)
+    B = oracle.Oracle(nx, n1, n2, 3.0, L1, L2, bc_y=1, bc_z=0, wall_model_y=1, **kw)
+    sw = lambda a: np.ascontiguousarray(np.swapaxes(a, 0, 1))
+    B.set_velocity(sw(uA), sw(qA), sw(pA))
+    tA, tB = A.wall_stress(), B.wall_stress_y()            # [wall][comp][ny=n2][nx] vs [wall][comp][nz=n2][nx]
+    assert np.max(np.abs(tA - tB)) <= 1e-13 * np.max(np.abs(tA))
+    nA, nB = A.eddy_viscosity(), B.eddy_viscosity()
+    assert np.max(np.abs(nA - sw(nB))) <= 1e-13 * np.max(np.abs(nA))
+    A.project(); B.project()
+    dt = 2e-4
+    for _ in range(2):
+        A.step(dt); B.step(dt)
+    for fa, fb in ((0, 0), (1, 2), (2, 1), (4, 4)):
+        a, b = A.get(fa), sw(B.get(fb))
+        assert np.max(np.abs(a - b)) <= 1e-11 * max(np.max(np.abs(a)), 1e-3), (fa, fb)
