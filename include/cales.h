@@ -69,6 +69,7 @@ typedef struct {
   size_t workspace_bytes;
   void* cuda_stream;         /* cudaStream_t of the caller */
   int device;                /* CUDA device ordinal the workspace lives on */
+  int wall_model_y;          /* log-law wall model on the y walls too (duct WMLES); needs bc_y = wall */
 } cales_params;
 
 typedef struct {
@@ -130,6 +131,10 @@ int cales_eddy_viscosity(cales_solver* s, const double* u, const double* v, cons
  * tau_dev DEVICE [wall(0 bottom,1 top)][comp(0: tau_xz at u points, 1: tau_yz at v points)][ny][nx]
  * (NULL = only refresh the internal planes).  Asynchronous. */
 int cales_wall_stress(cales_solver* s, double* tau_dev);
+
+/* The same for the y walls (wall_model_y): tau_dev DEVICE [wall(0: j = 0 side, 1: j = ny-1 side)][comp(0: tau_xy at u points,
+ * 1: tau_zy at w points)][nz][nx] (NULL = only refresh the internal planes).  Asynchronous. */
+int cales_wall_stress_y(cales_solver* s, double* tau_dev);
 
 /* Make the solver's velocity discretely solenoidal by one projection with gamma*dt = 1 (Eq. 12-13). */
 int cales_project(cales_solver* s);

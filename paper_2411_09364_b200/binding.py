@@ -25,6 +25,7 @@ class CalesParams(C.Structure):
         ("implicit_z", C.c_int),
         ("const_flow_rate", C.c_int), ("u_bulk", C.c_double),
         ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t), ("cuda_stream", C.c_void_p), ("device", C.c_int),
+        ("wall_model_y", C.c_int),
     ]
 
 
@@ -38,7 +39,7 @@ class CalesDiag(C.Structure):
 # every symbol include/cales.h declares
 SYMBOLS = ["cales_default_params", "cales_workspace_bytes", "cales_create", "cales_create_basic", "cales_destroy",
            "cales_set_field", "cales_get_field", "cales_step", "cales_poisson_solve", "cales_eddy_viscosity",
-           "cales_wall_stress", "cales_project", "cales_cfl_dt", "cales_plane_stats", "cales_get_cs", "cales_transform", "cales_transpose_xy",
+           "cales_wall_stress", "cales_wall_stress_y", "cales_project", "cales_cfl_dt", "cales_plane_stats", "cales_get_cs", "cales_transform", "cales_transpose_xy",
            "cales_set_timing", "cales_set_graph", "cales_kernel_count", "cales_kernel_time", "cales_launches_per_step", "cales_diagnostics", "cales_last_error"]
 
 _lib = None
@@ -64,6 +65,7 @@ def lib():
         L.cales_poisson_solve.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.cales_eddy_viscosity.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.cales_wall_stress.argtypes = [C.c_void_p, C.c_void_p]
+        L.cales_wall_stress_y.argtypes = [C.c_void_p, C.c_void_p]
         L.cales_project.argtypes = [C.c_void_p]
         L.cales_get_cs.argtypes = [C.c_void_p, C.c_void_p]
         L.cales_cfl_dt.argtypes = [C.c_void_p, C.c_double, C.POINTER(C.c_double)]
@@ -213,6 +215,11 @@ class Solver:
     def wall_stress(self):
         tau = self._torch.empty((2, 2, self.ny, self.nx), dtype=self._torch.float64, device=self.device)
         _chk(lib().cales_wall_stress(self._h, C.c_void_p(tau.data_ptr())))
+        return tau
+
+    def wall_stress_y(self):
+        tau = self._torch.empty((2, 2, self.nz, self.nx), dtype=self._torch.float64, device=self.device)
+        _chk(lib().cales_wall_stress_y(self._h, C.c_void_p(tau.data_ptr())))
         return tau
 
     def project(self):

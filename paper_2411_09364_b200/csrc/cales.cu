@@ -38,7 +38,7 @@ struct cales_solver {
   long long N, nxy;
   // fields
   double *u, *v, *w, *p, *nut, *us, *vs, *ws, *Ru, *Rv, *Rw, *W, *CP, *CQ, *smag;
-  double *tau;
+  double *tau, *tau_y;
   // tables
   double *dzf, *dzc, *rdzf, *rdzc, *delta, *zc, *ak, *ck, *lamx, *lamy, *cncoef, *partial, *stage1, *scal, *dsm_part, *dsm_cs;
   double2 *twx, *twy, *dctw;
@@ -73,6 +73,7 @@ static size_t carve(cales_solver* s, const cales_params* p, double* base) {
   double* CQ = p->bc_z == CALES_BC_PERIODIC ? take(N) : nullptr;
   double* smag = p->sgs_model == CALES_SGS_DSMAG ? take(N) : nullptr;
   double* tau = take(4 * nxy);
+  double* tau_y = take(4 * (size_t)p->nx * p->nz);
   double* dzf = take(p->nz + 2); double* dzc = take(p->nz + 2); double* zc = take(p->nz);
   double* rdzf = take(p->nz + 2); double* rdzc = take(p->nz + 2); double* delta = take(p->nz);
   double* ak = take(p->nz); double* ck = take(p->nz);
@@ -88,7 +89,7 @@ static size_t carve(cales_solver* s, const cales_params* p, double* base) {
   double* dsm_cs = p->sgs_model == CALES_SGS_DSMAG ? take((size_t)p->nz * p->ny) : nullptr;
   if (s && base) {
     s->u = f[0]; s->v = f[1]; s->w = f[2]; s->p = f[3]; s->nut = f[4]; s->us = f[5]; s->vs = f[6]; s->ws = f[7];
-    s->Ru = f[8]; s->Rv = f[9]; s->Rw = f[10]; s->W = f[11]; s->CP = CP; s->CQ = CQ; s->smag = smag; s->tau = tau;
+    s->Ru = f[8]; s->Rv = f[9]; s->Rw = f[10]; s->W = f[11]; s->CP = CP; s->CQ = CQ; s->smag = smag; s->tau = tau; s->tau_y = tau_y;
     s->dzf = dzf; s->dzc = dzc; s->zc = zc; s->rdzf = rdzf; s->rdzc = rdzc; s->delta = delta; s->ak = ak; s->ck = ck; s->lamx = lamx; s->lamy = lamy;
     s->twx = reinterpret_cast<double2*>(twx); s->twy = reinterpret_cast<double2*>(twy); s->dctw = reinterpret_cast<double2*>(dctw);
     s->cncoef = cncoef; s->partial = partial; s->stage1 = stage1; s->scal = scal; s->maxit = reinterpret_cast<int*>(scal + 16);
@@ -171,7 +172,7 @@ extern "C" int cales_create(const cales_params* p, cales_solver** out) {
   if (e == cudaSuccess) e = cudaStreamSynchronize(s->st);
   if (e != cudaSuccess) { delete s; return fail(CALES_ECUDA, std::string("table upload: ") + cudaGetErrorString(e)); }
   s->c = H.c;
-  s->c.dzf = s->dzf + 1; s->c.dzc = s->dzc + 1; s->c.zc = s->zc; s->c.rdzf = s->rdzf + 1; s->c.rdzc = s->rdzc + 1; s->c.delta = s->delta; s->c.tau = s->tau;
+  s->c.dzf = s->dzf + 1; s->c.dzc = s->dzc + 1; s->c.zc = s->zc; s->c.rdzf = s->rdzf + 1; s->c.rdzc = s->rdzc + 1; s->c.delta = s->delta; s->c.tau = s->tau; s->c.tau_y = s->tau_y;
   s->pt.ak = s->ak; s->pt.ck = s->ck; s->pt.lamx = s->lamx; s->pt.lamy = s->lamy;
   s->wg = H.wg;
   s->plx = H.plx; s->plx.tw = s->twx;
@@ -283,12 +284,19 @@ static int run_poisson_core(cales_solver* s) {
   return CALES_OK;
 }
 static int run_wall_stress(cales_solver* s) {
-  if (!s->c.wall_model) return CALES_OK;
+  if (!s->c.wall_model && !s->c.wall_model_y) return CALES_OK;
   CUDA_TRY(cudaMemsetAsync(s->maxit, 0, sizeof(int), s->st));
   tick(s, -1);
-  dim3 grid(s->pgrid.x, s->pgrid.y, 4);
-  k_wall_stress<<<grid, s->pblock, 0, s->st>>>(s->c, s->wg, s->u, s->v, s->tau, s->maxit);
-  LAUNCH_TRY(K_WALL);
+  if (s->c.wall_model) {
+    dim3 grid(s->pgrid.x, s->pgrid.y, 4);
+    k_wall_stress<<<grid, s->pblock, 0, s->st>>>(s->c, s->wg, s->u, s->v, s->tau, s->maxit);
+    LAUNCH_TRY(K_WALL);
+  }
+  if (s->c.wall_model_y) {
+    dim3 grid((s->c.nx + 31) / 32, (s->c.nz + 7) / 8, 4);
+    k_wall_stress_y<<<grid, dim3(32, 8), 0, s->st>>>(s->c, s->u, s->w, s->tau_y, s->maxit);
+    LAUNCH_TRY(K_WALL);
+  }
   return CALES_OK;
 }
 static int run_eddy_viscosity(cales_solver* s, const double* u, const double* v, const double* w, double* nut) {
@@ -440,7 +448,7 @@ extern "C" int cales_set_graph(cales_solver* s, int on) {
 extern "C" int cales_launches_per_step(cales_solver* s) {
   if (!s) return 0;
   const Ctx& c = s->c;
-  int per = 1 /*rhs*/ + (c.implicit_z ? 1 : 0) + (c.const_flow_rate ? 2 : 0) + 5 /*solver*/ + 1 /*correct*/ + (c.wall_model ? 1 : 0) +
+  int per = 1 /*rhs*/ + (c.implicit_z ? 1 : 0) + (c.const_flow_rate ? 2 : 0) + 5 /*solver*/ + 1 /*correct*/ + (c.wall_model ? 1 : 0) + (c.wall_model_y ? 1 : 0) +
             1 /*static nu_t or fill*/;
   if (c.sgs == CALES_SGS_DSMAG) {
     const bool ywall = c.bc_y == BC_WALL, split = ywall && c.ny >= 3 * DSM_TY;
@@ -471,6 +479,15 @@ extern "C" int cales_wall_stress(cales_solver* s, double* tau_dev) {
   int rc = run_wall_stress(s);
   if (rc) return rc;
   if (tau_dev) CUDA_TRY(cudaMemcpyAsync(tau_dev, s->tau, 4 * s->nxy * sizeof(double), cudaMemcpyDeviceToDevice, s->st));
+  return CALES_OK;
+}
+
+extern "C" int cales_wall_stress_y(cales_solver* s, double* tau_dev) {
+  if (!s) return fail(CALES_EINVAL, "null solver");
+  if (!s->c.wall_model_y) return fail(CALES_EINVAL, "solver has no wall model on the y walls");
+  int rc = run_wall_stress(s);
+  if (rc) return rc;
+  if (tau_dev) CUDA_TRY(cudaMemcpyAsync(tau_dev, s->tau_y, 4 * (size_t)s->c.nx * s->c.nz * sizeof(double), cudaMemcpyDeviceToDevice, s->st));
   return CALES_OK;
 }
 

@@ -56,6 +56,31 @@ CALES_HD int wall_stress_point(const Ctx& c, const WallGeom& g, const double* u,
   return it;
 }
 
+// y walls (duct WMLES): sampled at the first off-wall centre, h = dy/2.  comp 0: tau_xy at the u point
+// (i+1/2, k) from u and the 4 surrounding w points; comp 1: tau_zy at the w point (i, k+1/2) from w and the 4 surrounding u.
+// tau_y[wall][comp][k][i].
+CALES_HD int wall_stress_y_point(const Ctx& c, const double* u, const double* w, int wall, int comp, int i, int k, double* tau_y) {
+  const int j0 = wall == 0 ? 0 : c.ny - 1;
+  const double h = 0.5 * c.dy;
+  double a, b;
+  if (comp == 0) {
+    a = velg<0>(c, u, i, j0, k, GH_STRAIN);
+    b = 0.25 * (velg<2>(c, w, i, j0, k, GH_STRAIN) + velg<2>(c, w, i + 1, j0, k, GH_STRAIN) + velg<2>(c, w, i, j0, k - 1, GH_STRAIN) + velg<2>(c, w, i + 1, j0, k - 1, GH_STRAIN));
+  } else {
+    a = velg<2>(c, w, i, j0, k, GH_STRAIN);
+    b = 0.25 * (velg<0>(c, u, i, j0, k, GH_STRAIN) + velg<0>(c, u, i - 1, j0, k, GH_STRAIN) + velg<0>(c, u, i, j0, k + 1, GH_STRAIN) + velg<0>(c, u, i - 1, j0, k + 1, GH_STRAIN));
+  }
+  const double U = sqrt(a * a + b * b);
+  double t = 0.0; int it = 0;
+  if (U > 0.0) {
+    const double hp = loglaw_hplus(U * h / c.nu, c.kappa, c.Blog, c.wm_tol, c.wm_maxit, &it);
+    const double utau = hp * c.nu / h;
+    t = utau * utau * a / U;
+  }
+  tau_y[((long long)(wall * 2 + comp) * c.nz + k) * c.nx + i] = t;
+  return it;
+}
+
 // ------------------------------------------------------------------------------------------------------------
 // Strain rate at a cell centre: diagonals directly; off-diagonals at the 4 surrounding edge
 // midpoints, then averaged.  U(di,dj,dk), V, W return the face values at offsets from the cell.
@@ -182,14 +207,22 @@ CALES_HD void dsm_mid(int tid, int nth, const Ctx& c, int i0, int j0, int k, con
     const int cp = idx / per, r = idx % per;
     const int comp = cp / 3, pl = cp % 3, my = r / DSM_MX, mx = r % DSM_MX;
     const int gj = j0 - 1 + my;
-    double wy[3]; dsm_wy(c, gj, comp == 1 ? 1 : 0, wy);
-    double s = 0.0;
+    // filtered face value of mid row m (global row j0 - 1 + m)
+    auto fval = [&](int m) {
+      double wy[3]; dsm_wy(c, j0 - 1 + m, comp == 1 ? 1 : 0, wy);
+      double s = 0.0;
 #pragma unroll
-    for (int b = 0; b < 3; ++b) {
-      const double* row = raw + dsm_raw_off(comp, pl, my + b, mx);
-      s += wy[b] * (0.25 * row[0] + 0.5 * row[1] + 0.25 * row[2]);
-    }
-    flt[idx] = s;
+      for (int b = 0; b < 3; ++b) {
+        const double* row = raw + dsm_raw_off(comp, pl, m + b, mx);
+        s += wy[b] * (0.25 * row[0] + 0.5 * row[1] + 0.25 * row[2]);
+      }
+      return s;
+    };
+    // Ghost rows of the FILTERED velocity at a wall-model y wall: the boundary condition is applied to the filtered field
+    // (one-sided extrapolation of its first two rows), which is not the filter of the extrapolated raw field.
+    if (c.bc_y == BC_WALL && c.wall_model_y && comp != 1 && (gj < 0 || gj >= c.ny))
+      flt[idx] = gj < 0 ? 2.0 * fval(my + 1) - fval(my + 2) : 2.0 * fval(my - 1) - fval(my - 2);
+    else flt[idx] = fval(my);
   }
   const double rdx = c.rdx, rdy = c.rdy, rdzf = c.rdzf[k], rdzc = c.rdzc[k], rdzcm = c.rdzc[k - 1];
   for (int r = tid; r < per; r += nth) {
@@ -392,6 +425,14 @@ __global__ void k_wall_stress(Ctx c, WallGeom g, const double* __restrict__ u, c
   const int wall = blockIdx.z >> 1, comp = blockIdx.z & 1;
   int it = 0;
   if (i < c.nx && j < c.ny) it = wall_stress_point(c, g, u, v, wall, comp, i, j, tau);
+  it = __reduce_max_sync(0xffffffffu, it);
+  if ((threadIdx.x & 31) == 0 && it > 0) atomicMax(maxit, it);
+}
+// grid (ceil(nx/32), ceil(nz/8), 4), block (32, 8)
+__global__ void k_wall_stress_y(Ctx c, const double* __restrict__ u, const double* __restrict__ w, double* __restrict__ tau_y, int* __restrict__ maxit) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x, k = blockIdx.y * blockDim.y + threadIdx.y;
+  int it = 0;
+  if (i < c.nx && k < c.nz) it = wall_stress_y_point(c, u, w, blockIdx.z >> 1, blockIdx.z & 1, i, k, tau_y);
   it = __reduce_max_sync(0xffffffffu, it);
   if ((threadIdx.x & 31) == 0 && it > 0) atomicMax(maxit, it);
 }

@@ -18,7 +18,7 @@ enum { GH_VISC = 0, GH_STRAIN = 1 };  // ghost of the wall-parallel velocity at 
 // Grid, options and table pointers, passed by value to every kernel.
 struct Ctx {
   int nx, ny, nz;
-  int bc_y, bc_z, wall_model, sgs, van_driest, implicit_z, dsm_plane, dsm_clip_total, const_flow_rate;
+  int bc_y, bc_z, wall_model, wall_model_y, sgs, van_driest, implicit_z, dsm_plane, dsm_clip_total, const_flow_rate;
   int wm_maxit;
   long long N;     // nx*ny*nz
   long long nxy;   // nx*ny
@@ -31,6 +31,7 @@ struct Ctx {
   const double* rdzc;  // 1/dzc[-1 .. nz-1]
   const double* delta; // filter width Delta_k = (dx dy dzf[k])^(1/3), k = 0..nz-1 (S4)
   const double* tau;   // wall stress planes [wall][comp][ny][nx]
+  const double* tau_y; // y-wall stress planes [wall][comp (0 tau_xy at u points, 1 tau_zy at w points)][nz][nx]
 };
 
 CALES_HD long long idx3(const Ctx& c, int i, int j, int k) { return (long long)i + (long long)c.nx * ((long long)j + (long long)c.ny * (long long)k); }
@@ -42,31 +43,43 @@ CALES_HD int wrapi(int i, int n) { return i < 0 ? i + n : (i >= n ? i - n : i); 
 //   z periodic, or walls: w = 0 on the wall faces and beyond; u, v: no-slip mirror, or with the wall model
 //   GH_VISC   ghost = q0 - tau * dzc_wall / nu       (the modelled stress is the wall viscous flux)
 //   GH_STRAIN ghost = linear extrapolation of q0, q1 (one-sided derivative for the strain rate).
+// x already wrapped, 0 <= j < ny: periodic wrap or wall ghosts in z only
 template <int COMP>
-CALES_HD double velg(const Ctx& c, const double* __restrict__ q, int i, int j, int k, int mode) {
-  i = wrapi(i, c.nx);
-  double sy = 1.0;
-  if (c.bc_y == BC_PER) j = wrapi(j, c.ny);
-  else {
-    if (COMP == 1) { if (j < 0 || j >= c.ny - 1) return 0.0; }
-    else { if (j < 0) { j = 0; sy = -1.0; } else if (j >= c.ny) { j = c.ny - 1; sy = -1.0; } }
-  }
-  if (c.bc_z == BC_PER) return sy * q[idx3(c, i, j, wrapi(k, c.nz))];
-  if (COMP == 2) { if (k < 0 || k >= c.nz - 1) return 0.0; return sy * q[idx3(c, i, j, k)]; }
-  if (k >= 0 && k < c.nz) return sy * q[idx3(c, i, j, k)];
+CALES_HD double velg_z(const Ctx& c, const double* __restrict__ q, int i, int j, int k, int mode) {
+  if (c.bc_z == BC_PER) return q[idx3(c, i, j, wrapi(k, c.nz))];
+  if (COMP == 2) { if (k < 0 || k >= c.nz - 1) return 0.0; return q[idx3(c, i, j, k)]; }
+  if (k >= 0 && k < c.nz) return q[idx3(c, i, j, k)];
   const bool bottom = k < 0;
   const int k0 = bottom ? 0 : c.nz - 1;
   const double q0 = q[idx3(c, i, j, k0)];
-  if (!c.wall_model) return -sy * q0;
+  if (!c.wall_model) return -q0;
   if (mode == GH_VISC) {
     const double t = c.tau[((long long)((bottom ? 0 : 2) + COMP) * c.ny + j) * c.nx + i];
     const double dz = bottom ? c.dzc[-1] : c.dzc[c.nz - 1];
-    return sy * (q0 - t * dz / c.nu);
+    return q0 - t * dz / c.nu;
   }
   const int k1 = bottom ? 1 : c.nz - 2;
   const double q1 = q[idx3(c, i, j, k1)];
   const double r = bottom ? c.dzc[-1] / c.dzc[0] : c.dzc[c.nz - 1] / c.dzc[c.nz - 2];
-  return sy * (q0 + (q0 - q1) * r);
+  return q0 + (q0 - q1) * r;
+}
+template <int COMP>
+CALES_HD double velg(const Ctx& c, const double* __restrict__ q, int i, int j, int k, int mode) {
+  i = wrapi(i, c.nx);
+  if (c.bc_y == BC_PER) return velg_z<COMP>(c, q, i, wrapi(j, c.ny), k, mode);
+  if (COMP == 1) { if (j < 0 || j >= c.ny - 1) return 0.0; return velg_z<COMP>(c, q, i, j, k, mode); }
+  if (j >= 0 && j < c.ny) return velg_z<COMP>(c, q, i, j, k, mode);
+  const bool low = j < 0;
+  const int j0 = low ? 0 : c.ny - 1;
+  const double q0 = velg_z<COMP>(c, q, i, j0, k, mode);
+  if (!c.wall_model_y) return -q0;                       // no-slip mirror
+  // wall model on the y walls (duct WMLES): same two ghost kinds as in z, uniform spacing dy
+  if (mode == GH_VISC) {
+    const int kk = k < 0 ? 0 : (k >= c.nz ? c.nz - 1 : k);
+    const double t = c.tau_y[((long long)((low ? 0 : 2) + (COMP == 0 ? 0 : 1)) * c.nz + kk) * c.nx + i];
+    return q0 - t * c.dy / c.nu;
+  }
+  return 2.0 * q0 - velg_z<COMP>(c, q, i, low ? 1 : c.ny - 2, k, mode);
 }
 
 // Cell-centred scalar with ghost = sgn * interior at walls (sgn = +1: Neumann, p and phi; sgn = -1: nu_t,

@@ -36,6 +36,7 @@ static inline int validate(const cales_params* p) {
   if (p->bc_z == CALES_BC_PERIODIC && p->zstretch != CALES_Z_UNIFORM) return fail(CALES_EUNSUPPORTED, "periodic z requires a uniform grid");
   if (p->sgs_model < 0 || p->sgs_model > 2) return fail(CALES_EINVAL, "bad sgs_model");
   if (p->wall_model && p->bc_z != CALES_BC_WALL) return fail(CALES_EUNSUPPORTED, "wall model needs z walls");
+  if (p->wall_model_y && p->bc_y != CALES_BC_WALL) return fail(CALES_EUNSUPPORTED, "wall model on y walls needs y walls");
   if (p->implicit_z && p->bc_z != CALES_BC_WALL) return fail(CALES_EUNSUPPORTED, "implicit z needs z walls");
   if (p->wall_model && p->h_wm > 0.0 && !(p->h_wm < 0.5 * p->lz)) return fail(CALES_EINVAL, "h_wm must lie below the half height");
   if (p->van_driest && (p->bc_z != CALES_BC_WALL || p->bc_y == CALES_BC_WALL || p->wall_model))
@@ -145,12 +146,12 @@ static inline int build_setup(const cales_params* p, HostSetup& H) {
   // ---- device context (pointers are set by the owner of the tables)
   Ctx& c = H.c;
   c.nx = nx; c.ny = ny; c.nz = nz; c.N = (long long)nx * ny * nz; c.nxy = (long long)nx * ny;
-  c.bc_y = p->bc_y; c.bc_z = p->bc_z; c.wall_model = p->wall_model; c.sgs = p->sgs_model; c.van_driest = p->van_driest;
+  c.bc_y = p->bc_y; c.bc_z = p->bc_z; c.wall_model = p->wall_model; c.wall_model_y = p->wall_model_y; c.sgs = p->sgs_model; c.van_driest = p->van_driest;
   c.implicit_z = p->implicit_z; c.dsm_plane = p->dsm_avg_xy_plane; c.dsm_clip_total = p->dsm_clip_total; c.const_flow_rate = p->const_flow_rate;
   c.wm_maxit = H.P.wm_maxit; c.dx = dx; c.dy = dy; c.rdx = 1.0 / dx; c.rdy = 1.0 / dy; c.lz = p->lz; c.nu = p->nu; c.cs = p->cs; c.aplus = H.P.aplus; c.rnuap = 1.0 / (p->nu * H.P.aplus);
   c.alpha = p->dsm_alpha2d > 0.0 ? p->dsm_alpha2d : std::cbrt(4.0);
   c.kappa = H.P.kappa; c.Blog = p->B; c.h_wm = p->h_wm; c.wm_tol = H.P.wm_tol; c.u_bulk = p->u_bulk;
-  c.dzf = nullptr; c.dzc = nullptr; c.zc = nullptr; c.rdzf = nullptr; c.rdzc = nullptr; c.delta = nullptr; c.tau = nullptr;
+  c.dzf = nullptr; c.dzc = nullptr; c.zc = nullptr; c.rdzf = nullptr; c.rdzc = nullptr; c.delta = nullptr; c.tau = nullptr; c.tau_y = nullptr;
   // ---- wall-model sampling geometry (linear interpolation between locations 1 and 2)
   for (int wall = 0; wall < 2; ++wall) {
     auto dist = [&](int q) { return wall == 0 ? H.zc[q] : p->lz - H.zc[nz - 1 - q]; };

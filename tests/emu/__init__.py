@@ -76,6 +76,9 @@ class Emu:
     def wall_stress(self):
         tau = np.empty((2, 2, self.ny, self.nx)); lib().emu_wall_stress(self._h, _p(tau)); return tau
 
+    def wall_stress_y(self):
+        tau = np.empty((2, 2, self.nz, self.nx)); lib().emu_wall_stress_y(self._h, _p(tau)); return tau
+
     def get_cs(self):
         cs = np.empty(self.nz if self.per_plane else self.nz * self.ny); lib().emu_get_cs(self._h, _p(cs)); return cs
 

@@ -24,7 +24,7 @@ struct emu_solver {
   FftPlan plx, ply;
   PoissonTabs pt;
   long long N, nxy;
-  std::vector<double> u, v, w, p, nut, us, vs, ws, Ru, Rv, Rw, W, CP, CQ, smag, tau, cncoef, dsm_part, dsm_cs;
+  std::vector<double> u, v, w, p, nut, us, vs, ws, Ru, Rv, Rw, W, CP, CQ, smag, tau, tau_y, cncoef, dsm_part, dsm_cs;
   double scal[4];
   int maxit;
   bool fresh;
@@ -41,10 +41,11 @@ extern "C" int emu_create(const cales_params* p, emu_solver** out) {
   const size_t N = (size_t)s->N;
   for (auto* f : {&s->u, &s->v, &s->w, &s->p, &s->nut, &s->us, &s->vs, &s->ws, &s->Ru, &s->Rv, &s->Rw, &s->W, &s->CP, &s->CQ, &s->smag}) f->assign(N, 0.0);
   s->tau.assign(4 * (size_t)s->nxy, 0.0);
+  s->tau_y.assign(4 * (size_t)p->nx * p->nz, 0.0);
   s->cncoef.assign(6 * (size_t)p->nz, 0.0);
   s->dsm_part.assign((size_t)p->nz * p->ny * dsm_shape(p->nx).pslots * 2, 0.0);
   s->dsm_cs.assign((size_t)p->nz * p->ny, 0.0);
-  s->c.dzf = H.dzf.data() + 1; s->c.dzc = H.dzc.data() + 1; s->c.zc = H.zc.data(); s->c.rdzf = H.rdzf.data() + 1; s->c.rdzc = H.rdzc.data() + 1; s->c.delta = H.delta.data(); s->c.tau = s->tau.data();
+  s->c.dzf = H.dzf.data() + 1; s->c.dzc = H.dzc.data() + 1; s->c.zc = H.zc.data(); s->c.rdzf = H.rdzf.data() + 1; s->c.rdzc = H.rdzc.data() + 1; s->c.delta = H.delta.data(); s->c.tau = s->tau.data(); s->c.tau_y = s->tau_y.data();
   s->plx = H.plx; s->plx.tw = reinterpret_cast<const double2*>(H.twx.data());
   s->ply = H.ply; s->ply.tw = reinterpret_cast<const double2*>(H.twy.data()); s->ply.dctw = reinterpret_cast<const double2*>(H.dctw.data());
   s->pt.ak = H.ak.data(); s->pt.ck = H.ck.data(); s->pt.lamx = H.lamx.data(); s->pt.lamy = H.lamy.data();
@@ -143,6 +144,13 @@ static void emu_poisson_core(emu_solver* s) {
   emu_fft_y(s, s->W.data(), 1);
 }
 static void emu_tau(emu_solver* s) {
+  if (s->c.wall_model_y) {
+    if (!s->c.wall_model) s->maxit = 0;
+    std::vector<double> ty(s->tau_y.size());      // all stresses come from the velocity only: order of evaluation is immaterial
+    for (int z = 0; z < 4; ++z) for (int k = 0; k < s->c.nz; ++k) for (int i = 0; i < s->c.nx; ++i)
+      wall_stress_y_point(s->c, s->u.data(), s->w.data(), z >> 1, z & 1, i, k, ty.data());
+    s->tau_y = ty; s->c.tau_y = s->tau_y.data();
+  }
   if (!s->c.wall_model) return;
   s->maxit = 0;
   for (int z = 0; z < 4; ++z) for (int j = 0; j < s->c.ny; ++j) for (int i = 0; i < s->c.nx; ++i) {
@@ -357,3 +365,4 @@ extern "C" int emu_plane_stats(emu_solver* s, double* out) {
   }
   return 0;
 }
+extern "C" int emu_wall_stress_y(emu_solver* s, double* tau) { emu_tau(s); std::memcpy(tau, s->tau_y.data(), s->tau_y.size() * sizeof(double)); return 0; }

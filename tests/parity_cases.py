@@ -19,7 +19,9 @@ SMALL = {
     "cfg5_wmles_dsm": (5, (36, 24, 16), 2),
     "duct_static_smag": (4, (24, 12, 12), 2, dict(sgs_model=1, cs=0.1)),   # static model next to y walls
     "cfg5_hwm_interp": (5, (24, 12, 16), 2, dict(h_wm=0.1)),               # wall model sampled between centres
-    "cfg2_wm_implicit": (2, (24, 12, 16), 2, dict(implicit_z=1)),          # wall model + Crank-Nicolson in z (8(f) item 1)
+    "cfg2_wm_implicit": (2, (24, 12, 16), 2, dict(implicit_z=1)),
+    "duct_wmles_dsm": (4, (48, 24, 16), 2, dict(wall_model=1, wall_model_y=1, nu=1.0 / 40000)),   # duct WMLES: wall model on all four walls
+    "duct_wmles_smag_y_only": (4, (24, 12, 12), 2, dict(wall_model_y=1, sgs_model=1, cs=0.1, nu=1.0 / 40000)),          # wall model + Crank-Nicolson in z (8(f) item 1)
 }
 # the sizes the GPU parity tests use: several tiles in every direction plus ragged tails
 GPU_CASES = {
@@ -33,6 +35,8 @@ GPU_CASES = {
     "cfg4_duct_dsm_narrow": (4, (72, 4, 16), 2),
     "cfg2_wm_implicit": (2, (96, 48, 32), 3, dict(implicit_z=1)),
     "cfg5_wm_implicit_dsm": (5, (96, 48, 32), 2, dict(implicit_z=1, h_wm=0.1)),
+    "duct_wmles_dsm": (4, (192, 54, 48), 3, dict(wall_model=1, wall_model_y=1, nu=1.0 / 40000)),
+    "duct_wmles_smag_implicit": (4, (96, 36, 24), 2, dict(wall_model=1, wall_model_y=1, sgs_model=1, cs=0.1, implicit_z=1, nu=1.0 / 40000)),
 }
 
 

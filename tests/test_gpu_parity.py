@@ -394,3 +394,18 @@ def test_extreme_line_lengths(oracle, gpu, shape, bc_y):
     a, b = g.poisson_solve(torch.from_numpy(f).cuda()).cpu().numpy(), o.poisson_solve(f)
     assert np.max(np.abs(a - b)) <= 1e-10 * np.max(np.abs(b))
     g.close()
+
+
+def test_wall_stress_on_y_walls_parity(oracle, gpu):
+    """Duct WMLES: wall model on all four walls; both stress sets and nu_t."""
+    cfg, kw, (u, v, w), dt = pc.prepare(oracle, 4, (96, 36, 24), dict(wall_model=1, wall_model_y=1, nu=1.0 / 40000))
+    o = pc.make(oracle.Oracle, kw)
+    g = pc.make(gpu.Solver, kw)
+    o.set_velocity(u, v, w); g.set_velocity(u, v, w)
+    a, b = g.wall_stress_y().cpu().numpy(), o.wall_stress_y()
+    assert np.max(np.abs(a - b)) <= 1e-12 * np.max(np.abs(b))
+    a, b = g.wall_stress().cpu().numpy(), o.wall_stress()
+    assert np.max(np.abs(a - b)) <= 1e-12 * np.max(np.abs(b))
+    a, b = g.eddy_viscosity().cpu().numpy(), o.eddy_viscosity()
+    assert np.max(np.abs(a - b)) <= 1e-11 * max(np.max(np.abs(b)), kw["nu"])
+    g.close()
