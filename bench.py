@@ -46,7 +46,7 @@ ALGO_FLOPS = {"k_dsm_col": 415.0}
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture (profiles/r1_ncu_full.md),
 # keyed by (config, kernel); None where no capture of that kernel at that size is committed.
-NCU_TRAFFIC = {(5, "k_dsm_col"): 65.2e9, (5, "k_rhs"): 97.7e9, (5, "k_correct"): 63.9e9, (5, "k_poisson_z"): 37.0e9, (5, "k_fft_x_fwd"): 26.9e9,
+NCU_TRAFFIC = {(5, "k_dsm_col"): 65.2e9, (5, "k_rhs"): 98.5e9, (5, "k_correct"): 63.9e9, (5, "k_poisson_z"): 37.0e9, (5, "k_fft_x_fwd"): 26.9e9,
                (5, "k_fft_y_fwd"): 12.8e9, (5, "k_fft_y_inv"): 12.8e9, (5, "k_fft_x_inv"): 12.8e9, (5, "k_dsm_nut"): 12.8e9}
 
 
