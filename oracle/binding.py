@@ -20,7 +20,7 @@ class OracleParams(C.Structure):
         ("wm_tol", C.c_double), ("wm_maxit", C.c_int),
         ("implicit_z", C.c_int),
         ("const_flow_rate", C.c_int), ("u_bulk", C.c_double),
-        ("wall_model_y", C.c_int),
+        ("wall_model_y", C.c_int), ("dsm_filter3d", C.c_int),
     ]
 
 
@@ -97,7 +97,7 @@ def rk3_coeffs(k):
 PARAM_DEFAULTS = dict(
     zstretch=0, zstretch_factor=0.0, bc_y=0, bc_z=0, nu=1e-3, sgs_model=0, cs=0.17, van_driest=0, aplus=25.0,
     dsm_avg_xy_plane=1, dsm_clip_total=0, dsm_alpha2d=0.0, wall_model=0, kappa=0.41, B=5.2, h_wm=0.0,
-    wm_tol=1e-4, wm_maxit=50, implicit_z=0, const_flow_rate=0, u_bulk=0.0, wall_model_y=0)
+    wm_tol=1e-4, wm_maxit=50, implicit_z=0, const_flow_rate=0, u_bulk=0.0, wall_model_y=0, dsm_filter3d=0)
 
 
 class Oracle:
@@ -192,6 +192,10 @@ class Oracle:
     def filter_xy(self, q):
         q = _arr(q); out = np.empty(self.shape)
         _chk(lib().oracle_filter_xy(self._h, _p(q), _p(out))); return out
+
+    def test_filter(self, q, kind=0):
+        q = _arr(q); out = np.empty(self.shape)
+        _chk(lib().oracle_test_filter(self._h, _p(q), _p(out), C.c_int(kind))); return out
 
     def get_cs(self):
         n = self.nz if self.params["dsm_avg_xy_plane"] else self.nz * self.ny

@@ -650,6 +650,36 @@ static void filter_xy_vface(const oracle_solver& S, const double* q, double* out
   }
 }
 
+// z part of the 3-D box test filter ("2D or 3D box filters ... assumes uniform grid spacing"): the same
+// (1/4,1/2,1/4) weights along z.  "The 3D box filter cannot be used in the first off-wall layer, hence a 2D box filter
+// is applied through linear extrapolation ... to the ghost points, followed by ... a 3D filter": extrapolation followed
+// by the symmetric 3-point filter is the identity, so layers k = 0 and nz-1 of a wall-bounded z keep the identity in z.
+// wface = 1: data on z-faces (w): the wall faces k = -1, nz-1 hold 0, every interior face has both neighbours.
+static void filter_z(const oracle_solver& S, const double* q, double* out, int wface) {
+  int nx = S.nx, ny = S.ny, nz = S.nz;
+#pragma omp parallel for
+  for (int k = 0; k < nz; ++k) for (int j = 0; j < ny; ++j) for (int i = 0; i < nx; ++i) {
+    size_t n = S.id(i, j, k);
+    if (S.P.bc_z == BC_PER) { out[n] = 0.25 * q[S.id(i, j, (k + nz - 1) % nz)] + 0.5 * q[n] + 0.25 * q[S.id(i, j, (k + 1) % nz)]; continue; }
+    if (!wface) {
+      if (k == 0 || k == nz - 1) out[n] = q[n];
+      else out[n] = 0.25 * q[S.id(i, j, k - 1)] + 0.5 * q[n] + 0.25 * q[S.id(i, j, k + 1)];
+    } else {
+      if (k == nz - 1) { out[n] = 0.0; continue; }
+      double lo = (k == 0) ? 0.0 : q[S.id(i, j, k - 1)];
+      double hi = (k == nz - 2) ? 0.0 : q[S.id(i, j, k + 1)];
+      out[n] = 0.25 * lo + 0.5 * q[n] + 0.25 * hi;
+    }
+  }
+}
+// the test filter of the run: x-y (dsm_filter3d = 0) or x-y-z.  kind 0: centred data and u; 1: v (y-faces); 2: w (z-faces)
+static void test_filter(const oracle_solver& S, const double* q, double* out, int kind) {
+  if (!S.P.dsm_filter3d) { if (kind == 1) filter_xy_vface(S, q, out); else filter_xy_centre(S, q, out); return; }
+  std::vector<double> t(S.N);
+  if (kind == 1) filter_xy_vface(S, q, t.data()); else filter_xy_centre(S, q, t.data());
+  filter_z(S, t.data(), out, kind == 2);
+}
+
 // ------------------------------------------------------------------------------------------------
 // Eddy viscosity (O-step 9).  u,v,w ghosted in GH_STRAIN mode by the caller.
 // ------------------------------------------------------------------------------------------------
@@ -688,34 +718,38 @@ static void eddy_viscosity(oracle_solver& S, F3& u, F3& v, F3& w, double* nut) {
   }
   const double* vel[3] = {uc.data(), vc.data(), wc.data()};
   std::vector<double> fvel(3 * N), prod(N), fprod(N);
-  for (int c = 0; c < 3; ++c) filter_xy_centre(S, vel[c], &fvel[c * N]);
+  for (int c = 0; c < 3; ++c) test_filter(S, vel[c], &fvel[c * N], 0);
   const int pa[6] = {0, 1, 2, 0, 0, 1}, pb[6] = {0, 1, 2, 1, 2, 2};   // 11 22 33 12 13 23
   std::vector<double> L(6 * N), M(6 * N);
   for (int c = 0; c < 6; ++c) {   // Eq. 7: L_ij = F(u_i u_j) - F(u_i) F(u_j)
     for (size_t n = 0; n < N; ++n) prod[n] = vel[pa[c]][n] * vel[pb[c]][n];
-    filter_xy_centre(S, prod.data(), fprod.data());
+    test_filter(S, prod.data(), fprod.data(), 0);
     for (size_t n = 0; n < N; ++n) L[c * N + n] = fprod[n] - fvel[pa[c] * N + n] * fvel[pb[c] * N + n];
   }
   // Eq. 9: test-filtered strain from the face-wise filtered velocity, ghosted by the same BC routine
   F3 uf(nx, ny, nz), vf(nx, ny, nz), wf(nx, ny, nz);
   {
     std::vector<double> a(N), b(N);
-    u.to(a.data()); filter_xy_centre(S, a.data(), b.data()); uf.from(b.data());
-    v.to(a.data()); filter_xy_vface(S, a.data(), b.data()); vf.from(b.data());
-    w.to(a.data()); filter_xy_centre(S, a.data(), b.data()); wf.from(b.data());
+    u.to(a.data()); test_filter(S, a.data(), b.data(), 0); uf.from(b.data());
+    v.to(a.data()); test_filter(S, a.data(), b.data(), 1); vf.from(b.data());
+    w.to(a.data()); test_filter(S, a.data(), b.data(), 2); wf.from(b.data());
   }
   bc_velocity(S, uf, vf, wf, GH_STRAIN);
   std::vector<double> St(6 * N), stmag(N);
   strain(S, uf, vf, wf, St.data(), stmag.data());
   for (int c = 0; c < 6; ++c) {   // Eq. 8 (reading S2): M_ij = 2 Delta^2 [F(|S| S_ij) - alpha^2 |S~| S~_ij]
     for (size_t n = 0; n < N; ++n) prod[n] = smag[n] * Sij[c * N + n];
-    filter_xy_centre(S, prod.data(), fprod.data());
+    test_filter(S, prod.data(), fprod.data(), 0);
 #pragma omp parallel for
     for (int k = 0; k < nz; ++k) for (int j = 0; j < ny; ++j) for (int i = 0; i < nx; ++i) {
       size_t n = S.id(i, j, k);
       double d2 = std::pow(dx * dy * S.dzf(k), 2.0 / 3.0);
-      double al = S.alpha2d;
-      if (S.P.bc_y == BC_WALL && (j == 0 || j == ny - 1)) al = std::sqrt(S.alpha2d);   // 1-D (x only) filter there: 2^(1/3)
+      // filter-width ratio: (volume ratio)^(1/3) of the directions actually filtered at this point (PAPER.md:128:
+      // 4^(1/3) for a 2-D filter, 8^(1/3) = 2 for the 3-D one; reading S11: 2^(1/3) where only x is filtered)
+      int nf = 1;
+      if (!(S.P.bc_y == BC_WALL && (j == 0 || j == ny - 1))) ++nf;
+      if (S.P.dsm_filter3d && !(S.P.bc_z == BC_WALL && (k == 0 || k == nz - 1))) ++nf;
+      double al = nf == 2 ? S.alpha2d : (nf == 1 ? std::sqrt(S.alpha2d) : S.alpha2d * std::sqrt(S.alpha2d));
       M[c * N + n] = 2.0 * d2 * (fprod[n] - al * al * stmag[n] * St[c * N + n]);
     }
   }
@@ -992,6 +1026,7 @@ extern "C" int oracle_strain(oracle_solver* S, double* Sij, double* smag) {
   if (!S) return fail("null"); bc_velocity(*S, S->u, S->v, S->w, GH_STRAIN); strain(*S, S->u, S->v, S->w, Sij, smag); return 0;
 }
 extern "C" int oracle_filter_xy(oracle_solver* S, const double* q, double* out) { if (!S) return fail("null"); filter_xy_centre(*S, q, out); return 0; }
+extern "C" int oracle_test_filter(oracle_solver* S, const double* q, double* out, int kind) { if (!S || kind < 0 || kind > 2) return fail("bad argument"); test_filter(*S, q, out, kind); return 0; }
 extern "C" int oracle_get_cs(oracle_solver* S, double* cs) {
   if (!S || !cs) return fail("null"); for (size_t n = 0; n < S->cs.size(); ++n) cs[n] = S->cs[n]; return 0;
 }

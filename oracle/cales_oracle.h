@@ -39,6 +39,7 @@ typedef struct {
   int implicit_z;
   int const_flow_rate; double u_bulk;
   int wall_model_y;        /* log-law wall model on the y walls too (duct WMLES); needs bc_y = wall */
+  int dsm_filter3d;        /* 1: 3-D box test filter (x, y and z) with the first-off-wall-layer rule of PAPER.md:128; 0: x-y filter */
 } oracle_params;
 
 /* ---- 1-D primitives (pinned against numpy/scipy and O(N^2) definitions in tests) ---- */
@@ -85,6 +86,9 @@ int oracle_divergence(oracle_solver* s, double* div);                         /*
 int oracle_strain(oracle_solver* s, double* S, double* smag);
 /* x-y test filter (1/4,1/2,1/4)^2 of a centred field (reading S11) */
 int oracle_filter_xy(oracle_solver* s, const double* q, double* out);
+/* the run's test filter (x-y, or x-y-z with dsm_filter3d) of an interior array; kind 0: centred data and u,
+   1: v (y-faces), 2: w (z-faces) */
+int oracle_test_filter(oracle_solver* s, const double* q, double* out, int kind);
 /* dynamic coefficient of the last eddy-viscosity evaluation: cs[nz] (plane) or cs[nz*ny] (x-line) */
 int oracle_get_cs(oracle_solver* s, double* cs);
 /* L_ij, M_ij (6 x N each, order 11,22,33,12,13,23) of the last dynamic evaluation (Eq. 7-8) */

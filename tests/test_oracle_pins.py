@@ -305,15 +305,16 @@ def test_wall_stress_direction_interpolation_and_flux(oracle):
 
 
 # --------------------------------------------------------------------------------------------- P13
-def np_dsm_periodic(S, u, v, w, alpha2=4.0 ** (2.0 / 3.0)):
-    """Independent dense numpy evaluation of Eq. 5-9 in a triply periodic box (np.roll, 9-point filter)."""
+def np_dsm_periodic(S, u, v, w, alpha2=4.0 ** (2.0 / 3.0), filter3d=False):
+    """Independent dense numpy evaluation of Eq. 5-9 in a triply periodic box (np.roll, 9- or 27-point filter)."""
     dx, dy, dz = S.dx, S.dy, S.dzf[0]
     r = np.roll
     def filt(q):
         out = np.zeros_like(q)
-        for dj, wj in ((-1, .25), (0, .5), (1, .25)):
-            for di, wi in ((-1, .25), (0, .5), (1, .25)):
-                out += wi * wj * r(r(q, -dj, 1), -di, 2)
+        for dk, wk in (((-1, .25), (0, .5), (1, .25)) if filter3d else ((0, 1.0),)):
+            for dj, wj in ((-1, .25), (0, .5), (1, .25)):
+                for di, wi in ((-1, .25), (0, .5), (1, .25)):
+                    out += wi * wj * wk * r(r(r(q, -dk, 0), -dj, 1), -di, 2)
         return out
     def strain(u, v, w):
         s11 = (u - r(u, 1, 2)) / dx; s22 = (v - r(v, 1, 1)) / dy; s33 = (w - r(w, 1, 0)) / dz
@@ -412,6 +413,80 @@ def test_filter_commutes_with_strain_and_extrapolation_identity(oracle):
     assert rel(fq[:, 0], xonly[:, 0]) < 1e-14 and rel(fq[:, -1], xonly[:, -1]) < 1e-14
     ghost = 2 * xonly[:, 0] - xonly[:, 1]
     assert rel(0.25 * ghost + 0.5 * xonly[:, 0] + 0.25 * xonly[:, 1], fq[:, 0]) < 1e-13
+
+
+# ------------------------------------------------------------------------- 3-D box test filter
+def test_dynamic_model_3d_filter_vs_dense_bruteforce(oracle):
+    S = oracle.Oracle(8, 6, 6, 2.0, 3.0, 1.0, bc_y=0, bc_z=0, sgs_model=2, dsm_avg_xy_plane=1, dsm_filter3d=1)
+    u, v, w = random_solenoidal(S, seed=22)
+    nut = S.eddy_viscosity(u, v, w)
+    L, M, cs, nut_ref = np_dsm_periodic(S, u, v, w, alpha2=4.0, filter3d=True)     # alpha = 8^(1/3) = 2
+    Lo, Mo = S.dsm_tensors()
+    assert rel(Lo, L) < 1e-12 and rel(Mo, M) < 1e-12
+    assert rel(S.get_cs(), cs) < 1e-11 and rel(nut, nut_ref) < 1e-11
+    L2, _, _, _ = np_dsm_periodic(S, u, v, w)
+    assert rel(Lo, L2) > 1e-2                          # and it is not the x-y filter
+
+
+def test_dynamic_model_3d_filter_fourier_mode_in_z(oracle):
+    # u = A sin(m z): the x-y filter leaves it unchanged (L = 0); the z part gives L_11 in closed form with the
+    # transfer function T(m) = cos^2(m dz/2) of the (1/4,1/2,1/4) weights
+    nz, m, A = 12, 2, 0.7
+    x3 = oracle.Oracle(8, 6, nz, 2 * PI, 2 * PI, 2 * PI, sgs_model=2, dsm_filter3d=1)
+    z = x3.zc
+    u = A * np.sin(m * z)[:, None, None] * np.ones(x3.shape)
+    x3.eddy_viscosity(u, np.zeros(x3.shape), np.zeros(x3.shape))
+    L, M = x3.dsm_tensors()
+    dz = 2 * PI / nz
+    T = lambda q: math.cos(q * dz / 2) ** 2
+    want = 0.5 * A * A * ((1 - T(m) ** 2) - (T(2 * m) - T(m) ** 2) * np.cos(2 * m * z))
+    assert np.max(np.abs(L[0] - want[:, None, None])) < 1e-13
+    for c in range(1, 6):
+        assert np.max(np.abs(L[c])) < 1e-14
+    x2 = oracle.Oracle(8, 6, nz, 2 * PI, 2 * PI, 2 * PI, sgs_model=2)
+    x2.eddy_viscosity(u, np.zeros(x2.shape), np.zeros(x2.shape))
+    assert np.max(np.abs(x2.dsm_tensors()[0])) < 1e-14
+
+
+def test_3d_filter_first_layer_rule_and_filter_ratio(oracle):
+    # in the first off-wall layer the 3-D filter degenerates to the 2-D one (linear extrapolation to the
+    # ghost, then the symmetric filter = identity in z) and alpha = 4^(1/3) there, 8^(1/3) = 2 elsewhere
+    W = make(oracle, 12, 8, 10, (0, 1), False, sgs_model=2, dsm_filter3d=1)
+    q = np.random.default_rng(1).standard_normal(W.shape)
+    xy = W.filter_xy(q)
+    f = W.test_filter(q, 0)
+    assert rel(f[0], xy[0]) < 1e-15 and rel(f[-1], xy[-1]) < 1e-15
+    assert rel(f[1:-1], 0.25 * xy[:-2] + 0.5 * xy[1:-1] + 0.25 * xy[2:]) < 1e-14
+    ghost = 2 * xy[0] - xy[1]
+    assert rel(0.25 * ghost + 0.5 * xy[0] + 0.25 * xy[1], f[0]) < 1e-13
+    # w lives on z faces: wall faces (k = -1, nz-1) are 0, every interior face sees both neighbours
+    fw = W.test_filter(q, 2)
+    assert np.max(np.abs(fw[-1])) == 0.0
+    assert rel(fw[0], 0.5 * xy[0] + 0.25 * xy[1]) < 1e-14 and rel(fw[-2], 0.25 * xy[-3] + 0.5 * xy[-2]) < 1e-14
+    assert rel(fw[1:-2], 0.25 * xy[:-3] + 0.5 * xy[1:-2] + 0.25 * xy[2:-1]) < 1e-14
+    # a constant is preserved, the 2-dz wave is annihilated away from the walls
+    assert rel(W.test_filter(np.ones(W.shape), 0), np.ones(W.shape)) < 1e-15
+    saw = ((-1.0) ** np.arange(10))[:, None, None] * np.ones(W.shape)
+    assert np.max(np.abs(W.test_filter(saw, 0)[1:-1])) < 1e-15
+    # filter-width ratio: M_ij = A_ij - alpha^2 B_ij is affine in alpha^2 (Eq. 8); with dsm_alpha2d = a the ratio is
+    # a^(n/2), n = number of directions filtered at the point.  A = 2 Delta^2 F(|S| S_ij) from the pinned strain and
+    # filter, B from the run with a = 1; then the default run must give alpha^2 = 4 inside, 4^(2/3) in the first layer
+    D = make(oracle, 12, 8, 10, (1, 1), False, sgs_model=2, dsm_filter3d=1, dsm_avg_xy_plane=0)
+    u, v, w = random_solenoidal(D, seed=5)
+    D.eddy_viscosity(u, v, w)
+    _, M = D.dsm_tensors()
+    Sij, mag = D.strain()
+    d2 = (D.dx * D.dy * D.dzf) ** (2.0 / 3.0)
+    A = np.array([2 * d2[:, None, None] * D.test_filter(mag * Sij[c], 0) for c in range(6)])
+    D1 = make(oracle, 12, 8, 10, (1, 1), False, sgs_model=2, dsm_filter3d=1, dsm_avg_xy_plane=0, dsm_alpha2d=1.0)
+    D1.eddy_viscosity(u, v, w)
+    B = A - D1.dsm_tensors()[1]
+    nf = np.full(D.shape, 3)
+    nf[[0, -1]] -= 1; nf[:, [0, -1]] -= 1
+    a2 = (4.0 ** (1.0 / 3.0)) ** nf
+    assert a2[3, 3, 0] == pytest.approx(4.0) and a2[0, 3, 0] == pytest.approx(4.0 ** (2.0 / 3.0)) and a2[0, 0, 0] == pytest.approx(4.0 ** (1.0 / 3.0))
+    assert rel(M, A - a2[None] * B) < 1e-12
+    assert np.max(np.abs(B)) > 1e-3
 
 
 # --------------------------------------------------------------------------------------------- P6
