@@ -36,6 +36,7 @@ L2_BYTES = 126 * 1024 * 1024
 ALGO_BYTES = {
     "k_rhs": 96.0, "k_cn_z": 48.0, "k_fft_x_fwd": 32.0, "k_fft_y_fwd": 16.0, "k_poisson_z": 16.0, "k_fft_y_inv": 16.0,
     "k_fft_x_inv": 16.0, "k_correct": 72.0, "k_smag": 32.0, "k_dsm_col": 32.0, "k_dsm_nut": 16.0, "k_fill": 8.0,
+    "k_dsm3_pass1": 32.0,
 }
 
 
@@ -104,7 +105,7 @@ class ClockSampler:
 REPLICA = {1: None, 2: None, 3: (128, 128, 96), 4: (256, 64, 64), 5: (192, 128, 64)}   # bounded oracle samples
 
 
-def oracle_leg(cfg_no, steps, warmup):
+def oracle_leg(cfg_no, steps, warmup, overrides=None):
     """Time the CPU oracle as it stands (never tuned for this) on a bounded replica of config cfg_no's option set."""
     import numpy as np
     import oracle
@@ -113,6 +114,7 @@ def oracle_leg(cfg_no, steps, warmup):
     cfg = inputs.config(cfg_no, shape)
     u, v, w, ub = inputs.initial_fields(cfg)
     kw = inputs.solver_kwargs(cfg, ub)
+    kw.update(overrides or {})
     g = {k: kw.pop(k) for k in ("nx", "ny", "nz", "lx", "ly", "lz")}
     o = oracle.Oracle(g["nx"], g["ny"], g["nz"], g["lx"], g["ly"], g["lz"], **kw)
     o.set_velocity(u, v, w); o.project()
@@ -139,7 +141,7 @@ def run_reference(args):
     steps, warmup = args.steps, args.warmup
     if REPLICA[cfg_no] is not None:            # keep the whole run within a few minutes on a small host
         steps, warmup = min(steps, 5), min(warmup, 1)
-    r = oracle_leg(cfg_no, steps, warmup)
+    r = oracle_leg(cfg_no, steps, warmup, {"dsm_filter3d": 1} if args.dsm_filter3d else None)
     line = {"impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
             "warmup": warmup, "ms_per_step": r["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic", "config": {"workload": r["workload"], "sample": r["sample"]},
@@ -213,6 +215,11 @@ def run_ours(args):
     u, v, w, ub = inputs.initial_fields(cfg)
     dt = inputs.time_step(cfg, u, v, w)
     kw = inputs.solver_kwargs(cfg, ub)
+    if args.dsm_filter3d:
+        if kw["sgs_model"] != 2:
+            raise SystemExit("--dsm-filter3d needs a dynamic-model workload (config 4 or 5)")
+        kw["dsm_filter3d"] = 1
+        cfg["name"] += " + 3-D box test filter"
     g = {k: kw.pop(k) for k in ("nx", "ny", "nz", "lx", "ly", "lz")}
     npts = g["nx"] * g["ny"] * g["nz"]
     p_host = np.zeros_like(u)
@@ -345,7 +352,7 @@ def run_ours(args):
         dist.destroy_process_group()
     if rank == 0:
         if not args.no_cpu_baseline and world == 1:
-            r = oracle_leg(cfg_no, 2, 1)
+            r = oracle_leg(cfg_no, 2, 1, {"dsm_filter3d": 1} if args.dsm_filter3d else None)
             line["cpu_baseline"] = {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")}
         if not args.no_other_configs and world == 1:
             # north_star: all five workloads at 1 GPU.  The other four run as short child processes of this same script
@@ -382,6 +389,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-other-configs", action="store_true", help="skip the short side runs of the other four workloads")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg")
+    ap.add_argument("--dsm-filter3d", action="store_true", help="configs 4, 5 with the 3-D box test filter of PAPER.md:128 (SURVEY.md 8(f) item 2); "
+                    "not a BASELINE.json workload: the line is labelled and is for the widening table of DESIGN.md only")
     args = ap.parse_args()
     if args.impl == "reference":
         if not args.config:

@@ -70,6 +70,8 @@ typedef struct {
   void* cuda_stream;         /* cudaStream_t of the caller */
   int device;                /* CUDA device ordinal the workspace lives on */
   int wall_model_y;          /* log-law wall model on the y walls too (duct WMLES); needs bc_y = wall */
+  int dsm_filter3d;          /* dynamic model: 1 = 3-D box test filter (x, y, z; identity in z and alpha = 4^(1/3) in the first
+                                off-wall layer, alpha = 2 elsewhere); 0 = x-y filter */
 } cales_params;
 
 typedef struct {

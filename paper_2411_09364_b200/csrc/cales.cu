@@ -12,6 +12,7 @@
 #include "cales_rhs_tile.cuh"
 #include "cales_closures.cuh"
 #include "cales_smag_tile.cuh"
+#include "cales_dsm3.cuh"
 #include "cales_host.h"
 
 #include <cmath>
@@ -111,10 +112,10 @@ extern "C" size_t cales_workspace_bytes(const cales_params* p) {
 
 // Kernel ids for the per-kernel timing table (cales_kernel_time).
 enum { K_RHS = 0, K_CN_COEF, K_CN_Z, K_SUM, K_BULK, K_FFTX_FWD, K_FFTY_FWD, K_POISSON_Z, K_FFTY_INV, K_FFTX_INV, K_CORRECT,
-       K_WALL, K_SMAG, K_DSM_PASS1, K_DSM_COL, K_DSM_COEF, K_DSM_NUT, K_FILL, K_TRANSPOSE, K_DIAG, K_COUNT };
+       K_WALL, K_SMAG, K_DSM_PASS1, K_DSM_COL, K_DSM_COEF, K_DSM_NUT, K_FILL, K_TRANSPOSE, K_DIAG, K_DSM3, K_COUNT };
 static const char* const k_names[K_COUNT] = {"k_rhs", "k_cn_coef", "k_cn_z", "k_sum_stage1", "k_bulk_finish", "k_fft_x_fwd", "k_fft_y_fwd",
   "k_poisson_z", "k_fft_y_inv", "k_fft_x_inv", "k_correct", "k_wall_stress", "k_smag", "k_dsm_pass1", "k_dsm_col", "k_dsm_coef", "k_dsm_nut", "k_fill",
-  "k_transpose_xy", "k_diag"};
+  "k_transpose_xy", "k_diag", "k_dsm3_pass1"};
 
 // record an event on the stream tagged with the kernel that just finished (kid < 0: a separator)
 static void tick(cales_solver* s, int kid) {
@@ -186,6 +187,7 @@ extern "C" int cales_create(const cales_params* p, cales_solver** out) {
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rhs_tile, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(RT_SMEM_DOUBLES * sizeof(double)));
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_smag_tile, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(ST_SMEM_DOUBLES * sizeof(double)));
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dsm_pass1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(DSM_SMEM_DOUBLES * sizeof(double)));
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dsm3_pass1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(D3_SMEM_DOUBLES * sizeof(double)));
   if (e != cudaSuccess) { delete s; return fail(CALES_ECUDA, std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e)); }
   s->pblock = dim3(32, 8, 1);
   s->pgrid = dim3((nx + 31) / 32, (ny + 7) / 8, nz);
@@ -319,12 +321,15 @@ static int run_eddy_viscosity(cales_solver* s, const double* u, const double* v,
     const bool split = ywall && c.ny >= 3 * DSM_TY;
     const size_t tile_smem = DSM_SMEM_DOUBLES * sizeof(double);
     const unsigned ntile = (unsigned)((c.nx + DSM_TX - 1) / DSM_TX);
-    if (ywall) {
+    if (c.dsm_filter3d) {   // 3-D box filter: Eq. 9 literally on 3x3x3 patches, every row
+      k_dsm3_pass1<<<dim3((c.nx + D3_TX - 1) / D3_TX, (c.ny + D3_TY - 1) / D3_TY, c.nz), dim3(D3_TX, D3_TY), D3_SMEM_DOUBLES * sizeof(double), s->st>>>(c, u, v, w, ds.pslots, s->smag, s->dsm_part);
+      LAUNCH_TRY(K_DSM3);
+    } else if (ywall) {
       if (split) k_dsm_pass1<<<dim3(ntile, 2, c.nz), dim3(DSM_TX, DSM_TY), tile_smem, s->st>>>(c, u, v, w, c.ny - DSM_TY, DSM_TY, c.ny - DSM_TY, ds.pslots, s->smag, s->dsm_part);
       else k_dsm_pass1<<<dim3(ntile, (c.ny + DSM_TY - 1) / DSM_TY, c.nz), dim3(DSM_TX, DSM_TY), tile_smem, s->st>>>(c, u, v, w, DSM_TY, c.ny, c.ny, ds.pslots, s->smag, s->dsm_part);
       LAUNCH_TRY(K_DSM_PASS1);
     }
-    if (!ywall || split) {
+    if (!c.dsm_filter3d && (!ywall || split)) {
       const int jlo = ywall ? DSM_TY : 0, jhi = ywall ? c.ny - DSM_TY : c.ny;
       dim3 grid(ds.nbx, (jhi - jlo + DSMC_LY - 1) / DSMC_LY, c.nz);
       // <threads, min CTAs/SM, quantities with a register window>: measured on B200, (64, 6, 0) within 4 % of the best
@@ -452,7 +457,7 @@ extern "C" int cales_launches_per_step(cales_solver* s) {
             1 /*static nu_t or fill*/;
   if (c.sgs == CALES_SGS_DSMAG) {
     const bool ywall = c.bc_y == BC_WALL, split = ywall && c.ny >= 3 * DSM_TY;
-    per += -1 + (ywall ? 1 : 0) + ((!ywall || split) ? 1 : 0) + 2;   // pass 1 (tile and/or column kernel), coefficient, nu_t
+    per += -1 + (c.dsm_filter3d ? 1 : (ywall ? 1 : 0) + ((!ywall || split) ? 1 : 0)) + 2;   // pass 1 (tile and/or column kernel), coefficient, nu_t
   }
   return 3 * per;
 }

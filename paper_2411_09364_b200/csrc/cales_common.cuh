@@ -18,7 +18,7 @@ enum { GH_VISC = 0, GH_STRAIN = 1 };  // ghost of the wall-parallel velocity at 
 // Grid, options and table pointers, passed by value to every kernel.
 struct Ctx {
   int nx, ny, nz;
-  int bc_y, bc_z, wall_model, wall_model_y, sgs, van_driest, implicit_z, dsm_plane, dsm_clip_total, const_flow_rate;
+  int bc_y, bc_z, wall_model, wall_model_y, sgs, van_driest, implicit_z, dsm_plane, dsm_clip_total, dsm_filter3d, const_flow_rate;
   int wm_maxit;
   long long N;     // nx*ny*nz
   long long nxy;   // nx*ny

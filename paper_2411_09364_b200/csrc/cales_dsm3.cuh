@@ -1,0 +1,199 @@
+// cales_dsm3.cuh -- dynamic Smagorinsky, pass 1, with the 3-D box test filter.
+// The filter is separable (1/4,1/2,1/4) in x, y and z ("assumes uniform grid spacing").  In the first
+// off-wall layer of a wall-bounded direction that direction keeps the identity (the paper's "linear extrapolation to the
+// ghost points, followed by the 3D filter") and the filter-width ratio is the cube root of the volume ratio of the
+// directions actually filtered: 8^(1/3) = 2 inside, 4^(1/3) in the first layer, 2^(1/3) in a duct corner.
+//
+// One CTA = one D3_TX x D3_TY tile of one k-plane.  Shared memory holds
+//   raw : u, v, w on planes k-2 .. k+2 over the tile + halo 2 (ghosts by velg, GH_STRAIN mode),
+//   flt : the face-wise test-filtered velocity on planes k-1, k, k+1 over the tile + halo 1 (Eq. 9 takes its strain);
+//         its ghosts are the boundary condition applied to the FILTERED field (S24), z before y (S25),
+//   mid : centre velocities, |S| S_ij and |S| on planes k-1, k, k+1 over the tile + halo 1 (the filter reads 3x3x3).
+// Eq. 9 is evaluated literally (strain of the filtered velocity), so the kernel is valid next to walls in y and z.
+#pragma once
+#include "cales_common.cuh"
+#include "cales_closures.cuh"
+
+namespace cales {
+
+enum { D3_TX = 32, D3_TY = 8, D3_RX = D3_TX + 4, D3_RY = D3_TY + 4, D3_MX = D3_TX + 2, D3_MY = D3_TY + 2 };
+enum { D3_RAW = 15 * D3_RX * D3_RY, D3_FLT = 9 * D3_MX * D3_MY, D3_MID = 30 * D3_MX * D3_MY,
+       D3_SMEM_DOUBLES = D3_RAW + D3_FLT + D3_MID };
+
+CALES_HD int d3_raw_off(int comp, int pl /* 0..4 <-> plane k-2+pl */, int ry, int rx) { return ((comp * 5 + pl) * D3_RY + ry) * D3_RX + rx; }
+CALES_HD int d3_flt_off(int comp, int pl /* 0..2 <-> plane k-1+pl */, int my, int mx) { return ((comp * 3 + pl) * D3_MY + my) * D3_MX + mx; }
+CALES_HD int d3_mid_off(int q, int pl /* 0..2 <-> plane k-1+pl */, int my, int mx) { return ((q * 3 + pl) * D3_MY + my) * D3_MX + mx; }
+
+// z weights of the test filter for plane gk.  kind 0: data centred in z (u, v, centre quantities); 1: w faces.
+CALES_HD void d3_wz(const Ctx& c, int gk, int kind, double* wz) {
+  wz[0] = 0.25; wz[1] = 0.5; wz[2] = 0.25;
+  if (c.bc_z == BC_WALL) {
+    if (kind == 0) { if (gk <= 0 || gk >= c.nz - 1) { wz[0] = 0.0; wz[1] = 1.0; wz[2] = 0.0; } }
+    else { if (gk < 0 || gk >= c.nz - 1) { wz[0] = 0.0; wz[1] = 0.0; wz[2] = 0.0; } }
+  }
+}
+
+// phase 1: the raw tile, 3 components x 5 planes
+CALES_HD void d3_load(int tid, int nth, const Ctx& c, const double* u, const double* v, const double* w, int i0, int j0, int k, double* raw) {
+  const int per = D3_RX * D3_RY;
+  for (int idx = tid; idx < 15 * per; idx += nth) {
+    const int cp = idx / per, r = idx % per;
+    const int comp = cp / 5, pl = cp % 5, ry = r / D3_RX, rx = r % D3_RX;
+    const int gi = i0 - 2 + rx, gj = j0 - 2 + ry;
+    int gk = k - 2 + pl;
+    double val = 0.0;
+    bool ok = gi <= c.nx + 1 && gj <= c.ny + 1;
+    if (c.bc_z == BC_PER) gk = wrapi(gk, c.nz);
+    else if (gk < -1 || gk > c.nz) ok = false;            // beyond the ghost layer: never read with a non-zero weight
+    if (ok) {
+      if (comp == 0) val = velg<0>(c, u, gi, gj, gk, GH_STRAIN);
+      else if (comp == 1) val = velg<1>(c, v, gi, gj, gk, GH_STRAIN);
+      else val = velg<2>(c, w, gi, gj, gk, GH_STRAIN);
+    }
+    raw[idx] = val;
+  }
+}
+
+// phase 2: filtered face velocities (3 components x 3 planes) and the centre quantities on the mid region
+CALES_HD void d3_mid(int tid, int nth, const Ctx& c, int i0, int j0, int k, const double* raw, double* flt, double* mid) {
+  const int per = D3_MX * D3_MY;
+  for (int idx = tid; idx < 9 * per; idx += nth) {
+    const int cp = idx / per, r = idx % per;
+    const int comp = cp / 3, pl = cp % 3, my = r / D3_MX, mx = r % D3_MX;
+    const int gj = j0 - 1 + my, gk = k - 1 + pl;
+    // 3-D filtered face value on raw plane index p (global plane k-2+p, interior or periodic), mid row m
+    auto f0 = [&](int p, int m) {
+      double wz[3]; d3_wz(c, k - 2 + p, comp == 2 ? 1 : 0, wz);
+      double wy[3]; dsm_wy(c, j0 - 1 + m, comp == 1 ? 1 : 0, wy);
+      double s = 0.0;
+      for (int d = 0; d < 3; ++d) {
+        if (wz[d] == 0.0) continue;
+        double t = 0.0;
+        for (int b = 0; b < 3; ++b) {
+          const double* row = raw + d3_raw_off(comp, p - 1 + d, m + b, mx);
+          t += wy[b] * (0.25 * row[0] + 0.5 * row[1] + 0.25 * row[2]);
+        }
+        s += wz[d] * t;
+      }
+      return s;
+    };
+    // plane gk including the z ghosts of the filtered field: w = 0 on and beyond the wall faces; u, v no-slip mirror
+    // or, at a wall-model wall, the one-sided extrapolation of the first two filtered layers (as velg_z, GH_STRAIN)
+    auto fz = [&](int m) {
+      if (c.bc_z == BC_PER || (gk >= 0 && gk < c.nz)) return f0(pl + 1, m);
+      if (comp == 2) return 0.0;
+      const bool bottom = gk < 0;
+      const double q0 = f0(bottom ? pl + 2 : pl, m);
+      if (!c.wall_model) return -q0;
+      const double q1 = f0(bottom ? pl + 3 : pl - 1, m);
+      const double rr = bottom ? c.dzc[-1] / c.dzc[0] : c.dzc[c.nz - 1] / c.dzc[c.nz - 2];
+      return q0 + (q0 - q1) * rr;
+    };
+    // y ghost rows of the filtered u, w at a wall-model y wall: the same rule in y (after z)
+    if (c.bc_y == BC_WALL && c.wall_model_y && comp != 1 && (gj < 0 || gj >= c.ny))
+      flt[idx] = gj < 0 ? 2.0 * fz(my + 1) - fz(my + 2) : 2.0 * fz(my - 1) - fz(my - 2);
+    else flt[idx] = fz(my);
+  }
+  double wzc[3]; d3_wz(c, k, 0, wzc);
+  const double rdx = c.rdx, rdy = c.rdy;
+  for (int idx = tid; idx < 3 * per; idx += nth) {
+    const int pl = idx / per, r = idx % per, my = r / D3_MX, mx = r % D3_MX;
+    if (wzc[pl] == 0.0) {                                  // plane outside the filter stencil (first off-wall layer)
+      for (int q = 0; q < 10; ++q) mid[d3_mid_off(q, pl, my, mx)] = 0.0;
+      continue;
+    }
+    const int kk = c.bc_z == BC_PER ? wrapi(k - 1 + pl, c.nz) : k - 1 + pl;
+    auto U = [&](int a, int b, int d) { return raw[d3_raw_off(0, 1 + pl + d, my + 1 + b, mx + 1 + a)]; };
+    auto V = [&](int a, int b, int d) { return raw[d3_raw_off(1, 1 + pl + d, my + 1 + b, mx + 1 + a)]; };
+    auto W = [&](int a, int b, int d) { return raw[d3_raw_off(2, 1 + pl + d, my + 1 + b, mx + 1 + a)]; };
+    double S[6];
+    const double smag = strain_at(U, V, W, rdx, rdy, c.rdzf[kk], c.rdzc[kk], c.rdzc[kk - 1], S);
+    mid[d3_mid_off(0, pl, my, mx)] = 0.5 * (U(-1, 0, 0) + U(0, 0, 0));
+    mid[d3_mid_off(1, pl, my, mx)] = 0.5 * (V(0, -1, 0) + V(0, 0, 0));
+    mid[d3_mid_off(2, pl, my, mx)] = 0.5 * (W(0, 0, -1) + W(0, 0, 0));
+    for (int q = 0; q < 6; ++q) mid[d3_mid_off(3 + q, pl, my, mx)] = smag * S[q];
+    mid[d3_mid_off(9, pl, my, mx)] = smag;
+  }
+}
+
+// phase 3: one output point (tx, ty); L:M and M:M through lm, mm and |S| through smag_out
+CALES_HD void d3_point(const Ctx& c, int j0, int k, int tx, int ty, const double* flt, const double* mid, double* lm, double* mm, double* smag_out) {
+  const int gj = j0 + ty;
+  const int mx = tx + 1, my = ty + 1;
+  double wy[3]; dsm_wy(c, gj, 0, wy);
+  double wz[3]; d3_wz(c, k, 0, wz);
+  const double wx[3] = {0.25, 0.5, 0.25};
+  double Fv[3] = {0, 0, 0}, Fp[6] = {0, 0, 0, 0, 0, 0}, Fs[6] = {0, 0, 0, 0, 0, 0};
+  const int st = 3 * D3_MX * D3_MY;                        // stride between quantities
+  for (int d = 0; d < 3; ++d) {
+    if (wz[d] == 0.0) continue;
+#pragma unroll
+    for (int b = 0; b < 3; ++b) {
+#pragma unroll
+      for (int a = 0; a < 3; ++a) {
+        const double wgt = wz[d] * (wy[b] * wx[a]);
+        const int o = d3_mid_off(0, d, my - 1 + b, mx - 1 + a);
+        const double uc = mid[o], vc = mid[o + st], wc = mid[o + 2 * st];
+        Fv[0] += wgt * uc; Fv[1] += wgt * vc; Fv[2] += wgt * wc;
+        Fp[0] += wgt * (uc * uc); Fp[1] += wgt * (vc * vc); Fp[2] += wgt * (wc * wc);
+        Fp[3] += wgt * (uc * vc); Fp[4] += wgt * (uc * wc); Fp[5] += wgt * (vc * wc);
+#pragma unroll
+        for (int q = 0; q < 6; ++q) Fs[q] += wgt * mid[o + (3 + q) * st];
+      }
+    }
+  }
+  double L[6];
+  L[0] = Fp[0] - Fv[0] * Fv[0]; L[1] = Fp[1] - Fv[1] * Fv[1]; L[2] = Fp[2] - Fv[2] * Fv[2];
+  L[3] = Fp[3] - Fv[0] * Fv[1]; L[4] = Fp[4] - Fv[0] * Fv[2]; L[5] = Fp[5] - Fv[1] * Fv[2];
+  // Eq. 9: strain of the test-filtered velocity
+  auto U = [&](int a, int b, int d) { return flt[d3_flt_off(0, 1 + d, my + b, mx + a)]; };
+  auto V = [&](int a, int b, int d) { return flt[d3_flt_off(1, 1 + d, my + b, mx + a)]; };
+  auto W = [&](int a, int b, int d) { return flt[d3_flt_off(2, 1 + d, my + b, mx + a)]; };
+  double St[6];
+  const double stmag = strain_at(U, V, W, c.rdx, c.rdy, c.rdzf[k], c.rdzc[k], c.rdzc[k - 1], St);
+  const double d2 = c.delta[k] * c.delta[k];
+  int nf = 1;                                               // directions filtered at this point
+  if (!(c.bc_y == BC_WALL && (gj == 0 || gj == c.ny - 1))) ++nf;
+  if (!(c.bc_z == BC_WALL && (k == 0 || k == c.nz - 1))) ++nf;
+  const double al = nf == 2 ? c.alpha : (nf == 1 ? sqrt(c.alpha) : c.alpha * sqrt(c.alpha));
+  double ll = 0.0, m2 = 0.0;
+#pragma unroll
+  for (int q = 0; q < 6; ++q) {
+    const double M = 2.0 * d2 * (Fs[q] - al * al * stmag * St[q]);
+    const double f = q < 3 ? 1.0 : 2.0;
+    ll += f * L[q] * M; m2 += f * M * M;
+  }
+  *lm = ll; *mm = m2; *smag_out = mid[d3_mid_off(9, 1, my, mx)];
+}
+
+#ifdef __CUDACC__
+// grid (ceil(nx/D3_TX), ceil(ny/D3_TY), nz), block (D3_TX, D3_TY), dynamic smem D3_SMEM_DOUBLES*8.
+// part: [k][j][pslots][2]; this kernel fills slot blockIdx.x of every row (the other slots stay 0).
+__global__ void __launch_bounds__(D3_TX * D3_TY) k_dsm3_pass1(const __grid_constant__ Ctx c, const double* __restrict__ u, const double* __restrict__ v,
+                                                               const double* __restrict__ w, int pslots, double* __restrict__ smag, double* __restrict__ part) {
+  extern __shared__ double d3_sm[];
+  double* raw = d3_sm; double* flt = raw + D3_RAW; double* mid = flt + D3_FLT;
+  const int tid = threadIdx.x + D3_TX * threadIdx.y, nth = D3_TX * D3_TY;
+  const int i0 = blockIdx.x * D3_TX, j0 = blockIdx.y * D3_TY, k = blockIdx.z;
+  d3_load(tid, nth, c, u, v, w, i0, j0, k, raw);
+  __syncthreads();
+  d3_mid(tid, nth, c, i0, j0, k, raw, flt, mid);
+  __syncthreads();
+  const int i = i0 + threadIdx.x, j = j0 + threadIdx.y;
+  double lm = 0.0, mm = 0.0;
+  if (i < c.nx && j < c.ny) {
+    double sm;
+    d3_point(c, j0, k, threadIdx.x, threadIdx.y, flt, mid, &lm, &mm, &sm);
+    smag[idx3(c, i, j, k)] = sm;
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) { lm += __shfl_down_sync(0xffffffffu, lm, o); mm += __shfl_down_sync(0xffffffffu, mm, o); }
+  if (threadIdx.x == 0 && j < c.ny) {
+    const long long row = (long long)k * c.ny + j;
+    part[(row * pslots + blockIdx.x) * 2] = lm;
+    part[(row * pslots + blockIdx.x) * 2 + 1] = mm;
+  }
+}
+#endif
+
+}  // namespace cales

@@ -12,6 +12,7 @@
 #include "../../paper_2411_09364_b200/csrc/cales_momentum.cuh"
 #include "../../paper_2411_09364_b200/csrc/cales_rhs_tile.cuh"
 #include "../../paper_2411_09364_b200/csrc/cales_smag_tile.cuh"
+#include "../../paper_2411_09364_b200/csrc/cales_dsm3.cuh"
 
 #include <cstring>
 #include <vector>
@@ -184,7 +185,31 @@ static void emu_nut(emu_solver* s, const double* u, const double* v, const doubl
   const int ntx = dsh.pslots;
   const bool ywall = c.bc_y == BC_WALL, split = ywall && c.ny >= 3 * DSM_TY;
   std::fill(s->dsm_part.begin(), s->dsm_part.end(), 0.0);
-  if (ywall) {   // tile kernel: all rows, or the DSM_TY rows next to each y wall
+  if (c.dsm_filter3d) {   // k_dsm3_pass1: phases separated by the block barrier
+    const int ntile = (c.nx + D3_TX - 1) / D3_TX, nth = D3_TX * D3_TY;
+    std::vector<double> sm(D3_SMEM_DOUBLES);
+    double* raw = sm.data(); double* flt = raw + D3_RAW; double* mid = flt + D3_FLT;
+    for (int k = 0; k < c.nz; ++k) for (int by = 0; by * D3_TY < c.ny; ++by) for (int bx = 0; bx < ntile; ++bx) {
+      const int i0 = bx * D3_TX, j0 = by * D3_TY;
+      for (int tid = 0; tid < nth; ++tid) d3_load(tid, nth, c, u, v, w, i0, j0, k, raw);
+      for (int tid = 0; tid < nth; ++tid) d3_mid(tid, nth, c, i0, j0, k, raw, flt, mid);
+      for (int ty = 0; ty < D3_TY; ++ty) {
+        const int j = j0 + ty;
+        if (j >= c.ny) continue;
+        double lm = 0.0, mm = 0.0;
+        for (int tx = 0; tx < D3_TX; ++tx) {
+          const int i = i0 + tx;
+          if (i < c.nx) {
+            double a, b, sg;
+            d3_point(c, j0, k, tx, ty, flt, mid, &a, &b, &sg);
+            s->smag[idx3(c, i, j, k)] = sg; lm += a; mm += b;
+          }
+        }
+        const long long row = (long long)k * c.ny + j;
+        s->dsm_part[(row * ntx + bx) * 2] = lm; s->dsm_part[(row * ntx + bx) * 2 + 1] = mm;
+      }
+    }
+  } else if (ywall) {   // tile kernel: all rows, or the DSM_TY rows next to each y wall
     const int ntile = (c.nx + DSM_TX - 1) / DSM_TX, nth = DSM_TX * DSM_TY;
     const int nby = split ? 2 : (c.ny + DSM_TY - 1) / DSM_TY, jstride = split ? c.ny - DSM_TY : DSM_TY;
     const int row_hi = split ? DSM_TY : c.ny, row_lo2 = split ? c.ny - DSM_TY : c.ny;
@@ -212,7 +237,7 @@ static void emu_nut(emu_solver* s, const double* u, const double* v, const doubl
       }
     }
   }
-  if (!ywall || split) {   // column-marching kernel, stepped row by row with the block barrier between the phases
+  if (!c.dsm_filter3d && (!ywall || split)) {   // column-marching kernel, stepped row by row with the block barrier between the phases
     const int T = dsh.txb, jlo = ywall ? DSM_TY : 0, jhi = ywall ? c.ny - DSM_TY : c.ny;
     std::vector<double> sh(2 * DSMC_NB * T), breg((size_t)T * DSMC_NB);
     std::vector<double> ring(2 * DSMC_NQ * T), smprev(T);

@@ -93,6 +93,17 @@ def _fuzz_cases():
                   wall_model=wm, h_wm=float(rng.choice([0.0, 0.12])) if wm else 0.0, implicit_z=imp,
                   const_flow_rate=int(rng.integers(0, 2)), u_bulk=1.0)
         out.append((t, nx, ny, nz, kw))
+    rng = np.random.default_rng(20241128)           # dynamic model with the 3-D box test filter
+    for t in range(14, 22):
+        bc_z = int(rng.integers(0, 2)); bc_y = int(rng.integers(0, 2)) if bc_z else 0
+        nx, ny = int(rng.choice(sizes_xy)), int(rng.choice(sizes_xy)); nz = int(rng.integers(4, 14))
+        stretch = int(bc_z and rng.integers(0, 2))
+        wm = int(bc_z and rng.integers(0, 2))
+        kw = dict(bc_y=bc_y, bc_z=bc_z, zstretch=stretch, zstretch_factor=1.3 if stretch else 0.0, nu=float(rng.uniform(1e-3, 2e-2)),
+                  sgs_model=2, dsm_filter3d=1, dsm_avg_xy_plane=int(rng.integers(0, 2)), dsm_clip_total=int(rng.integers(0, 2)),
+                  wall_model=wm, wall_model_y=int(bc_y and rng.integers(0, 2)), h_wm=0.0, implicit_z=int(bc_z and rng.integers(0, 2)),
+                  const_flow_rate=int(rng.integers(0, 2)), u_bulk=1.0)
+        out.append((t, nx, ny, nz, kw))
     return out
 
 
