@@ -112,10 +112,10 @@ extern "C" size_t cales_workspace_bytes(const cales_params* p) {
 
 // Kernel ids for the per-kernel timing table (cales_kernel_time).
 enum { K_RHS = 0, K_CN_COEF, K_CN_Z, K_SUM, K_BULK, K_FFTX_FWD, K_FFTY_FWD, K_POISSON_Z, K_FFTY_INV, K_FFTX_INV, K_CORRECT,
-       K_WALL, K_SMAG, K_DSM_PASS1, K_DSM_COL, K_DSM_COEF, K_DSM_NUT, K_FILL, K_TRANSPOSE, K_DIAG, K_DSM3, K_COUNT };
+       K_WALL, K_SMAG, K_DSM_PASS1, K_DSM_COL, K_DSM_COEF, K_DSM_NUT, K_FILL, K_TRANSPOSE, K_DIAG, K_DSM3, K_DSM3_COL, K_COUNT };
 static const char* const k_names[K_COUNT] = {"k_rhs", "k_cn_coef", "k_cn_z", "k_sum_stage1", "k_bulk_finish", "k_fft_x_fwd", "k_fft_y_fwd",
   "k_poisson_z", "k_fft_y_inv", "k_fft_x_inv", "k_correct", "k_wall_stress", "k_smag", "k_dsm_pass1", "k_dsm_col", "k_dsm_coef", "k_dsm_nut", "k_fill",
-  "k_transpose_xy", "k_diag", "k_dsm3_pass1"};
+  "k_transpose_xy", "k_diag", "k_dsm3_pass1", "k_dsm3_col"};
 
 // record an event on the stream tagged with the kernel that just finished (kid < 0: a separator)
 static void tick(cales_solver* s, int kid) {
@@ -322,8 +322,27 @@ static int run_eddy_viscosity(cales_solver* s, const double* u, const double* v,
     const size_t tile_smem = DSM_SMEM_DOUBLES * sizeof(double);
     const unsigned ntile = (unsigned)((c.nx + DSM_TX - 1) / DSM_TX);
     if (c.dsm_filter3d) {   // 3-D box filter: Eq. 9 literally on 3x3x3 patches, every row
-      k_dsm3_pass1<<<dim3((c.nx + D3_TX - 1) / D3_TX, (c.ny + D3_TY - 1) / D3_TY, c.nz), dim3(D3_TX, D3_TY), D3_SMEM_DOUBLES * sizeof(double), s->st>>>(c, u, v, w, ds.pslots, s->smag, s->dsm_part);
-      LAUNCH_TRY(K_DSM3);
+      // column-marching kernel where filter and strain commute (uniform z, two layers away from every wall), the tile
+      // kernel on the planes and rows next to the walls (or everywhere on a stretched grid)
+      const D3Split sp = d3_split(c, s->P.zstretch == CALES_Z_UNIFORM);
+      const dim3 tb(D3_TX, D3_TY);
+      const unsigned ntx3 = (unsigned)((c.nx + D3_TX - 1) / D3_TX), nty3 = (unsigned)((c.ny + D3_TY - 1) / D3_TY);
+      const size_t sm3 = D3_SMEM_DOUBLES * sizeof(double);
+      if (!sp.col) {
+        k_dsm3_pass1<<<dim3(ntx3, nty3, c.nz), tb, sm3, s->st>>>(c, u, v, w, c.nz, 0, D3_TY, c.ny, c.ny, ds.pslots, s->smag, s->dsm_part);
+        LAUNCH_TRY(K_DSM3);
+      } else {
+        if (sp.klo > 0) {          // planes 0, 1, nz-2, nz-1: every row
+          k_dsm3_pass1<<<dim3(ntx3, nty3, 2 * sp.klo), tb, sm3, s->st>>>(c, u, v, w, sp.klo, c.nz - 2 * sp.klo, D3_TY, c.ny, c.ny, ds.pslots, s->smag, s->dsm_part);
+          LAUNCH_TRY(K_DSM3);
+        }
+        if (sp.jlo > 0) {          // the other planes: rows 0, 1, ny-2, ny-1
+          k_dsm3_pass1<<<dim3(ntx3, 2, sp.khi - sp.klo), tb, sm3, s->st>>>(c, u, v, w, 0, sp.klo, c.ny - D3_TY, sp.jlo, sp.jhi, ds.pslots, s->smag, s->dsm_part);
+          LAUNCH_TRY(K_DSM3);
+        }
+        k_dsm3_col<64, 4><<<dim3(ds.nbx, (sp.jhi - sp.jlo + DSMC_LY - 1) / DSMC_LY, sp.khi - sp.klo), 64, 0, s->st>>>(c, u, v, w, sp.klo, sp.jlo, sp.jhi, ds.pslots, s->smag, s->dsm_part);
+        LAUNCH_TRY(K_DSM3_COL);
+      }
     } else if (ywall) {
       if (split) k_dsm_pass1<<<dim3(ntile, 2, c.nz), dim3(DSM_TX, DSM_TY), tile_smem, s->st>>>(c, u, v, w, c.ny - DSM_TY, DSM_TY, c.ny - DSM_TY, ds.pslots, s->smag, s->dsm_part);
       else k_dsm_pass1<<<dim3(ntile, (c.ny + DSM_TY - 1) / DSM_TY, c.nz), dim3(DSM_TX, DSM_TY), tile_smem, s->st>>>(c, u, v, w, DSM_TY, c.ny, c.ny, ds.pslots, s->smag, s->dsm_part);
@@ -457,7 +476,12 @@ extern "C" int cales_launches_per_step(cales_solver* s) {
             1 /*static nu_t or fill*/;
   if (c.sgs == CALES_SGS_DSMAG) {
     const bool ywall = c.bc_y == BC_WALL, split = ywall && c.ny >= 3 * DSM_TY;
-    per += -1 + (c.dsm_filter3d ? 1 : (ywall ? 1 : 0) + ((!ywall || split) ? 1 : 0)) + 2;   // pass 1 (tile and/or column kernel), coefficient, nu_t
+    int pass1 = (ywall ? 1 : 0) + ((!ywall || split) ? 1 : 0);
+    if (c.dsm_filter3d) {
+      const D3Split sp = d3_split(c, s->P.zstretch == CALES_Z_UNIFORM);
+      pass1 = sp.col ? 1 + (sp.klo > 0 ? 1 : 0) + (sp.jlo > 0 ? 1 : 0) : 1;
+    }
+    per += -1 + pass1 + 2;   // pass 1 (tile and/or column kernel), coefficient, nu_t
   }
   return 3 * per;
 }

@@ -166,34 +166,142 @@ CALES_HD void d3_point(const Ctx& c, int j0, int k, int tx, int ty, const double
   *lm = ll; *mm = m2; *smag_out = mid[d3_mid_off(9, 1, my, mx)];
 }
 
+// ------------------------------------------------------------------------------------------------------------
+// Column-marching form (the production path where the 27 filter weights are uniform and the z grid is uniform: there F
+// commutes with the strain operator, S~_ij = F(S_ij), as in k_dsm_col_sm).  Same march as the x-y kernel, with the z part
+// of the separable filter applied first, point-wise: every thread evaluates the base values of its column on planes
+// k-1, k, k+1, forms  zq = (q(k-1) + 2 q(k) + q(k+1)) / 4  of the 21 quantities and publishes zq; the x-filter reads the
+// neighbours' zq, the y-filter is the two-row window in shared memory.  Planes / rows next to a wall (two of each: the
+// first-layer rule changes the weights of the layer itself and of its neighbour's stencil) go to k_dsm3_pass1.
+// ------------------------------------------------------------------------------------------------------------
+struct D3Split { int col, klo, khi, jlo, jhi; };    // col = 0: the tile kernel everywhere
+CALES_HD D3Split d3_split(const Ctx& c, int z_uniform) {
+  D3Split s; s.col = 0; s.klo = 0; s.khi = c.nz; s.jlo = 0; s.jhi = c.ny;
+  if (!z_uniform) return s;
+  if (c.bc_z == BC_WALL) { s.klo = 2; s.khi = c.nz - 2; }
+  if (c.bc_y == BC_WALL) { s.jlo = 2; s.jhi = c.ny - 2; }
+  if (s.khi - s.klo < 2 || (c.bc_y == BC_WALL && c.ny < 2 * D3_TY)) return s;
+  s.col = 1;
+  return s;
+}
+
+// phase A: zq of (column t, row gj) into shbuf[.][t] and the registers zq; |S| of plane k through smag_c
+CALES_HD void d3c_phaseA(const Ctx& c, const double* u, const double* v, const double* w, int txb, int t, int i0, int gj, int k,
+                         double* shbuf /* [DSMC_NQ][txb] */, double* zq, double* smag_c) {
+  const int gi = ((i0 - 1 + t) % c.nx + c.nx) % c.nx;
+#pragma unroll
+  for (int m = 0; m < DSMC_NQ; ++m) zq[m] = 0.0;
+#pragma unroll
+  for (int d = -1; d <= 1; ++d) {
+    const int kk = c.bc_z == BC_PER ? wrapi(k + d, c.nz) : k + d;
+    double b[DSMC_NB], q[DSMC_NQ];
+    dsmc_base(c, u, v, w, gi, gj, kk, b);
+    dsmc_q(b, q);
+    const double wgt = d == 0 ? 0.5 : 0.25;
+#pragma unroll
+    for (int m = 0; m < DSMC_NQ; ++m) zq[m] += wgt * q[m];
+    if (d == 0) *smag_c = b[9];
+  }
+#pragma unroll
+  for (int m = 0; m < DSMC_NQ; ++m) shbuf[m * txb + t] = zq[m];
+}
+
+// phase B (threads 1..txb-2): x-filter from the neighbours' zq, y-filter over the shared-memory window (as dsmc_phaseB_sm)
+CALES_HD bool d3c_phaseB(const Ctx& c, int txb, int t, int r, int k, const double* shbuf, const double* zq, double* ring,
+                         double* smag_prev, double smag_c, double* lm, double* mm, double* smag) {
+  double* r1 = ring + ((r + 1) & 1) * (DSMC_NQ * txb) + t;     // xq(r-1)
+  double* r2 = ring + (r & 1) * (DSMC_NQ * txb) + t;           // xq(r-2); overwritten with xq(r)
+  double Fq[DSMC_NQ];
+#pragma unroll
+  for (int m = 0; m < DSMC_NQ; ++m) {
+    const double xq = 0.25 * (shbuf[m * txb + t - 1] + shbuf[m * txb + t + 1]) + 0.5 * zq[m];
+    Fq[m] = 0.25 * (r2[m * txb] + xq) + 0.5 * r1[m * txb];
+    r2[m * txb] = xq;
+  }
+  bool done = false;
+  if (r >= 2) {
+    const double d2 = c.delta[k] * c.delta[k];
+    dsmc_contract(Fq, d2, c.alpha * sqrt(c.alpha), lm, mm);      // three filtered directions: alpha = 8^(1/3)
+    *smag = *smag_prev;
+    done = true;
+  }
+  *smag_prev = smag_c;
+  return done;
+}
+
 #ifdef __CUDACC__
-// grid (ceil(nx/D3_TX), ceil(ny/D3_TY), nz), block (D3_TX, D3_TY), dynamic smem D3_SMEM_DOUBLES*8.
-// part: [k][j][pslots][2]; this kernel fills slot blockIdx.x of every row (the other slots stay 0).
+// grid (ceil(nx/D3_TX), row tiles, planes), block (D3_TX, D3_TY), dynamic smem D3_SMEM_DOUBLES*8.
+// planes: k = blockIdx.z (+ kskip when blockIdx.z >= ksplit); rows: j0 = blockIdx.y * jstride, of which only the rows
+// j < row_hi || j >= row_lo2 are written (the others belong to k_dsm3_col).
+// part: [k][j][pslots][2]; this kernel fills slot blockIdx.x of its rows (the other slots stay 0).
 __global__ void __launch_bounds__(D3_TX * D3_TY) k_dsm3_pass1(const __grid_constant__ Ctx c, const double* __restrict__ u, const double* __restrict__ v,
-                                                               const double* __restrict__ w, int pslots, double* __restrict__ smag, double* __restrict__ part) {
+                                                               const double* __restrict__ w, int ksplit, int kskip, int jstride, int row_hi, int row_lo2,
+                                                               int pslots, double* __restrict__ smag, double* __restrict__ part) {
   extern __shared__ double d3_sm[];
   double* raw = d3_sm; double* flt = raw + D3_RAW; double* mid = flt + D3_FLT;
   const int tid = threadIdx.x + D3_TX * threadIdx.y, nth = D3_TX * D3_TY;
-  const int i0 = blockIdx.x * D3_TX, j0 = blockIdx.y * D3_TY, k = blockIdx.z;
+  const int i0 = blockIdx.x * D3_TX, j0 = blockIdx.y * jstride, k = (int)blockIdx.z + ((int)blockIdx.z >= ksplit ? kskip : 0);
   d3_load(tid, nth, c, u, v, w, i0, j0, k, raw);
   __syncthreads();
   d3_mid(tid, nth, c, i0, j0, k, raw, flt, mid);
   __syncthreads();
   const int i = i0 + threadIdx.x, j = j0 + threadIdx.y;
   double lm = 0.0, mm = 0.0;
-  if (i < c.nx && j < c.ny) {
+  const bool mine = j < c.ny && (j < row_hi || j >= row_lo2);      // warp-uniform (one row per warp)
+  if (i < c.nx && mine) {
     double sm;
     d3_point(c, j0, k, threadIdx.x, threadIdx.y, flt, mid, &lm, &mm, &sm);
     smag[idx3(c, i, j, k)] = sm;
   }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) { lm += __shfl_down_sync(0xffffffffu, lm, o); mm += __shfl_down_sync(0xffffffffu, mm, o); }
-  if (threadIdx.x == 0 && j < c.ny) {
+  if (threadIdx.x == 0 && mine) {
     const long long row = (long long)k * c.ny + j;
     part[(row * pslots + blockIdx.x) * 2] = lm;
     part[(row * pslots + blockIdx.x) * 2 + 1] = mm;
   }
 }
+// grid (ceil(nx/(TXB-2)), ceil((jhi-jlo)/DSMC_LY), khi-klo), block TXB; output rows [jlo, jhi) of planes [klo, khi).
+// part: slots blockIdx.x * (TXB/32) + warp.
+template <int TXB, int MINB>
+__global__ void __launch_bounds__(TXB, MINB) k_dsm3_col(const __grid_constant__ Ctx c, const double* __restrict__ u, const double* __restrict__ v,
+                                                        const double* __restrict__ w, int klo, int jlo, int jhi, int pslots, double* __restrict__ smag,
+                                                        double* __restrict__ part) {
+  __shared__ double sh[2][DSMC_NQ * TXB];
+  __shared__ double ring[2 * DSMC_NQ * TXB];
+  const int t = threadIdx.x, k = klo + blockIdx.z;
+  const int i0 = blockIdx.x * (TXB - 2);
+  const int j0 = jlo + blockIdx.y * DSMC_LY;
+  const int jend = min(j0 + DSMC_LY, jhi);
+  const int nrows = jend - j0 + 2;
+  const int gi = i0 - 1 + t;
+  const bool outcol = t >= 1 && t <= TXB - 2 && gi < c.nx;
+#pragma unroll
+  for (int m = 0; m < 2 * DSMC_NQ; ++m) ring[m * TXB + t] = 0.0;
+  double smag_prev = 0.0;
+  for (int r = 0; r < nrows; ++r) {
+    int gj = j0 - 1 + r;
+    gj = gj < 0 ? gj + c.ny : (gj >= c.ny ? gj - c.ny : gj);
+    double zq[DSMC_NQ], smag_c;
+    d3c_phaseA(c, u, v, w, TXB, t, i0, gj, k, sh[r & 1], zq, &smag_c);
+    __syncthreads();
+    double lm = 0.0, mm = 0.0, sm = 0.0;
+    bool done = false;
+    if (t >= 1 && t <= TXB - 2) done = d3c_phaseB(c, TXB, t, r, k, sh[r & 1], zq, ring, &smag_prev, smag_c, &lm, &mm, &sm);
+    if (r >= 2) {
+      const int jo = j0 + r - 2;
+      if (!(done && outcol)) { lm = 0.0; mm = 0.0; }
+      else smag[idx3(c, gi, jo, k)] = sm;
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) { lm += __shfl_down_sync(0xffffffffu, lm, o); mm += __shfl_down_sync(0xffffffffu, mm, o); }
+      if ((t & 31) == 0) {
+        const long long slot = ((long long)k * c.ny + jo) * pslots + blockIdx.x * (TXB / 32) + (t >> 5);
+        part[slot * 2] = lm; part[slot * 2 + 1] = mm;
+      }
+    }
+  }
+}
 #endif
+
 
 }  // namespace cales

@@ -189,13 +189,23 @@ static void emu_nut(emu_solver* s, const double* u, const double* v, const doubl
     const int ntile = (c.nx + D3_TX - 1) / D3_TX, nth = D3_TX * D3_TY;
     std::vector<double> sm(D3_SMEM_DOUBLES);
     double* raw = sm.data(); double* flt = raw + D3_RAW; double* mid = flt + D3_FLT;
-    for (int k = 0; k < c.nz; ++k) for (int by = 0; by * D3_TY < c.ny; ++by) for (int bx = 0; bx < ntile; ++bx) {
-      const int i0 = bx * D3_TX, j0 = by * D3_TY;
+    const D3Split sp = d3_split(c, s->H.P.zstretch == CALES_Z_UNIFORM);
+    // the tile kernel's launches: (planes, row tiles, jstride, row_hi, row_lo2)
+    struct TL { int k0, k1, nby, jstride, row_hi, row_lo2; };
+    std::vector<TL> tl;
+    if (!sp.col) tl.push_back({0, c.nz, (c.ny + D3_TY - 1) / D3_TY, D3_TY, c.ny, c.ny});
+    else {
+      if (sp.klo > 0) { tl.push_back({0, sp.klo, (c.ny + D3_TY - 1) / D3_TY, D3_TY, c.ny, c.ny}); tl.push_back({sp.khi, c.nz, (c.ny + D3_TY - 1) / D3_TY, D3_TY, c.ny, c.ny}); }
+      if (sp.jlo > 0) tl.push_back({sp.klo, sp.khi, 2, c.ny - D3_TY, sp.jlo, sp.jhi});
+    }
+    for (const TL& L : tl)
+    for (int k = L.k0; k < L.k1; ++k) for (int by = 0; by < L.nby; ++by) for (int bx = 0; bx < ntile; ++bx) {
+      const int i0 = bx * D3_TX, j0 = by * L.jstride;
       for (int tid = 0; tid < nth; ++tid) d3_load(tid, nth, c, u, v, w, i0, j0, k, raw);
       for (int tid = 0; tid < nth; ++tid) d3_mid(tid, nth, c, i0, j0, k, raw, flt, mid);
       for (int ty = 0; ty < D3_TY; ++ty) {
         const int j = j0 + ty;
-        if (j >= c.ny) continue;
+        if (!(j < c.ny && (j < L.row_hi || j >= L.row_lo2))) continue;
         double lm = 0.0, mm = 0.0;
         for (int tx = 0; tx < D3_TX; ++tx) {
           const int i = i0 + tx;
@@ -207,6 +217,30 @@ static void emu_nut(emu_solver* s, const double* u, const double* v, const doubl
         }
         const long long row = (long long)k * c.ny + j;
         s->dsm_part[(row * ntx + bx) * 2] = lm; s->dsm_part[(row * ntx + bx) * 2 + 1] = mm;
+      }
+    }
+    if (sp.col) {   // k_dsm3_col, stepped row by row with the block barrier between the phases
+      const int T = dsh.txb;
+      std::vector<double> sh(2 * DSMC_NQ * T), zq((size_t)T * DSMC_NQ), smc(T), ring(2 * DSMC_NQ * T), smprev(T);
+      for (int k = sp.klo; k < sp.khi; ++k) for (int by = 0; by * DSMC_LY < sp.jhi - sp.jlo; ++by) for (int bx = 0; bx < dsh.nbx; ++bx) {
+        const int i0 = bx * (T - 2), j0 = sp.jlo + by * DSMC_LY, jend = std::min(j0 + DSMC_LY, sp.jhi), nrows = jend - j0 + 2;
+        std::fill(ring.begin(), ring.end(), 0.0); std::fill(smprev.begin(), smprev.end(), 0.0);
+        for (int r = 0; r < nrows; ++r) {
+          int gj = j0 - 1 + r; gj = gj < 0 ? gj + c.ny : (gj >= c.ny ? gj - c.ny : gj);
+          double* buf = sh.data() + (r & 1) * DSMC_NQ * T;
+          for (int t = 0; t < T; ++t) d3c_phaseA(c, u, v, w, T, t, i0, gj, k, buf, &zq[(size_t)t * DSMC_NQ], &smc[t]);
+          std::vector<double> wl(T / 32, 0.0), wm(T / 32, 0.0);
+          for (int t = 1; t <= T - 2; ++t) {
+            double lm = 0.0, mm = 0.0, sg = 0.0;
+            const bool done = d3c_phaseB(c, T, t, r, k, buf, &zq[(size_t)t * DSMC_NQ], ring.data(), &smprev[t], smc[t], &lm, &mm, &sg);
+            const int gi = i0 - 1 + t;
+            if (r >= 2 && done && gi < c.nx) { s->smag[idx3(c, gi, j0 + r - 2, k)] = sg; wl[t >> 5] += lm; wm[t >> 5] += mm; }
+          }
+          if (r >= 2) for (int wq = 0; wq < T / 32; ++wq) {
+            const long long slot = ((long long)k * c.ny + (j0 + r - 2)) * ntx + bx * (T / 32) + wq;
+            s->dsm_part[slot * 2] = wl[wq]; s->dsm_part[slot * 2 + 1] = wm[wq];
+          }
+        }
       }
     }
   } else if (ywall) {   // tile kernel: all rows, or the DSM_TY rows next to each y wall
