@@ -13,6 +13,15 @@
 #include "cales_closures.cuh"
 #include "cales_smag_tile.cuh"
 #include "cales_dsm3.cuh"
+#ifndef CALES_D3C_TXB
+#define CALES_D3C_TXB 64
+#endif
+#ifndef CALES_D3C_MINB
+#define CALES_D3C_MINB 6
+#endif
+#ifndef CALES_D3C_NBUF
+#define CALES_D3C_NBUF 1
+#endif
 #include "cales_host.h"
 
 #include <cmath>
@@ -340,7 +349,8 @@ static int run_eddy_viscosity(cales_solver* s, const double* u, const double* v,
           k_dsm3_pass1<<<dim3(ntx3, 2, sp.khi - sp.klo), tb, sm3, s->st>>>(c, u, v, w, 0, sp.klo, c.ny - D3_TY, sp.jlo, sp.jhi, ds.pslots, s->smag, s->dsm_part);
           LAUNCH_TRY(K_DSM3);
         }
-        k_dsm3_col<64, 4><<<dim3(ds.nbx, (sp.jhi - sp.jlo + DSMC_LY - 1) / DSMC_LY, sp.khi - sp.klo), 64, 0, s->st>>>(c, u, v, w, sp.klo, sp.jlo, sp.jhi, ds.pslots, s->smag, s->dsm_part);
+        // <threads, min CTAs/SM, row buffers>: measured on B200 (config 4): (64,4,2) 6.46 ms, (64,6,1) 6.16 ms, (64,8,1) 7.45 ms (spills)
+      k_dsm3_col<CALES_D3C_TXB, CALES_D3C_MINB, CALES_D3C_NBUF><<<dim3(ds.nbx, (sp.jhi - sp.jlo + DSMC_LY - 1) / DSMC_LY, sp.khi - sp.klo), CALES_D3C_TXB, 0, s->st>>>(c, u, v, w, sp.klo, sp.jlo, sp.jhi, ds.pslots, s->smag, s->dsm_part);
         LAUNCH_TRY(K_DSM3_COL);
       }
     } else if (ywall) {

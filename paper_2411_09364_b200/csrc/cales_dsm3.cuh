@@ -263,11 +263,11 @@ __global__ void __launch_bounds__(D3_TX * D3_TY) k_dsm3_pass1(const __grid_const
 }
 // grid (ceil(nx/(TXB-2)), ceil((jhi-jlo)/DSMC_LY), khi-klo), block TXB; output rows [jlo, jhi) of planes [klo, khi).
 // part: slots blockIdx.x * (TXB/32) + warp.
-template <int TXB, int MINB>
+template <int TXB, int MINB, int NBUF>
 __global__ void __launch_bounds__(TXB, MINB) k_dsm3_col(const __grid_constant__ Ctx c, const double* __restrict__ u, const double* __restrict__ v,
                                                         const double* __restrict__ w, int klo, int jlo, int jhi, int pslots, double* __restrict__ smag,
                                                         double* __restrict__ part) {
-  __shared__ double sh[2][DSMC_NQ * TXB];
+  __shared__ double sh[NBUF][DSMC_NQ * TXB];
   __shared__ double ring[2 * DSMC_NQ * TXB];
   const int t = threadIdx.x, k = klo + blockIdx.z;
   const int i0 = blockIdx.x * (TXB - 2);
@@ -283,11 +283,12 @@ __global__ void __launch_bounds__(TXB, MINB) k_dsm3_col(const __grid_constant__ 
     int gj = j0 - 1 + r;
     gj = gj < 0 ? gj + c.ny : (gj >= c.ny ? gj - c.ny : gj);
     double zq[DSMC_NQ], smag_c;
-    d3c_phaseA(c, u, v, w, TXB, t, i0, gj, k, sh[r & 1], zq, &smag_c);
+    if (NBUF == 1) __syncthreads();     // the previous row's neighbours have read the buffer
+    d3c_phaseA(c, u, v, w, TXB, t, i0, gj, k, sh[r & (NBUF - 1)], zq, &smag_c);
     __syncthreads();
     double lm = 0.0, mm = 0.0, sm = 0.0;
     bool done = false;
-    if (t >= 1 && t <= TXB - 2) done = d3c_phaseB(c, TXB, t, r, k, sh[r & 1], zq, ring, &smag_prev, smag_c, &lm, &mm, &sm);
+    if (t >= 1 && t <= TXB - 2) done = d3c_phaseB(c, TXB, t, r, k, sh[r & (NBUF - 1)], zq, ring, &smag_prev, smag_c, &lm, &mm, &sm);
     if (r >= 2) {
       const int jo = j0 + r - 2;
       if (!(done && outcol)) { lm = 0.0; mm = 0.0; }
