@@ -191,16 +191,41 @@ CALES_HD void d3c_phaseA(const Ctx& c, const double* u, const double* v, const d
   const int gi = ((i0 - 1 + t) % c.nx + c.nx) % c.nx;
 #pragma unroll
   for (int m = 0; m < DSMC_NQ; ++m) zq[m] = 0.0;
-#pragma unroll
-  for (int d = -1; d <= 1; ++d) {
-    const int kk = c.bc_z == BC_PER ? wrapi(k + d, c.nz) : k + d;
-    double b[DSMC_NB], q[DSMC_NQ];
-    dsmc_base(c, u, v, w, gi, gj, kk, b);
+  // planes k-2 .. k+2 without wrap or ghost (and a row whose y neighbours are plain): one set of in-plane neighbour offsets
+  // and plane offsets that are multiples of nxy, so the loads shared by the three strain stencils are issued once
+  const bool plain = k >= 2 && k <= c.nz - 3 && (c.bc_y == BC_PER || (gj >= 1 && gj <= c.ny - 2));
+  auto add = [&](const double* b, int d) {
+    double q[DSMC_NQ];
     dsmc_q(b, q);
     const double wgt = d == 0 ? 0.5 : 0.25;
 #pragma unroll
     for (int m = 0; m < DSMC_NQ; ++m) zq[m] += wgt * q[m];
     if (d == 0) *smag_c = b[9];
+  };
+  if (plain) {
+    const long long n = idx3(c, gi, gj, k);
+    const Nbr o = neighbours(c, gi, gj, k);
+#pragma unroll
+    for (int d = -1; d <= 1; ++d) {
+      auto at = [&](const double* __restrict__ f, int a, int bb, int dd) {
+        return f[n + (long long)(d + dd) * c.nxy + ((a < 0 ? o.im : (a > 0 ? o.ip : 0)) + (bb < 0 ? o.jm : (bb > 0 ? o.jp : 0)))];
+      };
+      auto U = [&](int a, int bb, int dd) { return at(u, a, bb, dd); };
+      auto V = [&](int a, int bb, int dd) { return at(v, a, bb, dd); };
+      auto W = [&](int a, int bb, int dd) { return at(w, a, bb, dd); };
+      double b[DSMC_NB], S[6];
+      b[9] = strain_at(U, V, W, c.rdx, c.rdy, c.rdzf[k + d], c.rdzc[k + d], c.rdzc[k + d - 1], S);
+      b[0] = 0.5 * (U(-1, 0, 0) + U(0, 0, 0)); b[1] = 0.5 * (V(0, -1, 0) + V(0, 0, 0)); b[2] = 0.5 * (W(0, 0, -1) + W(0, 0, 0));
+#pragma unroll
+      for (int m = 0; m < 6; ++m) b[3 + m] = S[m];
+      add(b, d);
+    }
+  } else {
+    for (int d = -1; d <= 1; ++d) {
+      double b[DSMC_NB];
+      dsmc_base(c, u, v, w, gi, gj, c.bc_z == BC_PER ? wrapi(k + d, c.nz) : k + d, b);
+      add(b, d);
+    }
   }
 #pragma unroll
   for (int m = 0; m < DSMC_NQ; ++m) shbuf[m * txb + t] = zq[m];
