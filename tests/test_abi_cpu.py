@@ -56,6 +56,8 @@ def test_defaults_and_workspace_size(binding):
     (dict(implicit_z=1, bc_z=0), "implicit z needs z walls"),
     (dict(van_driest=1, bc_z=0), "van Driest"),
     (dict(nu=0.0), "nu must be positive"),
+    (dict(dsm_filter3d=1, sgs_model=1), "dsm_filter3d needs the dynamic model"),
+    (dict(wall_model_y=1, bc_y=0), "wall model on y walls needs y walls"),
     (dict(lx=-1.0), "positive"),
 ])
 def test_argument_errors_are_reported_at_create_time(binding, kw, msg):
