@@ -59,7 +59,9 @@ typedef struct {
   double dsm_alpha2d;        /* filter-width ratio of the x-y test filter; <= 0 -> 4^(1/3) */
   int wall_model;            /* log-law wall model on the z walls (Eq. 10) */
   double kappa, B;           /* <= 0 kappa -> 0.41; B as given (5.2 in the paper) */
-  double h_wm;               /* height of the wall-modelled layer; <= 0 -> first off-wall cell centre */
+  double h_wm;               /* height of the wall-modelled layer, the same at every modelled wall (z and y): linear interpolation
+                                between the two bracketing centres; <= 0 -> first off-wall cell centre; must lie
+                                below lz/2 (and ly/2 with wall_model_y) */
   double wm_tol;             /* relative tolerance on tau_w; <= 0 -> 1e-4 */
   int wm_maxit;              /* <= 0 -> 50 */
   int implicit_z;            /* Crank-Nicolson in z, Eq. 20-22 */

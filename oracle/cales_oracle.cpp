@@ -315,17 +315,22 @@ static void bc_velocity(oracle_solver& S, F3& u, F3& v, F3& w, int mode) {
 // (each interpolated to h_wm), U = sqrt(u_wm^2+v_wm^2), Newton for u_tau, tau_xz = u_tau^2 u_wm / U.
 // Same at v-points with u interpolated -> tau_yz.  Needs x/y ghosts of u, v (call after bc_velocity).
 // ------------------------------------------------------------------------------------------------
-// y walls (duct WMLES): sampled at the first off-wall centre, h = dy/2.  tau_xy at the u points (i+1/2, k) from u and the
+// y walls (duct WMLES): sampled at h_wm from the wall, linear interpolation between the two bracketing centres as in z
+// (default: the first off-wall centre, h = dy/2).  tau_xy at the u points (i+1/2, k) from u and the
 // 4 surrounding w points; tau_zy at the w points (i, k+1/2) from w and the 4 surrounding u points.
 static void wall_stress_y(oracle_solver& S, int& maxit) {
   int nx = S.nx, ny = S.ny, nz = S.nz;
-  const double h = 0.5 * S.dy;
+  auto dist = [&](int q) { return (q + 0.5) * S.dy; };        // centre number q counted from the wall
+  const double h = S.P.h_wm > 0.0 ? S.P.h_wm : dist(0);
+  int q1 = 0; while (q1 + 2 < ny / 2 && dist(q1 + 1) <= h) ++q1;
+  const double wgt = (h - dist(q1)) / (dist(q1 + 1) - dist(q1));
   for (int wall = 0; wall < 2; ++wall) {
-    const int j0 = wall == 0 ? 0 : ny - 1;
+    const int ja = wall == 0 ? q1 : ny - 1 - q1, jb = wall == 0 ? q1 + 1 : ny - 2 - q1;
+    auto at = [&](const F3& q, int ii, int kk) { return (1.0 - wgt) * q(ii, ja, kk) + wgt * q(ii, jb, kk); };
     for (int k = 0; k < nz; ++k) for (int i = 0; i < nx; ++i) for (int comp = 0; comp < 2; ++comp) {
       double a, b;
-      if (comp == 0) { a = S.u(i, j0, k); b = 0.25 * (S.w(i, j0, k) + S.w(i + 1, j0, k) + S.w(i, j0, k - 1) + S.w(i + 1, j0, k - 1)); }
-      else { a = S.w(i, j0, k); b = 0.25 * (S.u(i, j0, k) + S.u(i - 1, j0, k) + S.u(i, j0, k + 1) + S.u(i - 1, j0, k + 1)); }
+      if (comp == 0) { a = at(S.u, i, k); b = 0.25 * (at(S.w, i, k) + at(S.w, i + 1, k) + at(S.w, i, k - 1) + at(S.w, i + 1, k - 1)); }
+      else { a = at(S.w, i, k); b = 0.25 * (at(S.u, i, k) + at(S.u, i - 1, k) + at(S.u, i, k + 1) + at(S.u, i - 1, k + 1)); }
       double U = std::sqrt(a * a + b * b), t = 0.0;
       if (U > 0.0) {
         int it = 0;
@@ -794,6 +799,7 @@ extern "C" int oracle_create(const oracle_params* p, oracle_solver** out) {
   if (p->wall_model_y && p->bc_y != BC_WALL) return fail("wall model on y walls needs y walls");
   if (p->implicit_z && p->bc_z != BC_WALL) return fail("implicit z needs z walls");
   if (p->wall_model && p->h_wm > 0.0 && !(p->h_wm < 0.5 * p->lz)) return fail("h_wm must lie below the half height");
+  if (p->wall_model_y && p->h_wm > 0.0 && !(p->h_wm < 0.5 * p->ly)) return fail("h_wm must lie below the half width");
   if (p->van_driest && (p->bc_z != BC_WALL || p->bc_y == BC_WALL || p->wall_model)) return fail("van Driest: z walls only, no wall model");
   oracle_solver* S = new oracle_solver();
   S->P = *p; S->nx = p->nx; S->ny = p->ny; S->nz = p->nz; S->N = (size_t)p->nx * p->ny * p->nz;

@@ -60,16 +60,14 @@ CALES_HD int wall_stress_point(const Ctx& c, const WallGeom& g, const double* u,
 // (i+1/2, k) from u and the 4 surrounding w points; comp 1: tau_zy at the w point (i, k+1/2) from w and the 4 surrounding u.
 // tau_y[wall][comp][k][i].
 CALES_HD int wall_stress_y_point(const Ctx& c, const double* u, const double* w, int wall, int comp, int i, int k, double* tau_y) {
-  const int j0 = wall == 0 ? 0 : c.ny - 1;
-  const double h = 0.5 * c.dy;
+  const int ja = wall == 0 ? c.wy_q1 : c.ny - 1 - c.wy_q1, jb = wall == 0 ? c.wy_q1 + 1 : c.ny - 2 - c.wy_q1;
+  const double wg = c.wy_wgt, h = c.wy_h;
+  // linear interpolation in y between the two bracketing centres; wg = 0 at the default h = dy/2
+  auto atu = [&](int ii, int kk) { return (1.0 - wg) * velg<0>(c, u, ii, ja, kk, GH_STRAIN) + wg * velg<0>(c, u, ii, jb, kk, GH_STRAIN); };
+  auto atw = [&](int ii, int kk) { return (1.0 - wg) * velg<2>(c, w, ii, ja, kk, GH_STRAIN) + wg * velg<2>(c, w, ii, jb, kk, GH_STRAIN); };
   double a, b;
-  if (comp == 0) {
-    a = velg<0>(c, u, i, j0, k, GH_STRAIN);
-    b = 0.25 * (velg<2>(c, w, i, j0, k, GH_STRAIN) + velg<2>(c, w, i + 1, j0, k, GH_STRAIN) + velg<2>(c, w, i, j0, k - 1, GH_STRAIN) + velg<2>(c, w, i + 1, j0, k - 1, GH_STRAIN));
-  } else {
-    a = velg<2>(c, w, i, j0, k, GH_STRAIN);
-    b = 0.25 * (velg<0>(c, u, i, j0, k, GH_STRAIN) + velg<0>(c, u, i - 1, j0, k, GH_STRAIN) + velg<0>(c, u, i, j0, k + 1, GH_STRAIN) + velg<0>(c, u, i - 1, j0, k + 1, GH_STRAIN));
-  }
+  if (comp == 0) { a = atu(i, k); b = 0.25 * (atw(i, k) + atw(i + 1, k) + atw(i, k - 1) + atw(i + 1, k - 1)); }
+  else { a = atw(i, k); b = 0.25 * (atu(i, k) + atu(i - 1, k) + atu(i, k + 1) + atu(i - 1, k + 1)); }
   const double U = sqrt(a * a + b * b);
   double t = 0.0; int it = 0;
   if (U > 0.0) {

@@ -20,9 +20,10 @@ struct Ctx {
   int nx, ny, nz;
   int bc_y, bc_z, wall_model, wall_model_y, sgs, van_driest, implicit_z, dsm_plane, dsm_clip_total, dsm_filter3d, const_flow_rate;
   int wm_maxit;
+  int wy_q1;       // y-wall model: the sample lies between centres wy_q1 and wy_q1 + 1 counted from the wall
   long long N;     // nx*ny*nz
   long long nxy;   // nx*ny
-  double dx, dy, rdx, rdy, rnuap /* 1/(nu A+) */, lz, nu, cs, aplus, alpha, kappa, Blog, h_wm, wm_tol, u_bulk;
+  double dx, dy, rdx, rdy, rnuap /* 1/(nu A+) */, lz, nu, cs, aplus, alpha, kappa, Blog, h_wm, wm_tol, u_bulk, wy_wgt /* interpolation weight */, wy_h /* sampling distance */;
   // 1-D grid tables in device memory, offset so that the ghost entries are addressable:
   const double* dzf;   // dzf[-1 .. nz]   cell heights (ghost = neighbour's / wrapped)
   const double* dzc;   // dzc[-1 .. nz-1] centre spacings across face k+1 (mirrored ghost centre at walls)

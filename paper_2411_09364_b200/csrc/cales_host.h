@@ -40,6 +40,7 @@ static inline int validate(const cales_params* p) {
   if (p->dsm_filter3d && p->sgs_model != CALES_SGS_DSMAG) return fail(CALES_EINVAL, "dsm_filter3d needs the dynamic model");
   if (p->implicit_z && p->bc_z != CALES_BC_WALL) return fail(CALES_EUNSUPPORTED, "implicit z needs z walls");
   if (p->wall_model && p->h_wm > 0.0 && !(p->h_wm < 0.5 * p->lz)) return fail(CALES_EINVAL, "h_wm must lie below the half height");
+  if (p->wall_model_y && p->h_wm > 0.0 && !(p->h_wm < 0.5 * p->ly)) return fail(CALES_EINVAL, "h_wm must lie below the half width");
   if (p->van_driest && (p->bc_z != CALES_BC_WALL || p->bc_y == CALES_BC_WALL || p->wall_model))
     return fail(CALES_EUNSUPPORTED, "van Driest damping: z walls only, no wall model");
   return CALES_OK;
@@ -160,6 +161,12 @@ static inline int build_setup(const cales_params* p, HostSetup& H) {
     int q1 = 0; while (q1 + 2 < nz / 2 && dist(q1 + 1) <= h) ++q1;
     H.wg.wgt[wall] = (h - dist(q1)) / (dist(q1 + 1) - dist(q1));
     H.wg.ka[wall] = wall == 0 ? q1 : nz - 1 - q1; H.wg.kb[wall] = wall == 0 ? q1 + 1 : nz - 2 - q1; H.wg.h[wall] = h;
+  }
+  {   // the same for the y walls (uniform spacing): centre number q lies (q + 1/2) dy from its wall
+    auto dist = [&](int q) { return (q + 0.5) * dy; };
+    const double h = p->h_wm > 0.0 ? p->h_wm : dist(0);
+    int q1 = 0; while (q1 + 2 < ny / 2 && dist(q1 + 1) <= h) ++q1;
+    c.wy_q1 = q1; c.wy_wgt = (h - dist(q1)) / (dist(q1 + 1) - dist(q1)); c.wy_h = h;
   }
   // ---- transform plans and launch shapes
   make_plan(H.plx, nx);

@@ -689,7 +689,8 @@ def test_wall_model_with_implicit_z_momentum_balance(oracle):
 
 
 # ----------------------------------------------------------------------------- SURVEY.md 8(f) item 1, y walls
-def test_wall_model_on_y_walls_is_the_z_wall_model_rotated(oracle):
+@pytest.mark.parametrize("h_wm", [0.0, 0.3])        # default (first centre) and a sample between centres 1 and 2
+def test_wall_model_on_y_walls_is_the_z_wall_model_rotated(oracle, h_wm):
     """Duct WMLES: the wall model on the y walls must be the (already pinned) z-wall model with the roles of
     y and z exchanged.  Case A: z walls with the wall model, periodic y.  Case B: the same field with y and z swapped
     (v <-> w), y walls with the wall model, periodic z.  Stresses and one full step must agree under the swap."""
@@ -701,7 +702,7 @@ def test_wall_model_on_y_walls_is_the_z_wall_model_rotated(oracle):
     uA = prof[:, None, None] + 0.4 * rng.standard_normal((n1, n2, nx))
     pA = 0.4 * rng.standard_normal((n1, n2, nx))          # periodic-direction component
     qA = 0.4 * rng.standard_normal((n1, n2, nx)); qA[-1] = 0.0   # wall-normal component (faces; last = wall)
-    kw = dict(nu=1.0 / 800, sgs_model=1, cs=0.1)
+    kw = dict(nu=1.0 / 800, sgs_model=1, cs=0.1, h_wm=h_wm)
     A = oracle.Oracle(nx, n2, n1, 3.0, L2, L1, bc_z=1, wall_model=1, **kw)
     A.set_velocity(uA, pA, qA)
     B = oracle.Oracle(nx, n1, n2, 3.0, L1, L2, bc_y=1, bc_z=0, wall_model_y=1, **kw)
