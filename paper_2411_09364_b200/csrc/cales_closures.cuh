@@ -296,7 +296,10 @@ CALES_HD void dsm_point(const Ctx& c, int i0, int j0, int k, int tx, int ty, con
 // neighbours' base values, and keeps the separable y-filter as a two-row sliding window of Fx q in shared memory:
 //   xq(r) = Fx q(r);   F q(r-1) = (xq(r-2) + 2 xq(r-1) + xq(r)) / 4.
 // ------------------------------------------------------------------------------------------------------------
-enum { DSMC_LY = 32, DSMC_NB = 10, DSMC_NQ = 21 };
+#ifndef CALES_DSMC_LY
+#define CALES_DSMC_LY 32      // rows per CTA of the column march (experiments: -DCALES_DSMC_LY=64)
+#endif
+enum { DSMC_LY = CALES_DSMC_LY, DSMC_NB = 10, DSMC_NQ = 21 };
 
 // base values of column gi at row gj (both already wrapped / interior): b[0..2] = u^c, v^c, w^c; b[3..8] = S_ij; b[9] = |S|
 CALES_HD void dsmc_base(const Ctx& c, const double* __restrict__ u, const double* __restrict__ v, const double* __restrict__ w,
