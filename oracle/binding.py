@@ -146,6 +146,15 @@ class Oracle:
     def step(self, dt):
         _chk(lib().oracle_step(self._h, C.c_double(dt)))
 
+    def substep(self, rk, dt):
+        _chk(lib().oracle_substep(self._h, C.c_int(rk), C.c_double(dt)))
+
+    def ustar(self):
+        out = [np.empty(self.shape) for _ in range(3)]
+        for c in range(3):
+            _chk(lib().oracle_get_ustar(self._h, c, _p(out[c])))
+        return out
+
     def poisson_solve(self, rhs):
         rhs = _arr(rhs); phi = np.empty(self.shape)
         _chk(lib().oracle_poisson_solve(self._h, _p(rhs), _p(phi))); return phi

@@ -216,6 +216,7 @@ struct oracle_solver {
   std::vector<double> tauy;                   // y walls: [wall][comp (0 tau_xy at u points, 1 tau_zy at w points)][nz][nx]
   std::vector<double> cs;                     // dynamic coefficient per k or per (k,j)
   std::vector<double> Lij, Mij;               // tensors of the last dynamic evaluation (for the pins)
+  std::vector<double> ust, vst, wst;          // u*, v*, w* of the last substep, after O-step 6, before the bulk shift (for the pins)
   bool fresh = false;                         // wall stress + nu_t consistent with the velocity
   double forcing = 0.0; int wm_max_iters = 0;
   double alpha2d;
@@ -936,6 +937,8 @@ static void substep(oracle_solver& S, int rk, double dt) {
       }
     }
   }
+  S.ust.resize(N); S.vst.resize(N); S.wst.resize(N);     // kept for the pins of Eq. 21 / Eq. 22 (oracle_get_ustar)
+  us.to(S.ust.data()); vs.to(S.vst.data()); ws.to(S.wst.data());
   // O-step 7a: constant flow rate (reading S12): uniform shift of u* to the target bulk velocity
   S.forcing = 0.0;
   if (S.P.const_flow_rate) {
@@ -973,6 +976,21 @@ extern "C" int oracle_step(oracle_solver* S, double dt) {
   if (!S || !(dt > 0.0)) return fail("bad step arguments");
   if (!S->fresh) refresh_closures(*S);   // Alg. 1 l.1-2
   for (int rk = 0; rk < 3; ++rk) substep(*S, rk, dt);
+  return 0;
+}
+// One substep rk = 0, 1, 2 of Alg. 1 on its own (for the pins; a step is the three in order).
+extern "C" int oracle_substep(oracle_solver* S, int rk, double dt) {
+  if (!S || !(dt > 0.0) || rk < 0 || rk > 2) return fail("bad substep arguments");
+  if (!S->fresh) refresh_closures(*S);
+  substep(*S, rk, dt);
+  return 0;
+}
+// u* (comp 0), v* (1), w* (2) of the last substep: after the Crank-Nicolson solve of Eq. 21 (if any), before the bulk shift
+extern "C" int oracle_get_ustar(oracle_solver* S, int comp, double* dst) {
+  if (!S || !dst || comp < 0 || comp > 2) return fail("bad argument");
+  const std::vector<double>& q = comp == 0 ? S->ust : (comp == 1 ? S->vst : S->wst);
+  if (q.size() != S->N) return fail("no substep yet");
+  std::memcpy(dst, q.data(), S->N * sizeof(double));
   return 0;
 }
 extern "C" int oracle_poisson_solve(oracle_solver* S, const double* rhs, double* phi) {

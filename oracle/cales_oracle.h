@@ -67,6 +67,10 @@ int oracle_set_field(oracle_solver* s, int field, const double* src);
 int oracle_get_field(oracle_solver* s, int field, double* dst);
 /* one full RK3 step (3 substeps of Alg. 1) */
 int oracle_step(oracle_solver* s, double dt);
+/* one substep rk = 0, 1, 2 of Alg. 1 on its own, and u* / v* / w* (comp 0, 1, 2) of the last substep as it stands after
+   Eq. 11 or Eq. 20-21 and before the bulk shift (hooks for the pins of Eq. 21 and Eq. 22) */
+int oracle_substep(oracle_solver* s, int rk, double dt);
+int oracle_get_ustar(oracle_solver* s, int comp, double* dst);
 /* Poisson: L_h phi = rhs with the solver's BCs (Eq. 12); zero weighted-mean gauge (reading S15) */
 int oracle_poisson_solve(oracle_solver* s, const double* rhs, double* phi);
 /* plain 7-point stencil L_h phi (O-step 3 operator at centres, periodic/Neumann closure) */

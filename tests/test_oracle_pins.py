@@ -305,7 +305,7 @@ def test_wall_stress_direction_interpolation_and_flux(oracle):
 
 
 # --------------------------------------------------------------------------------------------- P13
-def np_dsm_periodic(S, u, v, w, alpha2=4.0 ** (2.0 / 3.0), filter3d=False):
+def np_dsm_periodic(S, u, v, w, alpha2=4.0 ** (2.0 / 3.0), filter3d=False, pointwise=False):
     """Independent dense numpy evaluation of Eq. 5-9 in a triply periodic box (np.roll, 9- or 27-point filter)."""
     dx, dy, dz = S.dx, S.dy, S.dzf[0]
     r = np.roll
@@ -335,8 +335,12 @@ def np_dsm_periodic(S, u, v, w, alpha2=4.0 ** (2.0 / 3.0), filter3d=False):
     d2 = (dx * dy * dz) ** (2.0 / 3.0)
     M = [2 * d2 * (filt(mag * s[k]) - alpha2 * stmag * st[k]) for k in range(6)]
     f = [1, 1, 1, 2, 2, 2]
-    lm = sum(f[k] * L[k] * M[k] for k in range(6)).sum(axis=(1, 2))
-    mm = sum(f[k] * M[k] * M[k] for k in range(6)).sum(axis=(1, 2))
+    lm_pt = sum(f[k] * L[k] * M[k] for k in range(6))
+    mm_pt = sum(f[k] * M[k] * M[k] for k in range(6))
+    if pointwise:
+        return lm_pt, mm_pt, d2, mag
+    lm = lm_pt.sum(axis=(1, 2))
+    mm = mm_pt.sum(axis=(1, 2))
     cs = lm / mm
     nut = np.maximum(cs, 0.0)[:, None, None] * d2 * mag
     return np.array(L), np.array(M), cs, nut
@@ -529,24 +533,21 @@ def test_taylor_green_decay(oracle, plane):
 
 
 # --------------------------------------------------------------------------------------------- P14
-@pytest.mark.parametrize("comp", ["u", "w"])
+@pytest.mark.parametrize("comp", ["u", "v"])
 def test_crank_nicolson_z_eigenmode(oracle, comp):
+    """Centred family (u, v): an eigenvector of L_zz with the no-slip mirror ghost is multiplied per substep by
+    (1 + c lam)/(1 - c lam).  The face family (w) is pinned by test_crank_nicolson_dense_matrix_on_tanh_grid[w]."""
     nz, nmode, nu, dt = 16, 3, 0.05, 0.02
     S = oracle.Oracle(8, 6, nz, 1.0, 1.0, 1.0, bc_z=1, nu=nu, implicit_z=1, sgs_model=0)
     dz = 1.0 / nz
     k = np.arange(nz)
     lam = -4.0 / dz ** 2 * math.sin(PI * nmode / (2 * nz)) ** 2
     zero = np.zeros(S.shape)
+    prof = np.sin(PI * nmode * (k + 0.5) / nz)
+    q0 = prof[:, None, None] * np.ones(S.shape)
     if comp == "u":
-        prof = np.sin(PI * nmode * (k + 0.5) / nz)
-        q0 = prof[:, None, None] * np.ones(S.shape)
         S.set_velocity(q0, zero, zero)
     else:
-        # w(z) alone is not solenoidal; use w = sin(pi n (k+1)/nz) * cos(2 pi x) pattern?  Instead keep the
-        # projection out of the way: a field w(x,y) independent of z is solenoidal but has no z-diffusion.
-        # So test v instead of w for the centred family and w through the Helmholtz residual below.
-        prof = np.sin(PI * nmode * (k + 0.5) / nz)
-        q0 = prof[:, None, None] * np.ones(S.shape)
         S.set_velocity(zero, q0, zero)
     S.step(dt)
     fac = 1.0
@@ -719,3 +720,324 @@ def test_wall_model_on_y_walls_is_the_z_wall_model_rotated(oracle, h_wm):
     for fa, fb in ((0, 0), (1, 2), (2, 1), (4, 4)):
         a, b = A.get(fa), sw(B.get(fb))
         assert np.max(np.abs(a - b)) <= 1e-11 * max(np.max(np.abs(a)), 1e-3), (fa, fb)
+
+
+# =============================================================================================================
+# Pins added after the round-1 review, which injected single-line mistakes into oracle/cales_oracle.cpp and found six
+# that no pin noticed.  Each test below names the mutant(s) it kills; tests/test_oracle_mutants.py re-injects all of
+# them (and the six that were already caught) and checks that the named pins turn red.
+#   M7  substep(), Eq. 22: drop "- cimp * lzz" from the pressure update
+#   M8  diffusion(), z part of u on a stretched grid: dzc(k) <-> dzc(k-1)
+#   M9  substep(), Crank-Nicolson matrix of u, v: the two metrics of ak, ck exchanged
+#   M10 substep(), Crank-Nicolson matrix of w: dzf(k) <-> dzf(k+1)
+#   M11 eddy_viscosity(), x-line averaging: c_s(j,k) written to row ny-1-j
+#   M12 eddy_viscosity(), total-viscosity clip: floor -nu/2 instead of -nu                    (reading S14)
+# =============================================================================================================
+def np_metrics(S):
+    """z metrics recomputed from the faces alone: zc, dzf[0..nz-1], dzc[-1..nz-1] stored at index k+1 (mirrored ghost
+    centre at the walls: dzc[-1] = 2 zc[0], dzc[nz-1] = 2 (lz - zc[nz-1]))."""
+    zf = S.zf
+    nz = S.nz
+    zc = 0.5 * (zf[:-1] + zf[1:])
+    dzf = zf[1:] - zf[:-1]
+    dzc = np.empty(nz + 1)
+    dzc[1:nz] = zc[1:] - zc[:-1]
+    dzc[0] = 2.0 * zc[0]
+    dzc[nz] = 2.0 * (S.params["lz"] - zc[-1])
+    return zc, dzf, dzc
+
+
+def np_lzz_matrices(S):
+    """Dense L_zz of SURVEY.md O-step 3/6: (centred family u, v with the no-slip mirror ghost; face family w on the
+    nz-1 interior faces with w = 0 on the wall faces)."""
+    nz = S.nz
+    _, dzf, dzc = np_metrics(S)
+    Lc = np.zeros((nz, nz))
+    for k in range(nz):
+        a = 1.0 / (dzf[k] * dzc[k])          # dzc[k-1] sits at index k
+        c = 1.0 / (dzf[k] * dzc[k + 1])      # dzc[k]
+        Lc[k, k] = -(a + c)
+        if k > 0:
+            Lc[k, k - 1] = a
+        else:
+            Lc[k, k] -= a                    # q[-1] = -q[0]
+        if k < nz - 1:
+            Lc[k, k + 1] = c
+        else:
+            Lc[k, k] -= c
+    m = nz - 1
+    Lw = np.zeros((m, m))
+    for k in range(m):
+        a = 1.0 / (dzc[k + 1] * dzf[k])
+        c = 1.0 / (dzc[k + 1] * dzf[k + 1])
+        Lw[k, k] = -(a + c)
+        if k > 0:
+            Lw[k, k - 1] = a
+        if k < m - 1:
+            Lw[k, k + 1] = c
+    return Lc, Lw
+
+
+def test_tanh_grid_formula(oracle):
+    """Reading S16: zf[k] = lz/2 (1 + tanh(a (2k/nz - 1)) / tanh a), and the worked sizes SURVEY.md quotes for config 3."""
+    S = oracle.Oracle(8, 6, 192, 1.0, 1.0, 2.0, bc_z=1, zstretch=1, zstretch_factor=1.5)
+    k = np.arange(193)
+    zf = 1.0 + np.tanh(1.5 * (2.0 * k / 192 - 1.0)) / math.tanh(1.5)
+    zf[0], zf[-1] = 0.0, 2.0
+    assert np.max(np.abs(S.zf - zf)) < 1e-15
+    zc, dzf, dzc = np_metrics(S)
+    assert np.max(np.abs(S.zc - zc)) < 1e-15 and np.max(np.abs(S.dzf - dzf)) < 1e-15
+    assert np.max(np.abs(np.array([S.dzc(q) for q in range(-1, 192)]) - dzc)) < 1e-15
+    assert abs(dzf[0] - 3.16e-3) < 5e-6 and abs(dzf[96] - 1.73e-2) < 5e-5      # SURVEY.md S16 worked values
+
+
+@pytest.mark.parametrize("comp", ["u", "v", "w"])
+def test_crank_nicolson_dense_matrix_on_tanh_grid(oracle, comp):
+    """Eq. 20-21 on the tanh grid, one component at a time, against numpy.linalg.solve with the dense
+    (1 - c L_zz) built from the faces: a z-only field has no x/y terms and no pressure gradient, so
+    (1 - c L) q* = q + dt alpha R + c L q with R the (separately pinned) advection term, zero for u and v.
+    Kills M9 (u, v) and M10 (w)."""
+    nx, ny, nz, nu, dt = 8, 6, 16, 0.05, 0.02
+    S = oracle.Oracle(nx, ny, nz, 1.0, 1.0, 2.0, bc_z=1, zstretch=1, zstretch_factor=1.5, nu=nu, implicit_z=1, sgs_model=0)
+    Lc, Lw = np_lzz_matrices(S)
+    rng = np.random.default_rng(31)
+    prof = rng.standard_normal(nz)
+    zero = np.zeros(S.shape)
+    ci = "uvw".index(comp)
+    if comp == "w":
+        prof[-1] = 0.0
+    q0 = prof[:, None, None] * np.ones(S.shape)
+    vel = [zero, zero, zero]
+    vel[ci] = q0
+    S.set_velocity(*vel)
+    R = S.advection()[ci][:, 0, 0]
+    assert (comp == "w") == (np.max(np.abs(R)) > 0)
+    al, _, ga = oracle.rk3_coeffs(0)
+    c = ga * nu * dt / 2
+    S.substep(0, dt)
+    got = S.ustar()[ci]
+    if comp == "w":
+        L, n = Lw, nz - 1
+    else:
+        L, n = Lc, nz
+    want = np.linalg.solve(np.eye(n) - c * L, prof[:n] + dt * al * R[:n] + c * (L @ prof[:n]))
+    assert np.max(np.abs(got[:n] - want[:, None, None])) < 1e-13 * np.max(np.abs(want))
+    if comp == "w":
+        assert np.max(np.abs(got[-1])) == 0.0
+    else:
+        # a z-only u or v stays solenoidal: the whole step is the product of the three substep operators
+        S2 = oracle.Oracle(nx, ny, nz, 1.0, 1.0, 2.0, bc_z=1, zstretch=1, zstretch_factor=1.5, nu=nu, implicit_z=1, sgs_model=0)
+        S2.set_velocity(*vel)
+        S2.step(dt)
+        w3 = prof.copy()
+        for rk in range(3):
+            cc = oracle.rk3_coeffs(rk)[2] * nu * dt / 2
+            w3 = np.linalg.solve(np.eye(nz) - cc * Lc, w3 + cc * (Lc @ w3))
+        assert np.max(np.abs(S2.velocity()[ci] - w3[:, None, None])) < 1e-13 * np.max(np.abs(w3))
+
+
+def np_pad_velocity(S, u, v, w):
+    """One ghost layer around u, v, w for a box with no-slip walls (no wall model), written independently of the oracle:
+    z first, then x, then y.  No-slip: wall-parallel ghost = -interior; wall-normal faces on and beyond a wall are 0."""
+    P = S.params
+    def pad(q, kind):
+        q = q.copy()
+        if P["bc_z"] == 1:
+            if kind == 2:
+                q[-1] = 0.0
+                q = np.concatenate([np.zeros_like(q[:1]), q, np.zeros_like(q[:1])], axis=0)
+            else:
+                q = np.concatenate([-q[:1], q, -q[-1:]], axis=0)
+        else:
+            q = np.concatenate([q[-1:], q, q[:1]], axis=0)
+        q = np.concatenate([q[:, :, -1:], q, q[:, :, :1]], axis=2)
+        if P["bc_y"] == 1:
+            if kind == 1:
+                q[:, -1, :] = 0.0
+                q = np.concatenate([np.zeros_like(q[:, :1]), q, np.zeros_like(q[:, :1])], axis=1)
+            else:
+                q = np.concatenate([-q[:, :1], q, -q[:, -1:]], axis=1)
+        else:
+            q = np.concatenate([q[:, -1:], q, q[:, :1]], axis=1)
+        return q
+    return pad(u, 0), pad(v, 1), pad(w, 2)
+
+
+def np_diffusion(S, u, v, w):
+    """nu L_jj u_i of Eq. 16, x-y part and z part separately, from the plain stencils of SURVEY.md O-step 3."""
+    nu, dx, dy = S.params["nu"], S.dx, S.dy
+    _, dzf, dzc = np_metrics(S)
+    nz = S.nz
+    if S.params["bc_z"] == 0:
+        dzc = np.full(nz + 1, dzf[0])
+    dzf_g = np.concatenate([dzf[:1], dzf, dzf[-1:]])            # dzf[-1 .. nz]
+    I = (slice(1, -1),) * 3
+    out_xy, out_z = [], []
+    for kind, q in enumerate(np_pad_velocity(S, u, v, w)):
+        c = q[I]
+        lxy = (q[1:-1, 1:-1, 2:] - 2 * c + q[1:-1, 1:-1, :-2]) / dx ** 2 + (q[1:-1, 2:, 1:-1] - 2 * c + q[1:-1, :-2, 1:-1]) / dy ** 2
+        up, dn = q[2:, 1:-1, 1:-1] - c, c - q[:-2, 1:-1, 1:-1]
+        if kind < 2:
+            lz = (up / dzc[1:, None, None] - dn / dzc[:-1, None, None]) / dzf[:, None, None]
+        else:
+            lz = (up / dzf_g[2:, None, None] - dn / dzf_g[1:-1, None, None]) / dzc[1:, None, None]
+        if kind == 1 and S.params["bc_y"] == 1:
+            lxy[:, -1, :] = 0.0; lz[:, -1, :] = 0.0
+        if kind == 2 and S.params["bc_z"] == 1:
+            lxy[-1] = 0.0; lz[-1] = 0.0
+        out_xy.append(nu * lxy); out_z.append(nu * lz)
+    return out_xy, out_z
+
+
+@pytest.mark.parametrize("bcs,stretch", CASES)
+def test_diffusion_vs_numpy_stencil(oracle, bcs, stretch):
+    """Eq. 16 term by term on every BC combination, uniform and tanh z, all three components (kills M8 and its v, w
+    siblings: every metric of the z part is distinct on the tanh grid)."""
+    S = make(oracle, 12, 8, 10, bcs, stretch, nu=0.37)
+    rng = np.random.default_rng(17)
+    u, v, w = (rng.standard_normal(S.shape) for _ in range(3))
+    if bcs[1] == 1:
+        w[-1] = 0.0
+    if bcs[0] == 1:
+        v[:, -1, :] = 0.0
+    S.set_velocity(u, v, w)
+    want_xy, want_z = np_diffusion(S, u, v, w)
+    for got, want in ((S.diffusion(1), want_xy), (S.diffusion(2), want_z)):
+        for g, e in zip(got, want):
+            assert np.max(np.abs(g - e)) < 1e-12 * np.max(np.abs(e))
+    for g, a, b in zip(S.diffusion(0), want_xy, want_z):
+        assert np.max(np.abs(g - (a + b))) < 1e-12 * np.max(np.abs(a + b))
+
+
+def test_sgs_with_constant_viscosity_is_the_laplacian_on_stretched_z(oracle):
+    """P9 'also on stretched z': with nu_t = const the SGS term equals nu_t L u_i + nu_t d_i(div u), i.e. nu_t L u_i on a
+    projected field -- the discrete operators commute on the tanh grid too.  Away from the walls only: there the
+    nu_t ghost (reading S7) makes the edge viscosity vanish."""
+    S = make(oracle, 12, 8, 14, (0, 1), True, nu=0.7, sgs_model=1)
+    random_solenoidal(S)
+    S.set(S.NUT, np.full(S.shape, 0.7))
+    for a, b in zip(S.sgs_term(), S.diffusion(0)):
+        assert np.max(np.abs(a[1:-2] - b[1:-2])) < 1e-11 * np.max(np.abs(b))
+    assert np.max(np.abs(S.sgs_term()[0][0] - S.diffusion(0)[0][0])) > 1e-3      # and the wall rows do differ
+
+
+@pytest.mark.parametrize("bcs", [(0, 1), (1, 1)])
+def test_pressure_update_eq22_on_tanh_grid(oracle, bcs):
+    """Eq. 22: with implicit z the pressure increment of a substep is phi - c L_zz phi, c = gamma nu dt/2.
+    phi is rebuilt outside the step from u* (oracle hook) with a numpy divergence and the (pinned) Poisson solve;
+    L_zz phi is the numpy stencil with the Neumann closure.  Kills M7."""
+    nu, dt = 0.05, 5e-3
+    S = make(oracle, 12, 8, 10, bcs, True, nu=nu, implicit_z=1, sgs_model=0)
+    random_solenoidal(S, seed=41)
+    _, dzf, dzc = np_metrics(S)
+    p_old = S.get(S.P)
+    assert np.max(np.abs(p_old)) == 0.0
+    for rk in (0, 1):
+        S.substep(rk, dt)
+        ga = oracle.rk3_coeffs(rk)[2]
+        us, vs, ws = S.ustar()
+        um = np.roll(us, 1, 2)
+        vm = np.roll(vs, 1, 1)
+        if bcs[0] == 1:
+            vm[:, 0, :] = 0.0
+        wm = np.roll(ws, 1, 0); wm[0] = 0.0
+        f = ((us - um) / S.dx + (vs - vm) / S.dy + (ws - wm) / dzf[:, None, None]) / (ga * dt)
+        phi = S.poisson_solve(f)
+        e = np.concatenate([phi[:1], phi, phi[-1:]], axis=0)
+        lzz = ((e[2:] - e[1:-1]) / dzc[1:, None, None] - (e[1:-1] - e[:-2]) / dzc[:-1, None, None]) / dzf[:, None, None]
+        c = ga * nu * dt / 2
+        p_new = S.get(S.P)
+        want = phi - c * lzz
+        assert np.max(np.abs((p_new - p_old) - want)) < 1e-11 * np.max(np.abs(want))
+        assert np.max(np.abs(c * lzz)) > 1e-5 * np.max(np.abs(phi))      # the Eq. 22 term is 1e6 x the tolerance here
+        p_old = p_new
+
+
+def test_dynamic_coefficient_per_x_line_vs_dense_bruteforce(oracle):
+    """Eq. 6 averaged along x only (duct): c_s(j,k) = sum_i L:M / sum_i M:M from the independent dense
+    evaluation, on a field with no symmetry in y.  Kills M11."""
+    S = oracle.Oracle(8, 6, 4, 2.0, 3.0, 1.0, bc_y=0, bc_z=0, sgs_model=2, dsm_avg_xy_plane=0, dsm_clip_total=1, nu=1e3)
+    u, v, w = random_solenoidal(S, seed=23)
+    nut = S.eddy_viscosity(u, v, w)
+    lm, mm, d2, mag = np_dsm_periodic(S, u, v, w, pointwise=True)
+    cs = lm.sum(axis=2) / mm.sum(axis=2)
+    got = S.get_cs().reshape(S.nz, S.ny)
+    assert rel(got, cs) < 1e-11
+    assert rel(got[:, ::-1], cs) > 1e-2                               # not y-symmetric: a mirrored row index would show
+    assert rel(nut, cs[:, :, None] * d2 * mag) < 1e-11                # nu = 1e3: the floor -nu never binds here
+
+
+def test_total_viscosity_clip_floor_binds(oracle):
+    """Reading S14, second mode (BASELINE config 4: nu + nu_t >= 0): nu_t = max(c_s Delta^2 |S|, -nu) with nu so small that
+    the floor binds at some points and not at others.  Expected values from the dense evaluation.  Kills M12."""
+    nu = 2e-3
+    S = oracle.Oracle(8, 6, 4, 2.0, 3.0, 1.0, bc_y=0, bc_z=0, sgs_model=2, dsm_avg_xy_plane=0, dsm_clip_total=1, nu=nu)
+    u, v, w = random_solenoidal(S, seed=23)
+    nut = S.eddy_viscosity(u, v, w)
+    lm, mm, d2, mag = np_dsm_periodic(S, u, v, w, pointwise=True)
+    raw = (lm.sum(axis=2) / mm.sum(axis=2))[:, :, None] * d2 * mag
+    bound = raw < -nu
+    assert bound.any() and (raw[~bound] < 0).any() and (raw > 0).any()
+    assert np.max(np.abs(nut - np.maximum(raw, -nu))) < 1e-11 * np.max(np.abs(raw))
+    assert np.all(nut[bound] == -nu)
+    # same rule next to walls (duct): expected from the oracle's own c_s and |S|, both pinned elsewhere
+    D = make(oracle, 12, 8, 10, (1, 1), False, sgs_model=2, dsm_avg_xy_plane=0, dsm_clip_total=1, nu=nu)
+    u, v, w = random_solenoidal(D, seed=4)
+    nut = D.eddy_viscosity(u, v, w)
+    D.set_velocity(u, v, w)
+    _, mag = D.strain()
+    d2 = ((D.dx * D.dy * D.dzf) ** (2.0 / 3.0))[:, None, None]
+    raw = D.get_cs().reshape(D.nz, D.ny)[:, :, None] * d2 * mag
+    assert (raw < -nu).any()
+    assert np.max(np.abs(nut - np.maximum(raw, -nu))) < 1e-12 * np.max(np.abs(raw))
+
+
+def np_advection(S, u, v, w):
+    """-d_j(u_i u_j) in divergence form on the staggered grid, written with shifted
+    views of the padded arrays: arithmetic means (1/2, 1/2) everywhere, except that in the x/y fluxes of the w equation
+    the advecting velocity is the dzf-weighted mean across the face (reading S3)."""
+    dx, dy = S.dx, S.dy
+    nz, ny, nx = S.shape
+    _, dzf, dzc = np_metrics(S)
+    if S.params["bc_z"] == 0:
+        dzc = np.full(nz + 1, dzf[0])
+    dzf_g = np.concatenate([dzf[-1:] if S.params["bc_z"] == 0 else dzf[:1], dzf, dzf[:1] if S.params["bc_z"] == 0 else dzf[-1:]])
+    U, V, W = np_pad_velocity(S, u, v, w)
+    def sh(q, di=0, dj=0, dk=0):
+        return q[1 + dk:1 + dk + nz, 1 + dj:1 + dj + ny, 1 + di:1 + di + nx]
+    av2 = lambda a, b: 0.5 * (a + b)
+    f0 = dzf[:, None, None]; f1 = dzf_g[2:, None, None]; c2 = 2.0 * dzc[1:, None, None]
+    # u
+    au = -((av2(sh(U), sh(U, 1)) ** 2 - av2(sh(U, -1), sh(U)) ** 2) / dx
+           + (av2(sh(U), sh(U, 0, 1)) * av2(sh(V), sh(V, 1)) - av2(sh(U, 0, -1), sh(U)) * av2(sh(V, 0, -1), sh(V, 1, -1))) / dy
+           + (av2(sh(U), sh(U, 0, 0, 1)) * av2(sh(W), sh(W, 1)) - av2(sh(U, 0, 0, -1), sh(U)) * av2(sh(W, 0, 0, -1), sh(W, 1, 0, -1))) / f0)
+    # v
+    avv = -((av2(sh(V), sh(V, 1)) * av2(sh(U), sh(U, 0, 1)) - av2(sh(V, -1), sh(V)) * av2(sh(U, -1), sh(U, -1, 1))) / dx
+            + (av2(sh(V), sh(V, 0, 1)) ** 2 - av2(sh(V, 0, -1), sh(V)) ** 2) / dy
+            + (av2(sh(V), sh(V, 0, 0, 1)) * av2(sh(W), sh(W, 0, 1)) - av2(sh(V, 0, 0, -1), sh(V)) * av2(sh(W, 0, 0, -1), sh(W, 0, 1, -1))) / f0)
+    # w: weighted advecting velocities
+    wz = lambda q, di=0, dj=0: (sh(q, di, dj) * f0 + sh(q, di, dj, 1) * f1) / c2
+    aw = -((av2(sh(W), sh(W, 1)) * wz(U) - av2(sh(W, -1), sh(W)) * wz(U, -1)) / dx
+           + (av2(sh(W), sh(W, 0, 1)) * wz(V) - av2(sh(W, 0, -1), sh(W)) * wz(V, 0, -1)) / dy
+           + (av2(sh(W), sh(W, 0, 0, 1)) ** 2 - av2(sh(W, 0, 0, -1), sh(W)) ** 2) / dzc[1:, None, None])
+    if S.params["bc_y"] == 1:
+        avv[:, -1, :] = 0.0
+    if S.params["bc_z"] == 1:
+        aw[-1] = 0.0
+    return au, avv, aw
+
+
+@pytest.mark.parametrize("bcs,stretch", CASES)
+def test_advection_vs_numpy_stencil(oracle, bcs, stretch):
+    """Every coefficient of the advective term, on every BC combination, uniform and tanh z (the conservation pins are
+    blind to a rescaled term; the Taylor-Green pressure check sees it only to 2 %)."""
+    S = make(oracle, 12, 8, 10, bcs, stretch)
+    rng = np.random.default_rng(19)
+    u, v, w = (rng.standard_normal(S.shape) for _ in range(3))
+    if bcs[1] == 1:
+        w[-1] = 0.0
+    if bcs[0] == 1:
+        v[:, -1, :] = 0.0
+    S.set_velocity(u, v, w)
+    for g, e in zip(S.advection(), np_advection(S, u, v, w)):
+        assert np.max(np.abs(g - e)) < 1e-12 * np.max(np.abs(e))
