@@ -178,6 +178,13 @@ int cales_kernel_time(cales_solver* s, int kid, const char** name, double* ms_to
  * timing is on).  on = 0 returns to plain stream launches. */
 int cales_set_graph(cales_solver* s, int on);
 
+/* Kernel-selection knobs, for tests and A/B timing only (results do not depend on them beyond round-off; the defaults are the
+ * measured best): "rhs_tile_min_points" (grids with fewer points run the momentum kernel one thread per point instead of the
+ * staged z-march; default 200000), "smag_tile_min_points" (the same for the static model; default 4000000),
+ * "dsm_col_variant" (0: register-window column march of the dynamic model, 1: the shared-memory-ring form).
+ * CALES_EINVAL on an unknown key or a value out of range. */
+int cales_set_option(cales_solver* s, const char* key, long long value);
+
 /* Number of kernels cales_step launches per call with the current parameters (for bench.py's gpu_launches). */
 int cales_launches_per_step(cales_solver* s);
 

@@ -12,6 +12,7 @@
 #include "cales_rhs_tile.cuh"
 #include "cales_closures.cuh"
 #include "cales_smag_tile.cuh"
+#include "cales_dsm_col.cuh"
 #include "cales_dsm3.cuh"
 #ifndef CALES_D3C_TXB
 #define CALES_D3C_TXB 64
@@ -62,6 +63,7 @@ struct cales_solver {
   bool fresh;
   long long rhs_tile_min;   // below this many points the momentum kernel runs one thread per point
   long long tile_min;   // grids with at least this many points use the staged z-march for the static model
+  int dsm_col_variant;  // 0: register-window column march (k_dsm_col_rw); 1: shared-ring form (k_dsm_col_sm)
   std::vector<double> h_dzf, h_dzc, h_cn; Ctx hc; double cn_dt;   // host copies for the per-dt CN coefficient tables
   int use_graph; cudaGraphExec_t gexec; double gdt;   // the three substeps captured as one CUDA graph, keyed by dt
   int timing; bool ev_valid;
@@ -205,8 +207,7 @@ extern "C" int cales_create(const cales_params* p, cales_solver** out) {
   s->h_dzf = H.dzf; s->h_dzc = H.dzc; s->hc = s->c; s->hc.dzf = s->h_dzf.data() + 1; s->hc.dzc = s->h_dzc.data() + 1; s->cn_dt = 0.0;
   s->tile_min = 4000000;
   s->rhs_tile_min = 200000;
-  if (const char* e = std::getenv("CALES_RHS_TILE_MIN_POINTS")) s->rhs_tile_min = std::atoll(e);   // tests force either path
-  if (const char* e = std::getenv("CALES_TILE_MIN_POINTS")) s->tile_min = std::atoll(e);   // tests force either path
+  s->dsm_col_variant = 0;
   for (int q = 0; q < 32; ++q) { s->kms[q] = 0.0; s->kcnt[q] = 0; }
   *out = s;
   return CALES_OK;
@@ -361,8 +362,12 @@ static int run_eddy_viscosity(cales_solver* s, const double* u, const double* v,
     if (!c.dsm_filter3d && (!ywall || split)) {
       const int jlo = ywall ? DSM_TY : 0, jhi = ywall ? c.ny - DSM_TY : c.ny;
       dim3 grid(ds.nbx, (jhi - jlo + DSMC_LY - 1) / DSMC_LY, c.nz);
-      // <threads, min CTAs/SM, quantities with a register window>: measured on B200, (64, 6, 0) within 4 % of the best
-      k_dsm_col_sm<64, 6, 0><<<dim3(ds.nbx, grid.y, grid.z), 64, 0, s->st>>>(c, u, v, w, jlo, jhi, ds.pslots, s->smag, s->dsm_part);
+      // register-window form (cales_dsm_col.cuh); the shared-ring form of round 1 stays selectable for A/B timing
+      // bulk copies need 16-byte aligned rows: nx is even, so the field pointers decide
+      const bool al16 = (((size_t)u | (size_t)v | (size_t)w) & 15) == 0;
+      if (s->dsm_col_variant == 2 && al16) k_dsm_col_tma<64, CALES_DSMR_MINB><<<dim3(ds.nbx, grid.z, grid.y), 64, 0, s->st>>>(c, u, v, w, jlo, jhi, ds.pslots, s->smag, s->dsm_part);
+      else if (s->dsm_col_variant != 1) k_dsm_col_rw<64, CALES_DSMR_MINB><<<dim3(ds.nbx, grid.z, grid.y), 64, 0, s->st>>>(c, u, v, w, jlo, jhi, ds.pslots, s->smag, s->dsm_part);
+      else k_dsm_col_sm<64, 6, 0><<<dim3(ds.nbx, grid.y, grid.z), 64, 0, s->st>>>(c, u, v, w, jlo, jhi, ds.pslots, s->smag, s->dsm_part);
       LAUNCH_TRY(K_DSM_COL);
     }
     k_dsm_coef<<<s->c.nz, 128, 0, s->st>>>(s->c, s->dsm_part, ds.pslots, s->dsm_cs);
@@ -476,6 +481,18 @@ extern "C" int cales_set_graph(cales_solver* s, int on) {
   if (!s) return fail(CALES_EINVAL, "null solver");
   s->use_graph = on ? 1 : 0;
   if (!on && s->gexec) { cudaGraphExecDestroy(s->gexec); s->gexec = nullptr; }
+  return CALES_OK;
+}
+
+// Kernel-selection knobs for tests and A/B timing (the defaults are the measured best).
+extern "C" int cales_set_option(cales_solver* s, const char* key, long long value) {
+  if (!s || !key) return fail(CALES_EINVAL, "null argument");
+  const std::string k(key);
+  if (k == "rhs_tile_min_points") s->rhs_tile_min = value;
+  else if (k == "smag_tile_min_points") s->tile_min = value;
+  else if (k == "dsm_col_variant") { if (value < 0 || value > 2) return fail(CALES_EINVAL, "dsm_col_variant must be 0, 1 or 2"); s->dsm_col_variant = (int)value; }
+  else return fail(CALES_EINVAL, "unknown option: " + k);
+  if (s->gexec) { cudaGraphExecDestroy(s->gexec); s->gexec = nullptr; }      // the captured step holds the old selection
   return CALES_OK;
 }
 

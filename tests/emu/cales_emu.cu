@@ -12,6 +12,7 @@
 #include "../../paper_2411_09364_b200/csrc/cales_momentum.cuh"
 #include "../../paper_2411_09364_b200/csrc/cales_rhs_tile.cuh"
 #include "../../paper_2411_09364_b200/csrc/cales_smag_tile.cuh"
+#include "../../paper_2411_09364_b200/csrc/cales_dsm_col.cuh"
 #include "../../paper_2411_09364_b200/csrc/cales_dsm3.cuh"
 
 #include <cstring>
@@ -271,28 +272,44 @@ static void emu_nut(emu_solver* s, const double* u, const double* v, const doubl
       }
     }
   }
-  if (!c.dsm_filter3d && (!ywall || split)) {   // column-marching kernel, stepped row by row with the block barrier between the phases
+  if (!c.dsm_filter3d && (!ywall || split)) {   // k_dsm_col_rw: stepped row by row with the block barrier between the phases; one register window per emulated thread
     const int T = dsh.txb, jlo = ywall ? DSM_TY : 0, jhi = ywall ? c.ny - DSM_TY : c.ny;
     std::vector<double> sh(2 * DSMC_NB * T), breg((size_t)T * DSMC_NB);
-    std::vector<double> ring(2 * DSMC_NQ * T), smprev(T);
+    std::vector<DsmrWin> win(T);
     for (int k = 0; k < c.nz; ++k) for (int by = 0; by * DSMC_LY < jhi - jlo; ++by) for (int bx = 0; bx < dsh.nbx; ++bx) {
       const int i0 = bx * (T - 2), j0 = jlo + by * DSMC_LY, jend = std::min(j0 + DSMC_LY, jhi), nrows = jend - j0 + 2;
-      std::fill(ring.begin(), ring.end(), 0.0); std::fill(smprev.begin(), smprev.end(), 0.0);
+      const double d2 = c.delta[k] * c.delta[k], a2 = c.alpha * c.alpha;
+      for (int t = 0; t < T; ++t) dsmr_win_init(win[t]);
+      std::vector<double> accl(T / 32, 0.0), accm(T / 32, 0.0);
       for (int r = 0; r < nrows; ++r) {
         int gj = j0 - 1 + r; gj = gj < 0 ? gj + c.ny : (gj >= c.ny ? gj - c.ny : gj);
         double* buf = sh.data() + (r & 1) * DSMC_NB * T;
-        for (int t = 0; t < T; ++t) dsmc_phaseA(c, u, v, w, T, t, i0, gj, k, buf, &breg[(size_t)t * DSMC_NB]);
+        for (int t = 0; t < T; ++t) {
+          const int gw = (((i0 - 1 + t) % c.nx) + c.nx) % c.nx;
+          dsmr_base(c, u, v, w, gw, gj, k, &breg[(size_t)t * DSMC_NB]);
+          for (int q = 0; q < DSMC_NB; ++q) buf[q * T + t] = breg[(size_t)t * DSMC_NB + q];
+        }
         std::vector<double> wl(T / 32, 0.0), wm(T / 32, 0.0);
-        for (int t = 1; t <= T - 2; ++t) {
-          double lm = 0.0, mm = 0.0, sg = 0.0;
-          double wnone[1]; const bool done = dsmc_phaseB_sm<0>(c, T, t, r, k, buf, &breg[(size_t)t * DSMC_NB], ring.data(), wnone, &smprev[t], &lm, &mm, &sg);
+        for (int t = 0; t < T; ++t) {
+          double lm = 0.0, mm = 0.0;
+          const bool inner = t >= 1 && t <= T - 2, emit = r >= 2;
+          if (inner) {
+            if (r & 1) dsmr_row<1>(buf, T, t, &breg[(size_t)t * DSMC_NB], win[t], emit, d2, a2, &lm, &mm);
+            else dsmr_row<0>(buf, T, t, &breg[(size_t)t * DSMC_NB], win[t], emit, d2, a2, &lm, &mm);
+          }
           const int gi = i0 - 1 + t;
-          if (r >= 2 && done && gi < c.nx) { s->smag[idx3(c, gi, j0 + r - 2, k)] = sg; wl[t >> 5] += lm; wm[t >> 5] += mm; }
+          if (emit && inner && gi < c.nx) { s->smag[idx3(c, gi, j0 + r - 2, k)] = win[t].smag_prev; wl[t >> 5] += lm; wm[t >> 5] += mm; }
+          win[t].smag_prev = breg[(size_t)t * DSMC_NB + 9];
         }
         if (r >= 2) for (int wq = 0; wq < T / 32; ++wq) {
           const long long slot = ((long long)k * c.ny + (j0 + r - 2)) * ntx + bx * (T / 32) + wq;
-          s->dsm_part[slot * 2] = wl[wq]; s->dsm_part[slot * 2 + 1] = wm[wq];
+          if (c.dsm_plane) { accl[wq] += wl[wq]; accm[wq] += wm[wq]; s->dsm_part[slot * 2] = 0.0; s->dsm_part[slot * 2 + 1] = 0.0; }
+          else { s->dsm_part[slot * 2] = wl[wq]; s->dsm_part[slot * 2 + 1] = wm[wq]; }
         }
+      }
+      if (c.dsm_plane) for (int wq = 0; wq < T / 32; ++wq) {
+        const long long slot = ((long long)k * c.ny + j0) * ntx + bx * (T / 32) + wq;
+        s->dsm_part[slot * 2] = accl[wq]; s->dsm_part[slot * 2 + 1] = accm[wq];
       }
     }
   }

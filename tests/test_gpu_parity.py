@@ -290,12 +290,12 @@ def test_cuda_graph_replay_is_bit_identical(oracle, gpu):
 
 
 @pytest.mark.parametrize("n,shape", [(1, (48, 24, 20)), (3, (72, 36, 40)), (2, (72, 48, 24))])
-def test_static_model_staged_kernel_parity(oracle, gpu, n, shape, monkeypatch):
+def test_static_model_staged_kernel_parity(oracle, gpu, n, shape):
     """k_smag_tile (the staged z-march used on HBM-sized grids) forced on at test sizes."""
-    monkeypatch.setenv("CALES_TILE_MIN_POINTS", "0")
     cfg, kw, (u, v, w), dt = pc.prepare(oracle, n, shape)
     o = pc.make(oracle.Oracle, kw)
     g = pc.make(gpu.Solver, kw)
+    g.set_option("smag_tile_min_points", 0)
     o.set_velocity(u, v, w); g.set_velocity(u, v, w)
     a, b = g.eddy_viscosity().cpu().numpy(), o.eddy_viscosity()
     assert np.max(np.abs(a - b)) <= 1e-11 * max(np.max(np.abs(b)), kw["nu"])
@@ -325,18 +325,38 @@ def test_cfl_dt_and_plane_stats_parity(oracle, gpu, n, shape):
 
 @pytest.mark.parametrize("min_points", ["0", "1000000000"])
 @pytest.mark.parametrize("n,shape", [(1, (48, 24, 20)), (2, (72, 48, 24)), (4, (96, 36, 24))])
-def test_momentum_kernel_both_forms_parity(oracle, gpu, n, shape, min_points, monkeypatch):
+def test_momentum_kernel_both_forms_parity(oracle, gpu, n, shape, min_points):
     """The staged z-marching momentum kernel (min_points = 0) and the one-thread-per-point form used on launch-bound
     grids (min_points huge), each forced on at test sizes."""
-    monkeypatch.setenv("CALES_RHS_TILE_MIN_POINTS", min_points)
     cfg, kw, (u, v, w), dt = pc.prepare(oracle, n, shape)
     o = pc.make(oracle.Oracle, kw)
     g = pc.make(gpu.Solver, kw)
+    g.set_option("rhs_tile_min_points", int(min_points))
     o.set_velocity(u, v, w); g.set_velocity(u, v, w)
-    for _ in range(2):
+    for s in range(2):
         o.step(dt); g.step(dt)
+        err = pc.field_errors(_gpu_fields(g), [o.get(f) for f in range(5)], o.dzf, kw["nu"])
+        assert max(err.values()) <= (TOL_1STEP if s == 0 else 1e-10), (s, err)
+    g.close()
+
+
+@pytest.mark.parametrize("variant", [0, 1, 2])
+@pytest.mark.parametrize("n,shape", [(5, (144, 72, 24)), (4, (128, 48, 20))])
+def test_dynamic_model_column_kernels_parity(oracle, gpu, n, shape, variant):
+    """Both forms of the column march of the dynamic model (register window / shared-memory ring): nu_t and the coefficient
+    against the oracle on grids spanning several 62-column blocks with a ragged tail and more than one 32-row band."""
+    cfg, kw, (u, v, w), dt = pc.prepare(oracle, n, shape)
+    o = pc.make(oracle.Oracle, kw)
+    g = pc.make(gpu.Solver, kw)
+    g.set_option("dsm_col_variant", variant)
+    o.set_velocity(u, v, w); g.set_velocity(u, v, w)
+    a, b = g.eddy_viscosity().cpu().numpy(), o.eddy_viscosity()
+    assert np.max(np.abs(a - b)) <= 1e-11 * max(np.max(np.abs(b)), kw["nu"])
+    ca, cb = g.get_cs(bool(kw["dsm_avg_xy_plane"])).cpu().numpy(), o.get_cs()
+    assert np.max(np.abs(ca - cb)) <= 1e-10 * np.max(np.abs(cb))
+    o.step(dt); g.step(dt)
     err = pc.field_errors(_gpu_fields(g), [o.get(f) for f in range(5)], o.dzf, kw["nu"])
-    assert max(err.values()) <= 1e-10, err
+    assert max(err.values()) <= TOL_1STEP, err
     g.close()
 
 
