@@ -181,7 +181,8 @@ int cales_set_graph(cales_solver* s, int on);
 /* Kernel-selection knobs, for tests and A/B timing only (results do not depend on them beyond round-off; the defaults are the
  * measured best): "rhs_tile_min_points" (grids with fewer points run the momentum kernel one thread per point instead of the
  * staged z-march; default 200000), "smag_tile_min_points" (the same for the static model; default 4000000),
- * "dsm_col_variant" (0: register-window column march of the dynamic model, 1: the shared-memory-ring form).
+ * "dsm_col_variant" (column march of the dynamic model -- 0: register window, rows staged by TMA bulk copies; 1: the
+ * shared-memory-ring form; 2: register window, direct loads).
  * CALES_EINVAL on an unknown key or a value out of range. */
 int cales_set_option(cales_solver* s, const char* key, long long value);
 

@@ -63,7 +63,7 @@ struct cales_solver {
   bool fresh;
   long long rhs_tile_min;   // below this many points the momentum kernel runs one thread per point
   long long tile_min;   // grids with at least this many points use the staged z-march for the static model
-  int dsm_col_variant;  // 0: register-window column march (k_dsm_col_rw); 1: shared-ring form (k_dsm_col_sm)
+  int dsm_col_variant;  // 0: TMA-staged register-window column march (k_dsm_col_tma); 1: shared-ring form of round 1 (k_dsm_col_sm); 2: direct loads (k_dsm_col_rw)
   std::vector<double> h_dzf, h_dzc, h_cn; Ctx hc; double cn_dt;   // host copies for the per-dt CN coefficient tables
   int use_graph; cudaGraphExec_t gexec; double gdt;   // the three substeps captured as one CUDA graph, keyed by dt
   int timing; bool ev_valid;
@@ -363,10 +363,15 @@ static int run_eddy_viscosity(cales_solver* s, const double* u, const double* v,
       const int jlo = ywall ? DSM_TY : 0, jhi = ywall ? c.ny - DSM_TY : c.ny;
       dim3 grid(ds.nbx, (jhi - jlo + DSMC_LY - 1) / DSMC_LY, c.nz);
       // register-window form (cales_dsm_col.cuh); the shared-ring form of round 1 stays selectable for A/B timing
-      // bulk copies need 16-byte aligned rows: nx is even, so the field pointers decide
-      const bool al16 = (((size_t)u | (size_t)v | (size_t)w) & 15) == 0;
-      if (s->dsm_col_variant == 2 && al16) k_dsm_col_tma<64, CALES_DSMR_MINB><<<dim3(ds.nbx, grid.z, grid.y), 64, 0, s->st>>>(c, u, v, w, jlo, jhi, ds.pslots, s->smag, s->dsm_part);
-      else if (s->dsm_col_variant != 1) k_dsm_col_rw<64, CALES_DSMR_MINB><<<dim3(ds.nbx, grid.z, grid.y), 64, 0, s->st>>>(c, u, v, w, jlo, jhi, ds.pslots, s->smag, s->dsm_part);
+      // variant 0 (default): TMA-staged march on the planes without z-wall ghosts, the direct-load march on the others;
+      // bulk copies need 16-byte aligned rows (nx is even, so the field pointers decide) and nx >= 66
+      const bool tma_ok = s->dsm_col_variant == 0 && (((size_t)u | (size_t)v | (size_t)w) & 15) == 0 && c.nx >= 66;
+      const unsigned nby = grid.y;
+      if (tma_ok) {
+        const int klo = c.bc_z == BC_PER ? 0 : 1, khi = c.bc_z == BC_PER ? c.nz : c.nz - 1;
+        k_dsm_col_tma<64, CALES_DSMR_MINB><<<dim3(ds.nbx, khi - klo, nby), 64, 0, s->st>>>(c, u, v, w, klo, jlo, jhi, ds.pslots, s->smag, s->dsm_part);
+        if (klo > 0) { LAUNCH_TRY(K_DSM_COL); k_dsm_col_rw<64, CALES_DSMR_MINB><<<dim3(ds.nbx, 2, nby), 64, 0, s->st>>>(c, u, v, w, 0, c.nz - 1, jlo, jhi, ds.pslots, s->smag, s->dsm_part); }
+      } else if (s->dsm_col_variant != 1) k_dsm_col_rw<64, CALES_DSMR_MINB><<<dim3(ds.nbx, c.nz, nby), 64, 0, s->st>>>(c, u, v, w, 0, 1, jlo, jhi, ds.pslots, s->smag, s->dsm_part);
       else k_dsm_col_sm<64, 6, 0><<<dim3(ds.nbx, grid.y, grid.z), 64, 0, s->st>>>(c, u, v, w, jlo, jhi, ds.pslots, s->smag, s->dsm_part);
       LAUNCH_TRY(K_DSM_COL);
     }
@@ -503,7 +508,8 @@ extern "C" int cales_launches_per_step(cales_solver* s) {
             1 /*static nu_t or fill*/;
   if (c.sgs == CALES_SGS_DSMAG) {
     const bool ywall = c.bc_y == BC_WALL, split = ywall && c.ny >= 3 * DSM_TY;
-    int pass1 = (ywall ? 1 : 0) + ((!ywall || split) ? 1 : 0);
+    const int ncol = (s->dsm_col_variant == 0 && c.nx >= 66 && c.bc_z == BC_WALL) ? 2 : 1;   // staged march + the two wall planes
+    int pass1 = (ywall ? 1 : 0) + ((!ywall || split) ? ncol : 0);
     if (c.dsm_filter3d) {
       const D3Split sp = d3_split(c, s->P.zstretch == CALES_Z_UNIFORM);
       pass1 = sp.col ? 1 + (sp.klo > 0 ? 1 : 0) + (sp.jlo > 0 ? 1 : 0) : 1;

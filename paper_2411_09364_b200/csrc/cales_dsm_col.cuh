@@ -94,8 +94,9 @@ CALES_HD void dsmr_row(const double* shbuf, int txb, int t, const double* b, Dsm
       const double l = sl[(3 + m) * txb], r = sr[(3 + m) * txb], cc = b[3 + m];
       const double xs = (l + r) + 2.0 * cc;
       const double xp = mc2 * cc + (ml * l + mr * r);
-      St[m] = (w2[15 + m] + xs) + 2.0 * w1[15 + m]; w2[15 + m] = xs;
-      Mp[m] = (w2[9 + m] + xp) + 2.0 * w1[9 + m]; w2[9 + m] = xp;
+      // old window value consumed first, so the new one can be formed in its register (no moves at the loop's merge points)
+      const double ts = w2[15 + m] + 2.0 * w1[15 + m]; w2[15 + m] = xs; St[m] = ts + xs;
+      const double tp = w2[9 + m] + 2.0 * w1[9 + m]; w2[9 + m] = xp; Mp[m] = tp + xp;
     }
   }
   double md = 0.0, mo = 0.0;
@@ -110,7 +111,7 @@ CALES_HD void dsmr_row(const double* shbuf, int txb, int t, const double* b, Dsm
   const double ul = sl[0], ur = sr[0], vl = sl[txb], vr = sr[txb], wl = sl[2 * txb], wr = sr[2 * txb];
   const double uc = b[0], vc = b[1], wc = b[2], uc2 = 2.0 * uc, vc2 = 2.0 * vc, wc2 = 2.0 * wc;
   double x, Fu, Fv, Fw, ld = 0.0, lo = 0.0;
-#define DSMR_PUSH(m, expr) x = (expr); const double F##m = (w2[m] + x) + 2.0 * w1[m]; w2[m] = x;
+#define DSMR_PUSH(m, expr) x = w2[m] + 2.0 * w1[m]; w2[m] = (expr); const double F##m = x + w2[m];
   DSMR_PUSH(0, (ul + ur) + uc2) Fu = F0;
   DSMR_PUSH(1, (vl + vr) + vc2) Fv = F1;
   DSMR_PUSH(2, (wl + wr) + wc2) Fw = F2;
@@ -128,15 +129,16 @@ CALES_HD void dsmr_row(const double* shbuf, int txb, int t, const double* b, Dsm
 }
 
 #ifdef __CUDACC__
-// grid (ceil(nx/(TXB-2)), nz, ceil((jhi-jlo)/DSMC_LY)), block TXB (multiple of 32).  Output rows [jlo, jhi).
+// grid (ceil(nx/(TXB-2)), planes, ceil((jhi-jlo)/DSMC_LY)), block TXB (multiple of 32).  Planes k0 + blockIdx.y * kstride,
+// output rows [jlo, jhi).
 // part: [k][j][pslots][2]; this kernel fills slots blockIdx.x*(TXB/32) + warp of its rows: per row with x-line averaging, the
 // CTA's total in its first row (zeros in the others) with plane averaging.
 template <int TXB, int MINB>
 __global__ void __launch_bounds__(TXB, MINB) k_dsm_col_rw(const __grid_constant__ Ctx c, const double* __restrict__ u, const double* __restrict__ v,
-                                                          const double* __restrict__ w, int jlo, int jhi, int pslots, double* __restrict__ smag,
-                                                          double* __restrict__ part) {
+                                                          const double* __restrict__ w, int k0, int kstride, int jlo, int jhi, int pslots,
+                                                          double* __restrict__ smag, double* __restrict__ part) {
   __shared__ double sh[2][DSMC_NB * TXB];
-  const int t = threadIdx.x, k = blockIdx.y;
+  const int t = threadIdx.x, k = k0 + blockIdx.y * kstride;
   const int i0 = blockIdx.x * (TXB - 2);
   const int j0 = jlo + blockIdx.z * DSMC_LY;
   const int jend = min(j0 + DSMC_LY, jhi);
@@ -202,121 +204,126 @@ __global__ void __launch_bounds__(TXB, MINB) k_dsm_col_rw(const __grid_constant_
 }
 
 // ---- the same march with the raw velocity rows staged by the TMA engine ---------------------------------------------------
-// ncu on k_dsm_col_rw (profiles/r2_ncu_dsm.md): the fp64 pipe is busy a third of the time and the warps wait on global loads
-// (long scoreboard) -- 30 strided loads per point, half of them L1 misses, with 8-12 warps per SM to hide them.  Here one
-// thread per CTA keeps a ring of DSMT_NS raw ROWS in shared memory, DSMT_NL = 8 lines each (u on planes k-1, k, k+1; v on
-// k-1, k, k+1; w on k-1, k), filled by cp.async.bulk (UBLKCP) copies that complete on an mbarrier DSMT_NS-3 rows ahead of
-// their first use; periodic wrap in x splits a line into two copies, wrap in y / z is address arithmetic of the issuing
-// thread.  The strain stencil then reads shared memory only.  Planes next to a z wall (wall ghosts) take the direct path.
-#ifndef CALES_DSMT_NS
-#define CALES_DSMT_NS 6
-#endif
-enum { DSMT_NS = CALES_DSMT_NS, DSMT_NL = 8 };
+// ncu on k_dsm_col_rw (profiles/r2_ncu_dsm.md): 577 instructions per warp and row of which only 219 are fp64 -- the rest is
+// 64-bit address arithmetic of 30 strided loads per point, wrap selects and branches -- and the warps wait on those loads.
+// Here eight lanes keep a ring of DSMT_NS = 4 raw ROWS in shared memory, DSMT_NL = 8 lines each (u on planes k-1, k, k+1; v on
+// k-1, k, k+1; w on k-1, k), filled by cp.async.bulk (UBLKCP) copies that complete on an mbarrier two rows ahead of their
+// first use: each producer lane issues one line, periodic wrap in x splits a line into two copies, wrap in y / z is pointer arithmetic of
+// the issuing lane.  The row loop is unrolled by four, so ring slots and window parity are compile-time and the strain
+// stencil is 30 shared-memory loads at immediate offsets.  Planes next to a z wall (wall ghosts) are left to k_dsm_col_rw.
+enum { DSMT_NS = 4, DSMT_NL = 8 };
 
+// grid (ceil(nx/(TXB-2)), khi-klo, ceil((jhi-jlo)/DSMC_LY)), block TXB = 64; planes [klo, khi), output rows [jlo, jhi).
+// Needs nx >= TXB + 2, 16-byte aligned fields, and every base row jlo-1 .. jhi an interior row (periodic y, or 1 <= j <= ny-2).
 template <int TXB, int MINB>
 __global__ void __launch_bounds__(TXB, MINB) k_dsm_col_tma(const __grid_constant__ Ctx c, const double* __restrict__ u, const double* __restrict__ v,
-                                                           const double* __restrict__ w, int jlo, int jhi, int pslots, double* __restrict__ smag,
+                                                           const double* __restrict__ w, int klo, int jlo, int jhi, int pslots, double* __restrict__ smag,
                                                            double* __restrict__ part) {
   constexpr int LW = TXB + 2;                  // columns i0-2 .. i0+TXB-1 of a line
   constexpr int STAGE = DSMT_NL * LW;
   __shared__ __align__(128) double raw[DSMT_NS * STAGE];
   __shared__ double sh[2][DSMC_NB * TXB];
   __shared__ unsigned long long full[DSMT_NS];
-  const int t = threadIdx.x, k = blockIdx.y;
+  const int t = threadIdx.x, k = klo + blockIdx.y;
   const int i0 = blockIdx.x * (TXB - 2);
   const int j0 = jlo + blockIdx.z * DSMC_LY;
   const int jend = min(j0 + DSMC_LY, jhi);
   const int nrows = jend - j0 + 2;             // base rows j0-1 .. jend; raw rows j0-2 .. jend+1 (nrows + 2 of them)
+  const int nraw = nrows + 2;
   const int gi = i0 - 1 + t;
-  const int gw = ((gi % c.nx) + c.nx) % c.nx;
   const bool inner = t >= 1 && t <= TXB - 2;
   const bool outcol = inner && gi < c.nx;
-  const bool staged = c.bc_z == BC_PER || (k >= 1 && k <= c.nz - 2);     // CTA-uniform
   const double d2 = c.delta[k] * c.delta[k], a2 = c.alpha * c.alpha;
-  const double rdzf = c.rdzf[k], rdzc = c.rdzc[k], rdzcm = c.rdzc[k - 1];
-  const long long pslot0 = ((long long)k * c.ny) * pslots + blockIdx.x * (TXB / 32) + (t >> 5);
-  // producer (thread 0): raw row rho (global row j0-2+rho) into slot rho % DSMT_NS
-  auto issue = [&](int rho) {
-    const int slot = rho % DSMT_NS;
-    int gj = j0 - 2 + rho;
-    gj = gj < 0 ? gj + c.ny : (gj >= c.ny ? gj - c.ny : gj);
-    mbar_expect_tx(&full[slot], STAGE * (unsigned)sizeof(double));
+  const double rdx = c.rdx, rdy = c.rdy, rdzf = c.rdzf[k], rdzc = c.rdzc[k], rdzcm = c.rdzc[k - 1];
+  // ---- producer state (lanes 0..7 of warp 0): source pointer of this lane's line at the next raw row, x segments
+  const double* src = nullptr; int gj_next = 0, segA = 0;
+  const bool producer = (t & 31) < DSMT_NL / 2 && t < 64;      // lanes 0..3 of warps 0 and 1: four lines each
+  const int line = (t & 31) + (t >> 5) * (DSMT_NL / 2);
+  if (producer) {
+    const int l = line;
+    const double* f = l < 3 ? u : (l < 6 ? v : w);
     const int km = k == 0 ? c.nz - 1 : k - 1, kp = k == c.nz - 1 ? 0 : k + 1;
+    const int kk = (l == 1 || l == 4 || l == 7) ? k : ((l == 2 || l == 5) ? kp : km);
+    gj_next = j0 - 2; gj_next = gj_next < 0 ? gj_next + c.ny : gj_next;
+    src = f + ((long long)kk * c.ny + gj_next) * c.nx;
     const int cw0 = (((i0 - 2) % c.nx) + c.nx) % c.nx;
-#pragma unroll
-    for (int l = 0; l < DSMT_NL; ++l) {
-      const double* f = l < 3 ? u : (l < 6 ? v : w);
-      const int kk = (l == 1 || l == 4 || l == 7) ? k : ((l == 2 || l == 5) ? kp : km);
-      const double* src = f + ((long long)kk * c.ny + gj) * c.nx;
-      double* dst = raw + slot * STAGE + l * LW;
-      int done = 0, cw = cw0;
-      while (done < LW) {
-        const int len = min(LW - done, c.nx - cw);
-        bulk_g2s(dst + done, src + cw, (unsigned)len * (unsigned)sizeof(double), &full[slot]);
-        done += len; cw = 0;
-      }
-    }
+    segA = min(LW, c.nx - cw0);
+    src += cw0;                                // segment A starts at column cw0, segment B (if any) at column 0 of the row
+  }
+  auto issue = [&](int slot) {                 // next raw row into `slot` (called by the eight producer lanes)
+    unsigned long long* bar = &full[slot];
+    if (t == 0) mbar_expect_tx(bar, STAGE * (unsigned)sizeof(double));
+    double* dst = raw + slot * STAGE + line * LW;
+    bulk_g2s(dst, src, (unsigned)segA * 8u, bar);
+    if (segA < LW) bulk_g2s(dst + segA, src - (c.nx - segA), (unsigned)(LW - segA) * 8u, bar);
+    ++gj_next;
+    if (gj_next == c.ny) { gj_next = 0; src -= (long long)(c.ny - 1) * c.nx; } else src += c.nx;
   };
-  if (staged) {
-    if (t == 0) {
-      for (int s = 0; s < DSMT_NS; ++s) mbar_init(&full[s], 1);
-      mbar_fence_init();
-    }
-    __syncthreads();
-    if (t == 0) for (int rho = 0; rho < DSMT_NS && rho < nrows + 2; ++rho) issue(rho);
+  if (t == 0) {
+#pragma unroll
+    for (int s = 0; s < DSMT_NS; ++s) mbar_init(&full[s], 1);
+    mbar_fence_init();
+  }
+  __syncthreads();
+  if (producer) {
+#pragma unroll
+    for (int s = 0; s < DSMT_NS; ++s) if (s < nraw) issue(s);
   }
   DsmrWin win;
   dsmr_win_init(win);
   double accl = 0.0, accm = 0.0;
-  auto row = [&](auto par, int r) {
-    constexpr int PAR = decltype(par)::value;
+  double* sm_out = smag + idx3(c, gi < c.nx ? gi : 0, j0, k);           // |S| of output row j0, bumped by nx per emitted row
+  long long pslot = ((long long)k * c.ny + j0) * pslots + blockIdx.x * (TXB / 32) + (t >> 5);
+  const double* Rt = raw + t + 1;
+  auto row = [&](auto ph, int r) {
+    constexpr int PH = decltype(ph)::value;    // r & 3
+    constexpr int PAR = PH & 1, S0 = PH, S1 = (PH + 1) & 3, S2 = (PH + 2) & 3;
+    if (r == 0) { mbar_wait(&full[0], 0); mbar_wait(&full[1], 0); }
+    mbar_wait(&full[S2], ((r + 2) >> 2) & 1);
     double b[DSMC_NB];
-    if (staged) {
-      if (r == 0) { mbar_wait(&full[0], 0); mbar_wait(&full[1 % DSMT_NS], 0); }
-      mbar_wait(&full[(r + 2) % DSMT_NS], ((r + 2) / DSMT_NS) & 1);
-      const double* R0 = raw + (r % DSMT_NS) * STAGE + t + 1;            // raw row of base row - 1
-      const double* R1 = raw + ((r + 1) % DSMT_NS) * STAGE + t + 1;      // the base row
-      const double* R2 = raw + ((r + 2) % DSMT_NS) * STAGE + t + 1;      // base row + 1
+    {
+      const double* R0 = Rt + S0 * STAGE;      // raw row below the base row
+      const double* R1 = Rt + S1 * STAGE;      // the base row
+      const double* R2 = Rt + S2 * STAGE;      // the row above
       auto U = [&](int a, int bb, int d) { return (bb < 0 ? R0 : (bb > 0 ? R2 : R1))[(1 + d) * LW + a]; };
       auto V = [&](int a, int bb, int d) { return (bb < 0 ? R0 : (bb > 0 ? R2 : R1))[(4 + d) * LW + a]; };
       auto W = [&](int a, int bb, int d) { return (bb < 0 ? R0 : (bb > 0 ? R2 : R1))[(7 + d) * LW + a]; };
-      dsmr_base_from(U, V, W, c.rdx, c.rdy, rdzf, rdzc, rdzcm, b);
-    } else {
-      int gj = j0 - 1 + r;
-      gj = gj < 0 ? gj + c.ny : (gj >= c.ny ? gj - c.ny : gj);
-      dsmr_base(c, u, v, w, gw, gj, k, b);
+      dsmr_base_from(U, V, W, rdx, rdy, rdzf, rdzc, rdzcm, b);
     }
 #pragma unroll
     for (int q = 0; q < DSMC_NB; ++q) sh[PAR][q * TXB + t] = b[q];
     __syncthreads();
-    if (staged && t == 0 && r + DSMT_NS < nrows + 2) issue(r + DSMT_NS);     // slot of raw row r: every thread is past its last read
+    if (producer && r + DSMT_NS < nraw) issue(S0);     // the slot of raw row r: every thread is past its last read
     double lm = 0.0, mm = 0.0;
     const bool emit = r >= 2;
     if (inner) dsmr_row<PAR>(sh[PAR], TXB, t, b, win, emit, d2, a2, &lm, &mm);
     if (emit) {
-      const int jo = j0 + r - 2;
-      if (outcol) smag[idx3(c, gi, jo, k)] = win.smag_prev;
+      if (outcol) *sm_out = win.smag_prev;
       else { lm = 0.0; mm = 0.0; }
+      sm_out += c.nx;
       if (c.dsm_plane) { accl += lm; accm += mm; }
       else {
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) { lm += __shfl_down_sync(0xffffffffu, lm, o); mm += __shfl_down_sync(0xffffffffu, mm, o); }
-        if ((t & 31) == 0) { const long long slot = pslot0 + (long long)jo * pslots; part[slot * 2] = lm; part[slot * 2 + 1] = mm; }
+        if ((t & 31) == 0) { part[pslot * 2] = lm; part[pslot * 2 + 1] = mm; }
+        pslot += pslots;
       }
     }
     win.smag_prev = b[9];
   };
-  for (int r = 0; r < nrows; r += 2) {
+  for (int r = 0; r < nrows; r += 4) {
     row(std::integral_constant<int, 0>{}, r);
     if (r + 1 < nrows) row(std::integral_constant<int, 1>{}, r + 1);
+    if (r + 2 < nrows) row(std::integral_constant<int, 2>{}, r + 2);
+    if (r + 3 < nrows) row(std::integral_constant<int, 3>{}, r + 3);
   }
   if (c.dsm_plane) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) { accl += __shfl_down_sync(0xffffffffu, accl, o); accm += __shfl_down_sync(0xffffffffu, accm, o); }
     if ((t & 31) == 0)
       for (int jo = j0; jo < jend; ++jo) {
-        const long long slot = pslot0 + (long long)jo * pslots;
-        part[slot * 2] = jo == j0 ? accl : 0.0; part[slot * 2 + 1] = jo == j0 ? accm : 0.0;
+        part[pslot * 2] = jo == j0 ? accl : 0.0; part[pslot * 2 + 1] = jo == j0 ? accm : 0.0;
+        pslot += pslots;
       }
   }
 }

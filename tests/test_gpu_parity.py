@@ -341,11 +341,13 @@ def test_momentum_kernel_both_forms_parity(oracle, gpu, n, shape, min_points):
 
 
 @pytest.mark.parametrize("variant", [0, 1, 2])
-@pytest.mark.parametrize("n,shape", [(5, (144, 72, 24)), (4, (128, 48, 20))])
-def test_dynamic_model_column_kernels_parity(oracle, gpu, n, shape, variant):
+@pytest.mark.parametrize("n,shape,over", [(5, (144, 72, 24), {}), (4, (128, 48, 20), {}), (1, (96, 72, 12), dict(sgs_model=2)),
+                                          (5, (48, 36, 16), {}), (4, (192, 36, 12), dict(wall_model=1, wall_model_y=1, nu=1.0 / 40000))])
+def test_dynamic_model_column_kernels_parity(oracle, gpu, n, shape, over, variant):
     """Both forms of the column march of the dynamic model (register window / shared-memory ring): nu_t and the coefficient
-    against the oracle on grids spanning several 62-column blocks with a ragged tail and more than one 32-row band."""
-    cfg, kw, (u, v, w), dt = pc.prepare(oracle, n, shape)
+    against the oracle on grids spanning several 62-column blocks with a ragged tail and more than one 32-row band, a triply
+    periodic box (wrap of the staged rows in y and z), a grid narrower than one block, and wall models on all four walls."""
+    cfg, kw, (u, v, w), dt = pc.prepare(oracle, n, shape, over)
     o = pc.make(oracle.Oracle, kw)
     g = pc.make(gpu.Solver, kw)
     g.set_option("dsm_col_variant", variant)
