@@ -181,6 +181,7 @@ int cales_set_graph(cales_solver* s, int on);
 /* Kernel-selection knobs, for tests and A/B timing only (results do not depend on them beyond round-off; the defaults are the
  * measured best): "rhs_tile_min_points" (grids with fewer points run the momentum kernel one thread per point instead of the
  * staged z-march; default 200000), "smag_tile_min_points" (the same for the static model; default 4000000),
+ * "rhs_variant" (staged momentum kernel -- 1 (default): halo planes moved by 8-byte cp.async, 0: by tiled TMA copies),
  * "dsm_col_variant" (column march of the dynamic model -- 0: register window, rows staged by TMA bulk copies; 1: the
  * shared-memory-ring form; 2: register window, direct loads).
  * CALES_EINVAL on an unknown key or a value out of range. */

@@ -20,7 +20,7 @@ class OracleParams(C.Structure):
         ("wm_tol", C.c_double), ("wm_maxit", C.c_int),
         ("implicit_z", C.c_int),
         ("const_flow_rate", C.c_int), ("u_bulk", C.c_double),
-        ("wall_model_y", C.c_int), ("dsm_filter3d", C.c_int),
+        ("wall_model_y", C.c_int), ("dsm_filter3d", C.c_int), ("implicit_xyz", C.c_int),
     ]
 
 
@@ -97,7 +97,7 @@ def rk3_coeffs(k):
 PARAM_DEFAULTS = dict(
     zstretch=0, zstretch_factor=0.0, bc_y=0, bc_z=0, nu=1e-3, sgs_model=0, cs=0.17, van_driest=0, aplus=25.0,
     dsm_avg_xy_plane=1, dsm_clip_total=0, dsm_alpha2d=0.0, wall_model=0, kappa=0.41, B=5.2, h_wm=0.0,
-    wm_tol=1e-4, wm_maxit=50, implicit_z=0, const_flow_rate=0, u_bulk=0.0, wall_model_y=0, dsm_filter3d=0)
+    wm_tol=1e-4, wm_maxit=50, implicit_z=0, const_flow_rate=0, u_bulk=0.0, wall_model_y=0, dsm_filter3d=0, implicit_xyz=0)
 
 
 class Oracle:
@@ -158,6 +158,10 @@ class Oracle:
     def poisson_solve(self, rhs):
         rhs = _arr(rhs); phi = np.empty(self.shape)
         _chk(lib().oracle_poisson_solve(self._h, _p(rhs), _p(phi))); return phi
+
+    def helmholtz_solve(self, comp, c, rhs):
+        rhs = _arr(rhs); out = np.empty(self.shape)
+        _chk(lib().oracle_helmholtz_solve(self._h, C.c_int(comp), C.c_double(c), _p(rhs), _p(out))); return out
 
     def laplacian(self, phi):
         phi = _arr(phi); out = np.empty(self.shape)

@@ -492,7 +492,46 @@ static double lam_y(const oracle_solver& S, int n) {
   double s = (S.P.bc_y == BC_PER) ? std::sin(PI * n / (double)S.ny) : std::sin(PI * n / (2.0 * S.ny));
   return -4.0 / (S.dy * S.dy) * s * s;
 }
-static void poisson(const oracle_solver& S, const double* rhs, double* phi) {
+// z system of the Poisson equation for mode (i, j): a_k phi[k-1] + b_k phi[k] + c_k phi[k+1] = f, a_k = 1/(dzf[k] dzc[k-1]),
+// c_k = 1/(dzf[k] dzc[k]), b_k = -(a_k + c_k) + lam_x + lam_y; Neumann: a_0, c_{nz-1} dropped from b; periodic z: cyclic.
+static void poisson_zsolve(const oracle_solver& S, int i, int j, double* dr, double* di) {
+  int nz = S.nz;
+  std::vector<double> a(nz), b(nz), c(nz), xr(nz), xi(nz);
+  double lam = lam_x(S, i) + lam_y(S, j);
+  for (int k = 0; k < nz; ++k) {
+    a[k] = 1.0 / (S.dzf(k) * S.dzc(k - 1)); c[k] = 1.0 / (S.dzf(k) * S.dzc(k));
+    double aa = a[k], cc = c[k];
+    if (S.P.bc_z == BC_WALL) { if (k == 0) aa = 0.0; if (k == nz - 1) cc = 0.0; }
+    b[k] = -(aa + cc) + lam;
+  }
+  bool cyclic = (S.P.bc_z == BC_PER);
+  if (i == 0 && j == 0) {
+    // singular zero mode (reading S15): drop the dzf-weighted mean of f, pin phi[0] = 0, solve, then
+    // shift to zero dzf-weighted mean.
+    double mr = 0, mi = 0;
+    for (int k = 0; k < nz; ++k) { mr += dr[k] * S.dzf(k); mi += di[k] * S.dzf(k); }
+    mr /= S.P.lz; mi /= S.P.lz;
+    for (int k = 0; k < nz; ++k) { dr[k] -= mr; di[k] -= mi; }
+    b[0] = 1.0; c[0] = 0.0; dr[0] = 0.0; di[0] = 0.0;   // row 0: phi[0] = 0 (this also breaks the cycle)
+    oracle_thomas(nz, a.data(), b.data(), c.data(), dr, xr.data());
+    oracle_thomas(nz, a.data(), b.data(), c.data(), di, xi.data());
+    double sr = 0, si = 0;
+    for (int k = 0; k < nz; ++k) { sr += xr[k] * S.dzf(k); si += xi[k] * S.dzf(k); }
+    sr /= S.P.lz; si /= S.P.lz;
+    for (int k = 0; k < nz; ++k) { xr[k] -= sr; xi[k] -= si; }
+  } else if (cyclic) {
+    oracle_thomas_cyclic(nz, a.data(), b.data(), c.data(), dr, xr.data());
+    oracle_thomas_cyclic(nz, a.data(), b.data(), c.data(), di, xi.data());
+  } else {
+    oracle_thomas(nz, a.data(), b.data(), c.data(), dr, xr.data());
+    oracle_thomas(nz, a.data(), b.data(), c.data(), di, xi.data());
+  }
+  for (int k = 0; k < nz; ++k) { dr[k] = xr[k]; di[k] = xi[k]; }
+}
+// The transform scaffold shared by the Poisson solve (Eq. 12) and the Helmholtz solves of Eq. 18: forward DFT along x, forward
+// DFT / DCT-II along y, zsolve(i, j, re[nz], im[nz]) overwrites the z column of mode (i, j) with its solution, inverse y, inverse x.
+template <class ZSolve>
+static void eigen_expansion_solve(const oracle_solver& S, const double* rhs, double* phi, ZSolve zsolve) {
   int nx = S.nx, ny = S.ny, nz = S.nz;
   std::vector<cd> A(S.N);
   // forward x
@@ -524,45 +563,16 @@ static void poisson(const oracle_solver& S, const double* rhs, double* phi) {
       }
     }
   }
-  // z: a_k phi[k-1] + b_k phi[k] + c_k phi[k+1] = f, a_k = 1/(dzf[k] dzc[k-1]), c_k = 1/(dzf[k] dzc[k]),
-  // b_k = -(a_k + c_k) + lam_x + lam_y; Neumann: a_0, c_{nz-1} dropped from b; periodic z: cyclic.
+  // z: one tridiagonal system per mode (i, j), real and imaginary parts share the matrix
 #pragma omp parallel
   {
-    std::vector<double> a(nz), b(nz), c(nz), dr(nz), di(nz), xr(nz), xi(nz);
+    std::vector<double> dr(nz), di(nz);
 #pragma omp for
     for (int l = 0; l < nx * ny; ++l) {
       int i = l % nx, j = l / nx;
-      double lam = lam_x(S, i) + lam_y(S, j);
-      for (int k = 0; k < nz; ++k) {
-        a[k] = 1.0 / (S.dzf(k) * S.dzc(k - 1)); c[k] = 1.0 / (S.dzf(k) * S.dzc(k));
-        double aa = a[k], cc = c[k];
-        if (S.P.bc_z == BC_WALL) { if (k == 0) aa = 0.0; if (k == nz - 1) cc = 0.0; }
-        b[k] = -(aa + cc) + lam;
-        dr[k] = A[S.id(i, j, k)].real(); di[k] = A[S.id(i, j, k)].imag();
-      }
-      bool cyclic = (S.P.bc_z == BC_PER);
-      if (i == 0 && j == 0) {
-        // singular zero mode (reading S15): drop the dzf-weighted mean of f, pin phi[0] = 0, solve, then
-        // shift to zero dzf-weighted mean.
-        double mr = 0, mi = 0;
-        for (int k = 0; k < nz; ++k) { mr += dr[k] * S.dzf(k); mi += di[k] * S.dzf(k); }
-        mr /= S.P.lz; mi /= S.P.lz;
-        for (int k = 0; k < nz; ++k) { dr[k] -= mr; di[k] -= mi; }
-        b[0] = 1.0; c[0] = 0.0; dr[0] = 0.0; di[0] = 0.0;   // row 0: phi[0] = 0 (this also breaks the cycle)
-        oracle_thomas(nz, a.data(), b.data(), c.data(), dr.data(), xr.data());
-        oracle_thomas(nz, a.data(), b.data(), c.data(), di.data(), xi.data());
-        double sr = 0, si = 0;
-        for (int k = 0; k < nz; ++k) { sr += xr[k] * S.dzf(k); si += xi[k] * S.dzf(k); }
-        sr /= S.P.lz; si /= S.P.lz;
-        for (int k = 0; k < nz; ++k) { xr[k] -= sr; xi[k] -= si; }
-      } else if (cyclic) {
-        oracle_thomas_cyclic(nz, a.data(), b.data(), c.data(), dr.data(), xr.data());
-        oracle_thomas_cyclic(nz, a.data(), b.data(), c.data(), di.data(), xi.data());
-      } else {
-        oracle_thomas(nz, a.data(), b.data(), c.data(), dr.data(), xr.data());
-        oracle_thomas(nz, a.data(), b.data(), c.data(), di.data(), xi.data());
-      }
-      for (int k = 0; k < nz; ++k) A[S.id(i, j, k)] = cd(xr[k], xi[k]);
+      for (int k = 0; k < nz; ++k) { dr[k] = A[S.id(i, j, k)].real(); di[k] = A[S.id(i, j, k)].imag(); }
+      zsolve(i, j, dr.data(), di.data());
+      for (int k = 0; k < nz; ++k) A[S.id(i, j, k)] = cd(dr[k], di[k]);
     }
   }
   // inverse y
@@ -594,6 +604,46 @@ static void poisson(const oracle_solver& S, const double* rhs, double* phi) {
       for (int i = 0; i < nx; ++i) phi[(size_t)l * nx + i] = b[i].real() / (double)nx;
     }
   }
+}
+
+static void poisson(const oracle_solver& S, const double* rhs, double* phi) {
+  eigen_expansion_solve(S, rhs, phi, [&](int i, int j, double* dr, double* di) { poisson_zsolve(S, i, j, dr, di); });
+}
+
+// Modified Helmholtz equation of the fully implicit Crank-Nicolson scheme, Eq. 18 ("solved with the same
+// direct solver used for the Poisson equation"):  (1 - c L_jj) q = rhs  for velocity component comp (0 u, 1 v: centred in z;
+// 2 w: on z faces), c = gamma nu dt / 2.  x and y are periodic (the transforms need homogeneous conditions there), so
+// the eigenvalues are those of the Poisson solve; the z system carries the component's wall closure: no-slip mirror ghost for
+// u, v (or the zero-flux closure with the wall model, whose lagged stress is a source outside the operator), w = 0 on the wall
+// faces (unknowns k = 0 .. nz-2), cyclic when z is periodic.
+static void helmholtz(const oracle_solver& S, int comp, double c, const double* rhs, double* out) {
+  int nz = S.nz;
+  bool per = S.P.bc_z == BC_PER;
+  eigen_expansion_solve(S, rhs, out, [&](int i, int j, double* dr, double* di) {
+    double lam = lam_x(S, i) + lam_y(S, j);
+    int m = (comp == 2 && !per) ? nz - 1 : nz;
+    std::vector<double> a(m), b(m), cc(m), xr(m), xi(m);
+    for (int k = 0; k < m; ++k) {
+      double ak, ck;
+      if (comp < 2) { ak = 1.0 / (S.dzf(k) * S.dzc(k - 1)); ck = 1.0 / (S.dzf(k) * S.dzc(k)); }
+      else { ak = 1.0 / (S.dzc(k) * S.dzf(k)); ck = 1.0 / (S.dzc(k) * S.dzf(k + 1)); }
+      a[k] = -c * ak; cc[k] = -c * ck; b[k] = 1.0 + c * (ak + ck) - c * lam;
+      if (!per && comp < 2) {
+        double sg = S.P.wall_model ? -1.0 : 1.0;          // mirror ghost q[-1] = -q[0], or zero flux q[-1] = q[0]
+        if (k == 0) b[k] += sg * c * ak;
+        if (k == nz - 1) b[k] += sg * c * ck;
+      }
+    }
+    if (per) {
+      oracle_thomas_cyclic(m, a.data(), b.data(), cc.data(), dr, xr.data());
+      oracle_thomas_cyclic(m, a.data(), b.data(), cc.data(), di, xi.data());
+    } else {
+      oracle_thomas(m, a.data(), b.data(), cc.data(), dr, xr.data());
+      oracle_thomas(m, a.data(), b.data(), cc.data(), di, xi.data());
+    }
+    for (int k = 0; k < m; ++k) { dr[k] = xr[k]; di[k] = xi[k]; }
+    for (int k = m; k < nz; ++k) { dr[k] = 0.0; di[k] = 0.0; }       // the wall face of w
+  });
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -799,6 +849,8 @@ extern "C" int oracle_create(const oracle_params* p, oracle_solver** out) {
   if (p->wall_model && p->bc_z != BC_WALL) return fail("wall model needs z walls");
   if (p->wall_model_y && p->bc_y != BC_WALL) return fail("wall model on y walls needs y walls");
   if (p->implicit_z && p->bc_z != BC_WALL) return fail("implicit z needs z walls");
+  if (p->implicit_xyz && p->bc_y != BC_PER) return fail("fully implicit diffusion needs periodic y (PAPER.md:136)");
+  if (p->implicit_xyz && p->implicit_z) return fail("implicit_z and implicit_xyz exclude each other");
   if (p->wall_model && p->h_wm > 0.0 && !(p->h_wm < 0.5 * p->lz)) return fail("h_wm must lie below the half height");
   if (p->wall_model_y && p->h_wm > 0.0 && !(p->h_wm < 0.5 * p->ly)) return fail("h_wm must lie below the half width");
   if (p->van_driest && (p->bc_z != BC_WALL || p->bc_y == BC_WALL || p->wall_model)) return fail("van Driest: z walls only, no wall model");
@@ -878,17 +930,20 @@ static void substep(oracle_solver& S, int rk, double dt) {
   if (S.P.sgs_model != 0) sgs_term(S, S.u, S.v, S.w, S.nut, su.data(), sv.data(), sw.data());
   // O-step 5: R^k and the RK update, Eq. 11 (explicit) / Eq. 20 (implicit z)
   F3 us(nx, ny, nz), vs(nx, ny, nz), ws(nx, ny, nz);
-  bool imp = S.P.implicit_z != 0;
+  bool imp = S.P.implicit_z != 0, imp3 = S.P.implicit_xyz != 0;
+  // Eq. 11: R = H + nu L_jj u;  Eq. 20: R = H + nu (L_xx + L_yy) u, the z part goes with gamma;  Eq. 17: R = H, all of nu L_jj u
+  // goes with gamma (H = advection + SGS, Eq. 15)
 #pragma omp parallel for
   for (int k = 0; k < nz; ++k) for (int j = 0; j < ny; ++j) for (int i = 0; i < nx; ++i) {
     size_t n = S.id(i, j, k);
-    double Ru = au[n] + su[n] + dxu[n] + (imp ? 0.0 : dzu[n]);
-    double Rv = av[n] + sv[n] + dxv[n] + (imp ? 0.0 : dzv[n]);
-    double Rw = aw[n] + sw[n] + dxw[n] + (imp ? 0.0 : dzw[n]);
+    double Ru = au[n] + su[n] + (imp3 ? 0.0 : dxu[n]) + ((imp || imp3) ? 0.0 : dzu[n]);
+    double Rv = av[n] + sv[n] + (imp3 ? 0.0 : dxv[n]) + ((imp || imp3) ? 0.0 : dzv[n]);
+    double Rw = aw[n] + sw[n] + (imp3 ? 0.0 : dxw[n]) + ((imp || imp3) ? 0.0 : dzw[n]);
     double gpx = (S.p(i + 1, j, k) - S.p(i, j, k)) / dx, gpy = (S.p(i, j + 1, k) - S.p(i, j, k)) / dy, gpz = (S.p(i, j, k + 1) - S.p(i, j, k)) / S.dzc(k);
-    us(i, j, k) = S.u(i, j, k) + dt * (al * Ru + be * S.Ru[n] - ga * gpx + (imp ? ga * dzu[n] : 0.0));
-    vs(i, j, k) = (j < jvmax) ? S.v(i, j, k) + dt * (al * Rv + be * S.Rv[n] - ga * gpy + (imp ? ga * dzv[n] : 0.0)) : 0.0;
-    ws(i, j, k) = (k < kwmax) ? S.w(i, j, k) + dt * (al * Rw + be * S.Rw[n] - ga * gpz + (imp ? ga * dzw[n] : 0.0)) : 0.0;
+    double gu = imp ? dzu[n] : (imp3 ? dxu[n] + dzu[n] : 0.0), gv = imp ? dzv[n] : (imp3 ? dxv[n] + dzv[n] : 0.0), gw = imp ? dzw[n] : (imp3 ? dxw[n] + dzw[n] : 0.0);
+    us(i, j, k) = S.u(i, j, k) + dt * (al * Ru + be * S.Ru[n] - ga * gpx + ga * gu);
+    vs(i, j, k) = (j < jvmax) ? S.v(i, j, k) + dt * (al * Rv + be * S.Rv[n] - ga * gpy + ga * gv) : 0.0;
+    ws(i, j, k) = (k < kwmax) ? S.w(i, j, k) + dt * (al * Rw + be * S.Rw[n] - ga * gpz + ga * gw) : 0.0;
     S.Ru[n] = Ru; S.Rv[n] = (j < jvmax) ? Rv : 0.0; S.Rw[n] = (k < kwmax) ? Rw : 0.0;
   }
   // O-step 6: (1 - c L_zz) u* = u** - c L_zz u^k, c = gamma nu dt / 2 (Eq. 21), plain Thomas per (i,j)
@@ -937,6 +992,28 @@ static void substep(oracle_solver& S, int rk, double dt) {
       }
     }
   }
+  // Eq. 18: (1 - c L_jj) u* = u** - c L_jj u^k, three modified Helmholtz solves by the eigen-expansion solver.
+  // With the wall model (z walls only) the lagged stress is a source outside the implicit operator, as in Eq. 21:
+  // the right-hand side uses the zero-flux z operator applied to u^k.
+  if (imp3) {
+    std::vector<double> rhs(N), sol(N);
+    for (int comp = 0; comp < 3; ++comp) {
+      F3& q = comp == 0 ? us : (comp == 1 ? vs : ws);
+      const F3& q0 = comp == 0 ? S.u : (comp == 1 ? S.v : S.w);
+      const double* lxy = comp == 0 ? dxu.data() : (comp == 1 ? dxv.data() : dxw.data());
+      const double* lz = comp == 0 ? dzu.data() : (comp == 1 ? dzv.data() : dzw.data());
+#pragma omp parallel for
+      for (int k = 0; k < nz; ++k) for (int j = 0; j < ny; ++j) for (int i = 0; i < nx; ++i) {
+        size_t n = S.id(i, j, k);
+        double lzz = lz[n] / nu;
+        if (S.P.wall_model && comp < 2)
+          lzz = ((k < nz - 1 ? (q0(i, j, k + 1) - q0(i, j, k)) / S.dzc(k) : 0.0) - (k > 0 ? (q0(i, j, k) - q0(i, j, k - 1)) / S.dzc(k - 1) : 0.0)) / S.dzf(k);
+        rhs[n] = q(i, j, k) - cimp * (lxy[n] / nu + lzz);
+      }
+      helmholtz(S, comp, cimp, rhs.data(), sol.data());
+      q.from(sol.data());
+    }
+  }
   S.ust.resize(N); S.vst.resize(N); S.wst.resize(N);     // kept for the pins of Eq. 21 / Eq. 22 (oracle_get_ustar)
   us.to(S.ust.data()); vs.to(S.vst.data()); ws.to(S.wst.data());
   // O-step 7a: constant flow rate (reading S12): uniform shift of u* to the target bulk velocity
@@ -966,7 +1043,8 @@ static void substep(oracle_solver& S, int rk, double dt) {
     S.v(i, j, k) = (j < jvmax) ? vs(i, j, k) - ga * dt * (ph(i, j + 1, k) - ph(i, j, k)) / dy : 0.0;
     S.w(i, j, k) = (k < kwmax) ? ws(i, j, k) - ga * dt * (ph(i, j, k + 1) - ph(i, j, k)) / S.dzc(k) : 0.0;
     double lzz = ((ph(i, j, k + 1) - ph(i, j, k)) / S.dzc(k) - (ph(i, j, k) - ph(i, j, k - 1)) / S.dzc(k - 1)) / S.dzf(k);
-    S.p(i, j, k) += ph(i, j, k) - (imp ? cimp * lzz : 0.0);
+    double lxy = (ph(i + 1, j, k) - 2.0 * ph(i, j, k) + ph(i - 1, j, k)) / (dx * dx) + (ph(i, j + 1, k) - 2.0 * ph(i, j, k) + ph(i, j - 1, k)) / (dy * dy);
+    S.p(i, j, k) += ph(i, j, k) - (imp ? cimp * lzz : 0.0) - (imp3 ? cimp * (lxy + lzz) : 0.0);     // Eq. 14 / Eq. 22 / Eq. 19
   }
   // O-steps 8-9
   refresh_closures(S);
@@ -995,6 +1073,11 @@ extern "C" int oracle_get_ustar(oracle_solver* S, int comp, double* dst) {
 }
 extern "C" int oracle_poisson_solve(oracle_solver* S, const double* rhs, double* phi) {
   if (!S || !rhs || !phi) return fail("null"); poisson(*S, rhs, phi); return 0;
+}
+extern "C" int oracle_helmholtz_solve(oracle_solver* S, int comp, double c, const double* rhs, double* out) {
+  if (!S || !rhs || !out || comp < 0 || comp > 2) return fail("bad argument");
+  if (S->P.bc_y != BC_PER) return fail("helmholtz: periodic y only");
+  helmholtz(*S, comp, c, rhs, out); return 0;
 }
 extern "C" int oracle_laplacian(oracle_solver* S, const double* phi, double* out) {
   if (!S || !phi || !out) return fail("null");

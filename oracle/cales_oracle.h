@@ -40,6 +40,7 @@ typedef struct {
   int const_flow_rate; double u_bulk;
   int wall_model_y;        /* log-law wall model on the y walls too (duct WMLES); needs bc_y = wall */
   int dsm_filter3d;        /* 1: 3-D box test filter (x, y and z) with the first-off-wall-layer rule of PAPER.md:128; 0: x-y filter */
+  int implicit_xyz;        /* 1: Crank-Nicolson in all three directions, Eq. 17-19; needs periodic y; excludes implicit_z */
 } oracle_params;
 
 /* ---- 1-D primitives (pinned against numpy/scipy and O(N^2) definitions in tests) ---- */
@@ -73,6 +74,8 @@ int oracle_substep(oracle_solver* s, int rk, double dt);
 int oracle_get_ustar(oracle_solver* s, int comp, double* dst);
 /* Poisson: L_h phi = rhs with the solver's BCs (Eq. 12); zero weighted-mean gauge (reading S15) */
 int oracle_poisson_solve(oracle_solver* s, const double* rhs, double* phi);
+/* (1 - c L_jj) q = rhs for velocity component comp (0 u, 1 v, 2 w) with its boundary closure (Eq. 18; needs periodic y) */
+int oracle_helmholtz_solve(oracle_solver* s, int comp, double c, const double* rhs, double* out);
 /* plain 7-point stencil L_h phi (O-step 3 operator at centres, periodic/Neumann closure) */
 int oracle_laplacian(oracle_solver* s, const double* phi, double* out);
 /* nu_t from a velocity field (NULL -> internal state); uses the stored wall stresses for van Driest */

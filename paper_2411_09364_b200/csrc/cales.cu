@@ -26,6 +26,8 @@
 #include "cales_host.h"
 
 #include <cmath>
+#include <cuda.h>
+#include <cudaTypedefs.h>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -63,6 +65,8 @@ struct cales_solver {
   bool fresh;
   long long rhs_tile_min;   // below this many points the momentum kernel runs one thread per point
   long long tile_min;   // grids with at least this many points use the staged z-march for the static model
+  int rhs_variant;      // 1 (default): halo planes by 8-byte cp.async (k_rhs_tile); 0: by tiled TMA copies (k_rhs_tile_tma)
+  RhsMaps* rmaps; bool rmaps_ok;   // tensor maps of u, v, w, nu_t, p in device memory (workspace)
   int dsm_col_variant;  // 0: TMA-staged register-window column march (k_dsm_col_tma); 1: shared-ring form of round 1 (k_dsm_col_sm); 2: direct loads (k_dsm_col_rw)
   std::vector<double> h_dzf, h_dzc, h_cn; Ctx hc; double cn_dt;   // host copies for the per-dt CN coefficient tables
   int use_graph; cudaGraphExec_t gexec; double gdt;   // the three substeps captured as one CUDA graph, keyed by dt
@@ -96,6 +100,7 @@ static size_t carve(cales_solver* s, const cales_params* p, double* base) {
   double* partial = take(nblk > nxy ? nblk : nxy);
   double* stage1 = take(4 * 1024);
   double* scal = take(32);
+  double* tmaps = take(128);      // 5 tensor maps of 128 bytes (cales_rhs_tile.cuh)
   const size_t pslots = (size_t)dsm_shape(p->nx).pslots;
   double* dsm_part = p->sgs_model == CALES_SGS_DSMAG ? take((size_t)p->nz * p->ny * pslots * 2) : nullptr;
   double* dsm_cs = p->sgs_model == CALES_SGS_DSMAG ? take((size_t)p->nz * p->ny) : nullptr;
@@ -105,7 +110,7 @@ static size_t carve(cales_solver* s, const cales_params* p, double* base) {
     s->dzf = dzf; s->dzc = dzc; s->zc = zc; s->rdzf = rdzf; s->rdzc = rdzc; s->delta = delta; s->ak = ak; s->ck = ck; s->lamx = lamx; s->lamy = lamy;
     s->twx = reinterpret_cast<double2*>(twx); s->twy = reinterpret_cast<double2*>(twy); s->dctw = reinterpret_cast<double2*>(dctw);
     s->cncoef = cncoef; s->partial = partial; s->stage1 = stage1; s->scal = scal; s->maxit = reinterpret_cast<int*>(scal + 16);
-    s->dsm_part = dsm_part; s->dsm_cs = dsm_cs; s->nblk = (long long)nblk;
+    s->dsm_part = dsm_part; s->dsm_cs = dsm_cs; s->nblk = (long long)nblk; s->rmaps = reinterpret_cast<RhsMaps*>(tmaps);
   }
   return off * sizeof(double);
 }
@@ -145,6 +150,22 @@ static int check_launch(cales_solver* s, int kid) {
 }
 #define LAUNCH_TRY(kid)                                  \
   do { int rc_ = check_launch(s, kid); if (rc_) return rc_; } while (0)
+
+// Tiled tensor map of an (nx, ny, nz) fp64 field with box (bx, by, 1) (cuTensorMapEncodeTiled through the runtime's driver
+// entry point: libcuda is not linked).  False if the driver call is unavailable or rejects the shape.
+static bool make_field_map(CUtensorMap* m, const double* base, int nx, int ny, int nz, int bx, int by) {
+  static PFN_cuTensorMapEncodeTiled enc = nullptr;
+  if (!enc) {
+    void* fn = nullptr; cudaDriverEntryPointQueryResult qr;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr) != cudaSuccess || qr != cudaDriverEntryPointSuccess || !fn) { cudaGetLastError(); return false; }
+    enc = (PFN_cuTensorMapEncodeTiled)fn;
+  }
+  const cuuint64_t dims[3] = {(cuuint64_t)nx, (cuuint64_t)ny, (cuuint64_t)nz};
+  const cuuint64_t strides[2] = {(cuuint64_t)nx * 8, (cuuint64_t)nx * ny * 8};
+  const cuuint32_t box[3] = {(cuuint32_t)bx, (cuuint32_t)by, 1}, es[3] = {1, 1, 1};
+  return enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<double*>(base), dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+             CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
 
 extern "C" int cales_create(const cales_params* p, cales_solver** out) {
   if (!out) return fail(CALES_EINVAL, "null output pointer");
@@ -196,6 +217,7 @@ extern "C" int cales_create(const cales_params* p, cales_solver** out) {
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fft2_x_inv, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fft2_y, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rhs_tile, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(RT_SMEM_DOUBLES * sizeof(double)));
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rhs_tile_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RT_SMEM_TMA_BYTES);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_smag_tile, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(ST_SMEM_DOUBLES * sizeof(double)));
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dsm_pass1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(DSM_SMEM_DOUBLES * sizeof(double)));
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dsm3_pass1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(D3_SMEM_DOUBLES * sizeof(double)));
@@ -208,6 +230,14 @@ extern "C" int cales_create(const cales_params* p, cales_solver** out) {
   s->tile_min = 4000000;
   s->rhs_tile_min = 200000;
   s->dsm_col_variant = 0;
+  s->rhs_variant = 1;      // measured on B200 at config 5: cp.async ring 22.7 ms, tiled TMA ring 25.1 ms per launch
+  {
+    const double* fl[RT_NF] = {s->u, s->v, s->w, s->nut, s->p};
+    RhsMaps hm;
+    s->rmaps_ok = true;
+    for (int f = 0; f < RT_NF; ++f) s->rmaps_ok = s->rmaps_ok && make_field_map(&hm.m[f], fl[f], nx, ny, nz, RTT_TW, RT_TH);
+    if (s->rmaps_ok && (cudaMemcpyAsync(s->rmaps, &hm, sizeof(hm), cudaMemcpyHostToDevice, s->st) != cudaSuccess || cudaStreamSynchronize(s->st) != cudaSuccess)) { cudaGetLastError(); s->rmaps_ok = false; }
+  }
   for (int q = 0; q < 32; ++q) { s->kms[q] = 0.0; s->kcnt[q] = 0; }
   *out = s;
   return CALES_OK;
@@ -402,7 +432,8 @@ static int substep(cales_solver* s, int rk, double dt) {
   a.us = s->us; a.vs = s->vs; a.ws = s->ws; a.dt = dt; a.al = al; a.be = be; a.ga = ga; a.store_R = rk < 2 ? 1 : 0;
   const int kz = rt_chunk(c.nx, c.ny, c.nz);
   dim3 rgrid((c.nx + RT_TX - 1) / RT_TX, (c.ny + RT_TY - 1) / RT_TY, (c.nz + kz - 1) / kz);
-  if (s->N >= s->rhs_tile_min) k_rhs_tile<<<rgrid, RT_THREADS, RT_SMEM_DOUBLES * sizeof(double), s->st>>>(c, a, kz, (cfr && !imp) ? s->partial : nullptr);
+  if (s->N >= s->rhs_tile_min && s->rhs_variant == 0 && s->rmaps_ok) k_rhs_tile_tma<<<rgrid, RT_THREADS, RT_SMEM_TMA_BYTES, s->st>>>(c, a, s->rmaps, kz, (cfr && !imp) ? s->partial : nullptr);
+  else if (s->N >= s->rhs_tile_min) k_rhs_tile<<<rgrid, RT_THREADS, RT_SMEM_DOUBLES * sizeof(double), s->st>>>(c, a, kz, (cfr && !imp) ? s->partial : nullptr);
   else { rgrid = s->pgrid; k_rhs_point<<<s->pgrid, s->pblock, 0, s->st>>>(c, a, (cfr && !imp) ? s->partial : nullptr); }
   LAUNCH_TRY(K_RHS);
   long long npart = (long long)rgrid.x * rgrid.y * rgrid.z;
@@ -495,6 +526,7 @@ extern "C" int cales_set_option(cales_solver* s, const char* key, long long valu
   const std::string k(key);
   if (k == "rhs_tile_min_points") s->rhs_tile_min = value;
   else if (k == "smag_tile_min_points") s->tile_min = value;
+  else if (k == "rhs_variant") { if (value < 0 || value > 1) return fail(CALES_EINVAL, "rhs_variant must be 0 or 1"); s->rhs_variant = (int)value; }
   else if (k == "dsm_col_variant") { if (value < 0 || value > 2) return fail(CALES_EINVAL, "dsm_col_variant must be 0, 1 or 2"); s->dsm_col_variant = (int)value; }
   else return fail(CALES_EINVAL, "unknown option: " + k);
   if (s->gexec) { cudaGraphExecDestroy(s->gexec); s->gexec = nullptr; }      // the captured step holds the old selection

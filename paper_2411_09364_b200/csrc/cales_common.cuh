@@ -154,6 +154,17 @@ __device__ __forceinline__ void bulk_g2s(void* smem_dst, const void* gsrc, unsig
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n" ::"r"(smem_u32(smem_dst)), "l"(gsrc), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
+// plain arrival (no bytes expected): flips the phase of a barrier of count 1
+__device__ __forceinline__ void mbar_arrive(unsigned long long* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(smem_u32(bar)) : "memory");
+}
+// 3-D tiled TMA load (cp.async.bulk.tensor, SASS: UTMALDG): box of the tensor map at element coordinates (c0, c1, c2) into
+// shared memory (128-byte aligned), completing on the mbarrier; out-of-range elements arrive as zeros.
+__device__ __forceinline__ void tma_load_3d(void* smem_dst, const void* tmap, int c0, int c1, int c2, unsigned long long* bar) {
+  asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];\n"
+               ::"r"(smem_u32(smem_dst)), "l"(tmap), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar)) : "memory");
+}
+
 // Sum over the thread block (result valid in thread 0).  blockDim.x*y*z <= 1024, multiple of 32.
 __device__ __forceinline__ double block_sum(double v, double* sh /* >= 32 doubles */) {
   const int tid = threadIdx.x + blockDim.x * (threadIdx.y + blockDim.y * threadIdx.z);

@@ -12,6 +12,9 @@
 #pragma once
 #include "cales_common.cuh"
 #include "cales_momentum.cuh"
+#ifdef __CUDACC__
+#include <cuda.h>
+#endif
 
 namespace cales {
 
@@ -132,15 +135,17 @@ CALES_HD double rt_elem(const Ctx& c, const RhsArgs& a, int f, int gi, int gj, i
 }
 
 // Accessor over three staged planes (k-1, k, k+1): sl[d] points at field 0 of the slot, ctr = (ly+1)*RT_TW + lx+1.
-struct TileAcc {
+template <int FSTRIDE, int PITCH>
+struct TileAccT {
   const double* sl[3]; int ctr;
-  CALES_HD double at(int f, int di, int dj, int dk) const { return sl[dk + 1][f * RT_PLANE + ctr + dj * RT_TW + di]; }
+  CALES_HD double at(int f, int di, int dj, int dk) const { return sl[dk + 1][f * FSTRIDE + ctr + dj * PITCH + di]; }
   CALES_HD double U(int di, int dj, int dk) const { return at(0, di, dj, dk); }
   CALES_HD double V(int di, int dj, int dk) const { return at(1, di, dj, dk); }
   CALES_HD double W(int di, int dj, int dk) const { return at(2, di, dj, dk); }
   CALES_HD double NT(int di, int dj, int dk) const { return at(3, di, dj, dk); }
   CALES_HD double P(int di, int dj, int dk) const { return at(4, di, dj, dk); }
 };
+typedef TileAccT<RT_PLANE, RT_TW> TileAcc;
 
 // k-planes per CTA: enough chunks for ~8 waves of 2 CTAs/SM on 148 SMs, at least 8 planes per chunk
 static inline int rt_chunk(int nx, int ny, int nz) {
@@ -238,6 +243,109 @@ __global__ void __launch_bounds__(RT_THREADS, 2) k_rhs_tile(const __grid_constan
       const int ly = ty * RT_RPT + r, i = i0 + tx, j = j0 + ly;   // adjacent rows: their stencils share shared-memory loads
       if (i < c.nx && j < c.ny) {
         q.ctr = (ly + 1) * RT_TW + tx + 1;
+        acc += rhs_core(c, a, q, i, j, k, zm) * dz;
+      }
+    }
+  }
+  if (partial) {
+    const double t = block_sum(acc, red);
+    if (tid == 0) partial[blockIdx.x + gridDim.x * (blockIdx.y + (long long)gridDim.y * blockIdx.z)] = t;
+  }
+}
+
+// ---- the same kernel with the halo planes moved by the TMA engine -----------------------------------------------------------
+// ncu on k_rhs_tile (profiles/r1_ncu_full.md): 16 warps per SM, top stalls long scoreboard and wait, L1 pipe 59 % -- every
+// plane costs each thread 12 eight-byte LDGSTS with their address arithmetic.  Here thread 0 issues ONE tiled tensor copy per
+// field and plane (cp.async.bulk.tensor.3d, box 36 x 18 x 1 at (i0-2, j0-1, k), SASS UTMALDG), completing on an mbarrier two
+// planes ahead of its use.  (The box starts one column left of the halo because the TMA engine wants the innermost
+// coordinate on a 16-byte boundary -- an odd fp64 column is an illegal instruction, measured on B200.)  Elements outside the array arrive as zeros and are then overwritten with the boundary rule of
+// Alg. 2 (periodic wrap, wall ghosts) by the threads that own them -- only tiles on the edge of the x-y plane have any.
+// Planes beyond a z wall are filled by the generic path as before.  Field planes are padded to RT_FS doubles (128-byte slots).
+enum { RTT_TW = RT_TX + 4, RTT_PLANE = RTT_TW * RT_TH, RT_FS = 656, RT_SMEM_TMA_BYTES = RT_NSLOT * RT_NF * RT_FS * 8 + 128,
+       RTT_EPT = (RTT_PLANE + RT_THREADS - 1) / RT_THREADS };
+struct RhsMaps { CUtensorMap m[RT_NF]; };      // u, v, w, nu_t, p as (nx, ny, nz) fp64 tensors, box (RTT_TW, RT_TH, 1); lives in device memory
+
+__global__ void __launch_bounds__(RT_THREADS, 2) k_rhs_tile_tma(const __grid_constant__ Ctx c, const __grid_constant__ RhsArgs a,
+                                                                const RhsMaps* __restrict__ maps, int kz, double* __restrict__ partial) {
+  extern __shared__ double rt_sm_raw[];
+  __shared__ double red[32];
+  __shared__ unsigned long long full[RT_NSLOT];
+  double* rt_sm = reinterpret_cast<double*>((reinterpret_cast<size_t>(rt_sm_raw) + 127) & ~(size_t)127);
+  const int tid = threadIdx.x, tx = tid & 31, ty = tid >> 5;
+  const int i0 = blockIdx.x * RT_TX, j0 = blockIdx.y * RT_TY, k0 = blockIdx.z * kz, k1 = min(k0 + kz, c.nz);
+  // tiles on the edge of the x-y plane hold elements outside the array (zeros from the TMA, replaced in land())
+  const bool edge = i0 == 0 || i0 + RT_TX >= c.nx || j0 == 0 || j0 + RT_TY >= c.ny;
+  if (tid == 0) {
+#pragma unroll
+    for (int s = 0; s < RT_NSLOT; ++s) mbar_init(&full[s], 1);
+    mbar_fence_init();
+  }
+  __syncthreads();
+  // plane kk (k0-1 <= kk <= k1) lives in slot q & 3, q = kk - (k0 - 1); its barrier phase is (q >> 2) & 1
+  auto issue = [&](int kk) {
+    const int q = kk - (k0 - 1);
+    double* slot = rt_sm + (q & 3) * (RT_NF * RT_FS);
+    const bool zreg = c.bc_z == BC_PER || (kk >= 0 && kk < c.nz);
+    if (zreg) {
+      if (tid == 0) {
+        const int kw = kk < 0 ? kk + c.nz : (kk >= c.nz ? kk - c.nz : kk);
+        const int nf = c.sgs ? RT_NF : RT_NF - 1;
+        mbar_expect_tx(&full[q & 3], (unsigned)(nf * RTT_PLANE * sizeof(double)));
+#pragma unroll
+        for (int f = 0; f < RT_NF; ++f) if (f != 3 || c.sgs) tma_load_3d(slot + f * RT_FS, &maps->m[f], i0 - 2, j0 - 1, kw, &full[q & 3]);
+      }
+    } else {
+      for (int pos = tid; pos < RTT_PLANE; pos += RT_THREADS) {
+        const int ry = pos / RTT_TW, rx = pos - ry * RTT_TW, gi = i0 - 2 + rx, gj = j0 - 1 + ry;
+        if (rx < 1 || gi > c.nx || gj > c.ny) continue;
+        for (int f = 0; f < RT_NF; ++f) slot[f * RT_FS + pos] = rt_elem(c, a, f, gi, gj, kk);
+      }
+      if (tid == 0) mbar_arrive(&full[q & 3]);       // keeps the phase count of the slot in step
+    }
+  };
+  // wait for plane kk and replace the out-of-array zeros (x / y ghosts) of a TMA plane
+  auto land = [&](int kk) {
+    const int q = kk - (k0 - 1);
+    mbar_wait(&full[q & 3], (q >> 2) & 1);
+    const bool zreg = c.bc_z == BC_PER || (kk >= 0 && kk < c.nz);
+    if (!zreg || !edge) return;
+    double* slot = rt_sm + (q & 3) * (RT_NF * RT_FS);
+    for (int pos = tid; pos < RTT_PLANE; pos += RT_THREADS) {
+      const int ry = pos / RTT_TW, rx = pos - ry * RTT_TW, gi = i0 - 2 + rx, gj = j0 - 1 + ry;
+      if (rx < 1 || gi > c.nx || gj > c.ny || (gi >= 0 && gi < c.nx && gj >= 0 && gj < c.ny)) continue;
+      for (int f = 0; f < RT_NF; ++f) slot[f * RT_FS + pos] = rt_elem(c, a, f, gi, gj, kk);
+    }
+  };
+  issue(k0 - 1); issue(k0);
+  if (k0 + 1 <= k1) issue(k0 + 1);
+  land(k0 - 1); land(k0);
+  double acc = 0.0;
+  for (int k = k0; k < k1; ++k) {
+    land(k + 1);
+    __syncthreads();
+    if (k + 2 <= k1) issue(k + 2);
+    if (a.be != 0.0 && k + 1 < k1) {     // R^{k-1} of the next plane: pull the lines towards L1 while this plane is computed
+#pragma unroll
+      for (int r = 0; r < RT_RPT; ++r) {
+        const int i = i0 + tx, j = j0 + ty * RT_RPT + r;
+        if (i < c.nx && j < c.ny && (tx & 3) == 0) {
+          const long long nn = idx3(c, i, j, k + 1);
+          asm volatile("prefetch.global.L1 [%0];" ::"l"(a.Ru0 + nn));
+          asm volatile("prefetch.global.L1 [%0];" ::"l"(a.Rv0 + nn));
+          asm volatile("prefetch.global.L1 [%0];" ::"l"(a.Rw0 + nn));
+        }
+      }
+    }
+    const int qc = k - (k0 - 1);
+    TileAccT<RT_FS, RTT_TW> q;
+    q.sl[0] = rt_sm + ((qc - 1) & 3) * (RT_NF * RT_FS); q.sl[1] = rt_sm + (qc & 3) * (RT_NF * RT_FS); q.sl[2] = rt_sm + ((qc + 1) & 3) * (RT_NF * RT_FS);
+    const ZMet zm = zmet_at(c, k);
+    const double dz = zm.dzfk;
+#pragma unroll
+    for (int r = 0; r < RT_RPT; ++r) {
+      const int ly = ty * RT_RPT + r, i = i0 + tx, j = j0 + ly;
+      if (i < c.nx && j < c.ny) {
+        q.ctr = (ly + 1) * RTT_TW + tx + 2;
         acc += rhs_core(c, a, q, i, j, k, zm) * dz;
       }
     }

@@ -323,15 +323,16 @@ def test_cfl_dt_and_plane_stats_parity(oracle, gpu, n, shape):
     g.close()
 
 
-@pytest.mark.parametrize("min_points", ["0", "1000000000"])
-@pytest.mark.parametrize("n,shape", [(1, (48, 24, 20)), (2, (72, 48, 24)), (4, (96, 36, 24))])
-def test_momentum_kernel_both_forms_parity(oracle, gpu, n, shape, min_points):
-    """The staged z-marching momentum kernel (min_points = 0) and the one-thread-per-point form used on launch-bound
-    grids (min_points huge), each forced on at test sizes."""
+@pytest.mark.parametrize("min_points,variant", [("0", 0), ("0", 1), ("1000000000", 0)])
+@pytest.mark.parametrize("n,shape", [(1, (48, 24, 20)), (2, (72, 48, 24)), (4, (96, 36, 24)), (3, (72, 36, 40)), (5, (48, 36, 24))])
+def test_momentum_kernel_all_forms_parity(oracle, gpu, n, shape, min_points, variant):
+    """The staged z-marching momentum kernel (min_points = 0) with its halo planes moved by TMA (variant 0) or by cp.async
+    (variant 1), and the one-thread-per-point form used on launch-bound grids (min_points huge), each forced on at test sizes."""
     cfg, kw, (u, v, w), dt = pc.prepare(oracle, n, shape)
     o = pc.make(oracle.Oracle, kw)
     g = pc.make(gpu.Solver, kw)
     g.set_option("rhs_tile_min_points", int(min_points))
+    g.set_option("rhs_variant", variant)
     o.set_velocity(u, v, w); g.set_velocity(u, v, w)
     for s in range(2):
         o.step(dt); g.step(dt)

@@ -2,7 +2,7 @@
 oracle/cales_oracle.cpp, the copy is built, and tests/test_oracle_pins.py is run against it; at least the pin named
 beside the mutant must turn red.  M1-M6 are the mistakes the round-1 review found already caught, M7-M12 the six it
 found surviving (config-3 and config-4 arithmetic: Eq. 22, tanh-grid metrics, x-line averaging, total-viscosity clip);
-the pins that kill those were added in round 2.  Test infrastructure only; nothing here touches the CUDA path.
+the pins that kill those were added in round 2; M13-M16 are mistakes in the fully implicit scheme (Eq. 17-19) added in round 2.  Test infrastructure only; nothing here touches the CUDA path.
 """
 import os
 import subprocess
@@ -28,7 +28,7 @@ MUTANTS = [
      "test_wall_model_on_y_walls_is_the_z_wall_model_rotated"),
     ("M6_alpha_not_reduced_on_y_wall_rows", "if (!(S.P.bc_y == BC_WALL && (j == 0 || j == ny - 1))) ++nf;", "++nf;",
      "test_3d_filter_first_layer_rule_and_filter_ratio"),
-    ("M7_eq22_term_dropped", "S.p(i, j, k) += ph(i, j, k) - (imp ? cimp * lzz : 0.0);", "S.p(i, j, k) += ph(i, j, k);",
+    ("M7_eq22_term_dropped", "S.p(i, j, k) += ph(i, j, k) - (imp ? cimp * lzz : 0.0) -", "S.p(i, j, k) += ph(i, j, k) -",
      "test_pressure_update_eq22_on_tanh_grid"),
     ("M8_diffusion_z_metrics_swapped",
      "lz = ((u(i, j, k + 1) - u(i, j, k)) / S.dzc(k) - (u(i, j, k) - u(i, j, k - 1)) / S.dzc(k - 1)) / S.dzf(k);\n    du[n]",
@@ -41,6 +41,10 @@ MUTANTS = [
      "double ak = 1.0 / (S.dzc(k) * S.dzf(k + 1)), ck = 1.0 / (S.dzc(k) * S.dzf(k));", "test_crank_nicolson_dense_matrix_on_tanh_grid"),
     ("M11_x_line_coefficient_mirrored_row", "if (!per_plane) S.cs[(size_t)k * ny + j] = (mm > 0.0) ? ll / mm : 0.0;",
      "if (!per_plane) S.cs[(size_t)k * ny + (ny - 1 - j)] = (mm > 0.0) ? ll / mm : 0.0;", "test_dynamic_coefficient_per_x_line_vs_dense_bruteforce"),
+    ("M13_eq19_xy_part_dropped", "- (imp3 ? cimp * (lxy + lzz) : 0.0);", "- (imp3 ? cimp * lzz : 0.0);", "test_pressure_update_eq19"),
+    ("M14_helmholtz_wall_closure_sign", "double sg = S.P.wall_model ? -1.0 : 1.0;", "double sg = S.P.wall_model ? 1.0 : -1.0;", "test_helmholtz_manufactured_discrete"),
+    ("M15_eq17_diffusion_counted_in_R", "double Ru = au[n] + su[n] + (imp3 ? 0.0 : dxu[n])", "double Ru = au[n] + su[n] + dxu[n]", "test_fully_implicit_ustar_is_the_helmholtz_solution"),
+    ("M16_helmholtz_w_metrics_swapped", "else { ak = 1.0 / (S.dzc(k) * S.dzf(k)); ck = 1.0 / (S.dzc(k) * S.dzf(k + 1)); }", "else { ak = 1.0 / (S.dzc(k) * S.dzf(k + 1)); ck = 1.0 / (S.dzc(k) * S.dzf(k)); }", "test_helmholtz_manufactured_discrete"),
     ("M12_total_clip_floor_halved", "nut[n] = (t < -nu) ? -nu : t;", "nut[n] = (t < -0.5 * nu) ? -0.5 * nu : t;", "test_total_viscosity_clip_floor_binds"),
 ]
 

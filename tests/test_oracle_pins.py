@@ -1041,3 +1041,139 @@ def test_advection_vs_numpy_stencil(oracle, bcs, stretch):
     S.set_velocity(u, v, w)
     for g, e in zip(S.advection(), np_advection(S, u, v, w)):
         assert np.max(np.abs(g - e)) < 1e-12 * np.max(np.abs(e))
+
+
+# ======================================================================= fully implicit Crank-Nicolson, Eq. 17-19
+# three modified Helmholtz solves with the eigen-expansion solver, periodic y.
+def np_lap_comp(S, q, comp, zero_flux=False):
+    """L_jj q for one velocity component in a box with periodic x, y: u, v centred in z (no-slip mirror ghost, or the
+    zero-flux ghost of the wall-model closure), w on z faces (0 on and beyond the wall faces); periodic z wraps."""
+    dx, dy = S.dx, S.dy
+    nz = S.nz
+    _, dzf, dzc = np_metrics(S)
+    out = (np.roll(q, -1, 2) - 2 * q + np.roll(q, 1, 2)) / dx ** 2 + (np.roll(q, -1, 1) - 2 * q + np.roll(q, 1, 1)) / dy ** 2
+    if S.params["bc_z"] == 0:
+        return out + (np.roll(q, -1, 0) - 2 * q + np.roll(q, 1, 0)) / dzf[0] ** 2
+    if comp < 2:
+        sg = 1.0 if zero_flux else -1.0
+        e = np.concatenate([sg * q[:1], q, sg * q[-1:]], axis=0)
+        return out + ((e[2:] - e[1:-1]) / dzc[1:, None, None] - (e[1:-1] - e[:-2]) / dzc[:-1, None, None]) / dzf[:, None, None]
+    e = np.concatenate([np.zeros_like(q[:1]), q, np.zeros_like(q[:1])], axis=0)
+    dzf_g = np.concatenate([dzf, dzf[-1:]])
+    lz = ((e[2:] - e[1:-1]) / dzf_g[1:, None, None] - (e[1:-1] - e[:-2]) / dzf[:, None, None]) / dzc[1:, None, None]
+    out = out + lz
+    out[-1] = 0.0
+    return out
+
+
+@pytest.mark.parametrize("comp", [0, 1, 2])
+@pytest.mark.parametrize("bc_z,stretch,wm", [(0, False, 0), (1, False, 0), (1, True, 0), (1, True, 1)])
+def test_helmholtz_manufactured_discrete(oracle, bc_z, stretch, wm, comp):
+    """(1 - c L_jj) q = rhs, Eq. 18: random q -> rhs by the numpy stencil -> oracle solve -> q back, per component and closure."""
+    S = make(oracle, 24, 12, 16, (0, bc_z), stretch, wall_model=wm, sgs_model=1 if wm else 0)
+    q = np.random.default_rng(5 + comp).standard_normal(S.shape)
+    if comp == 2 and bc_z == 1:
+        q[-1] = 0.0
+    for c in (0.37, 3e-3):
+        rhs = q - c * np_lap_comp(S, q, comp, zero_flux=bool(wm))
+        got = S.helmholtz_solve(comp, c, rhs)
+        assert np.max(np.abs(got - q)) < 1e-12 * np.max(np.abs(q))
+
+
+@pytest.mark.parametrize("plane", ["xy", "xz", "yz"])
+def test_fully_implicit_fourier_mode_amplification(oracle, plane):
+    """Taylor-Green in a triply periodic box under Eq. 17-19: the nonlinear term is an exact discrete gradient and the
+    Helmholtz operator commutes with the projection, so the velocity is multiplied per substep by (1 + c lam)/(1 - c lam),
+    lam = -2 k_eff^2 the eigenvalue of the discrete Laplacian, c = gamma nu dt / 2."""
+    n, nu, dt, steps = 16, 5e-2, 2e-2, 3
+    S = oracle.Oracle(n, n, n, 2 * PI, 2 * PI, 2 * PI, nu=nu, sgs_model=0, implicit_xyz=1)
+    d = 2 * PI / n
+    c_ = (np.arange(n) + 0.5) * d
+    f = (np.arange(n) + 1.0) * d
+    one = np.ones((n, n, n))
+    ax = {"x": 2, "y": 1, "z": 0}
+    def along(a, vals):
+        sh = [1, 1, 1]; sh[ax[a]] = n
+        return vals.reshape(sh) * one
+    a, b = plane
+    ua = along(a, np.sin(f)) * along(b, np.cos(c_))
+    ub = -along(a, np.cos(c_)) * along(b, np.sin(f))
+    vel = {"x": np.zeros_like(one), "y": np.zeros_like(one), "z": np.zeros_like(one)}
+    vel[a], vel[b] = ua, ub
+    S.set_velocity(vel["x"], vel["y"], vel["z"])
+    for _ in range(steps):
+        S.step(dt)
+    lam = -2.0 * (math.sin(d / 2) / (d / 2)) ** 2
+    G = 1.0
+    for rk in range(3):
+        c = oracle.rk3_coeffs(rk)[2] * nu * dt / 2
+        G *= (1 + c * lam) / (1 - c * lam)
+    got = dict(zip("xyz", S.velocity()))
+    assert rel(got[a], G ** steps * ua) < 1e-12 and rel(got[b], G ** steps * ub) < 1e-12
+    assert np.max(np.abs(S.divergence())) < 1e-12
+    assert abs(G - math.exp(-2 * nu * dt)) < 1e-3          # and it is the viscous decay
+
+
+def test_fully_implicit_matches_explicit_to_second_order(oracle):
+    """Eq. 17-19 and Eq. 11-14 discretise the same equation: between walls, on the tanh grid, with the SGS model on, their
+    results after a fixed number of steps differ by O(dt^2)."""
+    errs = []
+    base = None
+    for dt in (2.5e-4, 1.25e-4, 6.25e-5):      # c lam_max << 1 on the tanh grid: the asymptotic range of the difference
+        res = []
+        for imp in (0, 1):
+            S = make(oracle, 16, 8, 16, (0, 1), True, nu=0.05, sgs_model=1, cs=0.1, implicit_xyz=imp)
+            if base is None:
+                random_solenoidal(S, seed=6, amp=0.3)
+                base = S.velocity()
+            S.set_velocity(*base)
+            for _ in range(4):
+                S.step(dt)
+            res.append(np.array(S.velocity()))
+        errs.append(np.max(np.abs(res[0] - res[1])))
+    assert errs[0] < 1e-4 and 3.3 < errs[0] / errs[1] < 4.7 and 3.3 < errs[1] / errs[2] < 4.7, errs
+
+
+@pytest.mark.parametrize("bc_z,stretch", [(0, False), (1, True)])
+def test_pressure_update_eq19(oracle, bc_z, stretch):
+    """Eq. 19 (PAPER.md:114): the pressure increment of a fully implicit substep is phi - c L_jj phi with the full Laplacian;
+    phi rebuilt outside the step from u* as in the Eq. 22 pin."""
+    nu, dt = 0.05, 5e-3
+    S = make(oracle, 12, 8, 10, (0, bc_z), stretch, nu=nu, implicit_xyz=1, sgs_model=0)
+    random_solenoidal(S, seed=43)
+    _, dzf, _ = np_metrics(S)
+    p_old = S.get(S.P)
+    for rk in (0, 1):
+        S.substep(rk, dt)
+        ga = oracle.rk3_coeffs(rk)[2]
+        us, vs, ws = S.ustar()
+        wm = np.roll(ws, 1, 0)
+        if bc_z == 1:
+            wm[0] = 0.0
+        f = ((us - np.roll(us, 1, 2)) / S.dx + (vs - np.roll(vs, 1, 1)) / S.dy + (ws - wm) / dzf[:, None, None]) / (ga * dt)
+        phi = S.poisson_solve(f)
+        c = ga * nu * dt / 2
+        p_new = S.get(S.P)
+        want = phi - c * np_laplacian(S, phi)
+        assert np.max(np.abs((p_new - p_old) - want)) < 1e-11 * np.max(np.abs(want))
+        assert np.max(np.abs(c * np_laplacian(S, phi))) > 1e-5 * np.max(np.abs(phi))
+        p_old = p_new
+
+
+def test_fully_implicit_ustar_is_the_helmholtz_solution(oracle):
+    """Eq. 17-18 assembled outside the step: u** from the (pinned) advection and diffusion terms of a projected field with
+    p = 0, then (1 - c L) u* = u** - c L u^k by dense-free numpy: apply (1 - c L) to the oracle's u* and compare."""
+    nu, dt = 0.05, 5e-3
+    S = make(oracle, 12, 8, 10, (0, 1), True, nu=nu, implicit_xyz=1, sgs_model=0)
+    u0 = random_solenoidal(S, seed=47)
+    adv = S.advection()
+    al, _, ga = oracle.rk3_coeffs(0)
+    c = ga * nu * dt / 2
+    S.substep(0, dt)
+    for comp, (q0, a, qs) in enumerate(zip(u0, adv, S.ustar())):
+        lq0 = np_lap_comp(S, q0, comp)
+        rhs = q0 + dt * al * a + 2 * c * lq0 - c * lq0            # u** - c L u^k, Eq. 17 with H = advection only, p = 0
+        lhs = qs - c * np_lap_comp(S, qs, comp)
+        if comp == 2:
+            rhs[-1] = 0.0
+        assert np.max(np.abs(lhs - rhs)) < 1e-12 * np.max(np.abs(rhs))
