@@ -74,6 +74,10 @@ typedef struct {
   int wall_model_y;          /* log-law wall model on the y walls too (duct WMLES); needs bc_y = wall */
   int dsm_filter3d;          /* dynamic model: 1 = 3-D box test filter (x, y, z; identity in z and alpha = 4^(1/3) in the first
                                 off-wall layer, alpha = 2 elsewhere); 0 = x-y filter */
+  int implicit_xyz;          /* Crank-Nicolson in all three directions, Eq. 17-19: three modified Helmholtz solves
+                                per substep with the eigen-expansion solver.  Needs periodic y (the transforms want
+                                homogeneous conditions); the wall model stays available on the z walls; excludes
+                                implicit_z */
 } cales_params;
 
 typedef struct {
@@ -95,7 +99,8 @@ size_t cales_workspace_bytes(const cales_params* p);
 
 /* Create a solver.  Validates the parameters (CALES_EINVAL: bad sizes / null pointers / workspace too small;
  * CALES_EUNSUPPORTED: sizes that do not factor into 2 and 3, odd nx or ny, periodic z with stretching, wall model
- * without z walls, van Driest without z walls / with y walls / with the wall model),
+ * without z walls, van Driest without z walls / with y walls / with the wall model, implicit_xyz with y walls or together
+ * with implicit_z),
  * builds the grid and the transform tables on the host, uploads them into the workspace, zeroes all fields.
  * Synchronises the stream. */
 int cales_create(const cales_params* p, cales_solver** out);

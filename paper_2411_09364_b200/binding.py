@@ -25,7 +25,7 @@ class CalesParams(C.Structure):
         ("implicit_z", C.c_int),
         ("const_flow_rate", C.c_int), ("u_bulk", C.c_double),
         ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t), ("cuda_stream", C.c_void_p), ("device", C.c_int),
-        ("wall_model_y", C.c_int), ("dsm_filter3d", C.c_int),
+        ("wall_model_y", C.c_int), ("dsm_filter3d", C.c_int), ("implicit_xyz", C.c_int),
     ]
 
 

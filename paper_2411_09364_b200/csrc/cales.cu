@@ -128,10 +128,10 @@ extern "C" size_t cales_workspace_bytes(const cales_params* p) {
 
 // Kernel ids for the per-kernel timing table (cales_kernel_time).
 enum { K_RHS = 0, K_CN_COEF, K_CN_Z, K_SUM, K_BULK, K_FFTX_FWD, K_FFTY_FWD, K_POISSON_Z, K_FFTY_INV, K_FFTX_INV, K_CORRECT,
-       K_WALL, K_SMAG, K_DSM_PASS1, K_DSM_COL, K_DSM_COEF, K_DSM_NUT, K_FILL, K_TRANSPOSE, K_DIAG, K_DSM3, K_DSM3_COL, K_COUNT };
+       K_WALL, K_SMAG, K_DSM_PASS1, K_DSM_COL, K_DSM_COEF, K_DSM_NUT, K_FILL, K_TRANSPOSE, K_DIAG, K_DSM3, K_DSM3_COL, K_HELM_Z, K_COUNT };
 static const char* const k_names[K_COUNT] = {"k_rhs", "k_cn_coef", "k_cn_z", "k_sum_stage1", "k_bulk_finish", "k_fft_x_fwd", "k_fft_y_fwd",
   "k_poisson_z", "k_fft_y_inv", "k_fft_x_inv", "k_correct", "k_wall_stress", "k_smag", "k_dsm_pass1", "k_dsm_col", "k_dsm_coef", "k_dsm_nut", "k_fill",
-  "k_transpose_xy", "k_diag", "k_dsm3_pass1", "k_dsm3_col"};
+  "k_transpose_xy", "k_diag", "k_dsm3_pass1", "k_dsm3_col", "k_helm_z"};
 
 // record an event on the stream tagged with the kernel that just finished (kid < 0: a separator)
 static void tick(cales_solver* s, int kid) {
@@ -425,22 +425,41 @@ static int substep(cales_solver* s, int rk, double dt) {
   int rc;
   double al, be, ga; rk3_coeffs(rk, al, be, ga);
   const Ctx& c = s->c;
-  const bool cfr = c.const_flow_rate != 0, imp = c.implicit_z != 0;
+  const bool cfr = c.const_flow_rate != 0, imp = c.implicit_z == 1, imp3 = c.implicit_z == 2;
   RhsArgs a;
   a.u = s->u; a.v = s->v; a.w = s->w; a.p = s->p; a.nut = s->nut;
   a.Ru0 = s->Ru; a.Rv0 = s->Rv; a.Rw0 = s->Rw; a.Ru1 = s->Ru; a.Rv1 = s->Rv; a.Rw1 = s->Rw;
   a.us = s->us; a.vs = s->vs; a.ws = s->ws; a.dt = dt; a.al = al; a.be = be; a.ga = ga; a.store_R = rk < 2 ? 1 : 0;
   const int kz = rt_chunk(c.nx, c.ny, c.nz);
   dim3 rgrid((c.nx + RT_TX - 1) / RT_TX, (c.ny + RT_TY - 1) / RT_TY, (c.nz + kz - 1) / kz);
-  if (s->N >= s->rhs_tile_min && s->rhs_variant == 0 && s->rmaps_ok) k_rhs_tile_tma<<<rgrid, RT_THREADS, RT_SMEM_TMA_BYTES, s->st>>>(c, a, s->rmaps, kz, (cfr && !imp) ? s->partial : nullptr);
-  else if (s->N >= s->rhs_tile_min) k_rhs_tile<<<rgrid, RT_THREADS, RT_SMEM_DOUBLES * sizeof(double), s->st>>>(c, a, kz, (cfr && !imp) ? s->partial : nullptr);
-  else { rgrid = s->pgrid; k_rhs_point<<<s->pgrid, s->pblock, 0, s->st>>>(c, a, (cfr && !imp) ? s->partial : nullptr); }
+  if (s->N >= s->rhs_tile_min && s->rhs_variant == 0 && s->rmaps_ok) k_rhs_tile_tma<<<rgrid, RT_THREADS, RT_SMEM_TMA_BYTES, s->st>>>(c, a, s->rmaps, kz, (cfr && !imp && !imp3) ? s->partial : nullptr);
+  else if (s->N >= s->rhs_tile_min) k_rhs_tile<<<rgrid, RT_THREADS, RT_SMEM_DOUBLES * sizeof(double), s->st>>>(c, a, kz, (cfr && !imp && !imp3) ? s->partial : nullptr);
+  else { rgrid = s->pgrid; k_rhs_point<<<s->pgrid, s->pblock, 0, s->st>>>(c, a, (cfr && !imp && !imp3) ? s->partial : nullptr); }
   LAUNCH_TRY(K_RHS);
   long long npart = (long long)rgrid.x * rgrid.y * rgrid.z;
   if (imp) {
     const int th = (s->nxy / 128 < 4 * 148) ? 64 : 128; const unsigned g = (unsigned)((s->nxy + th - 1) / th);
     k_cn_z<<<dim3(g, 3), th, 0, s->st>>>(c, s->cncoef + (size_t)rk * 6 * c.nz, s->us, s->vs, s->ws, cfr ? s->partial : nullptr); LAUNCH_TRY(K_CN_Z);
     npart = g;
+  }
+  if (imp3) {
+    // Eq. 18: three modified Helmholtz solves with the transforms of the Poisson solver and a shifted tridiagonal system in z;
+    // us, vs, ws hold the right-hand sides u** - c L u^k and receive u*
+    const double cimp = 0.5 * ga * c.nu * dt;
+    double* Q[3] = {s->us, s->vs, s->ws};
+    const int th = (s->nxy / 128 < 4 * 148) ? 64 : 128;
+    for (int comp = 0; comp < 3; ++comp) {
+      if ((rc = run_transform_x_fwd(s, Q[comp], nullptr, s->W))) return rc;
+      if ((rc = run_transform_y(s, s->W, 0))) return rc;
+      k_helm_z<<<(unsigned)((s->nxy + th - 1) / th), th, 0, s->st>>>(c, s->pt, comp == 2 ? 1 : 0, cimp, s->W, s->CP, s->CQ);
+      LAUNCH_TRY(K_HELM_Z);
+      if ((rc = run_transform_y(s, s->W, 1))) return rc;
+      if ((rc = run_transform_x_inv(s, s->W, Q[comp]))) return rc;
+    }
+    if (cfr) {
+      k_weighted_sum<<<s->pgrid, s->pblock, 0, s->st>>>(c, s->us, s->partial); LAUNCH_TRY(K_SUM);
+      npart = s->nblk;
+    }
   }
   if (cfr) {
     const int g1 = (int)(npart < 1024 ? npart : 1024);
@@ -453,7 +472,7 @@ static int substep(cales_solver* s, int rk, double dt) {
   if ((rc = run_transform_x_inv(s, s->W, s->W))) return rc;
   CorrArgs ca;
   ca.phi = s->W; ca.us = s->us; ca.vs = s->vs; ca.ws = s->ws; ca.u = s->u; ca.v = s->v; ca.w = s->w; ca.p = s->p;
-  ca.shift = cfr ? s->scal : nullptr; ca.gdt = ga * dt; ca.cimp = imp ? 0.5 * ga * c.nu * dt : 0.0; ca.update_p = 1;
+  ca.shift = cfr ? s->scal : nullptr; ca.gdt = ga * dt; ca.cimp = (imp || imp3) ? 0.5 * ga * c.nu * dt : 0.0; ca.cxy = imp3 ? ca.cimp : 0.0; ca.update_p = 1;
   k_correct<<<s->pgrid, s->pblock, 0, s->st>>>(c, ca);
   LAUNCH_TRY(K_CORRECT);
   if ((rc = run_wall_stress(s))) return rc;
@@ -468,7 +487,7 @@ extern "C" int cales_step(cales_solver* s, double dt) {
   int rc;
   s->launches = 0; s->evn = 0; s->ev_valid = false;
   if (!s->fresh && (rc = refresh_closures(s))) return rc;
-  if (s->c.implicit_z && dt != s->cn_dt) {
+  if (s->c.implicit_z == 1 && dt != s->cn_dt) {
     // Eq. 21's tridiagonal coefficients depend on k and on gamma*nu*dt only: like the grid metrics they are a host-built table,
     // rebuilt when dt changes (the forward elimination of the constant matrix is a serial recurrence over nz levels)
     s->h_cn.resize(18 * (size_t)s->c.nz);
@@ -536,7 +555,7 @@ extern "C" int cales_set_option(cales_solver* s, const char* key, long long valu
 extern "C" int cales_launches_per_step(cales_solver* s) {
   if (!s) return 0;
   const Ctx& c = s->c;
-  int per = 1 /*rhs*/ + (c.implicit_z ? 1 : 0) + (c.const_flow_rate ? 2 : 0) + 5 /*solver*/ + 1 /*correct*/ + (c.wall_model ? 1 : 0) + (c.wall_model_y ? 1 : 0) +
+  int per = 1 /*rhs*/ + (c.implicit_z == 1 ? 1 : 0) + (c.implicit_z == 2 ? 15 + (c.const_flow_rate ? 1 : 0) : 0) + (c.const_flow_rate ? 2 : 0) + 5 /*solver*/ + 1 /*correct*/ + (c.wall_model ? 1 : 0) + (c.wall_model_y ? 1 : 0) +
             1 /*static nu_t or fill*/;
   if (c.sgs == CALES_SGS_DSMAG) {
     const bool ywall = c.bc_y == BC_WALL, split = ywall && c.ny >= 3 * DSM_TY;
@@ -594,7 +613,7 @@ extern "C" int cales_project(cales_solver* s) {
   if ((rc = run_transform_x_inv(s, s->W, s->W))) return rc;
   CorrArgs ca;
   ca.phi = s->W; ca.us = s->u; ca.vs = s->v; ca.ws = s->w; ca.u = s->u; ca.v = s->v; ca.w = s->w; ca.p = s->p;
-  ca.shift = nullptr; ca.gdt = 1.0; ca.cimp = 0.0; ca.update_p = 0;
+  ca.shift = nullptr; ca.gdt = 1.0; ca.cimp = 0.0; ca.cxy = 0.0; ca.update_p = 0;
   k_correct<<<s->pgrid, s->pblock, 0, s->st>>>(s->c, ca);
   LAUNCH_TRY(K_CORRECT);
   s->fresh = false;
@@ -709,9 +728,9 @@ extern "C" int cales_diagnostics(cales_solver* s, cales_diag* out) {
   const double vol = (double)s->c.nx * s->c.ny * s->c.lz;
   out->max_div = md; out->u_bulk = ub / vol; out->kinetic_energy = ke / vol; out->nan_count = (int)bad;
   out->forcing = s->c.const_flow_rate ? scal[1] : 0.0; out->wm_max_iters = mi;
-  out->ms_rhs = s->kms[K_RHS]; out->ms_implicit = s->kms[K_CN_COEF] + s->kms[K_CN_Z];
+  out->ms_rhs = s->kms[K_RHS]; out->ms_implicit = s->kms[K_CN_COEF] + s->kms[K_CN_Z] + s->kms[K_HELM_Z];
   out->ms_solver = s->kms[K_SUM] + s->kms[K_BULK] + s->kms[K_FFTX_FWD] + s->kms[K_FFTY_FWD] + s->kms[K_POISSON_Z] + s->kms[K_FFTY_INV] + s->kms[K_FFTX_INV];
   out->ms_correction = s->kms[K_CORRECT]; out->ms_wall = s->kms[K_WALL];
-  out->ms_sgs = s->kms[K_SMAG] + s->kms[K_DSM_PASS1] + s->kms[K_DSM_COL] + s->kms[K_DSM_COEF] + s->kms[K_DSM_NUT] + s->kms[K_FILL];
+  out->ms_sgs = s->kms[K_SMAG] + s->kms[K_DSM_PASS1] + s->kms[K_DSM_COL] + s->kms[K_DSM_COEF] + s->kms[K_DSM_NUT] + s->kms[K_FILL] + s->kms[K_DSM3] + s->kms[K_DSM3_COL];
   return CALES_OK;
 }

@@ -19,7 +19,7 @@ enum { GH_VISC = 0, GH_STRAIN = 1 };  // ghost of the wall-parallel velocity at 
 struct Ctx {
   int nx, ny, nz;
   int bc_y, bc_z, wall_model, wall_model_y, sgs, van_driest, implicit_z, dsm_plane, dsm_clip_total, dsm_filter3d, const_flow_rate;
-  int wm_maxit;
+  int wm_maxit;   // implicit_z above: 0 explicit diffusion, 1 Crank-Nicolson in z (Eq. 20-22), 2 in all three directions (Eq. 17-19)
   int wy_q1;       // y-wall model: the sample lies between centres wy_q1 and wy_q1 + 1 counted from the wall
   long long N;     // nx*ny*nz
   long long nxy;   // nx*ny

@@ -39,6 +39,8 @@ static inline int validate(const cales_params* p) {
   if (p->wall_model_y && p->bc_y != CALES_BC_WALL) return fail(CALES_EUNSUPPORTED, "wall model on y walls needs y walls");
   if (p->dsm_filter3d && p->sgs_model != CALES_SGS_DSMAG) return fail(CALES_EINVAL, "dsm_filter3d needs the dynamic model");
   if (p->implicit_z && p->bc_z != CALES_BC_WALL) return fail(CALES_EUNSUPPORTED, "implicit z needs z walls");
+  if (p->implicit_xyz && p->bc_y != CALES_BC_PERIODIC) return fail(CALES_EUNSUPPORTED, "fully implicit diffusion needs periodic y (PAPER.md:136)");
+  if (p->implicit_xyz && p->implicit_z) return fail(CALES_EINVAL, "implicit_z and implicit_xyz exclude each other");
   if (p->wall_model && p->h_wm > 0.0 && !(p->h_wm < 0.5 * p->lz)) return fail(CALES_EINVAL, "h_wm must lie below the half height");
   if (p->wall_model_y && p->h_wm > 0.0 && !(p->h_wm < 0.5 * p->ly)) return fail(CALES_EINVAL, "h_wm must lie below the half width");
   if (p->van_driest && (p->bc_z != CALES_BC_WALL || p->bc_y == CALES_BC_WALL || p->wall_model))
@@ -149,7 +151,7 @@ static inline int build_setup(const cales_params* p, HostSetup& H) {
   Ctx& c = H.c;
   c.nx = nx; c.ny = ny; c.nz = nz; c.N = (long long)nx * ny * nz; c.nxy = (long long)nx * ny;
   c.bc_y = p->bc_y; c.bc_z = p->bc_z; c.wall_model = p->wall_model; c.wall_model_y = p->wall_model_y; c.dsm_filter3d = p->dsm_filter3d; c.sgs = p->sgs_model; c.van_driest = p->van_driest;
-  c.implicit_z = p->implicit_z; c.dsm_plane = p->dsm_avg_xy_plane; c.dsm_clip_total = p->dsm_clip_total; c.const_flow_rate = p->const_flow_rate;
+  c.implicit_z = p->implicit_xyz ? 2 : (p->implicit_z ? 1 : 0); c.dsm_plane = p->dsm_avg_xy_plane; c.dsm_clip_total = p->dsm_clip_total; c.const_flow_rate = p->const_flow_rate;
   c.wm_maxit = H.P.wm_maxit; c.dx = dx; c.dy = dy; c.rdx = 1.0 / dx; c.rdy = 1.0 / dy; c.lz = p->lz; c.nu = p->nu; c.cs = p->cs; c.aplus = H.P.aplus; c.rnuap = 1.0 / (p->nu * H.P.aplus);
   c.alpha = p->dsm_alpha2d > 0.0 ? p->dsm_alpha2d : std::cbrt(4.0);
   c.kappa = H.P.kappa; c.Blog = p->B; c.h_wm = p->h_wm; c.wm_tol = H.P.wm_tol; c.u_bulk = p->u_bulk;

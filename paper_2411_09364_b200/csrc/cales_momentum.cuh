@@ -25,7 +25,8 @@ struct CorrArgs {
   double *u, *v, *w, *p;
   const double* shift;     // device scalar: uniform shift of u* that restores the bulk velocity (0 if no forcing)
   double gdt;              // gamma dt
-  double cimp;             // gamma nu dt / 2 if implicit z else 0
+  double cimp;             // gamma nu dt / 2 if implicit z (or fully implicit) else 0
+  double cxy;              // gamma nu dt / 2 if fully implicit (Eq. 19: the x and y parts of L_jj phi) else 0
   int update_p;
 };
 
@@ -52,6 +53,10 @@ CALES_HD void correct_point(const Ctx& c, const CorrArgs& a, int i, int j, int k
   if (a.update_p) {
     double dp = ph;
     if (a.cimp != 0.0) dp -= a.cimp * (((phz - ph) * rdzc - (ph - phm) * c.rdzc[k - 1]) * c.rdzf[k]);
+    if (a.cxy != 0.0) {      // Eq. 19 (periodic x and y)
+      const double pxm = scalg(c, a.phi, i - 1, j, k, 1.0), pym = scalg(c, a.phi, i, j - 1, k, 1.0);
+      dp -= a.cxy * ((phx - 2.0 * ph + pxm) * c.rdx * c.rdx + (phy - 2.0 * ph + pym) * c.rdy * c.rdy);
+    }
     a.p[n] += dp;
   }
 }

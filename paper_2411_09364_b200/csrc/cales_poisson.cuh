@@ -111,6 +111,63 @@ CALES_HD void poisson_column(const Ctx& c, const PoissonTabs& T, int i, int j, d
   for (int k = 0; k < nz; ++k) A[col + st * k] -= f * CQ[col + st * k];
 }
 
+// Helmholtz column (i,j) of Eq. 18: (1 - c (L_zz + lam_x + lam_y)) q = d in place, for a velocity
+// component in the spectral (packed real) layout.  fam 0: centred in z (u, v) with the no-slip mirror ghost folded into the
+// diagonal, or the zero-flux closure with the wall model (its lagged stress is a source outside the operator);
+// fam 1: on z faces (w), unknowns k = 0..nz-2, w = 0 on the wall faces.  Periodic z: cyclic Thomas (Sherman-Morrison).
+CALES_HD void helm_column(const Ctx& c, const PoissonTabs& T, int fam, double cimp, int i, int j, double* __restrict__ A,
+                          double* __restrict__ CP, double* __restrict__ CQ) {
+  const int nz = c.nz;
+  const long long col = (long long)i + (long long)c.nx * j, st = c.nxy;
+  const bool per = c.bc_z == BC_PER;
+  const int m = (fam == 1 && !per) ? nz - 1 : nz;
+  const double e = fam == 1 ? 1.0 : (c.wall_model ? 0.0 : 2.0);
+  const double sh = 1.0 - cimp * (T.lamx[i] + T.lamy[j]);
+  auto ak = [&](int k) { return fam == 0 ? T.ak[k] : c.rdzc[k] * c.rdzf[k]; };
+  auto ck = [&](int k) { return fam == 0 ? T.ck[k] : c.rdzc[k] * c.rdzf[k + 1]; };
+  auto diag = [&](int k) { return sh + cimp * (((k == 0 && !per) ? e : 1.0) * ak(k) + ((k == m - 1 && !per) ? e : 1.0) * ck(k)); };
+  if (!per) {
+    double cp = 0.0, dp = 0.0;
+    for (int k = 0; k < m; ++k) {
+      const double lo = -cimp * ak(k), up = -cimp * ck(k);
+      const double r = 1.0 / (k == 0 ? diag(k) : diag(k) - lo * cp);
+      cp = up * r; dp = (k == 0 ? A[col + st * k] : A[col + st * k] - lo * dp) * r;
+      CP[col + st * k] = cp; A[col + st * k] = dp;
+    }
+    double x = dp;
+    for (int k = m - 2; k >= 0; --k) { x = A[col + st * k] - CP[col + st * k] * x; A[col + st * k] = x; }
+    for (int k = m; k < nz; ++k) A[col + st * k] = 0.0;
+    return;
+  }
+  const double l0 = -cimp * ak(0), un = -cimp * ck(nz - 1);
+  const double g = -diag(0);
+  double cp = 0.0, dp = 0.0, qp = 0.0;
+  for (int k = 0; k < nz; ++k) {
+    const double lo = -cimp * ak(k), up = -cimp * ck(k);
+    double b = diag(k);
+    if (k == 0) b -= g;
+    if (k == nz - 1) b -= l0 * un / g;
+    const double uu = k == 0 ? g : (k == nz - 1 ? un : 0.0);
+    const double d = A[col + st * k];
+    const double r = 1.0 / (k == 0 ? b : b - lo * cp);
+    cp = up * r;
+    dp = (k == 0 ? d : d - lo * dp) * r;
+    qp = (k == 0 ? uu : uu - lo * qp) * r;
+    CP[col + st * k] = cp; A[col + st * k] = dp; CQ[col + st * k] = qp;
+  }
+  double y = dp, q = qp;
+  const double yn = y, qn = q;
+  for (int k = nz - 2; k >= 0; --k) {
+    const double cpk = CP[col + st * k];
+    y = A[col + st * k] - cpk * y;
+    q = CQ[col + st * k] - cpk * q;
+    A[col + st * k] = y; CQ[col + st * k] = q;
+  }
+  const double vy = y + l0 * yn / g, vq = q + l0 * qn / g;
+  const double f = vy / (1.0 + vq);
+  for (int k = 0; k < nz; ++k) A[col + st * k] -= f * CQ[col + st * k];
+}
+
 // Crank-Nicolson coefficients of Eq. 21 for substep constant cimp = gamma nu dt / 2, computed once per substep by one
 // thread: for the centred components (u, v; no-slip ghost folded into the diagonal) and for w (faces 0..nz-2).
 // Layout of `coef`: [0] lower a, [1] c' (modified upper), [2] 1/den for u,v; [3],[4],[5] the same for w.
@@ -184,6 +241,19 @@ __global__ void k_poisson_z(Ctx c, PoissonTabs T, double* __restrict__ A, double
   const long long col = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (col >= c.nxy) return;
   poisson_column(c, T, (int)(col % c.nx), (int)(col / c.nx), A, CP, CQ);
+}
+__global__ void k_helm_z(Ctx c, PoissonTabs T, int fam, double cimp, double* __restrict__ A, double* __restrict__ CP, double* __restrict__ CQ) {
+  const long long col = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (col >= c.nxy) return;
+  helm_column(c, T, fam, cimp, (int)(col % c.nx), (int)(col / c.nx), A, CP, CQ);
+}
+// partial[block] = sum over the block's points of q dzf[k] (bulk velocity of u* after the Helmholtz solves); grid/block of the point kernels
+__global__ void __launch_bounds__(256) k_weighted_sum(Ctx c, const double* __restrict__ q, double* __restrict__ partial) {
+  __shared__ double red[32];
+  const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y * blockDim.y + threadIdx.y, k = blockIdx.z;
+  const double s = (i < c.nx && j < c.ny) ? q[idx3(c, i, j, k)] * c.dzf[k] : 0.0;
+  const double t = block_sum(s, red);
+  if (threadIdx.x == 0 && threadIdx.y == 0) partial[blockIdx.x + gridDim.x * (blockIdx.y + (long long)gridDim.y * blockIdx.z)] = t;
 }
 // grid (ceil(nxy / blockDim), 3): blockIdx.y = component (0 u, 1 v, 2 w), one launch for the three independent solves so that
 // small planes still fill the machine.  For u the dzf-weighted column sums are reduced per block into partial[blockIdx.x].

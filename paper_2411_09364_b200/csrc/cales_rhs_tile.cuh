@@ -66,8 +66,9 @@ CALES_HD double rhs_core(const Ctx& c, const RhsArgs& a, const A& q, int i, int 
   double du = (up00 - 2.0 * u000 + um00) * rdx2 + (u0p0 - 2.0 * u000 + u0m0) * rdy2;
   double dv = (vp00 - 2.0 * v000 + vm00) * rdx2 + (v0p0 - 2.0 * v000 + v0m0) * rdy2;
   double dw = (wp00 - 2.0 * w000 + wm00) * rdx2 + (w0p0 - 2.0 * w000 + w0m0) * rdy2;
+  const double lxu = du, lxv = dv, lxw = dw;      // (L_xx + L_yy) u_i
   if (!c.implicit_z) { du += lzu; dv += lzv; dw += lzw; }
-  Ru += c.nu * du; Rv += c.nu * dv; Rw += c.nu * dw;
+  if (c.implicit_z != 2) { Ru += c.nu * du; Rv += c.nu * dv; Rw += c.nu * dw; }      // Eq. 17: all of nu L_jj u goes with gamma
   if (c.sgs) {   // d_j(2 nu_t S_ij), edge viscosity = mean of the 4 surrounding centres (S6)
     const double n000 = q.NT(0, 0, 0), np00 = q.NT(1, 0, 0), nm00 = q.NT(-1, 0, 0), n0p0 = q.NT(0, 1, 0), n0m0 = q.NT(0, -1, 0),
                  n00p = q.NT(0, 0, 1), n00m = q.NT(0, 0, -1), npp0 = q.NT(1, 1, 0), npm0 = q.NT(1, -1, 0), nmp0 = q.NT(-1, 1, 0),
@@ -105,6 +106,7 @@ CALES_HD double rhs_core(const Ctx& c, const RhsArgs& a, const A& q, int i, int 
       ltv = (up * (v00p - v000) * rdzc - lo * (v000 - v00m) * rdzcm) * rdzf;
     }
     us += fe * lzu - fi * ltu; vs += fe * lzv - fi * ltv; ws += (fe - fi) * lzw;
+    if (c.implicit_z == 2) { us += (fe - fi) * lxu; vs += (fe - fi) * lxv; ws += (fe - fi) * lxw; }   // Eq. 17 explicit half + right-hand side of Eq. 18
   }
   if (!vact) vs = 0.0;
   if (!wact) ws = 0.0;

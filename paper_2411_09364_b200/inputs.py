@@ -18,7 +18,7 @@ KAPPA, BLOG = 0.41, 5.2
 def _base(**kw):
     d = dict(zstretch=0, zstretch_factor=0.0, bc_y=0, bc_z=0, nu=1e-3, sgs_model=0, cs=0.17, van_driest=0,
              aplus=25.0, dsm_avg_xy_plane=1, dsm_clip_total=0, dsm_alpha2d=0.0, wall_model=0, kappa=KAPPA,
-             B=BLOG, h_wm=0.0, wm_tol=1e-4, wm_maxit=50, implicit_z=0, const_flow_rate=0, u_bulk=0.0, wall_model_y=0, dsm_filter3d=0)
+             B=BLOG, h_wm=0.0, wm_tol=1e-4, wm_maxit=50, implicit_z=0, const_flow_rate=0, u_bulk=0.0, wall_model_y=0, dsm_filter3d=0, implicit_xyz=0)
     d.update(kw)
     return d
 

@@ -334,7 +334,7 @@ static void emu_refresh(emu_solver* s) {
 static void emu_substep(emu_solver* s, int rk, double dt) {
   const Ctx& c = s->c;
   double al, be, ga; rk3_coeffs(rk, al, be, ga);
-  const bool cfr = c.const_flow_rate != 0, imp = c.implicit_z != 0;
+  const bool cfr = c.const_flow_rate != 0, imp = c.implicit_z == 1;      // the fully implicit scheme (implicit_z == 2) is covered on the GPU only
   RhsArgs a;
   a.u = s->u.data(); a.v = s->v.data(); a.w = s->w.data(); a.p = s->p.data(); a.nut = s->nut.data();
   a.Ru0 = s->Ru.data(); a.Rv0 = s->Rv.data(); a.Rw0 = s->Rw.data(); a.Ru1 = s->Ru.data(); a.Rv1 = s->Rv.data(); a.Rw1 = s->Rw.data();
@@ -377,7 +377,7 @@ static void emu_substep(emu_solver* s, int rk, double dt) {
   CorrArgs ca;
   ca.phi = s->W.data(); ca.us = s->us.data(); ca.vs = s->vs.data(); ca.ws = s->ws.data();
   ca.u = s->u.data(); ca.v = s->v.data(); ca.w = s->w.data(); ca.p = s->p.data();
-  ca.shift = cfr ? s->scal : nullptr; ca.gdt = ga * dt; ca.cimp = imp ? 0.5 * ga * c.nu * dt : 0.0; ca.update_p = 1;
+  ca.shift = cfr ? s->scal : nullptr; ca.gdt = ga * dt; ca.cimp = imp ? 0.5 * ga * c.nu * dt : 0.0; ca.cxy = 0.0; ca.update_p = 1;
   for (int k = 0; k < c.nz; ++k) for (int j = 0; j < c.ny; ++j) for (int i = 0; i < c.nx; ++i) correct_point(c, ca, i, j, k);
   emu_refresh(s);
 }
@@ -412,7 +412,7 @@ extern "C" int emu_project(emu_solver* s) {
   CorrArgs ca;
   ca.phi = s->W.data(); ca.us = s->u.data(); ca.vs = s->v.data(); ca.ws = s->w.data();
   ca.u = s->u.data(); ca.v = s->v.data(); ca.w = s->w.data(); ca.p = s->p.data();
-  ca.shift = nullptr; ca.gdt = 1.0; ca.cimp = 0.0; ca.update_p = 0;
+  ca.shift = nullptr; ca.gdt = 1.0; ca.cimp = 0.0; ca.cxy = 0.0; ca.update_p = 0;
   for (int k = 0; k < c.nz; ++k) for (int j = 0; j < c.ny; ++j) for (int i = 0; i < c.nx; ++i) correct_point(c, ca, i, j, k);
   s->fresh = false;
   return 0;

@@ -48,6 +48,12 @@ GPU_CASES = {
     "cfg4_duct_dsm_filter3d": (4, (72, 36, 24), 2, dict(dsm_filter3d=1)),
     "duct_wmles_dsm_filter3d": (4, (72, 36, 24), 2, dict(wall_model=1, wall_model_y=1, nu=1.0 / 40000, dsm_filter3d=1)),
     "cfg1_dsm_filter3d": (1, None, 3, dict(sgs_model=2, dsm_filter3d=1)),
+    # fully implicit Crank-Nicolson (8(f) item 3, Eq. 17-19): triply periodic box, tanh channel with van Driest + forcing,
+    # wall-modelled channel (wall model restricted to the z walls)
+    "cfg1_implicit_xyz": (1, None, 3, dict(implicit_xyz=1)),
+    "cfg3_implicit_xyz": (3, (96, 72, 48), 3, dict(implicit_z=0, implicit_xyz=1)),
+    "cfg2_wm_implicit_xyz": (2, (96, 48, 32), 2, dict(implicit_xyz=1)),
+    "cfg5_dsm_implicit_xyz": (5, (96, 48, 32), 2, dict(implicit_xyz=1, h_wm=0.1)),
 }
 
 
