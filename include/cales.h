@@ -121,9 +121,18 @@ int cales_get_field(cales_solver* s, int field, double* dst, int dst_on_device);
 
 /* One full RK3 step = 3 substeps of Alg. 1 with the coefficients of PAPER.md:100:
  * u* from Eq. 11 (or Eq. 20-21), bulk forcing, Poisson Eq. 12, correction Eq. 13, pressure Eq. 14 / 22,
- * wall stress Eq. 10, nu_t Eq. 4 / Eq. 5-9.  Asynchronous, except that the first call with a new dt in implicit-z mode
- * uploads the Crank-Nicolson coefficient tables of that dt and synchronises the stream once.  dt > 0. */
+ * wall stress Eq. 10, nu_t Eq. 4 / Eq. 5-9.  Asynchronous for every dt: dt and the scalars derived from it (and the Crank-Nicolson
+ * tables of Eq. 21) are kept in device memory, so a change of dt costs two tiny kernels and neither a synchronisation nor a new
+ * CUDA graph.  dt > 0. */
 int cales_step(cales_solver* s, double dt);
+
+/* The same with the time step chosen on the device: dt = cfl / max over cells of (|u_c|/dx + |v_c|/dy + |w_c|/dzf) of the current
+ * velocity ("maximum allowable value ... multiplied by a safety factor of 0.95"; formula: DESIGN.md reading S18).
+ * Asynchronous, no host synchronisation; cales_last_dt reads the value back. */
+int cales_step_adaptive(cales_solver* s, double cfl);
+
+/* dt of the last step: HOST output; synchronises the stream if that dt was computed on the device. */
+int cales_last_dt(cales_solver* s, double* dt_host);
 
 /* Solve L_h phi = rhs with the solver's boundary conditions (Eq. 12; eigenfunction expansion,
  * PAPER.md:126): real FFT along x, real FFT or DCT-II along y, (cyclic) Thomas along z.  The component of rhs
@@ -157,6 +166,18 @@ int cales_cfl_dt(cales_solver* s, double cfl, double* dt_host);
  * out_dev: DEVICE, [8][nz].  Asynchronous. */
 int cales_plane_stats(cales_solver* s, double* out_dev);
 
+/* Time-accumulated statistics ("mean quantities"; C_f and Re_tau of Tables 3-5).  cales_stats_accumulate adds
+ * weight x (the plane means of cales_plane_stats, the wall-shear means) of the current state to device accumulators (asynchronous;
+ * weight > 0, e.g. dt); cales_stats_reset zeroes them.  cales_stats_get (synchronises; HOST outputs, any may be NULL) returns the
+ * weighted time averages: prof [8][nz]; wall [8] = mean wall shear stress on the z walls ((tau_xz, tau_yz) bottom, then top) and on
+ * the y walls ((tau_xy, tau_zy) at j = 0, then j = ny-1; dzf-weighted), 0 in periodic directions, positive when the wall retards a
+ * flow in the positive direction; modelled walls report the wall-model stress, no-slip walls nu x the one-sided difference to the
+ * mirror ghost; derived [4] = tau_w (mean of the streamwise components over the walls), u_tau = sqrt(tau_w),
+ * Re_tau = u_tau (lz/2) / nu, C_f = 2 tau_w / u_b^2 with u_b the dzf-weighted mean of the averaged <u> profile; *weight = total. */
+int cales_stats_reset(cales_solver* s);
+int cales_stats_accumulate(cales_solver* s, double weight);
+int cales_stats_get(cales_solver* s, double* prof_host, double* wall_host, double* derived_host, double* weight_host);
+
 /* Dynamic coefficient of the last eddy-viscosity evaluation: cs_dev DEVICE, nz (plane averaging) or nz*ny. */
 int cales_get_cs(cales_solver* s, double* cs_dev);
 
@@ -179,7 +200,7 @@ int cales_kernel_count(void);
  * the three may be NULL).  Synchronises the stream. */
 int cales_kernel_time(cales_solver* s, int kid, const char** name, double* ms_total, int* launches);
 
-/* cales_step replays its three substeps as one CUDA graph (captured per value of dt; on by default, bypassed while
+/* cales_step replays its three substeps as one CUDA graph (captured once: dt lives in device memory; on by default, bypassed while
  * timing is on).  on = 0 returns to plain stream launches. */
 int cales_set_graph(cales_solver* s, int on);
 

@@ -224,6 +224,17 @@ class Oracle:
     def plane_stats(self):
         out = np.empty((8, self.nz)); _chk(lib().oracle_plane_stats(self._h, _p(out))); return out
 
+    def stats_reset(self):
+        _chk(lib().oracle_stats_reset(self._h))
+
+    def stats_accumulate(self, weight=1.0):
+        _chk(lib().oracle_stats_accumulate(self._h, C.c_double(weight)))
+
+    def stats_get(self):
+        prof = np.empty((8, self.nz)); wall = np.empty(8); der = np.empty(4); w = C.c_double()
+        _chk(lib().oracle_stats_get(self._h, _p(prof), _p(wall), _p(der), C.byref(w)))
+        return dict(profiles=prof, wall=wall, tau_w=der[0], u_tau=der[1], re_tau=der[2], cf=der[3], weight=w.value)
+
     def project(self):
         _chk(lib().oracle_project(self._h))
 

@@ -216,6 +216,7 @@ struct oracle_solver {
   std::vector<double> tauy;                   // y walls: [wall][comp (0 tau_xy at u points, 1 tau_zy at w points)][nz][nx]
   std::vector<double> cs;                     // dynamic coefficient per k or per (k,j)
   std::vector<double> Lij, Mij;               // tensors of the last dynamic evaluation (for the pins)
+  std::vector<double> st_prof, st_wall; double st_weight = 0.0;   // time accumulators of the on-line statistics
   std::vector<double> ust, vst, wst;          // u*, v*, w* of the last substep, after O-step 6, before the bulk shift (for the pins)
   bool fresh = false;                         // wall stress + nu_t consistent with the velocity
   double forcing = 0.0; int wm_max_iters = 0;
@@ -1208,5 +1209,73 @@ extern "C" int oracle_plane_stats(oracle_solver* S, double* out) {
     }
     for (int q = 0; q < 8; ++q) out[(size_t)q * nz + k] = a[q] / ((double)nx * ny);
   }
+  return 0;
+}
+
+// ---- on-line statistics accumulated in time ("mean quantities"; Tables 3-5 report C_f and Re_tau) ------------------
+// Instantaneous wall shear stress, averaged over each wall.  wall[0..3]: z walls, (tau_xz, tau_yz) at the bottom then the top;
+// wall[4..7]: y walls, (tau_xy, tau_zy) at the j = 0 side then the j = ny-1 side; 0 in periodic directions.  Sign: positive when
+// the wall retards a flow in the positive direction (the convention of the wall-model planes).  Modelled walls: the mean of the
+// wall-model stress planes; no-slip walls: nu times the one-sided difference to the mirror ghost, 2 nu q_first / (ghost spacing).
+static void wall_shear_means(oracle_solver& S, double* wall) {
+  int nx = S.nx, ny = S.ny, nz = S.nz; double nu = S.P.nu;
+  for (int q = 0; q < 8; ++q) wall[q] = 0.0;
+  if (S.P.bc_z == BC_WALL) {
+    for (int wl = 0; wl < 2; ++wl) for (int comp = 0; comp < 2; ++comp) {
+      const F3& f = comp == 0 ? S.u : S.v;
+      int k0 = wl == 0 ? 0 : nz - 1; double dz = wl == 0 ? S.dzc(-1) : S.dzc(nz - 1);
+      double a = 0.0;
+      for (int j = 0; j < ny; ++j) for (int i = 0; i < nx; ++i) a += S.P.wall_model ? S.tw(wl, comp, i, j) : 2.0 * nu * f(i, j, k0) / dz;
+      wall[wl * 2 + comp] = a / ((double)nx * ny);
+    }
+  }
+  if (S.P.bc_y == BC_WALL) {
+    for (int wl = 0; wl < 2; ++wl) for (int comp = 0; comp < 2; ++comp) {
+      const F3& f = comp == 0 ? S.u : S.w;
+      int j0 = wl == 0 ? 0 : ny - 1;
+      double a = 0.0;
+      for (int k = 0; k < nz; ++k) for (int i = 0; i < nx; ++i)
+        a += (S.P.wall_model_y ? S.tauy[((size_t)(wl * 2 + comp) * nz + k) * nx + i] : 2.0 * nu * f(i, j0, k) / S.dy) * S.dzf(k);
+      wall[4 + wl * 2 + comp] = a / ((double)nx * S.P.lz);
+    }
+  }
+}
+extern "C" int oracle_stats_reset(oracle_solver* S) {
+  if (!S) return fail("null");
+  S->st_prof.assign((size_t)8 * S->nz, 0.0); S->st_wall.assign(8, 0.0); S->st_weight = 0.0; return 0;
+}
+// adds weight x (the instantaneous plane means of oracle_plane_stats, the wall-shear means) to the accumulators
+extern "C" int oracle_stats_accumulate(oracle_solver* S, double weight) {
+  if (!S || !(weight > 0.0)) return fail("bad argument");
+  if (S->st_prof.empty()) oracle_stats_reset(S);
+  if (!S->fresh) refresh_closures(*S);       // the wall-model planes must belong to the current velocity
+  std::vector<double> pr((size_t)8 * S->nz); double wl[8];
+  oracle_plane_stats(S, pr.data());
+  wall_shear_means(*S, wl);
+  for (size_t q = 0; q < pr.size(); ++q) S->st_prof[q] += weight * pr[q];
+  for (int q = 0; q < 8; ++q) S->st_wall[q] += weight * wl[q];
+  S->st_weight += weight;
+  return 0;
+}
+// time averages: prof[8][nz], wall[8]; derived[0] = tau_w (mean of the x components on the z walls, or on all four walls of a
+// duct), [1] = u_tau = sqrt(tau_w), [2] = Re_tau = u_tau (lz/2) / nu, [3] = C_f = 2 tau_w / u_b^2 with u_b the dzf-weighted mean
+// of the averaged <u> profile; *weight = accumulated weight
+extern "C" int oracle_stats_get(oracle_solver* S, double* prof, double* wall, double* derived, double* weight) {
+  if (!S || !(S->st_weight > 0.0)) return fail("no statistics accumulated");
+  double w = S->st_weight; int nz = S->nz;
+  std::vector<double> pr(S->st_prof); for (double& q : pr) q /= w;
+  double wl[8]; for (int q = 0; q < 8; ++q) wl[q] = S->st_wall[q] / w;
+  if (prof) std::memcpy(prof, pr.data(), pr.size() * sizeof(double));
+  if (wall) std::memcpy(wall, wl, sizeof(wl));
+  if (derived) {
+    double tw = 0.0; int nw = 0;
+    if (S->P.bc_z == BC_WALL) { tw += wl[0] + wl[2]; nw += 2; }
+    if (S->P.bc_y == BC_WALL) { tw += wl[4] + wl[6]; nw += 2; }
+    tw = nw ? tw / nw : 0.0;
+    double ub = 0.0; for (int k = 0; k < nz; ++k) ub += pr[k] * S->dzf(k); ub /= S->P.lz;
+    derived[0] = tw; derived[1] = tw > 0.0 ? std::sqrt(tw) : 0.0; derived[2] = derived[1] * 0.5 * S->P.lz / S->P.nu;
+    derived[3] = ub != 0.0 ? 2.0 * tw / (ub * ub) : 0.0;
+  }
+  if (weight) *weight = w;
   return 0;
 }

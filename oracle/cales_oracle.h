@@ -108,6 +108,12 @@ int oracle_diagnostics(oracle_solver* s, double* max_div, double* u_bulk, double
 int oracle_cfl_dt(oracle_solver* s, double cfl, double* dt);
 /* x-y plane means per k: out[q][k], q = <u>,<v>,<w>,<uu>,<vv>,<ww>,<uw>,<nu_t> of the centre-averaged velocity */
 int oracle_plane_stats(oracle_solver* s, double* out);
+/* time-accumulated statistics: accumulate adds weight x (plane means of oracle_plane_stats, wall-shear means);
+   get returns the averages prof[8][nz], wall[8] (z walls: tau_xz, tau_yz bottom then top; y walls: tau_xy, tau_zy low then high),
+   derived[4] = tau_w, u_tau, Re_tau = u_tau (lz/2)/nu, C_f = 2 tau_w / u_b^2, and the accumulated weight */
+int oracle_stats_reset(oracle_solver* s);
+int oracle_stats_accumulate(oracle_solver* s, double weight);
+int oracle_stats_get(oracle_solver* s, double* prof, double* wall, double* derived, double* weight);
 /* threads used by the OpenMP loops */
 int oracle_num_threads(void);
 

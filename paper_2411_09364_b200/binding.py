@@ -38,8 +38,8 @@ class CalesDiag(C.Structure):
 
 # every symbol include/cales.h declares
 SYMBOLS = ["cales_default_params", "cales_workspace_bytes", "cales_create", "cales_create_basic", "cales_destroy",
-           "cales_set_field", "cales_get_field", "cales_step", "cales_poisson_solve", "cales_eddy_viscosity",
-           "cales_wall_stress", "cales_wall_stress_y", "cales_project", "cales_cfl_dt", "cales_plane_stats", "cales_get_cs", "cales_transform", "cales_transpose_xy",
+           "cales_set_field", "cales_get_field", "cales_step", "cales_step_adaptive", "cales_last_dt", "cales_poisson_solve", "cales_eddy_viscosity",
+           "cales_wall_stress", "cales_wall_stress_y", "cales_project", "cales_cfl_dt", "cales_plane_stats", "cales_stats_reset", "cales_stats_accumulate", "cales_stats_get", "cales_get_cs", "cales_transform", "cales_transpose_xy",
            "cales_set_timing", "cales_set_graph", "cales_set_option", "cales_kernel_count", "cales_kernel_time", "cales_launches_per_step", "cales_diagnostics", "cales_last_error"]
 
 _lib = None
@@ -62,6 +62,8 @@ def lib():
         L.cales_set_field.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_int]
         L.cales_get_field.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_int]
         L.cales_step.argtypes = [C.c_void_p, C.c_double]
+        L.cales_step_adaptive.argtypes = [C.c_void_p, C.c_double]
+        L.cales_last_dt.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
         L.cales_poisson_solve.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.cales_eddy_viscosity.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.cales_wall_stress.argtypes = [C.c_void_p, C.c_void_p]
@@ -70,6 +72,9 @@ def lib():
         L.cales_get_cs.argtypes = [C.c_void_p, C.c_void_p]
         L.cales_cfl_dt.argtypes = [C.c_void_p, C.c_double, C.POINTER(C.c_double)]
         L.cales_plane_stats.argtypes = [C.c_void_p, C.c_void_p]
+        L.cales_stats_reset.argtypes = [C.c_void_p]
+        L.cales_stats_accumulate.argtypes = [C.c_void_p, C.c_double]
+        L.cales_stats_get.argtypes = [C.c_void_p, _dp, _dp, _dp, C.POINTER(C.c_double)]
         L.cales_transform.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int]
         L.cales_transpose_xy.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.cales_set_timing.argtypes = [C.c_void_p, C.c_int]
@@ -197,6 +202,14 @@ class Solver:
     def step(self, dt):
         _chk(lib().cales_step(self._h, float(dt)))
 
+    def step_adaptive(self, cfl):
+        _chk(lib().cales_step_adaptive(self._h, float(cfl)))
+
+    def last_dt(self):
+        dt = C.c_double()
+        _chk(lib().cales_last_dt(self._h, C.byref(dt)))
+        return dt.value
+
     def poisson_solve(self, rhs, phi=None):
         if phi is None:
             phi = self._torch.empty_like(rhs)
@@ -235,6 +248,18 @@ class Solver:
         out = self._torch.empty((8, self.nz), dtype=self._torch.float64, device=self.device)
         _chk(lib().cales_plane_stats(self._h, C.c_void_p(out.data_ptr())))
         return out
+
+    def stats_reset(self):
+        _chk(lib().cales_stats_reset(self._h))
+
+    def stats_accumulate(self, weight=1.0):
+        _chk(lib().cales_stats_accumulate(self._h, float(weight)))
+
+    def stats_get(self):
+        import numpy as np
+        prof = np.empty((8, self.nz)); wall = np.empty(8); der = np.empty(4); w = C.c_double()
+        _chk(lib().cales_stats_get(self._h, prof.ctypes.data_as(_dp), wall.ctypes.data_as(_dp), der.ctypes.data_as(_dp), C.byref(w)))
+        return dict(profiles=prof, wall=wall, tau_w=der[0], u_tau=der[1], re_tau=der[2], cf=der[3], weight=w.value)
 
     def get_cs(self, per_plane=True):
         n = self.nz if per_plane else self.nz * self.ny

@@ -68,8 +68,10 @@ struct cales_solver {
   int rhs_variant;      // 1 (default): halo planes by 8-byte cp.async (k_rhs_tile); 0: by tiled TMA copies (k_rhs_tile_tma)
   RhsMaps* rmaps; bool rmaps_ok;   // tensor maps of u, v, w, nu_t, p in device memory (workspace)
   int dsm_col_variant;  // 0: TMA-staged register-window column march (k_dsm_col_tma); 1: shared-ring form of round 1 (k_dsm_col_sm); 2: direct loads (k_dsm_col_rw)
-  std::vector<double> h_dzf, h_dzc, h_cn; Ctx hc; double cn_dt;   // host copies for the per-dt CN coefficient tables
-  int use_graph; cudaGraphExec_t gexec; double gdt;   // the three substeps captured as one CUDA graph, keyed by dt
+  double cn_dt;   // dt the Crank-Nicolson tables on the device were built for (0: none, or a device-side dt)
+  int use_graph; cudaGraphExec_t gexec;   // the three substeps captured as one CUDA graph (dt lives in device memory: one graph serves every dt)
+  double* stats;   // [8 nz + 8 wall + 1 weight] accumulators, the same again as scratch
+  double* rks; double* dtdev; double last_dt;   // substep scalar blocks [3][RK_STRIDE], device-side dt of cales_step_adaptive
   int timing; bool ev_valid;
   std::vector<cudaEvent_t> evpool; std::vector<int> evkid; int evn;   // per-launch events of the last timed step
   double kms[32]; int kcnt[32];                                       // per-kernel totals of the last timed step
@@ -100,6 +102,7 @@ static size_t carve(cales_solver* s, const cales_params* p, double* base) {
   double* partial = take(nblk > nxy ? nblk : nxy);
   double* stage1 = take(4 * 1024);
   double* scal = take(32);
+  double* stats = take(2 * (8 * (size_t)p->nz + 16));      // on-line statistics: accumulators, then scratch
   double* tmaps = take(128);      // 5 tensor maps of 128 bytes (cales_rhs_tile.cuh)
   const size_t pslots = (size_t)dsm_shape(p->nx).pslots;
   double* dsm_part = p->sgs_model == CALES_SGS_DSMAG ? take((size_t)p->nz * p->ny * pslots * 2) : nullptr;
@@ -110,7 +113,8 @@ static size_t carve(cales_solver* s, const cales_params* p, double* base) {
     s->dzf = dzf; s->dzc = dzc; s->zc = zc; s->rdzf = rdzf; s->rdzc = rdzc; s->delta = delta; s->ak = ak; s->ck = ck; s->lamx = lamx; s->lamy = lamy;
     s->twx = reinterpret_cast<double2*>(twx); s->twy = reinterpret_cast<double2*>(twy); s->dctw = reinterpret_cast<double2*>(dctw);
     s->cncoef = cncoef; s->partial = partial; s->stage1 = stage1; s->scal = scal; s->maxit = reinterpret_cast<int*>(scal + 16);
-    s->dsm_part = dsm_part; s->dsm_cs = dsm_cs; s->nblk = (long long)nblk; s->rmaps = reinterpret_cast<RhsMaps*>(tmaps);
+    s->rks = scal + 18; s->dtdev = scal + 30;
+    s->dsm_part = dsm_part; s->dsm_cs = dsm_cs; s->nblk = (long long)nblk; s->rmaps = reinterpret_cast<RhsMaps*>(tmaps); s->stats = stats;
   }
   return off * sizeof(double);
 }
@@ -225,8 +229,8 @@ extern "C" int cales_create(const cales_params* p, cales_solver** out) {
   s->pblock = dim3(32, 8, 1);
   s->pgrid = dim3((nx + 31) / 32, (ny + 7) / 8, nz);
   s->fresh = false; s->timing = 0; s->ev_valid = false; s->launches = 0; s->evn = 0;
-  s->use_graph = 1; s->gexec = nullptr; s->gdt = 0.0;
-  s->h_dzf = H.dzf; s->h_dzc = H.dzc; s->hc = s->c; s->hc.dzf = s->h_dzf.data() + 1; s->hc.dzc = s->h_dzc.data() + 1; s->cn_dt = 0.0;
+  s->use_graph = 1; s->gexec = nullptr; s->last_dt = 0.0;
+  s->cn_dt = 0.0;
   s->tile_min = 4000000;
   s->rhs_tile_min = 200000;
   s->dsm_col_variant = 0;
@@ -294,7 +298,7 @@ static int run_transform_x_fwd(cales_solver* s, const double* src, const DivSrc*
   const long long nlines = (long long)s->c.ny * s->c.nz;
   const unsigned grid = (unsigned)((nlines + s->xB - 1) / s->xB);
   if (ds) k_fft2_x_fwd<true><<<grid, s->x_threads, s->x_smem, s->st>>>(s->c, s->plx, s->xB, nullptr, *ds, dst);
-  else { DivSrc z{nullptr, nullptr, nullptr, 0.0}; k_fft2_x_fwd<false><<<grid, s->x_threads, s->x_smem, s->st>>>(s->c, s->plx, s->xB, src, z, dst); }
+  else { DivSrc z{nullptr, nullptr, nullptr, 0.0, nullptr}; k_fft2_x_fwd<false><<<grid, s->x_threads, s->x_smem, s->st>>>(s->c, s->plx, s->xB, src, z, dst); }
   LAUNCH_TRY(K_FFTX_FWD);
   return CALES_OK;
 }
@@ -421,7 +425,7 @@ static int refresh_closures(cales_solver* s) {
   return CALES_OK;
 }
 
-static int substep(cales_solver* s, int rk, double dt) {
+static int substep(cales_solver* s, int rk) {
   int rc;
   double al, be, ga; rk3_coeffs(rk, al, be, ga);
   const Ctx& c = s->c;
@@ -429,7 +433,8 @@ static int substep(cales_solver* s, int rk, double dt) {
   RhsArgs a;
   a.u = s->u; a.v = s->v; a.w = s->w; a.p = s->p; a.nut = s->nut;
   a.Ru0 = s->Ru; a.Rv0 = s->Rv; a.Rw0 = s->Rw; a.Ru1 = s->Ru; a.Rv1 = s->Rv; a.Rw1 = s->Rw;
-  a.us = s->us; a.vs = s->vs; a.ws = s->ws; a.dt = dt; a.al = al; a.be = be; a.ga = ga; a.store_R = rk < 2 ? 1 : 0;
+  const double* sc = s->rks + rk * RK_STRIDE;      // dt, gamma dt, 1/(gamma dt), gamma nu dt / 2 of this substep, in device memory
+  a.us = s->us; a.vs = s->vs; a.ws = s->ws; a.dt = 0.0; a.al = al; a.be = be; a.ga = ga; a.store_R = rk < 2 ? 1 : 0; a.sc = sc;
   const int kz = rt_chunk(c.nx, c.ny, c.nz);
   dim3 rgrid((c.nx + RT_TX - 1) / RT_TX, (c.ny + RT_TY - 1) / RT_TY, (c.nz + kz - 1) / kz);
   if (s->N >= s->rhs_tile_min && s->rhs_variant == 0 && s->rmaps_ok) k_rhs_tile_tma<<<rgrid, RT_THREADS, RT_SMEM_TMA_BYTES, s->st>>>(c, a, s->rmaps, kz, (cfr && !imp && !imp3) ? s->partial : nullptr);
@@ -445,13 +450,12 @@ static int substep(cales_solver* s, int rk, double dt) {
   if (imp3) {
     // Eq. 18: three modified Helmholtz solves with the transforms of the Poisson solver and a shifted tridiagonal system in z;
     // us, vs, ws hold the right-hand sides u** - c L u^k and receive u*
-    const double cimp = 0.5 * ga * c.nu * dt;
     double* Q[3] = {s->us, s->vs, s->ws};
     const int th = (s->nxy / 128 < 4 * 148) ? 64 : 128;
     for (int comp = 0; comp < 3; ++comp) {
       if ((rc = run_transform_x_fwd(s, Q[comp], nullptr, s->W))) return rc;
       if ((rc = run_transform_y(s, s->W, 0))) return rc;
-      k_helm_z<<<(unsigned)((s->nxy + th - 1) / th), th, 0, s->st>>>(c, s->pt, comp == 2 ? 1 : 0, cimp, s->W, s->CP, s->CQ);
+      k_helm_z<<<(unsigned)((s->nxy + th - 1) / th), th, 0, s->st>>>(c, s->pt, comp == 2 ? 1 : 0, sc, s->W, s->CP, s->CQ);
       LAUNCH_TRY(K_HELM_Z);
       if ((rc = run_transform_y(s, s->W, 1))) return rc;
       if ((rc = run_transform_x_inv(s, s->W, Q[comp]))) return rc;
@@ -464,15 +468,15 @@ static int substep(cales_solver* s, int rk, double dt) {
   if (cfr) {
     const int g1 = (int)(npart < 1024 ? npart : 1024);
     k_sum_stage1<<<g1, 256, 0, s->st>>>(s->partial, npart, s->stage1); LAUNCH_TRY(K_SUM);
-    k_bulk_finish<<<1, 256, 0, s->st>>>(c, s->stage1, g1, ga * dt, s->scal); LAUNCH_TRY(K_BULK);
+    k_bulk_finish<<<1, 256, 0, s->st>>>(c, s->stage1, g1, 0.0, sc, s->scal); LAUNCH_TRY(K_BULK);
   }
-  DivSrc ds{s->us, s->vs, s->ws, 1.0 / (ga * dt)};
+  DivSrc ds{s->us, s->vs, s->ws, 0.0, sc};
   if ((rc = run_transform_x_fwd(s, nullptr, &ds, s->W))) return rc;
   if ((rc = run_poisson_core(s))) return rc;
   if ((rc = run_transform_x_inv(s, s->W, s->W))) return rc;
   CorrArgs ca;
   ca.phi = s->W; ca.us = s->us; ca.vs = s->vs; ca.ws = s->ws; ca.u = s->u; ca.v = s->v; ca.w = s->w; ca.p = s->p;
-  ca.shift = cfr ? s->scal : nullptr; ca.gdt = ga * dt; ca.cimp = (imp || imp3) ? 0.5 * ga * c.nu * dt : 0.0; ca.cxy = imp3 ? ca.cimp : 0.0; ca.update_p = 1;
+  ca.shift = cfr ? s->scal : nullptr; ca.gdt = 0.0; ca.cimp = (imp || imp3) ? 1.0 : 0.0; ca.cxy = imp3 ? 1.0 : 0.0; ca.update_p = 1; ca.sc = sc;
   k_correct<<<s->pgrid, s->pblock, 0, s->st>>>(c, ca);
   LAUNCH_TRY(K_CORRECT);
   if ((rc = run_wall_stress(s))) return rc;
@@ -482,44 +486,29 @@ static int substep(cales_solver* s, int rk, double dt) {
 
 extern "C" int cales_launches_per_step(cales_solver* s);
 
-extern "C" int cales_step(cales_solver* s, double dt) {
-  if (!s || !(dt > 0.0)) return fail(CALES_EINVAL, "bad step arguments");
+// The three substeps on the stream: replayed as one CUDA graph (launch-bound sizes: ~25-120 launches of a few microseconds
+// each), or as plain launches while per-kernel timing is on.  dt and everything derived from it live in device memory
+// (s->rks), so the captured graph serves every dt and nothing here synchronises.
+static int run_substeps(cales_solver* s) {
   int rc;
-  s->launches = 0; s->evn = 0; s->ev_valid = false;
-  if (!s->fresh && (rc = refresh_closures(s))) return rc;
-  if (s->c.implicit_z == 1 && dt != s->cn_dt) {
-    // Eq. 21's tridiagonal coefficients depend on k and on gamma*nu*dt only: like the grid metrics they are a host-built table,
-    // rebuilt when dt changes (the forward elimination of the constant matrix is a serial recurrence over nz levels)
-    s->h_cn.resize(18 * (size_t)s->c.nz);
-    for (int rk = 0; rk < 3; ++rk) {
-      double al, be, ga; rk3_coeffs(rk, al, be, ga);
-      cn_coefficients(s->hc, 0.5 * ga * s->c.nu * dt, s->h_cn.data() + (size_t)rk * 6 * s->c.nz);
-    }
-    CUDA_TRY(cudaMemcpyAsync(s->cncoef, s->h_cn.data(), s->h_cn.size() * sizeof(double), cudaMemcpyHostToDevice, s->st));
-    CUDA_TRY(cudaStreamSynchronize(s->st));     // h_cn may be rewritten by the next call
-    s->cn_dt = dt;
-  }
-  // Launch-bound sizes (configs 1-2: ~25-40 launches of a few microseconds each): replay the three substeps as one CUDA
-  // graph.  The graph is captured on first use for a given dt (kernel arguments are baked in) and re-captured when dt
-  // changes; per-kernel timing needs the individual launches, so it bypasses the graph.
   if (s->use_graph && !s->timing) {
-    if (s->gexec && s->gdt == dt) {
+    if (s->gexec) {
       CUDA_TRY(cudaGraphLaunch(s->gexec, s->st));
-      s->launches = cales_launches_per_step(s);
+      s->launches += cales_launches_per_step(s);
       return CALES_OK;
     }
-    if (s->gexec) { cudaGraphExecDestroy(s->gexec); s->gexec = nullptr; }
     cudaGraph_t g = nullptr;
     if (cudaStreamBeginCapture(s->st, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
       rc = CALES_OK;
-      for (int rk = 0; rk < 3 && rc == CALES_OK; ++rk) rc = substep(s, rk, dt);
+      const int l0 = s->launches;
+      for (int rk = 0; rk < 3 && rc == CALES_OK; ++rk) rc = substep(s, rk);
       const cudaError_t ee = cudaStreamEndCapture(s->st, &g);
       if (rc == CALES_OK && ee == cudaSuccess && g && cudaGraphInstantiate(&s->gexec, g, 0) == cudaSuccess) {
         cudaGraphDestroy(g);
-        s->gdt = dt;
         CUDA_TRY(cudaGraphLaunch(s->gexec, s->st));
         return CALES_OK;
       }
+      s->launches = l0;
       if (g) cudaGraphDestroy(g);
       s->gexec = nullptr; s->use_graph = 0;      // capture unavailable: plain launches from now on
       cudaGetLastError();
@@ -527,8 +516,70 @@ extern "C" int cales_step(cales_solver* s, double dt) {
     } else { s->use_graph = 0; cudaGetLastError(); }
   }
   tick(s, -1);
-  for (int rk = 0; rk < 3; ++rk) if ((rc = substep(s, rk, dt))) return rc;
+  for (int rk = 0; rk < 3; ++rk) if ((rc = substep(s, rk))) return rc;
   s->ev_valid = s->timing != 0;
+  return CALES_OK;
+}
+
+// dt-dependent device tables of a step: the substep scalar blocks and, with implicit z, the Crank-Nicolson tables of Eq. 21
+// (the forward elimination of the constant matrix is a serial recurrence over nz levels, one thread per substep).
+static int prepare_dt(cales_solver* s, double dt, const double* dt_dev) {
+  k_rk_scalars<<<1, 32, 0, s->st>>>(dt, dt_dev, s->c.nu, s->rks);
+  LAUNCH_TRY(K_CN_COEF);
+  if (s->c.implicit_z == 1 && (dt_dev || dt != s->cn_dt)) {
+    k_cn_coef<<<1, 32, 0, s->st>>>(s->c, s->rks, s->cncoef);
+    LAUNCH_TRY(K_CN_COEF);
+    s->cn_dt = dt_dev ? 0.0 : dt;
+  }
+  return CALES_OK;
+}
+
+extern "C" int cales_step(cales_solver* s, double dt) {
+  if (!s || !(dt > 0.0)) return fail(CALES_EINVAL, "bad step arguments");
+  int rc;
+  s->launches = 0; s->evn = 0; s->ev_valid = false;
+  if (!s->fresh && (rc = refresh_closures(s))) return rc;
+  const int timing_was = s->timing; s->timing = 0;      // the two table kernels are not part of the timed step
+  rc = prepare_dt(s, dt, nullptr);
+  s->timing = timing_was;
+  if (rc) return rc;
+  s->last_dt = dt;
+  return run_substeps(s);
+}
+
+// One step with dt = cfl / max(|u_c|/dx + |v_c|/dy + |w_c|/dzf) of the current field (a fixed fraction of the
+// stability limit, reading S18), the reduction and everything derived from dt staying on the device: no host synchronisation.
+extern "C" int cales_step_adaptive(cales_solver* s, double cfl) {
+  if (!s || !(cfl > 0.0)) return fail(CALES_EINVAL, "bad step arguments");
+  int rc;
+  s->launches = 0; s->evn = 0; s->ev_valid = false;
+  if (!s->fresh && (rc = refresh_closures(s))) return rc;
+  const int timing_was = s->timing; s->timing = 0;
+  rc = CALES_OK;
+  do {
+    double* part = s->CP;   // scratch, nblk <= N
+    k_cfl_rate<<<s->pgrid, s->pblock, 0, s->st>>>(s->c, s->u, s->v, s->w, part);
+    if ((rc = check_launch(s, K_DIAG))) break;
+    const long long nb = s->nblk; const int g1 = (int)(nb < 1024 ? nb : 1024);
+    k_max_stage<<<g1, 256, 0, s->st>>>(part, nb, s->stage1);
+    if ((rc = check_launch(s, K_SUM))) break;
+    k_dt_finish<<<1, 256, 0, s->st>>>(s->stage1, g1, cfl, s->dtdev);
+    if ((rc = check_launch(s, K_SUM))) break;
+    rc = prepare_dt(s, 0.0, s->dtdev);
+  } while (0);
+  s->timing = timing_was;
+  if (rc) return rc;
+  s->last_dt = -1.0;      // on the device: cales_last_dt reads it back
+  return run_substeps(s);
+}
+
+// dt of the last step (HOST output; synchronises when that dt was computed on the device).
+extern "C" int cales_last_dt(cales_solver* s, double* dt_host) {
+  if (!s || !dt_host) return fail(CALES_EINVAL, "null argument");
+  if (s->last_dt < 0.0) {
+    CUDA_TRY(cudaMemcpyAsync(dt_host, s->dtdev, sizeof(double), cudaMemcpyDeviceToHost, s->st));
+    CUDA_TRY(cudaStreamSynchronize(s->st));
+  } else *dt_host = s->last_dt;
   return CALES_OK;
 }
 
@@ -607,13 +658,13 @@ extern "C" int cales_wall_stress_y(cales_solver* s, double* tau_dev) {
 extern "C" int cales_project(cales_solver* s) {
   if (!s) return fail(CALES_EINVAL, "null solver");
   int rc;
-  DivSrc ds{s->u, s->v, s->w, 1.0};
+  DivSrc ds{s->u, s->v, s->w, 1.0, nullptr};
   if ((rc = run_transform_x_fwd(s, nullptr, &ds, s->W))) return rc;
   if ((rc = run_poisson_core(s))) return rc;
   if ((rc = run_transform_x_inv(s, s->W, s->W))) return rc;
   CorrArgs ca;
   ca.phi = s->W; ca.us = s->u; ca.vs = s->v; ca.ws = s->w; ca.u = s->u; ca.v = s->v; ca.w = s->w; ca.p = s->p;
-  ca.shift = nullptr; ca.gdt = 1.0; ca.cimp = 0.0; ca.cxy = 0.0; ca.update_p = 0;
+  ca.shift = nullptr; ca.gdt = 1.0; ca.cimp = 0.0; ca.cxy = 0.0; ca.update_p = 0; ca.sc = nullptr;
   k_correct<<<s->pgrid, s->pblock, 0, s->st>>>(s->c, ca);
   LAUNCH_TRY(K_CORRECT);
   s->fresh = false;
@@ -646,6 +697,58 @@ extern "C" int cales_plane_stats(cales_solver* s, double* out_dev) {
   const int rc = check_launch(s, K_DIAG);
   s->timing = timing_was;
   return rc;
+}
+
+// ---- time-accumulated statistics (Tables 3-5) ------------------------------------------
+extern "C" int cales_stats_reset(cales_solver* s) {
+  if (!s) return fail(CALES_EINVAL, "null solver");
+  CUDA_TRY(cudaMemsetAsync(s->stats, 0, (8 * (size_t)s->c.nz + 16) * sizeof(double), s->st));
+  return CALES_OK;
+}
+extern "C" int cales_stats_accumulate(cales_solver* s, double weight) {
+  if (!s || !(weight > 0.0)) return fail(CALES_EINVAL, "bad stats arguments");
+  int rc;
+  const int timing_was = s->timing; s->timing = 0;
+  rc = CALES_OK;
+  do {
+    if (!s->fresh && (rc = refresh_closures(s))) break;      // the wall-model planes must belong to the current velocity
+    const int n = 8 * s->c.nz + 8;
+    double* tmp = s->stats + (8 * (size_t)s->c.nz + 16);
+    k_plane_stats<<<s->c.nz, 1024, 0, s->st>>>(s->c, s->u, s->v, s->w, s->nut, tmp);
+    if ((rc = check_launch(s, K_DIAG))) break;
+    k_wall_shear<<<8, 1024, 0, s->st>>>(s->c, s->u, s->v, s->w, tmp + 8 * (size_t)s->c.nz);
+    if ((rc = check_launch(s, K_DIAG))) break;
+    k_stats_axpy<<<(n + 1 + 255) / 256, 256, 0, s->st>>>(s->stats, tmp, weight, n);
+    rc = check_launch(s, K_DIAG);
+  } while (0);
+  s->timing = timing_was;
+  return rc;
+}
+extern "C" int cales_stats_get(cales_solver* s, double* prof_host, double* wall_host, double* derived_host, double* weight_host) {
+  if (!s) return fail(CALES_EINVAL, "null solver");
+  const int nz = s->c.nz, n = 8 * nz + 8;
+  std::vector<double> h(n + 1), dzf(nz);
+  CUDA_TRY(cudaMemcpyAsync(h.data(), s->stats, (n + 1) * sizeof(double), cudaMemcpyDeviceToHost, s->st));
+  CUDA_TRY(cudaMemcpyAsync(dzf.data(), s->dzf + 1, nz * sizeof(double), cudaMemcpyDeviceToHost, s->st));
+  CUDA_TRY(cudaStreamSynchronize(s->st));
+  const double wsum = h[n];
+  if (!(wsum > 0.0)) return fail(CALES_EINVAL, "no statistics accumulated");
+  for (int q = 0; q < n; ++q) h[q] /= wsum;
+  if (prof_host) std::memcpy(prof_host, h.data(), 8 * (size_t)nz * sizeof(double));
+  const double* wl = h.data() + 8 * (size_t)nz;
+  if (wall_host) std::memcpy(wall_host, wl, 8 * sizeof(double));
+  if (derived_host) {
+    double tw = 0.0; int nw = 0;
+    if (s->c.bc_z == BC_WALL) { tw += wl[0] + wl[2]; nw += 2; }
+    if (s->c.bc_y == BC_WALL) { tw += wl[4] + wl[6]; nw += 2; }
+    tw = nw ? tw / nw : 0.0;
+    double ub = 0.0; for (int k = 0; k < nz; ++k) ub += h[k] * dzf[k];
+    ub /= s->c.lz;
+    derived_host[0] = tw; derived_host[1] = tw > 0.0 ? std::sqrt(tw) : 0.0; derived_host[2] = derived_host[1] * 0.5 * s->c.lz / s->c.nu;
+    derived_host[3] = ub != 0.0 ? 2.0 * tw / (ub * ub) : 0.0;
+  }
+  if (weight_host) *weight_host = wsum;
+  return CALES_OK;
 }
 
 extern "C" int cales_get_cs(cales_solver* s, double* cs_dev) {

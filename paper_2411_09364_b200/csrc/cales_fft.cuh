@@ -147,7 +147,7 @@ CALES_HD int perm_fwd(int r, int n, bool dct) {
 // input on the fly as the Poisson right-hand side f = div(u*)/(gamma dt) (Eq. 12), so the
 // divergence never touches HBM.  Phases (load / passes / store) are separated by block barriers.
 // ------------------------------------------------------------------------------------------------------------
-struct DivSrc { const double* us; const double* vs; const double* ws; double inv_gdt; };
+struct DivSrc { const double* us; const double* vs; const double* ws; double inv_gdt; const double* sc; };   // sc: substep scalar block (1/(gamma dt) at index 2) or nullptr
 
 CALES_HD double2 ld2(const double* p, int t) { return reinterpret_cast<const double2*>(p)[t]; }
 

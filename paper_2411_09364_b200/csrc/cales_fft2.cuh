@@ -133,7 +133,7 @@ struct F2SmemSt { double2* buf; const Fft2Lay& lay; CALES_HD void operator()(int
 // ---- accessors: x transforms (lines contiguous in global memory) ---------------------------------------------------
 // forward: packed complex element t of line l0+b, either from src or as the divergence of u* / (gamma dt) (Eq. 12)
 struct F2XFwdLd {
-  const Ctx& c; const FftPlan& pl; long long l0; int nb; const double* src; const DivSrc& ds; bool div;
+  const Ctx& c; const FftPlan& pl; long long l0; int nb; const double* src; const DivSrc& ds; bool div; double inv;   // inv = 1 / (gamma dt)
   CALES_HD double2 operator()(int b, int t) const {
     if (b >= nb) return make_double2(0.0, 0.0);
     const int n = pl.n; const long long l = l0 + b;
@@ -148,8 +148,8 @@ struct F2XFwdLd {
     const double um = ul[t == 0 ? n - 1 : 2 * t - 1];
     const double2 vv = ld2(vl, t), ww = ld2(wl, t);
     const double2 vvm = vm ? ld2(vm, t) : make_double2(0.0, 0.0), wwm = wm ? ld2(wm, t) : make_double2(0.0, 0.0);
-    return make_double2(((uu.x - um) * rdx + (vv.x - vvm.x) * rdy + (ww.x - wwm.x) * rdz) * ds.inv_gdt,
-                        ((uu.y - uu.x) * rdx + (vv.y - vvm.y) * rdy + (ww.y - wwm.y) * rdz) * ds.inv_gdt);
+    return make_double2(((uu.x - um) * rdx + (vv.x - vvm.x) * rdy + (ww.x - wwm.x) * rdz) * inv,
+                        ((uu.y - uu.x) * rdx + (vv.y - vvm.y) * rdy + (ww.y - wwm.y) * rdz) * inv);
   }
 };
 // inverse: Z[t] merged on the fly from the packed half-complex line (h[0] = X0, h[1] = X_{n/2}, h[2m], h[2m+1] = X_m)
@@ -252,7 +252,7 @@ __global__ void __launch_bounds__(512) k_fft2_x_fwd(const __grid_constant__ Ctx 
   const Fft2Lay lay{L, sm_line(pl.n2), 0, false};
   const long long nlines = (long long)c.ny * c.nz, l0 = (long long)blockIdx.x * L;
   const int nb = (int)min((long long)L, nlines - l0);
-  F2XFwdLd first{c, pl, l0, nb, src, ds, DIV};
+  F2XFwdLd first{c, pl, l0, nb, src, ds, DIV, DIV ? (ds.sc ? ds.sc[2] : ds.inv_gdt) : 0.0};
   f2_passes<false>(lay, pl, -1, f2_sm, first, F2SmemSt{f2_sm, lay});
   f2x_split_store(threadIdx.x, blockDim.x, pl, lay, l0, nb, f2_sm, dst);
 }

@@ -18,7 +18,16 @@ struct RhsArgs {
   double *us, *vs, *ws;                  // u* (explicit) or the right-hand side of Eq. 21 (implicit z)
   double dt, al, be, ga;
   int store_R;
+  const double* sc;                      // substep scalar block in device memory (RK_*), or nullptr: dt above is used
 };
+
+// Substep scalars kept in device memory so that one captured CUDA graph serves every dt (and dt itself may be computed on the
+// device, cales_step_adaptive): block rk holds dt, gamma dt, 1 / (gamma dt), gamma nu dt / 2.
+enum { RK_DT = 0, RK_GDT = 1, RK_INV_GDT = 2, RK_CIMP = 3, RK_STRIDE = 4 };
+CALES_HD void rk_scalars(int rk, double dt, double nu, double* sc) {
+  double al, be, ga; rk3_coeffs(rk, al, be, ga);
+  sc[RK_DT] = dt; sc[RK_GDT] = ga * dt; sc[RK_INV_GDT] = 1.0 / (ga * dt); sc[RK_CIMP] = 0.5 * ga * nu * dt;
+}
 
 struct CorrArgs {
   const double *phi, *us, *vs, *ws;
@@ -28,6 +37,7 @@ struct CorrArgs {
   double cimp;             // gamma nu dt / 2 if implicit z (or fully implicit) else 0
   double cxy;              // gamma nu dt / 2 if fully implicit (Eq. 19: the x and y parts of L_jj phi) else 0
   int update_p;
+  const double* sc;        // substep scalar block (RK_*) or nullptr; when given, gdt / cimp / cxy above only say which terms are on
 };
 
 // Eq. 13: u = u* - gamma dt grad(phi) (+ the bulk shift of u*); Eq. 14 / 22: p += phi (- c L_zz phi).
@@ -47,15 +57,17 @@ CALES_HD void correct_point(const Ctx& c, const CorrArgs& a, int i, int j, int k
   const bool wact = !(c.bc_z == BC_WALL && k == c.nz - 1);
   const double sh = a.shift ? *a.shift : 0.0;
   const double rdzc = c.rdzc[k];
-  a.u[n] = (a.us[n] + sh) - a.gdt * (phx - ph) * c.rdx;
-  a.v[n] = vact ? a.vs[n] - a.gdt * (phy - ph) * c.rdy : 0.0;
-  a.w[n] = wact ? a.ws[n] - a.gdt * (phz - ph) * rdzc : 0.0;
+  const double gdt = a.sc ? a.sc[RK_GDT] : a.gdt;
+  a.u[n] = (a.us[n] + sh) - gdt * (phx - ph) * c.rdx;
+  a.v[n] = vact ? a.vs[n] - gdt * (phy - ph) * c.rdy : 0.0;
+  a.w[n] = wact ? a.ws[n] - gdt * (phz - ph) * rdzc : 0.0;
   if (a.update_p) {
     double dp = ph;
-    if (a.cimp != 0.0) dp -= a.cimp * (((phz - ph) * rdzc - (ph - phm) * c.rdzc[k - 1]) * c.rdzf[k]);
+    const double cimp = a.sc ? a.sc[RK_CIMP] : a.cimp;
+    if (a.cimp != 0.0) dp -= cimp * (((phz - ph) * rdzc - (ph - phm) * c.rdzc[k - 1]) * c.rdzf[k]);
     if (a.cxy != 0.0) {      // Eq. 19 (periodic x and y)
       const double pxm = scalg(c, a.phi, i - 1, j, k, 1.0), pym = scalg(c, a.phi, i, j - 1, k, 1.0);
-      dp -= a.cxy * ((phx - 2.0 * ph + pxm) * c.rdx * c.rdx + (phy - 2.0 * ph + pym) * c.rdy * c.rdy);
+      dp -= cimp * ((phx - 2.0 * ph + pxm) * c.rdx * c.rdx + (phy - 2.0 * ph + pym) * c.rdy * c.rdy);
     }
     a.p[n] += dp;
   }
@@ -83,7 +95,10 @@ __global__ void k_sum_stage1(const double* __restrict__ in, long long n, double*
   if (threadIdx.x == 0) out1[blockIdx.x] = t;
 }
 // scal[0] = shift = u_bulk - sum/(nx ny lz); scal[1] = forcing = shift / (gamma dt); scal[2] = mean
-__global__ void k_bulk_finish(Ctx c, const double* __restrict__ in, int n, double gdt, double* __restrict__ scal) {
+__global__ void k_rk_scalars(double dt, const double* __restrict__ dt_dev, double nu, double* __restrict__ sc) {
+  if (threadIdx.x < 3) rk_scalars(threadIdx.x, dt_dev ? *dt_dev : dt, nu, sc + threadIdx.x * RK_STRIDE);
+}
+__global__ void k_bulk_finish(Ctx c, const double* __restrict__ in, int n, double gdt, const double* __restrict__ sc, double* __restrict__ scal) {
   __shared__ double sh[32];
   double s = 0.0;
   for (int q = threadIdx.x; q < n; q += blockDim.x) s += in[q];
@@ -91,7 +106,7 @@ __global__ void k_bulk_finish(Ctx c, const double* __restrict__ in, int n, doubl
   if (threadIdx.x == 0) {
     const double m = t / ((double)c.nx * (double)c.ny * c.lz);
     const double shf = c.u_bulk - m;
-    scal[0] = shf; scal[1] = shf / gdt; scal[2] = m;
+    scal[0] = shf; scal[1] = shf / (sc ? sc[RK_GDT] : gdt); scal[2] = m;
   }
 }
 // diagnostics: per-block partials of max|div|, sum u dzf, sum ke dzf, non-finite count
@@ -155,6 +170,43 @@ __global__ void __launch_bounds__(1024) k_plane_stats(Ctx c, const double* u, co
     if (threadIdx.x == 0) out[(long long)m * c.nz + k] = t / (double)c.nxy;
   }
 }
+// Wall-shear means (C_f and Re_tau of Tables 3-5): grid 8, block 1024; out[q], q = 0..3 the z walls ((tau_xz, tau_yz) bottom,
+// top), 4..7 the y walls ((tau_xy, tau_zy) low, high; dzf-weighted); 0 in periodic directions.  Modelled walls: mean of the wall-model
+// planes; no-slip walls: nu x the one-sided difference to the mirror ghost, 2 nu q_first / (ghost spacing).
+__global__ void __launch_bounds__(1024) k_wall_shear(Ctx c, const double* __restrict__ u, const double* __restrict__ v, const double* __restrict__ w,
+                                                     double* __restrict__ out) {
+  __shared__ double sh[32];
+  const int q = blockIdx.x, wl = (q >> 1) & 1, comp = q & 1;
+  double a = 0.0, norm = 1.0;
+  if (q < 4) {
+    if (c.bc_z == BC_WALL) {
+      const double* f = comp == 0 ? u : v;
+      const int k0 = wl == 0 ? 0 : c.nz - 1;
+      const double fac = 2.0 * c.nu / (wl == 0 ? c.dzc[-1] : c.dzc[c.nz - 1]);
+      for (long long n = threadIdx.x; n < c.nxy; n += blockDim.x)
+        a += c.wall_model ? c.tau[(long long)(wl * 2 + comp) * c.nxy + n] : fac * f[(long long)k0 * c.nxy + n];
+      norm = (double)c.nxy;
+    }
+  } else if (c.bc_y == BC_WALL) {
+    const double* f = comp == 0 ? u : w;
+    const int j0 = wl == 0 ? 0 : c.ny - 1;
+    const double fac = 2.0 * c.nu * c.rdy;
+    const long long nxz = (long long)c.nx * c.nz;
+    for (long long n = threadIdx.x; n < nxz; n += blockDim.x) {
+      const int k = (int)(n / c.nx), i = (int)(n - (long long)k * c.nx);
+      a += (c.wall_model_y ? c.tau_y[(long long)(wl * 2 + comp) * nxz + n] : fac * f[idx3(c, i, j0, k)]) * c.dzf[k];
+    }
+    norm = (double)c.nx * c.lz;
+  }
+  const double t = block_sum(a, sh);
+  if (threadIdx.x == 0) out[q] = t / norm;
+}
+// acc[0..n) += weight * tmp[0..n); acc[n] += weight (the accumulated weight)
+__global__ void k_stats_axpy(double* __restrict__ acc, const double* __restrict__ tmp, double weight, int n) {
+  const int q = blockIdx.x * blockDim.x + threadIdx.x;
+  if (q < n) acc[q] += weight * tmp[q];
+  if (q == n) acc[q] += weight;
+}
 __global__ void k_max_stage(const double* __restrict__ in, long long n, double* __restrict__ out) {
   __shared__ double sh[32];
   const long long per = (n + gridDim.x - 1) / gridDim.x;
@@ -163,6 +215,14 @@ __global__ void k_max_stage(const double* __restrict__ in, long long n, double* 
   for (long long q = b0 + threadIdx.x; q < b1; q += blockDim.x) s = fmax(s, in[q]);
   const double t = block_max(s, sh);
   if (threadIdx.x == 0) out[blockIdx.x] = t;
+}
+// dt = cfl / max rate (0 if the field is at rest), one block
+__global__ void k_dt_finish(const double* __restrict__ in, int n, double cfl, double* __restrict__ dt_dev) {
+  __shared__ double sh[32];
+  double s = 0.0;
+  for (int q = threadIdx.x; q < n; q += blockDim.x) s = fmax(s, in[q]);
+  const double t = block_max(s, sh);
+  if (threadIdx.x == 0) *dt_dev = t > 0.0 ? cfl / t : 0.0;
 }
 #endif
 

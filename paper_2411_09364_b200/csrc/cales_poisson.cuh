@@ -242,10 +242,15 @@ __global__ void k_poisson_z(Ctx c, PoissonTabs T, double* __restrict__ A, double
   if (col >= c.nxy) return;
   poisson_column(c, T, (int)(col % c.nx), (int)(col / c.nx), A, CP, CQ);
 }
-__global__ void k_helm_z(Ctx c, PoissonTabs T, int fam, double cimp, double* __restrict__ A, double* __restrict__ CP, double* __restrict__ CQ) {
+__global__ void k_helm_z(Ctx c, PoissonTabs T, int fam, const double* __restrict__ sc, double* __restrict__ A, double* __restrict__ CP, double* __restrict__ CQ) {
   const long long col = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (col >= c.nxy) return;
-  helm_column(c, T, fam, cimp, (int)(col % c.nx), (int)(col / c.nx), A, CP, CQ);
+  helm_column(c, T, fam, sc[3], (int)(col % c.nx), (int)(col / c.nx), A, CP, CQ);
+}
+// Crank-Nicolson tables of the three substeps built on the device from the substep scalar blocks (one thread per substep: the
+// forward elimination of the constant matrix is a serial recurrence over nz levels).  coef: [3][6][nz], sc: [3][4].
+__global__ void k_cn_coef(Ctx c, const double* __restrict__ sc, double* __restrict__ coef) {
+  if (threadIdx.x < 3) cn_coefficients(c, sc[threadIdx.x * 4 + 3], coef + (size_t)threadIdx.x * 6 * c.nz);
 }
 // partial[block] = sum over the block's points of q dzf[k] (bulk velocity of u* after the Helmholtz solves); grid/block of the point kernels
 __global__ void __launch_bounds__(256) k_weighted_sum(Ctx c, const double* __restrict__ q, double* __restrict__ partial) {

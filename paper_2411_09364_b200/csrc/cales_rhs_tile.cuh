@@ -94,11 +94,12 @@ CALES_HD double rhs_core(const Ctx& c, const RhsArgs& a, const A& q, int i, int 
   if (a.be != 0.0) { ru0 = a.Ru0[n]; rv0 = a.Rv0[n]; rw0 = a.Rw0[n]; }
   if (!vact) Rv = 0.0;
   if (!wact) Rw = 0.0;
-  double us = u000 + a.dt * (a.al * Ru + a.be * ru0 - a.ga * gpx);
-  double vs = v000 + a.dt * (a.al * Rv + a.be * rv0 - a.ga * gpy);
-  double ws = w000 + a.dt * (a.al * Rw + a.be * rw0 - a.ga * gpz);
+  const double dt = a.sc ? a.sc[RK_DT] : a.dt;
+  double us = u000 + dt * (a.al * Ru + a.be * ru0 - a.ga * gpx);
+  double vs = v000 + dt * (a.al * Rv + a.be * rv0 - a.ga * gpy);
+  double ws = w000 + dt * (a.al * Rw + a.be * rw0 - a.ga * gpz);
   if (c.implicit_z) {   // Eq. 20 explicit half + right-hand side of Eq. 21
-    const double fe = a.dt * a.ga * c.nu, fi = 0.5 * a.ga * c.nu * a.dt;
+    const double fe = dt * a.ga * c.nu, fi = 0.5 * a.ga * c.nu * dt;
     double ltu = lzu, ltv = lzv;        // L_zz of the implicit operator applied to u^k
     if (c.wall_model) {                 // zero-flux closure: the modelled wall stress is a source outside the implicit operator
       const double up = (k < c.nz - 1) ? 1.0 : 0.0, lo = (k > 0) ? 1.0 : 0.0;

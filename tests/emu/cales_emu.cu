@@ -101,10 +101,10 @@ static void emu_fft_x_fwd(emu_solver* s, const double* src, const DivSrc* ds, do
   const Fft2Lay lay{L, sm_line(pl.n2), 0, false};
   std::vector<double2> sm((size_t)L * lay.ls);
   const long long nlines = (long long)c.ny * c.nz;
-  DivSrc none{nullptr, nullptr, nullptr, 0.0};
+  DivSrc none{nullptr, nullptr, nullptr, 0.0, nullptr};
   for (long long l0 = 0; l0 < nlines; l0 += L) {
     const int nb = (int)std::min<long long>(L, nlines - l0);
-    F2XFwdLd first{c, pl, l0, nb, src, ds ? *ds : none, ds != nullptr};
+    F2XFwdLd first{c, pl, l0, nb, src, ds ? *ds : none, ds != nullptr, ds ? ds->inv_gdt : 0.0};
     emu_f2_passes<false>(lay, pl, -1, sm.data(), nth, first, F2SmemSt{sm.data(), lay});
     for (int tid = 0; tid < nth; ++tid) f2x_split_store(tid, nth, pl, lay, l0, nb, sm.data(), dst);
   }
@@ -338,7 +338,7 @@ static void emu_substep(emu_solver* s, int rk, double dt) {
   RhsArgs a;
   a.u = s->u.data(); a.v = s->v.data(); a.w = s->w.data(); a.p = s->p.data(); a.nut = s->nut.data();
   a.Ru0 = s->Ru.data(); a.Rv0 = s->Rv.data(); a.Rw0 = s->Rw.data(); a.Ru1 = s->Ru.data(); a.Rv1 = s->Rv.data(); a.Rw1 = s->Rw.data();
-  a.us = s->us.data(); a.vs = s->vs.data(); a.ws = s->ws.data(); a.dt = dt; a.al = al; a.be = be; a.ga = ga; a.store_R = rk < 2 ? 1 : 0;
+  a.us = s->us.data(); a.vs = s->vs.data(); a.ws = s->ws.data(); a.dt = dt; a.al = al; a.be = be; a.ga = ga; a.store_R = rk < 2 ? 1 : 0; a.sc = nullptr;
   double sum = 0.0;
   {  // k_rhs_tile: per CTA tile and plane, stage the three halo planes with the staging rule of the kernel (rt_elem), then
      // evaluate rhs_core through the shared-memory accessor
@@ -370,14 +370,14 @@ static void emu_substep(emu_solver* s, int rk, double dt) {
     const double m = sum / ((double)c.nx * (double)c.ny * c.lz);
     s->scal[0] = c.u_bulk - m; s->scal[1] = s->scal[0] / (ga * dt); s->scal[2] = m;
   }
-  DivSrc ds{s->us.data(), s->vs.data(), s->ws.data(), 1.0 / (ga * dt)};
+  DivSrc ds{s->us.data(), s->vs.data(), s->ws.data(), 1.0 / (ga * dt), nullptr};
   emu_fft_x_fwd(s, nullptr, &ds, s->W.data());
   emu_poisson_core(s);
   emu_fft_x_inv(s, s->W.data(), s->W.data());
   CorrArgs ca;
   ca.phi = s->W.data(); ca.us = s->us.data(); ca.vs = s->vs.data(); ca.ws = s->ws.data();
   ca.u = s->u.data(); ca.v = s->v.data(); ca.w = s->w.data(); ca.p = s->p.data();
-  ca.shift = cfr ? s->scal : nullptr; ca.gdt = ga * dt; ca.cimp = imp ? 0.5 * ga * c.nu * dt : 0.0; ca.cxy = 0.0; ca.update_p = 1;
+  ca.shift = cfr ? s->scal : nullptr; ca.gdt = ga * dt; ca.cimp = imp ? 0.5 * ga * c.nu * dt : 0.0; ca.cxy = 0.0; ca.update_p = 1; ca.sc = nullptr;
   for (int k = 0; k < c.nz; ++k) for (int j = 0; j < c.ny; ++j) for (int i = 0; i < c.nx; ++i) correct_point(c, ca, i, j, k);
   emu_refresh(s);
 }
@@ -405,14 +405,14 @@ extern "C" int emu_transform(emu_solver* s, double* f, int dir, int inverse) {
 }
 extern "C" int emu_project(emu_solver* s) {
   const Ctx& c = s->c;
-  DivSrc ds{s->u.data(), s->v.data(), s->w.data(), 1.0};
+  DivSrc ds{s->u.data(), s->v.data(), s->w.data(), 1.0, nullptr};
   emu_fft_x_fwd(s, nullptr, &ds, s->W.data());
   emu_poisson_core(s);
   emu_fft_x_inv(s, s->W.data(), s->W.data());
   CorrArgs ca;
   ca.phi = s->W.data(); ca.us = s->u.data(); ca.vs = s->v.data(); ca.ws = s->w.data();
   ca.u = s->u.data(); ca.v = s->v.data(); ca.w = s->w.data(); ca.p = s->p.data();
-  ca.shift = nullptr; ca.gdt = 1.0; ca.cimp = 0.0; ca.cxy = 0.0; ca.update_p = 0;
+  ca.shift = nullptr; ca.gdt = 1.0; ca.cimp = 0.0; ca.cxy = 0.0; ca.update_p = 0; ca.sc = nullptr;
   for (int k = 0; k < c.nz; ++k) for (int j = 0; j < c.ny; ++j) for (int i = 0; i < c.nx; ++i) correct_point(c, ca, i, j, k);
   s->fresh = false;
   return 0;

@@ -281,7 +281,7 @@ def test_cuda_graph_replay_is_bit_identical(oracle, gpu):
             g.set_velocity(u, v, w)
             for _ in range(4):
                 g.step(dt)
-            g.step(0.5 * dt)            # a new dt forces a re-capture
+            g.step(0.5 * dt)            # a new dt: same graph, the scalars live in device memory
             st.synchronize()
             res.append(_gpu_fields(g))
             g.close()
@@ -434,4 +434,58 @@ def test_wall_stress_on_y_walls_parity(oracle, gpu):
     assert np.max(np.abs(a - b)) <= 1e-12 * np.max(np.abs(b))
     a, b = g.eddy_viscosity().cpu().numpy(), o.eddy_viscosity()
     assert np.max(np.abs(a - b)) <= 1e-11 * max(np.max(np.abs(b)), kw["nu"])
+    g.close()
+
+
+@pytest.mark.parametrize("n,shape,over", [(2, (48, 24, 16), {}), (3, (48, 24, 24), {}), (1, (24, 16, 12), {}), (3, (48, 24, 24), dict(implicit_z=0, implicit_xyz=1))])
+def test_adaptive_dt_stepping_parity(oracle, gpu, n, shape, over):
+    """cales_step_adaptive: dt chosen on the device every step with no host synchronisation, one CUDA graph for
+    every dt, the Crank-Nicolson tables rebuilt on the device (config 3).  The oracle steps with the dt the GPU reports."""
+    cfg, kw, (u, v, w), dt = pc.prepare(oracle, n, shape, over)
+    o = pc.make(oracle.Oracle, kw)
+    g = pc.make(gpu.Solver, kw)
+    o.set_velocity(u, v, w); g.set_velocity(u, v, w)
+    dts = []
+    for s in range(4):
+        want = o.cfl_dt(0.4)
+        g.step_adaptive(0.4)
+        got = g.last_dt()
+        assert abs(got - want) <= 1e-11 * want, (s, got, want)
+        o.step(got)
+        dts.append(got)
+        err = pc.field_errors(_gpu_fields(g), [o.get(f) for f in range(5)], o.dzf, kw["nu"])
+        assert max(err.values()) <= (TOL_1STEP if s == 0 else TOL_1STEP * 10 * (s + 1)), (s, err)
+    assert len(set(dts)) == 4          # the step really changed every time
+    # and a host-side dt after device-side ones
+    o.step(0.5 * dts[-1]); g.step(0.5 * dts[-1])
+    assert g.last_dt() == 0.5 * dts[-1]
+    err = pc.field_errors(_gpu_fields(g), [o.get(f) for f in range(5)], o.dzf, kw["nu"])
+    assert max(err.values()) <= TOL_1STEP * 60, err
+    g.close()
+
+
+@pytest.mark.parametrize("n,shape,over", [(3, (72, 36, 40), {}), (5, (72, 48, 24), {}), (4, (96, 36, 24), {}),
+                                          (4, (96, 36, 24), dict(wall_model=1, wall_model_y=1, nu=1.0 / 40000))])
+def test_time_accumulated_statistics_parity(oracle, gpu, n, shape, over):
+    """cales_stats_*: dt-weighted time averages of the plane profiles and of the wall shear (no-slip and modelled walls, z and y),
+    C_f and Re_tau (Tables 3-5) against the oracle's accumulators over three steps."""
+    cfg, kw, (u, v, w), dt = pc.prepare(oracle, n, shape, over)
+    o = pc.make(oracle.Oracle, kw)
+    g = pc.make(gpu.Solver, kw)
+    o.set_velocity(u, v, w); g.set_velocity(u, v, w)
+    o.stats_reset(); g.stats_reset()
+    for s in range(3):
+        wgt = dt * (1 + s)
+        o.stats_accumulate(wgt); g.stats_accumulate(wgt)
+        o.step(dt); g.step(dt)
+    a, b = g.stats_get(), o.stats_get()
+    U = float(np.max(np.abs(o.get(0))))
+    scale = [U, U, U, U * U, U * U, U * U, U * U, max(float(np.max(np.abs(b["profiles"][7]))), kw["nu"])]
+    for q in range(8):
+        assert np.max(np.abs(a["profiles"][q] - b["profiles"][q])) <= 1e-10 * scale[q], q
+    ws = max(float(np.max(np.abs(b["wall"]))), 1e-300)
+    assert np.max(np.abs(a["wall"] - b["wall"])) <= 1e-10 * ws
+    assert b["tau_w"] > 0 and b["re_tau"] > 0 and b["cf"] > 0
+    for key in ("tau_w", "u_tau", "re_tau", "cf", "weight"):
+        assert abs(a[key] - b[key]) <= 1e-10 * abs(b[key]), key
     g.close()

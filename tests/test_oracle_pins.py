@@ -1177,3 +1177,60 @@ def test_fully_implicit_ustar_is_the_helmholtz_solution(oracle):
         if comp == 2:
             rhs[-1] = 0.0
         assert np.max(np.abs(lhs - rhs)) < 1e-12 * np.max(np.abs(rhs))
+
+
+# ----------------------------------------------------------------------------- SURVEY.md 8(f) item 4, second half
+@pytest.mark.parametrize("stretch", [False, True])
+def test_wall_shear_statistics_poiseuille_closed_form(oracle, stretch):
+    """C_f and Re_tau (Tables 3-5) from the time-accumulated statistics on a Poiseuille profile between no-slip
+    walls: the one-sided difference to the mirror ghost gives tau_w = nu u(z0)/z0 = 1.5 nu u_b (2 - z0) exactly, z0 the first
+    centre; the weights of the time average are honoured."""
+    nu, ub = 2e-3, 1.3
+    S = make(oracle, 8, 6, 16, (0, 1), stretch, nu=nu, sgs_model=0)
+    z = S.zc
+    prof = 1.5 * ub * (1.0 - (z - 1.0) ** 2)
+    u = prof[:, None, None] * np.ones(S.shape)
+    zero = np.zeros(S.shape)
+    S.set_velocity(u, zero, zero)
+    S.stats_reset(); S.stats_accumulate(1.0)
+    S.set_velocity(3.0 * u, zero, zero)
+    S.stats_accumulate(3.0)
+    st = S.stats_get()
+    tau = 1.5 * nu * ub * (2.0 - z[0]) * (1.0 + 3.0 * 3.0) / 4.0
+    assert abs(st["wall"][0] - tau) < 1e-13 * tau and abs(st["wall"][2] - tau) < 1e-13 * tau
+    assert np.max(np.abs(st["wall"][[1, 3, 4, 5, 6, 7]])) == 0.0
+    um = (1.0 + 9.0) / 4.0 * prof
+    assert np.max(np.abs(st["profiles"][0] - um)) < 1e-13 * np.max(um)
+    assert np.max(np.abs(st["profiles"][3] - (1.0 + 27.0) / 4.0 * prof ** 2)) < 1e-12 * np.max(um) ** 2
+    ubm = np.sum(um * S.dzf) / 2.0
+    assert abs(st["tau_w"] - tau) < 1e-13 * tau and abs(st["u_tau"] - math.sqrt(tau)) < 1e-13
+    assert abs(st["re_tau"] - math.sqrt(tau) / nu) < 1e-10 * st["re_tau"] and abs(st["cf"] - 2 * tau / ubm ** 2) < 1e-12 * st["cf"]
+    assert st["weight"] == 4.0
+    # continuous value for context: tau_w -> 3 nu u_b as z0 -> 0
+    assert abs(1.5 * nu * ub * (2.0 - z[0]) / (3 * nu * ub) - 1.0) < z[0]
+
+
+def test_wall_shear_statistics_wall_model_and_duct(oracle):
+    """Modelled walls report the mean of the wall-model planes (z walls and, for the duct, y walls: dzf-weighted); no-slip y walls the
+    one-sided difference 2 nu q / dy."""
+    nu = 1.0 / 800
+    W = make(oracle, 12, 8, 10, (0, 1), False, nu=nu, wall_model=1, sgs_model=1, cs=0.1)
+    rng = np.random.default_rng(12)
+    prof = np.log(np.minimum(W.zc, 2 - W.zc) * 800) / 0.41 + 5.2
+    W.set_velocity(prof[:, None, None] + 0.3 * rng.standard_normal(W.shape), 0.3 * rng.standard_normal(W.shape), np.zeros(W.shape))
+    tau = W.wall_stress()
+    W.stats_reset(); W.stats_accumulate(2.0)
+    st = W.stats_get()
+    want = [tau[0, 0].mean(), tau[0, 1].mean(), tau[1, 0].mean(), tau[1, 1].mean()]
+    assert np.max(np.abs(st["wall"][:4] - want)) < 1e-14 * abs(want[0])
+    assert st["tau_w"] == pytest.approx(0.5 * (want[0] + want[2]), rel=1e-14)
+    D = make(oracle, 12, 8, 10, (1, 1), True, nu=nu, sgs_model=0)
+    u = rng.standard_normal(D.shape); w = rng.standard_normal(D.shape); w[-1] = 0.0
+    D.set_velocity(u, np.zeros(D.shape), w)
+    D.stats_reset(); D.stats_accumulate(1.0)
+    st = D.stats_get()
+    wz = D.dzf[:, None] / 2.0
+    assert abs(st["wall"][4] - np.sum(2 * nu * u[:, 0, :] / D.dy * wz) / 12) < 1e-13
+    assert abs(st["wall"][7] - np.sum(2 * nu * w[:, -1, :] / D.dy * wz) / 12) < 1e-13
+    dzc_b = 2 * D.zc[0]
+    assert abs(st["wall"][0] - np.mean(2 * nu * u[0] / dzc_b)) < 1e-13
