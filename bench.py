@@ -40,15 +40,29 @@ ALGO_BYTES = {
 }
 
 
-# fp64 operations per grid point of the one kernel that is bound by the plain fp64 ALUs (ncu op counts of round 1,
-# profiles/r1_ncu_full.md: 0.30 DADD + 0.35 DMUL + 0.30 DFMA of 315 fp64 instructions per point; an FMA counts 2).
-ALGO_FLOPS = {"k_dsm_col": 415.0}
-# B200 plain fp64 peak derived in DESIGN.md section 4: 148 SMs x 64 FMA lanes x 2 flop x 1.965 GHz
-FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture (profiles/r1_ncu_full.md),
-# keyed by (config, kernel); None where no capture of that kernel at that size is committed.
-NCU_TRAFFIC = {(5, "k_dsm_col"): 65.2e9, (5, "k_rhs"): 98.5e9, (5, "k_correct"): 63.9e9, (5, "k_poisson_z"): 37.0e9, (5, "k_fft_x_fwd"): 26.9e9,
-               (5, "k_fft_y_fwd"): 12.8e9, (5, "k_fft_y_inv"): 12.8e9, (5, "k_fft_x_inv"): 12.8e9, (5, "k_dsm_nut"): 12.8e9}
+# fp64 operations per grid point of the one kernel that is bound by the plain fp64 ALUs rather than by HBM (ncu instruction counts of
+# round 2, profiles/r2_ncu_dsm.md: 95 DFMA + 69 DADD + 55 DMUL = 219 fp64 instructions per point; an FMA counts 2).
+ALGO_FLOPS = {"k_dsm_col": 314.0}
+# fallback if the in-process measurement (cales_fp64_peak) fails: 148 SMs x 64 FMA lanes x 2 flop x 1.965 GHz
+FP64_PEAK_TFLOPS_DERIVED = 148 * 64 * 2 * 1.965e9 / 1e12
+TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r2_ncu_traffic.csv")
+
+
+def ncu_traffic():
+    """{(config, kernel): (dram bytes per launch, source)} from the committed ncu --set full capture (profiles/r2_ncu_traffic.csv,
+    made by the command in profiles/r2_ncu_full.md): dram__bytes_read.sum + dram__bytes_write.sum, averaged over the launches
+    of that kernel in the capture."""
+    out = {}
+    try:
+        with open(TRAFFIC_CSV) as f:
+            for line in f:
+                if line.startswith("#") or not line.strip() or line.startswith("config,"):
+                    continue
+                c, k, rd, wr = line.strip().split(",")[:4]
+                out[(int(c), k)] = (float(rd) + float(wr), "profiles/r2_ncu_traffic.csv (ncu --set full, see profiles/r2_ncu_full.md)")
+    except OSError:
+        pass
+    return out
 
 
 def measured_peaks():
@@ -102,7 +116,7 @@ class ClockSampler:
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
-REPLICA = {1: None, 2: None, 3: (128, 128, 96), 4: (256, 64, 64), 5: (192, 128, 64)}   # bounded oracle samples
+REPLICA = {1: None, 2: None, 3: (128, 128, 96), 4: (256, 64, 64), 5: (192, 128, 128)}   # bounded oracle samples (seconds each)
 
 
 def oracle_leg(cfg_no, steps, warmup, overrides=None):
@@ -252,6 +266,10 @@ def run_ours(args):
         for name, (ms, n) in s.kernel_times().items():
             a = ktot.setdefault(name, [0.0, 0]); a[0] += ms; a[1] += n
     sampler = ClockSampler(local); sampler.start()
+    try:
+        fp64_peak, fp64_src = s.fp64_peak(), "measured in this process (cales_fp64_peak: register-resident DFMA loop, best of 3)"
+    except Exception as e:       # keep the line
+        fp64_peak, fp64_src = FP64_PEAK_TFLOPS_DERIVED, "derived 148 x 64 x 2 x 1.965 GHz (measurement failed: %r)" % (e,)
     s.set_timing(big)
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
     for k in range(K):
@@ -280,33 +298,82 @@ def run_ours(args):
     ms = max_over_ranks(ms, "cuda")
     value = aggregate_value(npts, K, world, ms)
 
-    # ---- e2e: the same metric through the C ABI with HOST buffers, copies inside the timed region
-    Ke = max(1, min(K, 3)) if not args.no_e2e else 0
-    hosts = [torch.from_numpy(a) for a in (u, v, w, p_host)]
-    def e2e_step():
-        for f in range(3):
-            s.set_field(f, hosts[f])            # H2D, synchronous (cales_set_field with a host pointer)
-        s.step(dt)
-        for f in range(4):
-            s.get_field(f, hosts[f])            # D2H of the step's result
+    # ---- e2e: the same metric with HOST buffers: every step uploads that step's input velocity (3 fields) from pinned host memory and
+    # downloads the step's result (u, v, w, p); both copies are inside the timed region.  The three stages are pipelined the way a
+    # user streaming fields through the solver would: H2D of step n+1 (copy stream) and D2H of step n-1 (second copy stream) run
+    # while step n computes; device staging tensors decouple them from the solver state, which is read and written through the
+    # C ABI (cales_set_field / cales_step / cales_get_field with device pointers).  PCIe is full duplex, so the steady state is
+    # max(H2D, D2H, compute + 7 field copies on the device).
+    Ke = max(1, min(K, 4)) if not args.no_e2e else 0
+    e2e = None
     if Ke:
-        e2e_step()                              # warm-up
-    torch.cuda.synchronize()
-    if world > 1:
-        dist.barrier()
-    t0 = time.perf_counter()
-    for _ in range(Ke):
-        e2e_step()
-    torch.cuda.synchronize()
-    te = time.perf_counter() - t0
-    te = max_over_ranks(te, "cuda")
-    e2e = None if not Ke else {"value": aggregate_value(npts, Ke, world, te * 1e3), "unit": UNIT, "h2d_bytes_per_step": 3 * npts * 8, "d2h_bytes_per_step": 4 * npts * 8,
-           "steps": Ke, "ms_per_step": 1e3 * te / Ke, "host_memory": "pinned (cudaHostRegister)" if pinned else "pageable",
-           "note": "each step: cales_set_field(u,v,w) from host, cales_step, cales_get_field(u,v,w,p) to host; a new velocity makes "
-                   "the library re-evaluate the wall stress and nu_t first"}
+        free, _ = torch.cuda.mem_get_info()
+        staged = free > 8 * npts * 8 + (2 << 30)
+        hosts = [torch.from_numpy(a) for a in (u, v, w, p_host)]
+        if staged:
+            st_in = [torch.empty(s.shape, dtype=torch.float64, device="cuda") for _ in range(3)]
+            st_out = [torch.empty(s.shape, dtype=torch.float64, device="cuda") for _ in range(4)]
+            h2d, d2h = torch.cuda.Stream(device=local), torch.cuda.Stream(device=local)
+            in_ready, in_free = torch.cuda.Event(), torch.cuda.Event()
+            out_ready, out_free = torch.cuda.Event(), torch.cuda.Event()
+            in_free.record(stream); out_free.record(stream)
+            def upload():
+                with torch.cuda.stream(h2d):
+                    h2d.wait_event(in_free)
+                    for f in range(3):
+                        st_in[f].copy_(hosts[f], non_blocking=True)
+                    in_ready.record(h2d)
+            def e2e_step(last):
+                stream.wait_event(in_ready)
+                for f in range(3):
+                    s.set_field(f, st_in[f])
+                in_free.record(stream)
+                if not last:
+                    upload()                        # the next step's input travels while this step computes
+                s.step(dt)
+                stream.wait_event(out_free)
+                for f in range(4):
+                    s.get_field(f, st_out[f])
+                out_ready.record(stream)
+                with torch.cuda.stream(d2h):
+                    d2h.wait_event(out_ready)
+                    for f in range(4):
+                        hosts[f].copy_(st_out[f], non_blocking=True)
+                    out_free.record(d2h)
+            def e2e_run(n):
+                upload()
+                for q in range(n):
+                    e2e_step(q == n - 1)
+                torch.cuda.synchronize()
+        else:
+            def e2e_run(n):
+                for _ in range(n):
+                    for f in range(3):
+                        s.set_field(f, hosts[f])        # H2D, synchronous (cales_set_field with a host pointer)
+                    s.step(dt)
+                    for f in range(4):
+                        s.get_field(f, hosts[f])        # D2H of the step's result
+                torch.cuda.synchronize()
+        e2e_run(1)                              # warm-up
+        if world > 1:
+            dist.barrier()
+        t0 = time.perf_counter()
+        e2e_run(Ke)
+        te = time.perf_counter() - t0
+        te = max_over_ranks(te, "cuda")
+        e2e = {"value": aggregate_value(npts, Ke, world, te * 1e3), "unit": UNIT, "h2d_bytes_per_step": 3 * npts * 8, "d2h_bytes_per_step": 4 * npts * 8,
+               "steps": Ke, "ms_per_step": 1e3 * te / Ke, "host_memory": "pinned (cudaHostRegister)" if pinned else "pageable",
+               "pipeline": "H2D / compute / D2H overlapped on three streams through device staging tensors" if staged else "sequential (no room for staging)",
+               "note": "each step: upload u,v,w from host, cales_set_field x3, cales_step, cales_get_field x4, download u,v,w,p to host; a new "
+                       "velocity makes the library re-evaluate the wall stress and nu_t first; wall time over the Ke steps including the "
+                       "pipeline fill and drain"}
+        if staged:
+            del st_in, st_out
+        del hosts
 
     # ---- per-kernel roofline table (algorithmic bytes / mean launch duration) and the dominant kernel
     peak, peak_src = measured_peaks()
+    traffic = ncu_traffic()
     kernels = {}
     step_ms = sum(a[0] for a in ktot.values()) / K
     for name, (tot, n) in sorted(ktot.items(), key=lambda kv: -kv[1][0]):
@@ -315,19 +382,25 @@ def run_ours(args):
         if name in ALGO_BYTES:
             gbs = ALGO_BYTES[name] * npts / (per * 1e-3) / 1e9
             row.update({"algo_bytes_per_pt": ALGO_BYTES[name], "achieved_gbs": gbs, "frac": gbs / peak})
+        if name in ALGO_FLOPS:       # the kernel bound by the plain fp64 ALUs: also against the fp64 peak measured in this process
+            tf = ALGO_FLOPS[name] * npts / (per * 1e-3) / 1e12
+            row.update({"algo_flops_per_pt": ALGO_FLOPS[name], "achieved_tflops": tf, "fp64_frac": tf / fp64_peak})
+        if (cfg_no, name) in traffic:
+            row["ncu_dram_bytes_per_launch"] = traffic[(cfg_no, name)][0]
         kernels[name] = row
+    # the dominant kernel = the largest total time per step among the kernels of the byte model (a kernel launched twice per
+    # substep, like k_dsm_col with its wall planes, counts with both launches)
     top = next((n for n in kernels if n in ALGO_BYTES), None)
     roofline = None
     if top:
         r = kernels[top]
+        tr = traffic.get((cfg_no, top))
         roofline = {"kernel": top, "bound": "hbm", "achieved": r["achieved_gbs"], "peak": peak, "unit": "GB/s", "frac": r["frac"],
-                    "traffic": NCU_TRAFFIC.get((cfg_no, top)), "peak_source": peak_src, "algo_bytes_per_launch": ALGO_BYTES[top] * npts,
-                    "ms_per_launch": r["ms_per_launch"], "share_of_step": r["share_of_step"]}
+                    "traffic": tr[0] if tr else None, "traffic_source": tr[1] if tr else None, "peak_source": peak_src,
+                    "algo_bytes_per_launch": ALGO_BYTES[top] * npts, "ms_per_launch": r["ms_per_launch"], "share_of_step": r["share_of_step"]}
         if top in ALGO_FLOPS:        # bound by the plain fp64 ALUs, not by HBM: report it against that peak
-            tf = ALGO_FLOPS[top] * npts / (r["ms_per_launch"] * 1e-3) / 1e12
-            roofline.update({"bound": "alu", "achieved": tf, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": tf / FP64_PEAK_TFLOPS,
-                             "peak_source": "derived: 148 SMs x 64 fp64 FMA lanes x 2 x 1.965 GHz (DESIGN.md section 4)",
-                             "algo_flops_per_launch": ALGO_FLOPS[top] * npts, "hbm_frac_of_measured_peak": r["frac"]})
+            roofline.update({"bound": "alu", "achieved": r["achieved_tflops"], "peak": fp64_peak, "unit": "TFLOP/s", "frac": r["fp64_frac"],
+                             "peak_source": fp64_src, "algo_flops_per_launch": ALGO_FLOPS[top] * npts, "hbm_frac_of_measured_peak": r["frac"]})
     # whole-step algorithmic traffic: the sum over the step's launches of the table above
     step_bytes = sum(ALGO_BYTES.get(n, 0.0) * (a[1] // K) for n, a in ktot.items()) * npts
     step_gbs = step_bytes / (ms / K * 1e-3) / 1e9
@@ -343,6 +416,7 @@ def run_ours(args):
             "step_hbm": {"algo_bytes_per_pt_step": step_bytes / npts, "achieved_gbs": step_gbs, "frac_of_measured_peak": step_gbs / peak,
                          "frac_of_8TBs": step_gbs / 8000.0},
             "e2e": e2e, "gpu_launches": launches, "clocks": clocks, "roofline": roofline, "kernels": kernels,
+            "fp64_peak": {"tflops": fp64_peak, "source": fp64_src, "derived_for_comparison": FP64_PEAK_TFLOPS_DERIVED},
             "diagnostics": {k: diag[k] for k in ("max_div", "u_bulk", "kinetic_energy", "wm_max_iters", "nan_count")},
             "input_generation_s": t_gen}
     s.close()
@@ -359,7 +433,7 @@ def run_ours(args):
             # (device-resident timing only) after this process has released its device memory.
             for a in (u, v, w, p_host):
                 torch.cuda.cudart().cudaHostUnregister(a.ctypes.data)
-            del hosts, u, v, w, p_host
+            del u, v, w, p_host
             others = {}
             for cno in (1, 2, 3, 4, 5):
                 if cno == cfg_no:
@@ -375,6 +449,12 @@ def run_ours(args):
                                                  "top_kernels": {k: round(v["share_of_step"], 3) for k, v in list(d["kernels"].items())[:3]}}
                 except Exception as e:      # a failed side run must not lose the main line
                     others["config %d" % cno] = {"error": repr(e)[:200]}
+                if not args.no_cpu_baseline:      # the oracle timed on every workload (bounded replicas, two steps)
+                    try:
+                        r = oracle_leg(cno, 2, 1)
+                        others["config %d" % cno]["cpu_baseline"] = {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")}
+                    except Exception as e:
+                        others["config %d" % cno]["cpu_baseline"] = {"error": repr(e)[:200]}
             line["other_configs"] = others
         print(json.dumps(line), flush=True)
 

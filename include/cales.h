@@ -16,6 +16,8 @@
  *  - Ownership: the caller owns every buffer, including the workspace blob (size from
  *    cales_workspace_bytes) that the library carves into its fields, work arrays and tables.  The
  *    library never allocates device memory.  The workspace and the stream must outlive the solver.
+ *  - Every entry point runs on the device given at cales_create whatever the caller's current device is, and leaves the caller's
+ *    current device as it found it.
  *  - All work is enqueued on the caller's CUDA stream (`cuda_stream`, a cudaStream_t; NULL = the
  *    legacy default stream).  cales_step / cales_poisson_solve / cales_eddy_viscosity / cales_wall_stress
  *    are asynchronous; cales_create, cales_set_field / cales_get_field with host pointers and
@@ -142,7 +144,10 @@ int cales_poisson_solve(cales_solver* s, const double* rhs_dev, double* phi_dev)
 
 /* nu_t (Eq. 4 or Eq. 5-9) of a velocity field.  u, v, w: DEVICE fields, or all NULL = the solver's own velocity;
  * nut: DEVICE output, nz*ny*nx (NULL = the solver's own nu_t).  External fields must hold 0 on the wall faces
- * (v[.][ny-1][.] with y walls, w[nz-1] with z walls), as the solver's own fields always do.  Asynchronous. */
+ * (v[.][ny-1][.] with y walls, w[nz-1] with z walls), as the solver's own fields always do.  External fields need an external
+ * nut (CALES_EINVAL otherwise).  The evaluation shares the solver's scratch: cales_get_cs afterwards returns the coefficient of
+ * THIS evaluation, and the wall-model ghosts / van Driest wall shear of an external field use the wall stresses of the solver's
+ * own velocity as they stand.  Asynchronous. */
 int cales_eddy_viscosity(cales_solver* s, const double* u, const double* v, const double* w, double* nut);
 
 /* Wall stresses of the log-law wall model from the solver's velocity (Eq. 10):
@@ -203,6 +208,11 @@ int cales_kernel_time(cales_solver* s, int kid, const char** name, double* ms_to
 /* cales_step replays its three substeps as one CUDA graph (captured once: dt lives in device memory; on by default, bypassed while
  * timing is on).  on = 0 returns to plain stream launches. */
 int cales_set_graph(cales_solver* s, int on);
+
+/* Measured fp64 FMA throughput of the device in TFLOP/s (an FMA counts 2): a register-resident DFMA loop on the solver's stream,
+ * best of three timed launches -- the roofline denominator bench.py uses for the one kernel bound by the plain fp64 ALUs.
+ * HOST output; synchronises. */
+int cales_fp64_peak(cales_solver* s, double* tflops_host);
 
 /* Kernel-selection knobs, for tests and A/B timing only (results do not depend on them beyond round-off; the defaults are the
  * measured best): "rhs_tile_min_points" (grids with fewer points run the momentum kernel one thread per point instead of the

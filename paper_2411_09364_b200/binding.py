@@ -40,7 +40,7 @@ class CalesDiag(C.Structure):
 SYMBOLS = ["cales_default_params", "cales_workspace_bytes", "cales_create", "cales_create_basic", "cales_destroy",
            "cales_set_field", "cales_get_field", "cales_step", "cales_step_adaptive", "cales_last_dt", "cales_poisson_solve", "cales_eddy_viscosity",
            "cales_wall_stress", "cales_wall_stress_y", "cales_project", "cales_cfl_dt", "cales_plane_stats", "cales_stats_reset", "cales_stats_accumulate", "cales_stats_get", "cales_get_cs", "cales_transform", "cales_transpose_xy",
-           "cales_set_timing", "cales_set_graph", "cales_set_option", "cales_kernel_count", "cales_kernel_time", "cales_launches_per_step", "cales_diagnostics", "cales_last_error"]
+           "cales_set_timing", "cales_set_graph", "cales_set_option", "cales_fp64_peak", "cales_kernel_count", "cales_kernel_time", "cales_launches_per_step", "cales_diagnostics", "cales_last_error"]
 
 _lib = None
 
@@ -79,6 +79,7 @@ def lib():
         L.cales_transpose_xy.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.cales_set_timing.argtypes = [C.c_void_p, C.c_int]
         L.cales_set_graph.argtypes = [C.c_void_p, C.c_int]
+        L.cales_fp64_peak.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
         L.cales_set_option.argtypes = [C.c_void_p, C.c_char_p, C.c_longlong]
         L.cales_launches_per_step.argtypes = [C.c_void_p]
         L.cales_kernel_time.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_char_p), C.POINTER(C.c_double), C.POINTER(C.c_int)]
@@ -291,6 +292,11 @@ class Solver:
 
     def set_graph(self, on=True):
         _chk(lib().cales_set_graph(self._h, 1 if on else 0))
+
+    def fp64_peak(self):
+        tf = C.c_double()
+        _chk(lib().cales_fp64_peak(self._h, C.byref(tf)))
+        return tf.value
 
     def set_option(self, key, value):
         _chk(lib().cales_set_option(self._h, key.encode(), int(value)))

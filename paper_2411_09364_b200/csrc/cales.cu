@@ -76,7 +76,24 @@ struct cales_solver {
   std::vector<cudaEvent_t> evpool; std::vector<int> evkid; int evn;   // per-launch events of the last timed step
   double kms[32]; int kcnt[32];                                       // per-kernel totals of the last timed step
   int launches;
+  int device;
 };
+
+// Every entry point runs on the solver's device whatever the caller's current device is, and restores the latter.
+struct DevGuard {
+  int prev = -1; bool sw = false;
+  explicit DevGuard(int dev) { if (dev >= 0 && cudaGetDevice(&prev) == cudaSuccess && prev != dev) sw = cudaSetDevice(dev) == cudaSuccess; }
+  ~DevGuard() { if (sw) cudaSetDevice(prev); }
+};
+// Switches the per-kernel timing off for launches that are not part of a step; restored on every return path.
+struct TimingOff {
+  cales_solver* s; int was;
+  explicit TimingOff(cales_solver* s_);
+  ~TimingOff();
+};
+
+TimingOff::TimingOff(cales_solver* s_) : s(s_), was(s_->timing) { s->timing = 0; }
+TimingOff::~TimingOff() { s->timing = was; }
 
 static size_t al32(size_t n) { return (n + 31) / 32 * 32; }
 
@@ -180,11 +197,13 @@ extern "C" int cales_create(const cales_params* p, cales_solver** out) {
   if (((size_t)p->workspace) % 256) return fail(CALES_EINVAL, "workspace must be 256-byte aligned");
   const size_t need = carve(nullptr, p, nullptr);
   if (p->workspace_bytes < need) return fail(CALES_EINVAL, "workspace too small");
-  CUDA_TRY(cudaSetDevice(p->device));
+  DevGuard dg_(p->device);      // the caller's current device is restored on return
+  { int cur = -1; if (cudaGetDevice(&cur) != cudaSuccess || cur != p->device) return fail(CALES_ECUDA, "cannot select the device of the workspace"); }
   HostSetup H;
   if ((rc = build_setup(p, H))) return rc;
   cales_solver* s = new cales_solver();
   s->P = H.P;
+  s->device = p->device;
   s->st = (cudaStream_t)p->cuda_stream;
   const int nx = p->nx, ny = p->ny, nz = p->nz;
   s->N = (long long)nx * ny * nz; s->nxy = (long long)nx * ny;
@@ -258,6 +277,7 @@ extern "C" int cales_create_basic(int nx, int ny, int nz, double lx, double ly, 
 }
 
 extern "C" int cales_destroy(cales_solver* s) {
+  DevGuard dg_(s ? s->device : -1);
   if (!s) return CALES_OK;
   for (cudaEvent_t e : s->evpool) cudaEventDestroy(e);
   if (s->gexec) cudaGraphExecDestroy(s->gexec);
@@ -271,6 +291,7 @@ static double* field_ptr(cales_solver* s, int f) {
 }
 
 extern "C" int cales_set_field(cales_solver* s, int field, const double* src, int on_device) {
+  DevGuard dg_(s ? s->device : -1);
   if (!s || !src) return fail(CALES_EINVAL, "null argument");
   double* d = field_ptr(s, field);
   if (!d) return fail(CALES_EINVAL, "bad field id");
@@ -285,6 +306,7 @@ extern "C" int cales_set_field(cales_solver* s, int field, const double* src, in
   return CALES_OK;
 }
 extern "C" int cales_get_field(cales_solver* s, int field, double* dst, int on_device) {
+  DevGuard dg_(s ? s->device : -1);
   if (!s || !dst) return fail(CALES_EINVAL, "null argument");
   double* d = field_ptr(s, field);
   if (!d) return fail(CALES_EINVAL, "bad field id");
@@ -535,13 +557,12 @@ static int prepare_dt(cales_solver* s, double dt, const double* dt_dev) {
 }
 
 extern "C" int cales_step(cales_solver* s, double dt) {
+  DevGuard dg_(s ? s->device : -1);
   if (!s || !(dt > 0.0)) return fail(CALES_EINVAL, "bad step arguments");
   int rc;
   s->launches = 0; s->evn = 0; s->ev_valid = false;
   if (!s->fresh && (rc = refresh_closures(s))) return rc;
-  const int timing_was = s->timing; s->timing = 0;      // the two table kernels are not part of the timed step
-  rc = prepare_dt(s, dt, nullptr);
-  s->timing = timing_was;
+  { TimingOff toff(s); rc = prepare_dt(s, dt, nullptr); }      // the two table kernels are not part of the timed step
   if (rc) return rc;
   s->last_dt = dt;
   return run_substeps(s);
@@ -550,13 +571,14 @@ extern "C" int cales_step(cales_solver* s, double dt) {
 // One step with dt = cfl / max(|u_c|/dx + |v_c|/dy + |w_c|/dzf) of the current field (a fixed fraction of the
 // stability limit, reading S18), the reduction and everything derived from dt staying on the device: no host synchronisation.
 extern "C" int cales_step_adaptive(cales_solver* s, double cfl) {
+  DevGuard dg_(s ? s->device : -1);
   if (!s || !(cfl > 0.0)) return fail(CALES_EINVAL, "bad step arguments");
   int rc;
   s->launches = 0; s->evn = 0; s->ev_valid = false;
   if (!s->fresh && (rc = refresh_closures(s))) return rc;
-  const int timing_was = s->timing; s->timing = 0;
   rc = CALES_OK;
   do {
+    TimingOff toff(s);
     double* part = s->CP;   // scratch, nblk <= N
     k_cfl_rate<<<s->pgrid, s->pblock, 0, s->st>>>(s->c, s->u, s->v, s->w, part);
     if ((rc = check_launch(s, K_DIAG))) break;
@@ -567,7 +589,6 @@ extern "C" int cales_step_adaptive(cales_solver* s, double cfl) {
     if ((rc = check_launch(s, K_SUM))) break;
     rc = prepare_dt(s, 0.0, s->dtdev);
   } while (0);
-  s->timing = timing_was;
   if (rc) return rc;
   s->last_dt = -1.0;      // on the device: cales_last_dt reads it back
   return run_substeps(s);
@@ -575,6 +596,7 @@ extern "C" int cales_step_adaptive(cales_solver* s, double cfl) {
 
 // dt of the last step (HOST output; synchronises when that dt was computed on the device).
 extern "C" int cales_last_dt(cales_solver* s, double* dt_host) {
+  DevGuard dg_(s ? s->device : -1);
   if (!s || !dt_host) return fail(CALES_EINVAL, "null argument");
   if (s->last_dt < 0.0) {
     CUDA_TRY(cudaMemcpyAsync(dt_host, s->dtdev, sizeof(double), cudaMemcpyDeviceToHost, s->st));
@@ -584,6 +606,7 @@ extern "C" int cales_last_dt(cales_solver* s, double* dt_host) {
 }
 
 extern "C" int cales_set_graph(cales_solver* s, int on) {
+  DevGuard dg_(s ? s->device : -1);
   if (!s) return fail(CALES_EINVAL, "null solver");
   s->use_graph = on ? 1 : 0;
   if (!on && s->gexec) { cudaGraphExecDestroy(s->gexec); s->gexec = nullptr; }
@@ -592,6 +615,7 @@ extern "C" int cales_set_graph(cales_solver* s, int on) {
 
 // Kernel-selection knobs for tests and A/B timing (the defaults are the measured best).
 extern "C" int cales_set_option(cales_solver* s, const char* key, long long value) {
+  DevGuard dg_(s ? s->device : -1);
   if (!s || !key) return fail(CALES_EINVAL, "null argument");
   const std::string k(key);
   if (k == "rhs_tile_min_points") s->rhs_tile_min = value;
@@ -622,6 +646,7 @@ extern "C" int cales_launches_per_step(cales_solver* s) {
 }
 
 extern "C" int cales_poisson_solve(cales_solver* s, const double* rhs, double* phi) {
+  DevGuard dg_(s ? s->device : -1);
   if (!s || !rhs || !phi) return fail(CALES_EINVAL, "null argument");
   int rc;
   if ((rc = run_transform_x_fwd(s, rhs, nullptr, s->W))) return rc;
@@ -631,13 +656,16 @@ extern "C" int cales_poisson_solve(cales_solver* s, const double* rhs, double* p
 }
 
 extern "C" int cales_eddy_viscosity(cales_solver* s, const double* u, const double* v, const double* w, double* nut) {
+  DevGuard dg_(s ? s->device : -1);
   if (!s) return fail(CALES_EINVAL, "null solver");
   const bool own = !u && !v && !w;
   if (!own && (!u || !v || !w)) return fail(CALES_EINVAL, "u, v, w must be all given or all NULL");
+  if (!own && !nut) return fail(CALES_EINVAL, "external u, v, w need an external nut: the solver's own nu_t belongs to its own velocity");
   return run_eddy_viscosity(s, own ? s->u : u, own ? s->v : v, own ? s->w : w, nut ? nut : s->nut);
 }
 
 extern "C" int cales_wall_stress(cales_solver* s, double* tau_dev) {
+  DevGuard dg_(s ? s->device : -1);
   if (!s) return fail(CALES_EINVAL, "null solver");
   if (!s->c.wall_model) return fail(CALES_EINVAL, "solver has no wall model");
   int rc = run_wall_stress(s);
@@ -647,6 +675,7 @@ extern "C" int cales_wall_stress(cales_solver* s, double* tau_dev) {
 }
 
 extern "C" int cales_wall_stress_y(cales_solver* s, double* tau_dev) {
+  DevGuard dg_(s ? s->device : -1);
   if (!s) return fail(CALES_EINVAL, "null solver");
   if (!s->c.wall_model_y) return fail(CALES_EINVAL, "solver has no wall model on the y walls");
   int rc = run_wall_stress(s);
@@ -656,6 +685,7 @@ extern "C" int cales_wall_stress_y(cales_solver* s, double* tau_dev) {
 }
 
 extern "C" int cales_project(cales_solver* s) {
+  DevGuard dg_(s ? s->device : -1);
   if (!s) return fail(CALES_EINVAL, "null solver");
   int rc;
   DivSrc ds{s->u, s->v, s->w, 1.0, nullptr};
@@ -673,8 +703,9 @@ extern "C" int cales_project(cales_solver* s) {
 
 // adaptive time step (0.95 x the stability limit in the paper; reading S18)
 extern "C" int cales_cfl_dt(cales_solver* s, double cfl, double* dt_host) {
+  DevGuard dg_(s ? s->device : -1);
   if (!s || !dt_host || !(cfl > 0.0)) return fail(CALES_EINVAL, "bad cfl_dt arguments");
-  const int timing_was = s->timing; s->timing = 0;
+  TimingOff toff(s);
   double* part = s->CP;   // scratch, nblk <= N
   k_cfl_rate<<<s->pgrid, s->pblock, 0, s->st>>>(s->c, s->u, s->v, s->w, part);
   LAUNCH_TRY(K_DIAG);
@@ -683,7 +714,6 @@ extern "C" int cales_cfl_dt(cales_solver* s, double cfl, double* dt_host) {
   std::vector<double> h(g1);
   CUDA_TRY(cudaMemcpyAsync(h.data(), s->stage1, g1 * sizeof(double), cudaMemcpyDeviceToHost, s->st));
   CUDA_TRY(cudaStreamSynchronize(s->st));
-  s->timing = timing_was;
   double r = 0.0; for (int q = 0; q < g1; ++q) r = std::fmax(r, h[q]);
   *dt_host = r > 0.0 ? cfl / r : 0.0;
   return CALES_OK;
@@ -691,25 +721,25 @@ extern "C" int cales_cfl_dt(cales_solver* s, double cfl, double* dt_host) {
 
 // x-y plane means of u, v, w, uu, vv, ww, uw (centre-averaged) and nu_t: out_dev DEVICE [8][nz] (PAPER.md:237 profiles)
 extern "C" int cales_plane_stats(cales_solver* s, double* out_dev) {
+  DevGuard dg_(s ? s->device : -1);
   if (!s || !out_dev) return fail(CALES_EINVAL, "null argument");
-  const int timing_was = s->timing; s->timing = 0;
+  TimingOff toff(s);
   k_plane_stats<<<s->c.nz, 1024, 0, s->st>>>(s->c, s->u, s->v, s->w, s->nut, out_dev);
-  const int rc = check_launch(s, K_DIAG);
-  s->timing = timing_was;
-  return rc;
+  return check_launch(s, K_DIAG);
 }
 
 // ---- time-accumulated statistics (Tables 3-5) ------------------------------------------
 extern "C" int cales_stats_reset(cales_solver* s) {
+  DevGuard dg_(s ? s->device : -1);
   if (!s) return fail(CALES_EINVAL, "null solver");
   CUDA_TRY(cudaMemsetAsync(s->stats, 0, (8 * (size_t)s->c.nz + 16) * sizeof(double), s->st));
   return CALES_OK;
 }
 extern "C" int cales_stats_accumulate(cales_solver* s, double weight) {
+  DevGuard dg_(s ? s->device : -1);
   if (!s || !(weight > 0.0)) return fail(CALES_EINVAL, "bad stats arguments");
-  int rc;
-  const int timing_was = s->timing; s->timing = 0;
-  rc = CALES_OK;
+  int rc = CALES_OK;
+  TimingOff toff(s);
   do {
     if (!s->fresh && (rc = refresh_closures(s))) break;      // the wall-model planes must belong to the current velocity
     const int n = 8 * s->c.nz + 8;
@@ -721,10 +751,10 @@ extern "C" int cales_stats_accumulate(cales_solver* s, double weight) {
     k_stats_axpy<<<(n + 1 + 255) / 256, 256, 0, s->st>>>(s->stats, tmp, weight, n);
     rc = check_launch(s, K_DIAG);
   } while (0);
-  s->timing = timing_was;
   return rc;
 }
 extern "C" int cales_stats_get(cales_solver* s, double* prof_host, double* wall_host, double* derived_host, double* weight_host) {
+  DevGuard dg_(s ? s->device : -1);
   if (!s) return fail(CALES_EINVAL, "null solver");
   const int nz = s->c.nz, n = 8 * nz + 8;
   std::vector<double> h(n + 1), dzf(nz);
@@ -751,7 +781,48 @@ extern "C" int cales_stats_get(cales_solver* s, double* prof_host, double* wall_
   return CALES_OK;
 }
 
+// ---- measured fp64 ALU peak (roofline denominator of the ALU-bound kernel) --------------------------------------------------
+// 16 independent DFMA chains per thread, 1024 resident threads per SM: nothing but the fp64 pipe limits it.
+__global__ void __launch_bounds__(256) k_fp64_peak(double* __restrict__ out, int iters, double a, double b) {
+  double x[16];
+#pragma unroll
+  for (int q = 0; q < 16; ++q) x[q] = 1.0 + 1e-3 * (threadIdx.x + q);
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int q = 0; q < 16; ++q) x[q] = fma(x[q], a, b);
+  }
+  double s = 0.0;
+#pragma unroll
+  for (int q = 0; q < 16; ++q) s += x[q];
+  if (s == 123.456) out[0] = s;      // never true: keeps the chains alive
+}
+extern "C" int cales_fp64_peak(cales_solver* s, double* tflops_host) {
+  DevGuard dg_(s ? s->device : -1);
+  if (!s || !tflops_host) return fail(CALES_EINVAL, "null argument");
+  TimingOff toff(s);
+  cudaDeviceProp prop;
+  CUDA_TRY(cudaGetDeviceProperties(&prop, s->device));
+  const int blocks = prop.multiProcessorCount * 4, threads = 256, iters = 1 << 16;
+  cudaEvent_t e0, e1;
+  CUDA_TRY(cudaEventCreate(&e0)); CUDA_TRY(cudaEventCreate(&e1));
+  double best = 0.0;
+  for (int rep = 0; rep < 4; ++rep) {      // the first is the warm-up
+    cudaEventRecord(e0, s->st);
+    k_fp64_peak<<<blocks, threads, 0, s->st>>>(s->scal + 31, iters, 0.999999, 1e-6);
+    cudaEventRecord(e1, s->st);
+    if (cudaEventSynchronize(e1) != cudaSuccess) break;
+    float ms = 0.f; cudaEventElapsedTime(&ms, e0, e1);
+    const double tf = 2.0 * 16.0 * (double)iters * blocks * threads / (ms * 1e-3) / 1e12;
+    if (rep > 0 && tf > best) best = tf;
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  CUDA_TRY(cudaGetLastError());
+  *tflops_host = best;
+  return CALES_OK;
+}
+
 extern "C" int cales_get_cs(cales_solver* s, double* cs_dev) {
+  DevGuard dg_(s ? s->device : -1);
   if (!s || !cs_dev) return fail(CALES_EINVAL, "null argument");
   if (s->c.sgs != CALES_SGS_DSMAG) return fail(CALES_EINVAL, "not a dynamic-model solver");
   const size_t n = s->c.dsm_plane ? (size_t)s->c.nz : (size_t)s->c.nz * s->c.ny;
@@ -760,6 +831,7 @@ extern "C" int cales_get_cs(cales_solver* s, double* cs_dev) {
 }
 
 extern "C" int cales_transform(cales_solver* s, double* f, int dir, int inverse) {
+  DevGuard dg_(s ? s->device : -1);
   if (!s || !f) return fail(CALES_EINVAL, "null argument");
   if (dir == 0) return inverse ? run_transform_x_inv(s, f, f) : run_transform_x_fwd(s, f, nullptr, f);
   if (dir == 1) return run_transform_y(s, f, inverse ? 1 : 0);
@@ -767,6 +839,7 @@ extern "C" int cales_transform(cales_solver* s, double* f, int dir, int inverse)
 }
 
 extern "C" int cales_transpose_xy(cales_solver* s, const double* src, double* dst) {
+  DevGuard dg_(s ? s->device : -1);
   if (!s || !src || !dst || src == dst) return fail(CALES_EINVAL, "bad transpose arguments");
   dim3 grid((s->c.nx + 31) / 32, (s->c.ny + 31) / 32, s->c.nz);
   k_transpose_xy<<<grid, dim3(32, 8), 0, s->st>>>(s->c.nx, s->c.ny, src, dst);
@@ -792,6 +865,7 @@ static int collect_times(cales_solver* s) {
 extern "C" int cales_kernel_count(void) { return K_COUNT; }
 
 extern "C" int cales_kernel_time(cales_solver* s, int kid, const char** name, double* ms_total, int* launches) {
+  DevGuard dg_(s ? s->device : -1);
   if (!s || kid < 0 || kid >= K_COUNT) return fail(CALES_EINVAL, "bad kernel id");
   int rc = collect_times(s);
   if (rc) return rc;
@@ -802,17 +876,19 @@ extern "C" int cales_kernel_time(cales_solver* s, int kid, const char** name, do
 }
 
 extern "C" int cales_set_timing(cales_solver* s, int on) {
+  DevGuard dg_(s ? s->device : -1);
   if (!s) return fail(CALES_EINVAL, "null solver");
   s->timing = on ? 1 : 0; s->ev_valid = false; s->evn = 0;
   return CALES_OK;
 }
 
 extern "C" int cales_diagnostics(cales_solver* s, cales_diag* out) {
+  DevGuard dg_(s ? s->device : -1);
   if (!s || !out) return fail(CALES_EINVAL, "null argument");
   std::memset(out, 0, sizeof(*out));
   int rc0 = collect_times(s);
   if (rc0) return rc0;
-  const int timing_was = s->timing; s->timing = 0;   // the diagnostic kernels are not part of a step
+  TimingOff toff(s);   // the diagnostic kernels are not part of a step
   const long long nb = s->nblk;
   double* part = s->CP;   // scratch (4*nblk <= N)
   k_diag<<<s->pgrid, s->pblock, 0, s->st>>>(s->c, s->u, s->v, s->w, s->p, part);
@@ -825,7 +901,6 @@ extern "C" int cales_diagnostics(cales_solver* s, cales_diag* out) {
   CUDA_TRY(cudaMemcpyAsync(scal, s->scal, sizeof(scal), cudaMemcpyDeviceToHost, s->st));
   CUDA_TRY(cudaMemcpyAsync(&mi, s->maxit, sizeof(int), cudaMemcpyDeviceToHost, s->st));
   CUDA_TRY(cudaStreamSynchronize(s->st));
-  s->timing = timing_was;
   double md = 0, ub = 0, ke = 0, bad = 0;
   for (int q = 0; q < g1; ++q) { md = std::fmax(md, h[q]); ub += h[1024 + q]; ke += h[2048 + q]; bad += h[3072 + q]; }
   const double vol = (double)s->c.nx * s->c.ny * s->c.lz;

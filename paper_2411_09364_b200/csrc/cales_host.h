@@ -70,19 +70,14 @@ static inline void make_plan(FftPlan& pl, int n) {
   }
 }
 
-// Launch shape of the dynamic-model pass 1: block width TXB of k_dsm_col (64, 96 or 128: least padded columns),
+// Launch shape of the dynamic-model pass 1: block width TXB of the column march,
 // its number of x blocks, and the number of partial-sum slots per (k, j) row shared with the tile kernel.
 struct DsmShape { int txb, nbx, pslots; };
 static inline DsmShape dsm_shape(int nx) {
-  DsmShape d{64, 0, 0};
-  long long best = -1;
-  for (int t : {64}) {   // measured on B200: 64-thread CTAs (4 per SM at 224 registers) beat 32, 96 and 128
-    const long long cost = (long long)((nx + t - 3) / (t - 2)) * t;
-    if (best < 0 || cost < best) { best = cost; d.txb = t; }
-  }
+  DsmShape d{64, 0, 0};   // 64-thread CTAs (62 output columns + 2 halo columns): measured best of 32 / 64 / 96 / 128 on B200
   d.nbx = (nx + d.txb - 3) / (d.txb - 2);
   d.pslots = (nx + DSM_TX - 1) / DSM_TX;
-  for (int t : {32, 64, 96, 128}) { const int cs = ((nx + t - 3) / (t - 2)) * (t / 32); if (cs > d.pslots) d.pslots = cs; }
+  { const int cs = d.nbx * (d.txb / 32); if (cs > d.pslots) d.pslots = cs; }      // one partial-sum slot per warp of the column march
   return d;
 }
 

@@ -21,7 +21,7 @@ SMALL = {
     "cfg5_hwm_interp": (5, (24, 12, 16), 2, dict(h_wm=0.1)),               # wall model sampled between centres
     "cfg2_wm_implicit": (2, (24, 12, 16), 2, dict(implicit_z=1)),
     "duct_wmles_dsm": (4, (48, 24, 16), 2, dict(wall_model=1, wall_model_y=1, nu=1.0 / 40000)),   # duct WMLES: wall model on all four walls
-    "duct_wmles_smag_y_only": (4, (24, 12, 12), 2, dict(wall_model_y=1, sgs_model=1, cs=0.1, nu=1.0 / 40000)),          # wall model + Crank-Nicolson in z (8(f) item 1)
+    "duct_wmles_smag_y_only": (4, (24, 12, 12), 2, dict(wall_model_y=1, sgs_model=1, cs=0.1, nu=1.0 / 40000)),          # wall model on the y walls only, no-slip z walls
     "duct_wmles_hwm_interp": (4, (24, 12, 12), 2, dict(wall_model=1, wall_model_y=1, sgs_model=1, cs=0.1, nu=1.0 / 40000, h_wm=0.12)),   # sampled between centres on all four walls
     # 3-D box test filter (8(f) item 2): WMLES channel, no-slip duct, duct WMLES, triply periodic box
     "cfg5_dsm_filter3d": (5, (36, 24, 16), 2, dict(dsm_filter3d=1)),
