@@ -499,7 +499,8 @@ static int substep(cales_solver* s, int rk) {
   CorrArgs ca;
   ca.phi = s->W; ca.us = s->us; ca.vs = s->vs; ca.ws = s->ws; ca.u = s->u; ca.v = s->v; ca.w = s->w; ca.p = s->p;
   ca.shift = cfr ? s->scal : nullptr; ca.gdt = 0.0; ca.cimp = (imp || imp3) ? 1.0 : 0.0; ca.cxy = imp3 ? 1.0 : 0.0; ca.update_p = 1; ca.sc = sc;
-  k_correct<<<s->pgrid, s->pblock, 0, s->st>>>(c, ca);
+  if (imp3) k_correct<true><<<s->pgrid, s->pblock, 0, s->st>>>(c, ca);
+  else k_correct<false><<<s->pgrid, s->pblock, 0, s->st>>>(c, ca);
   LAUNCH_TRY(K_CORRECT);
   if ((rc = run_wall_stress(s))) return rc;
   if ((rc = run_eddy_viscosity(s, s->u, s->v, s->w, s->nut))) return rc;
@@ -620,6 +621,16 @@ extern "C" int cales_set_option(cales_solver* s, const char* key, long long valu
   const std::string k(key);
   if (k == "rhs_tile_min_points") s->rhs_tile_min = value;
   else if (k == "smag_tile_min_points") s->tile_min = value;
+  else if (k == "fft_x_lines") {      // lines per CTA of the x transforms (default: ~256 threads per CTA)
+    if (value < 1 || value > 64) return fail(CALES_EINVAL, "fft_x_lines must be 1..64");
+    const int n2 = s->c.nx / 2; const int L = (int)value;
+    bool has3 = false; for (int q = 0; q < s->plx.npass; ++q) has3 |= s->plx.radix[q] == 3;
+    const int per_thread = has3 ? 3 * (F2_E / 3) : F2_E;
+    long long th = ((long long)L * n2 + per_thread - 1) / per_thread; th = (th + 31) / 32 * 32; if (th < 32) th = 32;
+    const size_t sm = (size_t)L * sm_line(n2) * 16;
+    if (th > 512 || sm > 200 * 1024) return fail(CALES_EINVAL, "fft_x_lines: CTA too large");
+    s->xB = L; s->x_threads = (int)th; s->x_smem = sm;
+  }
   else if (k == "rhs_variant") { if (value < 0 || value > 1) return fail(CALES_EINVAL, "rhs_variant must be 0 or 1"); s->rhs_variant = (int)value; }
   else if (k == "dsm_col_variant") { if (value < 0 || value > 2) return fail(CALES_EINVAL, "dsm_col_variant must be 0, 1 or 2"); s->dsm_col_variant = (int)value; }
   else return fail(CALES_EINVAL, "unknown option: " + k);
@@ -695,7 +706,7 @@ extern "C" int cales_project(cales_solver* s) {
   CorrArgs ca;
   ca.phi = s->W; ca.us = s->u; ca.vs = s->v; ca.ws = s->w; ca.u = s->u; ca.v = s->v; ca.w = s->w; ca.p = s->p;
   ca.shift = nullptr; ca.gdt = 1.0; ca.cimp = 0.0; ca.cxy = 0.0; ca.update_p = 0; ca.sc = nullptr;
-  k_correct<<<s->pgrid, s->pblock, 0, s->st>>>(s->c, ca);
+  k_correct<false><<<s->pgrid, s->pblock, 0, s->st>>>(s->c, ca);
   LAUNCH_TRY(K_CORRECT);
   s->fresh = false;
   return CALES_OK;

@@ -41,8 +41,13 @@ struct CorrArgs {
 };
 
 // Eq. 13: u = u* - gamma dt grad(phi) (+ the bulk shift of u*); Eq. 14 / 22: p += phi (- c L_zz phi).
+template <bool IMP3 = true>
 CALES_HD void correct_point(const Ctx& c, const CorrArgs& a, int i, int j, int k) {
   const long long n = idx3(c, i, j, k);
+  // the substep scalars first: a load placed after the stores below could not be moved above them (possible aliasing)
+  const double gdt = a.sc ? ld_scalar(a.sc + RK_GDT) : a.gdt;
+  const double cimp = (a.sc && a.cimp != 0.0) ? ld_scalar(a.sc + RK_CIMP) : a.cimp;
+  const double sh = a.shift ? ld_scalar(a.shift) : 0.0;
   const double ph = a.phi[n];
   double phx, phy, phz, phm = 0.0;
   if (interior_row(c, j, k)) {
@@ -55,17 +60,14 @@ CALES_HD void correct_point(const Ctx& c, const CorrArgs& a, int i, int j, int k
   }
   const bool vact = !(c.bc_y == BC_WALL && j == c.ny - 1);
   const bool wact = !(c.bc_z == BC_WALL && k == c.nz - 1);
-  const double sh = a.shift ? *a.shift : 0.0;
   const double rdzc = c.rdzc[k];
-  const double gdt = a.sc ? a.sc[RK_GDT] : a.gdt;
   a.u[n] = (a.us[n] + sh) - gdt * (phx - ph) * c.rdx;
   a.v[n] = vact ? a.vs[n] - gdt * (phy - ph) * c.rdy : 0.0;
   a.w[n] = wact ? a.ws[n] - gdt * (phz - ph) * rdzc : 0.0;
   if (a.update_p) {
     double dp = ph;
-    const double cimp = a.sc ? a.sc[RK_CIMP] : a.cimp;
     if (a.cimp != 0.0) dp -= cimp * (((phz - ph) * rdzc - (ph - phm) * c.rdzc[k - 1]) * c.rdzf[k]);
-    if (a.cxy != 0.0) {      // Eq. 19 (periodic x and y)
+    if (IMP3 && a.cxy != 0.0) {      // Eq. 19 (periodic x and y)
       const double pxm = scalg(c, a.phi, i - 1, j, k, 1.0), pym = scalg(c, a.phi, i, j - 1, k, 1.0);
       dp -= cimp * ((phx - 2.0 * ph + pxm) * c.rdx * c.rdx + (phy - 2.0 * ph + pym) * c.rdy * c.rdy);
     }
@@ -80,9 +82,12 @@ CALES_HD double divergence_point(const Ctx& c, const double* u, const double* v,
 }
 
 #ifdef __CUDACC__
-__global__ void __launch_bounds__(256) k_correct(Ctx c, CorrArgs a) {
+// IMP3: the Eq. 19 terms of the fully implicit scheme compiled in (the common kernel stays at 32 registers: 64 warps per SM in
+// flight, which is what a streaming kernel lives on -- at 40 registers it ran 10.7 -> 14 ms on B200 at config 5)
+template <bool IMP3>
+__global__ void __launch_bounds__(256, IMP3 ? 4 : 8) k_correct(Ctx c, CorrArgs a) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y * blockDim.y + threadIdx.y, k = blockIdx.z;
-  if (i < c.nx && j < c.ny) correct_point(c, a, i, j, k);
+  if (i < c.nx && j < c.ny) correct_point<IMP3>(c, a, i, j, k);
 }
 // deterministic two-stage sum of `n` partials: stage 1 -> out1[gridDim.x], stage 2 (one block) -> scalar
 __global__ void k_sum_stage1(const double* __restrict__ in, long long n, double* __restrict__ out1) {

@@ -31,8 +31,9 @@ enum { RT_TX = 32, RT_TY = 16, RT_RPT = 2, RT_TW = RT_TX + 2, RT_TH = RT_TY + 2,
 struct ZMet { double dzfk, dzfp, rdzf, rdzfp, rdzc, rdzcm; };
 CALES_HD ZMet zmet_at(const Ctx& c, int k) { return ZMet{c.dzf[k], c.dzf[k + 1], c.rdzf[k], c.rdzf[k + 1], c.rdzc[k], c.rdzc[k - 1]}; }
 
+// ru0, rv0, rw0: R^{k-1} at the point (read by the caller ahead of the stencil arithmetic so that the loads are in flight early)
 template <class A>
-CALES_HD double rhs_core(const Ctx& c, const RhsArgs& a, const A& q, int i, int j, int k, const ZMet& zm) {
+CALES_HD double rhs_core_r(const Ctx& c, const RhsArgs& a, const A& q, int i, int j, int k, const ZMet& zm, double ru0, double rv0, double rw0) {
   const long long n = idx3(c, i, j, k);
   const double rdx = c.rdx, rdy = c.rdy;
   const double dzfk = zm.dzfk, dzfp = zm.dzfp, rdzf = zm.rdzf, rdzfp = zm.rdzfp, rdzc = zm.rdzc, rdzcm = zm.rdzcm;
@@ -90,11 +91,9 @@ CALES_HD double rhs_core(const Ctx& c, const RhsArgs& a, const A& q, int i, int 
   }
   const double p000 = q.P(0, 0, 0);
   const double gpx = (q.P(1, 0, 0) - p000) * rdx, gpy = (q.P(0, 1, 0) - p000) * rdy, gpz = (q.P(0, 0, 1) - p000) * rdzc;
-  double ru0 = 0.0, rv0 = 0.0, rw0 = 0.0;
-  if (a.be != 0.0) { ru0 = a.Ru0[n]; rv0 = a.Rv0[n]; rw0 = a.Rw0[n]; }
   if (!vact) Rv = 0.0;
   if (!wact) Rw = 0.0;
-  const double dt = a.sc ? a.sc[RK_DT] : a.dt;
+  const double dt = a.sc ? ld_scalar(a.sc + RK_DT) : a.dt;
   double us = u000 + dt * (a.al * Ru + a.be * ru0 - a.ga * gpx);
   double vs = v000 + dt * (a.al * Rv + a.be * rv0 - a.ga * gpy);
   double ws = w000 + dt * (a.al * Rw + a.be * rw0 - a.ga * gpz);
@@ -114,6 +113,13 @@ CALES_HD double rhs_core(const Ctx& c, const RhsArgs& a, const A& q, int i, int 
   a.us[n] = us; a.vs[n] = vs; a.ws[n] = ws;
   if (a.store_R) { a.Ru1[n] = Ru; a.Rv1[n] = Rv; a.Rw1[n] = Rw; }
   return us;
+}
+
+template <class A>
+CALES_HD double rhs_core(const Ctx& c, const RhsArgs& a, const A& q, int i, int j, int k, const ZMet& zm) {
+  double ru0 = 0.0, rv0 = 0.0, rw0 = 0.0;
+  if (a.be != 0.0) { const long long n = idx3(c, i, j, k); ru0 = a.Ru0[n]; rv0 = a.Rv0[n]; rw0 = a.Rw0[n]; }
+  return rhs_core_r(c, a, q, i, j, k, zm, ru0, rv0, rw0);
 }
 
 // Accessor over the generic boundary-condition accessors (any point, any boundary).
@@ -220,35 +226,35 @@ __global__ void __launch_bounds__(RT_THREADS, 2) k_rhs_tile(const __grid_constan
   if (k0 + 1 <= k1) issue(k0 + 1);
   cp_async_commit();
   double acc = 0.0;
+  const bool useR = a.be != 0.0;
+  ZMet zm = zmet_at(c, k0);
   for (int k = k0; k < k1; ++k) {
+    // R^{k-1} of this plane and the metrics of the next one: issued before the wait on the staged planes, consumed at the end
+    // of the stencil arithmetic (ncu, profiles/r2_ncu_full.md: their first use was a quarter of all stall samples)
+    double r0[RT_RPT][3];
+#pragma unroll
+    for (int r = 0; r < RT_RPT; ++r) {
+      const int i = i0 + tx, j = j0 + ty * RT_RPT + r;
+      r0[r][0] = 0.0; r0[r][1] = 0.0; r0[r][2] = 0.0;
+      if (useR && i < c.nx && j < c.ny) { const long long nn = idx3(c, i, j, k); r0[r][0] = ldg_early(a.Ru0 + nn); r0[r][1] = ldg_early(a.Rv0 + nn); r0[r][2] = ldg_early(a.Rw0 + nn); }
+    }
+    const ZMet zn = zmet_at(c, k + 1 < k1 ? k + 1 : k);
     cp_async_wait_all();
     __syncthreads();
     if (k + 2 <= k1) issue(k + 2);
     cp_async_commit();
-    if (a.be != 0.0 && k + 1 < k1) {     // R^{k-1} of the next plane: pull the lines towards L1 while this plane is computed
-#pragma unroll
-      for (int r = 0; r < RT_RPT; ++r) {
-        const int i = i0 + tx, j = j0 + ty * RT_RPT + r;
-        if (i < c.nx && j < c.ny && (tx & 3) == 0) {       // one prefetch per 32-byte sector
-          const long long nn = idx3(c, i, j, k + 1);
-          asm volatile("prefetch.global.L1 [%0];" ::"l"(a.Ru0 + nn));
-          asm volatile("prefetch.global.L1 [%0];" ::"l"(a.Rv0 + nn));
-          asm volatile("prefetch.global.L1 [%0];" ::"l"(a.Rw0 + nn));
-        }
-      }
-    }
     TileAcc q;
     q.sl[0] = rt_sm + ((k + 3) & 3) * (RT_NF * RT_PLANE); q.sl[1] = rt_sm + (k & 3) * (RT_NF * RT_PLANE); q.sl[2] = rt_sm + ((k + 1) & 3) * (RT_NF * RT_PLANE);
-    const ZMet zm = zmet_at(c, k);
     const double dz = zm.dzfk;
 #pragma unroll
     for (int r = 0; r < RT_RPT; ++r) {
       const int ly = ty * RT_RPT + r, i = i0 + tx, j = j0 + ly;   // adjacent rows: their stencils share shared-memory loads
       if (i < c.nx && j < c.ny) {
         q.ctr = (ly + 1) * RT_TW + tx + 1;
-        acc += rhs_core(c, a, q, i, j, k, zm) * dz;
+        acc += rhs_core_r(c, a, q, i, j, k, zm, r0[r][0], r0[r][1], r0[r][2]) * dz;
       }
     }
+    zm = zn;
   }
   if (partial) {
     const double t = block_sum(acc, red);
