@@ -43,6 +43,7 @@ ALGO_BYTES = {
 # fp64 operations per grid point of the one kernel that is bound by the plain fp64 ALUs rather than by HBM (ncu instruction counts of
 # round 2, profiles/r2_ncu_dsm.md: 95 DFMA + 69 DADD + 55 DMUL = 219 fp64 instructions per point; an FMA counts 2).
 ALGO_FLOPS = {"k_dsm_col": 314.0}
+SPLIT_KERNELS = {"k_dsm_col"}      # names whose launches of one substep share the grid between them
 # fallback if the in-process measurement (cales_fp64_peak) fails: 148 SMs x 64 FMA lanes x 2 flop x 1.965 GHz
 FP64_PEAK_TFLOPS_DERIVED = 148 * 64 * 2 * 1.965e9 / 1e12
 TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r2_ncu_traffic.csv")
@@ -379,11 +380,15 @@ def run_ours(args):
     for name, (tot, n) in sorted(ktot.items(), key=lambda kv: -kv[1][0]):
         per = tot / n
         row = {"ms_per_launch": per, "launches_per_step": n // K, "share_of_step": (tot / K) / step_ms if step_ms else None}
+        # a kernel name launched more than once per substep (k_dsm_col: the staged march on the inner planes + the direct-load march on
+        # the two wall planes) covers the grid ONCE per substep with all its launches together: its per-launch share of the work
+        cover = 3.0 / max(n // K, 1) if (name in SPLIT_KERNELS and (n // K) > 3) else 1.0
+        row["grid_fraction_per_launch"] = cover
         if name in ALGO_BYTES:
-            gbs = ALGO_BYTES[name] * npts / (per * 1e-3) / 1e9
+            gbs = ALGO_BYTES[name] * cover * npts / (per * 1e-3) / 1e9
             row.update({"algo_bytes_per_pt": ALGO_BYTES[name], "achieved_gbs": gbs, "frac": gbs / peak})
         if name in ALGO_FLOPS:       # the kernel bound by the plain fp64 ALUs: also against the fp64 peak measured in this process
-            tf = ALGO_FLOPS[name] * npts / (per * 1e-3) / 1e12
+            tf = ALGO_FLOPS[name] * cover * npts / (per * 1e-3) / 1e12
             row.update({"algo_flops_per_pt": ALGO_FLOPS[name], "achieved_tflops": tf, "fp64_frac": tf / fp64_peak})
         if (cfg_no, name) in traffic:
             row["ncu_dram_bytes_per_launch"] = traffic[(cfg_no, name)][0]
@@ -397,12 +402,13 @@ def run_ours(args):
         tr = traffic.get((cfg_no, top))
         roofline = {"kernel": top, "bound": "hbm", "achieved": r["achieved_gbs"], "peak": peak, "unit": "GB/s", "frac": r["frac"],
                     "traffic": tr[0] if tr else None, "traffic_source": tr[1] if tr else None, "peak_source": peak_src,
-                    "algo_bytes_per_launch": ALGO_BYTES[top] * npts, "ms_per_launch": r["ms_per_launch"], "share_of_step": r["share_of_step"]}
+                    "algo_bytes_per_launch": ALGO_BYTES[top] * r["grid_fraction_per_launch"] * npts, "ms_per_launch": r["ms_per_launch"],
+                    "share_of_step": r["share_of_step"]}
         if top in ALGO_FLOPS:        # bound by the plain fp64 ALUs, not by HBM: report it against that peak
             roofline.update({"bound": "alu", "achieved": r["achieved_tflops"], "peak": fp64_peak, "unit": "TFLOP/s", "frac": r["fp64_frac"],
-                             "peak_source": fp64_src, "algo_flops_per_launch": ALGO_FLOPS[top] * npts, "hbm_frac_of_measured_peak": r["frac"]})
+                             "peak_source": fp64_src, "algo_flops_per_launch": ALGO_FLOPS[top] * r["grid_fraction_per_launch"] * npts, "hbm_frac_of_measured_peak": r["frac"]})
     # whole-step algorithmic traffic: the sum over the step's launches of the table above
-    step_bytes = sum(ALGO_BYTES.get(n, 0.0) * (a[1] // K) for n, a in ktot.items()) * npts
+    step_bytes = sum(ALGO_BYTES.get(n, 0.0) * (a[1] // K) * kernels[n]["grid_fraction_per_launch"] for n, a in ktot.items()) * npts
     step_gbs = step_bytes / (ms / K * 1e-3) / 1e9
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms / K,
