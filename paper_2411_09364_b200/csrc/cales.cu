@@ -67,6 +67,8 @@ struct cales_solver {
   long long tile_min;   // grids with at least this many points use the staged z-march for the static model
   int rhs_variant;      // 1 (default): halo planes by 8-byte cp.async (k_rhs_tile); 0: by tiled TMA copies (k_rhs_tile_tma)
   RhsMaps* rmaps; bool rmaps_ok;   // tensor maps of u, v, w, nu_t, p in device memory (workspace)
+  bool nut_lazy, nut_valid; int graph_lazy;   // dynamic model: the momentum kernel forms nu_t from |S| and c_s (nut_lazy); s->nut holds it only when nut_valid
+  int lazy_nut;         // option: 1 (default) skips the |S| -> nu_t pass of the dynamic model
   int dsm_col_variant;  // 0: TMA-staged register-window column march (k_dsm_col_tma); 1: shared-ring form of round 1 (k_dsm_col_sm); 2: direct loads (k_dsm_col_rw)
   double cn_dt;   // dt the Crank-Nicolson tables on the device were built for (0: none, or a device-side dt)
   int use_graph; cudaGraphExec_t gexec;   // the three substeps captured as one CUDA graph (dt lives in device memory: one graph serves every dt)
@@ -253,6 +255,7 @@ extern "C" int cales_create(const cales_params* p, cales_solver** out) {
   s->tile_min = 4000000;
   s->rhs_tile_min = 200000;
   s->dsm_col_variant = 0;
+  s->nut_lazy = false; s->nut_valid = true; s->graph_lazy = -1; s->lazy_nut = 1;
   s->rhs_variant = 1;      // measured on B200 at config 5: cp.async ring 22.7 ms, tiled TMA ring 25.1 ms per launch
   {
     const double* fl[RT_NF] = {s->u, s->v, s->w, s->nut, s->p};
@@ -285,6 +288,7 @@ extern "C" int cales_destroy(cales_solver* s) {
   return CALES_OK;
 }
 
+static int ensure_nut(cales_solver* s);
 static double* field_ptr(cales_solver* s, int f) {
   switch (f) { case CALES_U: return s->u; case CALES_V: return s->v; case CALES_W: return s->w; case CALES_P: return s->p; case CALES_NUT: return s->nut; }
   return nullptr;
@@ -303,6 +307,7 @@ extern "C" int cales_set_field(cales_solver* s, int field, const double* src, in
     CUDA_TRY(cudaMemsetAsync(d + (size_t)(s->c.nz - 1) * s->nxy, 0, (size_t)s->nxy * sizeof(double), s->st));
   if (!on_device) CUDA_TRY(cudaStreamSynchronize(s->st));
   if (field <= CALES_W) s->fresh = false;
+  if (field == CALES_NUT) { s->nut_lazy = false; s->nut_valid = true; }      // the caller's nu_t is taken as it is
   return CALES_OK;
 }
 extern "C" int cales_get_field(cales_solver* s, int field, double* dst, int on_device) {
@@ -310,6 +315,7 @@ extern "C" int cales_get_field(cales_solver* s, int field, double* dst, int on_d
   if (!s || !dst) return fail(CALES_EINVAL, "null argument");
   double* d = field_ptr(s, field);
   if (!d) return fail(CALES_EINVAL, "bad field id");
+  if (field == CALES_NUT) { int rc = ensure_nut(s); if (rc) return rc; }
   CUDA_TRY(cudaMemcpyAsync(dst, d, s->N * sizeof(double), on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, s->st));
   if (!on_device) CUDA_TRY(cudaStreamSynchronize(s->st));
   return CALES_OK;
@@ -367,6 +373,8 @@ static int run_wall_stress(cales_solver* s) {
   }
   return CALES_OK;
 }
+// the |S| -> nu_t pass can be skipped when the momentum kernel that will consume nu_t forms it itself (every form but the TMA variant)
+static bool lazy_ok(const cales_solver* s) { return s->lazy_nut != 0 && !(s->rhs_variant == 0 && s->rmaps_ok && s->N >= s->rhs_tile_min); }
 static int run_eddy_viscosity(cales_solver* s, const double* u, const double* v, const double* w, double* nut) {
   if (s->c.sgs == CALES_SGS_NONE) {
     k_fill<<<1184, 256, 0, s->st>>>(nut, s->N, 0.0);
@@ -433,9 +441,27 @@ static int run_eddy_viscosity(cales_solver* s, const double* u, const double* v,
     }
     k_dsm_coef<<<s->c.nz, 128, 0, s->st>>>(s->c, s->dsm_part, ds.pslots, s->dsm_cs);
     LAUNCH_TRY(K_DSM_COEF);
-    k_dsm_nut<<<s->pgrid, s->pblock, 0, s->st>>>(s->c, s->dsm_cs, s->smag, nut);
-    LAUNCH_TRY(K_DSM_NUT);
+    if (nut == s->nut && lazy_ok(s)) {
+      // the solver's own nu_t stays implicit: |S| in s->smag, c_s in s->dsm_cs; the momentum kernel forms c_s Delta^2 |S| (with the
+      // clip) when it stages the plane, cales_get_field / the statistics materialise it on demand (ensure_nut)
+      s->nut_lazy = true; s->nut_valid = false;
+    } else {
+      k_dsm_nut<<<s->pgrid, s->pblock, 0, s->st>>>(s->c, s->dsm_cs, s->smag, nut);
+      LAUNCH_TRY(K_DSM_NUT);
+      if (nut == s->nut) { s->nut_lazy = false; s->nut_valid = true; }
+    }
+    return CALES_OK;
   }
+  if (nut == s->nut) { s->nut_lazy = false; s->nut_valid = true; }
+  return CALES_OK;
+}
+// s->nut as an array of nu_t values (the lazy dynamic model keeps |S| and c_s instead)
+static int ensure_nut(cales_solver* s) {
+  if (!s->nut_lazy || s->nut_valid) return CALES_OK;
+  TimingOff toff(s);
+  k_dsm_nut<<<s->pgrid, s->pblock, 0, s->st>>>(s->c, s->dsm_cs, s->smag, s->nut);
+  LAUNCH_TRY(K_DSM_NUT);
+  s->nut_valid = true;
   return CALES_OK;
 }
 // Alg. 2 on the current velocity, then nu_t (Alg. 1 l.2 / l.12)
@@ -453,7 +479,7 @@ static int substep(cales_solver* s, int rk) {
   const Ctx& c = s->c;
   const bool cfr = c.const_flow_rate != 0, imp = c.implicit_z == 1, imp3 = c.implicit_z == 2;
   RhsArgs a;
-  a.u = s->u; a.v = s->v; a.w = s->w; a.p = s->p; a.nut = s->nut;
+  a.u = s->u; a.v = s->v; a.w = s->w; a.p = s->p; a.nut = s->nut_lazy ? s->smag : s->nut; a.cs = s->nut_lazy ? s->dsm_cs : nullptr;
   a.Ru0 = s->Ru; a.Rv0 = s->Rv; a.Rw0 = s->Rw; a.Ru1 = s->Ru; a.Rv1 = s->Rv; a.Rw1 = s->Rw;
   const double* sc = s->rks + rk * RK_STRIDE;      // dt, gamma dt, 1/(gamma dt), gamma nu dt / 2 of this substep, in device memory
   a.us = s->us; a.vs = s->vs; a.ws = s->ws; a.dt = 0.0; a.al = al; a.be = be; a.ga = ga; a.store_R = rk < 2 ? 1 : 0; a.sc = sc;
@@ -515,7 +541,10 @@ extern "C" int cales_launches_per_step(cales_solver* s);
 static int run_substeps(cales_solver* s) {
   int rc;
   if (s->use_graph && !s->timing) {
+    if (s->gexec && s->graph_lazy != (int)s->nut_lazy) { cudaGraphExecDestroy(s->gexec); s->gexec = nullptr; }   // the first substep's nu_t source is baked in
     if (s->gexec) {
+      const bool dsm = s->c.sgs == CALES_SGS_DSMAG;
+      if (dsm) { s->nut_lazy = lazy_ok(s); s->nut_valid = !s->nut_lazy; }      // what the replayed substeps leave behind
       CUDA_TRY(cudaGraphLaunch(s->gexec, s->st));
       s->launches += cales_launches_per_step(s);
       return CALES_OK;
@@ -524,6 +553,7 @@ static int run_substeps(cales_solver* s) {
     if (cudaStreamBeginCapture(s->st, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
       rc = CALES_OK;
       const int l0 = s->launches;
+      s->graph_lazy = (int)s->nut_lazy;
       for (int rk = 0; rk < 3 && rc == CALES_OK; ++rk) rc = substep(s, rk);
       const cudaError_t ee = cudaStreamEndCapture(s->st, &g);
       if (rc == CALES_OK && ee == cudaSuccess && g && cudaGraphInstantiate(&s->gexec, g, 0) == cudaSuccess) {
@@ -565,6 +595,7 @@ extern "C" int cales_step(cales_solver* s, double dt) {
   if (!s->fresh && (rc = refresh_closures(s))) return rc;
   { TimingOff toff(s); rc = prepare_dt(s, dt, nullptr); }      // the two table kernels are not part of the timed step
   if (rc) return rc;
+  if (s->nut_lazy && !lazy_ok(s)) { if ((rc = ensure_nut(s))) return rc; s->nut_lazy = false; }
   s->last_dt = dt;
   return run_substeps(s);
 }
@@ -591,6 +622,7 @@ extern "C" int cales_step_adaptive(cales_solver* s, double cfl) {
     rc = prepare_dt(s, 0.0, s->dtdev);
   } while (0);
   if (rc) return rc;
+  if (s->nut_lazy && !lazy_ok(s)) { if ((rc = ensure_nut(s))) return rc; s->nut_lazy = false; }
   s->last_dt = -1.0;      // on the device: cales_last_dt reads it back
   return run_substeps(s);
 }
@@ -631,6 +663,7 @@ extern "C" int cales_set_option(cales_solver* s, const char* key, long long valu
     if (th > 512 || sm > 200 * 1024) return fail(CALES_EINVAL, "fft_x_lines: CTA too large");
     s->xB = L; s->x_threads = (int)th; s->x_smem = sm;
   }
+  else if (k == "lazy_nut") { if (value < 0 || value > 1) return fail(CALES_EINVAL, "lazy_nut must be 0 or 1"); s->lazy_nut = (int)value; }
   else if (k == "rhs_variant") { if (value < 0 || value > 1) return fail(CALES_EINVAL, "rhs_variant must be 0 or 1"); s->rhs_variant = (int)value; }
   else if (k == "dsm_col_variant") { if (value < 0 || value > 2) return fail(CALES_EINVAL, "dsm_col_variant must be 0, 1 or 2"); s->dsm_col_variant = (int)value; }
   else return fail(CALES_EINVAL, "unknown option: " + k);
@@ -651,7 +684,7 @@ extern "C" int cales_launches_per_step(cales_solver* s) {
       const D3Split sp = d3_split(c, s->P.zstretch == CALES_Z_UNIFORM);
       pass1 = sp.col ? 1 + (sp.klo > 0 ? 1 : 0) + (sp.jlo > 0 ? 1 : 0) : 1;
     }
-    per += -1 + pass1 + 2;   // pass 1 (tile and/or column kernel), coefficient, nu_t
+    per += -1 + pass1 + (lazy_ok(s) ? 1 : 2);   // pass 1 (tile and/or column kernel), coefficient, nu_t (formed by the momentum kernel when lazy)
   }
   return 3 * per;
 }
@@ -672,6 +705,12 @@ extern "C" int cales_eddy_viscosity(cales_solver* s, const double* u, const doub
   const bool own = !u && !v && !w;
   if (!own && (!u || !v || !w)) return fail(CALES_EINVAL, "u, v, w must be all given or all NULL");
   if (!own && !nut) return fail(CALES_EINVAL, "external u, v, w need an external nut: the solver's own nu_t belongs to its own velocity");
+  if (nut && nut != s->nut && s->nut_lazy) {      // the evaluation below reuses the |S| / c_s scratch the solver's own lazy nu_t lives in
+    int rc = ensure_nut(s);
+    if (rc) return rc;
+    s->nut_lazy = false;
+    if (s->gexec) { cudaGraphExecDestroy(s->gexec); s->gexec = nullptr; }
+  }
   return run_eddy_viscosity(s, own ? s->u : u, own ? s->v : v, own ? s->w : w, nut ? nut : s->nut);
 }
 
@@ -735,6 +774,7 @@ extern "C" int cales_plane_stats(cales_solver* s, double* out_dev) {
   DevGuard dg_(s ? s->device : -1);
   if (!s || !out_dev) return fail(CALES_EINVAL, "null argument");
   TimingOff toff(s);
+  { int rc = ensure_nut(s); if (rc) return rc; }
   k_plane_stats<<<s->c.nz, 1024, 0, s->st>>>(s->c, s->u, s->v, s->w, s->nut, out_dev);
   return check_launch(s, K_DIAG);
 }
@@ -753,6 +793,7 @@ extern "C" int cales_stats_accumulate(cales_solver* s, double weight) {
   TimingOff toff(s);
   do {
     if (!s->fresh && (rc = refresh_closures(s))) break;      // the wall-model planes must belong to the current velocity
+    if ((rc = ensure_nut(s))) break;
     const int n = 8 * s->c.nz + 8;
     double* tmp = s->stats + (8 * (size_t)s->c.nz + 16);
     k_plane_stats<<<s->c.nz, 1024, 0, s->st>>>(s->c, s->u, s->v, s->w, s->nut, tmp);

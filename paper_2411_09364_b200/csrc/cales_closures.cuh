@@ -411,13 +411,15 @@ CALES_HD void dsm_row_sums(const double* part, int ntx, long long row, double* l
 }
 
 // pass 2: nu_t = c_s Delta^2 |S| with the clip of PAPER.md:128 (c_s >= 0) or of the total viscosity (S14)
-CALES_HD double dsm_nut_point(const Ctx& c, const double* cs, const double* smag, int i, int j, int k) {
+CALES_HD double dsm_nut_value(const Ctx& c, const double* cs, double sm, int j, int k) {
   const double cc = c.dsm_plane ? cs[k] : cs[(long long)k * c.ny + j];
   const double d2 = c.delta[k] * c.delta[k];
-  const double sm = smag[idx3(c, i, j, k)];
   if (!c.dsm_clip_total) return (cc < 0.0 ? 0.0 : cc) * d2 * sm;
   const double t = cc * d2 * sm;
   return t < -c.nu ? -c.nu : t;
+}
+CALES_HD double dsm_nut_point(const Ctx& c, const double* cs, const double* smag, int i, int j, int k) {
+  return dsm_nut_value(c, cs, smag[idx3(c, i, j, k)], j, k);
 }
 
 #ifdef __CUDACC__

@@ -19,6 +19,8 @@ struct RhsArgs {
   double dt, al, be, ga;
   int store_R;
   const double* sc;                      // substep scalar block in device memory (RK_*), or nullptr: dt above is used
+  const double* cs;                      // dynamic model, lazy nu_t: `nut` holds |S| and nu_t = dsm_nut_value(cs, |S|, j, k) is formed when
+                                         // the momentum kernel stages it (saves the |S| -> nu_t pass, 16 B/pt per substep); nullptr: nut is nu_t
 };
 
 // Substep scalars kept in device memory so that one captured CUDA graph serves every dt (and dt itself may be computed on the

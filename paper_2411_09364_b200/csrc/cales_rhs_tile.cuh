@@ -12,6 +12,7 @@
 #pragma once
 #include "cales_common.cuh"
 #include "cales_momentum.cuh"
+#include "cales_closures.cuh"
 #ifdef __CUDACC__
 #include <cuda.h>
 #endif
@@ -122,13 +123,26 @@ CALES_HD double rhs_core(const Ctx& c, const RhsArgs& a, const A& q, int i, int 
   return rhs_core_r(c, a, q, i, j, k, zm, ru0, rv0, rw0);
 }
 
+// nu_t with ghosts (ghost = -interior at walls, S7; periodic wrap otherwise).  With the lazy dynamic model (a.cs) the
+// array holds |S| and the value is formed here from the coefficient of the row / plane the (possibly mirrored) element lies in.
+CALES_HD double nutg(const Ctx& c, const RhsArgs& a, int i, int j, int k) {
+  i = wrapi(i, c.nx);
+  double s = 1.0;
+  if (c.bc_y == BC_PER) j = wrapi(j, c.ny);
+  else { if (j < 0) { j = 0; s = -s; } else if (j >= c.ny) { j = c.ny - 1; s = -s; } }
+  if (c.bc_z == BC_PER) k = wrapi(k, c.nz);
+  else { if (k < 0) { k = 0; s = -s; } else if (k >= c.nz) { k = c.nz - 1; s = -s; } }
+  const double q = a.nut[idx3(c, i, j, k)];
+  return s * (a.cs ? dsm_nut_value(c, a.cs, q, j, k) : q);
+}
+
 // Accessor over the generic boundary-condition accessors (any point, any boundary).
 struct GhostAcc {
   const Ctx& c; const RhsArgs& a; int i, j, k;
   CALES_HD double U(int di, int dj, int dk) const { return velg<0>(c, a.u, i + di, j + dj, k + dk, GH_VISC); }
   CALES_HD double V(int di, int dj, int dk) const { return velg<1>(c, a.v, i + di, j + dj, k + dk, GH_VISC); }
   CALES_HD double W(int di, int dj, int dk) const { return velg<2>(c, a.w, i + di, j + dj, k + dk, GH_VISC); }
-  CALES_HD double NT(int di, int dj, int dk) const { return scalg(c, a.nut, i + di, j + dj, k + dk, -1.0); }
+  CALES_HD double NT(int di, int dj, int dk) const { return nutg(c, a, i + di, j + dj, k + dk); }
   CALES_HD double P(int di, int dj, int dk) const { return scalg(c, a.p, i + di, j + dj, k + dk, 1.0); }
 };
 
@@ -138,7 +152,7 @@ CALES_HD double rt_elem(const Ctx& c, const RhsArgs& a, int f, int gi, int gj, i
     case 0: return velg<0>(c, a.u, gi, gj, gk, GH_VISC);
     case 1: return velg<1>(c, a.v, gi, gj, gk, GH_VISC);
     case 2: return velg<2>(c, a.w, gi, gj, gk, GH_VISC);
-    case 3: return c.sgs ? scalg(c, a.nut, gi, gj, gk, -1.0) : 0.0;
+    case 3: return c.sgs ? nutg(c, a, gi, gj, gk) : 0.0;
     default: return scalg(c, a.p, gi, gj, gk, 1.0);
   }
 }
@@ -222,24 +236,32 @@ __global__ void __launch_bounds__(RT_THREADS, 2) k_rhs_tile(const __grid_constan
       }
     }
   };
+  // the elements of plane kk this thread copied asynchronously (the synchronous ghost path has formed nu_t already)
+  auto scale_nut = [&](int kk) {
+    if (!(c.bc_z == BC_PER || (kk >= 0 && kk < c.nz))) return;
+    double* pl = rt_sm + ((kk + 4) & 3) * (RT_NF * RT_PLANE) + 3 * RT_PLANE;
+    const int kw = kk < 0 ? kk + c.nz : (kk >= c.nz ? kk - c.nz : kk);
+#pragma unroll
+    for (int e = 0; e < RT_EPT; ++e) {
+      if (goff[e] < 0) continue;
+      const int gj = c.dsm_plane ? 0 : (int)((unsigned)goff[e] / (unsigned)c.nx);
+      pl[soff[e]] = dsm_nut_value(c, a.cs, pl[soff[e]], gj, kw);
+    }
+  };
   issue(k0 - 1); issue(k0);
   if (k0 + 1 <= k1) issue(k0 + 1);
   cp_async_commit();
   double acc = 0.0;
-  const bool useR = a.be != 0.0;
   ZMet zm = zmet_at(c, k0);
   for (int k = k0; k < k1; ++k) {
-    // R^{k-1} of this plane and the metrics of the next one: issued before the wait on the staged planes, consumed at the end
-    // of the stencil arithmetic (ncu, profiles/r2_ncu_full.md: their first use was a quarter of all stall samples)
-    double r0[RT_RPT][3];
-#pragma unroll
-    for (int r = 0; r < RT_RPT; ++r) {
-      const int i = i0 + tx, j = j0 + ty * RT_RPT + r;
-      r0[r][0] = 0.0; r0[r][1] = 0.0; r0[r][2] = 0.0;
-      if (useR && i < c.nx && j < c.ny) { const long long nn = idx3(c, i, j, k); r0[r][0] = ldg_early(a.Ru0 + nn); r0[r][1] = ldg_early(a.Rv0 + nn); r0[r][2] = ldg_early(a.Rw0 + nn); }
-    }
+    // the metrics of the next plane are read one plane ahead; R^{k-1} is read inside rhs_core (early, pinned loads of it were
+    // measured: no gain at 12 more live registers)
     const ZMet zn = zmet_at(c, k + 1 < k1 ? k + 1 : k);
     cp_async_wait_all();
+    if (a.cs && c.sgs) {      // lazy dynamic model: this thread's |S| elements of the planes that have just landed become nu_t
+#pragma unroll 1
+      for (int kk = (k == k0) ? k0 - 1 : k + 1; kk <= k + 1; ++kk) scale_nut(kk);
+    }
     __syncthreads();
     if (k + 2 <= k1) issue(k + 2);
     cp_async_commit();
@@ -251,7 +273,7 @@ __global__ void __launch_bounds__(RT_THREADS, 2) k_rhs_tile(const __grid_constan
       const int ly = ty * RT_RPT + r, i = i0 + tx, j = j0 + ly;   // adjacent rows: their stencils share shared-memory loads
       if (i < c.nx && j < c.ny) {
         q.ctr = (ly + 1) * RT_TW + tx + 1;
-        acc += rhs_core_r(c, a, q, i, j, k, zm, r0[r][0], r0[r][1], r0[r][2]) * dz;
+        acc += rhs_core(c, a, q, i, j, k, zm) * dz;
       }
     }
     zm = zn;

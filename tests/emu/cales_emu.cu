@@ -338,7 +338,7 @@ static void emu_substep(emu_solver* s, int rk, double dt) {
   RhsArgs a;
   a.u = s->u.data(); a.v = s->v.data(); a.w = s->w.data(); a.p = s->p.data(); a.nut = s->nut.data();
   a.Ru0 = s->Ru.data(); a.Rv0 = s->Rv.data(); a.Rw0 = s->Rw.data(); a.Ru1 = s->Ru.data(); a.Rv1 = s->Rv.data(); a.Rw1 = s->Rw.data();
-  a.us = s->us.data(); a.vs = s->vs.data(); a.ws = s->ws.data(); a.dt = dt; a.al = al; a.be = be; a.ga = ga; a.store_R = rk < 2 ? 1 : 0; a.sc = nullptr;
+  a.us = s->us.data(); a.vs = s->vs.data(); a.ws = s->ws.data(); a.dt = dt; a.al = al; a.be = be; a.ga = ga; a.store_R = rk < 2 ? 1 : 0; a.sc = nullptr; a.cs = nullptr;
   double sum = 0.0;
   {  // k_rhs_tile: per CTA tile and plane, stage the three halo planes with the staging rule of the kernel (rt_elem), then
      // evaluate rhs_core through the shared-memory accessor

@@ -520,3 +520,33 @@ def test_repeated_runs_are_bit_identical(oracle, gpu, n, shape, over):
                 for a, b in zip(out, ref[key]):
                     assert np.array_equal(a, b), (key, rep)
             g.close()
+
+
+@pytest.mark.parametrize("n,shape", [(5, (96, 48, 32)), (4, (96, 36, 24))])
+def test_lazy_nu_t_is_the_same_nu_t(oracle, gpu, n, shape):
+    """Dynamic model: by default the |S| -> nu_t pass is skipped and the momentum kernel forms c_s Delta^2 |S| (with the clip) when it
+    stages a plane.  Same bits as the materialised form; an external cales_eddy_viscosity call in between (it shares the scratch the
+    lazy nu_t lives in) must not disturb the run; the statistics and cales_get_field see a proper nu_t."""
+    import torch
+    cfg, kw, (u, v, w), dt = pc.prepare(oracle, n, shape)
+    o = pc.make(oracle.Oracle, kw)
+    a = pc.make(gpu.Solver, kw)
+    b = pc.make(gpu.Solver, kw); b.set_option("lazy_nut", 0)
+    for s_ in (o, a, b):
+        s_.set_velocity(u, v, w)
+    assert a.launches_per_step() == b.launches_per_step() - 3
+    for s in range(2):
+        o.step(dt); a.step(dt); b.step(dt)
+    for f in range(5):
+        assert np.array_equal(a.get_numpy(f), b.get_numpy(f)), f
+    # an evaluation on a foreign field, then go on
+    ext = [torch.from_numpy(q * 1.7).cuda() for q in (u, v, w)]
+    a.eddy_viscosity(*ext)
+    st_a, st_o = a.plane_stats().cpu().numpy(), o.plane_stats()
+    assert np.max(np.abs(st_a[7] - st_o[7])) <= 1e-11 * max(float(np.max(np.abs(st_o[7]))), kw["nu"])
+    o.step(dt); a.step(dt); b.step(dt)
+    err = pc.field_errors(_gpu_fields(a), [o.get(f) for f in range(5)], o.dzf, kw["nu"])
+    assert max(err.values()) <= TOL_1STEP * 30, err
+    for f in range(5):
+        assert np.array_equal(a.get_numpy(f), b.get_numpy(f)), f
+    a.close(); b.close()
