@@ -217,6 +217,7 @@ int cales_fp64_peak(cales_solver* s, double* tflops_host);
 /* Kernel-selection knobs, for tests and A/B timing only (results do not depend on them beyond round-off; the defaults are the
  * measured best): "rhs_tile_min_points" (grids with fewer points run the momentum kernel one thread per point instead of the
  * staged z-march; default 200000), "smag_tile_min_points" (the same for the static model; default 4000000),
+ * "dsm_col_rows" (output rows per CTA of the column march of the dynamic model; 0 (default): chosen from the grid),
  * "lazy_nut" (dynamic model -- 1 (default): the |S| -> nu_t pass is skipped, the momentum kernel forms c_s Delta^2 |S| when it stages
  * the plane and cales_get_field(CALES_NUT) / the statistics materialise it on demand; 0: nu_t is written after every evaluation),
  * "rhs_variant" (staged momentum kernel -- 1 (default): halo planes moved by 8-byte cp.async, 0: by tiled TMA copies),

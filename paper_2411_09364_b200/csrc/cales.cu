@@ -68,6 +68,7 @@ struct cales_solver {
   int rhs_variant;      // 1 (default): halo planes by 8-byte cp.async (k_rhs_tile); 0: by tiled TMA copies (k_rhs_tile_tma)
   RhsMaps* rmaps; bool rmaps_ok;   // tensor maps of u, v, w, nu_t, p in device memory (workspace)
   bool nut_lazy, nut_valid; int graph_lazy;   // dynamic model: the momentum kernel forms nu_t from |S| and c_s (nut_lazy); s->nut holds it only when nut_valid
+  int dsm_col_rows;     // option: output rows per CTA of the column march (0: chosen from the grid)
   int lazy_nut;         // option: 1 (default) skips the |S| -> nu_t pass of the dynamic model
   int dsm_col_variant;  // 0: TMA-staged register-window column march (k_dsm_col_tma); 1: shared-ring form of round 1 (k_dsm_col_sm); 2: direct loads (k_dsm_col_rw)
   double cn_dt;   // dt the Crank-Nicolson tables on the device were built for (0: none, or a device-side dt)
@@ -255,7 +256,7 @@ extern "C" int cales_create(const cales_params* p, cales_solver** out) {
   s->tile_min = 4000000;
   s->rhs_tile_min = 200000;
   s->dsm_col_variant = 0;
-  s->nut_lazy = false; s->nut_valid = true; s->graph_lazy = -1; s->lazy_nut = 1;
+  s->nut_lazy = false; s->nut_valid = true; s->graph_lazy = -1; s->lazy_nut = 1; s->dsm_col_rows = 0;
   s->rhs_variant = 1;      // measured on B200 at config 5: cp.async ring 22.7 ms, tiled TMA ring 25.1 ms per launch
   {
     const double* fl[RT_NF] = {s->u, s->v, s->w, s->nut, s->p};
@@ -430,12 +431,17 @@ static int run_eddy_viscosity(cales_solver* s, const double* u, const double* v,
       // variant 0 (default): TMA-staged march on the planes without z-wall ghosts, the direct-load march on the others;
       // bulk copies need 16-byte aligned rows (nx is even, so the field pointers decide) and nx >= 66
       const bool tma_ok = s->dsm_col_variant == 0 && (((size_t)u | (size_t)v | (size_t)w) & 15) == 0 && c.nx >= 66;
-      const unsigned nby = grid.y;
+      // rows per CTA of the register-window marches: every CTA spends two rows filling its y-window, long bands leave a ragged
+      // tail.  Measured on B200 (eddy viscosity, ms): config 5 (1024 rows) 32: 22.9, 64: 22.1, 128: 22.4, 256: 23.5; config 4
+      // (252 rows) 32: 2.99, 64: 3.38, 128: 4.32
+      int ly = s->dsm_col_rows;
+      if (ly <= 0) ly = (jhi - jlo >= 512) ? 64 : 32;
+      const unsigned nby = (unsigned)((jhi - jlo + ly - 1) / ly);
       if (tma_ok) {
         const int klo = c.bc_z == BC_PER ? 0 : 1, khi = c.bc_z == BC_PER ? c.nz : c.nz - 1;
-        k_dsm_col_tma<64, CALES_DSMR_MINB><<<dim3(ds.nbx, khi - klo, nby), 64, 0, s->st>>>(c, u, v, w, klo, jlo, jhi, ds.pslots, s->smag, s->dsm_part);
-        if (klo > 0) { LAUNCH_TRY(K_DSM_COL); k_dsm_col_rw<64, CALES_DSMR_MINB><<<dim3(ds.nbx, 2, nby), 64, 0, s->st>>>(c, u, v, w, 0, c.nz - 1, jlo, jhi, ds.pslots, s->smag, s->dsm_part); }
-      } else if (s->dsm_col_variant != 1) k_dsm_col_rw<64, CALES_DSMR_MINB><<<dim3(ds.nbx, c.nz, nby), 64, 0, s->st>>>(c, u, v, w, 0, 1, jlo, jhi, ds.pslots, s->smag, s->dsm_part);
+        k_dsm_col_tma<64, CALES_DSMR_MINB><<<dim3(ds.nbx, khi - klo, nby), 64, 0, s->st>>>(c, u, v, w, klo, jlo, jhi, ly, ds.pslots, s->smag, s->dsm_part);
+        if (klo > 0) { LAUNCH_TRY(K_DSM_COL); k_dsm_col_rw<64, CALES_DSMR_MINB><<<dim3(ds.nbx, 2, nby), 64, 0, s->st>>>(c, u, v, w, 0, c.nz - 1, jlo, jhi, ly, ds.pslots, s->smag, s->dsm_part); }
+      } else if (s->dsm_col_variant != 1) k_dsm_col_rw<64, CALES_DSMR_MINB><<<dim3(ds.nbx, c.nz, nby), 64, 0, s->st>>>(c, u, v, w, 0, 1, jlo, jhi, ly, ds.pslots, s->smag, s->dsm_part);
       else k_dsm_col_sm<64, 6, 0><<<dim3(ds.nbx, grid.y, grid.z), 64, 0, s->st>>>(c, u, v, w, jlo, jhi, ds.pslots, s->smag, s->dsm_part);
       LAUNCH_TRY(K_DSM_COL);
     }
@@ -663,6 +669,7 @@ extern "C" int cales_set_option(cales_solver* s, const char* key, long long valu
     if (th > 512 || sm > 200 * 1024) return fail(CALES_EINVAL, "fft_x_lines: CTA too large");
     s->xB = L; s->x_threads = (int)th; s->x_smem = sm;
   }
+  else if (k == "dsm_col_rows") { if (value < 0 || value > 4096) return fail(CALES_EINVAL, "dsm_col_rows must be 0..4096"); s->dsm_col_rows = (int)value; }
   else if (k == "lazy_nut") { if (value < 0 || value > 1) return fail(CALES_EINVAL, "lazy_nut must be 0 or 1"); s->lazy_nut = (int)value; }
   else if (k == "rhs_variant") { if (value < 0 || value > 1) return fail(CALES_EINVAL, "rhs_variant must be 0 or 1"); s->rhs_variant = (int)value; }
   else if (k == "dsm_col_variant") { if (value < 0 || value > 2) return fail(CALES_EINVAL, "dsm_col_variant must be 0, 1 or 2"); s->dsm_col_variant = (int)value; }

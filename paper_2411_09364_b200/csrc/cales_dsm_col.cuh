@@ -129,19 +129,19 @@ CALES_HD void dsmr_row(const double* shbuf, int txb, int t, const double* b, Dsm
 }
 
 #ifdef __CUDACC__
-// grid (ceil(nx/(TXB-2)), planes, ceil((jhi-jlo)/DSMC_LY)), block TXB (multiple of 32).  Planes k0 + blockIdx.y * kstride,
+// grid (ceil(nx/(TXB-2)), planes, ceil((jhi-jlo)/ly)), block TXB (multiple of 32); ly = output rows per CTA.  Planes k0 + blockIdx.y * kstride,
 // output rows [jlo, jhi).
 // part: [k][j][pslots][2]; this kernel fills slots blockIdx.x*(TXB/32) + warp of its rows: per row with x-line averaging, the
 // CTA's total in its first row (zeros in the others) with plane averaging.
 template <int TXB, int MINB>
 __global__ void __launch_bounds__(TXB, MINB) k_dsm_col_rw(const __grid_constant__ Ctx c, const double* __restrict__ u, const double* __restrict__ v,
-                                                          const double* __restrict__ w, int k0, int kstride, int jlo, int jhi, int pslots,
+                                                          const double* __restrict__ w, int k0, int kstride, int jlo, int jhi, int ly, int pslots,
                                                           double* __restrict__ smag, double* __restrict__ part) {
   __shared__ double sh[2][DSMC_NB * TXB];
   const int t = threadIdx.x, k = k0 + blockIdx.y * kstride;
   const int i0 = blockIdx.x * (TXB - 2);
-  const int j0 = jlo + blockIdx.z * DSMC_LY;
-  const int jend = min(j0 + DSMC_LY, jhi);
+  const int j0 = jlo + blockIdx.z * ly;
+  const int jend = min(j0 + ly, jhi);
   const int nrows = jend - j0 + 2;
   const int gi = i0 - 1 + t;
   const int gw = ((gi % c.nx) + c.nx) % c.nx;
@@ -213,12 +213,12 @@ __global__ void __launch_bounds__(TXB, MINB) k_dsm_col_rw(const __grid_constant_
 // stencil is 30 shared-memory loads at immediate offsets.  Planes next to a z wall (wall ghosts) are left to k_dsm_col_rw.
 enum { DSMT_NS = 4, DSMT_NL = 8 };
 
-// grid (ceil(nx/(TXB-2)), khi-klo, ceil((jhi-jlo)/DSMC_LY)), block TXB = 64; planes [klo, khi), output rows [jlo, jhi).
+// grid (ceil(nx/(TXB-2)), khi-klo, ceil((jhi-jlo)/ly)), block TXB = 64; planes [klo, khi), output rows [jlo, jhi).
 // Needs nx >= TXB + 2, 16-byte aligned fields, and every base row jlo-1 .. jhi an interior row (periodic y, or 1 <= j <= ny-2).
 template <int TXB, int MINB>
 __global__ void __launch_bounds__(TXB, MINB) k_dsm_col_tma(const __grid_constant__ Ctx c, const double* __restrict__ u, const double* __restrict__ v,
-                                                           const double* __restrict__ w, int klo, int jlo, int jhi, int pslots, double* __restrict__ smag,
-                                                           double* __restrict__ part) {
+                                                           const double* __restrict__ w, int klo, int jlo, int jhi, int ly, int pslots,
+                                                           double* __restrict__ smag, double* __restrict__ part) {
   constexpr int LW = TXB + 2;                  // columns i0-2 .. i0+TXB-1 of a line
   constexpr int STAGE = DSMT_NL * LW;
   __shared__ __align__(128) double raw[DSMT_NS * STAGE];
@@ -226,8 +226,8 @@ __global__ void __launch_bounds__(TXB, MINB) k_dsm_col_tma(const __grid_constant
   __shared__ unsigned long long full[DSMT_NS];
   const int t = threadIdx.x, k = klo + blockIdx.y;
   const int i0 = blockIdx.x * (TXB - 2);
-  const int j0 = jlo + blockIdx.z * DSMC_LY;
-  const int jend = min(j0 + DSMC_LY, jhi);
+  const int j0 = jlo + blockIdx.z * ly;
+  const int jend = min(j0 + ly, jhi);
   const int nrows = jend - j0 + 2;             // base rows j0-1 .. jend; raw rows j0-2 .. jend+1 (nrows + 2 of them)
   const int nraw = nrows + 2;
   const int gi = i0 - 1 + t;
