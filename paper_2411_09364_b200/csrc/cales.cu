@@ -69,6 +69,7 @@ struct cales_solver {
   RhsMaps* rmaps; bool rmaps_ok;   // tensor maps of u, v, w, nu_t, p in device memory (workspace)
   bool nut_lazy, nut_valid; int graph_lazy;   // dynamic model: the momentum kernel forms nu_t from |S| and c_s (nut_lazy); s->nut holds it only when nut_valid
   int dsm_col_rows;     // option: output rows per CTA of the column march (0: chosen from the grid)
+  int rhs_kz;           // option: k-planes per CTA of the staged momentum kernel (0: rt_chunk)
   int lazy_nut;         // option: 1 (default) skips the |S| -> nu_t pass of the dynamic model
   int dsm_col_variant;  // 0: TMA-staged register-window column march (k_dsm_col_tma); 1: shared-ring form of round 1 (k_dsm_col_sm); 2: direct loads (k_dsm_col_rw)
   double cn_dt;   // dt the Crank-Nicolson tables on the device were built for (0: none, or a device-side dt)
@@ -256,7 +257,7 @@ extern "C" int cales_create(const cales_params* p, cales_solver** out) {
   s->tile_min = 4000000;
   s->rhs_tile_min = 200000;
   s->dsm_col_variant = 0;
-  s->nut_lazy = false; s->nut_valid = true; s->graph_lazy = -1; s->lazy_nut = 1; s->dsm_col_rows = 0;
+  s->nut_lazy = false; s->nut_valid = true; s->graph_lazy = -1; s->lazy_nut = 1; s->dsm_col_rows = 0; s->rhs_kz = 0;
   s->rhs_variant = 1;      // measured on B200 at config 5: cp.async ring 22.7 ms, tiled TMA ring 25.1 ms per launch
   {
     const double* fl[RT_NF] = {s->u, s->v, s->w, s->nut, s->p};
@@ -489,7 +490,7 @@ static int substep(cales_solver* s, int rk) {
   a.Ru0 = s->Ru; a.Rv0 = s->Rv; a.Rw0 = s->Rw; a.Ru1 = s->Ru; a.Rv1 = s->Rv; a.Rw1 = s->Rw;
   const double* sc = s->rks + rk * RK_STRIDE;      // dt, gamma dt, 1/(gamma dt), gamma nu dt / 2 of this substep, in device memory
   a.us = s->us; a.vs = s->vs; a.ws = s->ws; a.dt = 0.0; a.al = al; a.be = be; a.ga = ga; a.store_R = rk < 2 ? 1 : 0; a.sc = sc;
-  const int kz = rt_chunk(c.nx, c.ny, c.nz);
+  const int kz = s->rhs_kz > 0 ? s->rhs_kz : rt_chunk(c.nx, c.ny, c.nz);
   dim3 rgrid((c.nx + RT_TX - 1) / RT_TX, (c.ny + RT_TY - 1) / RT_TY, (c.nz + kz - 1) / kz);
   if (s->N >= s->rhs_tile_min && s->rhs_variant == 0 && s->rmaps_ok) k_rhs_tile_tma<<<rgrid, RT_THREADS, RT_SMEM_TMA_BYTES, s->st>>>(c, a, s->rmaps, kz, (cfr && !imp && !imp3) ? s->partial : nullptr);
   else if (s->N >= s->rhs_tile_min) k_rhs_tile<<<rgrid, RT_THREADS, RT_SMEM_DOUBLES * sizeof(double), s->st>>>(c, a, kz, (cfr && !imp && !imp3) ? s->partial : nullptr);
@@ -670,6 +671,7 @@ extern "C" int cales_set_option(cales_solver* s, const char* key, long long valu
     s->xB = L; s->x_threads = (int)th; s->x_smem = sm;
   }
   else if (k == "dsm_col_rows") { if (value < 0 || value > 4096) return fail(CALES_EINVAL, "dsm_col_rows must be 0..4096"); s->dsm_col_rows = (int)value; }
+  else if (k == "rhs_planes_per_cta") { if (value < 0 || value > 65535) return fail(CALES_EINVAL, "rhs_planes_per_cta out of range"); s->rhs_kz = (int)value; }
   else if (k == "lazy_nut") { if (value < 0 || value > 1) return fail(CALES_EINVAL, "lazy_nut must be 0 or 1"); s->lazy_nut = (int)value; }
   else if (k == "rhs_variant") { if (value < 0 || value > 1) return fail(CALES_EINVAL, "rhs_variant must be 0 or 1"); s->rhs_variant = (int)value; }
   else if (k == "dsm_col_variant") { if (value < 0 || value > 2) return fail(CALES_EINVAL, "dsm_col_variant must be 0, 1 or 2"); s->dsm_col_variant = (int)value; }
