@@ -72,6 +72,7 @@ struct cales_solver {
   int rhs_kz;           // option: k-planes per CTA of the staged momentum kernel (0: rt_chunk)
   int lazy_nut;         // option: 1 (default) skips the |S| -> nu_t pass of the dynamic model
   int dsm_col_variant;  // 0: TMA-staged register-window column march (k_dsm_col_tma); 1: shared-ring form of round 1 (k_dsm_col_sm); 2: direct loads (k_dsm_col_rw)
+  double rk_dt;   // dt the substep scalar blocks on the device hold (0: none, or a device-side dt)
   double cn_dt;   // dt the Crank-Nicolson tables on the device were built for (0: none, or a device-side dt)
   int use_graph; cudaGraphExec_t gexec;   // the three substeps captured as one CUDA graph (dt lives in device memory: one graph serves every dt)
   double* stats;   // [8 nz + 8 wall + 1 weight] accumulators, the same again as scratch
@@ -253,7 +254,7 @@ extern "C" int cales_create(const cales_params* p, cales_solver** out) {
   s->pgrid = dim3((nx + 31) / 32, (ny + 7) / 8, nz);
   s->fresh = false; s->timing = 0; s->ev_valid = false; s->launches = 0; s->evn = 0;
   s->use_graph = 1; s->gexec = nullptr; s->last_dt = 0.0;
-  s->cn_dt = 0.0;
+  s->cn_dt = 0.0; s->rk_dt = 0.0;
   s->tile_min = 4000000;
   s->rhs_tile_min = 200000;
   s->dsm_col_variant = 0;
@@ -584,8 +585,11 @@ static int run_substeps(cales_solver* s) {
 // dt-dependent device tables of a step: the substep scalar blocks and, with implicit z, the Crank-Nicolson tables of Eq. 21
 // (the forward elimination of the constant matrix is a serial recurrence over nz levels, one thread per substep).
 static int prepare_dt(cales_solver* s, double dt, const double* dt_dev) {
-  k_rk_scalars<<<1, 32, 0, s->st>>>(dt, dt_dev, s->c.nu, s->rks);
-  LAUNCH_TRY(K_CN_COEF);
+  if (dt_dev || dt != s->rk_dt) {      // the blocks persist in device memory: a repeated host-side dt costs nothing
+    k_rk_scalars<<<1, 32, 0, s->st>>>(dt, dt_dev, s->c.nu, s->rks);
+    LAUNCH_TRY(K_CN_COEF);
+    s->rk_dt = dt_dev ? 0.0 : dt;
+  }
   if (s->c.implicit_z == 1 && (dt_dev || dt != s->cn_dt)) {
     k_cn_coef<<<1, 32, 0, s->st>>>(s->c, s->rks, s->cncoef);
     LAUNCH_TRY(K_CN_COEF);
