@@ -249,6 +249,9 @@ def run_ours(args):
     stream = torch.cuda.Stream(device=local)
     torch.cuda.set_stream(stream)
     s = binding.Solver(g["nx"], g["ny"], g["nz"], g["lx"], g["ly"], g["lz"], device=local, stream=stream, **kw)
+    for kv in args.option:
+        key, val = kv.split("=")
+        s.set_option(key, int(val))
     s.set_velocity(u, v, w)
     s.project()                      # discretely solenoidal start, by the GPU solver itself
     for f, a in zip(range(3), (u, v, w)):
@@ -423,7 +426,8 @@ def run_ours(args):
                        "launch": "cales_step replays one CUDA graph per step" if not big else "plain stream launches (per-kernel events on)",
                        "l2": "L2 flushed between timed steps" if small else "state (%.1f GB) larger than L2" % (s.workspace_bytes / 1e9),
                        "options": {k: kw[k] for k in ("bc_y", "bc_z", "zstretch", "sgs_model", "wall_model", "implicit_z", "const_flow_rate",
-                                                      "dsm_avg_xy_plane", "dsm_clip_total", "van_driest")}},
+                                                      "dsm_avg_xy_plane", "dsm_clip_total", "van_driest")},
+                       "kernel_options": args.option or "defaults"},
             "step_hbm": {"algo_bytes_per_pt_step": SURVEY_STEP_BYTES[cfg_no], "achieved_gbs": survey_gbs, "frac_of_measured_peak": survey_gbs / peak,
                          "frac_of_8TBs": survey_gbs / 8000.0, "model": "SURVEY.md 8(d) bytes per point and step x points / measured step time",
                          "own_passes_bytes_per_pt_step": step_bytes / npts, "own_passes_frac_of_measured_peak": step_gbs / peak},
@@ -481,6 +485,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-other-configs", action="store_true", help="skip the short side runs of the other four workloads")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg")
+    ap.add_argument("--option", action="append", default=[], metavar="KEY=VALUE",
+                    help="cales_set_option knob for A/B timing (e.g. dsm_col_variant=2, rhs_variant=0, lazy_nut=0); repeatable")
     ap.add_argument("--dsm-filter3d", action="store_true", help="configs 4, 5 with the 3-D box test filter of PAPER.md:128 (SURVEY.md 8(f) item 2); "
                     "not a BASELINE.json workload: the line is labelled and is for the widening table of DESIGN.md only")
     args = ap.parse_args()

@@ -19,7 +19,13 @@
 
 namespace cales {
 
-enum { RT_TX = 32, RT_TY = 16, RT_RPT = 2, RT_TW = RT_TX + 2, RT_TH = RT_TY + 2, RT_PLANE = RT_TW * RT_TH, RT_NF = 5, RT_NSLOT = 4,
+#ifndef CALES_RT_TY
+#define CALES_RT_TY 16
+#endif
+#ifndef CALES_RT_MINB
+#define CALES_RT_MINB 2
+#endif
+enum { RT_TX = 32, RT_TY = CALES_RT_TY, RT_RPT = 2, RT_TW = RT_TX + 2, RT_TH = RT_TY + 2, RT_PLANE = RT_TW * RT_TH, RT_NF = 5, RT_NSLOT = 4,
        RT_THREADS = RT_TX * RT_TY / RT_RPT, RT_SMEM_DOUBLES = RT_NSLOT * RT_NF * RT_PLANE,
        RT_EPT = (RT_PLANE + RT_THREADS - 1) / RT_THREADS };   // halo-tile positions per thread
 
@@ -196,7 +202,7 @@ __global__ void __launch_bounds__(256) k_rhs_point(const __grid_constant__ Ctx c
 
 // grid (ceil(nx/RT_TX), ceil(ny/RT_TY), ceil(nz/kz)), block RT_THREADS, dynamic smem RT_SMEM_DOUBLES*8.
 // partial[linear block id] = sum over the CTA's points of u* dzf[k] (or nullptr).
-__global__ void __launch_bounds__(RT_THREADS, 2) k_rhs_tile(const __grid_constant__ Ctx c, const __grid_constant__ RhsArgs a, int kz,
+__global__ void __launch_bounds__(RT_THREADS, CALES_RT_MINB) k_rhs_tile(const __grid_constant__ Ctx c, const __grid_constant__ RhsArgs a, int kz,
                                                             double* __restrict__ partial) {
   extern __shared__ double rt_sm[];
   __shared__ double red[32];
