@@ -1234,3 +1234,61 @@ def test_wall_shear_statistics_wall_model_and_duct(oracle):
     assert abs(st["wall"][7] - np.sum(2 * nu * w[:, -1, :] / D.dy * wz) / 12) < 1e-13
     dzc_b = 2 * D.zc[0]
     assert abs(st["wall"][0] - np.mean(2 * nu * u[0] / dzc_b)) < 1e-13
+
+
+def np_pad_scalar(S, q, sgn):
+    """One ghost layer around a centred scalar: periodic wrap, or ghost = sgn x interior at walls (z, then x, then y)."""
+    P = S.params
+    q = np.concatenate([sgn * q[:1], q, sgn * q[-1:]], axis=0) if P["bc_z"] == 1 else np.concatenate([q[-1:], q, q[:1]], axis=0)
+    q = np.concatenate([q[:, :, -1:], q, q[:, :, :1]], axis=2)
+    return np.concatenate([sgn * q[:, :1], q, sgn * q[:, -1:]], axis=1) if P["bc_y"] == 1 else np.concatenate([q[:, -1:], q, q[:, :1]], axis=1)
+
+
+def np_sgs(S, u, v, w, nt):
+    """d_j(2 nu_t S_ij) of SURVEY.md O-step 4 with whole-array edge fluxes: edge viscosity = mean of the 4 surrounding centres
+    (reading S6), nu_t ghost = -interior at walls (reading S7), natural two-point edge derivatives."""
+    dx, dy = S.dx, S.dy
+    nz, ny, nx = S.shape
+    _, dzf, dzc = np_metrics(S)
+    if S.params["bc_z"] == 0:
+        dzc = np.full(nz + 1, dzf[0])
+    dzf_g = np.concatenate([dzf, dzf[-1:]])
+    U, V, W = np_pad_velocity(S, u, v, w)
+    N = np_pad_scalar(S, nt, -1.0)
+    ze = dzc[:, None, None]                                   # spacing across z edge K = 0..nz (between padded K and K+1)
+    exy = 0.25 * (N[:, :-1, :-1] + N[:, :-1, 1:] + N[:, 1:, :-1] + N[:, 1:, 1:]) * ((U[:, 1:, :-1] - U[:, :-1, :-1]) / dy + (V[:, :-1, 1:] - V[:, :-1, :-1]) / dx)
+    exz = 0.25 * (N[:-1, :, :-1] + N[:-1, :, 1:] + N[1:, :, :-1] + N[1:, :, 1:]) * ((U[1:, :, :-1] - U[:-1, :, :-1]) / ze + (W[:-1, :, 1:] - W[:-1, :, :-1]) / dx)
+    eyz = 0.25 * (N[:-1, :-1, :] + N[:-1, 1:, :] + N[1:, :-1, :] + N[1:, 1:, :]) * ((V[1:, :-1, :] - V[:-1, :-1, :]) / ze + (W[:-1, 1:, :] - W[:-1, :-1, :]) / dy)
+    I = (slice(1, -1),) * 3
+    k1, j1, i1 = slice(1, nz + 1), slice(1, ny + 1), slice(1, nx + 1)       # interior in padded coordinates / upper edges
+    k0, j0, i0 = slice(0, nz), slice(0, ny), slice(0, nx)                   # lower edges
+    f = dzf[:, None, None]
+    su = ((2 * N[k1, j1, 2:] * (U[k1, j1, 2:] - U[I]) - 2 * N[I] * (U[I] - U[k1, j1, :-2])) / dx ** 2
+          + (exy[k1, j1, i1] - exy[k1, j0, i1]) / dy + (exz[k1, j1, i1] - exz[k0, j1, i1]) / f)
+    sv = ((exy[k1, j1, i1] - exy[k1, j1, i0]) / dx
+          + (2 * N[k1, 2:, i1] * (V[k1, 2:, i1] - V[I]) - 2 * N[I] * (V[I] - V[k1, :-2, i1])) / dy ** 2
+          + (eyz[k1, j1, i1] - eyz[k0, j1, i1]) / f)
+    sw = ((exz[k1, j1, i1] - exz[k1, j1, i0]) / dx + (eyz[k1, j1, i1] - eyz[k1, j0, i1]) / dy
+          + (2 * N[2:, j1, i1] * (W[2:, j1, i1] - W[I]) / dzf_g[1:, None, None] - 2 * N[I] * (W[I] - W[:-2, j1, i1]) / f) / dzc[1:, None, None])
+    if S.params["bc_y"] == 1:
+        sv[:, -1, :] = 0.0
+    if S.params["bc_z"] == 1:
+        sw[-1] = 0.0
+    return su, sv, sw
+
+
+@pytest.mark.parametrize("bcs,stretch", CASES)
+def test_sgs_term_vs_numpy_stencil(oracle, bcs, stretch):
+    """Every coefficient of d_j(2 nu_t S_ij) with a random, non-constant nu_t on every BC combination, uniform and tanh z."""
+    S = make(oracle, 12, 8, 10, bcs, stretch, sgs_model=1)
+    rng = np.random.default_rng(29)
+    u, v, w = (rng.standard_normal(S.shape) for _ in range(3))
+    if bcs[1] == 1:
+        w[-1] = 0.0
+    if bcs[0] == 1:
+        v[:, -1, :] = 0.0
+    nt = rng.random(S.shape) + 0.1
+    S.set_velocity(u, v, w)
+    S.set(S.NUT, nt)
+    for g, e in zip(S.sgs_term(), np_sgs(S, u, v, w, nt)):
+        assert np.max(np.abs(g - e)) < 1e-12 * np.max(np.abs(e))
