@@ -130,6 +130,15 @@ CALES_HD double ld_scalar(const double* p) {
 #endif
 }
 
+// two adjacent scalars (16-byte aligned) in one load
+CALES_HD void ld_scalar2(const double* p, double& a, double& b) {
+#ifdef __CUDA_ARCH__
+  asm("ld.global.nc.L1::evict_last.v2.f64 {%0, %1}, [%2];" : "=d"(a), "=d"(b) : "l"(p));
+#else
+  a = p[0]; b = p[1];
+#endif
+}
+
 // RK3 coefficients of PAPER.md:100.
 CALES_HD void rk3_coeffs(int rk, double& al, double& be, double& ga) {
   al = rk == 0 ? 8.0 / 15.0 : (rk == 1 ? 5.0 / 12.0 : 3.0 / 4.0);

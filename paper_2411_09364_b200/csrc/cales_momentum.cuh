@@ -47,9 +47,10 @@ template <bool IMP3 = true>
 CALES_HD void correct_point(const Ctx& c, const CorrArgs& a, int i, int j, int k) {
   const long long n = idx3(c, i, j, k);
   // the substep scalars first: a load placed after the stores below could not be moved above them (possible aliasing)
-  const double gdt = a.sc ? ld_scalar(a.sc + RK_GDT) : a.gdt;
+  double gdt, sh = 0.0;
+  if (a.sc && a.shift) ld_scalar2(a.shift + 4, sh, gdt);      // k_bulk_finish leaves (shift, gamma dt) side by side: one load
+  else { gdt = a.sc ? ld_scalar(a.sc + RK_GDT) : a.gdt; if (a.shift) sh = ld_scalar(a.shift); }
   const double cimp = (a.sc && a.cimp != 0.0) ? ld_scalar(a.sc + RK_CIMP) : a.cimp;
-  const double sh = a.shift ? ld_scalar(a.shift) : 0.0;
   const double ph = a.phi[n];
   double phx, phy, phz, phm = 0.0;
   if (interior_row(c, j, k)) {
@@ -101,7 +102,8 @@ __global__ void k_sum_stage1(const double* __restrict__ in, long long n, double*
   const double t = block_sum(s, sh);
   if (threadIdx.x == 0) out1[blockIdx.x] = t;
 }
-// scal[0] = shift = u_bulk - sum/(nx ny lz); scal[1] = forcing = shift / (gamma dt); scal[2] = mean
+// scal[0] = shift = u_bulk - sum/(nx ny lz); scal[1] = forcing = shift / (gamma dt); scal[2] = mean; scal[4], scal[5] = (shift, gamma dt)
+// side by side for the correction kernel
 __global__ void k_rk_scalars(double dt, const double* __restrict__ dt_dev, double nu, double* __restrict__ sc) {
   if (threadIdx.x < 3) rk_scalars(threadIdx.x, dt_dev ? *dt_dev : dt, nu, sc + threadIdx.x * RK_STRIDE);
 }
@@ -113,7 +115,8 @@ __global__ void k_bulk_finish(Ctx c, const double* __restrict__ in, int n, doubl
   if (threadIdx.x == 0) {
     const double m = t / ((double)c.nx * (double)c.ny * c.lz);
     const double shf = c.u_bulk - m;
-    scal[0] = shf; scal[1] = shf / (sc ? sc[RK_GDT] : gdt); scal[2] = m;
+    const double g = sc ? sc[RK_GDT] : gdt;
+    scal[0] = shf; scal[1] = shf / g; scal[2] = m; scal[4] = shf; scal[5] = g;
   }
 }
 // diagnostics: per-block partials of max|div|, sum u dzf, sum ke dzf, non-finite count
