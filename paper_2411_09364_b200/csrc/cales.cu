@@ -69,6 +69,7 @@ struct cales_solver {
   RhsMaps* rmaps; bool rmaps_ok;   // tensor maps of u, v, w, nu_t, p in device memory (workspace)
   bool nut_lazy, nut_valid; int graph_lazy;   // dynamic model: the momentum kernel forms nu_t from |S| and c_s (nut_lazy); s->nut holds it only when nut_valid
   int dsm_col_rows;     // option: output rows per CTA of the column march (0: chosen from the grid)
+  int fft_stage;        // option: 1 (default) stages the lines of the inverse x transform in shared memory by bulk copies
   int rhs_kz;           // option: k-planes per CTA of the staged momentum kernel (0: rt_chunk)
   int lazy_nut;         // option: 1 (default) skips the |S| -> nu_t pass of the dynamic model
   int dsm_col_variant;  // 0: TMA-staged register-window column march (k_dsm_col_tma); 1: shared-ring form of round 1 (k_dsm_col_sm); 2: direct loads (k_dsm_col_rw)
@@ -258,7 +259,7 @@ extern "C" int cales_create(const cales_params* p, cales_solver** out) {
   s->tile_min = 4000000;
   s->rhs_tile_min = 200000;
   s->dsm_col_variant = 0;
-  s->nut_lazy = false; s->nut_valid = true; s->graph_lazy = -1; s->lazy_nut = 1; s->dsm_col_rows = 0; s->rhs_kz = 0;
+  s->nut_lazy = false; s->nut_valid = true; s->graph_lazy = -1; s->lazy_nut = 1; s->dsm_col_rows = 0; s->rhs_kz = 0; s->fft_stage = 1;
   s->rhs_variant = 1;      // measured on B200 at config 5: cp.async ring 22.7 ms, tiled TMA ring 25.1 ms per launch
   {
     const double* fl[RT_NF] = {s->u, s->v, s->w, s->nut, s->p};
@@ -328,21 +329,23 @@ extern "C" int cales_get_field(cales_solver* s, int field, double* dst, int on_d
 static int run_transform_x_fwd(cales_solver* s, const double* src, const DivSrc* ds, double* dst) {
   const long long nlines = (long long)s->c.ny * s->c.nz;
   const unsigned grid = (unsigned)((nlines + s->xB - 1) / s->xB);
-  if (ds) k_fft2_x_fwd<true><<<grid, s->x_threads, s->x_smem, s->st>>>(s->c, s->plx, s->xB, nullptr, *ds, dst);
-  else { DivSrc z{nullptr, nullptr, nullptr, 0.0, nullptr}; k_fft2_x_fwd<false><<<grid, s->x_threads, s->x_smem, s->st>>>(s->c, s->plx, s->xB, src, z, dst); }
+  if (ds) k_fft2_x_fwd<true><<<grid, s->x_threads, s->x_smem, s->st>>>(s->c, s->plx, s->xB, nullptr, *ds, dst, (s->fft_stage && s->plx.npass > 0) ? 1 : 0);
+  else { DivSrc z{nullptr, nullptr, nullptr, 0.0, nullptr}; k_fft2_x_fwd<false><<<grid, s->x_threads, s->x_smem, s->st>>>(s->c, s->plx, s->xB, src, z, dst, 0); }
   LAUNCH_TRY(K_FFTX_FWD);
   return CALES_OK;
 }
 static int run_transform_x_inv(cales_solver* s, const double* src, double* dst) {
   const long long nlines = (long long)s->c.ny * s->c.nz;
   const unsigned grid = (unsigned)((nlines + s->xB - 1) / s->xB);
-  k_fft2_x_inv<<<grid, s->x_threads, s->x_smem, s->st>>>(s->c, s->plx, s->xB, src, dst);
+  const int staged = s->fft_stage && (((size_t)src) & 15) == 0 && s->plx.npass > 0;
+  k_fft2_x_inv<<<grid, s->x_threads, s->x_smem, s->st>>>(s->c, s->plx, s->xB, src, dst, staged);
   LAUNCH_TRY(K_FFTX_INV);
   return CALES_OK;
 }
 static int run_transform_y(cales_solver* s, double* A, int inverse) {
   dim3 grid((s->c.nx + s->yTI - 1) / s->yTI, s->c.nz);
-  k_fft2_y<<<grid, s->y_threads, s->y_smem, s->st>>>(s->c, s->ply, s->y_tish, s->c.bc_y == BC_WALL ? 1 : 0, inverse, A);
+  const int staged = s->fft_stage && inverse && (((size_t)A) & 15) == 0 && s->ply.npass > 0 && (size_t)s->c.ny * s->yTI * 8 <= s->y_smem;
+  k_fft2_y<<<grid, s->y_threads, s->y_smem, s->st>>>(s->c, s->ply, s->y_tish, s->c.bc_y == BC_WALL ? 1 : 0, inverse, A, staged);
   LAUNCH_TRY(inverse ? K_FFTY_INV : K_FFTY_FWD);
   return CALES_OK;
 }
@@ -676,6 +679,7 @@ extern "C" int cales_set_option(cales_solver* s, const char* key, long long valu
   }
   else if (k == "dsm_col_rows") { if (value < 0 || value > 4096) return fail(CALES_EINVAL, "dsm_col_rows must be 0..4096"); s->dsm_col_rows = (int)value; }
   else if (k == "rhs_planes_per_cta") { if (value < 0 || value > 65535) return fail(CALES_EINVAL, "rhs_planes_per_cta out of range"); s->rhs_kz = (int)value; }
+  else if (k == "fft_stage") { if (value < 0 || value > 1) return fail(CALES_EINVAL, "fft_stage must be 0 or 1"); s->fft_stage = (int)value; }
   else if (k == "lazy_nut") { if (value < 0 || value > 1) return fail(CALES_EINVAL, "lazy_nut must be 0 or 1"); s->lazy_nut = (int)value; }
   else if (k == "rhs_variant") { if (value < 0 || value > 1) return fail(CALES_EINVAL, "rhs_variant must be 0 or 1"); s->rhs_variant = (int)value; }
   else if (k == "dsm_col_variant") { if (value < 0 || value > 2) return fail(CALES_EINVAL, "dsm_col_variant must be 0, 1 or 2"); s->dsm_col_variant = (int)value; }

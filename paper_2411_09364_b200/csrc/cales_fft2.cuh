@@ -152,6 +152,11 @@ struct F2XFwdLd {
                         ((uu.y - uu.x) * rdx + (vv.y - vvm.y) * rdy + (ww.y - wwm.y) * rdz) * inv);
   }
 };
+// forward from lines staged in shared memory: packed complex element t of line b at buf[b * ls + t]
+struct F2XFwdLdS {
+  int nb; const double2* buf; int ls;
+  CALES_HD double2 operator()(int b, int t) const { return b < nb ? buf[b * ls + t] : make_double2(0.0, 0.0); }
+};
 // inverse: Z[t] merged on the fly from the packed half-complex line (h[0] = X0, h[1] = X_{n/2}, h[2m], h[2m+1] = X_m)
 struct F2XInvLd {
   const FftPlan& pl; long long l0; int nb; const double* src;
@@ -163,6 +168,20 @@ struct F2XInvLd {
   CALES_HD double2 operator()(int b, int t) const {
     if (b >= nb) return make_double2(0.0, 0.0);
     const double* h = src + (l0 + b) * pl.n;
+    return f2_merge(pl, t, mode(h, t), mode(h, pl.n2 - t));
+  }
+};
+// the same from lines staged in shared memory (raw packed layout, `stride` doubles between lines)
+struct F2XInvLdS {
+  const FftPlan& pl; int nb; const double* base; int stride;
+  CALES_HD double2 mode(const double* h, int m) const {
+    if (m == 0) return make_double2(h[0], 0.0);
+    if (m == pl.n2) return make_double2(h[1], 0.0);
+    return ld2(h, m);
+  }
+  CALES_HD double2 operator()(int b, int t) const {
+    if (b >= nb) return make_double2(0.0, 0.0);
+    const double* h = base + b * stride;
     return f2_merge(pl, t, mode(h, t), mode(h, pl.n2 - t));
   }
 };
@@ -185,6 +204,20 @@ struct F2YInvLd {
   const Ctx& c; const FftPlan& pl; const double* base; int nb; bool dct;
   CALES_HD double row(int r, int b) const { return base[(long long)r * c.nx + b]; }
   CALES_HD double2 mode(int m, int b) const {      // X[m] (FFT rows) or V[m] (DCT rows), see hc_mode
+    if (m == 0) return make_double2(row(0, b), 0.0);
+    if (!dct) return m == pl.n2 ? make_double2(row(1, b), 0.0) : make_double2(row(2 * m, b), row(2 * m + 1, b));
+    return cmulc(make_double2(row(m, b), -row(pl.n - m, b)), pl.dctw[m]);
+  }
+  CALES_HD double2 operator()(int b, int t) const {
+    if (b >= nb) return make_double2(0.0, 0.0);
+    return f2_merge(pl, t, mode(t, b), mode(pl.n2 - t, b));
+  }
+};
+// the same from a tile staged in shared memory (row r, column b at base[r * rs + b])
+struct F2YInvLdS {
+  const FftPlan& pl; const double* base; int rs; int nb; bool dct;
+  CALES_HD double row(int r, int b) const { return base[r * rs + b]; }
+  CALES_HD double2 mode(int m, int b) const {
     if (m == 0) return make_double2(row(0, b), 0.0);
     if (!dct) return m == pl.n2 ? make_double2(row(1, b), 0.0) : make_double2(row(2 * m, b), row(2 * m + 1, b));
     return cmulc(make_double2(row(m, b), -row(pl.n - m, b)), pl.dctw[m]);
@@ -245,29 +278,88 @@ __device__ __forceinline__ void f2_passes(const Fft2Lay& lay, const FftPlan& pl,
   }
 }
 
+// staged != 0 (DIV only): the divergence of u* / (gamma dt) of the CTA's lines is first formed into the line slots by a pre-pass whose
+// loads are batched four elements deep (24 independent loads in flight per thread) instead of one load -> use chain per element inside
+// the first butterfly pass; that pass then reads shared memory.
 template <bool DIV>
 __global__ void __launch_bounds__(512) k_fft2_x_fwd(const __grid_constant__ Ctx c, const __grid_constant__ FftPlan pl, int L, const double* __restrict__ src,
-                                                       DivSrc ds, double* __restrict__ dst) {
+                                                       DivSrc ds, double* __restrict__ dst, int staged) {
   extern __shared__ double2 f2_sm[];
   const Fft2Lay lay{L, sm_line(pl.n2), 0, false};
   const long long nlines = (long long)c.ny * c.nz, l0 = (long long)blockIdx.x * L;
   const int nb = (int)min((long long)L, nlines - l0);
-  F2XFwdLd first{c, pl, l0, nb, src, ds, DIV, DIV ? (ds.sc ? ds.sc[2] : ds.inv_gdt) : 0.0};
-  f2_passes<false>(lay, pl, -1, f2_sm, first, F2SmemSt{f2_sm, lay});
+  if (DIV && staged) {
+    const int n = pl.n, n2 = pl.n2, nth = blockDim.x;
+    const double inv = ds.sc ? ds.sc[2] : ds.inv_gdt, rdx = c.rdx, rdy = c.rdy;
+    enum { UB = 4 };
+    for (int b = 0; b < nb; ++b) {
+      const long long l = l0 + b;
+      const int k = (int)((unsigned)l / (unsigned)c.ny), j = (int)l - k * c.ny;
+      const double* ul = ds.us + l * n; const double* vl = ds.vs + l * n; const double* wl = ds.ws + l * n;
+      const double* vm = nullptr; const double* wm = nullptr;          // v(j-1), w(k-1): ghosts of u*
+      if (j > 0) vm = vl - n; else if (c.bc_y == BC_PER) vm = vl + (long long)(c.ny - 1) * n;
+      if (k > 0) wm = wl - c.nxy; else if (c.bc_z == BC_PER) wm = wl + (long long)(c.nz - 1) * c.nxy;
+      const double rdz = c.rdzf[k];
+      double2* out = f2_sm + b * lay.ls;
+      for (int t0 = threadIdx.x; t0 < n2; t0 += UB * nth) {
+        double2 uu[UB], vv[UB], ww[UB], vvm[UB], wwm[UB]; double um[UB];
+#pragma unroll
+        for (int q = 0; q < UB; ++q) {
+          const int t = t0 + q * nth;
+          if (t < n2) {
+            uu[q] = ld2(ul, t); um[q] = ul[t == 0 ? n - 1 : 2 * t - 1]; vv[q] = ld2(vl, t); ww[q] = ld2(wl, t);
+            vvm[q] = vm ? ld2(vm, t) : make_double2(0.0, 0.0); wwm[q] = wm ? ld2(wm, t) : make_double2(0.0, 0.0);
+          }
+        }
+#pragma unroll
+        for (int q = 0; q < UB; ++q) {
+          const int t = t0 + q * nth;
+          if (t < n2) out[t] = make_double2(((uu[q].x - um[q]) * rdx + (vv[q].x - vvm[q].x) * rdy + (ww[q].x - wwm[q].x) * rdz) * inv,
+                                            ((uu[q].y - uu[q].x) * rdx + (vv[q].y - vvm[q].y) * rdy + (ww[q].y - wwm[q].y) * rdz) * inv);
+        }
+      }
+    }
+    __syncthreads();
+    F2XFwdLdS first{nb, f2_sm, lay.ls};
+    f2_passes<false>(lay, pl, -1, f2_sm, first, F2SmemSt{f2_sm, lay});
+  } else {
+    F2XFwdLd first{c, pl, l0, nb, src, ds, DIV, DIV ? (ds.sc ? ds.sc[2] : ds.inv_gdt) : 0.0};
+    f2_passes<false>(lay, pl, -1, f2_sm, first, F2SmemSt{f2_sm, lay});
+  }
   f2x_split_store(threadIdx.x, blockDim.x, pl, lay, l0, nb, f2_sm, dst);
 }
+// staged != 0: the CTA's packed lines are first brought into their shared-memory line slots by one cp.async.bulk copy each (whole
+// lines are contiguous; 16-byte aligned because n is even), so the merge of the first pass reads shared memory.  ncu on the direct
+// form (profiles/r2_ncu_full.md): 45 % of all stall samples sat on the sixteen load -> merge dependencies of that pass, one global
+// latency each; the transforms run at the same rate on L2-resident data, i.e. they were never DRAM-bound.
 __global__ void __launch_bounds__(512) k_fft2_x_inv(const __grid_constant__ Ctx c, const __grid_constant__ FftPlan pl, int L, const double* __restrict__ src,
-                                                       double* __restrict__ dst) {
+                                                       double* __restrict__ dst, int staged) {
   extern __shared__ double2 f2_sm[];
+  __shared__ unsigned long long bar;
   const Fft2Lay lay{L, sm_line(pl.n2), 0, false};
   const long long nlines = (long long)c.ny * c.nz, l0 = (long long)blockIdx.x * L;
   const int nb = (int)min((long long)L, nlines - l0);
-  F2XInvLd first{pl, l0, nb, src};
   F2XInvSt last{pl, l0, nb, dst, 1.0 / (double)pl.n2};
-  f2_passes<true>(lay, pl, +1, f2_sm, first, last);
+  if (staged) {
+    if (threadIdx.x == 0) { mbar_init(&bar, 1); mbar_fence_init(); }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      mbar_expect_tx(&bar, (unsigned)nb * (unsigned)pl.n * 8u);
+      for (int b = 0; b < nb; ++b) bulk_g2s(f2_sm + b * lay.ls, src + (l0 + b) * pl.n, (unsigned)pl.n * 8u, &bar);
+    }
+    mbar_wait(&bar, 0);
+    F2XInvLdS first{pl, nb, reinterpret_cast<const double*>(f2_sm), 2 * lay.ls};
+    f2_passes<true>(lay, pl, +1, f2_sm, first, last);
+  } else {
+    F2XInvLd first{pl, l0, nb, src};
+    f2_passes<true>(lay, pl, +1, f2_sm, first, last);
+  }
 }
 // grid (ceil(nx/TI), nz); in place on A
-__global__ void __launch_bounds__(512) k_fft2_y(const __grid_constant__ Ctx c, const __grid_constant__ FftPlan pl, int tish, int dct, int inverse, double* __restrict__ A) {
+// staged != 0 (inverse only): the raw [ny x TI] tile is first copied into the (equally large) shared buffer by batched, dependency-free
+// loads, and the merge of the first pass reads shared memory -- same reason as in k_fft2_x_inv.
+__global__ void __launch_bounds__(512) k_fft2_y(const __grid_constant__ Ctx c, const __grid_constant__ FftPlan pl, int tish, int dct, int inverse, double* __restrict__ A,
+                                                   int staged) {
   extern __shared__ double2 f2_sm[];
   const int TI = 1 << tish;
   const Fft2Lay lay{TI, 0, tish, true};
@@ -278,6 +370,23 @@ __global__ void __launch_bounds__(512) k_fft2_y(const __grid_constant__ Ctx c, c
     F2YFwdLd first{c, pl, base, nb, dct != 0};
     f2_passes<false>(lay, pl, -1, f2_sm, first, F2SmemSt{f2_sm, lay});
     f2y_split_store(threadIdx.x, blockDim.x, c, pl, lay, dct != 0, base, nb, f2_sm);
+  } else if (staged && nb == TI && TI >= 2) {
+    F2YInvSt last{c, pl, base, nb, dct != 0, 1.0 / (double)pl.n2};
+    const int hsh = tish - 1, total = pl.n << hsh;            // double2 elements of the tile: ny rows of TI/2
+    enum { UB = 8 };
+    for (int i0b = threadIdx.x; i0b < total; i0b += UB * blockDim.x) {
+      double2 tmp[UB];
+#pragma unroll
+      for (int q = 0; q < UB; ++q) {
+        const int idx = i0b + q * blockDim.x;
+        if (idx < total) { const int r = idx >> hsh, cq = idx & ((1 << hsh) - 1); tmp[q] = *reinterpret_cast<const double2*>(base + (long long)r * c.nx + 2 * cq); }
+      }
+#pragma unroll
+      for (int q = 0; q < UB; ++q) { const int idx = i0b + q * blockDim.x; if (idx < total) f2_sm[idx] = tmp[q]; }
+    }
+    __syncthreads();
+    F2YInvLdS first{pl, reinterpret_cast<const double*>(f2_sm), TI, nb, dct != 0};
+    f2_passes<true>(lay, pl, +1, f2_sm, first, last);
   } else {
     F2YInvLd first{c, pl, base, nb, dct != 0};
     F2YInvSt last{c, pl, base, nb, dct != 0, 1.0 / (double)pl.n2};
