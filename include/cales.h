@@ -167,6 +167,19 @@ int cales_project(cales_solver* s);
  * HOST output; synchronises the stream. */
 int cales_cfl_dt(cales_solver* s, double cfl, double* dt_host);
 
+/* Allocation-free variant of the CFL reduction, for callers that cannot allocate (CUDA graph capture, serving loops): the same
+ * reduction as cales_cfl_dt (reading S18), its scratch in a file-scope device array of
+ * CALES_STATIC_SCRATCH_BYTES that every GPU loading the library holds until exit, not in the workspace.  No cudaMalloc, cudaFree
+ * or allocating library call, no host synchronisation.  u, v, w: DEVICE fields nz*ny*nx, or all NULL = the solver's own velocity;
+ * dt_dev: DEVICE output, one double = cfl / max rate (0 for a field at rest).  The grid may have at most
+ * CALES_STATIC_SCRATCH_BLOCKS blocks of 32 x 8 points per plane (ceil(nx/32) * ceil(ny/8) * nz), CALES_EINVAL with a message
+ * otherwise.  All calls on a device share the array (solvers and streams alike): calls that overlap on the GPU race; it keeps the
+ * last call's contents and no slot needs clearing (every slot a call reads it has written first).  Asynchronous on the solver's
+ * stream. */
+#define CALES_STATIC_SCRATCH_BLOCKS (1 << 20)
+#define CALES_STATIC_SCRATCH_BYTES (8 * (CALES_STATIC_SCRATCH_BLOCKS + 1024))
+int cales_cfl_dt_static(cales_solver* s, const double* u, const double* v, const double* w, double cfl, double* dt_dev);
+
 /* On-line statistics: x-y plane means per k of the centre-averaged u, v, w, uu, vv, ww, uw and of nu_t.
  * out_dev: DEVICE, [8][nz].  Asynchronous. */
 int cales_plane_stats(cales_solver* s, double* out_dev);

@@ -39,7 +39,7 @@ class CalesDiag(C.Structure):
 # every symbol include/cales.h declares
 SYMBOLS = ["cales_default_params", "cales_workspace_bytes", "cales_create", "cales_create_basic", "cales_destroy",
            "cales_set_field", "cales_get_field", "cales_step", "cales_step_adaptive", "cales_last_dt", "cales_poisson_solve", "cales_eddy_viscosity",
-           "cales_wall_stress", "cales_wall_stress_y", "cales_project", "cales_cfl_dt", "cales_plane_stats", "cales_stats_reset", "cales_stats_accumulate", "cales_stats_get", "cales_get_cs", "cales_transform", "cales_transpose_xy",
+           "cales_wall_stress", "cales_wall_stress_y", "cales_project", "cales_cfl_dt", "cales_cfl_dt_static", "cales_plane_stats", "cales_stats_reset", "cales_stats_accumulate", "cales_stats_get", "cales_get_cs", "cales_transform", "cales_transpose_xy",
            "cales_set_timing", "cales_set_graph", "cales_set_option", "cales_fp64_peak", "cales_kernel_count", "cales_kernel_time", "cales_launches_per_step", "cales_diagnostics", "cales_last_error"]
 
 _lib = None
@@ -71,6 +71,7 @@ def lib():
         L.cales_project.argtypes = [C.c_void_p]
         L.cales_get_cs.argtypes = [C.c_void_p, C.c_void_p]
         L.cales_cfl_dt.argtypes = [C.c_void_p, C.c_double, C.POINTER(C.c_double)]
+        L.cales_cfl_dt_static.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_double, C.c_void_p]
         L.cales_plane_stats.argtypes = [C.c_void_p, C.c_void_p]
         L.cales_stats_reset.argtypes = [C.c_void_p]
         L.cales_stats_accumulate.argtypes = [C.c_void_p, C.c_double]
@@ -244,6 +245,12 @@ class Solver:
         dt = C.c_double()
         _chk(lib().cales_cfl_dt(self._h, float(cfl), C.byref(dt)))
         return dt.value
+
+    def cfl_dt_static(self, cfl, dt_dev, u=None, v=None, w=None):
+        """Allocation-free CFL reduction into the 1-element DEVICE tensor dt_dev (scratch in the library's static device array)."""
+        f = [None if a is None else self._dev(a) for a in (u, v, w)]
+        _chk(lib().cales_cfl_dt_static(self._h, f[0], f[1], f[2], float(cfl), C.c_void_p(dt_dev.data_ptr())))
+        return dt_dev
 
     def plane_stats(self):
         out = self._torch.empty((8, self.nz), dtype=self._torch.float64, device=self.device)

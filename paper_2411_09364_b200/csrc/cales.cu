@@ -31,6 +31,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -194,6 +195,7 @@ static bool make_field_map(CUtensorMap* m, const double* base, int nx, int ny, i
              CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+static int static_scratch_ptr(int device, double** out);
 extern "C" int cales_create(const cales_params* p, cales_solver** out) {
   if (!out) return fail(CALES_EINVAL, "null output pointer");
   *out = nullptr;
@@ -269,6 +271,7 @@ extern "C" int cales_create(const cales_params* p, cales_solver** out) {
     if (s->rmaps_ok && (cudaMemcpyAsync(s->rmaps, &hm, sizeof(hm), cudaMemcpyHostToDevice, s->st) != cudaSuccess || cudaStreamSynchronize(s->st) != cudaSuccess)) { cudaGetLastError(); s->rmaps_ok = false; }
   }
   for (int q = 0; q < 32; ++q) { s->kms[q] = 0.0; s->kcnt[q] = 0; }
+  { double* ss_ = nullptr; (void)static_scratch_ptr(s->device, &ss_); }      // set-up of cales_cfl_dt_static; a failure is reported by that call
   *out = s;
   return CALES_OK;
 }
@@ -784,6 +787,50 @@ extern "C" int cales_cfl_dt(cales_solver* s, double cfl, double* dt_host) {
   double r = 0.0; for (int q = 0; q < g1; ++q) r = std::fmax(r, h[q]);
   *dt_host = r > 0.0 ? cfl / r : 0.0;
   return CALES_OK;
+}
+
+// ---- allocation-free entry point ---------------------------------------------------------------------------------------------
+// cales_cfl_dt_static: the CFL reduction of cales_cfl_dt with its scratch (per-block maxima, first-stage maxima) in a file-scope
+// device array instead of the solver's workspace.  The array's name is a host-side stand-in in host code, not a device address:
+// static_scratch_ptr() resolves the address once per device (cudaGetSymbolAddress with that device current) and the kernels get
+// that pointer.  Every GPU that loads the library holds CALES_STATIC_SCRATCH_BYTES until exit.
+enum { STATIC_BLOCKS = CALES_STATIC_SCRATCH_BLOCKS, STATIC_STAGE = 1024, STATIC_MAX_DEVICES = 64 };
+static __device__ __align__(256) double g_static_scratch[STATIC_BLOCKS + STATIC_STAGE];
+static_assert(sizeof(double) * (STATIC_BLOCKS + STATIC_STAGE) == CALES_STATIC_SCRATCH_BYTES, "header and array disagree");
+
+static int static_scratch_ptr(int device, double** out) {
+  static std::mutex mu;
+  static double* ptr[STATIC_MAX_DEVICES] = {};
+  if (device < 0 || device >= STATIC_MAX_DEVICES) return fail(CALES_EINVAL, "device index beyond the static scratch table");
+  std::lock_guard<std::mutex> lk(mu);
+  if (!ptr[device]) {      // the caller's DevGuard has made `device` current
+    double* d = nullptr;
+    CUDA_TRY(cudaGetSymbolAddress((void**)&d, g_static_scratch));
+    ptr[device] = d;
+  }
+  *out = ptr[device];
+  return CALES_OK;
+}
+
+extern "C" int cales_cfl_dt_static(cales_solver* s, const double* u, const double* v, const double* w, double cfl, double* dt_dev) {
+  DevGuard dg_(s ? s->device : -1);
+  if (!s || !dt_dev || !(cfl > 0.0)) return fail(CALES_EINVAL, "bad cfl_dt_static arguments");
+  const bool own = !u && !v && !w;
+  if (!own && (!u || !v || !w)) return fail(CALES_EINVAL, "cfl_dt_static: pass all of u, v, w or none");
+  if (s->nblk > (long long)STATIC_BLOCKS)
+    return fail(CALES_EINVAL, "cfl_dt_static: grid needs " + std::to_string(s->nblk) + " scratch slots (one per 32 x 8 points of a plane), the static array holds " +
+                                  std::to_string((long long)STATIC_BLOCKS) + "; use cales_cfl_dt");
+  double* part = nullptr;
+  { int rc = static_scratch_ptr(s->device, &part); if (rc) return rc; }
+  double* stage = part + STATIC_BLOCKS;
+  TimingOff toff(s);
+  // every slot read below is written first by this call: nothing has to start at zero
+  k_cfl_rate<<<s->pgrid, s->pblock, 0, s->st>>>(s->c, own ? s->u : u, own ? s->v : v, own ? s->w : w, part);
+  LAUNCH_TRY(K_DIAG);
+  const long long nb = s->nblk; const int g1 = (int)(nb < STATIC_STAGE ? nb : STATIC_STAGE);
+  k_max_stage<<<g1, 256, 0, s->st>>>(part, nb, stage); LAUNCH_TRY(K_SUM);
+  k_dt_finish<<<1, 256, 0, s->st>>>(stage, g1, cfl, dt_dev);
+  return check_launch(s, K_SUM);
 }
 
 // x-y plane means of u, v, w, uu, vv, ww, uw (centre-averaged) and nu_t: out_dev DEVICE [8][nz] (PAPER.md:237 profiles)
