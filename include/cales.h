@@ -235,7 +235,10 @@ int cales_fp64_peak(cales_solver* s, double* tflops_host);
  * the plane and cales_get_field(CALES_NUT) / the statistics materialise it on demand; 0: nu_t is written after every evaluation),
  * "rhs_variant" (staged momentum kernel -- 1 (default): halo planes moved by 8-byte cp.async, 0: by tiled TMA copies),
  * "dsm_col_variant" (column march of the dynamic model -- 0: register window, rows staged by TMA bulk copies; 1: the
- * shared-memory-ring form; 2: register window, direct loads).
+ * shared-memory-ring form; 2: register window, direct loads),
+ * "fft_stage" (1 (default): the first passes of the inverse transforms and the divergence of the forward x transform read shared
+ * memory staged by bulk copies / batched loads; 0: they read global memory directly), "poisson_cp_table" (walls in z -- 1 (default):
+ * the Thomas solve of the Poisson solver reads c' from a table built once at create; 0: it recomputes and spills c' on every solve).
  * CALES_EINVAL on an unknown key or a value out of range. */
 int cales_set_option(cales_solver* s, const char* key, long long value);
 

@@ -70,6 +70,7 @@ struct cales_solver {
   RhsMaps* rmaps; bool rmaps_ok;   // tensor maps of u, v, w, nu_t, p in device memory (workspace)
   bool nut_lazy, nut_valid; int graph_lazy;   // dynamic model: the momentum kernel forms nu_t from |S| and c_s (nut_lazy); s->nut holds it only when nut_valid
   int dsm_col_rows;     // option: output rows per CTA of the column march (0: chosen from the grid)
+  double* CPT; int cpt_on;      // static c' table of k_poisson_z (walls in z), option poisson_cp_table
   int fft_stage;        // option: 1 (default) stages the lines of the inverse x transform in shared memory by bulk copies
   int rhs_kz;           // option: k-planes per CTA of the staged momentum kernel (0: rt_chunk)
   int lazy_nut;         // option: 1 (default) skips the |S| -> nu_t pass of the dynamic model
@@ -113,6 +114,7 @@ static size_t carve(cales_solver* s, const cales_params* p, double* base) {
   for (int q = 0; q < 12; ++q) f[q] = take(N);
   double* CP = take(N);
   double* CQ = p->bc_z == CALES_BC_PERIODIC ? take(N) : nullptr;
+  double* CPT = p->bc_z == CALES_BC_WALL ? take(N) : nullptr;      // static c' of the Poisson Thomas solve (k_poisson_cp)
   double* smag = p->sgs_model == CALES_SGS_DSMAG ? take(N) : nullptr;
   double* tau = take(4 * nxy);
   double* tau_y = take(4 * (size_t)p->nx * p->nz);
@@ -133,7 +135,7 @@ static size_t carve(cales_solver* s, const cales_params* p, double* base) {
   double* dsm_cs = p->sgs_model == CALES_SGS_DSMAG ? take((size_t)p->nz * p->ny) : nullptr;
   if (s && base) {
     s->u = f[0]; s->v = f[1]; s->w = f[2]; s->p = f[3]; s->nut = f[4]; s->us = f[5]; s->vs = f[6]; s->ws = f[7];
-    s->Ru = f[8]; s->Rv = f[9]; s->Rw = f[10]; s->W = f[11]; s->CP = CP; s->CQ = CQ; s->smag = smag; s->tau = tau; s->tau_y = tau_y;
+    s->Ru = f[8]; s->Rv = f[9]; s->Rw = f[10]; s->W = f[11]; s->CP = CP; s->CQ = CQ; s->CPT = CPT; s->smag = smag; s->tau = tau; s->tau_y = tau_y;
     s->dzf = dzf; s->dzc = dzc; s->zc = zc; s->rdzf = rdzf; s->rdzc = rdzc; s->delta = delta; s->ak = ak; s->ck = ck; s->lamx = lamx; s->lamy = lamy;
     s->twx = reinterpret_cast<double2*>(twx); s->twy = reinterpret_cast<double2*>(twy); s->dctw = reinterpret_cast<double2*>(dctw);
     s->cncoef = cncoef; s->partial = partial; s->stage1 = stage1; s->scal = scal; s->maxit = reinterpret_cast<int*>(scal + 16);
@@ -270,6 +272,13 @@ extern "C" int cales_create(const cales_params* p, cales_solver** out) {
     for (int f = 0; f < RT_NF; ++f) s->rmaps_ok = s->rmaps_ok && make_field_map(&hm.m[f], fl[f], nx, ny, nz, RTT_TW, RT_TH);
     if (s->rmaps_ok && (cudaMemcpyAsync(s->rmaps, &hm, sizeof(hm), cudaMemcpyHostToDevice, s->st) != cudaSuccess || cudaStreamSynchronize(s->st) != cudaSuccess)) { cudaGetLastError(); s->rmaps_ok = false; }
   }
+  s->cpt_on = s->CPT ? 1 : 0;
+  if (s->CPT) {      // static c' of the Poisson columns (the matrix never changes)
+    k_poisson_cp<<<(unsigned)((s->nxy + 127) / 128), 128, 0, s->st>>>(s->c, s->pt, s->CPT);
+    e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s->st);
+    if (e != cudaSuccess) { delete s; return fail(CALES_ECUDA, std::string("k_poisson_cp: ") + cudaGetErrorString(e)); }
+  }
   for (int q = 0; q < 32; ++q) { s->kms[q] = 0.0; s->kcnt[q] = 0; }
   { double* ss_ = nullptr; (void)static_scratch_ptr(s->device, &ss_); }      // set-up of cales_cfl_dt_static; a failure is reported by that call
   *out = s;
@@ -354,7 +363,7 @@ static int run_transform_y(cales_solver* s, double* A, int inverse) {
 }
 static int run_poisson_z(cales_solver* s, double* A) {
   const int th = (s->nxy / 128 < 4 * 148) ? 64 : 128;      // small planes: smaller CTAs spread over more SMs
-  k_poisson_z<<<(unsigned)((s->nxy + th - 1) / th), th, 0, s->st>>>(s->c, s->pt, A, s->CP, s->CQ);
+  k_poisson_z<<<(unsigned)((s->nxy + th - 1) / th), th, 0, s->st>>>(s->c, s->pt, A, s->CP, s->CQ, s->cpt_on ? s->CPT : nullptr);
   LAUNCH_TRY(K_POISSON_Z);
   return CALES_OK;
 }
@@ -683,6 +692,7 @@ extern "C" int cales_set_option(cales_solver* s, const char* key, long long valu
   else if (k == "dsm_col_rows") { if (value < 0 || value > 4096) return fail(CALES_EINVAL, "dsm_col_rows must be 0..4096"); s->dsm_col_rows = (int)value; }
   else if (k == "rhs_planes_per_cta") { if (value < 0 || value > 65535) return fail(CALES_EINVAL, "rhs_planes_per_cta out of range"); s->rhs_kz = (int)value; }
   else if (k == "fft_stage") { if (value < 0 || value > 1) return fail(CALES_EINVAL, "fft_stage must be 0 or 1"); s->fft_stage = (int)value; }
+  else if (k == "poisson_cp_table") { if (value < 0 || value > 1) return fail(CALES_EINVAL, "poisson_cp_table must be 0 or 1"); s->cpt_on = (value && s->CPT) ? 1 : 0; }
   else if (k == "lazy_nut") { if (value < 0 || value > 1) return fail(CALES_EINVAL, "lazy_nut must be 0 or 1"); s->lazy_nut = (int)value; }
   else if (k == "rhs_variant") { if (value < 0 || value > 1) return fail(CALES_EINVAL, "rhs_variant must be 0 or 1"); s->rhs_variant = (int)value; }
   else if (k == "dsm_col_variant") { if (value < 0 || value > 2) return fail(CALES_EINVAL, "dsm_col_variant must be 0, 1 or 2"); s->dsm_col_variant = (int)value; }

@@ -19,7 +19,10 @@ struct PoissonTabs {
 // Poisson column (i,j): [a_k, b_k, c_k] phi = f with b_k = -(a_k + c_k) + lam_x + lam_y, a_0 and c_{nz-1} dropped from
 // b at walls (Neumann) or wrapped (periodic z: cyclic Thomas via Sherman-Morrison).  The singular (0,0) mode drops the
 // dzf-weighted mean of f, pins phi[0] = 0, and returns the solution with zero dzf-weighted mean (S15).
-CALES_HD void poisson_column(const Ctx& c, const PoissonTabs& T, int i, int j, double* __restrict__ A, double* __restrict__ CP, double* __restrict__ CQ) {
+// CPT (walls in z only): c' of every column, computed once at set-up by poisson_cp_column -- the matrix does not depend on the right-
+// hand side, so the forward sweep need not spill c' (8 of its 46 B/pt of DRAM traffic) and the backward sweep reads the table.
+CALES_HD void poisson_column(const Ctx& c, const PoissonTabs& T, int i, int j, double* __restrict__ A, double* __restrict__ CP, double* __restrict__ CQ,
+                             const double* __restrict__ CPT = nullptr) {
   const int nz = c.nz;
   const long long col = (long long)i + (long long)c.nx * j, st = c.nxy;
   const double lam = T.lamx[i] + T.lamy[j];
@@ -51,10 +54,12 @@ CALES_HD void poisson_column(const Ctx& c, const PoissonTabs& T, int i, int j, d
             const double r = 1.0 / (b - a * cp);
             cp = cc * r; dp = (d - a * dp) * r;
           }
-          CP[col + st * k] = cp; A[col + st * k] = dp;
+          if (!CPT) CP[col + st * k] = cp;
+          A[col + st * k] = dp;
         }
       }
     }
+    const double* __restrict__ CR = CPT ? CPT : CP;
     double x = dp;
     double s = x * c.dzf[nz - 1];
     for (int k0 = nz - 2; k0 >= 0; k0 -= TZ) {
@@ -62,7 +67,7 @@ CALES_HD void poisson_column(const Ctx& c, const PoissonTabs& T, int i, int j, d
 #pragma unroll
       for (int q = 0; q < TZ; ++q) {
         const int k = k0 - q;
-        dd[q] = k >= 0 ? A[col + st * k] : 0.0; cc[q] = k >= 0 ? CP[col + st * k] : 0.0;
+        dd[q] = k >= 0 ? A[col + st * k] : 0.0; cc[q] = k >= 0 ? CR[col + st * k] : 0.0;
       }
 #pragma unroll
       for (int q = 0; q < TZ; ++q) {
@@ -109,6 +114,23 @@ CALES_HD void poisson_column(const Ctx& c, const PoissonTabs& T, int i, int j, d
   const double vy = y + a0 * yn / g, vq = q + a0 * qn / g;
   const double f = vy / (1.0 + vq);
   for (int k = 0; k < nz; ++k) A[col + st * k] -= f * CQ[col + st * k];
+}
+
+// c' of column (i,j) exactly as poisson_column's forward sweep forms it (same operations in the same order: the table holds the same
+// bits the sweep would have spilled).  Non-periodic z only.
+CALES_HD void poisson_cp_column(const Ctx& c, const PoissonTabs& T, int i, int j, double* __restrict__ CPT) {
+  const int nz = c.nz;
+  const long long col = (long long)i + (long long)c.nx * j, st = c.nxy;
+  const double lam = T.lamx[i] + T.lamy[j];
+  const bool zero = (i == 0 && j == 0);
+  double cp = 0.0;
+  for (int k = 0; k < nz; ++k) {
+    const double a = T.ak[k], cc = T.ck[k];
+    const double b = lam - (k > 0 ? a : 0.0) - (k < nz - 1 ? cc : 0.0);
+    if (zero && k == 0) cp = 0.0;
+    else { const double r = 1.0 / (b - a * cp); cp = cc * r; }
+    CPT[col + st * k] = cp;
+  }
 }
 
 // Helmholtz column (i,j) of Eq. 18: (1 - c (L_zz + lam_x + lam_y)) q = d in place, for a velocity
@@ -237,10 +259,15 @@ CALES_HD double cn_column(const Ctx& c, const double* coef, int m, long long col
 }
 
 #ifdef __CUDACC__
-__global__ void k_poisson_z(Ctx c, PoissonTabs T, double* __restrict__ A, double* __restrict__ CP, double* __restrict__ CQ) {
+__global__ void k_poisson_z(Ctx c, PoissonTabs T, double* __restrict__ A, double* __restrict__ CP, double* __restrict__ CQ, const double* __restrict__ CPT) {
   const long long col = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (col >= c.nxy) return;
-  poisson_column(c, T, (int)(col % c.nx), (int)(col / c.nx), A, CP, CQ);
+  poisson_column(c, T, (int)(col % c.nx), (int)(col / c.nx), A, CP, CQ, CPT);
+}
+__global__ void k_poisson_cp(Ctx c, PoissonTabs T, double* __restrict__ CPT) {
+  const long long col = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (col >= c.nxy) return;
+  poisson_cp_column(c, T, (int)(col % c.nx), (int)(col / c.nx), CPT);
 }
 __global__ void k_helm_z(Ctx c, PoissonTabs T, int fam, const double* __restrict__ sc, double* __restrict__ A, double* __restrict__ CP, double* __restrict__ CQ) {
   const long long col = (long long)blockIdx.x * blockDim.x + threadIdx.x;
