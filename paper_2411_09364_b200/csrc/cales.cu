@@ -72,6 +72,7 @@ struct cales_solver {
   int dsm_col_rows;     // option: output rows per CTA of the column march (0: chosen from the grid)
   double* CPT; int cpt_on;      // static c' table of k_poisson_z (walls in z), option poisson_cp_table
   int fft_stage;        // option: 1 (default) stages the lines of the inverse x transform in shared memory by bulk copies
+  int rhs_pf;           // option: R^{k-1} of the next plane prefetched by the staged momentum kernel (0 off, 1 to L1, 2 to L2)
   int rhs_kz;           // option: k-planes per CTA of the staged momentum kernel (0: rt_chunk)
   int lazy_nut;         // option: 1 (default) skips the |S| -> nu_t pass of the dynamic model
   int dsm_col_variant;  // 0: TMA-staged register-window column march (k_dsm_col_tma); 1: shared-ring form of round 1 (k_dsm_col_sm); 2: direct loads (k_dsm_col_rw)
@@ -263,7 +264,7 @@ extern "C" int cales_create(const cales_params* p, cales_solver** out) {
   s->tile_min = 4000000;
   s->rhs_tile_min = 200000;
   s->dsm_col_variant = 0;
-  s->nut_lazy = false; s->nut_valid = true; s->graph_lazy = -1; s->lazy_nut = 1; s->dsm_col_rows = 0; s->rhs_kz = 0; s->fft_stage = 1;
+  s->nut_lazy = false; s->nut_valid = true; s->graph_lazy = -1; s->lazy_nut = 1; s->dsm_col_rows = 0; s->rhs_kz = 0; s->rhs_pf = 1; s->fft_stage = 1;
   s->rhs_variant = 1;      // measured on B200 at config 5: cp.async ring 22.7 ms, tiled TMA ring 25.1 ms per launch
   {
     const double* fl[RT_NF] = {s->u, s->v, s->w, s->nut, s->p};
@@ -509,7 +510,7 @@ static int substep(cales_solver* s, int rk) {
   const int kz = s->rhs_kz > 0 ? s->rhs_kz : rt_chunk(c.nx, c.ny, c.nz);
   dim3 rgrid((c.nx + RT_TX - 1) / RT_TX, (c.ny + RT_TY - 1) / RT_TY, (c.nz + kz - 1) / kz);
   if (s->N >= s->rhs_tile_min && s->rhs_variant == 0 && s->rmaps_ok) k_rhs_tile_tma<<<rgrid, RT_THREADS, RT_SMEM_TMA_BYTES, s->st>>>(c, a, s->rmaps, kz, (cfr && !imp && !imp3) ? s->partial : nullptr);
-  else if (s->N >= s->rhs_tile_min) k_rhs_tile<<<rgrid, RT_THREADS, RT_SMEM_DOUBLES * sizeof(double), s->st>>>(c, a, kz, (cfr && !imp && !imp3) ? s->partial : nullptr);
+  else if (s->N >= s->rhs_tile_min) k_rhs_tile<<<rgrid, RT_THREADS, RT_SMEM_DOUBLES * sizeof(double), s->st>>>(c, a, kz, (cfr && !imp && !imp3) ? s->partial : nullptr, s->rhs_pf);
   else { rgrid = s->pgrid; k_rhs_point<<<s->pgrid, s->pblock, 0, s->st>>>(c, a, (cfr && !imp && !imp3) ? s->partial : nullptr); }
   LAUNCH_TRY(K_RHS);
   long long npart = (long long)rgrid.x * rgrid.y * rgrid.z;
@@ -690,6 +691,7 @@ extern "C" int cales_set_option(cales_solver* s, const char* key, long long valu
     s->xB = L; s->x_threads = (int)th; s->x_smem = sm;
   }
   else if (k == "dsm_col_rows") { if (value < 0 || value > 4096) return fail(CALES_EINVAL, "dsm_col_rows must be 0..4096"); s->dsm_col_rows = (int)value; }
+  else if (k == "rhs_prefetch") { if (value < 0 || value > 2) return fail(CALES_EINVAL, "rhs_prefetch must be 0, 1 or 2"); s->rhs_pf = (int)value; }
   else if (k == "rhs_planes_per_cta") { if (value < 0 || value > 65535) return fail(CALES_EINVAL, "rhs_planes_per_cta out of range"); s->rhs_kz = (int)value; }
   else if (k == "fft_stage") { if (value < 0 || value > 1) return fail(CALES_EINVAL, "fft_stage must be 0 or 1"); s->fft_stage = (int)value; }
   else if (k == "poisson_cp_table") { if (value < 0 || value > 1) return fail(CALES_EINVAL, "poisson_cp_table must be 0 or 1"); s->cpt_on = (value && s->CPT) ? 1 : 0; }

@@ -203,7 +203,7 @@ __global__ void __launch_bounds__(256) k_rhs_point(const __grid_constant__ Ctx c
 // grid (ceil(nx/RT_TX), ceil(ny/RT_TY), ceil(nz/kz)), block RT_THREADS, dynamic smem RT_SMEM_DOUBLES*8.
 // partial[linear block id] = sum over the CTA's points of u* dzf[k] (or nullptr).
 __global__ void __launch_bounds__(RT_THREADS, CALES_RT_MINB) k_rhs_tile(const __grid_constant__ Ctx c, const __grid_constant__ RhsArgs a, int kz,
-                                                            double* __restrict__ partial) {
+                                                            double* __restrict__ partial, int pf) {
   extern __shared__ double rt_sm[];
   __shared__ double red[32];
   const int tid = threadIdx.x, tx = tid & 31, ty = tid >> 5;
@@ -271,6 +271,22 @@ __global__ void __launch_bounds__(RT_THREADS, CALES_RT_MINB) k_rhs_tile(const __
     __syncthreads();
     if (k + 2 <= k1) issue(k + 2);
     cp_async_commit();
+    if (pf && a.be != 0.0 && k + 1 < k1) {     // R^{k-1} of the next plane: pull its sectors towards the SM while this plane is computed
+#pragma unroll
+      for (int r = 0; r < RT_RPT; ++r) {
+        const int i = i0 + tx, j = j0 + ty * RT_RPT + r;
+        if (i < c.nx && j < c.ny && (tx & 3) == 0) {
+          const long long nn = idx3(c, i, j, k + 1);
+          if (pf == 1) {
+            asm volatile("prefetch.global.L1 [%0];" ::"l"(a.Ru0 + nn)); asm volatile("prefetch.global.L1 [%0];" ::"l"(a.Rv0 + nn));
+            asm volatile("prefetch.global.L1 [%0];" ::"l"(a.Rw0 + nn));
+          } else {
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(a.Ru0 + nn)); asm volatile("prefetch.global.L2 [%0];" ::"l"(a.Rv0 + nn));
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(a.Rw0 + nn));
+          }
+        }
+      }
+    }
     TileAcc q;
     q.sl[0] = rt_sm + ((k + 3) & 3) * (RT_NF * RT_PLANE); q.sl[1] = rt_sm + (k & 3) * (RT_NF * RT_PLANE); q.sl[2] = rt_sm + ((k + 1) & 3) * (RT_NF * RT_PLANE);
     const double dz = zm.dzfk;
