@@ -55,7 +55,7 @@ TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r2_ncu_traffic.csv")
 
 def ncu_traffic():
     """{(config, kernel): (dram bytes per launch, source)} from the committed ncu --set full capture (profiles/r2_ncu_traffic.csv,
-    made by the command in profiles/r2_ncu_full.md): dram__bytes_read.sum + dram__bytes_write.sum, averaged over the launches
+    made by the command in profiles/r2b_ncu_full.md): dram__bytes_read.sum + dram__bytes_write.sum, averaged over the launches
     of that kernel in the capture."""
     out = {}
     try:
@@ -64,7 +64,7 @@ def ncu_traffic():
                 if line.startswith("#") or not line.strip() or line.startswith("config,"):
                     continue
                 c, k, rd, wr = line.strip().split(",")[:4]
-                out[(int(c), k)] = (float(rd) + float(wr), "profiles/r2_ncu_traffic.csv (ncu --set full, see profiles/r2_ncu_full.md)")
+                out[(int(c), k)] = (float(rd) + float(wr), "profiles/r2_ncu_traffic.csv (ncu --set full, see profiles/r2b_ncu_full.md)")
     except OSError:
         pass
     return out

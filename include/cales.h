@@ -238,6 +238,8 @@ int cales_fp64_peak(cales_solver* s, double* tflops_host);
  * 0 off), "rhs_planes_per_cta" (k-planes per CTA of that kernel; 0 (default): chosen from the grid),
  * "dsm_col_variant" (column march of the dynamic model -- 0: register window, rows staged by TMA bulk copies; 1: the
  * shared-memory-ring form; 2: register window, direct loads),
+ * "fft_x_lines" / "fft_y_cols" (lines per CTA of the x transforms / columns per CTA tile of the y transforms; default: about 256
+ * threads per CTA),
  * "fft_stage" (1 (default): the first passes of the inverse transforms and the divergence of the forward x transform read shared
  * memory staged by bulk copies / batched loads; 0: they read global memory directly), "poisson_cp_table" (walls in z -- 1 (default):
  * the Thomas solve of the Poisson solver reads c' from a table built once at create; 0: it recomputes and spills c' on every solve).

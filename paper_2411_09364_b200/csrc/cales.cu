@@ -690,6 +690,17 @@ extern "C" int cales_set_option(cales_solver* s, const char* key, long long valu
     if (th > 512 || sm > 200 * 1024) return fail(CALES_EINVAL, "fft_x_lines: CTA too large");
     s->xB = L; s->x_threads = (int)th; s->x_smem = sm;
   }
+  else if (k == "fft_y_cols") {      // columns per CTA tile of the y transforms (power of two; default: ~256 threads per CTA)
+    int tish = 0; while ((1LL << tish) < value) ++tish;
+    if (value < 1 || (1LL << tish) != value || value > s->c.nx || value > 64) return fail(CALES_EINVAL, "fft_y_cols must be a power of two <= min(nx, 64)");
+    const int n2 = s->c.ny / 2;
+    bool has3 = false; for (int q = 0; q < s->ply.npass; ++q) has3 |= s->ply.radix[q] == 3;
+    const int per_thread = has3 ? 3 * (F2_E / 3) : F2_E;
+    long long th = ((long long)value * n2 + per_thread - 1) / per_thread; th = (th + 31) / 32 * 32; if (th < 32) th = 32;
+    size_t sm = (size_t)value * n2 * 16; if (sm < 16) sm = 16;
+    if (th > 512 || sm > 200 * 1024) return fail(CALES_EINVAL, "fft_y_cols: CTA too large");
+    s->yTI = (int)value; s->y_tish = tish; s->y_threads = (int)th; s->y_smem = sm;
+  }
   else if (k == "dsm_col_rows") { if (value < 0 || value > 4096) return fail(CALES_EINVAL, "dsm_col_rows must be 0..4096"); s->dsm_col_rows = (int)value; }
   else if (k == "rhs_prefetch") { if (value < 0 || value > 2) return fail(CALES_EINVAL, "rhs_prefetch must be 0, 1 or 2"); s->rhs_pf = (int)value; }
   else if (k == "rhs_planes_per_cta") { if (value < 0 || value > 65535) return fail(CALES_EINVAL, "rhs_planes_per_cta out of range"); s->rhs_kz = (int)value; }
