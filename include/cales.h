@@ -237,7 +237,8 @@ int cales_fp64_peak(cales_solver* s, double* tflops_host);
  * "rhs_prefetch" (staged momentum kernel -- R^{k-1} of the next plane prefetched while a plane is computed: 1 (default) to L1, 2 to L2,
  * 0 off), "rhs_planes_per_cta" (k-planes per CTA of that kernel; 0 (default): chosen from the grid),
  * "dsm_col_variant" (column march of the dynamic model -- 0: register window, rows staged by TMA bulk copies; 1: the
- * shared-memory-ring form; 2: register window, direct loads),
+ * shared-memory-ring form; 2: register window, direct loads; with the 3-D test filter 0: staged rows + register window, 1 / 2: the
+ * shared-memory-ring march),
  * "fft_x_lines" / "fft_y_cols" (lines per CTA of the x transforms / columns per CTA tile of the y transforms; default: about 256
  * threads per CTA),
  * "fft_stage" (1 (default): the first passes of the inverse transforms and the divergence of the forward x transform read shared

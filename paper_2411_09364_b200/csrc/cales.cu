@@ -20,6 +20,9 @@
 #ifndef CALES_D3C_MINB
 #define CALES_D3C_MINB 6
 #endif
+#ifndef CALES_D3T_MINB
+#define CALES_D3T_MINB 4
+#endif
 #ifndef CALES_D3C_NBUF
 #define CALES_D3C_NBUF 1
 #endif
@@ -255,6 +258,7 @@ extern "C" int cales_create(const cales_params* p, cales_solver** out) {
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_smag_tile, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(ST_SMEM_DOUBLES * sizeof(double)));
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dsm_pass1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(DSM_SMEM_DOUBLES * sizeof(double)));
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dsm3_pass1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(D3_SMEM_DOUBLES * sizeof(double)));
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dsm3_col_tma<64, CALES_D3T_MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)DSM3T_RAW_BYTES);
   if (e != cudaSuccess) { delete s; return fail(CALES_ECUDA, std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e)); }
   s->pblock = dim3(32, 8, 1);
   s->pgrid = dim3((nx + 31) / 32, (ny + 7) / 8, nz);
@@ -434,7 +438,14 @@ static int run_eddy_viscosity(cales_solver* s, const double* u, const double* v,
           LAUNCH_TRY(K_DSM3);
         }
         // <threads, min CTAs/SM, row buffers>: measured on B200 (config 4): (64,4,2) 6.46 ms, (64,6,1) 6.16 ms, (64,8,1) 7.45 ms (spills)
-      k_dsm3_col<CALES_D3C_TXB, CALES_D3C_MINB, CALES_D3C_NBUF><<<dim3(ds.nbx, (sp.jhi - sp.jlo + DSMC_LY - 1) / DSMC_LY, sp.khi - sp.klo), CALES_D3C_TXB, 0, s->st>>>(c, u, v, w, sp.klo, sp.jlo, sp.jhi, ds.pslots, s->smag, s->dsm_part);
+        // dsm_col_variant 0 (default): rows staged by bulk copies, y-window in registers (k_dsm3_col_tma; needs 16-byte aligned rows and
+        // nx >= 66); otherwise the shared-ring march of round 1
+        if (s->dsm_col_variant == 0 && (((size_t)u | (size_t)v | (size_t)w) & 15) == 0 && c.nx >= 66) {
+          int ly = s->dsm_col_rows;
+          if (ly <= 0) ly = (sp.jhi - sp.jlo >= 512) ? 256 : ((sp.jhi - sp.jlo >= 192) ? 128 : 32);      // B200, config 5: 32: 40.6, 64: 39.5, 128: 38.9, 256: 38.3 ms
+          k_dsm3_col_tma<64, CALES_D3T_MINB><<<dim3(ds.nbx, sp.khi - sp.klo, (unsigned)((sp.jhi - sp.jlo + ly - 1) / ly)), 64, DSM3T_RAW_BYTES, s->st>>>(c, u, v, w, sp.klo, sp.jlo, sp.jhi, ly, ds.pslots, s->smag, s->dsm_part);
+        } else
+          k_dsm3_col<CALES_D3C_TXB, CALES_D3C_MINB, CALES_D3C_NBUF><<<dim3(ds.nbx, (sp.jhi - sp.jlo + DSMC_LY - 1) / DSMC_LY, sp.khi - sp.klo), CALES_D3C_TXB, 0, s->st>>>(c, u, v, w, sp.klo, sp.jlo, sp.jhi, ds.pslots, s->smag, s->dsm_part);
         LAUNCH_TRY(K_DSM3_COL);
       }
     } else if (ywall) {

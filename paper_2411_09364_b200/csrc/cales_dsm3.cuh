@@ -13,6 +13,7 @@
 #pragma once
 #include "cales_common.cuh"
 #include "cales_closures.cuh"
+#include "cales_dsm_col.cuh"
 
 namespace cales {
 
@@ -254,6 +255,59 @@ CALES_HD bool d3c_phaseB(const Ctx& c, int txb, int t, int r, int k, const doubl
   return done;
 }
 
+// ---- the column march in the register-window form of cales_dsm_col.cuh ------------------------------------------------------
+// One row for an output column: zq = the thread's own z-filtered 21 quantities, UNNORMALISED (zq' = q(k-1) + q(k+1) + 2 q(k) = 4 Fz q);
+// shbuf = the row's zq' of all columns ([DSMC_NQ][txb]).  x: xq' = l + r + 2 c = 16 Fx Fz q; y over the register window:
+// F' = w2 + xq' + 2 w1 = 64 F q.  With L' = 64 F'(u_i u_j) - F'(u_i) F'(u_j) = 4096 L and M' = 64 F'(|S| S_ij) - a2 |S~|' S~'_ij =
+// 4096 M / (2 Delta^2) the powers of two go into the constants of the contraction.  a2 = alpha^2 of three filtered directions.
+template <int PAR>
+CALES_HD void dsm3r_row(const double* shbuf, int txb, int t, const double* zq, DsmrWin& w, bool emit, double d2, double a2, double* lm, double* mm) {
+  const double* sl = shbuf + t - 1;
+  const double* sr = shbuf + t + 1;
+  double* w1 = w.q[1 - PAR];     // row r-1
+  double* w2 = w.q[PAR];         // row r-2, then row r
+  double F[DSMC_NQ];
+#pragma unroll
+  for (int m = 0; m < DSMC_NQ; ++m) {
+    const double x = (sl[m * txb] + sr[m * txb]) + 2.0 * zq[m];
+    const double ts = w2[m] + 2.0 * w1[m]; w2[m] = x; F[m] = ts + x;      // old window value consumed first (no moves)
+  }
+  if (!emit) return;
+  const double* St = F + 15;
+  const double stmag = sqrt(2.0 * (St[0] * St[0] + St[1] * St[1] + St[2] * St[2]) + 4.0 * (St[3] * St[3] + St[4] * St[4] + St[5] * St[5]));
+  const double a2s = a2 * stmag;
+  double Mp[6];
+#pragma unroll
+  for (int m = 0; m < 6; ++m) Mp[m] = 64.0 * F[9 + m] - a2s * St[m];
+  const double md = Mp[0] * Mp[0] + Mp[1] * Mp[1] + Mp[2] * Mp[2], mo = Mp[3] * Mp[3] + Mp[4] * Mp[4] + Mp[5] * Mp[5];
+  const double ld = (64.0 * F[3] - F[0] * F[0]) * Mp[0] + (64.0 * F[4] - F[1] * F[1]) * Mp[1] + (64.0 * F[5] - F[2] * F[2]) * Mp[2];
+  const double lo = (64.0 * F[6] - F[0] * F[1]) * Mp[3] + (64.0 * F[7] - F[0] * F[2]) * Mp[4] + (64.0 * F[8] - F[1] * F[2]) * Mp[5];
+  const double sc = 2.0 * d2 * (1.0 / 4096.0);
+  *lm = (ld + 2.0 * lo) * (sc * (1.0 / 4096.0));
+  *mm = (md + 2.0 * mo) * (sc * sc);
+}
+
+// zq' of one column from accessors to the raw velocities around (column, row) on planes k-2 .. k+2: U(a, b, d) = u at column offset a,
+// row offset b, plane k + d (the same for V, W).  Returns |S| of plane k.
+template <class GU, class GV, class GW>
+CALES_HD double dsm3r_zq(GU U, GV V, GW W, double rdx, double rdy, const double* rdzf3 /* k-1, k, k+1 */, const double* rdzc4 /* k-2 .. k+1 */, double* zq) {
+  double smag_c = 0.0;
+#pragma unroll
+  for (int s = 0; s < 3; ++s) {
+    const int d = s == 0 ? -1 : (s == 1 ? 1 : 0);      // the two outer planes first, the centre plane (weight 2) last
+    auto Ud = [&](int a, int b, int dd) { return U(a, b, d + dd); };
+    auto Vd = [&](int a, int b, int dd) { return V(a, b, d + dd); };
+    auto Wd = [&](int a, int b, int dd) { return W(a, b, d + dd); };
+    double b[DSMC_NB], q[DSMC_NQ];
+    dsmr_base_from(Ud, Vd, Wd, rdx, rdy, rdzf3[1 + d], rdzc4[2 + d], rdzc4[1 + d], b);
+    dsmc_q(b, q);
+#pragma unroll
+    for (int m = 0; m < DSMC_NQ; ++m) zq[m] = s == 0 ? q[m] : (s == 1 ? zq[m] + q[m] : zq[m] + 2.0 * q[m]);
+    if (d == 0) smag_c = b[9];
+  }
+  return smag_c;
+}
+
 #ifdef __CUDACC__
 // grid (ceil(nx/D3_TX), row tiles, planes), block (D3_TX, D3_TY), dynamic smem D3_SMEM_DOUBLES*8.
 // planes: k = blockIdx.z (+ kskip when blockIdx.z >= ksplit); rows: j0 = blockIdx.y * jstride, of which only the rows
@@ -325,6 +379,117 @@ __global__ void __launch_bounds__(TXB, MINB) k_dsm3_col(const __grid_constant__ 
         part[slot * 2] = lm; part[slot * 2 + 1] = mm;
       }
     }
+  }
+}
+
+// ---- the same march with the raw rows staged by the TMA engine and the y-window in registers (as k_dsm_col_tma) -----------
+// 14 lines per raw row: u on planes k-2 .. k+2, v on k-2 .. k+2, w on k-2 .. k+1, columns i0-2 .. i0+TXB-1, in a ring of DSMT_NS rows
+// filled by cp.async.bulk copies (seven producer lanes in each of the two warps) that complete on mbarriers two rows ahead.  Every
+// thread evaluates the strain rate of its column on the three planes from shared memory (immediate offsets), forms the unnormalised
+// zq', publishes it, and dsm3r_row runs the x filter, the register y-window and the contraction.
+// grid (ceil(nx/(TXB-2)), khi-klo, ceil((jhi-jlo)/ly)), block TXB = 64.  Needs nx >= TXB + 2, 16-byte aligned fields, planes klo-2 ..
+// khi+1 and rows jlo-2 .. jhi+1 plain (in the array or periodic wrap): the region d3_split gives the column march.
+enum { DSM3T_NL = 14, DSM3T_RAW_BYTES = DSMT_NS * DSM3T_NL * 66 * 8 };      // for TXB = 64
+template <int TXB, int MINB>
+__global__ void __launch_bounds__(TXB, MINB) k_dsm3_col_tma(const __grid_constant__ Ctx c, const double* __restrict__ u, const double* __restrict__ v,
+                                                            const double* __restrict__ w, int klo, int jlo, int jhi, int ly, int pslots,
+                                                            double* __restrict__ smag, double* __restrict__ part) {
+  constexpr int LW = TXB + 2;
+  constexpr int STAGE = DSM3T_NL * LW;
+  extern __shared__ __align__(128) double d3t_raw[];      // DSMT_NS * STAGE doubles (dynamic: with `sh` the CTA is past 48 KB)
+  double* raw = d3t_raw;
+  __shared__ double sh[2][DSMC_NQ * TXB];
+  __shared__ unsigned long long full[DSMT_NS];
+  const int t = threadIdx.x, k = klo + blockIdx.y;
+  const int i0 = blockIdx.x * (TXB - 2);
+  const int j0 = jlo + blockIdx.z * ly;
+  const int jend = min(j0 + ly, jhi);
+  const int nrows = jend - j0 + 2;             // base rows j0-1 .. jend; raw rows j0-2 .. jend+1
+  const int nraw = nrows + 2;
+  const int gi = i0 - 1 + t;
+  const bool inner = t >= 1 && t <= TXB - 2;
+  const bool outcol = inner && gi < c.nx;
+  const double d2 = c.delta[k] * c.delta[k], a2 = c.alpha * c.alpha * c.alpha;      // alpha = 8^(1/3) x the 2-D ratio^(1/2): (alpha^(3/2))^2
+  const double rdx = c.rdx, rdy = c.rdy;
+  auto wz = [&](int kk) { return kk < 0 ? kk + c.nz : (kk >= c.nz ? kk - c.nz : kk); };
+  const double rdzf3[3] = {c.rdzf[wz(k - 1)], c.rdzf[k], c.rdzf[wz(k + 1)]};
+  const double rdzc4[4] = {c.rdzc[wz(k - 2)], c.rdzc[wz(k - 1)], c.rdzc[k], c.rdzc[wz(k + 1)]};
+  // ---- producer state (lanes 0..6 of warps 0 and 1: seven lines each)
+  const double* src = nullptr; int gj_next = 0, segA = 0;
+  const bool producer = (t & 31) < DSM3T_NL / 2 && t < 64;
+  const int line = (t & 31) + (t >> 5) * (DSM3T_NL / 2);
+  if (producer) {
+    const int l = line;
+    const double* f = l < 5 ? u : (l < 10 ? v : w);
+    const int kk = wz(k - 2 + (l < 5 ? l : (l < 10 ? l - 5 : l - 10)));
+    gj_next = j0 - 2; gj_next = gj_next < 0 ? gj_next + c.ny : gj_next;
+    src = f + ((long long)kk * c.ny + gj_next) * c.nx;
+    const int cw0 = (((i0 - 2) % c.nx) + c.nx) % c.nx;
+    segA = min(LW, c.nx - cw0);
+    src += cw0;
+  }
+  auto issue = [&](int slot) {
+    unsigned long long* bar = &full[slot];
+    if (t == 0) mbar_expect_tx(bar, STAGE * (unsigned)sizeof(double));
+    double* dst = raw + slot * STAGE + line * LW;
+    bulk_g2s(dst, src, (unsigned)segA * 8u, bar);
+    if (segA < LW) bulk_g2s(dst + segA, src - (c.nx - segA), (unsigned)(LW - segA) * 8u, bar);
+    ++gj_next;
+    if (gj_next == c.ny) { gj_next = 0; src -= (long long)(c.ny - 1) * c.nx; } else src += c.nx;
+  };
+  if (t == 0) {
+#pragma unroll
+    for (int s = 0; s < DSMT_NS; ++s) mbar_init(&full[s], 1);
+    mbar_fence_init();
+  }
+  __syncthreads();
+  if (producer) {
+#pragma unroll
+    for (int s = 0; s < DSMT_NS; ++s) if (s < nraw) issue(s);
+  }
+  DsmrWin win;
+  dsmr_win_init(win);
+  double* sm_out = smag + idx3(c, gi < c.nx ? gi : 0, j0, k);           // |S| of output row j0, bumped by nx per emitted row
+  long long pslot = ((long long)k * c.ny + j0) * pslots + blockIdx.x * (TXB / 32) + (t >> 5);
+  const double* Rt = raw + t + 1;
+  auto row = [&](auto ph, int r) {
+    constexpr int PH = decltype(ph)::value;    // r & 3
+    constexpr int PAR = PH & 1, S0 = PH, S1 = (PH + 1) & 3, S2 = (PH + 2) & 3;
+    if (r == 0) { mbar_wait(&full[0], 0); mbar_wait(&full[1], 0); }
+    mbar_wait(&full[S2], ((r + 2) >> 2) & 1);
+    double zq[DSMC_NQ], smag_c;
+    {
+      const double* R0 = Rt + S0 * STAGE;      // raw row below the base row
+      const double* R1 = Rt + S1 * STAGE;      // the base row
+      const double* R2 = Rt + S2 * STAGE;      // the row above
+      auto U = [&](int a, int bb, int d) { return (bb < 0 ? R0 : (bb > 0 ? R2 : R1))[(2 + d) * LW + a]; };
+      auto V = [&](int a, int bb, int d) { return (bb < 0 ? R0 : (bb > 0 ? R2 : R1))[(7 + d) * LW + a]; };
+      auto W = [&](int a, int bb, int d) { return (bb < 0 ? R0 : (bb > 0 ? R2 : R1))[(12 + d) * LW + a]; };
+      smag_c = dsm3r_zq(U, V, W, rdx, rdy, rdzf3, rdzc4, zq);
+    }
+#pragma unroll
+    for (int q = 0; q < DSMC_NQ; ++q) sh[PAR][q * TXB + t] = zq[q];
+    __syncthreads();
+    if (producer && r + DSMT_NS < nraw) issue(S0);     // the slot of raw row r: every thread is past its last read
+    double lm = 0.0, mm = 0.0;
+    const bool emit = r >= 2;
+    if (inner) dsm3r_row<PAR>(sh[PAR], TXB, t, zq, win, emit, d2, a2, &lm, &mm);
+    if (emit) {
+      if (outcol) *sm_out = win.smag_prev;
+      else { lm = 0.0; mm = 0.0; }
+      sm_out += c.nx;
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) { lm += __shfl_down_sync(0xffffffffu, lm, o); mm += __shfl_down_sync(0xffffffffu, mm, o); }
+      if ((t & 31) == 0) { part[pslot * 2] = lm; part[pslot * 2 + 1] = mm; }
+      pslot += pslots;
+    }
+    win.smag_prev = smag_c;
+  };
+  for (int r = 0; r < nrows; r += 4) {
+    row(std::integral_constant<int, 0>{}, r);
+    if (r + 1 < nrows) row(std::integral_constant<int, 1>{}, r + 1);
+    if (r + 2 < nrows) row(std::integral_constant<int, 2>{}, r + 2);
+    if (r + 3 < nrows) row(std::integral_constant<int, 3>{}, r + 3);
   }
 }
 #endif

@@ -220,6 +220,48 @@ static void emu_nut(emu_solver* s, const double* u, const double* v, const doubl
         s->dsm_part[(row * ntx + bx) * 2] = lm; s->dsm_part[(row * ntx + bx) * 2 + 1] = mm;
       }
     }
+    if (sp.col && c.nx >= 66) {   // k_dsm3_col_tma: register window per emulated thread, zq' from the raw velocities on planes k-2 .. k+2
+      const int T = dsh.txb;
+      std::vector<double> sh(2 * DSMC_NQ * T), zq((size_t)T * DSMC_NQ), smc(T);
+      std::vector<DsmrWin> win(T);
+      auto wr = [](int a, int n) { return a < 0 ? a + n : (a >= n ? a - n : a); };
+      for (int k = sp.klo; k < sp.khi; ++k) for (int by = 0; by * DSMC_LY < sp.jhi - sp.jlo; ++by) for (int bx = 0; bx < dsh.nbx; ++bx) {
+        const int i0 = bx * (T - 2), j0 = sp.jlo + by * DSMC_LY, jend = std::min(j0 + DSMC_LY, sp.jhi), nrows = jend - j0 + 2;
+        const double d2 = c.delta[k] * c.delta[k], a2 = c.alpha * c.alpha * c.alpha;
+        const double rdzf3[3] = {c.rdzf[wr(k - 1, c.nz)], c.rdzf[k], c.rdzf[wr(k + 1, c.nz)]};
+        const double rdzc4[4] = {c.rdzc[wr(k - 2, c.nz)], c.rdzc[wr(k - 1, c.nz)], c.rdzc[k], c.rdzc[wr(k + 1, c.nz)]};
+        for (int t = 0; t < T; ++t) dsmr_win_init(win[t]);
+        for (int r = 0; r < nrows; ++r) {
+          const int gj = wr(j0 - 1 + r, c.ny);
+          double* buf = sh.data() + (r & 1) * DSMC_NQ * T;
+          for (int t = 0; t < T; ++t) {
+            const int gw = (((i0 - 1 + t) % c.nx) + c.nx) % c.nx;
+            auto at = [&](const double* f, int a, int b, int d) { return f[idx3(c, wr(gw + a, c.nx), wr(gj + b, c.ny), wr(k + d, c.nz))]; };
+            auto U = [&](int a, int b, int d) { return at(u, a, b, d); };
+            auto V = [&](int a, int b, int d) { return at(v, a, b, d); };
+            auto W = [&](int a, int b, int d) { return at(w, a, b, d); };
+            smc[t] = dsm3r_zq(U, V, W, c.rdx, c.rdy, rdzf3, rdzc4, &zq[(size_t)t * DSMC_NQ]);
+            for (int q = 0; q < DSMC_NQ; ++q) buf[q * T + t] = zq[(size_t)t * DSMC_NQ + q];
+          }
+          std::vector<double> wl(T / 32, 0.0), wm(T / 32, 0.0);
+          for (int t = 0; t < T; ++t) {
+            double lm = 0.0, mm = 0.0;
+            const bool inner = t >= 1 && t <= T - 2, emit = r >= 2;
+            if (inner) {
+              if (r & 1) dsm3r_row<1>(buf, T, t, &zq[(size_t)t * DSMC_NQ], win[t], emit, d2, a2, &lm, &mm);
+              else dsm3r_row<0>(buf, T, t, &zq[(size_t)t * DSMC_NQ], win[t], emit, d2, a2, &lm, &mm);
+            }
+            const int gi = i0 - 1 + t;
+            if (emit && inner && gi < c.nx) { s->smag[idx3(c, gi, j0 + r - 2, k)] = win[t].smag_prev; wl[t >> 5] += lm; wm[t >> 5] += mm; }
+            win[t].smag_prev = smc[t];
+          }
+          if (r >= 2) for (int wq = 0; wq < T / 32; ++wq) {
+            const long long slot = ((long long)k * c.ny + (j0 + r - 2)) * ntx + bx * (T / 32) + wq;
+            s->dsm_part[slot * 2] = wl[wq]; s->dsm_part[slot * 2 + 1] = wm[wq];
+          }
+        }
+      }
+    } else
     if (sp.col) {   // k_dsm3_col, stepped row by row with the block barrier between the phases
       const int T = dsh.txb;
       std::vector<double> sh(2 * DSMC_NQ * T), zq((size_t)T * DSMC_NQ), smc(T), ring(2 * DSMC_NQ * T), smprev(T);

@@ -28,6 +28,9 @@ SMALL = {
     "cfg4_duct_dsm_filter3d": (4, (48, 18, 12), 2, dict(dsm_filter3d=1)),
     "duct_wmles_dsm_filter3d": (4, (36, 12, 12), 1, dict(wall_model=1, wall_model_y=1, nu=1.0 / 40000, dsm_filter3d=1)),
     "cfg1_dsm_filter3d": (1, (24, 16, 12), 2, dict(sgs_model=2, dsm_filter3d=1)),
+    # nx >= 66: the register-window march with staged rows (k_dsm3_col_tma), two x blocks, periodic wrap in x and in z / walls
+    "cfg5_dsm_filter3d_wide": (5, (72, 12, 12), 1, dict(dsm_filter3d=1)),
+    "cfg1_dsm_filter3d_wide": (1, (72, 8, 8), 1, dict(sgs_model=2, dsm_filter3d=1)),
 }
 # the sizes the GPU parity tests use: several tiles in every direction plus ragged tails
 GPU_CASES = {

@@ -343,7 +343,11 @@ def test_momentum_kernel_all_forms_parity(oracle, gpu, n, shape, min_points, var
 
 @pytest.mark.parametrize("variant", [0, 1, 2])
 @pytest.mark.parametrize("n,shape,over", [(5, (144, 72, 24), {}), (4, (128, 48, 20), {}), (1, (96, 72, 12), dict(sgs_model=2)),
-                                          (5, (48, 36, 16), {}), (4, (192, 36, 12), dict(wall_model=1, wall_model_y=1, nu=1.0 / 40000))])
+                                          (5, (48, 36, 16), {}), (4, (192, 36, 12), dict(wall_model=1, wall_model_y=1, nu=1.0 / 40000)),
+                                          # 3-D box test filter: variant 0 = staged rows + register window (k_dsm3_col_tma), 1 / 2 = shared-ring march
+                                          (5, (144, 72, 24), dict(dsm_filter3d=1)), (4, (128, 48, 20), dict(dsm_filter3d=1)),
+                                          (1, (96, 72, 12), dict(sgs_model=2, dsm_filter3d=1)), (5, (72, 288, 16), dict(dsm_filter3d=1)),
+                                          (4, (192, 36, 12), dict(wall_model=1, wall_model_y=1, nu=1.0 / 40000, dsm_filter3d=1))])
 def test_dynamic_model_column_kernels_parity(oracle, gpu, n, shape, over, variant):
     """Both forms of the column march of the dynamic model (register window / shared-memory ring): nu_t and the coefficient
     against the oracle on grids spanning several 62-column blocks with a ragged tail and more than one 32-row band, a triply
