@@ -554,3 +554,27 @@ def test_lazy_nu_t_is_the_same_nu_t(oracle, gpu, n, shape):
     for f in range(5):
         assert np.array_equal(a.get_numpy(f), b.get_numpy(f)), f
     a.close(); b.close()
+
+
+@pytest.mark.parametrize("key,value", [("poisson_cp_table", 0), ("fft_stage", 0), ("rhs_prefetch", 0), ("rhs_prefetch", 2), ("fft_y_cols", 16),
+                                       ("fft_y_cols", 4), ("fft_x_lines", 2), ("rhs_planes_per_cta", 8), ("dsm_col_rows", 16)])
+@pytest.mark.parametrize("n,shape", [(5, (144, 96, 32)), (3, (96, 72, 40))])
+def test_kernel_selection_options_keep_oracle_parity(oracle, gpu, n, shape, key, value):
+    """Every kernel-selection knob of cales_set_option is a different way of computing the same step: two steps with the knob off its
+    default stay within the one-step tolerance of the oracle, and within round-off of the default build."""
+    cfg, kw, (u, v, w), dt = pc.prepare(oracle, n, shape)
+    o = pc.make(oracle.Oracle, kw)
+    a = pc.make(gpu.Solver, kw)
+    b = pc.make(gpu.Solver, kw)
+    b.set_option("rhs_tile_min_points", 0); a.set_option("rhs_tile_min_points", 0)
+    b.set_option(key, value)
+    for s_ in (o, a, b):
+        s_.set_velocity(u, v, w)
+    for s in range(2):
+        o.step(dt); a.step(dt); b.step(dt)
+    want = [o.get(f) for f in range(5)]
+    err = pc.field_errors(_gpu_fields(b), want, o.dzf, kw["nu"])
+    assert max(err.values()) <= 1e-10, err
+    dev = pc.field_errors(_gpu_fields(b), _gpu_fields(a), o.dzf, kw["nu"])
+    assert max(dev.values()) <= 1e-12, dev
+    a.close(); b.close()
