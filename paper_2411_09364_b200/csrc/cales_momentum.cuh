@@ -92,6 +92,41 @@ __global__ void __launch_bounds__(256, IMP3 ? 4 : 8) k_correct(Ctx c, CorrArgs a
   const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y * blockDim.y + threadIdx.y, k = blockIdx.z;
   if (i < c.nx && j < c.ny) correct_point<IMP3>(c, a, i, j, k);
 }
+// Two x-neighbours per thread with 16-byte loads and stores (explicit or implicit-z diffusion, nx even, 16-byte aligned fields): half the
+// instructions of k_correct for the same bytes.  grid (ceil(nx/64), ceil(ny/8), nz), block (32, 8).  Rows or planes that need a
+// ghost go through correct_point.
+__global__ void __launch_bounds__(256, 4) k_correct2(Ctx c, CorrArgs a) {
+  const int i = 2 * (blockIdx.x * blockDim.x + threadIdx.x), j = blockIdx.y * blockDim.y + threadIdx.y, k = blockIdx.z;
+  if (i >= c.nx || j >= c.ny) return;
+  if (!interior_row(c, j, k)) { correct_point<false>(c, a, i, j, k); correct_point<false>(c, a, i + 1, j, k); return; }
+  const long long n = idx3(c, i, j, k);
+  double gdt, sh = 0.0;
+  if (a.sc && a.shift) ld_scalar2(a.shift + 4, sh, gdt);
+  else { gdt = a.sc ? ld_scalar(a.sc + RK_GDT) : a.gdt; if (a.shift) sh = ld_scalar(a.shift); }
+  const Nbr o = neighbours(c, i, j, k);
+  auto l2 = [](const double* q) { return *reinterpret_cast<const double2*>(q); };
+  const double2 ph = l2(a.phi + n), phy = l2(a.phi + n + o.jp), phz = l2(a.phi + n + o.kp);
+  const double phx1 = a.phi[i + 2 < c.nx ? n + 2 : n + 2 - c.nx];
+  const double2 us = l2(a.us + n), vs = l2(a.vs + n), ws = l2(a.ws + n);
+  double2 p2 = l2(a.p + n);
+  const double rdzc = c.rdzc[k];
+  double2 u2, v2, w2;
+  u2.x = (us.x + sh) - gdt * (ph.y - ph.x) * c.rdx;  u2.y = (us.y + sh) - gdt * (phx1 - ph.y) * c.rdx;
+  v2.x = vs.x - gdt * (phy.x - ph.x) * c.rdy;        v2.y = vs.y - gdt * (phy.y - ph.y) * c.rdy;
+  w2.x = ws.x - gdt * (phz.x - ph.x) * rdzc;         w2.y = ws.y - gdt * (phz.y - ph.y) * rdzc;
+  *reinterpret_cast<double2*>(a.u + n) = u2; *reinterpret_cast<double2*>(a.v + n) = v2; *reinterpret_cast<double2*>(a.w + n) = w2;
+  if (a.update_p) {
+    double dx = ph.x, dy = ph.y;
+    if (a.cimp != 0.0) {      // Eq. 22: - c L_zz phi
+      const double cimp = a.sc ? ld_scalar(a.sc + RK_CIMP) : a.cimp;
+      const double2 phm = l2(a.phi + n + o.km);
+      const double rm = c.rdzc[k - 1], rf = c.rdzf[k];
+      dx -= cimp * (((phz.x - ph.x) * rdzc - (ph.x - phm.x) * rm) * rf);
+      dy -= cimp * (((phz.y - ph.y) * rdzc - (ph.y - phm.y) * rm) * rf);
+    }
+    p2.x += dx; p2.y += dy; *reinterpret_cast<double2*>(a.p + n) = p2;
+  }
+}
 // deterministic two-stage sum of `n` partials: stage 1 -> out1[gridDim.x], stage 2 (one block) -> scalar
 __global__ void k_sum_stage1(const double* __restrict__ in, long long n, double* __restrict__ out1) {
   __shared__ double sh[32];
