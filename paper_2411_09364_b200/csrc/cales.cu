@@ -278,7 +278,7 @@ extern "C" int cales_create(const cales_params* p, cales_solver** out) {
     for (int f = 0; f < RT_NF; ++f) s->rmaps_ok = s->rmaps_ok && make_field_map(&hm.m[f], fl[f], nx, ny, nz, RTT_TW, RT_TH);
     if (s->rmaps_ok && (cudaMemcpyAsync(s->rmaps, &hm, sizeof(hm), cudaMemcpyHostToDevice, s->st) != cudaSuccess || cudaStreamSynchronize(s->st) != cudaSuccess)) { cudaGetLastError(); s->rmaps_ok = false; }
   }
-  s->cpt_on = s->CPT ? 1 : 0;
+  s->cpt_on = s->CPT ? 2 : 0;
   if (s->CPT) {      // static c' of the Poisson columns (the matrix never changes)
     k_poisson_cp<<<(unsigned)((s->nxy + 127) / 128), 128, 0, s->st>>>(s->c, s->pt, s->CPT);
     e = cudaGetLastError();
@@ -369,7 +369,8 @@ static int run_transform_y(cales_solver* s, double* A, int inverse) {
 }
 static int run_poisson_z(cales_solver* s, double* A) {
   const int th = (s->nxy / 128 < 4 * 148) ? 64 : 128;      // small planes: smaller CTAs spread over more SMs
-  k_poisson_z<<<(unsigned)((s->nxy + th - 1) / th), th, 0, s->st>>>(s->c, s->pt, A, s->CP, s->CQ, s->cpt_on ? s->CPT : nullptr);
+  if (s->cpt_on == 2 && s->CPT && (((size_t)A) & 15) == 0) k_poisson_z2<<<(unsigned)((s->nxy / 2 + th - 1) / th), th, 0, s->st>>>(s->c, s->pt, A, s->CP, s->CPT);
+  else k_poisson_z<<<(unsigned)((s->nxy + th - 1) / th), th, 0, s->st>>>(s->c, s->pt, A, s->CP, s->CQ, s->cpt_on ? s->CPT : nullptr);
   LAUNCH_TRY(K_POISSON_Z);
   return CALES_OK;
 }
@@ -719,7 +720,7 @@ extern "C" int cales_set_option(cales_solver* s, const char* key, long long valu
   else if (k == "rhs_prefetch") { if (value < 0 || value > 2) return fail(CALES_EINVAL, "rhs_prefetch must be 0, 1 or 2"); s->rhs_pf = (int)value; }
   else if (k == "rhs_planes_per_cta") { if (value < 0 || value > 65535) return fail(CALES_EINVAL, "rhs_planes_per_cta out of range"); s->rhs_kz = (int)value; }
   else if (k == "fft_stage") { if (value < 0 || value > 1) return fail(CALES_EINVAL, "fft_stage must be 0 or 1"); s->fft_stage = (int)value; }
-  else if (k == "poisson_cp_table") { if (value < 0 || value > 1) return fail(CALES_EINVAL, "poisson_cp_table must be 0 or 1"); s->cpt_on = (value && s->CPT) ? 1 : 0; }
+  else if (k == "poisson_cp_table") { if (value < 0 || value > 2) return fail(CALES_EINVAL, "poisson_cp_table must be 0, 1 or 2"); s->cpt_on = s->CPT ? (int)value : 0; }
   else if (k == "lazy_nut") { if (value < 0 || value > 1) return fail(CALES_EINVAL, "lazy_nut must be 0 or 1"); s->lazy_nut = (int)value; }
   else if (k == "rhs_variant") { if (value < 0 || value > 1) return fail(CALES_EINVAL, "rhs_variant must be 0 or 1"); s->rhs_variant = (int)value; }
   else if (k == "dsm_col_variant") { if (value < 0 || value > 2) return fail(CALES_EINVAL, "dsm_col_variant must be 0, 1 or 2"); s->dsm_col_variant = (int)value; }
