@@ -236,6 +236,8 @@ int cales_fp64_peak(cales_solver* s, double* tflops_host);
  * "rhs_variant" (staged momentum kernel -- 1 (default): halo planes moved by 8-byte cp.async, 0: by tiled TMA copies),
  * "correct_pairs" (projection/correction kernel -- 1 (default): two x-neighbours per thread with 16-byte loads and stores, 0: one
  * point per thread),
+ * "correct_band" (launch order of that kernel: CTAs sweep k inside bands of this many 8-row CTA rows so that the phi plane k+1 is re-read
+ * from L2; 1: plane by plane; 0 (default): chosen from the grid),
  * "rhs_prefetch" (staged momentum kernel -- R^{k-1} of the next plane prefetched while a plane is computed: 1 (default) to L1, 2 to L2,
  * 0 off), "rhs_planes_per_cta" (k-planes per CTA of that kernel; 0 (default): chosen from the grid),
  * "dsm_col_variant" (column march of the dynamic model -- 0: register window, rows staged by TMA bulk copies; 1: the

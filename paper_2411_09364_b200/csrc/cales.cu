@@ -75,6 +75,7 @@ struct cales_solver {
   int dsm_col_rows;     // option: output rows per CTA of the column march (0: chosen from the grid)
   double* CPT; int cpt_on;      // static c' table of k_poisson_z (walls in z), option poisson_cp_table
   int fft_stage;        // option: 1 (default) stages the lines of the inverse x transform in shared memory by bulk copies
+  int corr_band;        // option: CTA rows per band of k_correct2's launch order (1: plane by plane; 0: chosen from the grid)
   int corr2;            // option: correction kernel with two points per thread and 16-byte accesses
   int rhs_pf;           // option: R^{k-1} of the next plane prefetched by the staged momentum kernel (0 off, 1 to L1, 2 to L2)
   int rhs_kz;           // option: k-planes per CTA of the staged momentum kernel (0: rt_chunk)
@@ -269,7 +270,7 @@ extern "C" int cales_create(const cales_params* p, cales_solver** out) {
   s->tile_min = 4000000;
   s->rhs_tile_min = 200000;
   s->dsm_col_variant = 0;
-  s->nut_lazy = false; s->nut_valid = true; s->graph_lazy = -1; s->lazy_nut = 1; s->dsm_col_rows = 0; s->rhs_kz = 0; s->rhs_pf = 1; s->corr2 = 1; s->fft_stage = 1;
+  s->nut_lazy = false; s->nut_valid = true; s->graph_lazy = -1; s->lazy_nut = 1; s->dsm_col_rows = 0; s->rhs_kz = 0; s->rhs_pf = 1; s->corr2 = 1; s->corr_band = 0; s->fft_stage = 1;
   s->rhs_variant = 1;      // measured on B200 at config 5: cp.async ring 22.7 ms, tiled TMA ring 25.1 ms per launch
   {
     const double* fl[RT_NF] = {s->u, s->v, s->w, s->nut, s->p};
@@ -510,6 +511,16 @@ static int refresh_closures(cales_solver* s) {
   return CALES_OK;
 }
 
+// CTA rows (8 grid rows each) per band of k_correct2's launch order.  A plane of its nine streams that fits L2 keeps the plane order;
+// otherwise bands of about 16 MB (B200, config 5, ms per launch: plane order 9.27, 16 rows 9.15, 32: 8.61, 64: 8.54, 128: 8.46, 256: 8.45,
+// 512: 8.65; config 4, whose plane is 19 MB: plane order 0.703, banded 0.706-0.741).
+static int corr_band(const cales_solver* s) {
+  if (s->corr_band > 0) return s->corr_band;
+  const double plane = 72.0 * (double)s->nxy;
+  if (plane <= 32.0 * 1048576.0) return 1;
+  const int b = (int)(16.0 * 1048576.0 / (72.0 * 8.0 * (double)s->c.nx));
+  return b < 1 ? 1 : b;
+}
 static int substep(cales_solver* s, int rk) {
   int rc;
   double al, be, ga; rk3_coeffs(rk, al, be, ga);
@@ -563,7 +574,7 @@ static int substep(cales_solver* s, int rk) {
   ca.phi = s->W; ca.us = s->us; ca.vs = s->vs; ca.ws = s->ws; ca.u = s->u; ca.v = s->v; ca.w = s->w; ca.p = s->p;
   ca.shift = cfr ? s->scal : nullptr; ca.gdt = 0.0; ca.cimp = (imp || imp3) ? 1.0 : 0.0; ca.cxy = imp3 ? 1.0 : 0.0; ca.update_p = 1; ca.sc = sc;
   if (imp3) k_correct<true><<<s->pgrid, s->pblock, 0, s->st>>>(c, ca);
-  else if (s->corr2 && c.nx >= 4) k_correct2<<<dim3((c.nx / 2 + 31) / 32, s->pgrid.y, s->pgrid.z), s->pblock, 0, s->st>>>(c, ca);
+  else if (s->corr2 && c.nx >= 4) k_correct2<<<dim3((c.nx / 2 + 31) / 32, s->pgrid.y, s->pgrid.z), s->pblock, 0, s->st>>>(c, ca, corr_band(s));
   else k_correct<false><<<s->pgrid, s->pblock, 0, s->st>>>(c, ca);
   LAUNCH_TRY(K_CORRECT);
   if ((rc = run_wall_stress(s))) return rc;
@@ -716,6 +727,7 @@ extern "C" int cales_set_option(cales_solver* s, const char* key, long long valu
     s->yTI = (int)value; s->y_tish = tish; s->y_threads = (int)th; s->y_smem = sm;
   }
   else if (k == "dsm_col_rows") { if (value < 0 || value > 4096) return fail(CALES_EINVAL, "dsm_col_rows must be 0..4096"); s->dsm_col_rows = (int)value; }
+  else if (k == "correct_band") { if (value < 0 || value > 1024) return fail(CALES_EINVAL, "correct_band must be 0..1024"); s->corr_band = (int)value; }
   else if (k == "correct_pairs") { if (value < 0 || value > 1) return fail(CALES_EINVAL, "correct_pairs must be 0 or 1"); s->corr2 = (int)value; }
   else if (k == "rhs_prefetch") { if (value < 0 || value > 2) return fail(CALES_EINVAL, "rhs_prefetch must be 0, 1 or 2"); s->rhs_pf = (int)value; }
   else if (k == "rhs_planes_per_cta") { if (value < 0 || value > 65535) return fail(CALES_EINVAL, "rhs_planes_per_cta out of range"); s->rhs_kz = (int)value; }

@@ -95,8 +95,17 @@ __global__ void __launch_bounds__(256, IMP3 ? 4 : 8) k_correct(Ctx c, CorrArgs a
 // Two x-neighbours per thread with 16-byte loads and stores (explicit or implicit-z diffusion, nx even, 16-byte aligned fields): half the
 // instructions of k_correct for the same bytes.  grid (ceil(nx/64), ceil(ny/8), nz), block (32, 8).  Rows or planes that need a
 // ghost go through correct_point.
-__global__ void __launch_bounds__(256, 4) k_correct2(Ctx c, CorrArgs a) {
-  const int i = 2 * (blockIdx.x * blockDim.x + threadIdx.x), j = blockIdx.y * blockDim.y + threadIdx.y, k = blockIdx.z;
+// band > 1: CTAs in launch order sweep k inside a band of `band` CTA rows (8 rows each) instead of finishing a plane first, so that the
+// phi plane k+1 read for the z difference is still in L2 when the CTAs of plane k+1 read it as their own.
+__global__ void __launch_bounds__(256, 4) k_correct2(Ctx c, CorrArgs a, int band) {
+  unsigned jb = blockIdx.y, kk = blockIdx.z;
+  if (band > 1) {
+    const unsigned gy = gridDim.y, bw = (unsigned)band, nfull = gy / bw, per = bw * gridDim.z;
+    const unsigned L = blockIdx.y + gy * blockIdx.z;
+    if (L < nfull * per) { const unsigned b = L / per, r = L - b * per; kk = r / bw; jb = b * bw + (r - kk * bw); }
+    else { const unsigned r = L - nfull * per, rw = gy - nfull * bw; kk = r / rw; jb = nfull * bw + (r - kk * rw); }
+  }
+  const int i = 2 * (blockIdx.x * blockDim.x + threadIdx.x), j = (int)jb * blockDim.y + threadIdx.y, k = (int)kk;
   if (i >= c.nx || j >= c.ny) return;
   if (!interior_row(c, j, k)) { correct_point<false>(c, a, i, j, k); correct_point<false>(c, a, i + 1, j, k); return; }
   const long long n = idx3(c, i, j, k);
