@@ -245,8 +245,9 @@ int cales_fp64_peak(cales_solver* s, double* tflops_host);
  * shared-memory-ring march),
  * "fft_x_lines" / "fft_y_cols" (lines per CTA of the x transforms / columns per CTA tile of the y transforms; default: about 256
  * threads per CTA),
- * "fft_stage" (1 (default): the first passes of the inverse transforms and the divergence of the forward x transform read shared
- * memory staged by bulk copies / batched loads; 0: they read global memory directly), "poisson_cp_table" (walls in z -- 2 (default):
+ * "fft_stage" (2 (default): the first passes of the inverse transforms and the divergence of the forward x transform read shared
+ * memory staged by bulk / 16-byte asynchronous copies and batched loads; 1: the inverse y tile is staged through registers instead;
+ * 0: they read global memory directly), "poisson_cp_table" (walls in z -- 2 (default):
  * the Thomas solve of the Poisson solver reads c' from a table built once at create, two columns per thread with 16-byte accesses; 1: the
  * same with one column per thread; 0: it recomputes and spills c' on every solve).
  * CALES_EINVAL on an unknown key or a value out of range. */

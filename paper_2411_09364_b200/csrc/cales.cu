@@ -74,7 +74,7 @@ struct cales_solver {
   bool nut_lazy, nut_valid; int graph_lazy;   // dynamic model: the momentum kernel forms nu_t from |S| and c_s (nut_lazy); s->nut holds it only when nut_valid
   int dsm_col_rows;     // option: output rows per CTA of the column march (0: chosen from the grid)
   double* CPT; int cpt_on;      // static c' table of k_poisson_z (walls in z), option poisson_cp_table
-  int fft_stage;        // option: 1 (default) stages the lines of the inverse x transform in shared memory by bulk copies
+  int fft_stage;        // option: 2 (default) stages the first-pass inputs of the transforms in shared memory (see cales.h); 1: inverse y through registers; 0: off
   int corr_band;        // option: CTA rows per band of k_correct2's launch order (1: plane by plane; 0: chosen from the grid)
   int corr2;            // option: correction kernel with two points per thread and 16-byte accesses
   int rhs_pf;           // option: R^{k-1} of the next plane prefetched by the staged momentum kernel (0 off, 1 to L1, 2 to L2)
@@ -270,7 +270,7 @@ extern "C" int cales_create(const cales_params* p, cales_solver** out) {
   s->tile_min = 4000000;
   s->rhs_tile_min = 200000;
   s->dsm_col_variant = 0;
-  s->nut_lazy = false; s->nut_valid = true; s->graph_lazy = -1; s->lazy_nut = 1; s->dsm_col_rows = 0; s->rhs_kz = 0; s->rhs_pf = 1; s->corr2 = 1; s->corr_band = 0; s->fft_stage = 1;
+  s->nut_lazy = false; s->nut_valid = true; s->graph_lazy = -1; s->lazy_nut = 1; s->dsm_col_rows = 0; s->rhs_kz = 0; s->rhs_pf = 1; s->corr2 = 1; s->corr_band = 0; s->fft_stage = 2;
   s->rhs_variant = 1;      // measured on B200 at config 5: cp.async ring 22.7 ms, tiled TMA ring 25.1 ms per launch
   {
     const double* fl[RT_NF] = {s->u, s->v, s->w, s->nut, s->p};
@@ -363,7 +363,8 @@ static int run_transform_x_inv(cales_solver* s, const double* src, double* dst) 
 }
 static int run_transform_y(cales_solver* s, double* A, int inverse) {
   dim3 grid((s->c.nx + s->yTI - 1) / s->yTI, s->c.nz);
-  const int staged = s->fft_stage && inverse && (((size_t)A) & 15) == 0 && s->ply.npass > 0 && (size_t)s->c.ny * s->yTI * 8 <= s->y_smem;
+  const bool stage_ok = s->fft_stage && (((size_t)A) & 15) == 0 && s->ply.npass > 0 && (size_t)s->c.ny * s->yTI * 8 <= s->y_smem;
+  const int staged = (stage_ok && inverse) ? (s->fft_stage >= 2 ? 2 : 1) : 0;
   k_fft2_y<<<grid, s->y_threads, s->y_smem, s->st>>>(s->c, s->ply, s->y_tish, s->c.bc_y == BC_WALL ? 1 : 0, inverse, A, staged);
   LAUNCH_TRY(inverse ? K_FFTY_INV : K_FFTY_FWD);
   return CALES_OK;
@@ -731,7 +732,7 @@ extern "C" int cales_set_option(cales_solver* s, const char* key, long long valu
   else if (k == "correct_pairs") { if (value < 0 || value > 1) return fail(CALES_EINVAL, "correct_pairs must be 0 or 1"); s->corr2 = (int)value; }
   else if (k == "rhs_prefetch") { if (value < 0 || value > 2) return fail(CALES_EINVAL, "rhs_prefetch must be 0, 1 or 2"); s->rhs_pf = (int)value; }
   else if (k == "rhs_planes_per_cta") { if (value < 0 || value > 65535) return fail(CALES_EINVAL, "rhs_planes_per_cta out of range"); s->rhs_kz = (int)value; }
-  else if (k == "fft_stage") { if (value < 0 || value > 1) return fail(CALES_EINVAL, "fft_stage must be 0 or 1"); s->fft_stage = (int)value; }
+  else if (k == "fft_stage") { if (value < 0 || value > 2) return fail(CALES_EINVAL, "fft_stage must be 0, 1 or 2"); s->fft_stage = (int)value; }
   else if (k == "poisson_cp_table") { if (value < 0 || value > 2) return fail(CALES_EINVAL, "poisson_cp_table must be 0, 1 or 2"); s->cpt_on = s->CPT ? (int)value : 0; }
   else if (k == "lazy_nut") { if (value < 0 || value > 1) return fail(CALES_EINVAL, "lazy_nut must be 0 or 1"); s->lazy_nut = (int)value; }
   else if (k == "rhs_variant") { if (value < 0 || value > 1) return fail(CALES_EINVAL, "rhs_variant must be 0 or 1"); s->rhs_variant = (int)value; }

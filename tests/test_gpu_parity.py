@@ -556,7 +556,7 @@ def test_lazy_nu_t_is_the_same_nu_t(oracle, gpu, n, shape):
     a.close(); b.close()
 
 
-@pytest.mark.parametrize("key,value", [("poisson_cp_table", 0), ("poisson_cp_table", 1), ("correct_pairs", 0), ("correct_band", 1), ("correct_band", 5), ("fft_stage", 0), ("rhs_prefetch", 0), ("rhs_prefetch", 2), ("fft_y_cols", 16),
+@pytest.mark.parametrize("key,value", [("poisson_cp_table", 0), ("poisson_cp_table", 1), ("correct_pairs", 0), ("correct_band", 1), ("correct_band", 5), ("fft_stage", 0), ("fft_stage", 1), ("rhs_prefetch", 0), ("rhs_prefetch", 2), ("fft_y_cols", 16),
                                        ("fft_y_cols", 4), ("fft_x_lines", 2), ("rhs_planes_per_cta", 8), ("dsm_col_rows", 16)])
 @pytest.mark.parametrize("n,shape", [(5, (144, 96, 32)), (3, (96, 72, 40))])
 def test_kernel_selection_options_keep_oracle_parity(oracle, gpu, n, shape, key, value):
