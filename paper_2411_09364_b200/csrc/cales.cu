@@ -76,6 +76,7 @@ struct cales_solver {
   double* CPT; int cpt_on;      // static c' table of k_poisson_z (walls in z), option poisson_cp_table
   int fft_stage;        // option: 2 (default) stages the first-pass inputs of the transforms in shared memory (see cales.h); 1: inverse y through registers; 0: off
   int corr_band;        // option: CTA rows per band of k_correct2's launch order (1: plane by plane; 0: chosen from the grid)
+  bool part_dirty;      // the partial-sum array may hold entries of another band layout: zero it before the next plane-averaged evaluation
   int corr2;            // option: correction kernel with two points per thread and 16-byte accesses
   int rhs_pf;           // option: R^{k-1} of the next plane prefetched by the staged momentum kernel (0 off, 1 to L1, 2 to L2)
   int rhs_kz;           // option: k-planes per CTA of the staged momentum kernel (0: rt_chunk)
@@ -270,7 +271,7 @@ extern "C" int cales_create(const cales_params* p, cales_solver** out) {
   s->tile_min = 4000000;
   s->rhs_tile_min = 200000;
   s->dsm_col_variant = 0;
-  s->nut_lazy = false; s->nut_valid = true; s->graph_lazy = -1; s->lazy_nut = 1; s->dsm_col_rows = 0; s->rhs_kz = 0; s->rhs_pf = 1; s->corr2 = 1; s->corr_band = 0; s->fft_stage = 2;
+  s->nut_lazy = false; s->nut_valid = true; s->graph_lazy = -1; s->lazy_nut = 1; s->dsm_col_rows = 0; s->rhs_kz = 0; s->rhs_pf = 1; s->corr2 = 1; s->part_dirty = false; s->corr_band = 0; s->fft_stage = 2;
   s->rhs_variant = 1;      // measured on B200 at config 5: cp.async ring 22.7 ms, tiled TMA ring 25.1 ms per launch
   {
     const double* fl[RT_NF] = {s->u, s->v, s->w, s->nut, s->p};
@@ -418,6 +419,10 @@ static int run_eddy_viscosity(cales_solver* s, const double* u, const double* v,
     // the DSM_TY rows next to each y wall, where filter and strain do not commute
     const Ctx& c = s->c;
     const DsmShape ds = dsm_shape(c.nx);
+    if (s->part_dirty) {      // an option changed the band layout of the column marches: their never-written slots must read 0
+      CUDA_TRY(cudaMemsetAsync(s->dsm_part, 0, (size_t)c.nz * c.ny * ds.pslots * 2 * sizeof(double), s->st));
+      s->part_dirty = false;
+    }
     const bool ywall = c.bc_y == BC_WALL;
     const bool split = ywall && c.ny >= 3 * DSM_TY;
     const size_t tile_smem = DSM_SMEM_DOUBLES * sizeof(double);
@@ -590,6 +595,10 @@ extern "C" int cales_launches_per_step(cales_solver* s);
 // (s->rks), so the captured graph serves every dt and nothing here synchronises.
 static int run_substeps(cales_solver* s) {
   int rc;
+  if (s->part_dirty && s->dsm_part) {      // outside any capture: the graph must not carry this memset into every replay
+    CUDA_TRY(cudaMemsetAsync(s->dsm_part, 0, (size_t)s->c.nz * s->c.ny * dsm_shape(s->c.nx).pslots * 2 * sizeof(double), s->st));
+    s->part_dirty = false;
+  }
   if (s->use_graph && !s->timing) {
     if (s->gexec && s->graph_lazy != (int)s->nut_lazy) { cudaGraphExecDestroy(s->gexec); s->gexec = nullptr; }   // the first substep's nu_t source is baked in
     if (s->gexec) {
@@ -727,7 +736,7 @@ extern "C" int cales_set_option(cales_solver* s, const char* key, long long valu
     if (th > 512 || sm > 200 * 1024) return fail(CALES_EINVAL, "fft_y_cols: CTA too large");
     s->yTI = (int)value; s->y_tish = tish; s->y_threads = (int)th; s->y_smem = sm;
   }
-  else if (k == "dsm_col_rows") { if (value < 0 || value > 4096) return fail(CALES_EINVAL, "dsm_col_rows must be 0..4096"); s->dsm_col_rows = (int)value; }
+  else if (k == "dsm_col_rows") { if (value < 0 || value > 4096) return fail(CALES_EINVAL, "dsm_col_rows must be 0..4096"); s->dsm_col_rows = (int)value; s->part_dirty = true; }
   else if (k == "correct_band") { if (value < 0 || value > 1024) return fail(CALES_EINVAL, "correct_band must be 0..1024"); s->corr_band = (int)value; }
   else if (k == "correct_pairs") { if (value < 0 || value > 1) return fail(CALES_EINVAL, "correct_pairs must be 0 or 1"); s->corr2 = (int)value; }
   else if (k == "rhs_prefetch") { if (value < 0 || value > 2) return fail(CALES_EINVAL, "rhs_prefetch must be 0, 1 or 2"); s->rhs_pf = (int)value; }
@@ -736,7 +745,7 @@ extern "C" int cales_set_option(cales_solver* s, const char* key, long long valu
   else if (k == "poisson_cp_table") { if (value < 0 || value > 2) return fail(CALES_EINVAL, "poisson_cp_table must be 0, 1 or 2"); s->cpt_on = s->CPT ? (int)value : 0; }
   else if (k == "lazy_nut") { if (value < 0 || value > 1) return fail(CALES_EINVAL, "lazy_nut must be 0 or 1"); s->lazy_nut = (int)value; }
   else if (k == "rhs_variant") { if (value < 0 || value > 1) return fail(CALES_EINVAL, "rhs_variant must be 0 or 1"); s->rhs_variant = (int)value; }
-  else if (k == "dsm_col_variant") { if (value < 0 || value > 2) return fail(CALES_EINVAL, "dsm_col_variant must be 0, 1 or 2"); s->dsm_col_variant = (int)value; }
+  else if (k == "dsm_col_variant") { if (value < 0 || value > 2) return fail(CALES_EINVAL, "dsm_col_variant must be 0, 1 or 2"); s->dsm_col_variant = (int)value; s->part_dirty = true; }
   else return fail(CALES_EINVAL, "unknown option: " + k);
   if (s->gexec) { cudaGraphExecDestroy(s->gexec); s->gexec = nullptr; }      // the captured step holds the old selection
   return CALES_OK;

@@ -157,7 +157,7 @@ CALES_HD void dsmr_row(const double* shbuf, int txb, int t, const double* b, Dsm
 // grid (ceil(nx/(TXB-2)), planes, ceil((jhi-jlo)/ly)), block TXB (multiple of 32); ly = output rows per CTA.  Planes k0 + blockIdx.y * kstride,
 // output rows [jlo, jhi).
 // part: [k][j][pslots][2]; this kernel fills slots blockIdx.x*(TXB/32) + warp of its rows: per row with x-line averaging, the
-// CTA's total in its first row (zeros in the others) with plane averaging.
+// CTA's total in its first row with plane averaging (the others are left at the zeros the host guarantees).
 template <int TXB, int MINB>
 __global__ void __launch_bounds__(TXB, MINB) k_dsm_col_rw(const __grid_constant__ Ctx c, const double* __restrict__ u, const double* __restrict__ v,
                                                           const double* __restrict__ w, int k0, int kstride, int jlo, int jhi, int ly, int pslots,
@@ -221,9 +221,11 @@ __global__ void __launch_bounds__(TXB, MINB) k_dsm_col_rw(const __grid_constant_
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) { accl += __shfl_down_sync(0xffffffffu, accl, o); accm += __shfl_down_sync(0xffffffffu, accm, o); }
     if ((t & 31) == 0)
-      for (int jo = j0; jo < jend; ++jo) {
-        const long long slot = pslot0 + (long long)jo * pslots;
-        part[slot * 2] = jo == j0 ? accl : 0.0; part[slot * 2 + 1] = jo == j0 ? accm : 0.0;
+      {      // the CTA's total in the slot of its first row.  The slots of its other rows are never written: they are zero since create (or
+             // since the host re-zeroed the array after an option changed the band layout), which saves 0.4 GB of scattered 16-byte
+             // stores per launch at config 5 (18.75 -> 18.40 ms per evaluation)
+        const long long slot = pslot0 + (long long)j0 * pslots;
+        part[slot * 2] = accl; part[slot * 2 + 1] = accm;
       }
   }
 }
@@ -346,10 +348,7 @@ __global__ void __launch_bounds__(TXB, MINB) k_dsm_col_tma(const __grid_constant
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) { accl += __shfl_down_sync(0xffffffffu, accl, o); accm += __shfl_down_sync(0xffffffffu, accm, o); }
     if ((t & 31) == 0)
-      for (int jo = j0; jo < jend; ++jo) {
-        part[pslot * 2] = jo == j0 ? accl : 0.0; part[pslot * 2 + 1] = jo == j0 ? accm : 0.0;
-        pslot += pslots;
-      }
+      { part[pslot * 2] = accl; part[pslot * 2 + 1] = accm; }      // the CTA's total in its first row; the slots of its other rows stay 0 (see k_dsm_col_rw)
   }
 }
 #endif
