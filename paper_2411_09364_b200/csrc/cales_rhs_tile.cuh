@@ -183,6 +183,11 @@ static inline int rt_chunk(int nx, int ny, int nz) {
   const long long maxc = nz / 8 > 0 ? nz / 8 : 1;
   if (want > maxc) want = maxc;
   if (want < 1) want = 1;
+  // at most ~96 planes per CTA: neighbouring CTAs that march a whole tall column drift apart by more planes than L2 holds, and the halo
+  // they share comes from DRAM twice (ncu, config 5, nz = 512: 66.8 GB read per launch with one chunk, 54.3 GB with chunks of 64 for
+  // 51.5 GB of fields; 24.56 -> 23.59 ms, interleaved A/B; 16 planes: 24.60, the two extra halo planes per chunk take over)
+  const long long cap = (nz + 95) / 96;
+  if (want < cap) want = cap;
   return (int)((nz + want - 1) / want);
 }
 
