@@ -243,8 +243,8 @@ int cales_fp64_peak(cales_solver* s, double* tflops_host);
  * "dsm_col_variant" (column march of the dynamic model -- 0: register window, rows staged by TMA bulk copies; 1: the
  * shared-memory-ring form; 2: register window, direct loads; with the 3-D test filter 0: staged rows + register window, 1 / 2: the
  * shared-memory-ring march),
- * "fft_x_lines" / "fft_y_cols" (lines per CTA of the x transforms / columns per CTA tile of the y transforms; default: about 256
- * threads per CTA),
+ * "fft_x_lines" / "fft_y_cols" (lines per CTA of the x transforms / columns per CTA tile of the y transforms; defaults: the forward x
+ * transform that forms the divergence about 32-64 threads per CTA, the inverse about 64-256, the y tiles 8 or 16 columns),
  * "fft_stage" (2 (default): the first passes of the inverse transforms and the divergence of the forward x transform read shared
  * memory staged by bulk / 16-byte asynchronous copies and batched loads; 1: the inverse y tile is staged through registers instead;
  * 0: they read global memory directly), "poisson_cp_table" (walls in z -- 2 (default):

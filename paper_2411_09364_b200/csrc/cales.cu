@@ -64,6 +64,7 @@ struct cales_solver {
   PoissonTabs pt;
   WallGeom wg;
   int xB, yTI, y_tish; size_t x_smem, y_smem; int x_threads, y_threads;
+  int xBf, xf_threads; size_t xf_smem;      // lines per CTA, threads and shared memory of the forward x transform that forms the divergence
   dim3 pgrid, pblock;   // point kernels
   long long nblk;
   bool fresh;
@@ -204,6 +205,17 @@ static bool make_field_map(CUtensorMap* m, const double* base, int nx, int ny, i
              CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+// Launch shape of an x transform with L lines per CTA; false if the CTA would be too large.
+static bool x_launch_shape(const FftPlan& plx, int nx, int L, int* threads, size_t* smem) {
+  const int n2 = nx / 2;
+  bool has3 = false; for (int q = 0; q < plx.npass; ++q) has3 |= plx.radix[q] == 3;
+  const int per_thread = has3 ? 3 * (F2_E / 3) : F2_E;
+  long long th = ((long long)L * n2 + per_thread - 1) / per_thread; th = (th + 31) / 32 * 32; if (th < 32) th = 32;
+  const size_t sm = (size_t)L * sm_line(n2) * 16;
+  if (th > 512 || sm > 200 * 1024 || L < 1 || L > 64 || L > 2 * th) return false;
+  *threads = (int)th; *smem = sm;
+  return true;
+}
 static int static_scratch_ptr(int device, double** out);
 extern "C" int cales_create(const cales_params* p, cales_solver** out) {
   if (!out) return fail(CALES_EINVAL, "null output pointer");
@@ -252,6 +264,23 @@ extern "C" int cales_create(const cales_params* p, cales_solver** out) {
   s->ply = H.ply; s->ply.tw = s->twy; s->ply.dctw = s->dctw;
   s->xB = H.xB; s->x_smem = H.x_smem; s->x_threads = H.x_threads;
   s->yTI = H.yTI; s->y_tish = H.y_tish; s->y_smem = H.y_smem; s->y_threads = H.y_threads;
+  s->xBf = s->xB; s->xf_threads = s->x_threads; s->xf_smem = s->x_smem;
+  {
+    // Small CTAs for the x transforms (B200, ms per launch).  Forward with the divergence pre-pass -- config 5 (n2 = 768): 5 lines 7.43,
+    // 2: 7.04, 1: 6.32; config 4 (512): 8 lines 0.680, 2: 0.510, 1: 0.520; config 3 (128): 32 lines 0.258, 8: 0.125, 4: 0.109, 2: 0.108;
+    // config 2 (96): 42 lines 0.053, 4: 0.020.  Its serial phases (batched loads of a line, butterflies, split) overlap across CTAs, not
+    // inside one: many CTAs of 32-64 threads hide the load latency that two CTAs of 256 could not.  Inverse (lines staged by bulk
+    // copies) -- config 5: 5 lines 4.13, 2: 4.25, 1: 4.52; config 4: 8 lines 0.341, 2: 0.296; config 3: 32 lines 0.0755, 4: 0.063.
+    const int n2 = nx / 2;
+    const long long nlines = (long long)ny * nz;
+    int Lf = 512 / (n2 > 0 ? n2 : 1); if (Lf < 1) Lf = 1; if (Lf > 64) Lf = 64; if (Lf > nlines) Lf = (int)nlines;
+    int th; size_t sm;
+    if (Lf < s->xB && x_launch_shape(s->plx, nx, Lf, &th, &sm)) { s->xBf = Lf; s->xf_threads = th; s->xf_smem = sm; }      // never more lines than the host plan (small grids: enough CTAs)
+    if (n2 < 640) {
+      int Li = 1024 / (n2 > 0 ? n2 : 1); if (Li < 1) Li = 1; if (Li > 64) Li = 64; if (Li > nlines) Li = (int)nlines;
+      if (Li < s->xB && x_launch_shape(s->plx, nx, Li, &th, &sm)) { s->xB = Li; s->x_threads = th; s->x_smem = sm; }
+    }
+  }
   e = cudaFuncSetAttribute(k_fft2_x_fwd<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fft2_x_fwd<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_fft2_x_inv, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
@@ -349,7 +378,7 @@ extern "C" int cales_get_field(cales_solver* s, int field, double* dst, int on_d
 static int run_transform_x_fwd(cales_solver* s, const double* src, const DivSrc* ds, double* dst) {
   const long long nlines = (long long)s->c.ny * s->c.nz;
   const unsigned grid = (unsigned)((nlines + s->xB - 1) / s->xB);
-  if (ds) k_fft2_x_fwd<true><<<grid, s->x_threads, s->x_smem, s->st>>>(s->c, s->plx, s->xB, nullptr, *ds, dst, (s->fft_stage && s->plx.npass > 0) ? 1 : 0);
+  if (ds) k_fft2_x_fwd<true><<<(unsigned)((nlines + s->xBf - 1) / s->xBf), s->xf_threads, s->xf_smem, s->st>>>(s->c, s->plx, s->xBf, nullptr, *ds, dst, (s->fft_stage && s->plx.npass > 0) ? 1 : 0);
   else { DivSrc z{nullptr, nullptr, nullptr, 0.0, nullptr}; k_fft2_x_fwd<false><<<grid, s->x_threads, s->x_smem, s->st>>>(s->c, s->plx, s->xB, src, z, dst, 0); }
   LAUNCH_TRY(K_FFTX_FWD);
   return CALES_OK;
@@ -724,6 +753,7 @@ extern "C" int cales_set_option(cales_solver* s, const char* key, long long valu
     const size_t sm = (size_t)L * sm_line(n2) * 16;
     if (th > 512 || sm > 200 * 1024) return fail(CALES_EINVAL, "fft_x_lines: CTA too large");
     s->xB = L; s->x_threads = (int)th; s->x_smem = sm;
+    s->xBf = L; s->xf_threads = (int)th; s->xf_smem = sm;
   }
   else if (k == "fft_y_cols") {      // columns per CTA tile of the y transforms (power of two; default: ~256 threads per CTA)
     int tish = 0; while ((1LL << tish) < value) ++tish;

@@ -187,7 +187,7 @@ static inline int build_setup(const cales_params* p, HostSetup& H) {
   }
   {
     const int n2 = ny / 2;
-    int tish = 5;                                                   // TI = 32 columns ...
+    int tish = 4;                                                   // TI = 16 columns (B200: config 4 0.322 / 0.337 ms against 0.345 / 0.343 with 32) ...
     while (tish > 3 && (long long)(1 << tish) * n2 > 256 * F2_E) --tish;   // ... down to 8 (64-byte row segments) for long lines
     while (tish > 0 && (1 << tish) > nx) --tish;
     while (tish > 3 && (long long)((nx + (1 << tish) - 1) >> tish) * nz < 2 * 148) --tish;
