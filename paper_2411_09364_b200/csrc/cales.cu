@@ -760,7 +760,7 @@ extern "C" int cales_set_option(cales_solver* s, const char* key, long long valu
     if (value < 1 || (1LL << tish) != value || value > s->c.nx || value > 64) return fail(CALES_EINVAL, "fft_y_cols must be a power of two <= min(nx, 64)");
     const int n2 = s->c.ny / 2;
     bool has3 = false; for (int q = 0; q < s->ply.npass; ++q) has3 |= s->ply.radix[q] == 3;
-    const int per_thread = has3 ? 3 * (F2_E / 3) : F2_E;
+    const int per_thread = has3 ? 3 * (F2_EY / 3) : F2_EY;
     long long th = ((long long)value * n2 + per_thread - 1) / per_thread; th = (th + 31) / 32 * 32; if (th < 32) th = 32;
     size_t sm = (size_t)value * n2 * 16; if (sm < 16) sm = 16;
     if (th > 512 || sm > 200 * 1024) return fail(CALES_EINVAL, "fft_y_cols: CTA too large");

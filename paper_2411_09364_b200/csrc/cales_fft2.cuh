@@ -19,6 +19,12 @@ namespace cales {
 #define CALES_F2_E 16
 #endif
 enum { F2_E = CALES_F2_E };     // complex elements per thread per pass (16: radix <= 16; 8: radix <= 8, half the registers)
+#ifndef CALES_F2_EY
+#define CALES_F2_EY 8
+#endif
+// the y transforms: 8 (64 registers, twice the warps per SM): B200, config 5, 3.85 / 4.52 ms against 4.3 / 4.6 with 16; the x transforms
+// lose with 8 (8.6 / 4.9 against 6.3 / 4.2 ms)
+enum { F2_EY = CALES_F2_EY };
 
 struct Fft2Lay { int L, ls, tish; bool ylay; };     // x: line stride ls (padded); y: TI = 1 << tish columns
 CALES_HD int f2_off(const Fft2Lay& g, int b, int t) { return g.ylay ? (t << g.tish) + b : b * g.ls + sm_pad(t); }
@@ -33,7 +39,7 @@ CALES_HD unsigned f2_div(unsigned n, unsigned d, unsigned magic) {
 #endif
 }
 
-template <int R> struct F2G { enum { G = (R == 3) ? F2_E / 3 : (F2_E / R > 0 ? F2_E / R : 1) }; };
+template <int R, int E = F2_E> struct F2G { enum { G = (R == 3) ? E / 3 : (E / R > 0 ? E / R : 1) }; };
 
 // butterfly g of this thread in pass p -> (line b, butterfly index j); false if beyond the work of the pass
 CALES_HD bool f2_item(const Fft2Lay& lay, const FftPlan& pl, int p, int tid, int nth, int g, int& b, int& j) {
@@ -46,11 +52,11 @@ CALES_HD bool f2_item(const Fft2Lay& lay, const FftPlan& pl, int p, int tid, int
 }
 
 // registers <- LD(b, element) for the butterflies of pass p
-template <int R, class LD>
+template <int R, int E, class LD>
 CALES_HD void f2_load(const Fft2Lay& lay, const FftPlan& pl, int p, int tid, int nth, LD ld, double2* v) {
   const int per = pl.per[p];
 #pragma unroll
-  for (int g = 0; g < F2G<R>::G; ++g) {
+  for (int g = 0; g < F2G<R, E>::G; ++g) {
     int b, j;
     if (!f2_item(lay, pl, p, tid, nth, g, b, j)) continue;
 #pragma unroll
@@ -59,12 +65,12 @@ CALES_HD void f2_load(const Fft2Lay& lay, const FftPlan& pl, int p, int tid, int
 }
 
 // twiddles + radix-R butterflies of pass p on the registers, then ST(b, element, value)
-template <int R, class ST>
+template <int R, int E, class ST>
 CALES_HD void f2_bfly_store(const Fft2Lay& lay, const FftPlan& pl, int p, int sign, int tid, int nth, double2* v, ST st) {
   const int Ns = pl.ns[p];
   const int tws = pl.n / (Ns * R);
 #pragma unroll
-  for (int g = 0; g < F2G<R>::G; ++g) {
+  for (int g = 0; g < F2G<R, E>::G; ++g) {
     int b, j;
     if (!f2_item(lay, pl, p, tid, nth, g, b, j)) continue;
     const int k = j - (int)f2_div((unsigned)j, (unsigned)Ns, pl.mns[p]) * Ns;
@@ -90,24 +96,24 @@ CALES_HD void f2_bfly_store(const Fft2Lay& lay, const FftPlan& pl, int p, int si
 }
 
 // dispatch on the radix of pass p
-template <class LD>
+template <int E = F2_E, class LD>
 CALES_HD void f2_load_any(const Fft2Lay& lay, const FftPlan& pl, int p, int tid, int nth, LD ld, double2* v) {
   switch (pl.radix[p]) {
-    case 2: f2_load<2>(lay, pl, p, tid, nth, ld, v); break;
-    case 3: f2_load<3>(lay, pl, p, tid, nth, ld, v); break;
-    case 4: f2_load<4>(lay, pl, p, tid, nth, ld, v); break;
-    case 8: f2_load<8>(lay, pl, p, tid, nth, ld, v); break;
-    default: f2_load<16>(lay, pl, p, tid, nth, ld, v); break;
+    case 2: f2_load<2, E>(lay, pl, p, tid, nth, ld, v); break;
+    case 3: f2_load<3, E>(lay, pl, p, tid, nth, ld, v); break;
+    case 4: f2_load<4, E>(lay, pl, p, tid, nth, ld, v); break;
+    case 8: f2_load<8, E>(lay, pl, p, tid, nth, ld, v); break;
+    default: f2_load<16, E>(lay, pl, p, tid, nth, ld, v); break;
   }
 }
-template <class ST>
+template <int E = F2_E, class ST>
 CALES_HD void f2_bfly_any(const Fft2Lay& lay, const FftPlan& pl, int p, int sign, int tid, int nth, double2* v, ST st) {
   switch (pl.radix[p]) {
-    case 2: f2_bfly_store<2>(lay, pl, p, sign, tid, nth, v, st); break;
-    case 3: f2_bfly_store<3>(lay, pl, p, sign, tid, nth, v, st); break;
-    case 4: f2_bfly_store<4>(lay, pl, p, sign, tid, nth, v, st); break;
-    case 8: f2_bfly_store<8>(lay, pl, p, sign, tid, nth, v, st); break;
-    default: f2_bfly_store<16>(lay, pl, p, sign, tid, nth, v, st); break;
+    case 2: f2_bfly_store<2, E>(lay, pl, p, sign, tid, nth, v, st); break;
+    case 3: f2_bfly_store<3, E>(lay, pl, p, sign, tid, nth, v, st); break;
+    case 4: f2_bfly_store<4, E>(lay, pl, p, sign, tid, nth, v, st); break;
+    case 8: f2_bfly_store<8, E>(lay, pl, p, sign, tid, nth, v, st); break;
+    default: f2_bfly_store<16, E>(lay, pl, p, sign, tid, nth, v, st); break;
   }
 }
 
@@ -255,10 +261,10 @@ CALES_HD void f2y_split_store(int tid, int nth, const Ctx& c, const FftPlan& pl,
 #ifdef __CUDACC__
 // The pass loop shared by the four kernels.  FIRST reads the pass-0 inputs, LAST (inverse only) consumes the outputs
 // of the final pass; forward transforms leave the complex FFT in shared memory for the split.
-template <bool TO_GLOBAL, class FIRST, class LAST>
+template <bool TO_GLOBAL, int E = F2_E, class FIRST, class LAST>
 __device__ __forceinline__ void f2_passes(const Fft2Lay& lay, const FftPlan& pl, int sign, double2* buf, FIRST first, LAST last) {
   const int tid = threadIdx.x, nth = blockDim.x, np = pl.npass;
-  double2 v[F2_E];
+  double2 v[E];
   F2SmemLd sld{buf, lay}; F2SmemSt sst{buf, lay};
   if (np == 0) {                 // n = 2: a single complex element per line (lines b = tid, tid + nth, ...; L <= 64 <= 2 * nth)
     double2 z0 = make_double2(0.0, 0.0), z1 = z0;
@@ -271,10 +277,10 @@ __device__ __forceinline__ void f2_passes(const Fft2Lay& lay, const FftPlan& pl,
     return;
   }
   for (int p = 0; p < np; ++p) {
-    if (p == 0) f2_load_any(lay, pl, 0, tid, nth, first, v); else f2_load_any(lay, pl, p, tid, nth, sld, v);
+    if (p == 0) f2_load_any<E>(lay, pl, 0, tid, nth, first, v); else f2_load_any<E>(lay, pl, p, tid, nth, sld, v);
     __syncthreads();             // in-place passes (and in-place global transforms): all reads before any write
-    if (TO_GLOBAL && p == np - 1) f2_bfly_any(lay, pl, p, sign, tid, nth, v, last);
-    else { f2_bfly_any(lay, pl, p, sign, tid, nth, v, sst); __syncthreads(); }
+    if (TO_GLOBAL && p == np - 1) f2_bfly_any<E>(lay, pl, p, sign, tid, nth, v, last);
+    else { f2_bfly_any<E>(lay, pl, p, sign, tid, nth, v, sst); __syncthreads(); }
   }
 }
 
@@ -370,7 +376,7 @@ __global__ void __launch_bounds__(512) k_fft2_y(const __grid_constant__ Ctx c, c
   double* base = A + (long long)k * c.nxy + i0;
   if (!inverse) {
     F2YFwdLd first{c, pl, base, nb, dct != 0};
-    f2_passes<false>(lay, pl, -1, f2_sm, first, F2SmemSt{f2_sm, lay});
+    f2_passes<false, F2_EY>(lay, pl, -1, f2_sm, first, F2SmemSt{f2_sm, lay});
     f2y_split_store(threadIdx.x, blockDim.x, c, pl, lay, dct != 0, base, nb, f2_sm);
   } else if ((staged & 3) && nb == TI && TI >= 2) {
     F2YInvSt last{c, pl, base, nb, dct != 0, 1.0 / (double)pl.n2};
@@ -396,11 +402,11 @@ __global__ void __launch_bounds__(512) k_fft2_y(const __grid_constant__ Ctx c, c
     }
     __syncthreads();
     F2YInvLdS first{pl, reinterpret_cast<const double*>(f2_sm), TI, nb, dct != 0};
-    f2_passes<true>(lay, pl, +1, f2_sm, first, last);
+    f2_passes<true, F2_EY>(lay, pl, +1, f2_sm, first, last);
   } else {
     F2YInvLd first{c, pl, base, nb, dct != 0};
     F2YInvSt last{c, pl, base, nb, dct != 0, 1.0 / (double)pl.n2};
-    f2_passes<true>(lay, pl, +1, f2_sm, first, last);
+    f2_passes<true, F2_EY>(lay, pl, +1, f2_sm, first, last);
   }
 }
 #endif

@@ -50,13 +50,13 @@ static inline int validate(const cales_params* p) {
 
 // Radix plan of the complex FFT of length n/2: the power of two 2^a split into ceil(a/4) passes of radix 2..16 of
 // (nearly) equal size, smallest first (the first passes write with stride R), then the factors of 3.
-static inline void make_plan(FftPlan& pl, int n) {
+static inline void make_plan(FftPlan& pl, int n, int E = F2_E) {
   pl.n = n; pl.n2 = n / 2; pl.npass = 0; pl.tw = nullptr; pl.dctw = nullptr;
   int m = pl.n2, n3 = 0;
   while (m % 3 == 0) { ++n3; m /= 3; }
   int a = 0; while (m % 2 == 0) { ++a; m /= 2; }
   if (a > 0) {
-    int maxbits = F2_E >= 16 ? 4 : 3;
+    int maxbits = E >= 16 ? 4 : 3;
     const int np = (a + maxbits - 1) / maxbits, base = a / np, extra = a % np;
     for (int q = 0; q < np; ++q) pl.radix[pl.npass++] = 1 << (base + (q >= np - extra ? 1 : 0));
   }
@@ -167,11 +167,11 @@ static inline int build_setup(const cales_params* p, HostSetup& H) {
   }
   // ---- transform plans and launch shapes
   make_plan(H.plx, nx);
-  make_plan(H.ply, ny);
+  make_plan(H.ply, ny, F2_EY);
   // every thread holds 16 complex elements per pass (15 when a radix-3 pass exists): ~256 threads per CTA
-  auto threads_for = [](long long elems, const FftPlan& pl) {
+  auto threads_for = [](long long elems, const FftPlan& pl, int E = F2_E) {
     bool has3 = false; for (int p = 0; p < pl.npass; ++p) has3 |= pl.radix[p] == 3;
-    const int per_thread = has3 ? 3 * (F2_E / 3) : F2_E;
+    const int per_thread = has3 ? 3 * (E / 3) : E;
     long long th = (elems + per_thread - 1) / per_thread;
     th = (th + 31) / 32 * 32;
     return (int)(th < 32 ? 32 : th);
@@ -188,12 +188,12 @@ static inline int build_setup(const cales_params* p, HostSetup& H) {
   {
     const int n2 = ny / 2;
     int tish = 4;                                                   // TI = 16 columns (B200: config 4 0.322 / 0.337 ms against 0.345 / 0.343 with 32) ...
-    while (tish > 3 && (long long)(1 << tish) * n2 > 256 * F2_E) --tish;   // ... down to 8 (64-byte row segments) for long lines
+    while (tish > 3 && (long long)(1 << tish) * n2 > 512 * F2_EY) --tish;   // ... down to 8 (64-byte row segments) for long lines
     while (tish > 0 && (1 << tish) > nx) --tish;
     while (tish > 3 && (long long)((nx + (1 << tish) - 1) >> tish) * nz < 2 * 148) --tish;
-    while (tish > 0 && (threads_for((long long)(1 << tish) * n2, H.ply) > 512 || (size_t)(1 << tish) * n2 * 16 > 200 * 1024)) --tish;
+    while (tish > 0 && (threads_for((long long)(1 << tish) * n2, H.ply, F2_EY) > 512 || (size_t)(1 << tish) * n2 * 16 > 200 * 1024)) --tish;
     H.yTI = 1 << tish; H.y_tish = tish; H.y_smem = (size_t)(1 << tish) * n2 * 16; if (H.y_smem < 16) H.y_smem = 16;
-    H.y_threads = threads_for((long long)(1 << tish) * n2, H.ply);
+    H.y_threads = threads_for((long long)(1 << tish) * n2, H.ply, F2_EY);
   }
   if (H.x_threads > 512 || H.y_threads > 512 || H.x_smem > 200 * 1024 || H.y_smem > 200 * 1024)
     return fail(CALES_EUNSUPPORTED, "line too long for the shared-memory transforms");

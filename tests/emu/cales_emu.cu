@@ -74,10 +74,10 @@ extern "C" int emu_get_field(emu_solver* s, int f, double* dst) { std::memcpy(ds
 // ---- kernel emulations: same block decomposition and phase order as the __global__ wrappers ----
 // f2_passes (cales_fft2.cuh) stepped on the host: one register file of F2_E complex numbers per emulated thread, the
 // phases separated where the kernel has its block barriers.
-template <bool TO_GLOBAL, class FIRST, class LAST>
+template <bool TO_GLOBAL, int E = F2_E, class FIRST, class LAST>
 static void emu_f2_passes(const Fft2Lay& lay, const FftPlan& pl, int sign, double2* buf, int nth, FIRST first, LAST last) {
   const int np = pl.npass;
-  std::vector<double2> regs((size_t)nth * F2_E);
+  std::vector<double2> regs((size_t)nth * E);
   F2SmemLd sld{buf, lay}; F2SmemSt sst{buf, lay};
   if (np == 0) {
     std::vector<double2> z(lay.L);
@@ -87,12 +87,12 @@ static void emu_f2_passes(const Fft2Lay& lay, const FftPlan& pl, int sign, doubl
   }
   for (int p = 0; p < np; ++p) {
     for (int tid = 0; tid < nth; ++tid) {
-      if (p == 0) f2_load_any(lay, pl, 0, tid, nth, first, &regs[(size_t)tid * F2_E]);
-      else f2_load_any(lay, pl, p, tid, nth, sld, &regs[(size_t)tid * F2_E]);
+      if (p == 0) f2_load_any<E>(lay, pl, 0, tid, nth, first, &regs[(size_t)tid * E]);
+      else f2_load_any<E>(lay, pl, p, tid, nth, sld, &regs[(size_t)tid * E]);
     }
     for (int tid = 0; tid < nth; ++tid) {
-      if (TO_GLOBAL && p == np - 1) f2_bfly_any(lay, pl, p, sign, tid, nth, &regs[(size_t)tid * F2_E], last);
-      else f2_bfly_any(lay, pl, p, sign, tid, nth, &regs[(size_t)tid * F2_E], sst);
+      if (TO_GLOBAL && p == np - 1) f2_bfly_any<E>(lay, pl, p, sign, tid, nth, &regs[(size_t)tid * E], last);
+      else f2_bfly_any<E>(lay, pl, p, sign, tid, nth, &regs[(size_t)tid * E], sst);
     }
   }
 }
@@ -131,12 +131,12 @@ static void emu_fft_y(emu_solver* s, double* A, int inverse) {
     double* base = A + (long long)k * c.nxy + i0;
     if (!inverse) {
       F2YFwdLd first{c, pl, base, nb, dct};
-      emu_f2_passes<false>(lay, pl, -1, sm.data(), nth, first, F2SmemSt{sm.data(), lay});
+      emu_f2_passes<false, F2_EY>(lay, pl, -1, sm.data(), nth, first, F2SmemSt{sm.data(), lay});
       for (int tid = 0; tid < nth; ++tid) f2y_split_store(tid, nth, c, pl, lay, dct, base, nb, sm.data());
     } else {
       F2YInvLd first{c, pl, base, nb, dct};
       F2YInvSt last{c, pl, base, nb, dct, 1.0 / (double)pl.n2};
-      emu_f2_passes<true>(lay, pl, +1, sm.data(), nth, first, last);
+      emu_f2_passes<true, F2_EY>(lay, pl, +1, sm.data(), nth, first, last);
     }
   }
 }
